@@ -1,0 +1,146 @@
+/* mipwa.h -- C ABI of libmipwa: the B200 (sm_100a) hot path of a model-independent partial wave analysis fit.
+ *
+ * What it computes (arXiv:1703.03284 = /root/reference/PAPER.md; readings in DESIGN.md section 3):
+ *
+ *   A(s12,s13) = S(s12) + S(s13) + sum_r c_r [ T_r(s12,s13) + T_r(s13,s12) ]
+ *       Eq. 1 truncated at L = 2, Bose-symmetrised in s12 <-> s13.
+ *       S   = natural cubic spline through N knots in m^2, S(s_k) = a_k exp(i phi_k), Re and Im splined
+ *             separately; the S-wave is one object without a coefficient of its own.
+ *       T_r = F_D F_R Z_L BW: relativistic Breit-Wigner with running width times Blatt-Weisskopf barrier factors
+ *             and the Zemach angular factor (PAPER.md:27 + its ref. [5]; forms fixed in DESIGN.md readings P9, P10).
+ *   NLL = - sum_i ln |A(event_i)|^2 + n_ev ln I,   I = sum_j w_j |A(norm_j)|^2
+ *       unbinned likelihood with the PDF normalised to unit integral every call.
+ *
+ * All arithmetic is IEEE fp64 and runs in CUDA kernels on one GPU; there is no CPU fallback: every entry point
+ * fails with MIPWA_ERR_CUDA when no usable device exists.  Plain C, no exceptions, nothing printed.
+ *
+ * Conventions
+ *   - Units: masses GeV, s12/s13/knots GeV^2, radii GeV^-1.
+ *   - Particle 1 is the odd-charge one; 2 and 3 are the identical pair (m2 == m3 required).
+ *     s12 = m^2(1,2), s13 = m^2(1,3).
+ *   - Parameter vector (HOST pointer, length mipwa_n_params()):
+ *       [ a_0 .. a_{N-1} | phi_0 .. phi_{N-1} | (|c_0|, arg c_0) .. (|c_{R-1}|, arg c_{R-1}) |
+ *         (mass, width) of every resonance created with shape_floats = 1, in list order ]
+ *   - Ownership: a `mem` argument says where the caller's arrays live.  MIPWA_MEM_HOST: the library copies them
+ *     into device memory it owns.  MIPWA_MEM_DEVICE: the library BORROWS the device pointers (zero copy, e.g.
+ *     torch tensors); the caller keeps them alive and unchanged until the next mipwa_set_* call on the same slot or
+ *     mipwa_destroy.  Outputs are caller-allocated HOST memory unless stated otherwise.
+ *   - Errors: every function returns MIPWA_OK (0) or a negative code; mipwa_last_error() gives the text of the
+ *     last failure on that context.  A |A|^2 of zero or a non-finite value propagates as IEEE inf/NaN in the
+ *     result with status MIPWA_OK.
+ *   - Threads: a context must not be used from two threads at once; distinct contexts are independent.
+ *   - Synchrony: mipwa_nll / mipwa_nll_grad / mipwa_eval_abs2 return when their result is in host memory.
+ *     Kernels are launched on the stream given to mipwa_set_stream (default: the legacy default stream).
+ */
+#ifndef MIPWA_H
+#define MIPWA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mipwa_ctx mipwa_ctx;                 /* opaque, owned by the library */
+
+typedef struct {
+    double m_parent, m1, m2, m3;                    /* GeV; m2 == m3 */
+} mipwa_kinematics;
+
+typedef struct {
+    double  mass, width;                            /* m0, Gamma0 in GeV (initial values when shape_floats = 1) */
+    int32_t spin;                                   /* L = 0, 1, 2; larger -> MIPWA_ERR_ARG */
+    int32_t shape_floats;                           /* 1: (mass, width) are read from the parameter vector */
+    double  r_res, r_parent;                        /* Blatt-Weisskopf radii, GeV^-1 */
+} mipwa_resonance;
+
+enum { MIPWA_OK = 0, MIPWA_ERR_ARG = -1, MIPWA_ERR_DOMAIN = -2, MIPWA_ERR_STATE = -3, MIPWA_ERR_CUDA = -4,
+       MIPWA_ERR_NOMEM = -5 };
+enum { MIPWA_MEM_HOST = 0, MIPWA_MEM_DEVICE = 1 };
+enum { MIPWA_PATH_AUTO = 0,            /* cached-dense if no shape floats and the basis fits, else recompute */
+       MIPWA_PATH_RECOMPUTE = 1,       /* every call re-evaluates every amplitude term (FP64-ALU bound) */
+       MIPWA_PATH_CACHED = 2,          /* fixed shapes: dense n_ev x K complex basis + K x K Gram (HBM bound) */
+       MIPWA_PATH_CACHED_COMPACT = 3 };/* fixed shapes: R complex resonance values per event; spline re-evaluated */
+
+#define MIPWA_MAX_KNOTS      128
+#define MIPWA_MAX_RESONANCES 16
+
+/* Create a context for one model on CUDA device `device`.
+ *   knots: n_knots strictly increasing positions in m^2 (HOST), 2 <= n_knots <= MIPWA_MAX_KNOTS
+ *   res:   n_res resonance descriptions (HOST), 0 <= n_res <= MIPWA_MAX_RESONANCES
+ * Errors: MIPWA_ERR_ARG (bad masses / knots / spin / radii / counts), MIPWA_ERR_CUDA (no device, not sm_100). */
+int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_knots,
+                 const mipwa_resonance* res, int32_t n_res, int32_t device, mipwa_ctx** out);
+void mipwa_destroy(mipwa_ctx* ctx);
+
+/* Use `cuda_stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream; NULL = default stream). */
+int mipwa_set_stream(mipwa_ctx* ctx, void* cuda_stream);
+
+/* Data events: n pairs (s12[i], s13[i]).  Every point is checked ON THE DEVICE against the Dalitz boundary
+ * ((m1+m2)^2 <= s12 <= (M-m3)^2 and s13 inside its band); a point outside -> MIPWA_ERR_DOMAIN and the slot is
+ * left empty.  n = 0 is allowed (the NLL is then 0).  Invalidates the cached basis. */
+int mipwa_set_events(mipwa_ctx* ctx, const double* s12, const double* s13, int64_t n, int32_t mem);
+
+/* Normalisation points with weights w (NULL: w_j = 1/n).  I = sum_j w_j |A_j|^2 stands for the integral of
+ * |A|^2 over the Dalitz plot ("calculated numerically based on evenly distributed grid points").
+ * Same boundary check and ownership rules as mipwa_set_events; n >= 1.  Invalidates the cached Gram matrix. */
+int mipwa_set_norm_points(mipwa_ctx* ctx, const double* s12, const double* s13, const double* w, int64_t n,
+                          int32_t mem);
+
+/* Length of the parameter vector: 2N + 2R + 2F (F = resonances with shape_floats). */
+int mipwa_n_params(const mipwa_ctx* ctx, int64_t* n);
+
+/* Select the evaluation path.  CACHED / CACHED_COMPACT with F > 0 -> MIPWA_ERR_STATE. */
+int mipwa_set_path(mipwa_ctx* ctx, int32_t path);
+
+/* Bytes of device memory the current path needs for its per-event cache with the current events
+ * (dense: n_ev * K * 16; compact: n_ev * (R * 16 + 16); recompute: 0), or a negative error code. */
+int64_t mipwa_basis_bytes(const mipwa_ctx* ctx);
+
+/* Optional caller-provided DEVICE storage for that cache (borrowed; >= mipwa_basis_bytes(), 256-byte aligned).
+ * Without it the library allocates on first use. */
+int mipwa_set_basis_buffer(mipwa_ctx* ctx, void* dev, int64_t bytes);
+
+/* One likelihood evaluation (what a minimiser calls once per step):  *nll = -sum ln|A|^2 + n_ev ln I.
+ * params: HOST, n_params doubles.  Errors: MIPWA_ERR_STATE before both mipwa_set_* calls, MIPWA_ERR_ARG on a
+ * wrong n_params or a non-positive floating mass/width. */
+int mipwa_nll(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll);
+
+/* Same, also returning the two pieces: sum_i ln|A_i|^2 and I (either pointer may be NULL). */
+int mipwa_nll_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* sum_log,
+                    double* integral);
+
+/* NLL and its analytic gradient with respect to the first 2N + 2R parameters (the linear coefficients in polar
+ * form; derivatives with respect to floating masses/widths are not provided, reading P16).
+ * grad: HOST, 2N + 2R doubles, laid out like params. */
+int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
+
+/* TEST HOOK: per-point |A|^2 from the same device function the NLL kernels use.
+ *   which = 0: the events slot, 1: the normalisation slot; out: HOST, n doubles, n = that slot's size. */
+int mipwa_eval_abs2(mipwa_ctx* ctx, const double* params, int64_t n_params, int32_t which, double* out, int64_t n);
+
+/* TEST HOOK: the cached basis row of `n` points of slot `which` as the CACHED path builds it:
+ *   out[(i*K + k)*2 + {0,1}] = Re, Im of B_ik, K = N + R (HOST, n*K*2 doubles), points i = first .. first+n-1. */
+int mipwa_eval_basis(mipwa_ctx* ctx, const double* params, int64_t n_params, int32_t which, int64_t first,
+                     int64_t n, double* out);
+
+/* Kernel timing (off by default: two extra event records per call).  When on, mipwa_last_kernel_ms returns the
+ * device time of the kernels of the last mipwa_nll / mipwa_nll_parts / mipwa_nll_grad call on this context in
+ * milliseconds, measured with CUDA events on the context's stream (for the benchmark's roofline numbers). */
+int mipwa_enable_timing(mipwa_ctx* ctx, int32_t on);
+int mipwa_last_kernel_ms(const mipwa_ctx* ctx, float* ms);
+
+/* Number of kernel launches issued by this context since creation (the benchmark's gpu_launches claim). */
+int64_t mipwa_launch_count(const mipwa_ctx* ctx);
+
+/* Measure the sustained FP64 FMA rate of the device with a register-resident DFMA loop on every SM for about
+ * `seconds` seconds; *tflops = 2 * FMAs / time.  Denominator of the ALU roofline. */
+int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops);
+
+const char* mipwa_last_error(const mipwa_ctx* ctx);   /* valid until the next call on ctx; "" if none */
+const char* mipwa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MIPWA_H */

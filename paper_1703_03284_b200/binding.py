@@ -1,0 +1,252 @@
+"""Thin ctypes binding of libmipwa.so (include/mipwa.h).  Argument marshalling only: every step of the hot path
+runs in the CUDA kernels behind the C ABI.  There is no CPU fallback: if the library is missing or no B200 is
+present, construction raises.
+
+Method names mirror the C entry points: Mipwa.set_events -> mipwa_set_events, Mipwa.nll -> mipwa_nll, ...
+Device arrays are passed as torch CUDA tensors (float64, contiguous) and are BORROWED by the library; host arrays
+are numpy float64 and are copied by the library.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmipwa.so")
+
+OK, ERR_ARG, ERR_DOMAIN, ERR_STATE, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4, -5
+MEM_HOST, MEM_DEVICE = 0, 1
+PATH_AUTO, PATH_RECOMPUTE, PATH_CACHED, PATH_CACHED_COMPACT = 0, 1, 2, 3
+_ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STATE: "MIPWA_ERR_STATE",
+              ERR_CUDA: "MIPWA_ERR_CUDA", ERR_NOMEM: "MIPWA_ERR_NOMEM"}
+
+# every symbol include/mipwa.h declares
+SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
+           "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
+           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
+           "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
+           "mipwa_version"]
+
+
+class MipwaError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"{_ERR_NAMES.get(code, code)}: {text}")
+        self.code = code
+
+
+class Kinematics(C.Structure):
+    _fields_ = [("m_parent", C.c_double), ("m1", C.c_double), ("m2", C.c_double), ("m3", C.c_double)]
+
+
+class Resonance(C.Structure):
+    _fields_ = [("mass", C.c_double), ("width", C.c_double), ("spin", C.c_int32), ("shape_floats", C.c_int32),
+                ("r_res", C.c_double), ("r_parent", C.c_double)]
+
+
+_dp = C.POINTER(C.c_double)
+_lib = None
+
+
+def load_library():
+    """dlopen libmipwa.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1703_03284_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, d = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    L.mipwa_create.restype = i32
+    L.mipwa_create.argtypes = [C.POINTER(Kinematics), _dp, i32, C.POINTER(Resonance), i32, i32, C.POINTER(vp)]
+    L.mipwa_destroy.restype = None; L.mipwa_destroy.argtypes = [vp]
+    L.mipwa_set_stream.restype = i32; L.mipwa_set_stream.argtypes = [vp, vp]
+    L.mipwa_set_events.restype = i32; L.mipwa_set_events.argtypes = [vp, vp, vp, i64, i32]
+    L.mipwa_set_norm_points.restype = i32; L.mipwa_set_norm_points.argtypes = [vp, vp, vp, vp, i64, i32]
+    L.mipwa_n_params.restype = i32; L.mipwa_n_params.argtypes = [vp, C.POINTER(i64)]
+    L.mipwa_set_path.restype = i32; L.mipwa_set_path.argtypes = [vp, i32]
+    L.mipwa_basis_bytes.restype = i64; L.mipwa_basis_bytes.argtypes = [vp]
+    L.mipwa_set_basis_buffer.restype = i32; L.mipwa_set_basis_buffer.argtypes = [vp, vp, i64]
+    L.mipwa_nll.restype = i32; L.mipwa_nll.argtypes = [vp, _dp, i64, _dp]
+    L.mipwa_nll_parts.restype = i32; L.mipwa_nll_parts.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
+    L.mipwa_nll_grad.restype = i32; L.mipwa_nll_grad.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_eval_abs2.restype = i32; L.mipwa_eval_abs2.argtypes = [vp, _dp, i64, i32, _dp, i64]
+    L.mipwa_eval_basis.restype = i32; L.mipwa_eval_basis.argtypes = [vp, _dp, i64, i32, i64, i64, _dp]
+    L.mipwa_enable_timing.restype = i32; L.mipwa_enable_timing.argtypes = [vp, i32]
+    L.mipwa_last_kernel_ms.restype = i32; L.mipwa_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.mipwa_launch_count.restype = i64; L.mipwa_launch_count.argtypes = [vp]
+    L.mipwa_measure_fp64_peak.restype = i32; L.mipwa_measure_fp64_peak.argtypes = [i32, d, _dp]
+    L.mipwa_last_error.restype = C.c_char_p; L.mipwa_last_error.argtypes = [vp]
+    L.mipwa_version.restype = C.c_char_p; L.mipwa_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _host(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _dev_ptr(t, n=None):
+    import torch
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("device arrays must be contiguous float64 CUDA tensors")
+    if n is not None and t.numel() != n:
+        raise ValueError("array lengths differ")
+    return C.c_void_p(t.data_ptr())
+
+
+class Mipwa:
+    """One model context (mipwa_create ... mipwa_destroy)."""
+
+    def __init__(self, kin, knots, resonances, device=0):
+        self.L = load_library()
+        if isinstance(kin, dict):
+            kin = (kin["M"], kin["m1"], kin["m2"], kin["m3"])
+        self._kin = Kinematics(*[float(v) for v in kin])
+        knots = _host(knots)
+        res = (Resonance * max(len(resonances), 1))()
+        for i, r in enumerate(resonances):
+            res[i] = Resonance(float(r["mass"]), float(r["width"]), int(r["spin"]), int(r.get("shape_floats", 0)),
+                               float(r["r_res"]), float(r["r_parent"]))
+        self.N, self.R = int(knots.size), len(resonances)
+        self.K = self.N + self.R
+        self._h = C.c_void_p()
+        rc = self.L.mipwa_create(C.byref(self._kin), knots.ctypes.data_as(_dp), self.N, res, self.R, int(device),
+                                 C.byref(self._h))
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise MipwaError(rc, "mipwa_create failed (bad model, or no sm_100 CUDA device: there is no CPU path)")
+        self.device = int(device)
+        self._keep = {}                     # borrowed tensors kept alive
+        n = C.c_int64()
+        self._check(self.L.mipwa_n_params(self._h, C.byref(n)))
+        self.n_params = n.value
+        self.n_events = self.n_norm = -1
+
+    def _check(self, rc):
+        if rc != OK:
+            raise MipwaError(rc, self.L.mipwa_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self.L.mipwa_destroy(self._h)
+            self._h = C.c_void_p()
+            self._keep = {}
+
+    __del__ = close
+
+    def set_stream(self, stream):
+        """stream: a torch.cuda.Stream, a raw cudaStream_t integer, or None (default stream)."""
+        ptr = getattr(stream, "cuda_stream", stream)
+        self._check(self.L.mipwa_set_stream(self._h, C.c_void_p(ptr or 0)))
+
+    def _set(self, fn, name, arrays, n_extra_ok):
+        s12 = arrays[0]
+        if _is_torch(s12):
+            n = s12.numel()
+            ptrs = [_dev_ptr(a, n) for a in arrays]
+            self._keep[name] = arrays
+            self._check(fn(self._h, *ptrs, n, MEM_DEVICE))
+        else:
+            host = [None if a is None else _host(a) for a in arrays]
+            n = host[0].size
+            if any(h is not None and h.size != n for h in host):
+                raise ValueError("array lengths differ")
+            ptrs = [None if h is None else C.c_void_p(h.ctypes.data) for h in host]
+            self._keep.pop(name, None)
+            self._check(fn(self._h, *ptrs, n, MEM_HOST))
+        return n
+
+    def set_events(self, s12, s13):
+        self.n_events = -1
+        self.n_events = self._set(self.L.mipwa_set_events, "ev", [s12, s13], False)
+
+    def set_norm_points(self, s12, s13, w=None):
+        self.n_norm = -1
+        self.n_norm = self._set(self.L.mipwa_set_norm_points, "nm", [s12, s13, w], True)
+
+    def set_path(self, path):
+        self._check(self.L.mipwa_set_path(self._h, int(path)))
+
+    def basis_bytes(self):
+        n = self.L.mipwa_basis_bytes(self._h)
+        if n < 0:
+            self._check(int(n))
+        return int(n)
+
+    def set_basis_buffer(self, tensor):
+        import torch
+        if not (tensor.is_cuda and tensor.is_contiguous()):
+            raise TypeError("basis buffer must be a contiguous CUDA tensor")
+        self._keep["basis"] = tensor
+        self._check(self.L.mipwa_set_basis_buffer(self._h, C.c_void_p(tensor.data_ptr()),
+                                                  tensor.numel() * tensor.element_size()))
+
+    def _params(self, params):
+        p = _host(params)
+        return p, p.ctypes.data_as(_dp), p.size
+
+    def nll(self, params):
+        p, pp, n = self._params(params)
+        out = C.c_double()
+        self._check(self.L.mipwa_nll(self._h, pp, n, C.byref(out)))
+        return out.value
+
+    def nll_parts(self, params):
+        p, pp, n = self._params(params)
+        out, sl, integ = C.c_double(), C.c_double(), C.c_double()
+        self._check(self.L.mipwa_nll_parts(self._h, pp, n, C.byref(out), C.byref(sl), C.byref(integ)))
+        return out.value, sl.value, integ.value
+
+    def nll_grad(self, params):
+        p, pp, n = self._params(params)
+        out = C.c_double()
+        grad = np.empty(2 * self.N + 2 * self.R)
+        self._check(self.L.mipwa_nll_grad(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
+        return out.value, grad
+
+    def eval_abs2(self, params, which=0):
+        p, pp, n = self._params(params)
+        size = self.n_events if which == 0 else self.n_norm
+        out = np.empty(max(size, 0))
+        self._check(self.L.mipwa_eval_abs2(self._h, pp, n, int(which), out.ctypes.data_as(_dp), size))
+        return out
+
+    def eval_basis(self, params, which=0, first=0, count=None):
+        p, pp, n = self._params(params)
+        size = self.n_events if which == 0 else self.n_norm
+        count = size - first if count is None else count
+        out = np.empty((count, self.K, 2))
+        self._check(self.L.mipwa_eval_basis(self._h, pp, n, int(which), int(first), int(count),
+                                            out.ctypes.data_as(_dp)))
+        return out[..., 0] + 1j * out[..., 1]
+
+    def enable_timing(self, on=True):
+        self._check(self.L.mipwa_enable_timing(self._h, int(bool(on))))
+
+    def last_kernel_ms(self):
+        ms = C.c_float()
+        self._check(self.L.mipwa_last_kernel_ms(self._h, C.byref(ms)))
+        return ms.value
+
+    def launch_count(self):
+        return int(self.L.mipwa_launch_count(self._h))
+
+
+def measure_fp64_peak(device=0, seconds=2.0):
+    L = load_library()
+    out = C.c_double()
+    rc = L.mipwa_measure_fp64_peak(int(device), float(seconds), C.byref(out))
+    if rc != OK:
+        raise MipwaError(rc, "mipwa_measure_fp64_peak failed")
+    return out.value
+
+
+def version():
+    return load_library().mipwa_version().decode()

@@ -1,0 +1,186 @@
+// dev_model.cuh -- the per-call model block handed to every kernel, and the per-point amplitude device function.
+//
+// Operation definitions: include/mipwa.h (Eq. 1; spline PAPER.md:29; Breit-Wigner x angular factor
+// PAPER.md:27; symmetrisation PAPER.md:47).  This file restates them in the form the FP64 pipe likes:
+//
+//   per channel x (= s12 or s13), other = y:
+//     lam1 = lambda(x, m1^2, m2^2) = (x - (m1+m2)^2)(x - (m1-m2)^2)          [factored: no cancellation at threshold]
+//     lam2 = lambda(M^2, x, m3^2)  = ((M-m3)^2 - x)((M+m3)^2 - x)
+//     ix = 1/x,  ql = lam1 ix = 4 q^2,  pl = lam2 ix,  g = sqrt(lam1) ix / 2 = sqrt(q^2 / x)
+//     Z1 = x + 2y - Sigma + kappa ix,  Z2 = Z1^2 - ql pl / 3
+//   per resonance (spin L, constants prepared on the host, step A3):
+//     D_R = den_L(cR ql), D_D = den_L(cD lam2), den_1(z) = 1 + z, den_2(z) = 9 + 3z + z^2
+//     W'  = Kw g ql^L                       [= m0 Gamma(x) D_R: the running width without its barrier denominator]
+//     dD  = (m0^2 - x) D_R,  E = dD^2 + W'^2
+//     F_D F_R BW = sqrt(n_R n_D) D_R (dD + i W') / (sqrt(D_R D_D) E) = sqrt(n_R n_D) D_R (dD + i W') rsqrt(D_R D_D E^2)
+//   so that ONE reciprocal square root per resonance and channel replaces two square roots and three divisions.
+//   sqrt(n_R n_D) is folded into the coefficient on the host.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define MIPWA_DEV_MAX_KNOTS 128
+#define MIPWA_DEV_MAX_RES 16
+#define MIPWA_DEV_LUT 512
+
+struct ResDev {
+    double m0sq;      // m0^2
+    double cR;        // r_res^2 / 4            (z_R = cR * ql);  0 for L = 0
+    double cD;        // r_parent^2 / (4 M^2)   (z_D = cD * lam2); 0 for L = 0
+    double Kw;        // m0^2 Gamma0 n_R / ((4 q0^2)^L sqrt(q0^2))
+    double cre, cim;  // c_r * sqrt(n_R n_D)
+    int32_t L;
+    int32_t pad;
+};
+
+// Everything a kernel needs for one likelihood call; passed by value as a __grid_constant__ kernel parameter.
+struct DevModel {
+    int32_t N;                 // knots
+    int32_t R;                 // resonances
+    int32_t nlut;              // buckets in lut
+    int32_t pad0;
+    double t_lo, t_d;          // (m1+m2)^2, (m1-m2)^2
+    double s_hi, s_top;        // (M-m3)^2, (M+m3)^2
+    double sigma;              // M^2 + m1^2 + m2^2 + m3^2
+    double kappa;              // (M^2 - m3^2)(m2^2 - m1^2)
+    double lut_x0, lut_inv;    // bucket = (s - lut_x0) * lut_inv
+    double knots[MIPWA_DEV_MAX_KNOTS];
+    double2 sc[4][MIPWA_DEV_MAX_KNOTS];   // segment j: S(s) = sc[0][j] + t(sc[1][j] + t(sc[2][j] + t sc[3][j])), t = s - x_j
+    uint8_t lut[MIPWA_DEV_LUT];           // segment that contains the left edge of each bucket
+    ResDev res[MIPWA_DEV_MAX_RES];
+};
+
+// Shared-memory copy of the spline tables (divergent lookups: constant memory would serialise them).
+struct SplineSmem {
+    double knots[MIPWA_DEV_MAX_KNOTS];
+    double2 sc[4][MIPWA_DEV_MAX_KNOTS];
+    uint8_t lut[MIPWA_DEV_LUT];
+};
+
+__device__ __forceinline__ void load_spline_smem(SplineSmem& sm, const DevModel& m)
+{
+    for (int i = threadIdx.x; i < m.N; i += blockDim.x) {
+        sm.knots[i] = m.knots[i];
+        sm.sc[0][i] = m.sc[0][i]; sm.sc[1][i] = m.sc[1][i]; sm.sc[2][i] = m.sc[2][i]; sm.sc[3][i] = m.sc[3][i];
+    }
+    for (int i = threadIdx.x; i < m.nlut; i += blockDim.x) sm.lut[i] = m.lut[i];
+    __syncthreads();
+}
+
+// ---- fp64 reciprocal / reciprocal square root: MUFU seed + ONE third-order correction step ----------------------
+// The seeds (MUFU.RCP64H / MUFU.RSQ64H) look only at the upper 32 bits of the argument: relative error <= ~2^-20.
+// With e = 1 - x y (resp. 1 - x y^2, |e| <= ~2^-19) the series 1/(1-e) = 1 + e + e^2 + O(e^3) and
+// (1-e)^(-1/2) = 1 + e/2 + 3e^2/8 + O(e^3) leave a truncation error below 2^-57, under the rounding of the last fma:
+// results are good to ~1 ulp.  Arguments here are finite, normal and positive (x >= (m1+m2)^2 > 0; denominators
+// are sums of squares plus positive constants), so the special-case paths of the library routines are not needed.
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);
+}
+
+__device__ __forceinline__ double fast_rsqrt(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x * y, y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
+}
+
+// segment index j with x_j <= s < x_{j+1}, clamped to [0, N-2] (beyond the end knots the end cubic is used)
+__device__ __forceinline__ int spline_segment(const SplineSmem& sm, const DevModel& m, double s, double& xj)
+{
+    int b = __double2int_rd((s - m.lut_x0) * m.lut_inv);
+    b = max(0, min(b, m.nlut - 1));
+    int j = sm.lut[b];
+    xj = sm.knots[j];
+    double xn = sm.knots[j + 1];
+    while (s >= xn && j < m.N - 2) { ++j; xj = xn; xn = sm.knots[j + 1]; }
+    if (s < xj && j > 0) { --j; xj = sm.knots[j]; }     // guards the rounding of the bucket index
+    return j;
+}
+
+__device__ __forceinline__ void spline_eval(const SplineSmem& sm, const DevModel& m, double s, double& re, double& im)
+{
+    double xj;
+    const int j = spline_segment(sm, m, s, xj);
+    const double t = s - xj;
+    const double2 c0 = sm.sc[0][j], c1 = sm.sc[1][j], c2 = sm.sc[2][j], c3 = sm.sc[3][j];
+    re = fma(t, fma(t, fma(t, c3.x, c2.x), c1.x), c0.x);
+    im = fma(t, fma(t, fma(t, c3.y, c2.y), c1.y), c0.y);
+}
+
+// per-channel kinematic quantities shared by all resonances
+struct Channel {
+    double x, lam2, ql, w0, Z1, Z2;      // w0 = g (L = 0 width factor); w1 = g ql; w2 = g ql^2 derived on the fly
+};
+
+__device__ __forceinline__ Channel make_channel(const DevModel& m, double x, double y)
+{
+    Channel c;
+    c.x = x;
+    const double lam1 = (x - m.t_lo) * (x - m.t_d);
+    c.lam2 = (m.s_hi - x) * (m.s_top - x);
+    const double ix = fast_rcp(x);
+    c.ql = lam1 * ix;
+    const double pl = c.lam2 * ix;
+    // sqrt(lam1) = lam1 * rsqrt(lam1); lam1 -> 0 at threshold, where the width vanishes
+    const double sq = lam1 > 1e-300 ? lam1 * fast_rsqrt(lam1) : 0.0;
+    c.w0 = 0.5 * sq * ix;
+    c.Z1 = fma(m.kappa, ix, fma(2.0, y, x) - m.sigma);
+    c.Z2 = fma(c.Z1, c.Z1, (-1.0 / 3.0) * (c.ql * pl));
+    return c;
+}
+
+// c_r sqrt(n_R n_D) is applied by the caller: returns F_D F_R Z_L BW / sqrt(n_R n_D) for one channel
+__device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel& c, double& tre, double& tim)
+{
+    double DR, DD, W, Z;
+    if (r.L == 1) {
+        DR = fma(r.cR, c.ql, 1.0);
+        DD = fma(r.cD, c.lam2, 1.0);
+        W = r.Kw * (c.w0 * c.ql);
+        Z = c.Z1;
+    } else if (r.L == 2) {
+        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
+        DR = fma(zR, zR + 3.0, 9.0);
+        DD = fma(zD, zD + 3.0, 9.0);
+        W = r.Kw * (c.w0 * c.ql * c.ql);
+        Z = c.Z2;
+    } else {
+        DR = 1.0; DD = 1.0;
+        W = r.Kw * c.w0;
+        Z = 1.0;
+    }
+    const double dD = (r.m0sq - c.x) * DR;
+    const double E = fma(dD, dD, W * W);
+    const double rs = fast_rsqrt((DR * DD) * (E * E));
+    const double t = Z * DR * rs;
+    tre = t * dD;
+    tim = t * W;
+}
+
+// A(s12,s13) = S(s12) + S(s13) + sum_r c_r [T_r(s12,s13) + T_r(s13,s12)]
+__device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& m, double s12, double s13,
+                                          double& are, double& aim)
+{
+    double r1, i1, r2, i2;
+    spline_eval(sm, m, s12, r1, i1);
+    spline_eval(sm, m, s13, r2, i2);
+    are = r1 + r2;
+    aim = i1 + i2;
+    if (m.R > 0) {
+        const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
+        for (int r = 0; r < m.R; ++r) {
+            const ResDev& rd = m.res[r];
+            double ar, ai, br, bi;
+            resonance_channel(rd, ca, ar, ai);
+            resonance_channel(rd, cb, br, bi);
+            const double tr = ar + br, ti = ai + bi;
+            are = fma(rd.cre, tr, fma(-rd.cim, ti, are));
+            aim = fma(rd.cre, ti, fma(rd.cim, tr, aim));
+        }
+    }
+}

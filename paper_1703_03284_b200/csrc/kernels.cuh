@@ -1,0 +1,183 @@
+// kernels.cuh -- the recompute path: fused amplitude + log-sum / normalisation reduction,
+// the per-point test hook, and the boundary check.  sm_100a only.
+#pragma once
+#include "dev_model.cuh"
+
+#define MIPWA_BLOCK 256
+
+// ---- deterministic block reduction of NV doubles per thread: warp shuffles, then shared memory -------------------
+template <int NV>
+__device__ __forceinline__ void block_reduce(double (&v)[NV], double* red /* [NV][32] in smem */)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v[k] += __shfl_down_sync(0xffffffffu, v[k], off);
+        if (lane == 0) red[k * 32 + warp] = v[k];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            double x = lane < nwarp ? red[k * 32 + lane] : 0.0;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+            v[k] = x;                                   // valid in thread 0
+        }
+    }
+    __syncthreads();
+}
+
+// Running product of |A|^2 with the exponents peeled off by integer operations: ln prod = ln(mantissa product)
+// + (exponent sum) ln 2.  One DMUL per event instead of a ~30-instruction fp64 log; the log is taken once per
+// LOGPROD_FLUSH events per thread.  Zero, denormal, inf and NaN values take the plain log so that IEEE specials
+// propagate exactly as in -sum ln|A|^2.
+#define LOGPROD_FLUSH 512
+struct LogProd {
+    double prod = 1.0, sum = 0.0;
+    int esum = 0, cnt = 0;
+    __device__ __forceinline__ void flush()
+    {
+        // ln2 split hi/lo so that esum * ln2 carries no rounding of its own
+        sum += fma((double)esum, 6.93147180369123816490e-01, fma((double)esum, 1.90821492927058770002e-10, log(prod)));
+        prod = 1.0; esum = 0; cnt = 0;
+    }
+    __device__ __forceinline__ void add(double v)
+    {
+        const int hi = __double2hiint(v);
+        const int ex = (hi >> 20) & 0x7ff;               // v >= 0 or NaN: the sign bit lands in the NaN branch
+        if (ex == 0 || ex == 0x7ff || hi < 0) {
+            sum += log(v);
+        } else {
+            esum += ex - 1023;
+            prod *= __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(v));
+            if (++cnt == LOGPROD_FLUSH) flush();
+        }
+    }
+    __device__ __forceinline__ double value() { flush(); return sum; }
+};
+
+// ---- A4-A6: one launch over [events | normalisation points] ------------------------------------------------------
+// Persistent grid (a multiple of the SM count).  Per thread: grid-stride over events (coalesced 8-byte loads of
+// s12[i], s13[i]; nothing is written per event), then over normalisation points.  Block partials go to
+// partials[block] = (sum ln|A|^2, sum w|A|^2); the last block to finish adds them in block order (fixed order:
+// bit-reproducible for a given grid) and writes the two totals to `result` (mapped pinned host memory).
+__global__ void __launch_bounds__(MIPWA_BLOCK, 2)
+k_nll_recompute(const __grid_constant__ DevModel m,
+                const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
+                const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
+                long long n_norm, double2* __restrict__ partials, unsigned int* __restrict__ ticket,
+                double* __restrict__ result)
+{
+    __shared__ SplineSmem sm;
+    __shared__ double red[2 * 32];
+    __shared__ bool is_last;
+    load_spline_smem(sm, m);
+
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+
+    LogProd lp;
+    for (long long i = t0; i < n_ev; i += stride) {
+        double re, im;
+        amplitude(sm, m, e12[i], e13[i], re, im);
+        lp.add(fma(re, re, im * im));
+    }
+    double integ = 0.0;
+    if (gw) {
+        for (long long j = t0; j < n_norm; j += stride) {
+            double re, im;
+            amplitude(sm, m, g12[j], g13[j], re, im);
+            integ = fma(gw[j], fma(re, re, im * im), integ);
+        }
+    } else {
+        for (long long j = t0; j < n_norm; j += stride) {
+            double re, im;
+            amplitude(sm, m, g12[j], g13[j], re, im);
+            integ += fma(re, re, im * im);
+        }
+    }
+
+    double v[2] = { lp.value(), integ };
+    block_reduce<2>(v, red);
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = make_double2(v[0], v[1]);
+        __threadfence();
+        is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double f[2] = { 0.0, 0.0 };
+        for (int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+            const double2 p = __ldcg(&partials[b]);
+            f[0] += p.x; f[1] += p.y;
+        }
+        block_reduce<2>(f, red);
+        if (threadIdx.x == 0) {
+            result[0] = f[0];
+            result[1] = f[1];
+            *ticket = 0;                                  // ready for the next call
+            __threadfence_system();
+        }
+    }
+}
+
+// ---- test hook: |A|^2 per point from the same device function ---------------------------------------------------
+__global__ void __launch_bounds__(MIPWA_BLOCK)
+k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
+       long long n, double* __restrict__ out)
+{
+    __shared__ SplineSmem sm;
+    load_spline_smem(sm, m);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        double re, im;
+        amplitude(sm, m, s12[i], s13[i], re, im);
+        out[i] = fma(re, re, im * im);
+    }
+}
+
+// ---- boundary check of mipwa_set_events / mipwa_set_norm_points ---------------------------------------------------
+// inside iff (m1+m2)^2 <= s12 <= (M-m3)^2 and |s13 - centre(s12)| <= half(s12); a relative slack of 1e-12 keeps
+// points that the caller's own fp64 boundary test placed exactly on the edge.  Counts offenders into *bad.
+struct DevKin { double M2, m1s, m2s, m3s, t_lo, t_d, s_hi, s_top; };
+
+__global__ void __launch_bounds__(MIPWA_BLOCK)
+k_validate(const DevKin k, const double* __restrict__ s12, const double* __restrict__ s13, long long n,
+           unsigned long long* __restrict__ bad)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    unsigned int mine = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const double x = s12[i], y = s13[i];
+        const double slack = 1e-12;
+        bool ok = x >= k.t_lo * (1.0 - slack) && x <= k.s_hi * (1.0 + slack);
+        if (ok) {
+            const double centre = k.m1s + k.m3s + (x + k.m1s - k.m2s) * (k.M2 - x - k.m3s) / (2.0 * x);
+            const double prod = ((x - k.t_lo) * (x - k.t_d)) * ((k.s_hi - x) * (k.s_top - x));
+            const double half = sqrt(fmax(prod, 0.0)) / (2.0 * x);
+            ok = fabs(y - centre) <= half + slack * (fabs(centre) + half) + 1e-13;
+        }
+        mine += ok ? 0u : 1u;                             // NaN compares false above -> counted as bad
+    }
+    mine = __reduce_add_sync(0xffffffffu, mine);
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(bad, (unsigned long long)mine);
+}
+
+// ---- FP64 peak: register-resident dependent-chain DFMA loop, 8 independent chains per thread --------------------
+__global__ void __launch_bounds__(256)
+k_dfma_peak(double* __restrict__ out, long long iters, double a, double b)
+{
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456) out[0] = s;                          // keeps the chains alive
+}

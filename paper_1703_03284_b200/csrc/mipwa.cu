@@ -1,0 +1,494 @@
+// mipwa.cu -- host side of libmipwa: context, per-call model preparation (A1-A3), launches, C ABI (include/mipwa.h).
+// No CPU fallback: every numeric result comes from the kernels in kernels.cuh / cached.cuh / grad.cuh.
+#include "../../include/mipwa.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+static_assert(MIPWA_DEV_MAX_KNOTS == MIPWA_MAX_KNOTS, "capacity mismatch");
+static_assert(MIPWA_DEV_MAX_RES == MIPWA_MAX_RESONANCES, "capacity mismatch");
+static_assert(sizeof(DevModel) < 32000, "DevModel must fit the kernel parameter space");
+
+namespace {
+
+struct Slot {                       // events or normalisation points
+    const double* s12 = nullptr;
+    const double* s13 = nullptr;
+    const double* w = nullptr;
+    int64_t n = -1;                 // -1: not set
+    void* owned[3] = { nullptr, nullptr, nullptr };
+};
+
+}  // namespace
+
+struct mipwa_ctx {
+    mipwa_kinematics kin;
+    int N = 0, R = 0, F = 0;
+    std::vector<double> knots;
+    std::vector<mipwa_resonance> res;
+    int device = 0;
+    int sm_count = 0;
+    cudaStream_t stream = nullptr;
+    int path = MIPWA_PATH_AUTO;
+
+    // natural-spline system (A2): the tridiagonal matrix depends on the knots only -> factor once
+    std::vector<double> sp_sub, sp_inv, sp_cp;     // sub-diagonal, 1/pivot, modified super-diagonal
+    std::vector<uint8_t> lut;
+    int nlut = 0;
+    double lut_x0 = 0, lut_inv = 0;
+
+    Slot ev, nm;
+
+    // workspaces
+    int blocks_per_sm = 0;
+    double2* d_partials = nullptr;
+    unsigned int* d_ticket = nullptr;
+    double* h_result = nullptr;     // mapped pinned: [0] sum ln|A|^2, [1] sum w|A|^2, [2..] spare
+    double* d_result = nullptr;     // device alias of h_result
+    unsigned long long* h_bad = nullptr;
+    unsigned long long* d_bad = nullptr;
+
+    DevModel model;                 // staging for the current call
+    std::vector<double> y_re, y_im, ypp_re, ypp_im;
+
+    bool timing = false;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    float last_ms = 0.f;
+    int64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(mipwa_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+
+#define CU(ctx, call)                                                                             \
+    do {                                                                                          \
+        cudaError_t e__ = (call);                                                                 \
+        if (e__ != cudaSuccess)                                                                   \
+            return fail(ctx, e__ == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, \
+                        std::string(#call) + ": " + cudaGetErrorString(e__));                     \
+    } while (0)
+
+double lam(double a, double b, double c) { return (a - b - c) * (a - b - c) - 4.0 * b * c; }
+
+double barrier_num(int L, double z0) { return L == 0 ? 1.0 : (L == 1 ? 1.0 + z0 : 9.0 + 3.0 * z0 + z0 * z0); }
+
+// A3: constants of one resonance for the device formulas of dev_model.cuh
+int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, double carg, ResDev* out)
+{
+    const mipwa_kinematics& k = c->kin;
+    const mipwa_resonance& d = c->res[r];
+    if (!(m0 > k.m1 + k.m2) || !(m0 < k.m_parent - k.m3) || !(g0 > 0.0) || !std::isfinite(m0) || !std::isfinite(g0))
+        return fail(c, MIPWA_ERR_ARG, "resonance " + std::to_string(r) + ": need m1+m2 < mass < M-m3 and width > 0");
+    const double M2 = k.m_parent * k.m_parent, m0sq = m0 * m0;
+    const double q0sq = lam(m0sq, k.m1 * k.m1, k.m2 * k.m2) / (4.0 * m0sq);
+    const double p0sq = lam(M2, m0sq, k.m3 * k.m3) / (4.0 * M2);
+    const int L = d.spin;
+    const double nR = barrier_num(L, d.r_res * d.r_res * q0sq), nD = barrier_num(L, d.r_parent * d.r_parent * p0sq);
+    out->m0sq = m0sq;
+    out->cR = L ? 0.25 * d.r_res * d.r_res : 0.0;
+    out->cD = L ? d.r_parent * d.r_parent / (4.0 * M2) : 0.0;
+    out->Kw = m0sq * g0 * nR / (std::pow(4.0 * q0sq, L) * std::sqrt(q0sq));
+    const double f = cmag * std::sqrt(nR * nD);
+    out->cre = f * std::cos(carg);
+    out->cim = f * std::sin(carg);
+    out->L = L;
+    out->pad = 0;
+    return MIPWA_OK;
+}
+
+// A2: second derivatives of the natural spline through (x_k, y_k) with the pre-factored tridiagonal system
+void spline_solve(const mipwa_ctx* c, const double* y, double* ypp)
+{
+    const int n = c->N;
+    const double* x = c->knots.data();
+    for (int i = 0; i < n; ++i) ypp[i] = 0.0;
+    const int m = n - 2;
+    if (m < 1) return;
+    std::vector<double> d(m);
+    for (int i = 0; i < m; ++i) {
+        const double rhs = (y[i + 2] - y[i + 1]) / (x[i + 2] - x[i + 1]) - (y[i + 1] - y[i]) / (x[i + 1] - x[i]);
+        d[i] = (i == 0 ? rhs : rhs - c->sp_sub[i] * d[i - 1]) * c->sp_inv[i];
+    }
+    ypp[m] = d[m - 1];
+    for (int i = m - 2; i >= 0; --i) ypp[i + 1] = d[i] - c->sp_cp[i] * ypp[i + 2];
+}
+
+void spline_factor(mipwa_ctx* c)
+{
+    const int n = c->N, m = n - 2;
+    const double* x = c->knots.data();
+    c->sp_sub.assign(std::max(m, 0), 0.0); c->sp_inv.assign(std::max(m, 0), 0.0); c->sp_cp.assign(std::max(m, 0), 0.0);
+    for (int i = 0; i < m; ++i) {
+        const double sub = (x[i + 1] - x[i]) / 6.0, dia = (x[i + 2] - x[i]) / 3.0, sup = (x[i + 2] - x[i + 1]) / 6.0;
+        const double piv = i == 0 ? dia : dia - sub * c->sp_cp[i - 1];
+        c->sp_sub[i] = sub;
+        c->sp_inv[i] = 1.0 / piv;
+        c->sp_cp[i] = sup / piv;
+    }
+    // bucket table for the segment search: lut[b] = segment containing the left edge of bucket b
+    c->nlut = std::min(MIPWA_DEV_LUT, std::max(64, 4 * n));
+    c->lut_x0 = x[0];
+    c->lut_inv = c->nlut / (x[n - 1] - x[0]);
+    c->lut.assign(c->nlut, 0);
+    for (int b = 0; b < c->nlut; ++b) {
+        const double edge = x[0] + b / c->lut_inv;
+        int j = 0;
+        while (j < n - 2 && edge >= x[j + 1]) ++j;
+        c->lut[b] = (uint8_t)j;
+    }
+}
+
+// A1-A3: parameters -> DevModel
+int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
+{
+    const int N = c->N, R = c->R;
+    if (n_params != 2 * N + 2 * R + 2 * c->F)
+        return fail(c, MIPWA_ERR_ARG, "n_params must be " + std::to_string(2 * N + 2 * R + 2 * c->F));
+    for (int64_t i = 0; i < n_params; ++i)
+        if (!std::isfinite(p[i])) return fail(c, MIPWA_ERR_ARG, "non-finite parameter " + std::to_string(i));
+    DevModel& m = c->model;
+    const mipwa_kinematics& k = c->kin;
+    m.N = N; m.R = R; m.nlut = c->nlut; m.pad0 = 0;
+    m.t_lo = (k.m1 + k.m2) * (k.m1 + k.m2);
+    m.t_d = (k.m1 - k.m2) * (k.m1 - k.m2);
+    m.s_hi = (k.m_parent - k.m3) * (k.m_parent - k.m3);
+    m.s_top = (k.m_parent + k.m3) * (k.m_parent + k.m3);
+    m.sigma = k.m_parent * k.m_parent + k.m1 * k.m1 + k.m2 * k.m2 + k.m3 * k.m3;
+    m.kappa = (k.m_parent * k.m_parent - k.m3 * k.m3) * (k.m2 * k.m2 - k.m1 * k.m1);
+    m.lut_x0 = c->lut_x0; m.lut_inv = c->lut_inv;
+    std::memcpy(m.lut, c->lut.data(), c->nlut);
+    for (int i = 0; i < N; ++i) {
+        m.knots[i] = c->knots[i];
+        c->y_re[i] = p[i] * std::cos(p[N + i]);            // y_k = a_k e^{i phi_k}
+        c->y_im[i] = p[i] * std::sin(p[N + i]);
+    }
+    spline_solve(c, c->y_re.data(), c->ypp_re.data());
+    spline_solve(c, c->y_im.data(), c->ypp_im.data());
+    for (int j = 0; j < N - 1; ++j) {                       // cubic in t = s - x_j on segment j
+        const double h = c->knots[j + 1] - c->knots[j];
+        const double* Y[2] = { c->y_re.data(), c->y_im.data() };
+        const double* P[2] = { c->ypp_re.data(), c->ypp_im.data() };
+        double co[4][2];
+        for (int q = 0; q < 2; ++q) {
+            co[0][q] = Y[q][j];
+            co[1][q] = (Y[q][j + 1] - Y[q][j]) / h - h * (2.0 * P[q][j] + P[q][j + 1]) / 6.0;
+            co[2][q] = 0.5 * P[q][j];
+            co[3][q] = (P[q][j + 1] - P[q][j]) / (6.0 * h);
+        }
+        for (int q = 0; q < 4; ++q) m.sc[q][j] = make_double2(co[q][0], co[q][1]);
+    }
+    for (int q = 0; q < 4; ++q) m.sc[q][N - 1] = make_double2(0.0, 0.0);
+    int f = 0;
+    for (int r = 0; r < R; ++r) {
+        double m0 = c->res[r].mass, g0 = c->res[r].width;
+        if (c->res[r].shape_floats) { m0 = p[2 * N + 2 * R + 2 * f]; g0 = p[2 * N + 2 * R + 2 * f + 1]; ++f; }
+        const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[r]);
+        if (rc) return rc;
+    }
+    return MIPWA_OK;
+}
+
+int use_device(mipwa_ctx* c)
+{
+    CU(c, cudaSetDevice(c->device));
+    return MIPWA_OK;
+}
+
+int grid_for(const mipwa_ctx* c, int64_t n, int blocks_per_sm)
+{
+    const int64_t full = (int64_t)c->sm_count * blocks_per_sm;
+    const int64_t need = (n + MIPWA_BLOCK - 1) / MIPWA_BLOCK;
+    return (int)std::max<int64_t>(1, std::min(full, need));
+}
+
+void free_slot(Slot& s)
+{
+    for (void*& p : s.owned) { if (p) cudaFree(p); p = nullptr; }
+    s = Slot();
+}
+
+}  // namespace
+
+// =================================================================================================================
+// C ABI
+// =================================================================================================================
+extern "C" {
+
+const char* mipwa_version(void) { return "mipwa-b200 0.1 (sm_100a)"; }
+
+const char* mipwa_last_error(const mipwa_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_knots, const mipwa_resonance* res,
+                 int32_t n_res, int32_t device, mipwa_ctx** out)
+{
+    if (!out) return MIPWA_ERR_ARG;
+    *out = nullptr;
+    if (!kin || !knots || n_knots < 2 || n_knots > MIPWA_MAX_KNOTS || n_res < 0 || n_res > MIPWA_MAX_RESONANCES ||
+        (n_res > 0 && !res))
+        return MIPWA_ERR_ARG;
+    if (!(kin->m1 > 0 && kin->m2 > 0 && kin->m3 > 0) || kin->m2 != kin->m3 || !(kin->m_parent > kin->m1 + kin->m2 + kin->m3))
+        return MIPWA_ERR_ARG;
+    for (int i = 0; i < n_knots; ++i)
+        if (!std::isfinite(knots[i]) || (i > 0 && !(knots[i] > knots[i - 1]))) return MIPWA_ERR_ARG;
+    for (int r = 0; r < n_res; ++r)
+        if (res[r].spin < 0 || res[r].spin > 2 || !(res[r].r_res >= 0) || !(res[r].r_parent >= 0) ||
+            !(res[r].mass > kin->m1 + kin->m2) || !(res[r].mass < kin->m_parent - kin->m3) || !(res[r].width > 0))
+            return MIPWA_ERR_ARG;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return MIPWA_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return MIPWA_ERR_CUDA;
+    if (prop.major != 10) return MIPWA_ERR_CUDA;          // built for sm_100a only
+    if (cudaSetDevice(device) != cudaSuccess) return MIPWA_ERR_CUDA;
+
+    mipwa_ctx* c = new (std::nothrow) mipwa_ctx();
+    if (!c) return MIPWA_ERR_NOMEM;
+    c->kin = *kin;
+    c->N = n_knots; c->R = n_res;
+    c->knots.assign(knots, knots + n_knots);
+    if (n_res) c->res.assign(res, res + n_res);
+    for (int r = 0; r < n_res; ++r) c->F += res[r].shape_floats ? 1 : 0;
+    c->device = device;
+    c->sm_count = prop.multiProcessorCount;
+    c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
+    spline_factor(c);
+    std::memset(&c->model, 0, sizeof(DevModel));
+
+    bool ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute, MIPWA_BLOCK, 0) == cudaSuccess;
+    if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
+    const size_t max_grid = (size_t)c->sm_count * 16;
+    ok = ok && cudaMalloc(&c->d_partials, max_grid * sizeof(double2) * 64) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->d_ticket, 64) == cudaSuccess && cudaMemset(c->d_ticket, 0, 64) == cudaSuccess;
+    ok = ok && cudaHostAlloc(&c->h_result, 4096 * sizeof(double), cudaHostAllocMapped) == cudaSuccess;
+    ok = ok && cudaHostGetDevicePointer(&c->d_result, c->h_result, 0) == cudaSuccess;
+    ok = ok && cudaHostAlloc(&c->h_bad, 64, cudaHostAllocMapped) == cudaSuccess;
+    ok = ok && cudaHostGetDevicePointer(&c->d_bad, c->h_bad, 0) == cudaSuccess;
+    ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+    if (!ok) { mipwa_destroy(c); return MIPWA_ERR_CUDA; }
+    *out = c;
+    return MIPWA_OK;
+}
+
+void mipwa_destroy(mipwa_ctx* c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    free_slot(c->ev); free_slot(c->nm);
+    if (c->d_partials) cudaFree(c->d_partials);
+    if (c->d_ticket) cudaFree(c->d_ticket);
+    if (c->h_result) cudaFreeHost(c->h_result);
+    if (c->h_bad) cudaFreeHost(c->h_bad);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+}
+
+int mipwa_set_stream(mipwa_ctx* c, void* s)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    c->stream = (cudaStream_t)s;
+    return MIPWA_OK;
+}
+
+int mipwa_enable_timing(mipwa_ctx* c, int32_t on)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    c->timing = on != 0;
+    return MIPWA_OK;
+}
+
+static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s13, const double* w, int64_t n,
+                    int32_t mem, bool allow_empty)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    if (n < (allow_empty ? 0 : 1) || (n > 0 && (!s12 || !s13)) || (mem != MIPWA_MEM_HOST && mem != MIPWA_MEM_DEVICE))
+        return fail(c, MIPWA_ERR_ARG, "bad pointer, count or mem flag");
+    int rc = use_device(c);
+    if (rc) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    free_slot(slot);
+    Slot s;
+    if (mem == MIPWA_MEM_HOST && n > 0) {
+        const double* src[3] = { s12, s13, w };
+        for (int q = 0; q < 3; ++q) {
+            if (!src[q]) continue;
+            cudaError_t e = cudaMalloc(&s.owned[q], (size_t)n * sizeof(double));
+            if (e == cudaSuccess) e = cudaMemcpyAsync(s.owned[q], src[q], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+            if (e != cudaSuccess) {
+                free_slot(s);
+                return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, cudaGetErrorString(e));
+            }
+        }
+        s.s12 = (const double*)s.owned[0]; s.s13 = (const double*)s.owned[1]; s.w = (const double*)s.owned[2];
+    } else {
+        s.s12 = s12; s.s13 = s13; s.w = w;
+    }
+    s.n = n;
+    if (n > 0) {                                           // boundary check on the device (north_star invariant)
+        const mipwa_kinematics& k = c->kin;
+        DevKin dk = { k.m_parent * k.m_parent, k.m1 * k.m1, k.m2 * k.m2, k.m3 * k.m3,
+                      (k.m1 + k.m2) * (k.m1 + k.m2), (k.m1 - k.m2) * (k.m1 - k.m2),
+                      (k.m_parent - k.m3) * (k.m_parent - k.m3), (k.m_parent + k.m3) * (k.m_parent + k.m3) };
+        *c->h_bad = 0;
+        k_validate<<<grid_for(c, n, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, s.s12, s.s13, n, c->d_bad);
+        ++c->launches;
+        cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) { free_slot(s); return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e)); }
+        if (*c->h_bad) {
+            const unsigned long long nb = *c->h_bad;
+            free_slot(s);
+            return fail(c, MIPWA_ERR_DOMAIN, std::to_string(nb) + " point(s) outside the Dalitz boundary");
+        }
+    }
+    slot = s;
+    return MIPWA_OK;
+}
+
+int mipwa_set_events(mipwa_ctx* c, const double* s12, const double* s13, int64_t n, int32_t mem)
+{
+    return set_slot(c, c->ev, s12, s13, nullptr, n, mem, true);
+}
+
+int mipwa_set_norm_points(mipwa_ctx* c, const double* s12, const double* s13, const double* w, int64_t n, int32_t mem)
+{
+    return set_slot(c, c->nm, s12, s13, w, n, mem, false);
+}
+
+int mipwa_n_params(const mipwa_ctx* c, int64_t* n)
+{
+    if (!c || !n) return MIPWA_ERR_ARG;
+    *n = 2 * c->N + 2 * c->R + 2 * c->F;
+    return MIPWA_OK;
+}
+
+int mipwa_set_path(mipwa_ctx* c, int32_t path)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    if (path < MIPWA_PATH_AUTO || path > MIPWA_PATH_CACHED_COMPACT) return fail(c, MIPWA_ERR_ARG, "unknown path");
+    if ((path == MIPWA_PATH_CACHED || path == MIPWA_PATH_CACHED_COMPACT) && c->F > 0)
+        return fail(c, MIPWA_ERR_STATE, "cached paths need fixed resonance shapes");
+    c->path = path;
+    return MIPWA_OK;
+}
+
+static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
+{
+    const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->blocks_per_sm);
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    k_nll_recompute<<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, c->ev.s12, c->ev.s13, c->ev.n, c->nm.s12, c->nm.s13,
+                                                       c->nm.w, c->nm.n, c->d_partials, c->d_ticket, c->d_result);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    *sum_log = c->h_result[0];
+    *integral = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
+    return MIPWA_OK;
+}
+
+int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* sum_log, double* integral)
+{
+    if (!c || !params || !nll) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    double S = 0, I = 0;
+    rc = nll_recompute(c, &S, &I);
+    if (rc) return rc;
+    *nll = -S + (double)c->ev.n * std::log(I);             // A7
+    if (sum_log) *sum_log = S;
+    if (integral) *integral = I;
+    return MIPWA_OK;
+}
+
+int mipwa_nll(mipwa_ctx* c, const double* params, int64_t n_params, double* nll)
+{
+    return mipwa_nll_parts(c, params, n_params, nll, nullptr, nullptr);
+}
+
+int mipwa_eval_abs2(mipwa_ctx* c, const double* params, int64_t n_params, int32_t which, double* out, int64_t n)
+{
+    if (!c || !params || (which != 0 && which != 1)) return c ? fail(c, MIPWA_ERR_ARG, "bad argument") : MIPWA_ERR_ARG;
+    const Slot& s = which == 0 ? c->ev : c->nm;
+    if (s.n < 0) return fail(c, MIPWA_ERR_STATE, "slot not set");
+    if (n != s.n || (n > 0 && !out)) return fail(c, MIPWA_ERR_ARG, "n must equal the slot size");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    if (n == 0) return MIPWA_OK;
+    double* d_out = nullptr;
+    CU(c, cudaMalloc(&d_out, (size_t)n * sizeof(double)));
+    k_abs2<<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, n, d_out);
+    ++c->launches;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(d_out);
+    if (e != cudaSuccess) return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e));
+    return MIPWA_OK;
+}
+
+int mipwa_last_kernel_ms(const mipwa_ctx* c, float* ms)
+{
+    if (!c || !ms) return MIPWA_ERR_ARG;
+    *ms = c->last_ms;
+    return MIPWA_OK;
+}
+
+int64_t mipwa_launch_count(const mipwa_ctx* c) { return c ? c->launches : -1; }
+
+int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops)
+{
+    if (!tflops || !(seconds > 0)) return MIPWA_ERR_ARG;
+    cudaDeviceProp prop;
+    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) return MIPWA_ERR_CUDA;
+    double* d = nullptr;
+    cudaEvent_t a, b;
+    if (cudaMalloc(&d, 64) != cudaSuccess || cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return MIPWA_ERR_CUDA;
+    const int grid = prop.multiProcessorCount * 8, block = 256;
+    long long iters = 2000;
+    double best = 0, spent = 0;
+    for (int rep = 0; rep < 64 && spent < seconds; ++rep) {
+        cudaEventRecord(a);
+        k_dfma_peak<<<grid, block>>>(d, iters, 0.999999, 1e-9);
+        cudaEventRecord(b);
+        if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(d); return MIPWA_ERR_CUDA; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, a, b);
+        const double fl = 2.0 * 64.0 * (double)iters * grid * block;
+        if (rep > 0) { best = std::max(best, fl / (ms * 1e-3) * 1e-12); spent += ms * 1e-3; }
+        if (ms < 50.0f) iters *= 2;                        // grow each launch to ~0.1 s
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d);
+    *tflops = best;
+    return MIPWA_OK;
+}
+
+}  // extern "C"
+
+// ---- placeholders until cached.cuh / grad.cuh land ---------------------------------------------------------------
+extern "C" {
+int64_t mipwa_basis_bytes(const mipwa_ctx* c) { return c ? 0 : MIPWA_ERR_ARG; }
+int mipwa_set_basis_buffer(mipwa_ctx* c, void*, int64_t) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
+int mipwa_nll_grad(mipwa_ctx* c, const double*, int64_t, double*, double*) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
+int mipwa_eval_basis(mipwa_ctx* c, const double*, int64_t, int32_t, int64_t, int64_t, double*) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
+}
