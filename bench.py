@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the MIPWA NLL hot path on B200 (contract: task prompt "Measurement").
+
+A "step" is one likelihood evaluation mipwa_nll(params) over the whole sample: every event and every
+normalisation point goes through the fused amplitude + reduction kernel once.
+Workload at N = 1: BASELINE.json configs[3] (the configuration the metric "at 10M events" is quoted on):
+50 knots + rho(770) [mass, width floating] + rho(1450) + f2(1270), 10 M events + 10 M normalisation points, fp64,
+full recompute every call.  N > 1: every rank holds its own 10 M + 10 M shard (weak scaling); the only exchange
+is three doubles per rank per call (paper_1703_03284_b200/sharding.py).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--events E] [--norm-points G]
+
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1703_03284_b200 import inputs as I  # noqa: E402
+
+METRIC = "MIPWA NLL events/s (full recompute, 10M events + 10M normalisation points per GPU, fp64)"
+UNIT = "events/s"
+
+
+# ---- algorithmic work per point: flops of the restated formulas, fma = 2, rcp/rsqrt = 1 + their
+# refinement; nothing padded, the log-product trick and shared sub-expressions already taken out -------------------
+def flops_per_point(resonances):
+    per_channel = 36 + 15                       # kinematics shared by all resonances + spline (index, Horner)
+    per_res_channel = {0: 20, 1: 27, 2: 32}
+    f = 2 * per_channel + 2 + 3 + 1             # two channels, S12+S13, |A|^2, product / weight
+    for r in resonances:
+        f += 2 * per_res_channel[r["spin"]] + 10
+    return f
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+
+    def summary(self, t0, t1):
+        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": float(np.median([float(r[0]) for r in rows])), "sm_max_mhz": float(rows[0][1]),
+                "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows), "reasons": reasons}
+
+
+def oracle_sample(cfg, n_ev, n_norm):
+    """Inputs for the oracle legs: generated with the oracle itself as the accept-reject density (no CUDA)."""
+    from oracle import oracle as orc
+    o = orc.Oracle(cfg.kin, cfg.knots, cfg.resonances)
+    f = lambda a, b: o.abs2(cfg.truth, a, b)
+    e12, e13 = cfg.events(f, I.envelope_of(f, cfg.kin), n=n_ev)
+    g12, g13 = I.phase_space_points(n_norm, cfg.key(I.S_NORM), cfg.kin)
+    w = np.full(n_norm, I.dalitz_area(cfg.kin) / n_norm)
+    return o, (e12, e13, g12, g13, w)
+
+
+def time_oracle(cfg, n_ev, n_norm, steps, warmup):
+    from oracle import oracle as orc
+    o, data = oracle_sample(cfg, n_ev, n_norm)
+    for t in range(warmup):
+        o.nll(cfg.perturbed(t), *data)
+    t0 = time.perf_counter()
+    for t in range(steps):
+        o.nll(cfg.perturbed(warmup + t), *data)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    return {"value": n_ev / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "seconds_per_call": dt,
+            "sample": f"first {n_ev} events + {n_norm} normalisation points of the workload, {steps} NLL call(s), "
+                      f"OpenMP over all host threads"}
+
+
+def run_reference(args, cfg, workload):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_ev = min(cfg.n_ev, 400_000)
+    n_norm = min(cfg.norm_size, 400_000)
+    steps = max(1, min(args.steps, 20))
+    warmup = min(args.warmup, 2)
+    cb = time_oracle(cfg, n_ev, n_norm, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * cb["seconds_per_call"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(workload, sample_events=n_ev, sample_norm_points=n_norm),
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def gpu_inputs(cfg, m, B, torch, rank):
+    """Events by accept-reject with the CUDA library's own per-point hook as the density,
+    normalisation points uniform in phase space; both end up resident in HBM as torch tensors."""
+    def abs2_fn(a, b):
+        m.set_events(np.ascontiguousarray(a), np.ascontiguousarray(b))
+        return m.eval_abs2(cfg.truth, 0)
+    env = I.envelope_of(abs2_fn, cfg.kin)
+    e12, e13 = cfg.events(abs2_fn, env, stream=rank, chunk=1 << 22)
+    g12, g13, w = cfg.norm_points(stream=rank)
+    host = [np.ascontiguousarray(a) for a in (e12, e13, g12, g13, w)]
+    dev = [torch.from_numpy(a).cuda() for a in host]
+    return host, dev
+
+
+def run_ours(args, cfg, workload):
+    import torch
+    import torch.distributed as dist
+    from paper_1703_03284_b200 import binding as B
+    from paper_1703_03284_b200 import sharding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    m = B.Mipwa(cfg.kin, cfg.knots, cfg.resonances, device=local)
+    stream = torch.cuda.Stream(device=dev)
+    m.set_stream(stream)
+    t_gen = time.perf_counter()
+    host, d = gpu_inputs(cfg, m, B, torch, rank)
+    t_gen = time.perf_counter() - t_gen
+    if world > 1:                                    # whole-sample weights so that per-rank integrals add
+        d[4] = d[4] / world
+        host[4] = host[4] / world
+    m.set_events(d[0], d[1])
+    m.set_norm_points(d[2], d[3], d[4])
+    m.set_path(B.PATH_RECOMPUTE)
+    m.enable_timing(True)
+    n_ev, n_norm = d[0].numel(), d[2].numel()
+
+    params = [cfg.perturbed(t) for t in range(args.warmup + args.steps)]
+
+    def step(p):
+        _, S, Iv = m.nll_parts(p)
+        return sharding.combine_parts(S, Iv, n_ev, device=dev)[0]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for t in range(args.warmup):
+        step(params[t])
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    launches0 = m.launch_count()
+    kernel_ms = []
+    w0 = time.perf_counter()
+    ev0.record(stream)
+    for t in range(args.steps):
+        nll = step(params[args.warmup + t])
+        kernel_ms.append(m.last_kernel_ms())
+    ev1.record(stream)
+    barrier()
+    w1 = time.perf_counter()
+    launches = m.launch_count() - launches0
+    ms_total = ev0.elapsed_time(ev1)
+    if world > 1:
+        tt = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+
+    # ---- e2e: the same evaluation through the C ABI from HOST buffers: H2D of the step's inputs (pinned), the
+    # boundary check, the NLL kernel and the D2H of the result are all inside the timed region -----------------------
+    pinned = [torch.from_numpy(a).pin_memory() for a in host]
+    ph = [t.numpy() for t in pinned]
+    e2e_steps = max(3, min(args.steps, 10))
+    def e2e_step(p):
+        m.set_events(ph[0], ph[1])
+        m.set_norm_points(ph[2], ph[3], ph[4])
+        _, S, Iv = m.nll_parts(p)
+        return sharding.combine_parts(S, Iv, n_ev, device=dev)[0]
+    e2e_step(params[0]); e2e_step(params[1])
+    barrier()
+    t0 = time.perf_counter()
+    for t in range(e2e_steps):
+        nll_e2e = e2e_step(params[args.warmup + t % args.steps])
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    h2d = sum(a.nbytes for a in ph) + params[0].nbytes
+    d2h = 16 + 16                                     # two boundary-check counters + (sum ln|A|^2, I)
+    # back to resident device arrays for the fit-step latency number
+    m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4])
+    t0 = time.perf_counter()
+    for t in range(args.steps):
+        step(params[args.warmup + t])
+    fit_step_s = (time.perf_counter() - t0) / args.steps
+
+    if rank == 0:
+        time.sleep(0.2)
+        sampler.stop()
+    clocks = sampler.summary(w0, w1) if rank == 0 else None
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_nll_recompute): plain FP64 ALU work ----------------------------------
+    peak = B.measure_fp64_peak(local, 2.0)
+    fl = flops_per_point(cfg.resonances) * (n_ev + n_norm)
+    k_ms = float(np.mean(kernel_ms))
+    achieved = fl / (k_ms * 1e-3) * 1e-12
+    nominal = None
+    if clocks and clocks.get("sm_max_mhz"):
+        nominal = 148 * 64 * 2 * clocks["sm_max_mhz"] * 1e6 * 1e-12
+    roofline = {"bound": "alu", "kernel": "k_nll_recompute", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": None,
+                "peak_source": "measured on this GPU by mipwa_measure_fp64_peak (register-resident DFMA, 2 s sustained); "
+                               "MEASURED_PEAKS.json has no FP64 entry",
+                "nominal_peak": nominal, "flops_per_point": flops_per_point(cfg.resonances),
+                "points_per_launch": n_ev + n_norm, "kernel_ms": k_ms,
+                "hbm_gbs": 16.0 * (n_ev + n_norm) / (k_ms * 1e-3) * 1e-9}
+
+    cpu = None
+    if world == 1:
+        cpu = time_oracle(cfg, min(n_ev, 2_000_000), min(n_norm, 2_000_000), 2, 1)
+
+    total_events = n_ev * world
+    line = {"metric": METRIC, "value": total_events / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(workload, events_per_gpu=n_ev, norm_points_per_gpu=n_norm,
+                           l2="inputs (16 B x 2 x 10M = 320 MB per step) exceed the 126 MB L2; no flush needed",
+                           parallelism=f"dp{world} (events and normalisation points sharded; 3 doubles all-gathered per call)"),
+            "nll_evals_per_s": 1e3 / ms_step, "points_per_s": (n_ev + n_norm) * world / (ms_step * 1e-3),
+            "nll": nll, "clocks": clocks, "gpu_launches": int(launches) * world,
+            "e2e": {"value": total_events / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                    "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_s, "nll": nll_e2e,
+                    "what": "mipwa_set_events + mipwa_set_norm_points from pinned HOST arrays + mipwa_nll, every step"},
+            "fit_step": {"ms_per_call": 1e3 * fit_step_s, "nll_evals_per_s": 1.0 / fit_step_s,
+                         "what": "wall clock of mipwa_nll(host params) -> host fp64 with events resident (what a minimiser sees)"},
+            "roofline": roofline, "cpu_baseline": cpu, "input_generation_s": t_gen, "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--events", type=int, default=None)
+    ap.add_argument("--norm-points", type=int, default=None)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    cfg = I.Config(args.config, n_ev=args.events, n_norm=args.norm_points)
+    workload = {"workload": f"BASELINE.json configs[{args.config}]: {cfg.N} knots + "
+                            + " + ".join(f"BW(m={r['mass']},G={r['width']},L={r['spin']}{',floating' if r['shape_floats'] else ''})"
+                                         for r in cfg.resonances)
+                            + f"; {cfg.n_ev} events + {cfg.norm_size} normalisation points per GPU; NLL value, full recompute",
+                "n_knots": cfg.N, "n_resonances": cfg.R, "n_params": int(cfg.n_params)}
+    if args.impl == "reference":
+        run_reference(args, cfg, workload)
+    else:
+        run_ours(args, cfg, workload)
+
+
+if __name__ == "__main__":
+    main()

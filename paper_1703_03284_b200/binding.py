@@ -120,7 +120,7 @@ class Mipwa:
         rc = self.L.mipwa_create(C.byref(self._kin), knots.ctypes.data_as(_dp), self.N, res, self.R, int(device),
                                  C.byref(self._h))
         if rc != OK:
-            self._h = C.c_void_p()
+            self._h = None
             raise MipwaError(rc, "mipwa_create failed (bad model, or no sm_100 CUDA device: there is no CPU path)")
         self.device = int(device)
         self._keep = {}                     # borrowed tensors kept alive
@@ -134,12 +134,17 @@ class Mipwa:
             raise MipwaError(rc, self.L.mipwa_last_error(self._h).decode())
 
     def close(self):
-        if getattr(self, "_h", None) and self._h.value:
-            self.L.mipwa_destroy(self._h)
-            self._h = C.c_void_p()
+        h = getattr(self, "_h", None)
+        if h is not None and h.value:
+            self._h = None
+            self.L.mipwa_destroy(h)
             self._keep = {}
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:           # interpreter shutdown: module globals may be gone
+            pass
 
     def set_stream(self, stream):
         """stream: a torch.cuda.Stream, a raw cudaStream_t integer, or None (default stream)."""

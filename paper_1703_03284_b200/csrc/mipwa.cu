@@ -320,13 +320,17 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
     int rc = use_device(c);
     if (rc) return rc;
     CU(c, cudaStreamSynchronize(c->stream));
-    free_slot(slot);
     Slot s;
+    if (mem == MIPWA_MEM_HOST && n > 0 && slot.n == n && slot.owned[0] && slot.owned[1]) {
+        for (int q = 0; q < 3; ++q) { s.owned[q] = slot.owned[q]; slot.owned[q] = nullptr; }   // same size: reuse
+        if (!w && s.owned[2]) { cudaFree(s.owned[2]); s.owned[2] = nullptr; }
+    }
+    free_slot(slot);
     if (mem == MIPWA_MEM_HOST && n > 0) {
         const double* src[3] = { s12, s13, w };
         for (int q = 0; q < 3; ++q) {
             if (!src[q]) continue;
-            cudaError_t e = cudaMalloc(&s.owned[q], (size_t)n * sizeof(double));
+            cudaError_t e = s.owned[q] ? cudaSuccess : cudaMalloc(&s.owned[q], (size_t)n * sizeof(double));
             if (e == cudaSuccess) e = cudaMemcpyAsync(s.owned[q], src[q], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
             if (e != cudaSuccess) {
                 free_slot(s);

@@ -142,18 +142,49 @@ def phase_space_points(n, key, kin=KIN, chunk=1 << 21):
     return np.concatenate(out12)[:n].copy(), np.concatenate(out13)[:n].copy()
 
 
+class Envelope:
+    """Piecewise-constant envelope of |A|^2 over an n_coarse x n_coarse partition of the bounding square.
+
+    env[cx, cy] = 1.2 x max |A|^2 over the cell centres of the n_side^2 fine grid that fall inside the Dalitz
+    boundary and inside coarse cell (cx, cy) (reading P22 applied per coarse cell; n_coarse = 1 is the single
+    global envelope).  A coarse cell without any fine point but next to one that has some takes the largest
+    neighbouring value, so thin slivers along the boundary stay covered.  Accept-reject against it samples
+    exactly the density |A|^2 / integral wherever the envelope bounds |A|^2; larger values clamp."""
+
+    def __init__(self, abs2_fn, kin=KIN, n_side=1024, n_coarse=64):
+        lo, hi = s_limits(kin)
+        self.lo, self.hi, self.nc = lo, hi, int(n_coarse)
+        self.H = (hi - lo) / self.nc
+        g12, g13, _ = grid_points(n_side, kin)
+        a2 = np.asarray(abs2_fn(g12, g13), dtype=np.float64)
+        cx = np.minimum(((g12 - lo) / self.H).astype(np.int64), self.nc - 1)
+        cy = np.minimum(((g13 - lo) / self.H).astype(np.int64), self.nc - 1)
+        own = np.zeros((self.nc, self.nc))
+        np.maximum.at(own, (cx, cy), a2)
+        pad = np.pad(own, 1)
+        neigh = np.max([pad[1 + dx:1 + dx + self.nc, 1 + dy:1 + dy + self.nc]
+                        for dx in (-1, 0, 1) for dy in (-1, 0, 1)], axis=0)
+        self.env = 1.2 * np.where(own > 0, own, neigh)
+        self.global_max = float(a2.max())
+        cum = np.cumsum(self.env.ravel())
+        self.cum = cum / cum[-1]
+
+    def draw(self, u_cell, u_x, u_y):
+        """coarse cell from u_cell (inverse CDF over cells weighted by env), then a uniform point in it."""
+        cell = np.minimum(np.searchsorted(self.cum, u_cell, side="right"), self.nc * self.nc - 1)
+        cx, cy = cell // self.nc, cell % self.nc
+        return self.lo + (cx + u_x) * self.H, self.lo + (cy + u_y) * self.H, self.env.ravel()[cell]
+
+
 def accept_reject(n, key, abs2_fn, envelope, kin=KIN, chunk=1 << 21):
-    """n events with density proportional to abs2_fn inside the boundary.  Candidate i uses uniforms 3i, 3i+1,
-    3i+2 of the stream: position in the bounding square and the accept threshold u*envelope < |A|^2 (values
-    above the envelope clamp, reading P22).  Events are the first n accepted candidates in counter order, so
-    the result does not depend on `chunk`."""
-    lo, hi = s_limits(kin)
+    """n events with density proportional to abs2_fn inside the boundary.  Candidate i uses uniforms 4i .. 4i+3 of
+    the stream: coarse cell, position in the cell, and the accept threshold u * env(cell) < |A|^2.  Events are the
+    first n accepted candidates in counter order, so the result does not depend on `chunk`."""
     out12, out13, have, ctr = [], [], 0, 0
     while have < n:
-        u = uniforms(key, 3 * ctr, 3 * chunk)
-        a = lo + (hi - lo) * u[0::3]
-        b = lo + (hi - lo) * u[1::3]
-        thr = u[2::3] * envelope
+        u = uniforms(key, 4 * ctr, 4 * chunk)
+        a, b, env = envelope.draw(u[0::4], u[1::4], u[2::4])
+        thr = u[3::4] * env
         keep = inside(a, b, kin)
         a, b, thr = a[keep], b[keep], thr[keep]
         acc = thr < np.asarray(abs2_fn(a, b))
@@ -162,10 +193,8 @@ def accept_reject(n, key, abs2_fn, envelope, kin=KIN, chunk=1 << 21):
     return np.concatenate(out12)[:n].copy(), np.concatenate(out13)[:n].copy()
 
 
-def envelope_of(abs2_fn, kin=KIN, n_side=1024):
-    """1.2 x max |A|^2 over the cell centres of an n_side^2 grid inside the boundary (reading P22)."""
-    g12, g13, _ = grid_points(n_side, kin)
-    return 1.2 * float(np.max(abs2_fn(g12, g13)))
+def envelope_of(abs2_fn, kin=KIN, n_side=1024, n_coarse=64):
+    return Envelope(abs2_fn, kin, n_side, n_coarse)
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -259,16 +288,17 @@ class Config:
         z = normals(self.key(S_PERTURB), t * self.n_params, self.n_params)
         return self.truth + 1e-3 * z
 
-    def norm_points(self):
+    def norm_points(self, stream=0):
         """(s12, s13, w): config 0 = cell-centre grid with w = cell area; others = uniform phase-space sample with
         w = Area / n (reading P12)."""
         if self.norm_kind == "grid":
             return grid_points(self.norm_size, self.kin)
-        g12, g13 = phase_space_points(self.norm_size, self.key(S_NORM), self.kin)
+        g12, g13 = phase_space_points(self.norm_size, self.key(S_NORM + 16 * stream), self.kin)
         return g12, g13, np.full(g12.size, dalitz_area(self.kin) / g12.size)
 
-    def events(self, abs2_fn, envelope=None, n=None):
+    def events(self, abs2_fn, envelope=None, n=None, stream=0, chunk=1 << 21):
         """accept-reject events from the truth model; abs2_fn(s12, s13) must evaluate |A|^2 at self.truth."""
         if envelope is None:
             envelope = envelope_of(abs2_fn, self.kin)
-        return accept_reject(self.n_ev if n is None else n, self.key(S_EVENTS), abs2_fn, envelope, self.kin)
+        return accept_reject(self.n_ev if n is None else n, self.key(S_EVENTS + 16 * stream), abs2_fn, envelope,
+                             self.kin, chunk=chunk)
