@@ -29,6 +29,7 @@ struct ResDev {
     double cD;        // r_parent^2 / (4 M^2)   (z_D = cD * lam2); 0 for L = 0
     double Kw;        // m0^2 Gamma0 n_R / ((4 q0^2)^L sqrt(q0^2))
     double cre, cim;  // c_r * sqrt(n_R n_D)
+    double pa, pb, pc;// barrier denominator den_L(z) = pc + z (pb + pa z)
     int32_t L;
     int32_t pad;
 };
@@ -114,7 +115,9 @@ __device__ __forceinline__ void spline_eval(const SplineSmem& sm, const DevModel
 
 // per-channel kinematic quantities shared by all resonances
 struct Channel {
-    double x, lam2, ql, w0, Z1, Z2;      // w0 = g (L = 0 width factor); w1 = g ql; w2 = g ql^2 derived on the fly
+    double x, lam2, ql;
+    double w[3];      // w[L] = g ql^L: the running-width factor of a spin-L resonance
+    double Z[3];      // Zemach factors Z_0 = 1, Z_1, Z_2
 };
 
 __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, double y)
@@ -126,43 +129,73 @@ __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, dou
     const double ix = fast_rcp(x);
     c.ql = lam1 * ix;
     const double pl = c.lam2 * ix;
-    // sqrt(lam1) = lam1 * rsqrt(lam1); lam1 -> 0 at threshold, where the width vanishes
-    const double sq = lam1 > 1e-300 ? lam1 * fast_rsqrt(lam1) : 0.0;
-    c.w0 = 0.5 * sq * ix;
-    c.Z1 = fma(m.kappa, ix, fma(2.0, y, x) - m.sigma);
-    c.Z2 = fma(c.Z1, c.Z1, (-1.0 / 3.0) * (c.ql * pl));
+    // sqrt(lam1) = l rsqrt(l) with l = max(lam1, tiny): no branch, ~1e-150 instead of 0 at threshold where the
+    // width vanishes anyway
+    const double lc = fmax(lam1, 1e-300);
+    const double sq = lc * fast_rsqrt(lc);
+    c.w[0] = 0.5 * sq * ix;
+    c.w[1] = c.w[0] * c.ql;
+    c.w[2] = c.w[1] * c.ql;
+    c.Z[0] = 1.0;
+    c.Z[1] = fma(m.kappa, ix, fma(2.0, y, x) - m.sigma);
+    c.Z[2] = fma(c.Z[1], c.Z[1], (-1.0 / 3.0) * (c.ql * pl));
     return c;
 }
 
-// c_r sqrt(n_R n_D) is applied by the caller: returns F_D F_R Z_L BW / sqrt(n_R n_D) for one channel
+__device__ __forceinline__ double pick(int L, const double (&v)[3]) { return L == 0 ? v[0] : (L == 1 ? v[1] : v[2]); }
+
+// One resonance in one channel.  Returns F_D F_R Z_L BW / sqrt(n_R n_D); c_r sqrt(n_R n_D) is applied by the caller.
+// LT = 0, 1, 2: spin known at compile time (no selects, unused factors vanish).  LT < 0: spin read from the model,
+// branch-free: den_L(z) = pc + z (pb + pa z) with (pa, pb, pc) = (0,0,1), (0,1,1), (1,3,9), factors selected.
+template <int LT>
 __device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel& c, double& tre, double& tim)
 {
     double DR, DD, W, Z;
-    if (r.L == 1) {
+    if (LT == 0) {
+        DR = 1.0; DD = 1.0; W = r.Kw * c.w[0]; Z = 1.0;
+    } else if (LT == 1) {
         DR = fma(r.cR, c.ql, 1.0);
         DD = fma(r.cD, c.lam2, 1.0);
-        W = r.Kw * (c.w0 * c.ql);
-        Z = c.Z1;
-    } else if (r.L == 2) {
+        W = r.Kw * c.w[1];
+        Z = c.Z[1];
+    } else if (LT == 2) {
         const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
         DR = fma(zR, zR + 3.0, 9.0);
         DD = fma(zD, zD + 3.0, 9.0);
-        W = r.Kw * (c.w0 * c.ql * c.ql);
-        Z = c.Z2;
+        W = r.Kw * c.w[2];
+        Z = c.Z[2];
     } else {
-        DR = 1.0; DD = 1.0;
-        W = r.Kw * c.w0;
-        Z = 1.0;
+        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
+        DR = fma(zR, fma(zR, r.pa, r.pb), r.pc);
+        DD = fma(zD, fma(zD, r.pa, r.pb), r.pc);
+        W = r.Kw * pick(r.L, c.w);
+        Z = pick(r.L, c.Z);
     }
     const double dD = (r.m0sq - c.x) * DR;
     const double E = fma(dD, dD, W * W);
     const double rs = fast_rsqrt((DR * DD) * (E * E));
-    const double t = Z * DR * rs;
+    const double t = (LT == 0 ? rs : Z * DR * rs);
     tre = t * dD;
     tim = t * W;
 }
 
+template <int LT>
+__device__ __forceinline__ void add_resonance(const ResDev& rd, const Channel& ca, const Channel& cb, double& are,
+                                              double& aim)
+{
+    double ar, ai, br, bi;
+    resonance_channel<LT>(rd, ca, ar, ai);
+    resonance_channel<LT>(rd, cb, br, bi);
+    const double tr = ar + br, ti = ai + bi;
+    are = fma(rd.cre, tr, fma(-rd.cim, ti, are));
+    aim = fma(rd.cre, ti, fma(rd.cim, tr, aim));
+}
+
 // A(s12,s13) = S(s12) + S(s13) + sum_r c_r [T_r(s12,s13) + T_r(s13,s12)]
+// Model signature <R1, R2>: the host orders the resonances spin 1 first (R1 of them), then spin 2 (R2), so that
+// the whole sum unrolls with compile-time spins and constants straight from the parameter bank (2 (R1 + R2)
+// independent chains).  <-1, -1>: any list (incl. spin 0), run-time loop over m.R.
+template <int R1, int R2>
 __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& m, double s12, double s13,
                                           double& are, double& aim)
 {
@@ -171,16 +204,37 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
     spline_eval(sm, m, s13, r2, i2);
     are = r1 + r2;
     aim = i1 + i2;
-    if (m.R > 0) {
-        const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
-        for (int r = 0; r < m.R; ++r) {
-            const ResDev& rd = m.res[r];
-            double ar, ai, br, bi;
-            resonance_channel(rd, ca, ar, ai);
-            resonance_channel(rd, cb, br, bi);
-            const double tr = ar + br, ti = ai + bi;
-            are = fma(rd.cre, tr, fma(-rd.cim, ti, are));
-            aim = fma(rd.cre, ti, fma(rd.cim, tr, aim));
-        }
+    if (R1 == 0 && R2 == 0) return;
+    const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
+    if (R1 >= 0) {
+#pragma unroll
+        for (int r = 0; r < R1; ++r) add_resonance<1>(m.res[r], ca, cb, are, aim);
+#pragma unroll
+        for (int r = 0; r < R2; ++r) add_resonance<2>(m.res[R1 + r], ca, cb, are, aim);
+    } else {
+        for (int r = 0; r < m.R; ++r) add_resonance<-1>(m.res[r], ca, cb, are, aim);
     }
 }
+
+#define MIPWA_SIG_MAX1 4
+#define MIPWA_SIG_MAX2 2
+// run CALL with constexpr R1, R2 matching the model signature (n0, n1, n2 = resonances of spin 0, 1, 2)
+#define MIPWA_DISPATCH_SIG(n0, n1, n2, CALL)                                                      \
+    switch (((n0) == 0 && (n1) <= MIPWA_SIG_MAX1 && (n2) <= MIPWA_SIG_MAX2) ? (n1) * 8 + (n2) : -1) { \
+        case 0: { constexpr int R1 = 0, R2 = 0; CALL; } break;                                    \
+        case 1: { constexpr int R1 = 0, R2 = 1; CALL; } break;                                    \
+        case 2: { constexpr int R1 = 0, R2 = 2; CALL; } break;                                    \
+        case 8: { constexpr int R1 = 1, R2 = 0; CALL; } break;                                    \
+        case 9: { constexpr int R1 = 1, R2 = 1; CALL; } break;                                    \
+        case 10: { constexpr int R1 = 1, R2 = 2; CALL; } break;                                   \
+        case 16: { constexpr int R1 = 2, R2 = 0; CALL; } break;                                   \
+        case 17: { constexpr int R1 = 2, R2 = 1; CALL; } break;                                   \
+        case 18: { constexpr int R1 = 2, R2 = 2; CALL; } break;                                   \
+        case 24: { constexpr int R1 = 3, R2 = 0; CALL; } break;                                   \
+        case 25: { constexpr int R1 = 3, R2 = 1; CALL; } break;                                   \
+        case 26: { constexpr int R1 = 3, R2 = 2; CALL; } break;                                   \
+        case 32: { constexpr int R1 = 4, R2 = 0; CALL; } break;                                   \
+        case 33: { constexpr int R1 = 4, R2 = 1; CALL; } break;                                   \
+        case 34: { constexpr int R1 = 4, R2 = 2; CALL; } break;                                   \
+        default: { constexpr int R1 = -1, R2 = -1; CALL; } break;                                 \
+    }

@@ -3,7 +3,15 @@
 #pragma once
 #include "dev_model.cuh"
 
+#ifndef MIPWA_BLOCK
 #define MIPWA_BLOCK 256
+#endif
+#ifndef MIPWA_MINBLOCKS
+#define MIPWA_MINBLOCKS 2
+#endif
+#ifndef MIPWA_PTS
+#define MIPWA_PTS 1
+#endif
 
 // ---- deterministic block reduction of NV doubles per thread: warp shuffles, then shared memory -------------------
 template <int NV>
@@ -60,10 +68,12 @@ struct LogProd {
 
 // ---- A4-A6: one launch over [events | normalisation points] ------------------------------------------------------
 // Persistent grid (a multiple of the SM count).  Per thread: grid-stride over events (coalesced 8-byte loads of
-// s12[i], s13[i]; nothing is written per event), then over normalisation points.  Block partials go to
-// partials[block] = (sum ln|A|^2, sum w|A|^2); the last block to finish adds them in block order (fixed order:
-// bit-reproducible for a given grid) and writes the two totals to `result` (mapped pinned host memory).
-__global__ void __launch_bounds__(MIPWA_BLOCK, 2)
+// s12[i], s13[i], the next point's pair prefetched before the current one is evaluated; nothing is written per
+// event), then over normalisation points.  Block partials go to partials[block] = (sum ln|A|^2, sum w|A|^2); the
+// last block to finish adds them in block order (fixed order: bit-reproducible for a given grid) and writes the
+// two totals to `result` (mapped pinned host memory).
+template <int R1, int R2>
+__global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_MINBLOCKS)
 k_nll_recompute(const __grid_constant__ DevModel m,
                 const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
                 const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
@@ -78,24 +88,65 @@ k_nll_recompute(const __grid_constant__ DevModel m,
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
 
+    // PTS points per thread and iteration: independent dependency chains for the FP64 pipe.  Out-of-range slots
+    // evaluate a harmless in-range point and contribute ln 1 = 0 (events) or weight 0 (normalisation).
+    constexpr int PTS = MIPWA_PTS;
     LogProd lp;
-    for (long long i = t0; i < n_ev; i += stride) {
-        double re, im;
-        amplitude(sm, m, e12[i], e13[i], re, im);
-        lp.add(fma(re, re, im * im));
+    {
+        double a[PTS], b[PTS];
+#pragma unroll
+        for (int q = 0; q < PTS; ++q) {
+            const long long i = t0 + q * stride;
+            a[q] = 1.0; b[q] = 1.0;
+            if (i < n_ev) { a[q] = e12[i]; b[q] = e13[i]; }
+        }
+        for (long long i = t0; i < n_ev; i += PTS * stride) {
+            double na[PTS], nb[PTS];
+#pragma unroll
+            for (int q = 0; q < PTS; ++q) {
+                const long long nx = i + (PTS + q) * stride;
+                na[q] = 1.0; nb[q] = 1.0;
+                if (nx < n_ev) { na[q] = e12[nx]; nb[q] = e13[nx]; }
+            }
+            double v[PTS];
+#pragma unroll
+            for (int q = 0; q < PTS; ++q) {
+                double re, im;
+                amplitude<R1, R2>(sm, m, a[q], b[q], re, im);
+                v[q] = fma(re, re, im * im);
+            }
+#pragma unroll
+            for (int q = 0; q < PTS; ++q) {
+                lp.add(i + q * stride < n_ev ? v[q] : 1.0);
+                a[q] = na[q]; b[q] = nb[q];
+            }
+        }
     }
     double integ = 0.0;
-    if (gw) {
-        for (long long j = t0; j < n_norm; j += stride) {
-            double re, im;
-            amplitude(sm, m, g12[j], g13[j], re, im);
-            integ = fma(gw[j], fma(re, re, im * im), integ);
+    {
+        double a[PTS], b[PTS], w[PTS];
+#pragma unroll
+        for (int q = 0; q < PTS; ++q) {
+            const long long j = t0 + q * stride;
+            a[q] = 1.0; b[q] = 1.0; w[q] = 0.0;
+            if (j < n_norm) { a[q] = g12[j]; b[q] = g13[j]; w[q] = gw ? gw[j] : 1.0; }
         }
-    } else {
-        for (long long j = t0; j < n_norm; j += stride) {
-            double re, im;
-            amplitude(sm, m, g12[j], g13[j], re, im);
-            integ += fma(re, re, im * im);
+        for (long long j = t0; j < n_norm; j += PTS * stride) {
+            double na[PTS], nb[PTS], nw[PTS];
+#pragma unroll
+            for (int q = 0; q < PTS; ++q) {
+                const long long nx = j + (PTS + q) * stride;
+                na[q] = 1.0; nb[q] = 1.0; nw[q] = 0.0;
+                if (nx < n_norm) { na[q] = g12[nx]; nb[q] = g13[nx]; nw[q] = gw ? gw[nx] : 1.0; }
+            }
+#pragma unroll
+            for (int q = 0; q < PTS; ++q) {
+                double re, im;
+                amplitude<R1, R2>(sm, m, a[q], b[q], re, im);
+                integ = fma(w[q], fma(re, re, im * im), integ);
+            }
+#pragma unroll
+            for (int q = 0; q < PTS; ++q) { a[q] = na[q]; b[q] = nb[q]; w[q] = nw[q]; }
         }
     }
 
@@ -125,6 +176,7 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 }
 
 // ---- test hook: |A|^2 per point from the same device function ---------------------------------------------------
+template <int R1, int R2>
 __global__ void __launch_bounds__(MIPWA_BLOCK)
 k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
        long long n, double* __restrict__ out)
@@ -134,7 +186,7 @@ k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         double re, im;
-        amplitude(sm, m, s12[i], s13[i], re, im);
+        amplitude<R1, R2>(sm, m, s12[i], s13[i], re, im);
         out[i] = fma(re, re, im * im);
     }
 }

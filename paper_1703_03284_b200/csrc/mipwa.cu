@@ -32,6 +32,8 @@ struct mipwa_ctx {
     int N = 0, R = 0, F = 0;
     std::vector<double> knots;
     std::vector<mipwa_resonance> res;
+    int n_spin[3] = { 0, 0, 0 };   // resonances of spin 0, 1, 2 (the kernel signature)
+    std::vector<int> perm;          // device slot d holds resonance perm[d]: spin 1 first, then spin 2, then spin 0
     int device = 0;
     int sm_count = 0;
     cudaStream_t stream = nullptr;
@@ -103,6 +105,9 @@ int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, 
     const double f = cmag * std::sqrt(nR * nD);
     out->cre = f * std::cos(carg);
     out->cim = f * std::sin(carg);
+    out->pa = L == 2 ? 1.0 : 0.0;
+    out->pb = L == 2 ? 3.0 : (L == 1 ? 1.0 : 0.0);
+    out->pc = L == 2 ? 9.0 : 1.0;
     out->L = L;
     out->pad = 0;
     return MIPWA_OK;
@@ -190,11 +195,13 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
         for (int q = 0; q < 4; ++q) m.sc[q][j] = make_double2(co[q][0], co[q][1]);
     }
     for (int q = 0; q < 4; ++q) m.sc[q][N - 1] = make_double2(0.0, 0.0);
-    int f = 0;
-    for (int r = 0; r < R; ++r) {
+    std::vector<int> fidx(R, -1);
+    for (int r = 0, f = 0; r < R; ++r) if (c->res[r].shape_floats) fidx[r] = f++;
+    for (int d = 0; d < R; ++d) {
+        const int r = c->perm[d];
         double m0 = c->res[r].mass, g0 = c->res[r].width;
-        if (c->res[r].shape_floats) { m0 = p[2 * N + 2 * R + 2 * f]; g0 = p[2 * N + 2 * R + 2 * f + 1]; ++f; }
-        const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[r]);
+        if (fidx[r] >= 0) { m0 = p[2 * N + 2 * R + 2 * fidx[r]]; g0 = p[2 * N + 2 * R + 2 * fidx[r] + 1]; }
+        const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[d]);
         if (rc) return rc;
     }
     return MIPWA_OK;
@@ -261,13 +268,19 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     c->knots.assign(knots, knots + n_knots);
     if (n_res) c->res.assign(res, res + n_res);
     for (int r = 0; r < n_res; ++r) c->F += res[r].shape_floats ? 1 : 0;
+    for (int L : { 1, 2, 0 })
+        for (int r = 0; r < n_res; ++r)
+            if (res[r].spin == L) { c->perm.push_back(r); ++c->n_spin[L]; }
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
     c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
     spline_factor(c);
     std::memset(&c->model, 0, sizeof(DevModel));
 
-    bool ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute, MIPWA_BLOCK, 0) == cudaSuccess;
+    bool ok = true;
+    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
+                       ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute<R1, R2>,
+                                                                          MIPWA_BLOCK, 0) == cudaSuccess);
     if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
     const size_t max_grid = (size_t)c->sm_count * 16;
     ok = ok && cudaMalloc(&c->d_partials, max_grid * sizeof(double2) * 64) == cudaSuccess;
@@ -394,8 +407,9 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
 {
     const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->blocks_per_sm);
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    k_nll_recompute<<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, c->ev.s12, c->ev.s13, c->ev.n, c->nm.s12, c->nm.s13,
-                                                       c->nm.w, c->nm.n, c->d_partials, c->d_ticket, c->d_result);
+    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2], (k_nll_recompute<R1, R2><<<grid, MIPWA_BLOCK, 0, c->stream>>>(
+                               c->model, c->ev.s12, c->ev.s13, c->ev.n, c->nm.s12, c->nm.s13, c->nm.w, c->nm.n,
+                               c->d_partials, c->d_ticket, c->d_result)));
     ++c->launches;
     CU(c, cudaGetLastError());
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
@@ -441,7 +455,8 @@ int mipwa_eval_abs2(mipwa_ctx* c, const double* params, int64_t n_params, int32_
     if (n == 0) return MIPWA_OK;
     double* d_out = nullptr;
     CU(c, cudaMalloc(&d_out, (size_t)n * sizeof(double)));
-    k_abs2<<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, n, d_out);
+    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
+                       (k_abs2<R1, R2><<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, n, d_out)));
     ++c->launches;
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
