@@ -57,7 +57,7 @@ typedef struct {
 enum { MIPWA_OK = 0, MIPWA_ERR_ARG = -1, MIPWA_ERR_DOMAIN = -2, MIPWA_ERR_STATE = -3, MIPWA_ERR_CUDA = -4,
        MIPWA_ERR_NOMEM = -5 };
 enum { MIPWA_MEM_HOST = 0, MIPWA_MEM_DEVICE = 1 };
-enum { MIPWA_PATH_AUTO = 0,            /* cached-dense if no shape floats and the basis fits, else recompute */
+enum { MIPWA_PATH_AUTO = 0,            /* cached-compact if no shape floats (fewest bytes), else recompute */
        MIPWA_PATH_RECOMPUTE = 1,       /* every call re-evaluates every amplitude term (FP64-ALU bound) */
        MIPWA_PATH_CACHED = 2,          /* fixed shapes: dense n_ev x K complex basis + K x K Gram (HBM bound) */
        MIPWA_PATH_CACHED_COMPACT = 3 };/* fixed shapes: R complex resonance values per event; spline re-evaluated */
@@ -93,8 +93,9 @@ int mipwa_n_params(const mipwa_ctx* ctx, int64_t* n);
 /* Select the evaluation path.  CACHED / CACHED_COMPACT with F > 0 -> MIPWA_ERR_STATE. */
 int mipwa_set_path(mipwa_ctx* ctx, int32_t path);
 
-/* Bytes of device memory the current path needs for its per-event cache with the current events
- * (dense: n_ev * K * 16; compact: n_ev * (R * 16 + 16); recompute: 0), or a negative error code. */
+/* Bytes of device memory the current path needs for its per-event cache with the current events, n_ev rounded up
+ * to a multiple of 256 (dense: n_ev * K * 16; compact: n_ev * (R * 16 + 16); recompute: 0), or a negative error
+ * code (MIPWA_ERR_STATE before mipwa_set_events). */
 int64_t mipwa_basis_bytes(const mipwa_ctx* ctx);
 
 /* Optional caller-provided DEVICE storage for that cache (borrowed; >= mipwa_basis_bytes(), 256-byte aligned).

@@ -179,14 +179,24 @@ __device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel
     tim = t * W;
 }
 
+// Bose-symmetrised term T_r(s12,s13) + T_r(s13,s12) without its coefficient (and without sqrt(n_R n_D))
 template <int LT>
-__device__ __forceinline__ void add_resonance(const ResDev& rd, const Channel& ca, const Channel& cb, double& are,
-                                              double& aim)
+__device__ __forceinline__ void resonance_sym(const ResDev& rd, const Channel& ca, const Channel& cb, double& tr,
+                                              double& ti)
 {
     double ar, ai, br, bi;
     resonance_channel<LT>(rd, ca, ar, ai);
     resonance_channel<LT>(rd, cb, br, bi);
-    const double tr = ar + br, ti = ai + bi;
+    tr = ar + br;
+    ti = ai + bi;
+}
+
+template <int LT>
+__device__ __forceinline__ void add_resonance(const ResDev& rd, const Channel& ca, const Channel& cb, double& are,
+                                              double& aim)
+{
+    double tr, ti;
+    resonance_sym<LT>(rd, ca, cb, tr, ti);
     are = fma(rd.cre, tr, fma(-rd.cim, ti, are));
     aim = fma(rd.cre, ti, fma(rd.cim, tr, aim));
 }

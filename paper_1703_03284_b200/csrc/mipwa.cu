@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "cached.cuh"
 
 static_assert(MIPWA_DEV_MAX_KNOTS == MIPWA_MAX_KNOTS, "capacity mismatch");
 static_assert(MIPWA_DEV_MAX_RES == MIPWA_MAX_RESONANCES, "capacity mismatch");
@@ -58,6 +59,20 @@ struct mipwa_ctx {
 
     DevModel model;                 // staging for the current call
     std::vector<double> y_re, y_im, ypp_re, ypp_im;
+
+    // fixed-shape path (A9, A10)
+    std::vector<double> Mx;         // N x N: y'' = Mx y (knots only)
+    double* d_Mx = nullptr;
+    void* d_cache = nullptr;        // per-event cache in use (owned or the caller's buffer)
+    void* owned_cache = nullptr;
+    int64_t owned_cache_bytes = 0;
+    void* user_cache = nullptr;
+    int64_t user_cache_bytes = 0;
+    int cache_kind = 0;             // MIPWA_PATH_CACHED / MIPWA_PATH_CACHED_COMPACT, valid iff cache_valid
+    bool cache_valid = false;
+    double2* d_gram = nullptr;
+    bool gram_valid = false;
+    int dense_blocks_per_sm = 0, compact_blocks_per_sm = 0;
 
     bool timing = false;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -276,6 +291,15 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
     spline_factor(c);
     std::memset(&c->model, 0, sizeof(DevModel));
+    c->Mx.assign((size_t)n_knots * n_knots, 0.0);          // column k = second derivatives of the cardinal spline k
+    {
+        std::vector<double> e(n_knots), pp(n_knots);
+        for (int k = 0; k < n_knots; ++k) {
+            for (int j = 0; j < n_knots; ++j) e[j] = j == k ? 1.0 : 0.0;
+            spline_solve(c, e.data(), pp.data());
+            for (int j = 0; j < n_knots; ++j) c->Mx[(size_t)j * n_knots + k] = pp[j];
+        }
+    }
 
     bool ok = true;
     MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
@@ -290,6 +314,9 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     ok = ok && cudaHostAlloc(&c->h_bad, 64, cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer(&c->d_bad, c->h_bad, 0) == cudaSuccess;
     ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->d_Mx, c->Mx.size() * sizeof(double)) == cudaSuccess &&
+         cudaMemcpy(c->d_Mx, c->Mx.data(), c->Mx.size() * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->d_gram, (size_t)(n_knots + n_res) * (n_knots + n_res) * sizeof(double2)) == cudaSuccess;
     if (!ok) { mipwa_destroy(c); return MIPWA_ERR_CUDA; }
     *out = c;
     return MIPWA_OK;
@@ -303,6 +330,9 @@ void mipwa_destroy(mipwa_ctx* c)
     free_slot(c->ev); free_slot(c->nm);
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_ticket) cudaFree(c->d_ticket);
+    if (c->d_Mx) cudaFree(c->d_Mx);
+    if (c->owned_cache) cudaFree(c->owned_cache);
+    if (c->d_gram) cudaFree(c->d_gram);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_bad) cudaFreeHost(c->h_bad);
     if (c->ev0) cudaEventDestroy(c->ev0);
@@ -378,11 +408,13 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
 
 int mipwa_set_events(mipwa_ctx* c, const double* s12, const double* s13, int64_t n, int32_t mem)
 {
+    if (c) c->cache_valid = false;
     return set_slot(c, c->ev, s12, s13, nullptr, n, mem, true);
 }
 
 int mipwa_set_norm_points(mipwa_ctx* c, const double* s12, const double* s13, const double* w, int64_t n, int32_t mem)
 {
+    if (c) c->gram_valid = false;
     return set_slot(c, c->nm, s12, s13, w, n, mem, false);
 }
 
@@ -420,16 +452,190 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     return MIPWA_OK;
 }
 
+// ---- fixed-shape path: host side of A9 / A10 ---------------------------------------------------------------------
+static int effective_path(const mipwa_ctx* c)
+{
+    if (c->path != MIPWA_PATH_AUTO) return c->path;
+    return c->F == 0 ? MIPWA_PATH_CACHED_COMPACT : MIPWA_PATH_RECOMPUTE;
+}
+
+static int64_t cache_bytes_for(const mipwa_ctx* c, int kind, int64_t n)
+{
+    const int64_t cols = kind == MIPWA_PATH_CACHED ? c->N + c->R : 1 + c->R;
+    const int64_t tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
+    return tiles * MIPWA_TILE * cols * (int64_t)sizeof(double2);
+}
+
+// unit-coefficient model (a_k = 1, phi_k = 0, c_r = 1) with the shapes of `params` (or the listed ones) -> c->model
+static int build_unit_model(mipwa_ctx* c, const double* params)
+{
+    const int N = c->N, R = c->R;
+    std::vector<double> p(2 * N + 2 * R + 2 * c->F, 0.0);
+    for (int i = 0; i < N; ++i) p[i] = 1.0;
+    for (int r = 0; r < R; ++r) p[2 * N + 2 * r] = 1.0;
+    for (int r = 0, f = 0; r < R; ++r)
+        if (c->res[r].shape_floats) {
+            p[2 * N + 2 * R + 2 * f] = params ? params[2 * N + 2 * R + 2 * f] : c->res[r].mass;
+            p[2 * N + 2 * R + 2 * f + 1] = params ? params[2 * N + 2 * R + 2 * f + 1] : c->res[r].width;
+            ++f;
+        }
+    return build_model(c, p.data(), (int64_t)p.size());
+}
+
+static BasisAux basis_aux(const mipwa_ctx* c)
+{
+    BasisAux a;
+    a.Mx = c->d_Mx;
+    std::memset(a.col_of_slot, 0, sizeof(a.col_of_slot));
+    for (int d = 0; d < c->R; ++d) a.col_of_slot[d] = (uint8_t)c->perm[d];
+    return a;
+}
+
+static int ensure_cache(mipwa_ctx* c, int kind)
+{
+    if (c->cache_valid && c->cache_kind == kind) return MIPWA_OK;
+    const int64_t need = cache_bytes_for(c, kind, c->ev.n);
+    c->cache_valid = false;
+    if (c->user_cache && c->user_cache_bytes >= need) {
+        c->d_cache = c->user_cache;
+    } else {
+        if (c->owned_cache_bytes < need) {
+            if (c->owned_cache) cudaFree(c->owned_cache);
+            c->owned_cache = nullptr; c->owned_cache_bytes = 0;
+            if (need > 0) CU(c, cudaMalloc(&c->owned_cache, (size_t)need));
+            c->owned_cache_bytes = need;
+        }
+        c->d_cache = c->owned_cache;
+    }
+    if (c->ev.n > 0) {
+        int rc = build_unit_model(c, nullptr);
+        if (rc) return rc;
+        const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
+        const int grid = (int)std::min<int64_t>(tiles, (int64_t)c->sm_count * 8);
+        if (kind == MIPWA_PATH_CACHED)
+            k_basis_build<false><<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
+                                                                      c->ev.n, (double2*)c->d_cache);
+        else
+            k_basis_build<true><<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
+                                                                     c->ev.n, (double2*)c->d_cache);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        CU(c, cudaStreamSynchronize(c->stream));
+    }
+    c->cache_kind = kind;
+    c->cache_valid = true;
+    return MIPWA_OK;
+}
+
+static int ensure_gram(mipwa_ctx* c)
+{
+    if (c->gram_valid) return MIPWA_OK;
+    int rc = build_unit_model(c, nullptr);
+    if (rc) return rc;
+    const int K = c->N + c->R, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2;
+    const int tpt = (ntile + MIPWA_BLOCK - 1) / MIPWA_BLOCK;
+    const int grid = (int)std::min<int64_t>((c->nm.n + GRAM_P - 1) / GRAM_P, c->sm_count);
+    const size_t smem = (size_t)4 * nt * GRAM_LD * sizeof(double2);
+    double2* partial = nullptr;
+    CU(c, cudaMalloc(&partial, (size_t)grid * K * K * sizeof(double2)));
+    const double wd = 1.0 / (double)c->nm.n;
+    cudaError_t e = cudaSuccess;
+#define MIPWA_GRAM_LAUNCH(T)                                                                                         \
+    do {                                                                                                             \
+        e = cudaFuncSetAttribute(k_gram<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                 \
+        if (e == cudaSuccess)                                                                                        \
+            k_gram<T><<<grid, MIPWA_BLOCK, smem, c->stream>>>(c->model, basis_aux(c), c->nm.s12, c->nm.s13, c->nm.w, \
+                                                              c->nm.n, wd, partial);                                 \
+    } while (0)
+    if (tpt <= 1) MIPWA_GRAM_LAUNCH(1); else if (tpt == 2) MIPWA_GRAM_LAUNCH(2); else MIPWA_GRAM_LAUNCH(3);
+#undef MIPWA_GRAM_LAUNCH
+    ++c->launches;
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        k_gram_reduce<<<(K * K + 255) / 256, 256, 0, c->stream>>>(partial, grid, K, c->d_gram);
+        ++c->launches;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(partial);
+    if (e != cudaSuccess) return fail(c, MIPWA_ERR_CUDA, std::string("gram: ") + cudaGetErrorString(e));
+    c->gram_valid = true;
+    return MIPWA_OK;
+}
+
+// A1 for the cached kernels: c = [y_0 .. y_{N-1}, c_0 .. c_{R-1}] (caller's resonance order); needs build_model first
+static void fill_coef(const mipwa_ctx* c, const double* p, CoefDev* cc)
+{
+    const int N = c->N, R = c->R;
+    cc->K = N + R; cc->N = N;
+    for (int k = 0; k < N; ++k) cc->c[k] = make_double2(c->y_re[k], c->y_im[k]);
+    for (int r = 0; r < R; ++r)
+        cc->c[N + r] = make_double2(p[2 * N + 2 * r] * std::cos(p[2 * N + 2 * r + 1]),
+                                    p[2 * N + 2 * r] * std::sin(p[2 * N + 2 * r + 1]));
+}
+
+static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_log, double* integral)
+{
+    int rc = ensure_cache(c, kind);
+    if (rc) return rc;
+    rc = ensure_gram(c);
+    if (rc) return rc;
+    rc = build_model(c, params, 2 * c->N + 2 * c->R);      // after the ensure_* calls: they overwrite c->model
+    if (rc) return rc;
+    CoefDev cc;
+    fill_coef(c, params, &cc);
+    const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
+    const double2* cache = (const double2*)c->d_cache;
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    if (kind == MIPWA_PATH_CACHED) {
+        if (!c->dense_blocks_per_sm) {
+            CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->dense_blocks_per_sm, k_nll_dense, MIPWA_BLOCK, 0));
+            if (c->dense_blocks_per_sm < 1) c->dense_blocks_per_sm = 1;
+        }
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->dense_blocks_per_sm));
+        k_nll_dense<<<grid, MIPWA_BLOCK, 0, c->stream>>>(cc, cache, c->ev.n, c->d_gram, (double*)c->d_partials,
+                                                         c->d_ticket, c->d_result);
+    } else {
+        if (!c->compact_blocks_per_sm) {
+            CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->compact_blocks_per_sm, k_nll_compact<-1>, MIPWA_BLOCK, 0));
+            if (c->compact_blocks_per_sm < 1) c->compact_blocks_per_sm = 1;
+        }
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->compact_blocks_per_sm));
+#define MIPWA_COMPACT_LAUNCH(T)                                                                                   \
+    k_nll_compact<T><<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, cc, cache, c->ev.n, c->d_gram,                \
+                                                          (double*)c->d_partials, c->d_ticket, c->d_result)
+        switch (c->R) {
+            case 0: MIPWA_COMPACT_LAUNCH(0); break;
+            case 1: MIPWA_COMPACT_LAUNCH(1); break;
+            case 2: MIPWA_COMPACT_LAUNCH(2); break;
+            case 3: MIPWA_COMPACT_LAUNCH(3); break;
+            case 4: MIPWA_COMPACT_LAUNCH(4); break;
+            case 6: MIPWA_COMPACT_LAUNCH(6); break;
+            default: MIPWA_COMPACT_LAUNCH(-1); break;
+        }
+#undef MIPWA_COMPACT_LAUNCH
+    }
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    *sum_log = c->h_result[0];
+    *integral = c->h_result[1];
+    return MIPWA_OK;
+}
+
 int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* sum_log, double* integral)
 {
     if (!c || !params || !nll) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
     if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
     int rc = use_device(c);
     if (rc) return rc;
-    rc = build_model(c, params, n_params);
+    rc = build_model(c, params, n_params);                 // validates n_params and the parameter values
     if (rc) return rc;
     double S = 0, I = 0;
-    rc = nll_recompute(c, &S, &I);
+    const int path = effective_path(c);
+    rc = path == MIPWA_PATH_RECOMPUTE ? nll_recompute(c, &S, &I) : nll_cached(c, path, params, &S, &I);
     if (rc) return rc;
     *nll = -S + (double)c->ev.n * std::log(I);             // A7
     if (sum_log) *sum_log = S;
@@ -504,10 +710,58 @@ int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops)
 
 }  // extern "C"
 
-// ---- placeholders until cached.cuh / grad.cuh land ---------------------------------------------------------------
+
 extern "C" {
-int64_t mipwa_basis_bytes(const mipwa_ctx* c) { return c ? 0 : MIPWA_ERR_ARG; }
-int mipwa_set_basis_buffer(mipwa_ctx* c, void*, int64_t) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
-int mipwa_nll_grad(mipwa_ctx* c, const double*, int64_t, double*, double*) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
-int mipwa_eval_basis(mipwa_ctx* c, const double*, int64_t, int32_t, int64_t, int64_t, double*) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
+
+int64_t mipwa_basis_bytes(const mipwa_ctx* c)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    const int path = effective_path(c);
+    if (path == MIPWA_PATH_RECOMPUTE) return 0;
+    if (c->ev.n < 0) return MIPWA_ERR_STATE;
+    return cache_bytes_for(c, path, c->ev.n);
 }
+
+int mipwa_set_basis_buffer(mipwa_ctx* c, void* dev, int64_t bytes)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    if ((dev && bytes <= 0) || ((uintptr_t)dev & 255)) return fail(c, MIPWA_ERR_ARG, "buffer must be 256-byte aligned with bytes > 0");
+    int rc = use_device(c);
+    if (rc) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->user_cache = dev;
+    c->user_cache_bytes = dev ? bytes : 0;
+    c->cache_valid = false;
+    return MIPWA_OK;
+}
+
+int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32_t which, int64_t first, int64_t n,
+                     double* out)
+{
+    if (!c || !params || (which != 0 && which != 1)) return c ? fail(c, MIPWA_ERR_ARG, "bad argument") : MIPWA_ERR_ARG;
+    const Slot& s = which == 0 ? c->ev : c->nm;
+    if (s.n < 0) return fail(c, MIPWA_ERR_STATE, "slot not set");
+    if (first < 0 || n < 0 || first + n > s.n || (n > 0 && !out)) return fail(c, MIPWA_ERR_ARG, "bad range");
+    if (n_params != 2 * c->N + 2 * c->R + 2 * c->F) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_unit_model(c, params);
+    if (rc) return rc;
+    if (n == 0) return MIPWA_OK;
+    const int K = c->N + c->R;
+    double2* d_out = nullptr;
+    CU(c, cudaMalloc(&d_out, (size_t)n * K * sizeof(double2)));
+    k_basis_rows<<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, basis_aux(c), s.s12, s.s13, first, n, d_out);
+    ++c->launches;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(d_out);
+    if (e != cudaSuccess) return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e));
+    return MIPWA_OK;
+}
+
+// ---- placeholder until grad.cuh lands -------------------------------------------------------------------------------
+int mipwa_nll_grad(mipwa_ctx* c, const double*, int64_t, double*, double*) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
+
+}  // extern "C"

@@ -1,0 +1,178 @@
+"""GPU parity: fixed-shape cached paths (k_basis_build, k_gram, k_nll_dense, k_nll_compact) through the C ABI against
+the CPU oracle (8(c) O8).
+
+Tolerances: basis entries absolute 1e-12 x max(1, |B|) (cardinal-spline values are O(1) and change sign, so a pure
+relative test is ill-posed at their zeros); NLL as in DESIGN.md reading P14 (relative 1e-10).
+"""
+import numpy as np
+import pytest
+
+from tests.helpers import make_case, nll_tol
+
+pytestmark = pytest.mark.gpu
+
+
+def _lib():
+    from paper_1703_03284_b200 import binding
+    return binding
+
+
+CASES = {
+    0: dict(),                                    # 10k events (39 tiles + ragged tail), 5954-cell grid
+    1: dict(n_ev=40_000, n_norm=50_000),
+    2: dict(n_ev=30_011, n_norm=20_003),          # non-uniform knots
+    4: dict(n_ev=20_000, n_norm=20_000),          # K = 56, incl. a narrow resonance
+}
+
+
+@pytest.fixture(scope="module", params=sorted(CASES))
+def case(request):
+    return make_case(request.param, **CASES[request.param])
+
+
+def _ctx(c, data, path):
+    B = _lib()
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0], data[1])
+    m.set_norm_points(data[2], data[3], data[4])
+    m.set_path(path)
+    return m
+
+
+def test_basis_rows_match_oracle(case):
+    c, o, data = case
+    B = _lib()
+    m = _ctx(c, data, B.PATH_CACHED)
+    for which, (a, b) in enumerate([(data[0], data[1]), (data[2], data[3])]):
+        n = min(a.size, 3000)
+        first = a.size - n                         # the ragged end of the slot
+        got = m.eval_basis(c.truth, which, first, n)
+        ref = o.basis(c.truth, a[first:], b[first:])
+        err = np.abs(got - ref) / np.maximum(1.0, np.abs(ref))
+        assert err.max() < 1e-12, (c.idx, which, err.max())
+        assert np.all(got[:, :c.N].imag == 0.0)    # spline columns are real
+    m.close()
+
+
+@pytest.mark.parametrize("path_name", ["PATH_CACHED", "PATH_CACHED_COMPACT"])
+def test_cached_nll_matches_oracle_and_recompute(case, path_name):
+    c, o, data = case
+    B = _lib()
+    m = _ctx(c, data, getattr(B, path_name))
+    mr = _ctx(c, data, B.PATH_RECOMPUTE)
+    cols = c.N + c.R if path_name == "PATH_CACHED" else 1 + c.R
+    assert m.basis_bytes() == -(-data[0].size // 256) * 256 * cols * 16
+    for t in range(3):
+        p = c.perturbed(t)
+        ref, sl, integ = o.nll(p, *data, parts=True)
+        got, gsl, ginteg = m.nll_parts(p)
+        tol = nll_tol(ref, sl, integ, data[0].size)
+        assert abs(got - ref) <= tol, (got, ref, tol)
+        assert gsl == pytest.approx(sl, rel=1e-12)
+        assert ginteg == pytest.approx(integ, rel=1e-12)          # c^H G c against the direct sum
+        assert abs(got - mr.nll(p)) <= tol
+        assert m.nll(p) == got                                     # bit-reproducible call to call
+    m.close(); mr.close()
+
+
+def test_gram_matches_oracle(case):
+    """I = c^H G c for unit vectors and pairs recovers every Gram entry the oracle computes directly."""
+    c, o, data = case
+    if c.idx not in (0, 2):
+        pytest.skip("covered on two configs")
+    B = _lib()
+    n = 4000
+    g12, g13, w = data[2][:n], data[3][:n], data[4][:n]
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0][:10], data[1][:10])
+    m.set_norm_points(g12, g13, w)
+    m.set_path(B.PATH_CACHED)
+    G = o.gram(c.truth, g12, g13, w)
+    N, R = c.N, c.R
+    rng = np.random.default_rng(5)
+    for _ in range(6):
+        coef = rng.normal(size=N + R) + 1j * rng.normal(size=N + R)
+        p = np.concatenate([np.abs(coef[:N]), np.angle(coef[:N]),
+                            np.stack([np.abs(coef[N:]), np.angle(coef[N:])], axis=1).ravel()])
+        _, _, integ = m.nll_parts(p)
+        assert integ == pytest.approx(float(np.real(np.conj(coef) @ G @ coef)), rel=1e-12)
+    m.close()
+
+
+def test_cache_management():
+    import torch
+    B = _lib()
+    c, o, (e12, e13, g12, g13, w) = make_case(1, n_ev=5000, n_norm=4000)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_path(B.PATH_CACHED)
+    with pytest.raises(B.MipwaError) as ei:
+        m.basis_bytes()
+    assert ei.value.code == B.ERR_STATE
+    m.set_events(e12, e13); m.set_norm_points(g12, g13, w)
+    p = c.perturbed(2)
+    ref, sl, integ = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    tol = nll_tol(ref, sl, integ, e12.size)
+    # caller-provided storage
+    buf = torch.empty(m.basis_bytes(), dtype=torch.uint8, device="cuda")
+    m.set_basis_buffer(buf)
+    assert abs(m.nll(p) - ref) <= tol
+    assert buf.view(torch.float64)[:2 * 256].abs().sum().item() > 0           # the library wrote into it
+    # new events invalidate the cache; a too-small buffer falls back to library storage
+    m.set_events(e12[:777], e13[:777])
+    ref2, sl2, integ2 = o.nll(p, e12[:777], e13[:777], g12, g13, w, parts=True)
+    assert abs(m.nll(p) - ref2) <= nll_tol(ref2, sl2, integ2, 777)
+    m.set_basis_buffer(torch.empty(256, dtype=torch.uint8, device="cuda"))
+    assert abs(m.nll(p) - ref2) <= nll_tol(ref2, sl2, integ2, 777)
+    # new normalisation points invalidate the Gram matrix
+    m.set_norm_points(g12[:1500], g13[:1500], None)
+    ref3, sl3, integ3 = o.nll(p, e12[:777], e13[:777], g12[:1500], g13[:1500], None, parts=True)
+    assert abs(m.nll(p) - ref3) <= nll_tol(ref3, sl3, integ3, 777)
+    # switching layouts rebuilds
+    m.set_path(B.PATH_CACHED_COMPACT)
+    assert abs(m.nll(p) - ref3) <= nll_tol(ref3, sl3, integ3, 777)
+    m.set_path(B.PATH_AUTO)                                                    # no shape floats -> a cached path
+    assert m.basis_bytes() > 0
+    assert abs(m.nll(p) - ref3) <= nll_tol(ref3, sl3, integ3, 777)
+    # empty event sample
+    m.set_events(np.empty(0), np.empty(0))
+    assert m.nll(p) == 0.0
+    m.close()
+    # floating shapes cannot be cached; AUTO then recomputes
+    c3, o3, d3 = make_case(3, n_ev=3000, n_norm=3000)
+    m3 = B.Mipwa(c3.kin, c3.knots, c3.resonances)
+    for path in (B.PATH_CACHED, B.PATH_CACHED_COMPACT):
+        with pytest.raises(B.MipwaError) as ei:
+            m3.set_path(path)
+        assert ei.value.code == B.ERR_STATE
+    m3.set_events(d3[0], d3[1]); m3.set_norm_points(d3[2], d3[3], d3[4])
+    assert m3.basis_bytes() == 0
+    ref, sl, integ = o3.nll(c3.truth, *d3, parts=True)
+    assert abs(m3.nll(c3.truth) - ref) <= nll_tol(ref, sl, integ, 3000)
+    # the basis hook follows floating shapes given in the parameter vector
+    p = c3.truth.copy(); p[-2:] = [0.781, 0.153]
+    got = m3.eval_basis(p, 0, 0, 500)
+    refb = o3.basis(p, d3[0][:500], d3[1][:500])
+    assert (np.abs(got - refb) / np.maximum(1.0, np.abs(refb))).max() < 1e-12
+    m3.close()
+
+
+def test_many_knots_gram_tiles():
+    """K = 100 + 2 needs more than one 4 x 4 register tile per thread in k_gram (TPT = 2)."""
+    B = _lib()
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    c = I.Config(1)
+    knots = I.knots_uniform(100)
+    o = orc.Oracle(c.kin, knots, c.resonances)
+    rng = np.random.default_rng(11)
+    p = np.concatenate([rng.uniform(0.5, 2, 100), rng.uniform(0, 3, 100), [0.7, 0.3, 1.4, 2.2]])
+    g12, g13 = I.phase_space_points(5000, c.key(I.S_NORM))
+    e12, e13 = g12[:2000], g13[:2000]
+    g12, g13 = g12[2000:], g13[2000:]
+    ref, sl, integ = o.nll(p, e12, e13, g12, g13, None, parts=True)
+    for path in (B.PATH_CACHED, B.PATH_CACHED_COMPACT):
+        m = B.Mipwa(c.kin, knots, c.resonances)
+        m.set_events(e12, e13); m.set_norm_points(g12, g13, None)
+        m.set_path(path)
+        assert abs(m.nll(p) - ref) <= nll_tol(ref, sl, integ, 2000)
+        m.close()
