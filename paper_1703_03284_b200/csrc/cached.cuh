@@ -16,7 +16,6 @@
 
 #define MIPWA_TILE 256
 #define MIPWA_MAX_K (MIPWA_DEV_MAX_KNOTS + MIPWA_DEV_MAX_RES)
-static_assert(MIPWA_TILE == MIPWA_BLOCK, "one event per thread and tile");
 
 struct CoefDev {                    // the linear coefficients of one call, a __grid_constant__ kernel parameter
     int32_t K, N;
@@ -76,7 +75,7 @@ __device__ __forceinline__ void basis_point(const SplineSmem& sm, const DevModel
 
 // ---- A9: build the per-event cache -------------------------------------------------------------------------------
 template <bool COMPACT>
-__global__ void __launch_bounds__(MIPWA_BLOCK)
+__global__ void __launch_bounds__(MIPWA_TILE)
 k_basis_build(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ s12,
               const double* __restrict__ s13, long long n, double2* __restrict__ cache)
 {
@@ -100,7 +99,7 @@ k_basis_build(const __grid_constant__ DevModel m, const BasisAux aux, const doub
 }
 
 // ---- test hook: basis rows, row-major out[i*K + k] ----------------------------------------------------------------
-__global__ void __launch_bounds__(MIPWA_BLOCK)
+__global__ void __launch_bounds__(MIPWA_TILE)
 k_basis_rows(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ s12,
              const double* __restrict__ s13, long long first, long long n, double2* __restrict__ out)
 {
@@ -173,7 +172,7 @@ __device__ __forceinline__ double2 ld_stream(const double2* p)
 #ifndef MIPWA_DENSE_MINBLOCKS
 #define MIPWA_DENSE_MINBLOCKS 4
 #endif
-__global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_DENSE_MINBLOCKS)
+__global__ void __launch_bounds__(MIPWA_TILE, MIPWA_DENSE_MINBLOCKS)
 k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cache, long long n_ev,
             const double2* __restrict__ G, double* __restrict__ partials, unsigned int* __restrict__ ticket,
             double* __restrict__ result)
@@ -224,7 +223,7 @@ k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cach
 // Streams 16 + 16 R bytes per event; the spline part comes from the per-call segment coefficients in shared memory
 // (same Horner evaluation as the recompute path).  cc.c[N + r] = c_r in the caller's resonance order.
 template <int RT>      // RT >= 0: number of resonances known at compile time; -1: run-time
-__global__ void __launch_bounds__(MIPWA_BLOCK, 4)
+__global__ void __launch_bounds__(MIPWA_TILE, 4)
 k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDev cc,
               const double2* __restrict__ cache, long long n_ev, const double2* __restrict__ G,
               double* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result)
@@ -291,7 +290,7 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
 #define GRAM_LD (GRAM_P + 1)
 
 template <int TPT>
-__global__ void __launch_bounds__(MIPWA_BLOCK, 1)
+__global__ void __launch_bounds__(MIPWA_TILE, 1)
 k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ g12,
        const double* __restrict__ g13, const double* __restrict__ gw, long long n, double w_default,
        double2* __restrict__ partial)
@@ -307,7 +306,7 @@ k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __r
     int ta[TPT], tb[TPT];
 #pragma unroll
     for (int u = 0; u < TPT; ++u) {                                // tile t -> (a, b), a <= b, row-major upper triangle
-        int t = threadIdx.x + u * MIPWA_BLOCK, a = 0;
+        int t = threadIdx.x + u * MIPWA_TILE, a = 0;
         if (t >= ntile) { ta[u] = -1; tb[u] = -1; continue; }
         while (t >= nt - a) { t -= nt - a; ++a; }
         ta[u] = a; tb[u] = a + t;
@@ -325,7 +324,7 @@ k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __r
     for (long long base = (long long)blockIdx.x * GRAM_P; base < n; base += (long long)gridDim.x * GRAM_P) {
         const long long j = base + p;
         if (j < n) {
-            basis_point(sm, m, aux, g12[j], g13[j], slice, MIPWA_BLOCK / 32, true,
+            basis_point(sm, m, aux, g12[j], g13[j], slice, MIPWA_TILE / 32, true,
                         [&](int k, double2 v) { Bs[k * GRAM_LD + p] = v; });
             if (slice == 0) ws[p] = gw ? gw[j] : w_default;
         } else if (slice == 0) {

@@ -1,0 +1,299 @@
+// grad.cuh -- analytic gradient of the NLL on the recompute path (BASELINE configs[3]).
+//
+// With calG_k := dNLL/dRe c_k + i dNLL/dIm c_k for every complex linear coefficient c_k of A = sum_k c_k B_k,
+//   calG_k = sum_i f_i conj(B_ik) + (2 n_ev / I) sum_j g_j conj(B_jk),   f_i = -2 / conj(A_i),  g_j = w_j A_j.
+// The kernel never forms the dense spline basis.  On segment j the S-wave is the cubic
+//   S(s) = sum_q sc[q][j] t^q,  t = s - x_j,
+// and sc is a REAL linear image of the knot values y (DevModel::sc, built on the host from y and y'' = Mx y), so it
+// is enough to accumulate the complex moments  M[q][j] = sum f t^q  over the points whose channel falls in segment
+// j (the adjoint of the Horner evaluation); the host applies the transposed map sc -> (y, y'') -> y and the polar
+// chain rule (O(N) work, one transposed tridiagonal relation via Mx^T).  Resonance coefficients get
+// F_r = sum f conj(T_r(s12,s13) + T_r(s13,s12)) in per-thread registers.
+//
+// Scatter without atomics in the inner loop: mipwa_nll_grad works on a copy of the points SORTED BY CELL
+// (cell = seg(s12) * (N-1) + seg(s13); knots are fixed, so the order is built once per mipwa_set_*).  Each warp owns
+// a contiguous chunk, so consecutive iterations of a warp stay in one cell for thousands of points: the 8 complex
+// moments (4 per channel) live in registers and are flushed (warp shuffle reduction, then 16 shared-memory
+// adds by lane 0) only when the warp's cell changes.  A warp-iteration that straddles a cell boundary takes a
+// per-lane shared-atomic slow path (at most once per cell boundary).
+#pragma once
+#include "cached.cuh"
+
+// segment index and offset of one channel, then the Horner value (same arithmetic as spline_eval)
+__device__ __forceinline__ void spline_eval_jt(const SplineSmem& sm, const DevModel& m, double s, int& j, double& t,
+                                               double& re, double& im)
+{
+    double xj;
+    j = spline_segment(sm, m, s, xj);
+    t = s - xj;
+    const double2 c0 = sm.sc[0][j], c1 = sm.sc[1][j], c2 = sm.sc[2][j], c3 = sm.sc[3][j];
+    re = fma(t, fma(t, fma(t, c3.x, c2.x), c1.x), c0.x);
+    im = fma(t, fma(t, fma(t, c3.y, c2.y), c1.y), c0.y);
+}
+
+#define MIPWA_GRAD_MAXR (MIPWA_DEV_MAX_RES)
+
+// amplitude with the pieces the gradient needs: segment/offset of both channels and every symmetrised resonance
+// term WITHOUT its coefficient (device slot order; the host multiplies by sqrt(n_R n_D))
+template <int R1, int R2>
+__device__ __forceinline__ void amplitude_parts(const SplineSmem& sm, const DevModel& m, double s12, double s13,
+                                                double& are, double& aim, int& j1, double& t1, int& j2, double& t2,
+                                                double (&tr)[R1 >= 0 ? (R1 + R2 > 0 ? R1 + R2 : 1) : MIPWA_GRAD_MAXR],
+                                                double (&ti)[R1 >= 0 ? (R1 + R2 > 0 ? R1 + R2 : 1) : MIPWA_GRAD_MAXR])
+{
+    double r1, i1, r2, i2;
+    spline_eval_jt(sm, m, s12, j1, t1, r1, i1);
+    spline_eval_jt(sm, m, s13, j2, t2, r2, i2);
+    are = r1 + r2;
+    aim = i1 + i2;
+    if (R1 == 0 && R2 == 0) return;
+    const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
+    if (R1 >= 0) {
+#pragma unroll
+        for (int r = 0; r < R1; ++r) resonance_sym<1>(m.res[r], ca, cb, tr[r], ti[r]);
+#pragma unroll
+        for (int r = 0; r < R2; ++r) resonance_sym<2>(m.res[R1 + r], ca, cb, tr[R1 + r], ti[R1 + r]);
+#pragma unroll
+        for (int r = 0; r < R1 + R2; ++r) {
+            are = fma(m.res[r].cre, tr[r], fma(-m.res[r].cim, ti[r], are));
+            aim = fma(m.res[r].cre, ti[r], fma(m.res[r].cim, tr[r], aim));
+        }
+    } else {
+        for (int r = 0; r < m.R; ++r) {
+            resonance_sym<-1>(m.res[r], ca, cb, tr[r], ti[r]);
+            are = fma(m.res[r].cre, tr[r], fma(-m.res[r].cim, ti[r], are));
+            aim = fma(m.res[r].cre, ti[r], fma(m.res[r].cim, tr[r], aim));
+        }
+    }
+}
+
+// per-warp running moments of the current cell
+struct CellAcc {
+    double v[16];          // [channel][q][re,im]
+    int j1, j2;            // segments of the cell, -1: empty
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = 0.0;
+    }
+    __device__ __forceinline__ void add(double fr, double fi, double t1, double t2) {
+        double p = 1.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { v[2 * q] = fma(fr, p, v[2 * q]); v[2 * q + 1] = fma(fi, p, v[2 * q + 1]); p *= t1; }
+        p = 1.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { v[8 + 2 * q] = fma(fr, p, v[8 + 2 * q]); v[8 + 2 * q + 1] = fma(fi, p, v[8 + 2 * q + 1]); p *= t2; }
+    }
+};
+
+// bins[(q * NS + j) * 2 + {0,1}], NS = N - 1 segments
+__device__ __forceinline__ void flush_warp(CellAcc& a, double* bins, int NS)
+{
+    if (a.j1 >= 0) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            double x = a.v[k];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+            a.v[k] = x;
+        }
+        if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                atomicAdd(&bins[(q * NS + a.j1) * 2], a.v[2 * q]);
+                atomicAdd(&bins[(q * NS + a.j1) * 2 + 1], a.v[2 * q + 1]);
+                atomicAdd(&bins[(q * NS + a.j2) * 2], a.v[8 + 2 * q]);
+                atomicAdd(&bins[(q * NS + a.j2) * 2 + 1], a.v[8 + 2 * q + 1]);
+            }
+        }
+    }
+    a.clear();
+    a.j1 = a.j2 = -1;
+}
+
+__device__ __forceinline__ void scatter_lane(double fr, double fi, int j1, double t1, int j2, double t2, double* bins, int NS)
+{
+    double p = 1.0;
+    for (int q = 0; q < 4; ++q) { atomicAdd(&bins[(q * NS + j1) * 2], fr * p); atomicAdd(&bins[(q * NS + j1) * 2 + 1], fi * p); p *= t1; }
+    p = 1.0;
+    for (int q = 0; q < 4; ++q) { atomicAdd(&bins[(q * NS + j2) * 2], fr * p); atomicAdd(&bins[(q * NS + j2) * 2 + 1], fi * p); p *= t2; }
+}
+
+// sum over the block of one value per thread (valid in thread 0); red32: 32 doubles of shared memory
+__device__ __forceinline__ double block_sum(double x, double* red32)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+    __syncthreads();                                       // red32 free again
+    if (lane == 0) red32[warp] = x;
+    __syncthreads();
+    x = (warp == 0 && lane < nwarp) ? red32[lane] : 0.0;
+    if (warp == 0) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+    }
+    return x;
+}
+
+template <int R1, int R2> struct GradDims {
+    static constexpr int RR = R1 >= 0 ? (R1 + R2 > 0 ? R1 + R2 : 1) : MIPWA_GRAD_MAXR;
+};
+
+// one pass over a cell-sorted point set.  EV: events (f = -2/conj(A), scalar = sum ln|A|^2);
+// otherwise normalisation points (f = w A, scalar = sum w |A|^2).
+template <int R1, int R2, bool EV>
+__device__ __forceinline__ void grad_pass(const SplineSmem& sm, const DevModel& m, const double* __restrict__ s12,
+                                          const double* __restrict__ s13, const double* __restrict__ w, long long n,
+                                          double* bins, double& scalar, double (&Fr)[GradDims<R1, R2>::RR],
+                                          double (&Fi)[GradDims<R1, R2>::RR])
+{
+    constexpr int RR = GradDims<R1, R2>::RR;
+    const int NS = m.N - 1, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long long W = (long long)gridDim.x * wpb, wg = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    const long long CH = (((n + W - 1) / W) + 31) & ~31LL;
+    const long long lo = wg * CH, hi = lo + CH < n ? lo + CH : n;
+    CellAcc acc;
+    acc.clear();
+    acc.j1 = acc.j2 = -1;
+    LogProd lp;
+    double integ = 0.0;
+    const int nres = R1 >= 0 ? R1 + R2 : m.R;
+    for (long long base = lo; base < hi; base += 32) {                     // warp-uniform trip count
+        const long long i = base + lane;
+        const bool valid = i < hi;
+        const long long ii = valid ? i : lo;
+        const double x = s12[ii], y = s13[ii];
+        const double wv = EV ? 0.0 : (valid ? (w ? w[ii] : 1.0) : 0.0);
+        double are, aim, t1, t2, tr[RR], ti[RR];
+        int j1, j2;
+        amplitude_parts<R1, R2>(sm, m, x, y, are, aim, j1, t1, j2, t2, tr, ti);
+        const double a2 = fma(are, are, aim * aim);
+        double fr, fi;
+        if (EV) {
+            const double k = valid ? -2.0 * fast_rcp(a2) : 0.0;
+            fr = k * are; fi = k * aim;
+            lp.add(valid ? a2 : 1.0);
+        } else {
+            fr = wv * are; fi = wv * aim;
+            integ = fma(wv, a2, integ);
+        }
+        if (R1 >= 0) {
+#pragma unroll
+            for (int r = 0; r < (R1 >= 0 ? R1 + R2 : 0); ++r) {
+                Fr[r] = fma(fr, tr[r], fma(fi, ti[r], Fr[r]));             // f conj(T)
+                Fi[r] = fma(fi, tr[r], fma(-fr, ti[r], Fi[r]));
+            }
+        } else {
+            for (int r = 0; r < nres; ++r) {
+                Fr[r] = fma(fr, tr[r], fma(fi, ti[r], Fr[r]));
+                Fi[r] = fma(fi, tr[r], fma(-fr, ti[r], Fi[r]));
+            }
+        }
+        const bool same = !valid || (j1 == acc.j1 && j2 == acc.j2);
+        if (__all_sync(0xffffffffu, same)) {
+            acc.add(fr, fi, t1, t2);
+        } else {
+            flush_warp(acc, bins, NS);
+            const int l1 = __shfl_sync(0xffffffffu, j1, 0), l2 = __shfl_sync(0xffffffffu, j2, 0);   // lane 0 is valid
+            const bool uni = !valid || (j1 == l1 && j2 == l2);
+            if (__all_sync(0xffffffffu, uni)) {
+                acc.j1 = l1; acc.j2 = l2;
+                acc.add(fr, fi, t1, t2);
+            } else if (valid) {
+                scatter_lane(fr, fi, j1, t1, j2, t2, bins, NS);
+            }
+        }
+    }
+    flush_warp(acc, bins, NS);
+    scalar = EV ? lp.value() : integ;
+}
+
+// result / partial layout (doubles): [0] sum ln|A|^2, [1] sum w|A|^2, [2 + 2d + {0,1}] F_ev of device slot d,
+// [2 + 2R + 2d + {0,1}] F_nm, then bins_ev[4][N-1][2], bins_nm[4][N-1][2];  NV = 2 + 4R + 16 (N-1).
+#ifndef MIPWA_GRAD_MINBLOCKS
+#define MIPWA_GRAD_MINBLOCKS 2
+#endif
+template <int R1, int R2>
+__global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_GRAD_MINBLOCKS)
+k_grad_recompute(const __grid_constant__ DevModel m,
+                 const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
+                 const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
+                 long long n_norm, double* __restrict__ partials, unsigned int* __restrict__ ticket,
+                 double* __restrict__ result)
+{
+    constexpr int RR = GradDims<R1, R2>::RR;
+    extern __shared__ double grad_bins[];                  // [2][4][N-1][2]
+    __shared__ SplineSmem sm;
+    __shared__ double red32[32];
+    __shared__ bool is_last;
+    const int NS = m.N - 1, R = m.R, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
+    for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) grad_bins[k] = 0.0;
+    load_spline_smem(sm, m);                               // ends with __syncthreads()
+
+    double S = 0.0, I = 0.0, Fer[RR], Fei[RR], Fnr[RR], Fni[RR];
+#pragma unroll
+    for (int r = 0; r < RR; ++r) Fer[r] = Fei[r] = Fnr[r] = Fni[r] = 0.0;
+    grad_pass<R1, R2, true>(sm, m, e12, e13, nullptr, n_ev, grad_bins, S, Fer, Fei);
+    grad_pass<R1, R2, false>(sm, m, g12, g13, gw, n_norm, grad_bins + nb, I, Fnr, Fni);
+
+    double* mine = partials + (size_t)blockIdx.x * NV;
+    double v = block_sum(S, red32);
+    if (threadIdx.x == 0) mine[0] = v;
+    v = block_sum(I, red32);
+    if (threadIdx.x == 0) mine[1] = v;
+    for (int r = 0; r < R; ++r) {
+        double a = 0, b = 0, c = 0, d = 0;
+        if (R1 >= 0) {
+#pragma unroll
+            for (int q = 0; q < RR; ++q) if (q == r) { a = Fer[q]; b = Fei[q]; c = Fnr[q]; d = Fni[q]; }
+        } else { a = Fer[r]; b = Fei[r]; c = Fnr[r]; d = Fni[r]; }
+        a = block_sum(a, red32); if (threadIdx.x == 0) mine[2 + 2 * r] = a;
+        b = block_sum(b, red32); if (threadIdx.x == 0) mine[2 + 2 * r + 1] = b;
+        c = block_sum(c, red32); if (threadIdx.x == 0) mine[2 + 2 * R + 2 * r] = c;
+        d = block_sum(d, red32); if (threadIdx.x == 0) mine[2 + 2 * R + 2 * r + 1] = d;
+    }
+    __syncthreads();                                       // all flushes into grad_bins are done
+    for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) mine[2 + 4 * R + k] = grad_bins[k];
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        for (int k = threadIdx.x; k < NV; k += blockDim.x) {
+            double s = 0.0;
+            for (int b = 0; b < gridDim.x; ++b) s += __ldcg(&partials[(size_t)b * NV + k]);      // block order
+            result[k] = s;
+        }
+        __threadfence_system();
+        if (threadIdx.x == 0) *ticket = 0;
+    }
+}
+
+// ---- cell sort (once per point set): key = seg(s12) * (N-1) + seg(s13) ---------------------------------------------
+__global__ void __launch_bounds__(MIPWA_TILE)
+k_cell_keys(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
+            long long n, unsigned int* __restrict__ keys, unsigned int* __restrict__ idx)
+{
+    __shared__ SplineSmem sm;
+    load_spline_smem(sm, m);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        double xj;
+        const int j1 = spline_segment(sm, m, s12[i], xj), j2 = spline_segment(sm, m, s13[i], xj);
+        keys[i] = (unsigned int)(j1 * (m.N - 1) + j2);
+        idx[i] = (unsigned int)i;
+    }
+}
+
+__global__ void __launch_bounds__(MIPWA_TILE)
+k_gather(const unsigned int* __restrict__ idx, long long n, const double* __restrict__ a, const double* __restrict__ b,
+         const double* __restrict__ c, double* __restrict__ oa, double* __restrict__ ob, double* __restrict__ oc)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const unsigned int s = idx[i];
+        oa[i] = a[s]; ob[i] = b[s];
+        if (c) oc[i] = c[s];
+    }
+}

@@ -11,6 +11,9 @@
 
 #include "kernels.cuh"
 #include "cached.cuh"
+#include "grad.cuh"
+
+#include <cub/device/device_radix_sort.cuh>
 
 static_assert(MIPWA_DEV_MAX_KNOTS == MIPWA_MAX_KNOTS, "capacity mismatch");
 static_assert(MIPWA_DEV_MAX_RES == MIPWA_MAX_RESONANCES, "capacity mismatch");
@@ -74,6 +77,14 @@ struct mipwa_ctx {
     bool gram_valid = false;
     int dense_blocks_per_sm = 0, compact_blocks_per_sm = 0;
 
+    // gradient (A8): cell-sorted copies of both point sets, per-block partial vectors
+    Slot ev_sorted, nm_sorted;
+    bool ev_sorted_valid = false, nm_sorted_valid = false;
+    int grad_blocks_per_sm = 0;
+    double* d_gpartials = nullptr;
+    size_t gpartials_len = 0;
+    double res_fold[MIPWA_MAX_RESONANCES];   // sqrt(n_R n_D) of device slot d for the current call
+
     bool timing = false;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     float last_ms = 0.f;
@@ -102,7 +113,7 @@ double lam(double a, double b, double c) { return (a - b - c) * (a - b - c) - 4.
 double barrier_num(int L, double z0) { return L == 0 ? 1.0 : (L == 1 ? 1.0 + z0 : 9.0 + 3.0 * z0 + z0 * z0); }
 
 // A3: constants of one resonance for the device formulas of dev_model.cuh
-int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, double carg, ResDev* out)
+int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, double carg, ResDev* out, double* fold)
 {
     const mipwa_kinematics& k = c->kin;
     const mipwa_resonance& d = c->res[r];
@@ -118,6 +129,7 @@ int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, 
     out->cD = L ? d.r_parent * d.r_parent / (4.0 * M2) : 0.0;
     out->Kw = m0sq * g0 * nR / (std::pow(4.0 * q0sq, L) * std::sqrt(q0sq));
     const double f = cmag * std::sqrt(nR * nD);
+    if (fold) *fold = std::sqrt(nR * nD);
     out->cre = f * std::cos(carg);
     out->cim = f * std::sin(carg);
     out->pa = L == 2 ? 1.0 : 0.0;
@@ -216,7 +228,7 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
         const int r = c->perm[d];
         double m0 = c->res[r].mass, g0 = c->res[r].width;
         if (fidx[r] >= 0) { m0 = p[2 * N + 2 * R + 2 * fidx[r]]; g0 = p[2 * N + 2 * R + 2 * fidx[r] + 1]; }
-        const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[d]);
+        const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[d], &c->res_fold[d]);
         if (rc) return rc;
     }
     return MIPWA_OK;
@@ -306,6 +318,9 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
                        ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute<R1, R2>,
                                                                           MIPWA_BLOCK, 0) == cudaSuccess);
     if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
+#ifdef MIPWA_FORCE_BPS
+    c->blocks_per_sm = MIPWA_FORCE_BPS;                    // experiments only
+#endif
     const size_t max_grid = (size_t)c->sm_count * 16;
     ok = ok && cudaMalloc(&c->d_partials, max_grid * sizeof(double2) * 64) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_ticket, 64) == cudaSuccess && cudaMemset(c->d_ticket, 0, 64) == cudaSuccess;
@@ -333,6 +348,8 @@ void mipwa_destroy(mipwa_ctx* c)
     if (c->d_Mx) cudaFree(c->d_Mx);
     if (c->owned_cache) cudaFree(c->owned_cache);
     if (c->d_gram) cudaFree(c->d_gram);
+    if (c->d_gpartials) cudaFree(c->d_gpartials);
+    free_slot(c->ev_sorted); free_slot(c->nm_sorted);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_bad) cudaFreeHost(c->h_bad);
     if (c->ev0) cudaEventDestroy(c->ev0);
@@ -408,13 +425,13 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
 
 int mipwa_set_events(mipwa_ctx* c, const double* s12, const double* s13, int64_t n, int32_t mem)
 {
-    if (c) c->cache_valid = false;
+    if (c) { c->cache_valid = false; c->ev_sorted_valid = false; }
     return set_slot(c, c->ev, s12, s13, nullptr, n, mem, true);
 }
 
 int mipwa_set_norm_points(mipwa_ctx* c, const double* s12, const double* s13, const double* w, int64_t n, int32_t mem)
 {
-    if (c) c->gram_valid = false;
+    if (c) { c->gram_valid = false; c->nm_sorted_valid = false; }
     return set_slot(c, c->nm, s12, s13, w, n, mem, false);
 }
 
@@ -513,10 +530,10 @@ static int ensure_cache(mipwa_ctx* c, int kind)
         const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
         const int grid = (int)std::min<int64_t>(tiles, (int64_t)c->sm_count * 8);
         if (kind == MIPWA_PATH_CACHED)
-            k_basis_build<false><<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
+            k_basis_build<false><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
                                                                       c->ev.n, (double2*)c->d_cache);
         else
-            k_basis_build<true><<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
+            k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
                                                                      c->ev.n, (double2*)c->d_cache);
         ++c->launches;
         CU(c, cudaGetLastError());
@@ -533,7 +550,7 @@ static int ensure_gram(mipwa_ctx* c)
     int rc = build_unit_model(c, nullptr);
     if (rc) return rc;
     const int K = c->N + c->R, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2;
-    const int tpt = (ntile + MIPWA_BLOCK - 1) / MIPWA_BLOCK;
+    const int tpt = (ntile + MIPWA_TILE - 1) / MIPWA_TILE;
     const int grid = (int)std::min<int64_t>((c->nm.n + GRAM_P - 1) / GRAM_P, c->sm_count);
     const size_t smem = (size_t)4 * nt * GRAM_LD * sizeof(double2);
     double2* partial = nullptr;
@@ -544,7 +561,7 @@ static int ensure_gram(mipwa_ctx* c)
     do {                                                                                                             \
         e = cudaFuncSetAttribute(k_gram<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                 \
         if (e == cudaSuccess)                                                                                        \
-            k_gram<T><<<grid, MIPWA_BLOCK, smem, c->stream>>>(c->model, basis_aux(c), c->nm.s12, c->nm.s13, c->nm.w, \
+            k_gram<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), c->nm.s12, c->nm.s13, c->nm.w, \
                                                               c->nm.n, wd, partial);                                 \
     } while (0)
     if (tpt <= 1) MIPWA_GRAM_LAUNCH(1); else if (tpt == 2) MIPWA_GRAM_LAUNCH(2); else MIPWA_GRAM_LAUNCH(3);
@@ -589,20 +606,20 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
     if (kind == MIPWA_PATH_CACHED) {
         if (!c->dense_blocks_per_sm) {
-            CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->dense_blocks_per_sm, k_nll_dense, MIPWA_BLOCK, 0));
+            CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->dense_blocks_per_sm, k_nll_dense, MIPWA_TILE, 0));
             if (c->dense_blocks_per_sm < 1) c->dense_blocks_per_sm = 1;
         }
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->dense_blocks_per_sm));
-        k_nll_dense<<<grid, MIPWA_BLOCK, 0, c->stream>>>(cc, cache, c->ev.n, c->d_gram, (double*)c->d_partials,
+        k_nll_dense<<<grid, MIPWA_TILE, 0, c->stream>>>(cc, cache, c->ev.n, c->d_gram, (double*)c->d_partials,
                                                          c->d_ticket, c->d_result);
     } else {
         if (!c->compact_blocks_per_sm) {
-            CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->compact_blocks_per_sm, k_nll_compact<-1>, MIPWA_BLOCK, 0));
+            CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->compact_blocks_per_sm, k_nll_compact<-1>, MIPWA_TILE, 0));
             if (c->compact_blocks_per_sm < 1) c->compact_blocks_per_sm = 1;
         }
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->compact_blocks_per_sm));
 #define MIPWA_COMPACT_LAUNCH(T)                                                                                   \
-    k_nll_compact<T><<<grid, MIPWA_BLOCK, 0, c->stream>>>(c->model, cc, cache, c->ev.n, c->d_gram,                \
+    k_nll_compact<T><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, cc, cache, c->ev.n, c->d_gram,                \
                                                           (double*)c->d_partials, c->d_ticket, c->d_result)
         switch (c->R) {
             case 0: MIPWA_COMPACT_LAUNCH(0); break;
@@ -751,7 +768,7 @@ int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32
     const int K = c->N + c->R;
     double2* d_out = nullptr;
     CU(c, cudaMalloc(&d_out, (size_t)n * K * sizeof(double2)));
-    k_basis_rows<<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, basis_aux(c), s.s12, s.s13, first, n, d_out);
+    k_basis_rows<<<grid_for(c, n, 4), MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), s.s12, s.s13, first, n, d_out);
     ++c->launches;
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
@@ -761,7 +778,137 @@ int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32
     return MIPWA_OK;
 }
 
-// ---- placeholder until grad.cuh lands -------------------------------------------------------------------------------
-int mipwa_nll_grad(mipwa_ctx* c, const double*, int64_t, double*, double*) { return fail(c, MIPWA_ERR_STATE, "not implemented yet"); }
+// ---- A8: gradient on the recompute path ---------------------------------------------------------------------------
+// cell-sorted copy of a point set (keys from the knots only: valid until the next mipwa_set_* on that slot)
+static int ensure_sorted(mipwa_ctx* c, const Slot& src, Slot& dst, bool& valid)
+{
+    if (valid) return MIPWA_OK;
+    free_slot(dst);
+    const int64_t n = src.n;
+    if (n > 0x7fffffffLL) return fail(c, MIPWA_ERR_ARG, "mipwa_nll_grad supports at most 2^31-1 points per set");
+    if (n > 0) {
+        unsigned int* buf = nullptr;                       // keys in, keys out, index in, index out
+        CU(c, cudaMalloc(&buf, (size_t)n * 4 * sizeof(unsigned int)));
+        unsigned int *k0 = buf, *k1 = buf + n, *i0 = buf + 2 * n, *i1 = buf + 3 * n;
+        void* tmp = nullptr;
+        size_t tmp_bytes = 0;
+        int bits = 1;
+        while ((1LL << bits) < (int64_t)(c->N - 1) * (c->N - 1)) ++bits;
+        cudaError_t e = cudaSuccess;
+        k_cell_keys<<<grid_for(c, n, 8), MIPWA_TILE, 0, c->stream>>>(c->model, src.s12, src.s13, n, k0, i0);
+        ++c->launches;
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, k0, k1, i0, i1, (int)n, 0, bits, c->stream);
+        if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 16);
+        if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k0, k1, i0, i1, (int)n, 0, bits, c->stream);
+        for (int q = 0; q < 3 && e == cudaSuccess; ++q)
+            if (q < 2 || src.w) e = cudaMalloc(&dst.owned[q], (size_t)n * sizeof(double));
+        if (e == cudaSuccess) {
+            k_gather<<<grid_for(c, n, 8), MIPWA_TILE, 0, c->stream>>>(i1, n, src.s12, src.s13, src.w, (double*)dst.owned[0],
+                                                                      (double*)dst.owned[1], (double*)dst.owned[2]);
+            ++c->launches;
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (tmp) cudaFree(tmp);
+        cudaFree(buf);
+        if (e != cudaSuccess) {
+            free_slot(dst);
+            return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, std::string("cell sort: ") + cudaGetErrorString(e));
+        }
+        dst.s12 = (const double*)dst.owned[0]; dst.s13 = (const double*)dst.owned[1]; dst.w = (const double*)dst.owned[2];
+    }
+    dst.n = n;
+    valid = true;
+    return MIPWA_OK;
+}
+
+int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+{
+    if (!c || !params || !nll || !grad) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    rc = ensure_sorted(c, c->ev, c->ev_sorted, c->ev_sorted_valid);
+    if (rc) return rc;
+    rc = ensure_sorted(c, c->nm, c->nm_sorted, c->nm_sorted_valid);
+    if (rc) return rc;
+
+    const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
+    const size_t smem = (size_t)2 * nb * sizeof(double);
+    if (!c->grad_blocks_per_sm) {
+        bool ok = true;
+        MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
+                           ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->grad_blocks_per_sm, k_grad_recompute<R1, R2>,
+                                                                              MIPWA_BLOCK, smem) == cudaSuccess);
+        if (!ok) return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
+        if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
+    }
+    const int grid = c->sm_count * c->grad_blocks_per_sm;
+    if (c->gpartials_len < (size_t)grid * NV) {
+        if (c->d_gpartials) cudaFree(c->d_gpartials);
+        c->d_gpartials = nullptr; c->gpartials_len = 0;
+        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NV * sizeof(double)));
+        c->gpartials_len = (size_t)grid * NV;
+    }
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
+                       (k_grad_recompute<R1, R2><<<grid, MIPWA_BLOCK, smem, c->stream>>>(
+                           c->model, c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.n, c->nm_sorted.s12, c->nm_sorted.s13,
+                           c->nm_sorted.w, c->nm_sorted.n, c->d_gpartials, c->d_ticket, c->d_result)));
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+
+    // ---- host: O(N + R) combine (A7) and adjoint of the coefficient maps ----------------------------------------------
+    const double* h = c->h_result;
+    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;          // w == NULL: kernel used weight 1
+    const double S = h[0], I = h[1] * wn;
+    const double n_ev = (double)c->ev.n;
+    *nll = -S + n_ev * std::log(I);
+    const double scale = c->ev.n > 0 ? 2.0 * n_ev / I * wn : 0.0;
+    const double* Fe = h + 2;
+    const double* Fn = h + 2 + 2 * R;
+    const double* Be = h + 2 + 4 * R;
+    const double* Bn = Be + nb;
+    std::vector<double> gy(2 * N, 0.0), gP(2 * N, 0.0);               // interleaved re, im
+    for (int j = 0; j < NS; ++j) {
+        const double hj = c->knots[j + 1] - c->knots[j];
+        for (int q = 0; q < 2; ++q) {                                  // re, im
+            const double G0 = Be[(0 * NS + j) * 2 + q] + scale * Bn[(0 * NS + j) * 2 + q];
+            const double G1 = Be[(1 * NS + j) * 2 + q] + scale * Bn[(1 * NS + j) * 2 + q];
+            const double G2 = Be[(2 * NS + j) * 2 + q] + scale * Bn[(2 * NS + j) * 2 + q];
+            const double G3 = Be[(3 * NS + j) * 2 + q] + scale * Bn[(3 * NS + j) * 2 + q];
+            // sc0 = y_j; sc1 = (y_j+1 - y_j)/h - h (2 P_j + P_j+1)/6; sc2 = P_j/2; sc3 = (P_j+1 - P_j)/(6h)
+            gy[2 * j + q] += G0 - G1 / hj;
+            gy[2 * (j + 1) + q] += G1 / hj;
+            gP[2 * j + q] += -G1 * hj / 3.0 + 0.5 * G2 - G3 / (6.0 * hj);
+            gP[2 * (j + 1) + q] += -G1 * hj / 6.0 + G3 / (6.0 * hj);
+        }
+    }
+    for (int k = 0; k < N; ++k) {
+        double gr = gy[2 * k], gi = gy[2 * k + 1];
+        for (int j = 0; j < N; ++j) {                                  // + Mx^T g_P  (P = Mx y)
+            const double mjk = c->Mx[(size_t)j * N + k];
+            gr += mjk * gP[2 * j]; gi += mjk * gP[2 * j + 1];
+        }
+        const double ph = params[N + k];
+        grad[k] = gr * std::cos(ph) + gi * std::sin(ph);               // Re(calG e^{-i phi})
+        grad[N + k] = -gr * c->y_im[k] + gi * c->y_re[k];              // Re(calG conj(i y_k))
+    }
+    for (int d = 0; d < R; ++d) {
+        const int r = c->perm[d];
+        const double gr = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
+        const double gi = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
+        const double mag = params[2 * N + 2 * r], th = params[2 * N + 2 * r + 1];
+        grad[2 * N + 2 * r] = gr * std::cos(th) + gi * std::sin(th);
+        grad[2 * N + 2 * r + 1] = mag * (-gr * std::sin(th) + gi * std::cos(th));
+    }
+    return MIPWA_OK;
+}
 
 }  // extern "C"

@@ -1,0 +1,115 @@
+"""GPU parity: analytic gradient on the recompute path (k_cell_keys, k_gather, k_grad_recompute) through the C ABI
+against the oracle's O9 gradient (dense cardinal-spline form), which tests/test_oracle_nll.py pins to finite
+differences and to the scale / phase Euler identities.
+
+Tolerance (reading P26): every component within 1e-9 of the LARGEST gradient component.  Each
+component is a sum of n_ev + n_norm terms of mixed sign whose partial sums are O(max component); fp64 summation in a
+different order than the oracle's long-double accumulation leaves ~1e-13 relative to that scale, so 1e-9 is loose
+for arithmetic and still catches any wrong slot, sign or missing term.
+"""
+import numpy as np
+import pytest
+
+from tests.helpers import make_case, nll_tol
+
+pytestmark = pytest.mark.gpu
+
+
+def _lib():
+    from paper_1703_03284_b200 import binding
+    return binding
+
+
+CASES = {
+    0: dict(),
+    1: dict(n_ev=40_000, n_norm=50_000),
+    2: dict(n_ev=30_011, n_norm=20_003),          # non-uniform knots
+    3: dict(n_ev=25_000, n_norm=25_000),          # floating rho(770) shape: gradient over the first 2N + 2R
+    4: dict(n_ev=20_000, n_norm=20_000),          # six resonances (run-time resonance loop)
+}
+
+
+@pytest.fixture(scope="module", params=sorted(CASES))
+def case(request):
+    return make_case(request.param, **CASES[request.param])
+
+
+def _check(got, ref):
+    scale = np.max(np.abs(ref))
+    err = np.max(np.abs(got - ref))
+    assert err <= 1e-9 * scale, (err, scale, int(np.argmax(np.abs(got - ref))))
+
+
+def test_gradient_matches_oracle(case):
+    c, o, data = case
+    B = _lib()
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], data[4])
+    m.set_path(B.PATH_RECOMPUTE)
+    for t in range(2):
+        p = c.perturbed(t)
+        ref_nll, ref_g = o.nll_grad(p, *data)
+        nll, g = m.nll_grad(p)
+        assert g.shape == (2 * c.N + 2 * c.R,)
+        _, sl, integ = o.nll(p, *data, parts=True)
+        assert abs(nll - ref_nll) <= nll_tol(ref_nll, sl, integ, data[0].size)
+        _check(g, ref_g)
+        assert abs(nll - m.nll(p)) <= nll_tol(ref_nll, sl, integ, data[0].size)      # value path agrees
+    m.close()
+
+
+def test_gradient_invariances_and_uniform_weights(case):
+    """Euler identities (scale and global phase leave the NLL unchanged) hold for the GPU gradient itself."""
+    c, o, data = case
+    if c.idx not in (1, 3):
+        pytest.skip("covered on two configs")
+    B = _lib()
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], None)         # w = NULL -> 1/n
+    p = c.perturbed(3)
+    _, g = m.nll_grad(p)
+    N, R = c.N, c.R
+    mags = np.concatenate([p[:N], p[2 * N:2 * N + 2 * R:2]])
+    gm = np.concatenate([g[:N], g[2 * N:2 * N + 2 * R:2]])
+    gph = np.concatenate([g[N:2 * N], g[2 * N + 1:2 * N + 2 * R:2]])
+    scale = np.max(np.abs(g))
+    assert abs(np.dot(mags, gm)) <= 1e-9 * scale * mags.size
+    assert abs(np.sum(gph)) <= 1e-9 * scale * mags.size
+    _, ref_g = o.nll_grad(p, data[0], data[1], data[2], data[3], None)
+    _check(g, ref_g)
+    m.close()
+
+
+def test_gradient_edge_cases():
+    B = _lib()
+    c, o, (e12, e13, g12, g13, w) = make_case(0, n_ev=700, n_norm=300)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    with pytest.raises(B.MipwaError) as ei:
+        m.nll_grad(c.truth)
+    assert ei.value.code == B.ERR_STATE
+    m.set_norm_points(g12, g13, w)
+    for n in (1, 31, 33, 700):                    # fewer points than warps in the grid; ragged chunks
+        m.set_events(e12[:n], e13[:n])
+        ref_nll, ref_g = o.nll_grad(c.truth, e12[:n], e13[:n], g12, g13, w)
+        nll, g = m.nll_grad(c.truth)
+        assert nll == pytest.approx(ref_nll, rel=1e-10)
+        _check(g, ref_g)
+    # a new event set must invalidate the sorted copy
+    m.set_events(e12[100:400], e13[100:400])
+    _, ref_g = o.nll_grad(c.truth, e12[100:400], e13[100:400], g12, g13, w)
+    _check(m.nll_grad(c.truth)[1], ref_g)
+    # empty sample: NLL = 0 and a zero gradient
+    m.set_events(np.empty(0), np.empty(0))
+    nll, g = m.nll_grad(c.truth)
+    assert nll == 0.0 and np.all(g == 0.0)
+    m.close()
+    # pure S-wave model (R = 0) and N = 2 knots
+    from oracle import oracle as orc
+    knots = np.array([0.05, 3.1])
+    o2 = orc.Oracle(c.kin, knots, [])
+    m2 = B.Mipwa(c.kin, knots, [])
+    m2.set_events(e12, e13); m2.set_norm_points(g12, g13, w)
+    p2 = np.array([1.1, 0.7, 0.2, 1.9])
+    _, ref_g = o2.nll_grad(p2, e12, e13, g12, g13, w)
+    _check(m2.nll_grad(p2)[1], ref_g)
+    m2.close()
