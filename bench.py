@@ -32,15 +32,17 @@ METRIC = "MIPWA NLL events/s (full recompute, 10M events + 10M normalisation poi
 UNIT = "events/s"
 
 
-# ---- algorithmic work per point: flops of the restated formulas, fma = 2, rcp/rsqrt = 1 + their
-# refinement; nothing padded, the log-product trick and shared sub-expressions already taken out -------------------
+# ---- algorithmic work per point: flops of the plain formulas, one per add / mul /
+# div / sqrt / log, fma = 2: two channels x [10 shared kinematics + 14 spline + 37 R] + 4, plus 2 (1 + 3R) divisions,
+# 2 (2 + R) square roots and one log = 59 + 82 R (305 at R = 3).  The kernel as built executes 297 (ncu-counted
+# dadd + dmul + 2 dfma per point, profiles/r1_recompute_ncu.md), so nothing is padded. -------------------------------
 def flops_per_point(resonances):
-    per_channel = 36 + 15                       # kinematics shared by all resonances + spline (index, Horner)
-    per_res_channel = {0: 20, 1: 27, 2: 32}
-    f = 2 * per_channel + 2 + 3 + 1             # two channels, S12+S13, |A|^2, product / weight
-    for r in resonances:
-        f += 2 * per_res_channel[r["spin"]] + 10
-    return f
+    return 59 + 82 * len(resonances)
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per k_nll_recompute launch at the bench size (10M events + 10M weighted
+# normalisation points), from the one `ncu --set full` capture summarised in profiles/r1_recompute_ncu.md
+NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 404.4e6}
 
 
 class ClockSampler:
@@ -233,6 +235,57 @@ def run_ours(args, cfg, workload):
         step(params[args.warmup + t])
     fit_step_s = (time.perf_counter() - t0) / args.steps
 
+    # ---- A8: value + analytic gradient (BASELINE configs[3]: "plus analytic gradient w.r.t. all 2N+2*3 parameters") ----
+    sub_steps = max(3, min(args.steps, 30))
+    m.nll_grad(params[0])                             # builds the cell-sorted copies (once per point set)
+    t0 = time.perf_counter(); m.set_events(d[0], d[1]); m.nll_grad(params[0]); t_sort = time.perf_counter() - t0
+    for t in range(3):
+        m.nll_grad(params[t])
+    grad_ms = []
+    barrier()
+    t0 = time.perf_counter()
+    for t in range(sub_steps):
+        nll_g, grad = m.nll_grad(params[args.warmup + t % args.steps])
+        grad_ms.append(m.last_kernel_ms())
+    barrier()
+    grad_wall = (time.perf_counter() - t0) / sub_steps
+    grad_info = {"ms_per_call": 1e3 * grad_wall, "kernel_ms": float(np.mean(grad_ms)),
+                 "events_per_s": n_ev * world / grad_wall, "n_grad": int(grad.size), "nll": nll_g,
+                 "first_call_s": t_sort, "what": "mipwa_nll_grad: NLL + d/d(a_k, phi_k, |c_r|, arg c_r), same sample, "
+                 "k_grad_recompute on cell-sorted points; first_call_s includes the one-off sort"}
+
+    # ---- A9/A10: fixed-shape cached paths on the SAME events (all shapes fixed at their listed values) ------------------
+    cached_info = {}
+    fixed = [dict(r, shape_floats=0) for r in cfg.resonances]
+    mc = B.Mipwa(cfg.kin, cfg.knots, fixed, device=local)
+    mc.set_stream(stream)
+    mc.set_events(d[0], d[1]); mc.set_norm_points(d[2], d[3], d[4])
+    mc.enable_timing(True)
+    pc = [p[:2 * cfg.N + 2 * cfg.R] for p in params]
+    for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT)):
+        mc.set_path(path)
+        t0 = time.perf_counter(); mc.nll(pc[0]); setup_s = time.perf_counter() - t0
+        for t in range(3):
+            mc.nll(pc[t])
+        kms = []
+        barrier()
+        t0 = time.perf_counter()
+        for t in range(sub_steps):
+            nll_c = mc.nll(pc[args.warmup + t % args.steps])
+            kms.append(mc.last_kernel_ms())
+        barrier()
+        wall = (time.perf_counter() - t0) / sub_steps
+        nbytes = mc.basis_bytes()
+        k = float(np.mean(kms))
+        cached_info[name] = {"ms_per_call": 1e3 * wall, "kernel_ms": k, "events_per_s": n_ev * world / wall,
+                             "bytes_per_event": nbytes / max(n_ev, 1), "cache_bytes": nbytes,
+                             "first_call_s": setup_s, "nll": nll_c,
+                             "roofline": {"bound": "hbm", "kernel": "k_nll_dense" if name == "dense" else "k_nll_compact",
+                                          "achieved": nbytes / (k * 1e-3) * 1e-9, "unit": "GB/s", "traffic": None}}
+    mc.set_path(B.PATH_RECOMPUTE)
+    cached_info["recompute_same_model_nll"] = mc.nll(pc[args.warmup + (sub_steps - 1) % args.steps])
+    mc.close()
+
     if rank == 0:
         time.sleep(0.2)
         sampler.stop()
@@ -243,7 +296,7 @@ def run_ours(args, cfg, workload):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (k_nll_recompute): plain FP64 ALU work ----------------------------------
+    # ---- roofline of the dominant kernel of the step (k_nll_recompute): plain FP64 ALU work -----------------------------
     peak = B.measure_fp64_peak(local, 2.0)
     fl = flops_per_point(cfg.resonances) * (n_ev + n_norm)
     k_ms = float(np.mean(kernel_ms))
@@ -252,16 +305,28 @@ def run_ours(args, cfg, workload):
     if clocks and clocks.get("sm_max_mhz"):
         nominal = 148 * 64 * 2 * clocks["sm_max_mhz"] * 1e6 * 1e-12
     roofline = {"bound": "alu", "kernel": "k_nll_recompute", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": None,
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((n_ev, n_norm)),
+                "traffic_source": "profiles/r1_recompute_ncu.md (ncu --set full, bytes per launch); algorithmic bytes "
+                                  "per launch = 16 B x events + 24 B x weighted normalisation points",
                 "peak_source": "measured on this GPU by mipwa_measure_fp64_peak (register-resident DFMA, 2 s sustained); "
-                               "MEASURED_PEAKS.json has no FP64 entry",
+                               "MEASURED_PEAKS.json has no FP64 entry; DESIGN.md section 6 derives the nominal peak",
                 "nominal_peak": nominal, "flops_per_point": flops_per_point(cfg.resonances),
                 "points_per_launch": n_ev + n_norm, "kernel_ms": k_ms,
-                "hbm_gbs": 16.0 * (n_ev + n_norm) / (k_ms * 1e-3) * 1e-9}
+                "algorithmic_bytes": 16.0 * n_ev + 24.0 * n_norm,
+                "hbm_gbs": (16.0 * n_ev + 24.0 * n_norm) / (k_ms * 1e-3) * 1e-9}
+    hbm_peak, hbm_src = 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            hbm_peak, hbm_src = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (copy, read+write)"
+    except (OSError, KeyError, ValueError):
+        pass
+    for name in ("dense", "compact"):
+        r = cached_info[name]["roofline"]
+        r.update(peak=hbm_peak, frac=r["achieved"] / hbm_peak, peak_source=hbm_src)
 
     cpu = None
     if world == 1:
-        cpu = time_oracle(cfg, min(n_ev, 2_000_000), min(n_norm, 2_000_000), 2, 1)
+        cpu = time_oracle(cfg, min(n_ev, 4_000_000), min(n_norm, 4_000_000), 3, 1)
 
     total_events = n_ev * world
     line = {"metric": METRIC, "value": total_events / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
@@ -277,7 +342,7 @@ def run_ours(args, cfg, workload):
                     "what": "mipwa_set_events + mipwa_set_norm_points from pinned HOST arrays + mipwa_nll, every step"},
             "fit_step": {"ms_per_call": 1e3 * fit_step_s, "nll_evals_per_s": 1.0 / fit_step_s,
                          "what": "wall clock of mipwa_nll(host params) -> host fp64 with events resident (what a minimiser sees)"},
-            "roofline": roofline, "cpu_baseline": cpu, "input_generation_s": t_gen, "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
+            "roofline": roofline, "grad": grad_info, "cached": cached_info, "cpu_baseline": cpu, "input_generation_s": t_gen, "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -286,7 +351,7 @@ def run_ours(args, cfg, workload):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
