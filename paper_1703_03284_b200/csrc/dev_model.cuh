@@ -39,7 +39,7 @@ struct DevModel {
     int32_t N;                 // knots
     int32_t R;                 // resonances
     int32_t nlut;              // buckets in lut
-    int32_t pad0;
+    int32_t lut_exact;         // 1: every bucket holds at most one knot (xk), so the segment needs no search
     double t_lo, t_d;          // (m1+m2)^2, (m1-m2)^2
     double s_hi, s_top;        // (M-m3)^2, (M+m3)^2
     double sigma;              // M^2 + m1^2 + m2^2 + m3^2
@@ -48,6 +48,7 @@ struct DevModel {
     double knots[MIPWA_DEV_MAX_KNOTS];
     double2 sc[4][MIPWA_DEV_MAX_KNOTS];   // segment j: S(s) = sc[0][j] + t(sc[1][j] + t(sc[2][j] + t sc[3][j])), t = s - x_j
     uint8_t lut[MIPWA_DEV_LUT];           // segment that contains the left edge of each bucket
+    double xk[MIPWA_DEV_LUT];             // the interior knot inside bucket b (+inf if none); valid iff lut_exact
     ResDev res[MIPWA_DEV_MAX_RES];
 };
 
@@ -56,6 +57,7 @@ struct SplineSmem {
     double knots[MIPWA_DEV_MAX_KNOTS];
     double2 sc[4][MIPWA_DEV_MAX_KNOTS];
     uint8_t lut[MIPWA_DEV_LUT];
+    double xk[MIPWA_DEV_LUT];
 };
 
 __device__ __forceinline__ void load_spline_smem(SplineSmem& sm, const DevModel& m)
@@ -64,7 +66,7 @@ __device__ __forceinline__ void load_spline_smem(SplineSmem& sm, const DevModel&
         sm.knots[i] = m.knots[i];
         sm.sc[0][i] = m.sc[0][i]; sm.sc[1][i] = m.sc[1][i]; sm.sc[2][i] = m.sc[2][i]; sm.sc[3][i] = m.sc[3][i];
     }
-    for (int i = threadIdx.x; i < m.nlut; i += blockDim.x) sm.lut[i] = m.lut[i];
+    for (int i = threadIdx.x; i < m.nlut; i += blockDim.x) { sm.lut[i] = m.lut[i]; sm.xk[i] = m.xk[i]; }
     __syncthreads();
 }
 
@@ -90,12 +92,22 @@ __device__ __forceinline__ double fast_rsqrt(double x)
     return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
-// segment index j with x_j <= s < x_{j+1}, clamped to [0, N-2] (beyond the end knots the end cubic is used)
+// segment index j with x_j <= s < x_{j+1}, clamped to [0, N-2] (beyond the end knots the end cubic is used).
+// Buckets are narrower than the smallest knot spacing (lut_exact), so one compare against the single knot a bucket
+// can hold replaces a search: two dependent shared-memory reads (bucket entry, then the segment's row) and no branch.
+// A point within rounding of a bucket edge or a knot may land in the neighbouring segment; the spline is C^2, so
+// the neighbouring cubic differs there by O(distance^3) - far below one ulp.  Knot tables too dense for the
+// MIPWA_DEV_LUT buckets fall back to the search.
 __device__ __forceinline__ int spline_segment(const SplineSmem& sm, const DevModel& m, double s, double& xj)
 {
     int b = __double2int_rd((s - m.lut_x0) * m.lut_inv);
     b = max(0, min(b, m.nlut - 1));
     int j = sm.lut[b];
+    if (m.lut_exact) {
+        j += s >= sm.xk[b] ? 1 : 0;
+        xj = sm.knots[j];
+        return j;
+    }
     xj = sm.knots[j];
     double xn = sm.knots[j + 1];
     while (s >= xn && j < m.N - 2) { ++j; xj = xn; xn = sm.knots[j + 1]; }
@@ -223,6 +235,40 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
         for (int r = 0; r < R2; ++r) add_resonance<2>(m.res[R1 + r], ca, cb, are, aim);
     } else {
         for (int r = 0; r < m.R; ++r) add_resonance<-1>(m.res[r], ca, cb, are, aim);
+    }
+}
+
+// One channel of one point (the "half-point" mapping: lane 2k evaluates the s12 channel of a point, lane 2k+1 its
+// s13 channel): P(x, y) = S(x) + sum_r c_r T_r(x, y), so that A(s12,s13) = P(s12,s13) + P(s13,s12).
+template <int R1, int R2>
+__device__ __forceinline__ void amplitude_half(const SplineSmem& sm, const DevModel& m, double x, double y,
+                                               double& pre, double& pim)
+{
+    spline_eval(sm, m, x, pre, pim);
+    if (R1 == 0 && R2 == 0) return;
+    const Channel c = make_channel(m, x, y);
+    if (R1 >= 0) {
+#pragma unroll
+        for (int r = 0; r < R1; ++r) {
+            double tr, ti;
+            resonance_channel<1>(m.res[r], c, tr, ti);
+            pre = fma(m.res[r].cre, tr, fma(-m.res[r].cim, ti, pre));
+            pim = fma(m.res[r].cre, ti, fma(m.res[r].cim, tr, pim));
+        }
+#pragma unroll
+        for (int r = 0; r < R2; ++r) {
+            double tr, ti;
+            resonance_channel<2>(m.res[R1 + r], c, tr, ti);
+            pre = fma(m.res[R1 + r].cre, tr, fma(-m.res[R1 + r].cim, ti, pre));
+            pim = fma(m.res[R1 + r].cre, ti, fma(m.res[R1 + r].cim, tr, pim));
+        }
+    } else {
+        for (int r = 0; r < m.R; ++r) {
+            double tr, ti;
+            resonance_channel<-1>(m.res[r], c, tr, ti);
+            pre = fma(m.res[r].cre, tr, fma(-m.res[r].cim, ti, pre));
+            pim = fma(m.res[r].cre, ti, fma(m.res[r].cim, tr, pim));
+        }
     }
 }
 

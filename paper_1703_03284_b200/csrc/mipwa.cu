@@ -46,6 +46,8 @@ struct mipwa_ctx {
     // natural-spline system (A2): the tridiagonal matrix depends on the knots only -> factor once
     std::vector<double> sp_sub, sp_inv, sp_cp;     // sub-diagonal, 1/pivot, modified super-diagonal
     std::vector<uint8_t> lut;
+    std::vector<double> xk;
+    bool lut_exact = false;
     int nlut = 0;
     double lut_x0 = 0, lut_inv = 0;
 
@@ -169,16 +171,24 @@ void spline_factor(mipwa_ctx* c)
         c->sp_inv[i] = 1.0 / piv;
         c->sp_cp[i] = sup / piv;
     }
-    // bucket table for the segment search: lut[b] = segment containing the left edge of bucket b
-    c->nlut = std::min(MIPWA_DEV_LUT, std::max(64, 4 * n));
+    // bucket table for the segment lookup: lut[b] = segment containing the left edge of bucket b, xk[b] = the
+    // interior knot inside bucket b.  Buckets no wider than 0.9 x the smallest knot spacing hold at most one knot.
+    double minsp = x[1] - x[0];
+    for (int i = 1; i < n - 1; ++i) minsp = std::min(minsp, x[i + 1] - x[i]);
+    const double range = x[n - 1] - x[0];
+    const double want = std::ceil(range / (0.9 * minsp));
+    c->nlut = (int)std::min<double>(MIPWA_DEV_LUT, std::max<double>(64.0, want));
+    c->lut_exact = range / c->nlut <= 0.9 * minsp;
     c->lut_x0 = x[0];
-    c->lut_inv = c->nlut / (x[n - 1] - x[0]);
+    c->lut_inv = c->nlut / range;
     c->lut.assign(c->nlut, 0);
+    c->xk.assign(c->nlut, HUGE_VAL);
     for (int b = 0; b < c->nlut; ++b) {
-        const double edge = x[0] + b / c->lut_inv;
+        const double lo = x[0] + b / c->lut_inv, hi = x[0] + (b + 1) / c->lut_inv;
         int j = 0;
-        while (j < n - 2 && edge >= x[j + 1]) ++j;
+        while (j < n - 2 && lo >= x[j + 1]) ++j;
         c->lut[b] = (uint8_t)j;
+        if (j + 1 <= n - 2 && x[j + 1] < hi) c->xk[b] = x[j + 1];
     }
 }
 
@@ -192,7 +202,7 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
         if (!std::isfinite(p[i])) return fail(c, MIPWA_ERR_ARG, "non-finite parameter " + std::to_string(i));
     DevModel& m = c->model;
     const mipwa_kinematics& k = c->kin;
-    m.N = N; m.R = R; m.nlut = c->nlut; m.pad0 = 0;
+    m.N = N; m.R = R; m.nlut = c->nlut; m.lut_exact = c->lut_exact ? 1 : 0;
     m.t_lo = (k.m1 + k.m2) * (k.m1 + k.m2);
     m.t_d = (k.m1 - k.m2) * (k.m1 - k.m2);
     m.s_hi = (k.m_parent - k.m3) * (k.m_parent - k.m3);
@@ -201,6 +211,7 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
     m.kappa = (k.m_parent * k.m_parent - k.m3 * k.m3) * (k.m2 * k.m2 - k.m1 * k.m1);
     m.lut_x0 = c->lut_x0; m.lut_inv = c->lut_inv;
     std::memcpy(m.lut, c->lut.data(), c->nlut);
+    std::memcpy(m.xk, c->xk.data(), c->nlut * sizeof(double));
     for (int i = 0; i < N; ++i) {
         m.knots[i] = c->knots[i];
         c->y_re[i] = p[i] * std::cos(p[N + i]);            // y_k = a_k e^{i phi_k}
