@@ -7,7 +7,7 @@
 #define MIPWA_BLOCK 256
 #endif
 #ifndef MIPWA_MINBLOCKS
-#define MIPWA_MINBLOCKS 2
+#define MIPWA_MINBLOCKS 3
 #endif
 #ifndef MIPWA_HALF
 #define MIPWA_HALF 0

@@ -1,0 +1,69 @@
+"""Multi-GPU host logic on CPU (gloo, world_size 2): the per-rank partial sums of a sharded likelihood combine to the
+single-process NLL.  The per-rank partials come from the ORACLE here (no GPU in this suite); on GPUs
+bench.py feeds the same helper with the partials of mipwa_nll_parts."""
+import os
+import socket
+
+import numpy as np
+import torch.multiprocessing as mp
+
+from paper_1703_03284_b200 import sharding
+
+
+def test_shard_range_partitions_exactly():
+    for n in (0, 1, 7, 100, 1_000_003):
+        for world in (1, 2, 3, 8):
+            cuts = [sharding.shard_range(n, r, world) for r in range(world)]
+            assert cuts[0][0] == 0 and cuts[-1][1] == n
+            assert all(cuts[r][1] == cuts[r + 1][0] for r in range(world - 1))
+            sizes = [hi - lo for lo, hi in cuts]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    c = I.Config(1, n_ev=4001, n_norm=3001)
+    o = orc.Oracle(c.kin, c.knots, c.resonances)
+    g12, g13, w = c.norm_points()                      # weights of the WHOLE sample (Area / n_norm)
+    e12, e13 = I.phase_space_points(c.n_ev, c.key(I.S_EVENTS))
+    p = c.perturbed(1)
+    full = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    lo, hi = sharding.shard_range(c.n_ev, rank, world)
+    glo, ghi = sharding.shard_range(g12.size, rank, world)
+    _, S, Iv = o.nll(p, e12[lo:hi], e13[lo:hi], g12[glo:ghi], g13[glo:ghi], w[glo:ghi], parts=True)
+    nll, St, It, nt = sharding.combine_parts(S, Iv, hi - lo)
+    q.put((rank, nll, St, It, nt, full))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_combine_matches_single_process():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = [q.get(timeout=240) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    nlls = set()
+    for rank, nll, St, It, nt, (full, fS, fI) in out:
+        assert nt == 4001
+        assert abs(St - fS) <= 1e-11 * abs(fS) and abs(It - fI) <= 1e-12 * abs(fI)
+        assert abs(nll - full) <= 1e-10 * max(abs(full), abs(fS) + nt * abs(np.log(fI)))
+        nlls.add(nll)
+    assert len(nlls) == 1                              # every rank forms the same bits (rank-ordered sum)
+
+
+def test_combine_without_process_group_is_step_a7():
+    nll, S, Iv, n = sharding.combine_parts(12.5, 3.0, 7)
+    assert (S, Iv, n) == (12.5, 3.0, 7) and nll == -12.5 + 7 * np.log(3.0)
