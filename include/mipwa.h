@@ -87,6 +87,14 @@ int mipwa_set_events(mipwa_ctx* ctx, const double* s12, const double* s13, int64
 int mipwa_set_norm_points(mipwa_ctx* ctx, const double* s12, const double* s13, const double* w, int64_t n,
                           int32_t mem);
 
+/* Optional, once per point set, for fits that evaluate the same sample many times ("in each fit
+ * iteration"): makes library-owned copies of the current events and normalisation points SORTED BY SPLINE CELL
+ * (segment of s12, segment of s13; +16 B per event, +16/24 B per normalisation point).  Every kernel then reads
+ * the copies: all lanes of a warp look up the same spline segment, so the shared-memory table reads become
+ * broadcasts.  Results change only by summation order.  The test hooks keep the caller's order.  Undone for a slot
+ * by the next mipwa_set_* on it; implied by mipwa_nll_grad.  Errors: MIPWA_ERR_STATE before both mipwa_set_*. */
+int mipwa_prepare(mipwa_ctx* ctx);
+
 /* Length of the parameter vector: 2N + 2R + 2F (F = resonances with shape_floats). */
 int mipwa_n_params(const mipwa_ctx* ctx, int64_t* n);
 

@@ -22,7 +22,7 @@ _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STAT
 
 # every symbol include/mipwa.h declares
 SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
-           "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
+           "mipwa_prepare", "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
            "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version"]
@@ -63,6 +63,7 @@ def load_library():
     L.mipwa_set_stream.restype = i32; L.mipwa_set_stream.argtypes = [vp, vp]
     L.mipwa_set_events.restype = i32; L.mipwa_set_events.argtypes = [vp, vp, vp, i64, i32]
     L.mipwa_set_norm_points.restype = i32; L.mipwa_set_norm_points.argtypes = [vp, vp, vp, vp, i64, i32]
+    L.mipwa_prepare.restype = i32; L.mipwa_prepare.argtypes = [vp]
     L.mipwa_n_params.restype = i32; L.mipwa_n_params.argtypes = [vp, C.POINTER(i64)]
     L.mipwa_set_path.restype = i32; L.mipwa_set_path.argtypes = [vp, i32]
     L.mipwa_basis_bytes.restype = i64; L.mipwa_basis_bytes.argtypes = [vp]
@@ -175,6 +176,9 @@ class Mipwa:
     def set_norm_points(self, s12, s13, w=None):
         self.n_norm = -1
         self.n_norm = self._set(self.L.mipwa_set_norm_points, "nm", [s12, s13, w], True)
+
+    def prepare(self):
+        self._check(self.L.mipwa_prepare(self._h))
 
     def set_path(self, path):
         self._check(self.L.mipwa_set_path(self._h, int(path)))

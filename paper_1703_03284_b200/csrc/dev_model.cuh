@@ -238,40 +238,6 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
     }
 }
 
-// One channel of one point (the "half-point" mapping: lane 2k evaluates the s12 channel of a point, lane 2k+1 its
-// s13 channel): P(x, y) = S(x) + sum_r c_r T_r(x, y), so that A(s12,s13) = P(s12,s13) + P(s13,s12).
-template <int R1, int R2>
-__device__ __forceinline__ void amplitude_half(const SplineSmem& sm, const DevModel& m, double x, double y,
-                                               double& pre, double& pim)
-{
-    spline_eval(sm, m, x, pre, pim);
-    if (R1 == 0 && R2 == 0) return;
-    const Channel c = make_channel(m, x, y);
-    if (R1 >= 0) {
-#pragma unroll
-        for (int r = 0; r < R1; ++r) {
-            double tr, ti;
-            resonance_channel<1>(m.res[r], c, tr, ti);
-            pre = fma(m.res[r].cre, tr, fma(-m.res[r].cim, ti, pre));
-            pim = fma(m.res[r].cre, ti, fma(m.res[r].cim, tr, pim));
-        }
-#pragma unroll
-        for (int r = 0; r < R2; ++r) {
-            double tr, ti;
-            resonance_channel<2>(m.res[R1 + r], c, tr, ti);
-            pre = fma(m.res[R1 + r].cre, tr, fma(-m.res[R1 + r].cim, ti, pre));
-            pim = fma(m.res[R1 + r].cre, ti, fma(m.res[R1 + r].cim, tr, pim));
-        }
-    } else {
-        for (int r = 0; r < m.R; ++r) {
-            double tr, ti;
-            resonance_channel<-1>(m.res[r], c, tr, ti);
-            pre = fma(m.res[r].cre, tr, fma(-m.res[r].cim, ti, pre));
-            pim = fma(m.res[r].cre, ti, fma(m.res[r].cim, tr, pim));
-        }
-    }
-}
-
 #define MIPWA_SIG_MAX1 4
 #define MIPWA_SIG_MAX2 2
 // run CALL with constexpr R1, R2 matching the model signature (n0, n1, n2 = resonances of spin 0, 1, 2)

@@ -230,27 +230,27 @@ k_grad_recompute(const __grid_constant__ DevModel m,
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) grad_bins[k] = 0.0;
     load_spline_smem(sm, m);                               // ends with __syncthreads()
 
-    double S = 0.0, I = 0.0, Fer[RR], Fei[RR], Fnr[RR], Fni[RR];
-#pragma unroll
-    for (int r = 0; r < RR; ++r) Fer[r] = Fei[r] = Fnr[r] = Fni[r] = 0.0;
-    grad_pass<R1, R2, true>(sm, m, e12, e13, nullptr, n_ev, grad_bins, S, Fer, Fei);
-    grad_pass<R1, R2, false>(sm, m, g12, g13, gw, n_norm, grad_bins + nb, I, Fnr, Fni);
-
     double* mine = partials + (size_t)blockIdx.x * NV;
-    double v = block_sum(S, red32);
-    if (threadIdx.x == 0) mine[0] = v;
-    v = block_sum(I, red32);
-    if (threadIdx.x == 0) mine[1] = v;
-    for (int r = 0; r < R; ++r) {
-        double a = 0, b = 0, c = 0, d = 0;
-        if (R1 >= 0) {
+    // events pass, then its scalars are reduced and stored before the second pass so that only one set of resonance
+    // accumulators is live at a time (register pressure)
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        double Sc = 0.0, Fr[RR], Fi[RR];
 #pragma unroll
-            for (int q = 0; q < RR; ++q) if (q == r) { a = Fer[q]; b = Fei[q]; c = Fnr[q]; d = Fni[q]; }
-        } else { a = Fer[r]; b = Fei[r]; c = Fnr[r]; d = Fni[r]; }
-        a = block_sum(a, red32); if (threadIdx.x == 0) mine[2 + 2 * r] = a;
-        b = block_sum(b, red32); if (threadIdx.x == 0) mine[2 + 2 * r + 1] = b;
-        c = block_sum(c, red32); if (threadIdx.x == 0) mine[2 + 2 * R + 2 * r] = c;
-        d = block_sum(d, red32); if (threadIdx.x == 0) mine[2 + 2 * R + 2 * r + 1] = d;
+        for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
+        if (pass == 0) grad_pass<R1, R2, true>(sm, m, e12, e13, nullptr, n_ev, grad_bins, Sc, Fr, Fi);
+        else grad_pass<R1, R2, false>(sm, m, g12, g13, gw, n_norm, grad_bins + nb, Sc, Fr, Fi);
+        double v = block_sum(Sc, red32);
+        if (threadIdx.x == 0) mine[pass] = v;
+        for (int r = 0; r < R; ++r) {
+            double a = 0, b = 0;
+            if (R1 >= 0) {
+#pragma unroll
+                for (int q = 0; q < RR; ++q) if (q == r) { a = Fr[q]; b = Fi[q]; }
+            } else { a = Fr[r]; b = Fi[r]; }
+            a = block_sum(a, red32); if (threadIdx.x == 0) mine[2 + 2 * R * pass + 2 * r] = a;
+            b = block_sum(b, red32); if (threadIdx.x == 0) mine[2 + 2 * R * pass + 2 * r + 1] = b;
+        }
     }
     __syncthreads();                                       // all flushes into grad_bins are done
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) mine[2 + 4 * R + k] = grad_bins[k];

@@ -9,9 +9,6 @@
 #ifndef MIPWA_MINBLOCKS
 #define MIPWA_MINBLOCKS 3
 #endif
-#ifndef MIPWA_HALF
-#define MIPWA_HALF 0
-#endif
 #ifndef MIPWA_PTS
 #define MIPWA_PTS 1
 #endif
@@ -91,42 +88,6 @@ k_nll_recompute(const __grid_constant__ DevModel m,
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
 
-#if MIPWA_HALF
-    // Half-point mapping: lane pair (2k, 2k+1) shares one point, each lane evaluates one channel; the pair exchanges
-    // its partial amplitudes with one shuffle.  Halves the live state per lane (twice the warps per SM for the same
-    // registers).  Loops are warp-uniform (the shuffle needs every lane); out-of-range slots evaluate a harmless point.
-    LogProd lp;
-    double integ = 0.0;
-    {
-        const long long hs = stride >> 1;
-        const bool odd = threadIdx.x & 1;
-        long long i = t0 >> 1, iw = (t0 - (threadIdx.x & 31)) >> 1;
-        double a = 1.0, b = 1.0;
-        if (i < n_ev) { a = e12[i]; b = e13[i]; }
-        for (; iw < n_ev; iw += hs, i += hs) {
-            double na = 1.0, nb = 1.0;
-            if (i + hs < n_ev) { na = e12[i + hs]; nb = e13[i + hs]; }
-            double pre, pim;
-            amplitude_half<R1, R2>(sm, m, odd ? b : a, odd ? a : b, pre, pim);
-            const double re = pre + __shfl_xor_sync(0xffffffffu, pre, 1), im = pim + __shfl_xor_sync(0xffffffffu, pim, 1);
-            lp.add((i < n_ev && !odd) ? fma(re, re, im * im) : 1.0);
-            a = na; b = nb;
-        }
-        i = t0 >> 1; iw = (t0 - (threadIdx.x & 31)) >> 1;
-        a = 1.0; b = 1.0;
-        double w = 0.0;
-        if (i < n_norm) { a = g12[i]; b = g13[i]; w = odd ? 0.0 : (gw ? gw[i] : 1.0); }
-        for (; iw < n_norm; iw += hs, i += hs) {
-            double na = 1.0, nb = 1.0, nw = 0.0;
-            if (i + hs < n_norm) { na = g12[i + hs]; nb = g13[i + hs]; nw = odd ? 0.0 : (gw ? gw[i + hs] : 1.0); }
-            double pre, pim;
-            amplitude_half<R1, R2>(sm, m, odd ? b : a, odd ? a : b, pre, pim);
-            const double re = pre + __shfl_xor_sync(0xffffffffu, pre, 1), im = pim + __shfl_xor_sync(0xffffffffu, pim, 1);
-            integ = fma(w, fma(re, re, im * im), integ);
-            a = na; b = nb; w = nw;
-        }
-    }
-#else
     // PTS points per thread and iteration: independent dependency chains for the FP64 pipe.  Out-of-range slots
     // evaluate a harmless in-range point and contribute ln 1 = 0 (events) or weight 0 (normalisation).
     constexpr int PTS = MIPWA_PTS;
@@ -189,7 +150,6 @@ k_nll_recompute(const __grid_constant__ DevModel m,
         }
     }
 
-#endif
     double v[2] = { lp.value(), integ };
     block_reduce<2>(v, red);
     if (threadIdx.x == 0) {

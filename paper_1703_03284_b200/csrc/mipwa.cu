@@ -266,6 +266,11 @@ void free_slot(Slot& s)
 
 }  // namespace
 
+
+// the library's working view of a point set: the cell-sorted copy once mipwa_prepare / mipwa_nll_grad built it
+static inline const Slot& evs(const mipwa_ctx* c) { return c->ev_sorted_valid ? c->ev_sorted : c->ev; }
+static inline const Slot& nms(const mipwa_ctx* c) { return c->nm_sorted_valid ? c->nm_sorted : c->nm; }
+
 // =================================================================================================================
 // C ABI
 // =================================================================================================================
@@ -468,7 +473,7 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->blocks_per_sm);
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
     MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2], (k_nll_recompute<R1, R2><<<grid, MIPWA_BLOCK, 0, c->stream>>>(
-                               c->model, c->ev.s12, c->ev.s13, c->ev.n, c->nm.s12, c->nm.s13, c->nm.w, c->nm.n,
+                               c->model, evs(c).s12, evs(c).s13, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w, nms(c).n,
                                c->d_partials, c->d_ticket, c->d_result)));
     ++c->launches;
     CU(c, cudaGetLastError());
@@ -541,10 +546,10 @@ static int ensure_cache(mipwa_ctx* c, int kind)
         const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
         const int grid = (int)std::min<int64_t>(tiles, (int64_t)c->sm_count * 8);
         if (kind == MIPWA_PATH_CACHED)
-            k_basis_build<false><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
+            k_basis_build<false><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), evs(c).s12, evs(c).s13,
                                                                       c->ev.n, (double2*)c->d_cache);
         else
-            k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), c->ev.s12, c->ev.s13,
+            k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), evs(c).s12, evs(c).s13,
                                                                      c->ev.n, (double2*)c->d_cache);
         ++c->launches;
         CU(c, cudaGetLastError());
@@ -572,7 +577,7 @@ static int ensure_gram(mipwa_ctx* c)
     do {                                                                                                             \
         e = cudaFuncSetAttribute(k_gram<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                 \
         if (e == cudaSuccess)                                                                                        \
-            k_gram<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), c->nm.s12, c->nm.s13, c->nm.w, \
+            k_gram<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), nms(c).s12, nms(c).s13, nms(c).w, \
                                                               c->nm.n, wd, partial);                                 \
     } while (0)
     if (tpt <= 1) MIPWA_GRAM_LAUNCH(1); else if (tpt == 2) MIPWA_GRAM_LAUNCH(2); else MIPWA_GRAM_LAUNCH(3);
@@ -834,17 +839,38 @@ static int ensure_sorted(mipwa_ctx* c, const Slot& src, Slot& dst, bool& valid)
     return MIPWA_OK;
 }
 
+// cell-sorted copies of both point sets; every kernel then reads them instead of the caller's arrays
+static int prepare_sorted(mipwa_ctx* c)
+{
+    if (c->ev_sorted_valid && c->nm_sorted_valid) return MIPWA_OK;
+    int rc = build_unit_model(c, nullptr);                 // knots and bucket table for k_cell_keys
+    if (rc) return rc;
+    if (!c->ev_sorted_valid) {
+        rc = ensure_sorted(c, c->ev, c->ev_sorted, c->ev_sorted_valid);
+        if (rc) return rc;
+        c->cache_valid = false;                            // the per-event cache follows the event order
+    }
+    return ensure_sorted(c, c->nm, c->nm_sorted, c->nm_sorted_valid);
+}
+
+int mipwa_prepare(mipwa_ctx* c)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    int rc = use_device(c);
+    if (rc) return rc;
+    return prepare_sorted(c);
+}
+
 int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
 {
     if (!c || !params || !nll || !grad) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
     if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
     int rc = use_device(c);
     if (rc) return rc;
+    rc = prepare_sorted(c);
+    if (rc) return rc;
     rc = build_model(c, params, n_params);
-    if (rc) return rc;
-    rc = ensure_sorted(c, c->ev, c->ev_sorted, c->ev_sorted_valid);
-    if (rc) return rc;
-    rc = ensure_sorted(c, c->nm, c->nm_sorted, c->nm_sorted_valid);
     if (rc) return rc;
 
     const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;

@@ -190,3 +190,37 @@ def test_unequal_mass_kinematics():
     ref_n, sl, integ = o.nll(p, g12[:3000], g13[:3000], g12[3000:], g13[3000:], None, parts=True)
     assert abs(m.nll(p) - ref_n) <= nll_tol(ref_n, sl, integ, 3000)
     m.close()
+
+
+def test_prepare_keeps_results_and_hook_order(case):
+    """mipwa_prepare: cell-sorted internal copies change only the summation order; hooks keep the caller's order;
+    a new mipwa_set_* drops the sorted copy of that slot."""
+    c, o, data = case
+    B = _lib()
+    m = _ctx(c, data, device_arrays=(c.idx % 2 == 0))
+    p = c.perturbed(5)
+    ref, sl, integ = o.nll(p, *data, parts=True)
+    tol = nll_tol(ref, sl, integ, data[0].size)
+    before = m.nll(p)
+    m.prepare()
+    after = m.nll(p)
+    assert abs(after - ref) <= tol and abs(before - ref) <= tol
+    assert m.nll(p) == after
+    got = m.eval_abs2(p, 0)                                  # still in the caller's order
+    refa = o.abs2(p, data[0], data[1])
+    assert np.max(np.abs(got - refa) / refa) < 1e-10
+    if not any(r.get("shape_floats") for r in c.resonances):
+        for path in (B.PATH_CACHED, B.PATH_CACHED_COMPACT):
+            m.set_path(path)
+            assert abs(m.nll(p) - ref) <= tol
+        m.set_path(B.PATH_RECOMPUTE)
+    n2 = data[0].size // 2
+    m.set_events(data[0][:n2], data[1][:n2])                # events change, normalisation copy stays sorted
+    ref2, sl2, integ2 = o.nll(p, data[0][:n2], data[1][:n2], data[2], data[3], data[4], parts=True)
+    assert abs(m.nll(p) - ref2) <= nll_tol(ref2, sl2, integ2, n2)
+    m.close()
+    m2 = B.Mipwa(c.kin, c.knots, c.resonances)
+    with pytest.raises(B.MipwaError) as ei:
+        m2.prepare()
+    assert ei.value.code == B.ERR_STATE
+    m2.close()
