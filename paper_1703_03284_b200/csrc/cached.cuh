@@ -235,36 +235,51 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
     const int R = RT >= 0 ? RT : m.R, C = 1 + R, N = cc.N;
     const long long n_tiles = (n_ev + MIPWA_TILE - 1) / MIPWA_TILE;
     LogProd lp;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const double2* p = cache + (size_t)tile * C * MIPWA_TILE + threadIdx.x;
-        const double2 s = ld_stream(p);
-        double re, im;
-        if (RT >= 0) {
-            double2 b[RT > 0 ? RT : 1];
+    if (RT >= 0) {
+        // two tiles per iteration: all 2 (1 + R) loads are in flight before the first value is used
+        constexpr int RC = RT > 0 ? RT : 1;
+        for (long long tile = blockIdx.x; tile < n_tiles; tile += 2LL * gridDim.x) {
+            const long long tiles[2] = { tile, tile + gridDim.x };
+            double2 s[2], b[2][RC];
 #pragma unroll
-            for (int r = 0; r < RT; ++r) b[r] = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE);
-            double r1, i1, r2, i2;
-            spline_eval(sm, m, s.x, r1, i1);
-            spline_eval(sm, m, s.y, r2, i2);
-            re = r1 + r2; im = i1 + i2;
+            for (int u = 0; u < 2; ++u) {
+                const long long tt = tiles[u] < n_tiles ? tiles[u] : tile;
+                const double2* p = cache + (size_t)tt * C * MIPWA_TILE + threadIdx.x;
+                s[u] = ld_stream(p);
 #pragma unroll
-            for (int r = 0; r < RT; ++r) {
-                const double2 c = cc.c[N + r];
-                re = fma(c.x, b[r].x, fma(-c.y, b[r].y, re));
-                im = fma(c.x, b[r].y, fma(c.y, b[r].x, im));
+                for (int r = 0; r < RT; ++r) b[u][r] = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE);
             }
-        } else {
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                double r1, i1, r2, i2;
+                spline_eval(sm, m, s[u].x, r1, i1);
+                spline_eval(sm, m, s[u].y, r2, i2);
+                double re = r1 + r2, im = i1 + i2;
+#pragma unroll
+                for (int r = 0; r < RT; ++r) {
+                    const double2 c = cc.c[N + r];
+                    re = fma(c.x, b[u][r].x, fma(-c.y, b[u][r].y, re));
+                    im = fma(c.x, b[u][r].y, fma(c.y, b[u][r].x, im));
+                }
+                const bool live = tiles[u] < n_tiles && tiles[u] * MIPWA_TILE + threadIdx.x < n_ev;
+                lp.add(live ? fma(re, re, im * im) : 1.0);
+            }
+        }
+    } else {
+        for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            const double2* p = cache + (size_t)tile * C * MIPWA_TILE + threadIdx.x;
+            const double2 s = ld_stream(p);
             double r1, i1, r2, i2;
             spline_eval(sm, m, s.x, r1, i1);
             spline_eval(sm, m, s.y, r2, i2);
-            re = r1 + r2; im = i1 + i2;
+            double re = r1 + r2, im = i1 + i2;
             for (int r = 0; r < R; ++r) {
                 const double2 b = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE), c = cc.c[N + r];
                 re = fma(c.x, b.x, fma(-c.y, b.y, re));
                 im = fma(c.x, b.y, fma(c.y, b.x, im));
             }
+            lp.add(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
         }
-        lp.add(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
     }
     double v[1] = { lp.value() };
     if (grid_reduce<1>(v, partials, ticket, red, &is_last)) {

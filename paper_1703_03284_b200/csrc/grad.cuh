@@ -158,12 +158,21 @@ __device__ __forceinline__ void grad_pass(const SplineSmem& sm, const DevModel& 
     LogProd lp;
     double integ = 0.0;
     const int nres = R1 >= 0 ? R1 + R2 : m.R;
+    double nx = 1.0, ny = 1.0, nw = 0.0;                                   // next iteration's point, loaded one ahead
+    if (lo < hi) {
+        const long long ii = lo + lane < hi ? lo + lane : lo;
+        nx = s12[ii]; ny = s13[ii];
+        if (!EV) nw = lo + lane < hi ? (w ? w[ii] : 1.0) : 0.0;
+    }
     for (long long base = lo; base < hi; base += 32) {                     // warp-uniform trip count
         const long long i = base + lane;
         const bool valid = i < hi;
-        const long long ii = valid ? i : lo;
-        const double x = s12[ii], y = s13[ii];
-        const double wv = EV ? 0.0 : (valid ? (w ? w[ii] : 1.0) : 0.0);
+        const double x = nx, y = ny, wv = nw;
+        if (base + 32 < hi) {
+            const long long ii = i + 32 < hi ? i + 32 : lo;
+            nx = s12[ii]; ny = s13[ii];
+            if (!EV) nw = i + 32 < hi ? (w ? w[ii] : 1.0) : 0.0;
+        }
         double are, aim, t1, t2, tr[RR], ti[RR];
         int j1, j2;
         amplitude_parts<R1, R2>(sm, m, x, y, are, aim, j1, t1, j2, t2, tr, ti);
@@ -218,14 +227,12 @@ __global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_GRAD_MINBLOCKS)
 k_grad_recompute(const __grid_constant__ DevModel m,
                  const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
                  const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
-                 long long n_norm, double* __restrict__ partials, unsigned int* __restrict__ ticket,
-                 double* __restrict__ result)
+                 long long n_norm, double* __restrict__ partials)
 {
     constexpr int RR = GradDims<R1, R2>::RR;
     extern __shared__ double grad_bins[];                  // [2][4][N-1][2]
     __shared__ SplineSmem sm;
     __shared__ double red32[32];
-    __shared__ bool is_last;
     const int NS = m.N - 1, R = m.R, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) grad_bins[k] = 0.0;
     load_spline_smem(sm, m);                               // ends with __syncthreads()
@@ -254,20 +261,21 @@ k_grad_recompute(const __grid_constant__ DevModel m,
     }
     __syncthreads();                                       // all flushes into grad_bins are done
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) mine[2 + 4 * R + k] = grad_bins[k];
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
-    __syncthreads();
-    if (is_last) {
-        __threadfence();
-        for (int k = threadIdx.x; k < NV; k += blockDim.x) {
-            double s = 0.0;
-            for (int b = 0; b < gridDim.x; ++b) s += __ldcg(&partials[(size_t)b * NV + k]);      // block order
-            result[k] = s;
-        }
-        __threadfence_system();
-        if (threadIdx.x == 0) *ticket = 0;
-    }
+}
+
+// fixed-order sum of the per-block partial vectors: one warp per value, lane l adds blocks l, l+32, .. then a shuffle
+// tree.  A separate tiny launch: done inside the last block of k_grad_recompute it would serialise ~NV x grid L2 reads
+// on one SM while the rest of the GPU idles.
+__global__ void __launch_bounds__(256)
+k_grad_finalize(const double* __restrict__ partials, int nblocks, int NV, double* __restrict__ result)
+{
+    const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (k >= NV) return;
+    double s = 0.0;
+    for (int b = lane; b < nblocks; b += 32) s += partials[(size_t)b * NV + k];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+    if (lane == 0) result[k] = s;
 }
 
 // ---- cell sort (once per point set): key = seg(s12) * (N-1) + seg(s13) ---------------------------------------------

@@ -894,7 +894,10 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
                        (k_grad_recompute<R1, R2><<<grid, MIPWA_BLOCK, smem, c->stream>>>(
                            c->model, c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.n, c->nm_sorted.s12, c->nm_sorted.s13,
-                           c->nm_sorted.w, c->nm_sorted.n, c->d_gpartials, c->d_ticket, c->d_result)));
+                           c->nm_sorted.w, c->nm_sorted.n, c->d_gpartials)));
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
