@@ -883,7 +883,7 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
         if (!ok) return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
         if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
     }
-    const int grid = c->sm_count * c->grad_blocks_per_sm;
+    const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->grad_blocks_per_sm);   // small samples: fewer partial vectors
     if (c->gpartials_len < (size_t)grid * NV) {
         if (c->d_gpartials) cudaFree(c->d_gpartials);
         c->d_gpartials = nullptr; c->gpartials_len = 0;
