@@ -10,7 +10,7 @@
 //     Z1 = x + 2y - Sigma + kappa ix,  Z2 = Z1^2 - ql pl / 3
 //   per resonance (spin L, constants prepared on the host, step A3):
 //     D_R = den_L(cR ql), D_D = den_L(cD lam2), den_1(z) = 1 + z, den_2(z) = 9 + 3z + z^2
-//     W'  = Kw g ql^L                       [= m0 Gamma(x) D_R: the running width without its barrier denominator]
+//     W'  = Kw (2g) ql^L                       [= m0 Gamma(x) D_R: the running width without its barrier denominator]
 //     dD  = (m0^2 - x) D_R,  E = dD^2 + W'^2
 //     F_D F_R BW = sqrt(n_R n_D) D_R (dD + i W') / (sqrt(D_R D_D) E) = sqrt(n_R n_D) D_R (dD + i W') rsqrt(D_R D_D E^2)
 //   so that ONE reciprocal square root per resonance and channel replaces two square roots and three divisions.
@@ -27,7 +27,7 @@ struct ResDev {
     double m0sq;      // m0^2
     double cR;        // r_res^2 / 4            (z_R = cR * ql);  0 for L = 0
     double cD;        // r_parent^2 / (4 M^2)   (z_D = cD * lam2); 0 for L = 0
-    double Kw;        // m0^2 Gamma0 n_R / ((4 q0^2)^L sqrt(q0^2))
+    double Kw;        // m0^2 Gamma0 n_R / (2 (4 q0^2)^L sqrt(q0^2))   (the 1/2 of g = sqrt(lam1)/(2x) lives here)
     double cre, cim;  // c_r * sqrt(n_R n_D)
     double pa, pb, pc;// barrier denominator den_L(z) = pc + z (pb + pa z)
     int32_t L;
@@ -44,7 +44,7 @@ struct DevModel {
     double s_hi, s_top;        // (M-m3)^2, (M+m3)^2
     double sigma;              // M^2 + m1^2 + m2^2 + m3^2
     double kappa;              // (M^2 - m3^2)(m2^2 - m1^2)
-    double lut_x0, lut_inv;    // bucket = (s - lut_x0) * lut_inv
+    double lut_off, lut_inv;   // bucket = floor(s * lut_inv + lut_off), lut_off = -x_0 * lut_inv
     double knots[MIPWA_DEV_MAX_KNOTS];
     double2 sc[4][MIPWA_DEV_MAX_KNOTS];   // segment j: S(s) = sc[0][j] + t(sc[1][j] + t(sc[2][j] + t sc[3][j])), t = s - x_j
     uint8_t lut[MIPWA_DEV_LUT];           // segment that contains the left edge of each bucket
@@ -100,7 +100,7 @@ __device__ __forceinline__ double fast_rsqrt(double x)
 // MIPWA_DEV_LUT buckets fall back to the search.
 __device__ __forceinline__ int spline_segment(const SplineSmem& sm, const DevModel& m, double s, double& xj)
 {
-    int b = __double2int_rd((s - m.lut_x0) * m.lut_inv);
+    int b = __double2int_rd(fma(s, m.lut_inv, m.lut_off));     // lut_off = -lut_x0 * lut_inv
     b = max(0, min(b, m.nlut - 1));
     int j = sm.lut[b];
     if (m.lut_exact) {
@@ -143,9 +143,14 @@ __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, dou
     const double pl = c.lam2 * ix;
     // sqrt(lam1) = l rsqrt(l) with l = max(lam1, tiny): no branch, ~1e-150 instead of 0 at threshold where the
     // width vanishes anyway
+    // (rsqrt refinement merged with the product: sqrt(l) = h + h e p(e), h = l y0, e = 1 - h y0, p = 1/2 + 3e/8;
+    // the factor 1/2 of g is folded into Kw on the host)
     const double lc = fmax(lam1, 1e-300);
-    const double sq = lc * fast_rsqrt(lc);
-    c.w[0] = 0.5 * sq * ix;
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(lc));
+    const double h = lc * y0, e = fma(-h, y0, 1.0);
+    const double sq = fma(h * e, fma(0.375, e, 0.5), h);
+    c.w[0] = sq * ix;
     c.w[1] = c.w[0] * c.ql;
     c.w[2] = c.w[1] * c.ql;
     c.Z[0] = 1.0;

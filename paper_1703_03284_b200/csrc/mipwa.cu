@@ -129,7 +129,7 @@ int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, 
     out->m0sq = m0sq;
     out->cR = L ? 0.25 * d.r_res * d.r_res : 0.0;
     out->cD = L ? d.r_parent * d.r_parent / (4.0 * M2) : 0.0;
-    out->Kw = m0sq * g0 * nR / (std::pow(4.0 * q0sq, L) * std::sqrt(q0sq));
+    out->Kw = 0.5 * m0sq * g0 * nR / (std::pow(4.0 * q0sq, L) * std::sqrt(q0sq));
     const double f = cmag * std::sqrt(nR * nD);
     if (fold) *fold = std::sqrt(nR * nD);
     out->cre = f * std::cos(carg);
@@ -209,7 +209,7 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
     m.s_top = (k.m_parent + k.m3) * (k.m_parent + k.m3);
     m.sigma = k.m_parent * k.m_parent + k.m1 * k.m1 + k.m2 * k.m2 + k.m3 * k.m3;
     m.kappa = (k.m_parent * k.m_parent - k.m3 * k.m3) * (k.m2 * k.m2 - k.m1 * k.m1);
-    m.lut_x0 = c->lut_x0; m.lut_inv = c->lut_inv;
+    m.lut_off = -c->lut_x0 * c->lut_inv; m.lut_inv = c->lut_inv;
     std::memcpy(m.lut, c->lut.data(), c->nlut);
     std::memcpy(m.xk, c->xk.data(), c->nlut * sizeof(double));
     for (int i = 0; i < N; ++i) {
