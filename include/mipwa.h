@@ -121,7 +121,9 @@ int mipwa_nll_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, doub
 
 /* NLL and its analytic gradient with respect to the first 2N + 2R parameters (the linear coefficients in polar
  * form; derivatives with respect to floating masses/widths are not provided, reading P16).
- * grad: HOST, 2N + 2R doubles, laid out like params. */
+ * grad: HOST, 2N + 2R doubles, laid out like params.  Works on cell-sorted copies of the points (implies
+ * mipwa_prepare).  With fixed shapes and the path MIPWA_PATH_CACHED_COMPACT (or AUTO) the events are streamed from
+ * the compact cache and the normalisation part comes from the Gram matrix; otherwise every term is recomputed. */
 int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
 /* TEST HOOK: per-point |A|^2 from the same device function the NLL kernels use.

@@ -305,3 +305,113 @@ k_gather(const unsigned int* __restrict__ idx, long long n, const double* __rest
         if (c) oc[i] = c[s];
     }
 }
+
+// ---- A8 on the compact cached path (fixed shapes) -------------------------------------------------------------------
+// Events only: the normalisation part of the gradient is (2 n_ev / I) (G c)_k from the Gram matrix (host, K^2 MACs).
+// Streams the compact cache (16 + 16 R bytes per event, cell-sorted event order), evaluates the spline part from
+// the shared-memory tables, and accumulates  f = -2/conj(A):  moments f t^q per segment (as k_grad_recompute) and
+// F_r = sum f conj(B_{N+r}) per resonance.  Partial vector per block: [S, F(2R), bins(8 (N-1))].
+template <int RT>
+__global__ void __launch_bounds__(MIPWA_TILE, 2)
+k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDev cc,
+               const double2* __restrict__ cache, long long n_ev, double* __restrict__ partials)
+{
+    constexpr int RC = RT > 0 ? RT : (RT == 0 ? 1 : MIPWA_GRAD_MAXR);
+    extern __shared__ double grad_bins[];                  // [4][N-1][2]
+    __shared__ SplineSmem sm;
+    __shared__ double red32[32];
+    const int R = RT >= 0 ? RT : m.R, C = 1 + R, N = cc.N, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;
+    for (int k = threadIdx.x; k < nb; k += blockDim.x) grad_bins[k] = 0.0;
+    load_spline_smem(sm, m);
+
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long long W = (long long)gridDim.x * wpb, wg = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    const long long CH = (((n_ev + W - 1) / W) + 31) & ~31LL;
+    const long long lo = wg * CH, hi = lo + CH < n_ev ? lo + CH : n_ev;
+    CellAcc acc;
+    acc.clear();
+    acc.j1 = acc.j2 = -1;
+    LogProd lp;
+    double Fr[RC], Fi[RC];
+#pragma unroll
+    for (int r = 0; r < RC; ++r) Fr[r] = Fi[r] = 0.0;
+    for (long long base = lo; base < hi; base += 32) {                     // warp-uniform trip count; base % 32 == 0
+        const long long i = base + lane;
+        const bool valid = i < hi;
+        const long long ii = valid ? i : lo;
+        const double2* p = cache + (size_t)(ii / MIPWA_TILE) * C * MIPWA_TILE + (ii % MIPWA_TILE);
+        const double2 s = ld_stream(p);
+        double2 b[RC];
+        if (RT >= 0) {
+#pragma unroll
+            for (int r = 0; r < RT; ++r) b[r] = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE);
+        } else {
+            for (int r = 0; r < R; ++r) b[r] = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE);
+        }
+        int j1, j2;
+        double t1, t2, r1, i1, r2, i2;
+        spline_eval_jt(sm, m, s.x, j1, t1, r1, i1);
+        spline_eval_jt(sm, m, s.y, j2, t2, r2, i2);
+        double are = r1 + r2, aim = i1 + i2;
+        if (RT >= 0) {
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                const double2 c = cc.c[N + r];
+                are = fma(c.x, b[r].x, fma(-c.y, b[r].y, are));
+                aim = fma(c.x, b[r].y, fma(c.y, b[r].x, aim));
+            }
+        } else {
+            for (int r = 0; r < R; ++r) {
+                const double2 c = cc.c[N + r];
+                are = fma(c.x, b[r].x, fma(-c.y, b[r].y, are));
+                aim = fma(c.x, b[r].y, fma(c.y, b[r].x, aim));
+            }
+        }
+        const double a2 = fma(are, are, aim * aim);
+        const double k = valid ? -2.0 * fast_rcp(a2) : 0.0;
+        const double fr = k * are, fi = k * aim;
+        lp.add(valid ? a2 : 1.0);
+        if (RT >= 0) {
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                Fr[r] = fma(fr, b[r].x, fma(fi, b[r].y, Fr[r]));
+                Fi[r] = fma(fi, b[r].x, fma(-fr, b[r].y, Fi[r]));
+            }
+        } else {
+            for (int r = 0; r < R; ++r) {
+                Fr[r] = fma(fr, b[r].x, fma(fi, b[r].y, Fr[r]));
+                Fi[r] = fma(fi, b[r].x, fma(-fr, b[r].y, Fi[r]));
+            }
+        }
+        const bool same = !valid || (j1 == acc.j1 && j2 == acc.j2);
+        if (__all_sync(0xffffffffu, same)) {
+            acc.add(fr, fi, t1, t2);
+        } else {
+            flush_warp(acc, grad_bins, NS);
+            const int l1 = __shfl_sync(0xffffffffu, j1, 0), l2 = __shfl_sync(0xffffffffu, j2, 0);
+            const bool uni = !valid || (j1 == l1 && j2 == l2);
+            if (__all_sync(0xffffffffu, uni)) {
+                acc.j1 = l1; acc.j2 = l2;
+                acc.add(fr, fi, t1, t2);
+            } else if (valid) {
+                scatter_lane(fr, fi, j1, t1, j2, t2, grad_bins, NS);
+            }
+        }
+    }
+    flush_warp(acc, grad_bins, NS);
+
+    double* mine = partials + (size_t)blockIdx.x * NV;
+    double v = block_sum(lp.value(), red32);
+    if (threadIdx.x == 0) mine[0] = v;
+    for (int r = 0; r < R; ++r) {
+        double a = 0, bb = 0;
+        if (RT >= 0) {
+#pragma unroll
+            for (int q = 0; q < RC; ++q) if (q == r) { a = Fr[q]; bb = Fi[q]; }
+        } else { a = Fr[r]; bb = Fi[r]; }
+        a = block_sum(a, red32); if (threadIdx.x == 0) mine[1 + 2 * r] = a;
+        bb = block_sum(bb, red32); if (threadIdx.x == 0) mine[1 + 2 * r + 1] = bb;
+    }
+    __syncthreads();
+    for (int k2 = threadIdx.x; k2 < nb; k2 += blockDim.x) mine[1 + 2 * R + k2] = grad_bins[k2];
+}

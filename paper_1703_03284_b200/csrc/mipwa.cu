@@ -76,6 +76,7 @@ struct mipwa_ctx {
     int cache_kind = 0;             // MIPWA_PATH_CACHED / MIPWA_PATH_CACHED_COMPACT, valid iff cache_valid
     bool cache_valid = false;
     double2* d_gram = nullptr;
+    std::vector<double> h_gram;     // host copy (K x K complex, row-major) for the cached-path gradient
     bool gram_valid = false;
     int dense_blocks_per_sm = 0, compact_blocks_per_sm = 0;
 
@@ -589,6 +590,9 @@ static int ensure_gram(mipwa_ctx* c)
         ++c->launches;
         e = cudaGetLastError();
     }
+    c->h_gram.resize((size_t)2 * K * K);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(c->h_gram.data(), c->d_gram, (size_t)K * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     cudaFree(partial);
     if (e != cudaSuccess) return fail(c, MIPWA_ERR_CUDA, std::string("gram: ") + cudaGetErrorString(e));
@@ -794,6 +798,51 @@ int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32
     return MIPWA_OK;
 }
 
+// adjoint of the map knot values y -> segment coefficients sc (build_model): from calG of sc[q][j] (Gsc[(q*NS+j)*2+ri])
+// to calG of y_k (Gy[2k+ri]).  sc0 = y_j; sc1 = (y_j+1 - y_j)/h - h (2 P_j + P_j+1)/6; sc2 = P_j/2;
+// sc3 = (P_j+1 - P_j)/(6h); P = Mx y  =>  Gy = g_y + Mx^T g_P.
+static void spline_adjoint(const mipwa_ctx* c, const double* Gsc, double* Gy)
+{
+    const int N = c->N, NS = N - 1;
+    std::vector<double> gy(2 * N, 0.0), gP(2 * N, 0.0);
+    for (int j = 0; j < NS; ++j) {
+        const double hj = c->knots[j + 1] - c->knots[j];
+        for (int q = 0; q < 2; ++q) {                                  // re, im
+            const double G0 = Gsc[(0 * NS + j) * 2 + q], G1 = Gsc[(1 * NS + j) * 2 + q];
+            const double G2 = Gsc[(2 * NS + j) * 2 + q], G3 = Gsc[(3 * NS + j) * 2 + q];
+            gy[2 * j + q] += G0 - G1 / hj;
+            gy[2 * (j + 1) + q] += G1 / hj;
+            gP[2 * j + q] += -G1 * hj / 3.0 + 0.5 * G2 - G3 / (6.0 * hj);
+            gP[2 * (j + 1) + q] += -G1 * hj / 6.0 + G3 / (6.0 * hj);
+        }
+    }
+    for (int k = 0; k < N; ++k) {
+        double gr = gy[2 * k], gi = gy[2 * k + 1];
+        for (int j = 0; j < N; ++j) {
+            const double mjk = c->Mx[(size_t)j * N + k];
+            gr += mjk * gP[2 * j]; gi += mjk * gP[2 * j + 1];
+        }
+        Gy[2 * k] = gr; Gy[2 * k + 1] = gi;
+    }
+}
+
+// polar chain rule: c = rho e^{i theta}: d/drho = Re(calG e^{-i theta}), d/dtheta = Re(calG conj(i c)).
+// Gy: calG of the knot values (2N), Gr: calG of the resonance coefficients in the caller's order (2R).
+static void polar_chain(const mipwa_ctx* c, const double* params, const double* Gy, const double* Gr, double* grad)
+{
+    const int N = c->N, R = c->R;
+    for (int k = 0; k < N; ++k) {
+        const double ph = params[N + k];
+        grad[k] = Gy[2 * k] * std::cos(ph) + Gy[2 * k + 1] * std::sin(ph);
+        grad[N + k] = -Gy[2 * k] * c->y_im[k] + Gy[2 * k + 1] * c->y_re[k];
+    }
+    for (int r = 0; r < R; ++r) {
+        const double mag = params[2 * N + 2 * r], th = params[2 * N + 2 * r + 1];
+        grad[2 * N + 2 * r] = Gr[2 * r] * std::cos(th) + Gr[2 * r + 1] * std::sin(th);
+        grad[2 * N + 2 * r + 1] = mag * (-Gr[2 * r] * std::sin(th) + Gr[2 * r + 1] * std::cos(th));
+    }
+}
+
 // ---- A8: gradient on the recompute path ---------------------------------------------------------------------------
 // cell-sorted copy of a point set (keys from the knots only: valid until the next mipwa_set_* on that slot)
 static int ensure_sorted(mipwa_ctx* c, const Slot& src, Slot& dst, bool& valid)
@@ -862,6 +911,78 @@ int mipwa_prepare(mipwa_ctx* c)
     return prepare_sorted(c);
 }
 
+// A8 on the compact cached path: events through k_grad_compact, normalisation part from the Gram matrix
+static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+{
+    int rc = ensure_cache(c, MIPWA_PATH_CACHED_COMPACT);
+    if (rc) return rc;
+    rc = ensure_gram(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);                 // spline tables of this call (after ensure_*: they use c->model)
+    if (rc) return rc;
+    CoefDev cc;
+    fill_coef(c, params, &cc);
+    const int N = c->N, R = c->R, K = N + R, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;
+    const size_t smem = (size_t)nb * sizeof(double);
+    const int grid = grid_for(c, c->ev.n, 2);
+    if (c->gpartials_len < (size_t)grid * NV) {
+        if (c->d_gpartials) cudaFree(c->d_gpartials);
+        c->d_gpartials = nullptr; c->gpartials_len = 0;
+        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NV * sizeof(double)));
+        c->gpartials_len = (size_t)grid * NV;
+    }
+    const double2* cache = (const double2*)c->d_cache;
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+#define MIPWA_GC_LAUNCH(T) \
+    k_grad_compact<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, cc, cache, c->ev.n, c->d_gpartials)
+    switch (R) {
+        case 0: MIPWA_GC_LAUNCH(0); break;
+        case 1: MIPWA_GC_LAUNCH(1); break;
+        case 2: MIPWA_GC_LAUNCH(2); break;
+        case 3: MIPWA_GC_LAUNCH(3); break;
+        case 4: MIPWA_GC_LAUNCH(4); break;
+        case 6: MIPWA_GC_LAUNCH(6); break;
+        default: MIPWA_GC_LAUNCH(-1); break;
+    }
+#undef MIPWA_GC_LAUNCH
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+
+    // host: g = G c, I = Re(c^H g) (K^2 complex MACs), then the adjoint maps
+    const double* h = c->h_result;
+    const double* G = c->h_gram.data();
+    std::vector<double> gc(2 * K, 0.0);
+    double I = 0.0;
+    for (int k = 0; k < K; ++k) {
+        double gr = 0.0, gi = 0.0;
+        for (int l = 0; l < K; ++l) {
+            const double a = G[2 * ((size_t)k * K + l)], b = G[2 * ((size_t)k * K + l) + 1];
+            gr += a * cc.c[l].x - b * cc.c[l].y;
+            gi += a * cc.c[l].y + b * cc.c[l].x;
+        }
+        gc[2 * k] = gr; gc[2 * k + 1] = gi;
+        I += cc.c[k].x * gr + cc.c[k].y * gi;
+    }
+    const double S = h[0], n_ev = (double)c->ev.n;
+    *nll = -S + n_ev * std::log(I);
+    const double scale = c->ev.n > 0 ? 2.0 * n_ev / I : 0.0;
+    std::vector<double> Gy(2 * N), Gr(2 * std::max(R, 1));
+    spline_adjoint(c, h + 1 + 2 * R, Gy.data());
+    for (int k = 0; k < 2 * N; ++k) Gy[k] += scale * gc[k];
+    for (int r = 0; r < R; ++r) {                           // cache columns are in the caller's order, fold included
+        Gr[2 * r] = h[1 + 2 * r] + scale * gc[2 * (N + r)];
+        Gr[2 * r + 1] = h[1 + 2 * r + 1] + scale * gc[2 * (N + r) + 1];
+    }
+    polar_chain(c, params, Gy.data(), Gr.data(), grad);
+    return MIPWA_OK;
+}
+
 int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
 {
     if (!c || !params || !nll || !grad) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
@@ -870,6 +991,7 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     if (rc) return rc;
     rc = prepare_sorted(c);
     if (rc) return rc;
+    if (effective_path(c) == MIPWA_PATH_CACHED_COMPACT) return nll_grad_compact(c, params, n_params, nll, grad);
     rc = build_model(c, params, n_params);
     if (rc) return rc;
 
@@ -915,39 +1037,15 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     const double* Fn = h + 2 + 2 * R;
     const double* Be = h + 2 + 4 * R;
     const double* Bn = Be + nb;
-    std::vector<double> gy(2 * N, 0.0), gP(2 * N, 0.0);               // interleaved re, im
-    for (int j = 0; j < NS; ++j) {
-        const double hj = c->knots[j + 1] - c->knots[j];
-        for (int q = 0; q < 2; ++q) {                                  // re, im
-            const double G0 = Be[(0 * NS + j) * 2 + q] + scale * Bn[(0 * NS + j) * 2 + q];
-            const double G1 = Be[(1 * NS + j) * 2 + q] + scale * Bn[(1 * NS + j) * 2 + q];
-            const double G2 = Be[(2 * NS + j) * 2 + q] + scale * Bn[(2 * NS + j) * 2 + q];
-            const double G3 = Be[(3 * NS + j) * 2 + q] + scale * Bn[(3 * NS + j) * 2 + q];
-            // sc0 = y_j; sc1 = (y_j+1 - y_j)/h - h (2 P_j + P_j+1)/6; sc2 = P_j/2; sc3 = (P_j+1 - P_j)/(6h)
-            gy[2 * j + q] += G0 - G1 / hj;
-            gy[2 * (j + 1) + q] += G1 / hj;
-            gP[2 * j + q] += -G1 * hj / 3.0 + 0.5 * G2 - G3 / (6.0 * hj);
-            gP[2 * (j + 1) + q] += -G1 * hj / 6.0 + G3 / (6.0 * hj);
-        }
-    }
-    for (int k = 0; k < N; ++k) {
-        double gr = gy[2 * k], gi = gy[2 * k + 1];
-        for (int j = 0; j < N; ++j) {                                  // + Mx^T g_P  (P = Mx y)
-            const double mjk = c->Mx[(size_t)j * N + k];
-            gr += mjk * gP[2 * j]; gi += mjk * gP[2 * j + 1];
-        }
-        const double ph = params[N + k];
-        grad[k] = gr * std::cos(ph) + gi * std::sin(ph);               // Re(calG e^{-i phi})
-        grad[N + k] = -gr * c->y_im[k] + gi * c->y_re[k];              // Re(calG conj(i y_k))
-    }
+    std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * R);
+    for (int k = 0; k < nb; ++k) Gsc[k] = Be[k] + scale * Bn[k];
+    spline_adjoint(c, Gsc.data(), Gy.data());
     for (int d = 0; d < R; ++d) {
         const int r = c->perm[d];
-        const double gr = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
-        const double gi = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
-        const double mag = params[2 * N + 2 * r], th = params[2 * N + 2 * r + 1];
-        grad[2 * N + 2 * r] = gr * std::cos(th) + gi * std::sin(th);
-        grad[2 * N + 2 * r + 1] = mag * (-gr * std::sin(th) + gi * std::cos(th));
+        Gr[2 * r] = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
+        Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
     }
+    polar_chain(c, params, Gy.data(), Gr.data(), grad);
     return MIPWA_OK;
 }
 

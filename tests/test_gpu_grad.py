@@ -113,3 +113,32 @@ def test_gradient_edge_cases():
     _, ref_g = o2.nll_grad(p2, e12, e13, g12, g13, w)
     _check(m2.nll_grad(p2)[1], ref_g)
     m2.close()
+
+
+def test_gradient_on_the_compact_cached_path(case):
+    """Fixed shapes: mipwa_nll_grad under MIPWA_PATH_CACHED_COMPACT / AUTO streams the compact cache (k_grad_compact)
+    and takes the normalisation part from the Gram matrix; under MIPWA_PATH_CACHED it recomputes.  All must agree
+    with the oracle."""
+    c, o, data = case
+    B = _lib()
+    if any(r.get("shape_floats") for r in c.resonances):
+        pytest.skip("floating shapes cannot be cached")
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], data[4])
+    p = c.perturbed(4)
+    ref_nll, ref_g = o.nll_grad(p, *data)
+    _, sl, integ = o.nll(p, *data, parts=True)
+    tol = nll_tol(ref_nll, sl, integ, data[0].size)
+    for path in (B.PATH_CACHED_COMPACT, B.PATH_AUTO, B.PATH_CACHED, B.PATH_RECOMPUTE, B.PATH_CACHED_COMPACT):
+        m.set_path(path)
+        nll, g = m.nll_grad(p)
+        assert abs(nll - ref_nll) <= tol, path
+        _check(g, ref_g)
+        assert abs(m.nll(p) - ref_nll) <= tol
+    # ragged and tiny samples on the cached gradient
+    m.set_path(B.PATH_CACHED_COMPACT)
+    for n in (1, 33, 257):
+        m.set_events(data[0][:n], data[1][:n])
+        _, ref_g = o.nll_grad(p, data[0][:n], data[1][:n], data[2], data[3], data[4])
+        _check(m.nll_grad(p)[1], ref_g)
+    m.close()
