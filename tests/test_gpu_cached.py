@@ -176,3 +176,38 @@ def test_many_knots_gram_tiles():
         m.set_path(path)
         assert abs(m.nll(p) - ref) <= nll_tol(ref, sl, integ, 2000)
         m.close()
+
+
+def test_maximum_model_size():
+    """MIPWA_MAX_KNOTS = 128 knots and MIPWA_MAX_RESONANCES = 16 resonances of mixed spin (run-time resonance loops,
+    K = 144: three Gram register tiles per thread): every path and both gradients against the oracle."""
+    B = _lib()
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    c = I.Config(1)
+    knots = I.knots_uniform(128)
+    rng = np.random.default_rng(3)
+    res = [dict(mass=float(rng.uniform(0.5, 1.6)), width=float(rng.uniform(0.05, 0.4)), spin=int(k % 3),
+                r_res=float(rng.uniform(1.0, 3.0)), r_parent=float(rng.uniform(1.0, 5.0))) for k in range(16)]
+    o = orc.Oracle(c.kin, knots, res)
+    p = np.concatenate([rng.uniform(0.5, 2, 128), rng.uniform(0, 3, 128),
+                        np.stack([rng.uniform(0.1, 2, 16), rng.uniform(0, 6, 16)], axis=1).ravel()])
+    g12, g13 = I.phase_space_points(9000, c.key(I.S_NORM))
+    e12, e13, g12, g13 = g12[:4001], g13[:4001], g12[4001:], g13[4001:]
+    ref, sl, integ = o.nll(p, e12, e13, g12, g13, None, parts=True)
+    tol = nll_tol(ref, sl, integ, e12.size)
+    _, ref_g = o.nll_grad(p, e12, e13, g12, g13, None)
+    m = B.Mipwa(c.kin, knots, res)
+    m.set_events(e12, e13); m.set_norm_points(g12, g13, None)
+    got, refa = m.eval_abs2(p, 0), o.abs2(p, e12, e13)
+    assert np.max(np.abs(got - refa) / refa) < 1e-10
+    for path in (B.PATH_RECOMPUTE, B.PATH_CACHED, B.PATH_CACHED_COMPACT):
+        m.set_path(path)
+        assert abs(m.nll(p) - ref) <= tol, path
+        _, g = m.nll_grad(p)
+        assert np.max(np.abs(g - ref_g)) <= 1e-9 * np.max(np.abs(ref_g)), path
+    m.close()
+    with pytest.raises(B.MipwaError):
+        B.Mipwa(c.kin, I.knots_uniform(129), res)
+    with pytest.raises(B.MipwaError):
+        B.Mipwa(c.kin, knots, res + [res[0]])
