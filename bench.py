@@ -108,10 +108,12 @@ def run_reference(args, cfg, workload):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_ev = min(cfg.n_ev, 400_000)
-    n_norm = min(cfg.norm_size, 400_000)
-    steps = max(1, min(args.steps, 20))
-    warmup = min(args.warmup, 2)
+    # exactly K timed steps; each step is one oracle NLL call on a bounded sample of the workload, sized so that
+    # K + W calls end within a few minutes (the oracle does ~1e7 points/s on 8-16 host threads)
+    steps, warmup = max(1, args.steps), args.warmup
+    per_set = int(max(10_000, min(400_000, 0.7e9 / (steps + warmup))))
+    n_ev = min(cfg.n_ev, per_set)
+    n_norm = min(cfg.norm_size, per_set)
     cb = time_oracle(cfg, n_ev, n_norm, steps, warmup)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * cb["seconds_per_call"], "higher_is_better": True,
