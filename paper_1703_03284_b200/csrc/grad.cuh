@@ -15,7 +15,7 @@
 // a contiguous chunk, so consecutive iterations of a warp stay in one cell for thousands of points: the 8 complex
 // moments (4 per channel) live in registers and are flushed (warp shuffle reduction, then 16 shared-memory
 // adds by lane 0) only when the warp's cell changes.  A warp-iteration that straddles a cell boundary takes a
-// per-lane shared-atomic slow path (at most once per cell boundary).
+// slower path: one shuffle-reduce round per distinct cell in the group (add_mixed).
 #pragma once
 #include "cached.cuh"
 
@@ -110,12 +110,23 @@ __device__ __forceinline__ void flush_warp(CellAcc& a, double* bins, int NS)
     a.j1 = a.j2 = -1;
 }
 
-__device__ __forceinline__ void scatter_lane(double fr, double fi, int j1, double t1, int j2, double t2, double* bins, int NS)
+// A warp-iteration whose 32 points fall into several cells (it straddles a cell boundary of the sorted order): one
+// round per distinct cell - the lanes of that cell contribute, the others add zeros - through the same
+// shuffle-reduce + lane-0 flush, instead of per-lane shared atomics that would all collide on the same bins.
+// `acc` must be empty on entry and is empty on return.
+__device__ __forceinline__ void add_mixed(CellAcc& acc, bool valid, int j1, int j2, double fr, double fi, double t1,
+                                          double t2, double* bins, int NS)
 {
-    double p = 1.0;
-    for (int q = 0; q < 4; ++q) { atomicAdd(&bins[(q * NS + j1) * 2], fr * p); atomicAdd(&bins[(q * NS + j1) * 2 + 1], fi * p); p *= t1; }
-    p = 1.0;
-    for (int q = 0; q < 4; ++q) { atomicAdd(&bins[(q * NS + j2) * 2], fr * p); atomicAdd(&bins[(q * NS + j2) * 2 + 1], fi * p); p *= t2; }
+    unsigned int remaining = __ballot_sync(0xffffffffu, valid);
+    while (remaining) {                                                    // warp-uniform
+        const int leader = __ffs(remaining) - 1;
+        const int l1 = __shfl_sync(0xffffffffu, j1, leader), l2 = __shfl_sync(0xffffffffu, j2, leader);
+        const bool mine = valid && j1 == l1 && j2 == l2;
+        acc.j1 = l1; acc.j2 = l2;
+        acc.add(mine ? fr : 0.0, mine ? fi : 0.0, t1, t2);
+        flush_warp(acc, bins, NS);
+        remaining &= ~__ballot_sync(0xffffffffu, mine);
+    }
 }
 
 // sum over the block of one value per thread (valid in thread 0); red32: 32 doubles of shared memory
@@ -208,8 +219,8 @@ __device__ __forceinline__ void grad_pass(const SplineSmem& sm, const DevModel& 
             if (__all_sync(0xffffffffu, uni)) {
                 acc.j1 = l1; acc.j2 = l2;
                 acc.add(fr, fi, t1, t2);
-            } else if (valid) {
-                scatter_lane(fr, fi, j1, t1, j2, t2, bins, NS);
+            } else {
+                add_mixed(acc, valid, j1, j2, fr, fi, t1, t2, bins, NS);
             }
         }
     }
@@ -393,8 +404,8 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
             if (__all_sync(0xffffffffu, uni)) {
                 acc.j1 = l1; acc.j2 = l2;
                 acc.add(fr, fi, t1, t2);
-            } else if (valid) {
-                scatter_lane(fr, fi, j1, t1, j2, t2, grad_bins, NS);
+            } else {
+                add_mixed(acc, valid, j1, j2, fr, fi, t1, t2, grad_bins, NS);
             }
         }
     }
