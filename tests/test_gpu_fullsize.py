@@ -1,0 +1,81 @@
+"""GPU parity at BASELINE.json's full size, in the launch configuration bench.py times: configs[3] (50 knots,
+rho(770) floating + rho(1450) + f2(1270), 10 M accept-reject events + 10 M weighted phase-space normalisation points,
+device-resident arrays, mipwa_prepare, full grid).  The oracle evaluates the whole sample here (seconds on the GPU
+box's host cores), so the comparison is on the complete NLL and gradient, plus per-event |A|^2 on a stride sample
+taken from the full-size launch of the hook.
+"""
+import numpy as np
+import pytest
+
+from tests.helpers import nll_tol
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def full():
+    import torch
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import binding as B
+    from paper_1703_03284_b200 import inputs as I
+    c = I.Config(3)
+    o = orc.Oracle(c.kin, c.knots, c.resonances)
+    f = lambda a, b: o.abs2(c.truth, a, b)
+    e12, e13 = c.events(f, I.envelope_of(f, c.kin, n_side=512), chunk=1 << 22)
+    g12, g13, w = c.norm_points()
+    assert e12.size == 10_000_000 and g12.size == 10_000_000
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (e12, e13, g12, g13, w)]
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(dev[0], dev[1]); m.set_norm_points(dev[2], dev[3], dev[4])
+    m.set_path(B.PATH_RECOMPUTE)
+    yield c, o, (e12, e13, g12, g13, w), m, dev
+    m.close()
+
+
+def test_full_size_nll_and_sampled_abs2(full):
+    c, o, data, m, _ = full
+    p = c.perturbed(0)
+    ref, sl, integ = o.nll(p, *data, parts=True)
+    tol = nll_tol(ref, sl, integ, data[0].size)
+    got, gsl, ginteg = m.nll_parts(p)                       # caller's order
+    assert abs(got - ref) <= tol, (got, ref, tol)
+    assert gsl == pytest.approx(sl, rel=1e-12) and ginteg == pytest.approx(integ, rel=1e-12)
+    m.prepare()                                             # cell-sorted copies, as bench.py runs it
+    got2 = m.nll(p)
+    assert abs(got2 - ref) <= tol and m.nll(p) == got2
+    a2 = m.eval_abs2(p, 0)
+    idx = np.arange(0, a2.size, 997)
+    refa = o.abs2(p, data[0][idx], data[1][idx])
+    assert np.max(np.abs(a2[idx] - refa) / refa) < 1e-12
+    assert np.all(np.isfinite(a2)) and a2.min() > 0.0
+
+
+def test_full_size_gradient(full):
+    c, o, data, m, _ = full
+    p = c.perturbed(1)
+    ref_nll, ref_g = o.nll_grad(p, *data)
+    nll, g = m.nll_grad(p)
+    _, sl, integ = o.nll(p, *data, parts=True)
+    assert abs(nll - ref_nll) <= nll_tol(ref_nll, sl, integ, data[0].size)
+    assert g.size == 106
+    assert np.max(np.abs(g - ref_g)) <= 1e-9 * np.max(np.abs(ref_g))
+
+
+def test_full_size_cached_paths(full):
+    """The same events with every shape fixed: dense (8.5 GB) and compact caches against the oracle."""
+    c, o, data, _, dev = full
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import binding as B
+    fixed = [dict(r, shape_floats=0) for r in c.resonances]
+    of = orc.Oracle(c.kin, c.knots, fixed)
+    p = c.perturbed(2)[:2 * c.N + 2 * c.R]
+    ref, sl, integ = of.nll(p, *data, parts=True)
+    tol = nll_tol(ref, sl, integ, data[0].size)
+    m = B.Mipwa(c.kin, c.knots, fixed)
+    m.set_events(dev[0], dev[1]); m.set_norm_points(dev[2], dev[3], dev[4]); m.prepare()
+    for path in (B.PATH_CACHED, B.PATH_CACHED_COMPACT):
+        m.set_path(path)
+        got, gsl, ginteg = m.nll_parts(p)
+        assert abs(got - ref) <= tol, (path, got, ref)
+        assert ginteg == pytest.approx(integ, rel=1e-11)
+    m.close()
