@@ -365,6 +365,99 @@ def run_ours(args, cfg, workload):
         dist.destroy_process_group()
 
 
+# ---- secondary measurements behind the numbers in BASELINE.md / profiles (not the driver's bench line) --------------
+def run_probe(args):
+    """--probe resonances | sweep4 | latency : prints one JSON line per row (kernel times: CUDA events in the library,
+    median over the calls after warm-up).  Phase-space points stand in for events where only the work per point
+    matters; every mode cross-checks its NLL against another path."""
+    import torch
+    from paper_1703_03284_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --probe needs a CUDA device")
+
+    def timed(m, p, calls=25, skip=5, grad=False):
+        ms, v = [], None
+        for _ in range(calls):
+            v = m.nll_grad(p)[0] if grad else m.nll(p)
+            ms.append(m.last_kernel_ms())
+        return float(np.median(ms[skip:])), v
+
+    if args.probe == "resonances":
+        # recompute kernel time against the number and spin of the resonances, 10 M + 10 M points, N = 50:
+        # the marginal cost of one resonance against the 2 clk per FP64 instruction of the pipe
+        c = I.Config(3)
+        n = args.events or 10_000_000
+        e12, e13 = I.phase_space_points(n, c.key(7)); g12, g13 = I.phase_space_points(n, c.key(8))
+        d = [torch.from_numpy(a).cuda() for a in (e12, e13, g12, g13)]
+        L1 = [I._res(*I.RHO770), I._res(*I.RHO1450), I._res(*I.SYN_A), I._res(*I.SYN_C)]
+        L2 = [I._res(*I.F2_1270), I._res(*I.SYN_B)]
+        for name, res in (("R=0", []), ("1xL1", L1[:1]), ("2xL1", L1[:2]), ("3xL1", L1[:3]), ("4xL1", L1[:4]),
+                          ("1xL2", L2[:1]), ("2xL2", L2[:2]), ("2xL1+1xL2", L1[:2] + L2[:1])):
+            m = B.Mipwa(c.kin, c.knots, res)
+            m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], None); m.set_path(B.PATH_RECOMPUTE)
+            m.prepare(); m.enable_timing(True)
+            p = np.concatenate([c.truth[:100], np.tile([1.0, 0.3], len(res))])
+            k, v = timed(m, p)
+            print(json.dumps({"probe": "resonances", "model": name, "points": 2 * n, "kernel_ms": k, "nll": v,
+                              "clk_per_warp_point_per_smsp_at_1965MHz": k * 1e-3 * 1.965e9 * 592 / (2 * n / 32)}), flush=True)
+            m.close()
+    elif args.probe == "sweep4":
+        # BASELINE.json configs[4]: K = 56 cached paths against the event count (default 1 M .. 100 M), 10 M-point Gram
+        c = I.Config(4)
+        sizes = [args.events] if args.events else [1_000_000, 2_000_000, 5_000_000, 10_000_000, 20_000_000,
+                                                   50_000_000, 100_000_000]
+        g12, g13 = I.phase_space_points(args.norm_points or 10_000_000, c.key(8))
+        dg = [torch.from_numpy(a).cuda() for a in (g12, g13)]
+        E12, E13 = I.phase_space_points(max(sizes), c.key(7), chunk=1 << 24)
+        m = B.Mipwa(c.kin, c.knots, c.resonances)
+        m.set_norm_points(dg[0], dg[1], None); m.enable_timing(True)
+        for n in sizes:
+            de = [torch.from_numpy(E12[:n]).cuda(), torch.from_numpy(E13[:n]).cuda()]
+            m.set_events(de[0], de[1]); m.prepare()
+            row = {"probe": "sweep4", "n_ev": n, "K": c.N + c.R}
+            for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT)):
+                m.set_path(path)
+                t0 = time.perf_counter(); m.nll(c.truth); setup = time.perf_counter() - t0
+                k, v = timed(m, c.perturbed(1), calls=22, skip=2)
+                byt = m.basis_bytes()
+                row[name] = {"kernel_ms": k, "cache_GB": byt / 1e9, "GB_per_s": byt / k * 1e-6, "events_per_s": n / k * 1e3,
+                             "evals_per_s": 1e3 / k, "first_call_s": setup, "nll": v}
+            if n <= 20_000_000:
+                m.set_path(B.PATH_RECOMPUTE)
+                row["recompute_nll"] = m.nll(c.perturbed(1))
+            print(json.dumps(row), flush=True)
+            del de
+            torch.cuda.empty_cache()
+        m.close()
+    elif args.probe == "latency":
+        # wall clock per call (timing events off) and kernel time at the small configs and at the paper's scale
+        for idx, n_ev, n_norm in ((0, None, None), (1, None, None), (2, 100_000, 1_000_000), (2, None, None)):
+            c = I.Config(idx, n_ev=n_ev, n_norm=n_norm)
+            e12, e13 = I.phase_space_points(c.n_ev, c.key(7))
+            g12, g13, w = c.norm_points()
+            d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (e12, e13, g12, g13, w)]
+            m = B.Mipwa(c.kin, c.knots, c.resonances)
+            m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4]); m.prepare()
+            ps = [c.perturbed(t) for t in range(120)]
+            row = {"probe": "latency", "config": idx, "n_ev": c.n_ev, "n_norm": int(g12.size)}
+            for name, path, grad in (("recompute", B.PATH_RECOMPUTE, False), ("compact", B.PATH_CACHED_COMPACT, False),
+                                     ("dense", B.PATH_CACHED, False), ("grad_recompute", B.PATH_RECOMPUTE, True),
+                                     ("grad_compact", B.PATH_CACHED_COMPACT, True)):
+                m.set_path(path)
+                f = (lambda q: m.nll_grad(q)[0]) if grad else m.nll
+                m.enable_timing(True)
+                km = []
+                for t in range(20):
+                    f(ps[t]); km.append(m.last_kernel_ms())
+                m.enable_timing(False)
+                t0 = time.perf_counter()
+                for t in range(100):
+                    f(ps[20 + t])
+                row[name] = {"wall_us": (time.perf_counter() - t0) / 100 * 1e6, "kernel_us": float(np.median(km[5:])) * 1e3}
+            print(json.dumps(row), flush=True)
+            m.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -374,7 +467,10 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--events", type=int, default=None)
     ap.add_argument("--norm-points", type=int, default=None)
+    ap.add_argument("--probe", default=None, choices=["resonances", "sweep4", "latency"])
     args = ap.parse_args()
+    if args.probe:
+        return run_probe(args)
     args.warmup = max(args.warmup, 3)
     cfg = I.Config(args.config, n_ev=args.events, n_norm=args.norm_points)
     workload = {"workload": f"BASELINE.json configs[{args.config}]: {cfg.N} knots + "

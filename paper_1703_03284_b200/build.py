@@ -12,7 +12,8 @@ NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a",
 
 
 def sources():
-    return sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu*")) + [os.path.join(HERE, "..", "include", "mipwa.h")])
+    return sorted(f for f in glob.glob(os.path.join(HERE, "csrc", "*.cu*")) if not f.endswith("fp64_microbench.cu")) \
+        + [os.path.join(HERE, "..", "include", "mipwa.h")]
 
 
 def build(force=False, verbose=False):
@@ -24,5 +25,17 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def build_microbench():
+    """Stand-alone FP64-pipe microbenchmarks (csrc/fp64_microbench.cu -> ./fp64_microbench); not part of the library."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    out = os.path.join(HERE, "fp64_microbench")
+    subprocess.run([nvcc, "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-o", out,
+                    os.path.join(HERE, "csrc", "fp64_microbench.cu")], check=True)
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--microbench" in sys.argv:
+        print(build_microbench())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
