@@ -431,9 +431,10 @@ def run_probe(args):
         m.close()
     elif args.probe == "latency":
         # wall clock per call (timing events off) and kernel time at the small configs and at the paper's scale
-        for idx, n_ev, n_norm in ((0, None, None), (1, None, None), (2, 100_000, 1_000_000), (2, None, None)):
+        for idx, n_ev, n_norm in ((0, None, None), (1, None, None), (2, 100_000, 1_000_000), (2, None, None),
+                                  (5, None, None)):       # 5 = the paper's own toy (K+K+K-, 100 K events, 918^2 grid)
             c = I.Config(idx, n_ev=n_ev, n_norm=n_norm)
-            e12, e13 = I.phase_space_points(c.n_ev, c.key(7))
+            e12, e13 = I.phase_space_points(c.n_ev, c.key(7), c.kin)
             g12, g13, w = c.norm_points()
             d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (e12, e13, g12, g13, w)]
             m = B.Mipwa(c.kin, c.knots, c.resonances)

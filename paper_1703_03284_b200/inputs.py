@@ -21,6 +21,8 @@ import numpy as np
 M_D = 1.86966          # GeV  (BASELINE.json configs[0])
 M_PI = 0.13957         # GeV
 KIN = {"M": M_D, "m1": M_PI, "m2": M_PI, "m3": M_PI}
+M_K = 0.493677         # GeV; the paper's own decay D+ -> K+ K+ K- 
+KIN_KKK = {"M": M_D, "m1": M_K, "m2": M_K, "m3": M_K}
 KNOT_LO, KNOT_HI = 0.0779, 2.9929          # GeV^2 (BASELINE.json configs[0])
 R_RES, R_PARENT = 1.5, 5.0                 # GeV^-1 (configs[0]; reading P11: the same for every resonance)
 
@@ -232,6 +234,12 @@ _SPECS = {
             norm=("mc", 1_000_000), calls=1000),
     3: dict(knots=lambda: knots_uniform(50), res=[_res(*RHO770, shape_floats=1), _res(*RHO1450), _res(*F2_1270)],
             n_ev=10_000_000, norm=("mc", 10_000_000), calls=1000),
+    # 5: not in BASELINE.json - the paper's own toy: D+ -> K+K+K-, 100 K events, 40 knots (39 slices)
+    # across the whole m^2(K+K-) range + phi(1020), normalisation grid of spacing 0.001 GeV^2 (918 x 918 cells).
+    # The paper prints no parameter values; the knot values follow the same recipe as configs 0-4, phi(1020) takes
+    # its PDG mass and width and the radii of reading P11.
+    5: dict(kin=KIN_KKK, knots=lambda: np.linspace(4 * M_K ** 2, (M_D - M_K) ** 2, 40), res=[_res(1.019461, 0.004249, 1)],
+            n_ev=100_000, norm=("grid", 918), calls=100),
     4: dict(knots=lambda: knots_uniform(50),
             res=[_res(*RHO770), _res(*RHO1450), _res(*F2_1270), _res(*SYN_A), _res(*SYN_B), _res(*SYN_C)],
             n_ev=1_000_000, norm=("mc", 10_000_000), calls=20),
@@ -248,7 +256,7 @@ class Config:
     def __init__(self, idx, seed=1, n_ev=None, n_norm=None):
         spec = _SPECS[idx]
         self.idx, self.seed = idx, seed
-        self.kin = dict(KIN)
+        self.kin = dict(spec.get("kin", KIN))
         self.knots = spec["knots"]()
         self.resonances = [dict(r) for r in spec["res"]]
         self.N, self.R = self.knots.size, len(self.resonances)

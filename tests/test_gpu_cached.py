@@ -21,6 +21,7 @@ CASES = {
     0: dict(),                                    # 10k events (39 tiles + ragged tail), 5954-cell grid
     1: dict(n_ev=40_000, n_norm=50_000),
     2: dict(n_ev=30_011, n_norm=20_003),          # non-uniform knots
+    5: dict(n_ev=30_000),                         # the paper's own toy (K+K+K-, phi(1020), 0.001 GeV^2 grid)
     4: dict(n_ev=20_000, n_norm=20_000),          # K = 56, incl. a narrow resonance
 }
 

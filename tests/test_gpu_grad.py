@@ -25,6 +25,7 @@ CASES = {
     1: dict(n_ev=40_000, n_norm=50_000),
     2: dict(n_ev=30_011, n_norm=20_003),          # non-uniform knots
     3: dict(n_ev=25_000, n_norm=25_000),          # floating rho(770) shape: gradient over the first 2N + 2R
+    5: dict(n_ev=30_000),                         # the paper's own toy (K+K+K-, phi(1020), 0.001 GeV^2 grid)
     4: dict(n_ev=20_000, n_norm=20_000),          # six resonances (run-time resonance loop)
 }
 

@@ -39,6 +39,7 @@ CASES = {
     2: dict(n_ev=30_011, n_norm=20_003),          # non-uniform knots, three resonances
     3: dict(n_ev=25_000, n_norm=25_000),          # floating rho(770) shape
     4: dict(n_ev=20_000, n_norm=20_000),          # six resonances incl. a narrow one
+    5: dict(n_ev=30_000),                         # the paper's own toy: D+ -> K+K+K-, 40 knots + phi(1020), 0.001 GeV^2 grid
 }
 
 

@@ -260,3 +260,29 @@ def test_config_recipes():
     d = c1.perturbed(4) - c1.truth
     assert 2e-4 < d.std() < 3e-3 and np.array_equal(c1.perturbed(4), c1.perturbed(4))
     assert not np.array_equal(c1.perturbed(4), c1.perturbed(5))
+
+
+def test_paper_toy_config_kkk():
+    """Config 5 = the paper's own toy: D+ -> K+K+K-, 40 knots over the whole m^2(K+K-) range + phi(1020),
+    100 K events, grid spacing 0.001 GeV^2.  Recipe checks + the oracle's invariants on the other kinematics."""
+    c = I.Config(5, n_ev=4000)
+    lo, hi = I.s_limits(c.kin)
+    assert c.N == 40 and c.R == 1 and c.knots[0] == pytest.approx(lo) and c.knots[-1] == pytest.approx(hi)
+    assert (hi - lo) / 918 == pytest.approx(0.001, rel=2e-3)                     # grid spacing of PAPER.md:47
+    g12, g13, w = c.norm_points()
+    assert w[0] == pytest.approx(((hi - lo) / 918) ** 2)
+    assert g12.size * w[0] == pytest.approx(I.dalitz_area(c.kin), rel=2e-3)       # grid covers the Dalitz plot
+    o = orc.Oracle(c.kin, c.knots, c.resonances)
+    f = lambda a, b: o.abs2(c.truth, a, b)
+    e12, e13 = c.events(f, I.envelope_of(f, c.kin, n_side=512))
+    assert o.inside(e12, e13).all()
+    # phi(1020) band: a visible excess of events within 3 widths of the pole in either K+K- mass
+    m0, g0 = c.resonances[0]["mass"], c.resonances[0]["width"]
+    band = (np.abs(np.sqrt(e12) - m0) < 3 * g0) | (np.abs(np.sqrt(e13) - m0) < 3 * g0)
+    flat = I.phase_space_points(20000, c.key(9), c.kin)
+    band_flat = (np.abs(np.sqrt(flat[0]) - m0) < 3 * g0) | (np.abs(np.sqrt(flat[1]) - m0) < 3 * g0)
+    assert band.mean() > 3 * band_flat.mean()
+    assert np.array_equal(o.abs2(c.truth, e12, e13), o.abs2(c.truth, e13, e12))
+    p = c.perturbed(0)
+    nll, grad = o.nll_grad(p, e12, e13, g12[::40], g13[::40], w[::40] * 40)
+    assert np.isfinite(nll) and abs(np.sum(grad[c.N:2 * c.N]) + grad[-1]) <= 1e-8 * np.max(np.abs(grad))
