@@ -12,6 +12,7 @@
 #include "kernels.cuh"
 #include "cached.cuh"
 #include "grad.cuh"
+#include "hybrid.cuh"
 
 #include <cub/device/device_radix_sort.cuh>
 
@@ -79,6 +80,16 @@ struct mipwa_ctx {
     std::vector<double> h_gram;     // host copy (K x K complex, row-major) for the cached-path gradient
     bool gram_valid = false;
     int dense_blocks_per_sm = 0, compact_blocks_per_sm = 0;
+
+    // hybrid path: floating resonances recomputed, fixed ones cached (events and normalisation points)
+    const std::vector<int>* active = nullptr;   // resonances (caller's indices, device-slot order) build_model packs; null: perm
+    std::vector<int> hyb_float, hyb_fixed;      // floating: spin 1 first, then spin 2; fixed: caller's order
+    int hyb_f1 = 0, hyb_f2 = 0;
+    bool hyb_ok = false;                        // a k_nll_hybrid instantiation exists for this model
+    void* d_hyb_ev = nullptr; void* d_hyb_nm = nullptr;
+    int64_t hyb_ev_bytes = 0, hyb_nm_bytes = 0;
+    bool hyb_ev_valid = false, hyb_nm_valid = false;
+    int hyb_blocks_per_sm = 0;
 
     // gradient (A8): cell-sorted copies of both point sets, per-block partial vectors
     Slot ev_sorted, nm_sorted;
@@ -236,8 +247,10 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
     for (int q = 0; q < 4; ++q) m.sc[q][N - 1] = make_double2(0.0, 0.0);
     std::vector<int> fidx(R, -1);
     for (int r = 0, f = 0; r < R; ++r) if (c->res[r].shape_floats) fidx[r] = f++;
-    for (int d = 0; d < R; ++d) {
-        const int r = c->perm[d];
+    const std::vector<int>& slots = c->active ? *c->active : c->perm;
+    m.R = (int)slots.size();
+    for (int d = 0; d < (int)slots.size(); ++d) {
+        const int r = slots[d];
         double m0 = c->res[r].mass, g0 = c->res[r].width;
         if (fidx[r] >= 0) { m0 = p[2 * N + 2 * R + 2 * fidx[r]]; g0 = p[2 * N + 2 * R + 2 * fidx[r] + 1]; }
         const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[d], &c->res_fold[d]);
@@ -249,6 +262,7 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
 int use_device(mipwa_ctx* c)
 {
     CU(c, cudaSetDevice(c->device));
+    (void)cudaGetLastError();                              // a stale error of an earlier, unchecked call is not ours to report
     return MIPWA_OK;
 }
 
@@ -315,6 +329,15 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     for (int L : { 1, 2, 0 })
         for (int r = 0; r < n_res; ++r)
             if (res[r].spin == L) { c->perm.push_back(r); ++c->n_spin[L]; }
+    for (int L : { 1, 2 })
+        for (int r = 0; r < n_res; ++r)
+            if (res[r].shape_floats && res[r].spin == L) { c->hyb_float.push_back(r); (L == 1 ? c->hyb_f1 : c->hyb_f2)++; }
+    for (int r = 0; r < n_res; ++r) if (!res[r].shape_floats) c->hyb_fixed.push_back(r);
+    {
+        bool supported = (int)c->hyb_float.size() == c->F && c->F > 0 && !c->hyb_fixed.empty();   // no floating spin 0
+        if (supported) { MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, (int)c->hyb_fixed.size(), (void)0); }
+        c->hyb_ok = supported;
+    }
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
     c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
@@ -366,6 +389,8 @@ void mipwa_destroy(mipwa_ctx* c)
     if (c->owned_cache) cudaFree(c->owned_cache);
     if (c->d_gram) cudaFree(c->d_gram);
     if (c->d_gpartials) cudaFree(c->d_gpartials);
+    if (c->d_hyb_ev) cudaFree(c->d_hyb_ev);
+    if (c->d_hyb_nm) cudaFree(c->d_hyb_nm);
     free_slot(c->ev_sorted); free_slot(c->nm_sorted);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_bad) cudaFreeHost(c->h_bad);
@@ -442,13 +467,13 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
 
 int mipwa_set_events(mipwa_ctx* c, const double* s12, const double* s13, int64_t n, int32_t mem)
 {
-    if (c) { c->cache_valid = false; c->ev_sorted_valid = false; }
+    if (c) { c->cache_valid = false; c->ev_sorted_valid = false; c->hyb_ev_valid = false; }
     return set_slot(c, c->ev, s12, s13, nullptr, n, mem, true);
 }
 
 int mipwa_set_norm_points(mipwa_ctx* c, const double* s12, const double* s13, const double* w, int64_t n, int32_t mem)
 {
-    if (c) { c->gram_valid = false; c->nm_sorted_valid = false; }
+    if (c) { c->gram_valid = false; c->nm_sorted_valid = false; c->hyb_nm_valid = false; }
     return set_slot(c, c->nm, s12, s13, w, n, mem, false);
 }
 
@@ -462,7 +487,9 @@ int mipwa_n_params(const mipwa_ctx* c, int64_t* n)
 int mipwa_set_path(mipwa_ctx* c, int32_t path)
 {
     if (!c) return MIPWA_ERR_ARG;
-    if (path < MIPWA_PATH_AUTO || path > MIPWA_PATH_CACHED_COMPACT) return fail(c, MIPWA_ERR_ARG, "unknown path");
+    if (path < MIPWA_PATH_AUTO || path > MIPWA_PATH_HYBRID) return fail(c, MIPWA_ERR_ARG, "unknown path");
+    if (path == MIPWA_PATH_HYBRID && !c->hyb_ok)
+        return fail(c, MIPWA_ERR_STATE, "the hybrid path needs 1-2 floating spin-1/2 resonances and 1-5 fixed ones");
     if ((path == MIPWA_PATH_CACHED || path == MIPWA_PATH_CACHED_COMPACT) && c->F > 0)
         return fail(c, MIPWA_ERR_STATE, "cached paths need fixed resonance shapes");
     c->path = path;
@@ -490,7 +517,8 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
 static int effective_path(const mipwa_ctx* c)
 {
     if (c->path != MIPWA_PATH_AUTO) return c->path;
-    return c->F == 0 ? MIPWA_PATH_CACHED_COMPACT : MIPWA_PATH_RECOMPUTE;
+    if (c->F == 0) return MIPWA_PATH_CACHED_COMPACT;
+    return c->hyb_ok ? MIPWA_PATH_HYBRID : MIPWA_PATH_RECOMPUTE;
 }
 
 static int64_t cache_bytes_for(const mipwa_ctx* c, int kind, int64_t n)
@@ -521,7 +549,8 @@ static BasisAux basis_aux(const mipwa_ctx* c)
     BasisAux a;
     a.Mx = c->d_Mx;
     std::memset(a.col_of_slot, 0, sizeof(a.col_of_slot));
-    for (int d = 0; d < c->R; ++d) a.col_of_slot[d] = (uint8_t)c->perm[d];
+    if (c->active) for (int d = 0; d < (int)c->active->size(); ++d) a.col_of_slot[d] = (uint8_t)d;   // subset: own order
+    else for (int d = 0; d < c->R; ++d) a.col_of_slot[d] = (uint8_t)c->perm[d];
     return a;
 }
 
@@ -662,6 +691,83 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
     return MIPWA_OK;
 }
 
+// ---- hybrid path: fixed-shape resonances cached per point, floating ones and the spline re-evaluated ---------------------
+static int64_t hyb_bytes_for(const mipwa_ctx* c, int64_t n)
+{
+    const int64_t tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
+    return tiles * MIPWA_TILE * (1 + (int64_t)c->hyb_fixed.size()) * (int64_t)sizeof(double2);
+}
+
+static int ensure_hyb_cache(mipwa_ctx* c, const Slot& pts, void** buf, int64_t* have, bool* valid)
+{
+    if (*valid) return MIPWA_OK;
+    const int64_t need = hyb_bytes_for(c, pts.n);
+    if (*have < need) {
+        if (*buf) cudaFree(*buf);
+        *buf = nullptr; *have = 0;
+        if (need > 0) CU(c, cudaMalloc(buf, (size_t)need));
+        *have = need;
+    }
+    if (pts.n > 0) {
+        c->active = &c->hyb_fixed;                         // unit model of the fixed resonances only
+        int rc = build_unit_model(c, nullptr);
+        const BasisAux aux = basis_aux(c);
+        c->active = nullptr;
+        if (rc) return rc;
+        const int64_t tiles = (pts.n + MIPWA_TILE - 1) / MIPWA_TILE;
+        const int grid = (int)std::min<int64_t>(tiles, (int64_t)c->sm_count * 8);
+        k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, aux, pts.s12, pts.s13, pts.n, (double2*)*buf);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        CU(c, cudaStreamSynchronize(c->stream));
+    }
+    *valid = true;
+    return MIPWA_OK;
+}
+
+static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, double* sum_log, double* integral)
+{
+    int rc = ensure_hyb_cache(c, evs(c), &c->d_hyb_ev, &c->hyb_ev_bytes, &c->hyb_ev_valid);
+    if (rc) return rc;
+    rc = ensure_hyb_cache(c, nms(c), &c->d_hyb_nm, &c->hyb_nm_bytes, &c->hyb_nm_valid);
+    if (rc) return rc;
+    c->active = &c->hyb_float;                             // spline tables + the floating resonances of this call
+    rc = build_model(c, params, n_params);
+    c->active = nullptr;
+    if (rc) return rc;
+    const int N = c->N, RC = (int)c->hyb_fixed.size();
+    HybCoef cc;
+    cc.RC = RC; cc.pad = 0;
+    for (int k = 0; k < RC; ++k) {
+        const int r = c->hyb_fixed[k];
+        cc.c[k] = make_double2(params[2 * N + 2 * r] * std::cos(params[2 * N + 2 * r + 1]),
+                               params[2 * N + 2 * r] * std::sin(params[2 * N + 2 * r + 1]));
+    }
+    bool supported = true;
+    if (!c->hyb_blocks_per_sm) {
+        MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, RC,
+                           supported = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->hyb_blocks_per_sm, k_nll_hybrid<R1, R2, RCT>,
+                                                                                     MIPWA_TILE, 0) == cudaSuccess);
+        if (!supported) return fail(c, MIPWA_ERR_CUDA, "hybrid: occupancy query failed");
+        if (c->hyb_blocks_per_sm < 1) c->hyb_blocks_per_sm = 1;
+    }
+    const int64_t tiles = (std::max(c->ev.n, c->nm.n) + MIPWA_TILE - 1) / MIPWA_TILE;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->hyb_blocks_per_sm));
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, RC,
+                       (k_nll_hybrid<R1, R2, RCT><<<grid, MIPWA_TILE, 0, c->stream>>>(
+                           c->model, cc, (const double2*)c->d_hyb_ev, c->ev.n, (const double2*)c->d_hyb_nm, nms(c).w, c->nm.n,
+                           c->d_partials, c->d_ticket, c->d_result)));
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    *sum_log = c->h_result[0];
+    *integral = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
+    return MIPWA_OK;
+}
+
 int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* sum_log, double* integral)
 {
     if (!c || !params || !nll) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
@@ -672,7 +778,9 @@ int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double
     if (rc) return rc;
     double S = 0, I = 0;
     const int path = effective_path(c);
-    rc = path == MIPWA_PATH_RECOMPUTE ? nll_recompute(c, &S, &I) : nll_cached(c, path, params, &S, &I);
+    if (path == MIPWA_PATH_RECOMPUTE) rc = nll_recompute(c, &S, &I);
+    else if (path == MIPWA_PATH_HYBRID) rc = nll_hybrid(c, params, n_params, &S, &I);
+    else rc = nll_cached(c, path, params, &S, &I);
     if (rc) return rc;
     *nll = -S + (double)c->ev.n * std::log(I);             // A7
     if (sum_log) *sum_log = S;
@@ -756,6 +864,7 @@ int64_t mipwa_basis_bytes(const mipwa_ctx* c)
     const int path = effective_path(c);
     if (path == MIPWA_PATH_RECOMPUTE) return 0;
     if (c->ev.n < 0) return MIPWA_ERR_STATE;
+    if (path == MIPWA_PATH_HYBRID) return hyb_bytes_for(c, c->ev.n) + (c->nm.n > 0 ? hyb_bytes_for(c, c->nm.n) : 0);
     return cache_bytes_for(c, path, c->ev.n);
 }
 
@@ -897,8 +1006,10 @@ static int prepare_sorted(mipwa_ctx* c)
     if (!c->ev_sorted_valid) {
         rc = ensure_sorted(c, c->ev, c->ev_sorted, c->ev_sorted_valid);
         if (rc) return rc;
-        c->cache_valid = false;                            // the per-event cache follows the event order
+        c->cache_valid = false;                            // the per-event caches follow the event order
+        c->hyb_ev_valid = false;
     }
+    if (!c->nm_sorted_valid) c->hyb_nm_valid = false;
     return ensure_sorted(c, c->nm, c->nm_sorted, c->nm_sorted_valid);
 }
 

@@ -146,7 +146,10 @@ def test_cache_management():
             m3.set_path(path)
         assert ei.value.code == B.ERR_STATE
     m3.set_events(d3[0], d3[1]); m3.set_norm_points(d3[2], d3[3], d3[4])
+    assert m3.basis_bytes() == 2 * -(-3000 // 256) * 256 * (1 + 2) * 16        # AUTO -> hybrid: two fixed resonances cached
+    m3.set_path(B.PATH_RECOMPUTE)
     assert m3.basis_bytes() == 0
+    m3.set_path(B.PATH_AUTO)
     ref, sl, integ = o3.nll(c3.truth, *d3, parts=True)
     assert abs(m3.nll(c3.truth) - ref) <= nll_tol(ref, sl, integ, 3000)
     # the basis hook follows floating shapes given in the parameter vector

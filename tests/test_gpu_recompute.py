@@ -225,3 +225,59 @@ def test_prepare_keeps_results_and_hook_order(case):
         m2.prepare()
     assert ei.value.code == B.ERR_STATE
     m2.close()
+
+
+def test_hybrid_path_matches_oracle():
+    """MIPWA_PATH_HYBRID (k_nll_hybrid): floating resonances recomputed, fixed ones cached for events and
+    normalisation points.  configs[3] (rho(770) floats) and models with two floating resonances / spin 2 floating."""
+    B = _lib()
+    from oracle import oracle as orc
+    c, o, data = make_case(3, n_ev=30_011, n_norm=20_003)
+    models = [c.resonances,
+              [dict(c.resonances[0], shape_floats=1), dict(c.resonances[1], shape_floats=1), dict(c.resonances[2])],
+              [dict(c.resonances[0], shape_floats=0), dict(c.resonances[1]), dict(c.resonances[2], shape_floats=1)]]
+    rng = np.random.default_rng(2)
+    for res in models:
+        oo = orc.Oracle(c.kin, c.knots, res)
+        F = sum(r.get("shape_floats", 0) for r in res)
+        shapes = []
+        for r in res:
+            if r.get("shape_floats"):
+                shapes += [r["mass"] * (1 + 0.01 * rng.normal()), r["width"] * (1 + 0.05 * rng.normal())]
+        p = np.concatenate([c.perturbed(1)[:2 * c.N + 2 * c.R], shapes])
+        assert p.size == 2 * c.N + 2 * c.R + 2 * F
+        ref, sl, integ = oo.nll(p, *data, parts=True)
+        tol = nll_tol(ref, sl, integ, data[0].size)
+        for prepared in (False, True):
+            m = B.Mipwa(c.kin, c.knots, res)
+            m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], data[4])
+            if prepared:
+                m.prepare()
+            m.set_path(B.PATH_HYBRID)
+            got, gsl, ginteg = m.nll_parts(p)
+            assert abs(got - ref) <= tol, (got, ref)
+            assert gsl == pytest.approx(sl, rel=1e-12) and ginteg == pytest.approx(integ, rel=1e-12)
+            assert m.nll(p) == got
+            p2 = p.copy(); p2[-2:] *= 1.003                  # shapes move between calls: nothing stale in the cache
+            ref2, sl2, integ2 = oo.nll(p2, *data, parts=True)
+            assert abs(m.nll(p2) - ref2) <= nll_tol(ref2, sl2, integ2, data[0].size)
+            m.set_path(B.PATH_AUTO)                          # AUTO picks the hybrid path here
+            assert m.basis_bytes() > 0 and abs(m.nll(p) - ref) <= tol
+            _, g = m.nll_grad(p)                             # gradient falls back to the recompute kernel
+            _, ref_g = oo.nll_grad(p, *data)
+            assert np.max(np.abs(g - ref_g)) <= 1e-9 * np.max(np.abs(ref_g))
+            m.set_norm_points(data[2][:5000], data[3][:5000], None)     # uniform weights, new normalisation cache
+            ref3, sl3, integ3 = oo.nll(p, data[0], data[1], data[2][:5000], data[3][:5000], None, parts=True)
+            assert abs(m.nll(p) - ref3) <= nll_tol(ref3, sl3, integ3, data[0].size)
+            m.close()
+    # not available without a fixed-shape or without a floating resonance
+    c1, _, _ = make_case(1, n_ev=100, n_norm=100)
+    m = B.Mipwa(c1.kin, c1.knots, c1.resonances)
+    with pytest.raises(B.MipwaError) as ei:
+        m.set_path(B.PATH_HYBRID)
+    assert ei.value.code == B.ERR_STATE
+    m.close()
+    m = B.Mipwa(c.kin, c.knots, [dict(r, shape_floats=1) for r in c.resonances])
+    with pytest.raises(B.MipwaError):
+        m.set_path(B.PATH_HYBRID)
+    m.close()
