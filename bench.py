@@ -35,13 +35,13 @@ UNIT = "events/s"
 # ---- algorithmic work per point: flops of the plain formulas, one per add / mul /
 # div / sqrt / log, fma = 2: two channels x [10 shared kinematics + 14 spline + 37 R] + 4, plus 2 (1 + 3R) divisions,
 # 2 (2 + R) square roots and one log = 59 + 82 R (305 at R = 3).  The kernel as built executes 297 (ncu-counted
-# dadd + dmul + 2 dfma per point, profiles/r1_recompute_ncu.md), so nothing is padded. -------------------------------
+# dadd + dmul + 2 dfma per point, profiles/r1_k_nll_recompute_ncu.md), so nothing is padded. -------------------------------
 def flops_per_point(resonances):
     return 59 + 82 * len(resonances)
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_nll_recompute launch at the bench size (10M events + 10M weighted
-# normalisation points), from the one `ncu --set full` capture summarised in profiles/r1_recompute_ncu.md
+# normalisation points), from the one `ncu --set full` capture summarised in profiles/r1_k_nll_recompute_ncu.md
 NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 404.4e6}
 
 
@@ -346,7 +346,7 @@ def run_ours(args, cfg, workload):
         nominal = 148 * 64 * 2 * clocks["sm_max_mhz"] * 1e6 * 1e-12
     roofline = {"bound": "alu", "kernel": "k_nll_recompute", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((n_ev, n_norm)),
-                "traffic_source": "profiles/r1_recompute_ncu.md (ncu --set full, bytes per launch); algorithmic bytes "
+                "traffic_source": "profiles/r1_k_nll_recompute_ncu.md (ncu --set full, bytes per launch); algorithmic bytes "
                                   "per launch = 16 B x events + 24 B x weighted normalisation points",
                 "peak_source": "measured on this GPU by mipwa_measure_fp64_peak (register-resident DFMA, 2 s sustained); "
                                "MEASURED_PEAKS.json has no FP64 entry; DESIGN.md section 6 derives the nominal peak",
