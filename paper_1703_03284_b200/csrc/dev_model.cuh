@@ -132,12 +132,37 @@ struct Channel {
     double Z[3];      // Zemach factors Z_0 = 1, Z_1, Z_2
 };
 
+// Model flags a kernel can be specialised on (decided on the host once per model, mipwa_create):
+//   MIPWA_FL_EQM  m1 == m2 (pi+pi-pi+, K+K-K+): lam1 = x (x - 4 m^2), so ql = x - 4 m^2 needs no reciprocal, kappa = 0,
+//                 and 2g = sqrt(ql / x) = ql rsqrt(ql x): the channel needs no 1/x at all
+//                 (Z2's ql pl = ql lam2 / x = (2g)^2 lam2)
+//   MIPWA_FL_SHR  every resonance of one spin has the same r_res and r_parent (the usual choice, e.g. 1.5 and
+//                 5 GeV^-1 for all): the barrier denominators D_R, D_D and rsqrt(D_R D_D) are per spin and channel
+#define MIPWA_FL_EQM 1
+#define MIPWA_FL_SHR 2
+
+template <int FL = 0>
 __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, double y)
 {
     Channel c;
     c.x = x;
-    const double lam1 = (x - m.t_lo) * (x - m.t_d);
     c.lam2 = (m.s_hi - x) * (m.s_top - x);
+    c.Z[0] = 1.0;
+    if (FL & MIPWA_FL_EQM) {
+        // ql clamped at 0 and lam1 + 1e-300: a point within rounding below threshold gives width 0, not NaN
+        c.ql = fmax(x - m.t_lo, 0.0);
+        const double lc = fma(c.ql, x, 1e-300);
+        double y0;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(lc));
+        const double u = c.ql * y0, e = fma(-(lc * y0), y0, 1.0);      // ql rsqrt(lc), refinement merged in
+        c.w[0] = fma(u * e, fma(0.375, e, 0.5), u);
+        c.w[1] = c.w[0] * c.ql;
+        c.w[2] = c.w[1] * c.ql;
+        c.Z[1] = fma(2.0, y, x) - m.sigma;
+        c.Z[2] = fma(c.Z[1], c.Z[1], (c.w[0] * c.w[0]) * (c.lam2 * (-1.0 / 3.0)));
+        return c;
+    }
+    const double lam1 = (x - m.t_lo) * (x - m.t_d);
     const double ix = fast_rcp(x);
     c.ql = lam1 * ix;
     const double pl = c.lam2 * ix;
@@ -153,7 +178,6 @@ __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, dou
     c.w[0] = sq * ix;
     c.w[1] = c.w[0] * c.ql;
     c.w[2] = c.w[1] * c.ql;
-    c.Z[0] = 1.0;
     c.Z[1] = fma(m.kappa, ix, fma(2.0, y, x) - m.sigma);
     c.Z[2] = fma(c.Z[1], c.Z[1], (-1.0 / 3.0) * (c.ql * pl));
     return c;
@@ -218,11 +242,48 @@ __device__ __forceinline__ void add_resonance(const ResDev& rd, const Channel& c
     aim = fma(rd.cre, ti, fma(rd.cim, tr, aim));
 }
 
+// MIPWA_FL_SHR: NR >= 2 resonances of spin LT (1 or 2) with common radii.  Per channel ONE barrier block
+// (D_R, D_D, rsqrt(D_R D_D), times Z_L D_R), then per resonance F_D F_R Z BW / sqrt(n_R n_D) = [Z D_R rsqrt(D_R D_D)]
+// (dD + i W') / E with one reciprocal of E = dD^2 + W'^2 (three DFMAs after the seed) instead of the five-instruction
+// reciprocal square root of D_R D_D E^2.
+template <int LT>
+__device__ __forceinline__ void group_barrier(const ResDev& r, const Channel& c, double& DR, double& FZ)
+{
+    double DD;
+    if (LT == 1) {
+        DR = fma(r.cR, c.ql, 1.0);
+        DD = fma(r.cD, c.lam2, 1.0);
+    } else {
+        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
+        DR = fma(zR, zR + 3.0, 9.0);
+        DD = fma(zD, zD + 3.0, 9.0);
+    }
+    FZ = (c.Z[LT] * DR) * fast_rsqrt(DR * DD);
+}
+
+template <int LT, int NR>
+__device__ __forceinline__ void add_group_shared(const ResDev* rd, const Channel& ca, const Channel& cb, double& are,
+                                                 double& aim)
+{
+    double DRa, FZa, DRb, FZb;
+    group_barrier<LT>(rd[0], ca, DRa, FZa);
+    group_barrier<LT>(rd[0], cb, DRb, FZb);
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+        const double Wa = rd[r].Kw * ca.w[LT], Wb = rd[r].Kw * cb.w[LT];
+        const double da = (rd[r].m0sq - ca.x) * DRa, db = (rd[r].m0sq - cb.x) * DRb;
+        const double ta = FZa * fast_rcp(fma(da, da, Wa * Wa)), tb = FZb * fast_rcp(fma(db, db, Wb * Wb));
+        const double tr = fma(ta, da, tb * db), ti = fma(ta, Wa, tb * Wb);
+        are = fma(rd[r].cre, tr, fma(-rd[r].cim, ti, are));
+        aim = fma(rd[r].cre, ti, fma(rd[r].cim, tr, aim));
+    }
+}
+
 // A(s12,s13) = S(s12) + S(s13) + sum_r c_r [T_r(s12,s13) + T_r(s13,s12)]
 // Model signature <R1, R2>: the host orders the resonances spin 1 first (R1 of them), then spin 2 (R2), so that
 // the whole sum unrolls with compile-time spins and constants straight from the parameter bank (2 (R1 + R2)
-// independent chains).  <-1, -1>: any list (incl. spin 0), run-time loop over m.R.
-template <int R1, int R2>
+// independent chains).  <-1, -1>: any list (incl. spin 0), run-time loop over m.R.  FL: MIPWA_FL_* of the model.
+template <int R1, int R2, int FL = 0>
 __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& m, double s12, double s13,
                                           double& are, double& aim)
 {
@@ -232,12 +293,20 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
     are = r1 + r2;
     aim = i1 + i2;
     if (R1 == 0 && R2 == 0) return;
-    const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
+    const Channel ca = make_channel<FL>(m, s12, s13), cb = make_channel<FL>(m, s13, s12);
     if (R1 >= 0) {
+        if ((FL & MIPWA_FL_SHR) && R1 >= 2) {
+            add_group_shared<1, (R1 >= 2 ? R1 : 2)>(&m.res[0], ca, cb, are, aim);
+        } else {
 #pragma unroll
-        for (int r = 0; r < R1; ++r) add_resonance<1>(m.res[r], ca, cb, are, aim);
+            for (int r = 0; r < R1; ++r) add_resonance<1>(m.res[r], ca, cb, are, aim);
+        }
+        if ((FL & MIPWA_FL_SHR) && R2 >= 2) {
+            add_group_shared<2, (R2 >= 2 ? R2 : 2)>(&m.res[R1 > 0 ? R1 : 0], ca, cb, are, aim);
+        } else {
 #pragma unroll
-        for (int r = 0; r < R2; ++r) add_resonance<2>(m.res[R1 + r], ca, cb, are, aim);
+            for (int r = 0; r < R2; ++r) add_resonance<2>(m.res[R1 + r], ca, cb, are, aim);
+        }
     } else {
         for (int r = 0; r < m.R; ++r) add_resonance<-1>(m.res[r], ca, cb, are, aim);
     }
@@ -264,4 +333,37 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
         case 33: { constexpr int R1 = 4, R2 = 1; CALL; } break;                                   \
         case 34: { constexpr int R1 = 4, R2 = 2; CALL; } break;                                   \
         default: { constexpr int R1 = -1, R2 = -1; CALL; } break;                                 \
+    }
+
+// As MIPWA_DISPATCH_SIG, with constexpr FL = the model's MIPWA_FL_* flags as far as the signature can use them
+// (MIPWA_FL_SHR only where a spin group has two or more members; none on the run-time <-1,-1> form).
+#define MIPWA_FL_CASES(r1, r2, fl, CALL)                                                          \
+    {                                                                                             \
+        constexpr int R1 = (r1), R2 = (r2);                                                       \
+        constexpr bool shr_useful = (r1) >= 2 || (r2) >= 2;                                       \
+        switch (shr_useful ? ((fl) & 3) : ((fl) & MIPWA_FL_EQM)) {                                \
+            case 0: { constexpr int FL = 0; CALL; } break;                                        \
+            case 1: { constexpr int FL = MIPWA_FL_EQM; CALL; } break;                             \
+            case 2: { constexpr int FL = shr_useful ? MIPWA_FL_SHR : 0; CALL; } break;            \
+            default: { constexpr int FL = shr_useful ? (MIPWA_FL_EQM | MIPWA_FL_SHR) : MIPWA_FL_EQM; CALL; } break; \
+        }                                                                                         \
+    }
+#define MIPWA_DISPATCH_SIGFL(n0, n1, n2, fl, CALL)                                                \
+    switch (((n0) == 0 && (n1) <= MIPWA_SIG_MAX1 && (n2) <= MIPWA_SIG_MAX2) ? (n1) * 8 + (n2) : -1) { \
+        case 0: MIPWA_FL_CASES(0, 0, 0, CALL) break;                                              \
+        case 1: MIPWA_FL_CASES(0, 1, fl, CALL) break;                                             \
+        case 2: MIPWA_FL_CASES(0, 2, fl, CALL) break;                                             \
+        case 8: MIPWA_FL_CASES(1, 0, fl, CALL) break;                                             \
+        case 9: MIPWA_FL_CASES(1, 1, fl, CALL) break;                                             \
+        case 10: MIPWA_FL_CASES(1, 2, fl, CALL) break;                                            \
+        case 16: MIPWA_FL_CASES(2, 0, fl, CALL) break;                                            \
+        case 17: MIPWA_FL_CASES(2, 1, fl, CALL) break;                                            \
+        case 18: MIPWA_FL_CASES(2, 2, fl, CALL) break;                                            \
+        case 24: MIPWA_FL_CASES(3, 0, fl, CALL) break;                                            \
+        case 25: MIPWA_FL_CASES(3, 1, fl, CALL) break;                                            \
+        case 26: MIPWA_FL_CASES(3, 2, fl, CALL) break;                                            \
+        case 32: MIPWA_FL_CASES(4, 0, fl, CALL) break;                                            \
+        case 33: MIPWA_FL_CASES(4, 1, fl, CALL) break;                                            \
+        case 34: MIPWA_FL_CASES(4, 2, fl, CALL) break;                                            \
+        default: { constexpr int R1 = -1, R2 = -1, FL = 0; CALL; } break;                         \
     }

@@ -72,7 +72,7 @@ struct LogProd {
 // event), then over normalisation points.  Block partials go to partials[block] = (sum ln|A|^2, sum w|A|^2); the
 // last block to finish adds them in block order (fixed order: bit-reproducible for a given grid) and writes the
 // two totals to `result` (mapped pinned host memory).
-template <int R1, int R2>
+template <int R1, int R2, int FL>
 __global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_MINBLOCKS)
 k_nll_recompute(const __grid_constant__ DevModel m,
                 const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
@@ -112,7 +112,7 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 double re, im;
-                amplitude<R1, R2>(sm, m, a[q], b[q], re, im);
+                amplitude<R1, R2, FL>(sm, m, a[q], b[q], re, im);
                 v[q] = fma(re, re, im * im);
             }
 #pragma unroll
@@ -142,7 +142,7 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 double re, im;
-                amplitude<R1, R2>(sm, m, a[q], b[q], re, im);
+                amplitude<R1, R2, FL>(sm, m, a[q], b[q], re, im);
                 integ = fma(w[q], fma(re, re, im * im), integ);
             }
 #pragma unroll
@@ -176,7 +176,7 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 }
 
 // ---- test hook: |A|^2 per point from the same device function ---------------------------------------------------
-template <int R1, int R2>
+template <int R1, int R2, int FL>
 __global__ void __launch_bounds__(MIPWA_BLOCK)
 k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
        long long n, double* __restrict__ out)
@@ -186,7 +186,7 @@ k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         double re, im;
-        amplitude<R1, R2>(sm, m, s12[i], s13[i], re, im);
+        amplitude<R1, R2, FL>(sm, m, s12[i], s13[i], re, im);
         out[i] = fma(re, re, im * im);
     }
 }

@@ -38,6 +38,7 @@ struct mipwa_ctx {
     std::vector<double> knots;
     std::vector<mipwa_resonance> res;
     int n_spin[3] = { 0, 0, 0 };   // resonances of spin 0, 1, 2 (the kernel signature)
+    int model_flags = 0;           // MIPWA_FL_*: equal daughter masses m1 == m2; radii shared within each spin
     std::vector<int> perm;          // device slot d holds resonance perm[d]: spin 1 first, then spin 2, then spin 0
     int device = 0;
     int sm_count = 0;
@@ -338,6 +339,18 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
         if (supported) { MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, (int)c->hyb_fixed.size(), (void)0); }
         c->hyb_ok = supported;
     }
+    if (kin->m1 == kin->m2) c->model_flags |= MIPWA_FL_EQM;
+    {
+        bool shared = true;
+        for (int a = 0; a < n_res; ++a)
+            for (int b = a + 1; b < n_res; ++b)
+                if (res[a].spin == res[b].spin && (res[a].r_res != res[b].r_res || res[a].r_parent != res[b].r_parent))
+                    shared = false;
+        if (shared) c->model_flags |= MIPWA_FL_SHR;
+    }
+#ifdef MIPWA_NO_MODEL_FLAGS
+    c->model_flags = 0;                                    // experiments only
+#endif
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
     c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
@@ -354,8 +367,8 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     }
 
     bool ok = true;
-    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
-                       ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute<R1, R2>,
+    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
+                       ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute<R1, R2, FL>,
                                                                           MIPWA_BLOCK, 0) == cudaSuccess);
     if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
 #ifdef MIPWA_FORCE_BPS
@@ -500,7 +513,7 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
 {
     const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->blocks_per_sm);
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2], (k_nll_recompute<R1, R2><<<grid, MIPWA_BLOCK, 0, c->stream>>>(
+    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags, (k_nll_recompute<R1, R2, FL><<<grid, MIPWA_BLOCK, 0, c->stream>>>(
                                c->model, evs(c).s12, evs(c).s13, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w, nms(c).n,
                                c->d_partials, c->d_ticket, c->d_result)));
     ++c->launches;
@@ -806,8 +819,8 @@ int mipwa_eval_abs2(mipwa_ctx* c, const double* params, int64_t n_params, int32_
     if (n == 0) return MIPWA_OK;
     double* d_out = nullptr;
     CU(c, cudaMalloc(&d_out, (size_t)n * sizeof(double)));
-    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
-                       (k_abs2<R1, R2><<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, n, d_out)));
+    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
+                       (k_abs2<R1, R2, FL><<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, n, d_out)));
     ++c->launches;
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
