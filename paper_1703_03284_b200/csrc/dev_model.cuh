@@ -125,6 +125,16 @@ __device__ __forceinline__ void spline_eval(const SplineSmem& sm, const DevModel
     im = fma(t, fma(t, fma(t, c3.y, c2.y), c1.y), c0.y);
 }
 
+// spline value on a known segment j (the segment pair of every point is computed once per point set, by the
+// boundary-check kernel of mipwa_set_*, and stored as one uint16 per point: j12 | j13 << 8)
+__device__ __forceinline__ void spline_eval_at(const SplineSmem& sm, double s, int j, double& re, double& im)
+{
+    const double t = s - sm.knots[j];
+    const double2 c0 = sm.sc[0][j], c1 = sm.sc[1][j], c2 = sm.sc[2][j], c3 = sm.sc[3][j];
+    re = fma(t, fma(t, fma(t, c3.x, c2.x), c1.x), c0.x);
+    im = fma(t, fma(t, fma(t, c3.y, c2.y), c1.y), c0.y);
+}
+
 // per-channel kinematic quantities shared by all resonances
 struct Channel {
     double x, lam2, ql;
@@ -284,14 +294,8 @@ __device__ __forceinline__ void add_group_shared(const ResDev* rd, const Channel
 // the whole sum unrolls with compile-time spins and constants straight from the parameter bank (2 (R1 + R2)
 // independent chains).  <-1, -1>: any list (incl. spin 0), run-time loop over m.R.  FL: MIPWA_FL_* of the model.
 template <int R1, int R2, int FL = 0>
-__device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& m, double s12, double s13,
-                                          double& are, double& aim)
+__device__ __forceinline__ void add_resonances(const DevModel& m, double s12, double s13, double& are, double& aim)
 {
-    double r1, i1, r2, i2;
-    spline_eval(sm, m, s12, r1, i1);
-    spline_eval(sm, m, s13, r2, i2);
-    are = r1 + r2;
-    aim = i1 + i2;
     if (R1 == 0 && R2 == 0) return;
     const Channel ca = make_channel<FL>(m, s12, s13), cb = make_channel<FL>(m, s13, s12);
     if (R1 >= 0) {
@@ -310,6 +314,31 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
     } else {
         for (int r = 0; r < m.R; ++r) add_resonance<-1>(m.res[r], ca, cb, are, aim);
     }
+}
+
+template <int R1, int R2, int FL = 0>
+__device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& m, double s12, double s13,
+                                          double& are, double& aim)
+{
+    double r1, i1, r2, i2;
+    spline_eval(sm, m, s12, r1, i1);
+    spline_eval(sm, m, s13, r2, i2);
+    are = r1 + r2;
+    aim = i1 + i2;
+    add_resonances<R1, R2, FL>(m, s12, s13, are, aim);
+}
+
+// the same with the segment pair of the point known (seg = j12 | j13 << 8)
+template <int R1, int R2, int FL = 0>
+__device__ __forceinline__ void amplitude_seg(const SplineSmem& sm, const DevModel& m, double s12, double s13,
+                                              unsigned int seg, double& are, double& aim)
+{
+    double r1, i1, r2, i2;
+    spline_eval_at(sm, s12, (int)(seg & 0xffu), r1, i1);
+    spline_eval_at(sm, s13, (int)(seg >> 8), r2, i2);
+    are = r1 + r2;
+    aim = i1 + i2;
+    add_resonances<R1, R2, FL>(m, s12, s13, are, aim);
 }
 
 #define MIPWA_SIG_MAX1 4

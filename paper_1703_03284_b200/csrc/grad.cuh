@@ -291,28 +291,26 @@ k_grad_finalize(const double* __restrict__ partials, int nblocks, int NV, double
 
 // ---- cell sort (once per point set): key = seg(s12) * (N-1) + seg(s13) ---------------------------------------------
 __global__ void __launch_bounds__(MIPWA_TILE)
-k_cell_keys(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
-            long long n, unsigned int* __restrict__ keys, unsigned int* __restrict__ idx)
+k_cell_keys(const unsigned short* __restrict__ seg, long long n, int NS, unsigned int* __restrict__ keys,
+            unsigned int* __restrict__ idx)
 {
-    __shared__ SplineSmem sm;
-    load_spline_smem(sm, m);
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        double xj;
-        const int j1 = spline_segment(sm, m, s12[i], xj), j2 = spline_segment(sm, m, s13[i], xj);
-        keys[i] = (unsigned int)(j1 * (m.N - 1) + j2);
+        const unsigned int sg = seg[i];                    // j12 | j13 << 8, stored by k_validate
+        keys[i] = (sg & 0xffu) * (unsigned int)NS + (sg >> 8);
         idx[i] = (unsigned int)i;
     }
 }
 
 __global__ void __launch_bounds__(MIPWA_TILE)
 k_gather(const unsigned int* __restrict__ idx, long long n, const double* __restrict__ a, const double* __restrict__ b,
-         const double* __restrict__ c, double* __restrict__ oa, double* __restrict__ ob, double* __restrict__ oc)
+         const double* __restrict__ c, const unsigned short* __restrict__ sg, double* __restrict__ oa,
+         double* __restrict__ ob, double* __restrict__ oc, unsigned short* __restrict__ osg)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         const unsigned int s = idx[i];
-        oa[i] = a[s]; ob[i] = b[s];
+        oa[i] = a[s]; ob[i] = b[s]; osg[i] = sg[s];
         if (c) oc[i] = c[s];
     }
 }

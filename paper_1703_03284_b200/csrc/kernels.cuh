@@ -75,9 +75,10 @@ struct LogProd {
 template <int R1, int R2, int FL>
 __global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_MINBLOCKS)
 k_nll_recompute(const __grid_constant__ DevModel m,
-                const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
+                const double* __restrict__ e12, const double* __restrict__ e13, const unsigned short* __restrict__ eseg,
+                long long n_ev,
                 const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
-                long long n_norm, double2* __restrict__ partials, unsigned int* __restrict__ ticket,
+                const unsigned short* __restrict__ gseg, long long n_norm, double2* __restrict__ partials, unsigned int* __restrict__ ticket,
                 double* __restrict__ result)
 {
     __shared__ SplineSmem sm;
@@ -94,59 +95,63 @@ k_nll_recompute(const __grid_constant__ DevModel m,
     LogProd lp;
     {
         double a[PTS], b[PTS];
+        unsigned int sg[PTS];
 #pragma unroll
         for (int q = 0; q < PTS; ++q) {
             const long long i = t0 + q * stride;
-            a[q] = 1.0; b[q] = 1.0;
-            if (i < n_ev) { a[q] = e12[i]; b[q] = e13[i]; }
+            a[q] = 1.0; b[q] = 1.0; sg[q] = 0u;
+            if (i < n_ev) { a[q] = e12[i]; b[q] = e13[i]; sg[q] = eseg[i]; }
         }
         for (long long i = t0; i < n_ev; i += PTS * stride) {
             double na[PTS], nb[PTS];
+            unsigned int ns[PTS];
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 const long long nx = i + (PTS + q) * stride;
-                na[q] = 1.0; nb[q] = 1.0;
-                if (nx < n_ev) { na[q] = e12[nx]; nb[q] = e13[nx]; }
+                na[q] = 1.0; nb[q] = 1.0; ns[q] = 0u;
+                if (nx < n_ev) { na[q] = e12[nx]; nb[q] = e13[nx]; ns[q] = eseg[nx]; }
             }
             double v[PTS];
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 double re, im;
-                amplitude<R1, R2, FL>(sm, m, a[q], b[q], re, im);
+                amplitude_seg<R1, R2, FL>(sm, m, a[q], b[q], sg[q], re, im);
                 v[q] = fma(re, re, im * im);
             }
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 lp.add(i + q * stride < n_ev ? v[q] : 1.0);
-                a[q] = na[q]; b[q] = nb[q];
+                a[q] = na[q]; b[q] = nb[q]; sg[q] = ns[q];
             }
         }
     }
     double integ = 0.0;
     {
         double a[PTS], b[PTS], w[PTS];
+        unsigned int sg[PTS];
 #pragma unroll
         for (int q = 0; q < PTS; ++q) {
             const long long j = t0 + q * stride;
-            a[q] = 1.0; b[q] = 1.0; w[q] = 0.0;
-            if (j < n_norm) { a[q] = g12[j]; b[q] = g13[j]; w[q] = gw ? gw[j] : 1.0; }
+            a[q] = 1.0; b[q] = 1.0; w[q] = 0.0; sg[q] = 0u;
+            if (j < n_norm) { a[q] = g12[j]; b[q] = g13[j]; w[q] = gw ? gw[j] : 1.0; sg[q] = gseg[j]; }
         }
         for (long long j = t0; j < n_norm; j += PTS * stride) {
             double na[PTS], nb[PTS], nw[PTS];
+            unsigned int ns[PTS];
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 const long long nx = j + (PTS + q) * stride;
-                na[q] = 1.0; nb[q] = 1.0; nw[q] = 0.0;
-                if (nx < n_norm) { na[q] = g12[nx]; nb[q] = g13[nx]; nw[q] = gw ? gw[nx] : 1.0; }
+                na[q] = 1.0; nb[q] = 1.0; nw[q] = 0.0; ns[q] = 0u;
+                if (nx < n_norm) { na[q] = g12[nx]; nb[q] = g13[nx]; nw[q] = gw ? gw[nx] : 1.0; ns[q] = gseg[nx]; }
             }
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 double re, im;
-                amplitude<R1, R2, FL>(sm, m, a[q], b[q], re, im);
+                amplitude_seg<R1, R2, FL>(sm, m, a[q], b[q], sg[q], re, im);
                 integ = fma(w[q], fma(re, re, im * im), integ);
             }
 #pragma unroll
-            for (int q = 0; q < PTS; ++q) { a[q] = na[q]; b[q] = nb[q]; w[q] = nw[q]; }
+            for (int q = 0; q < PTS; ++q) { a[q] = na[q]; b[q] = nb[q]; w[q] = nw[q]; sg[q] = ns[q]; }
         }
     }
 
@@ -179,14 +184,14 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 template <int R1, int R2, int FL>
 __global__ void __launch_bounds__(MIPWA_BLOCK)
 k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
-       long long n, double* __restrict__ out)
+       const unsigned short* __restrict__ seg, long long n, double* __restrict__ out)
 {
     __shared__ SplineSmem sm;
     load_spline_smem(sm, m);
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         double re, im;
-        amplitude<R1, R2, FL>(sm, m, s12[i], s13[i], re, im);
+        amplitude_seg<R1, R2, FL>(sm, m, s12[i], s13[i], seg[i], re, im);
         out[i] = fma(re, re, im * im);
     }
 }
@@ -196,10 +201,15 @@ k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const
 // points that the caller's own fp64 boundary test placed exactly on the edge.  Counts offenders into *bad.
 struct DevKin { double M2, m1s, m2s, m3s, t_lo, t_d, s_hi, s_top; };
 
+// Also stores the spline segment pair of every point, seg[i] = j12 | j13 << 8 (knots are fixed at mipwa_create, so
+// the pair is a property of the point set): the per-call kernels then index the coefficient tables directly.
 __global__ void __launch_bounds__(MIPWA_BLOCK)
-k_validate(const DevKin k, const double* __restrict__ s12, const double* __restrict__ s13, long long n,
+k_validate(const DevKin k, const __grid_constant__ DevModel m, const double* __restrict__ s12,
+           const double* __restrict__ s13, long long n, unsigned short* __restrict__ seg,
            unsigned long long* __restrict__ bad)
 {
+    __shared__ SplineSmem sm;
+    load_spline_smem(sm, m);
     const long long stride = (long long)gridDim.x * blockDim.x;
     unsigned int mine = 0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
@@ -213,6 +223,9 @@ k_validate(const DevKin k, const double* __restrict__ s12, const double* __restr
             ok = fabs(y - centre) <= half + slack * (fabs(centre) + half) + 1e-13;
         }
         mine += ok ? 0u : 1u;                             // NaN compares false above -> counted as bad
+        double xj;
+        const int j1 = spline_segment(sm, m, x, xj), j2 = spline_segment(sm, m, y, xj);
+        seg[i] = (unsigned short)(j1 | (j2 << 8));
     }
     mine = __reduce_add_sync(0xffffffffu, mine);
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(bad, (unsigned long long)mine);

@@ -26,8 +26,9 @@ struct Slot {                       // events or normalisation points
     const double* s12 = nullptr;
     const double* s13 = nullptr;
     const double* w = nullptr;
+    const unsigned short* seg = nullptr;   // spline segment pair per point, j12 | j13 << 8 (always library-owned)
     int64_t n = -1;                 // -1: not set
-    void* owned[3] = { nullptr, nullptr, nullptr };
+    void* owned[4] = { nullptr, nullptr, nullptr, nullptr };   // s12, s13, w, seg
 };
 
 }  // namespace
@@ -205,17 +206,13 @@ void spline_factor(mipwa_ctx* c)
     }
 }
 
-// A1-A3: parameters -> DevModel
-int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
+// the parameter-independent part of DevModel (kinematics, knots, bucket table): valid from mipwa_create on, so that
+// k_validate can compute segment pairs before any likelihood call
+void fill_static_model(mipwa_ctx* c)
 {
-    const int N = c->N, R = c->R;
-    if (n_params != 2 * N + 2 * R + 2 * c->F)
-        return fail(c, MIPWA_ERR_ARG, "n_params must be " + std::to_string(2 * N + 2 * R + 2 * c->F));
-    for (int64_t i = 0; i < n_params; ++i)
-        if (!std::isfinite(p[i])) return fail(c, MIPWA_ERR_ARG, "non-finite parameter " + std::to_string(i));
     DevModel& m = c->model;
     const mipwa_kinematics& k = c->kin;
-    m.N = N; m.R = R; m.nlut = c->nlut; m.lut_exact = c->lut_exact ? 1 : 0;
+    m.N = c->N; m.R = c->R; m.nlut = c->nlut; m.lut_exact = c->lut_exact ? 1 : 0;
     m.t_lo = (k.m1 + k.m2) * (k.m1 + k.m2);
     m.t_d = (k.m1 - k.m2) * (k.m1 - k.m2);
     m.s_hi = (k.m_parent - k.m3) * (k.m_parent - k.m3);
@@ -225,8 +222,20 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
     m.lut_off = -c->lut_x0 * c->lut_inv; m.lut_inv = c->lut_inv;
     std::memcpy(m.lut, c->lut.data(), c->nlut);
     std::memcpy(m.xk, c->xk.data(), c->nlut * sizeof(double));
+    for (int i = 0; i < c->N; ++i) m.knots[i] = c->knots[i];
+}
+
+// A1-A3: parameters -> DevModel
+int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
+{
+    const int N = c->N, R = c->R;
+    if (n_params != 2 * N + 2 * R + 2 * c->F)
+        return fail(c, MIPWA_ERR_ARG, "n_params must be " + std::to_string(2 * N + 2 * R + 2 * c->F));
+    for (int64_t i = 0; i < n_params; ++i)
+        if (!std::isfinite(p[i])) return fail(c, MIPWA_ERR_ARG, "non-finite parameter " + std::to_string(i));
+    DevModel& m = c->model;
+    fill_static_model(c);
     for (int i = 0; i < N; ++i) {
-        m.knots[i] = c->knots[i];
         c->y_re[i] = p[i] * std::cos(p[N + i]);            // y_k = a_k e^{i phi_k}
         c->y_im[i] = p[i] * std::sin(p[N + i]);
     }
@@ -356,6 +365,7 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
     spline_factor(c);
     std::memset(&c->model, 0, sizeof(DevModel));
+    fill_static_model(c);
     c->Mx.assign((size_t)n_knots * n_knots, 0.0);          // column k = second derivatives of the cardinal spline k
     {
         std::vector<double> e(n_knots), pp(n_knots);
@@ -437,8 +447,10 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
     CU(c, cudaStreamSynchronize(c->stream));
     Slot s;
     if (mem == MIPWA_MEM_HOST && n > 0 && slot.n == n && slot.owned[0] && slot.owned[1]) {
-        for (int q = 0; q < 3; ++q) { s.owned[q] = slot.owned[q]; slot.owned[q] = nullptr; }   // same size: reuse
+        for (int q = 0; q < 4; ++q) { s.owned[q] = slot.owned[q]; slot.owned[q] = nullptr; }   // same size: reuse
         if (!w && s.owned[2]) { cudaFree(s.owned[2]); s.owned[2] = nullptr; }
+    } else if (n > 0 && slot.n == n && slot.owned[3]) {
+        s.owned[3] = slot.owned[3]; slot.owned[3] = nullptr;                                    // segment pairs: reuse
     }
     free_slot(slot);
     if (mem == MIPWA_MEM_HOST && n > 0) {
@@ -457,13 +469,22 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
         s.s12 = s12; s.s13 = s13; s.w = w;
     }
     s.n = n;
+    if (n > 0 && !s.owned[3]) {
+        cudaError_t e = cudaMalloc(&s.owned[3], (size_t)n * sizeof(unsigned short));
+        if (e != cudaSuccess) {
+            free_slot(s);
+            return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, cudaGetErrorString(e));
+        }
+    }
+    s.seg = (const unsigned short*)s.owned[3];
     if (n > 0) {                                           // boundary check on the device (north_star invariant)
         const mipwa_kinematics& k = c->kin;
         DevKin dk = { k.m_parent * k.m_parent, k.m1 * k.m1, k.m2 * k.m2, k.m3 * k.m3,
                       (k.m1 + k.m2) * (k.m1 + k.m2), (k.m1 - k.m2) * (k.m1 - k.m2),
                       (k.m_parent - k.m3) * (k.m_parent - k.m3), (k.m_parent + k.m3) * (k.m_parent + k.m3) };
         *c->h_bad = 0;
-        k_validate<<<grid_for(c, n, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, s.s12, s.s13, n, c->d_bad);
+        k_validate<<<grid_for(c, n, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, c->model, s.s12, s.s13, n,
+                                                                     (unsigned short*)s.owned[3], c->d_bad);
         ++c->launches;
         cudaError_t e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
@@ -514,8 +535,8 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->blocks_per_sm);
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
     MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags, (k_nll_recompute<R1, R2, FL><<<grid, MIPWA_BLOCK, 0, c->stream>>>(
-                               c->model, evs(c).s12, evs(c).s13, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w, nms(c).n,
-                               c->d_partials, c->d_ticket, c->d_result)));
+                               c->model, evs(c).s12, evs(c).s13, evs(c).seg, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w,
+                               nms(c).seg, nms(c).n, c->d_partials, c->d_ticket, c->d_result)));
     ++c->launches;
     CU(c, cudaGetLastError());
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
@@ -820,7 +841,7 @@ int mipwa_eval_abs2(mipwa_ctx* c, const double* params, int64_t n_params, int32_
     double* d_out = nullptr;
     CU(c, cudaMalloc(&d_out, (size_t)n * sizeof(double)));
     MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
-                       (k_abs2<R1, R2, FL><<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, n, d_out)));
+                       (k_abs2<R1, R2, FL><<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, s.seg, n, d_out)));
     ++c->launches;
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
@@ -982,7 +1003,7 @@ static int ensure_sorted(mipwa_ctx* c, const Slot& src, Slot& dst, bool& valid)
         int bits = 1;
         while ((1LL << bits) < (int64_t)(c->N - 1) * (c->N - 1)) ++bits;
         cudaError_t e = cudaSuccess;
-        k_cell_keys<<<grid_for(c, n, 8), MIPWA_TILE, 0, c->stream>>>(c->model, src.s12, src.s13, n, k0, i0);
+        k_cell_keys<<<grid_for(c, n, 8), MIPWA_TILE, 0, c->stream>>>(src.seg, n, c->N - 1, k0, i0);
         ++c->launches;
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, k0, k1, i0, i1, (int)n, 0, bits, c->stream);
@@ -990,9 +1011,11 @@ static int ensure_sorted(mipwa_ctx* c, const Slot& src, Slot& dst, bool& valid)
         if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k0, k1, i0, i1, (int)n, 0, bits, c->stream);
         for (int q = 0; q < 3 && e == cudaSuccess; ++q)
             if (q < 2 || src.w) e = cudaMalloc(&dst.owned[q], (size_t)n * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc(&dst.owned[3], (size_t)n * sizeof(unsigned short));
         if (e == cudaSuccess) {
-            k_gather<<<grid_for(c, n, 8), MIPWA_TILE, 0, c->stream>>>(i1, n, src.s12, src.s13, src.w, (double*)dst.owned[0],
-                                                                      (double*)dst.owned[1], (double*)dst.owned[2]);
+            k_gather<<<grid_for(c, n, 8), MIPWA_TILE, 0, c->stream>>>(i1, n, src.s12, src.s13, src.w, src.seg,
+                                                                      (double*)dst.owned[0], (double*)dst.owned[1],
+                                                                      (double*)dst.owned[2], (unsigned short*)dst.owned[3]);
             ++c->launches;
             e = cudaGetLastError();
         }
@@ -1004,6 +1027,7 @@ static int ensure_sorted(mipwa_ctx* c, const Slot& src, Slot& dst, bool& valid)
             return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, std::string("cell sort: ") + cudaGetErrorString(e));
         }
         dst.s12 = (const double*)dst.owned[0]; dst.s13 = (const double*)dst.owned[1]; dst.w = (const double*)dst.owned[2];
+        dst.seg = (const unsigned short*)dst.owned[3];
     }
     dst.n = n;
     valid = true;
