@@ -60,13 +60,41 @@ struct SplineSmem {
     double xk[MIPWA_DEV_LUT];
 };
 
+// The coefficient tables alone, for kernels that get the segment of every point from the stored segment pairs.
+struct SplineCoefSmem {
+    double knots[MIPWA_DEV_MAX_KNOTS];
+    double2 sc[4][MIPWA_DEV_MAX_KNOTS];
+};
+
+// The model arrives in the kernel parameter (constant) bank.  A constant-bank read whose index differs between the
+// lanes of a warp is replayed once per distinct address, so the tables are copied with a warp-uniform index: every
+// lane reads entry i, lane 0 stores it (a thread-indexed copy of the 13.5 KB tables took ~20 us per block).
+template <class Tables>
+__device__ __forceinline__ void copy_coef_rows(Tables& sm, const DevModel& m)
+{
+    const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5, lane = threadIdx.x & 31;
+    for (int i = warp; i < m.N; i += nwarp) {
+        const double k = m.knots[i];
+        const double2 c0 = m.sc[0][i], c1 = m.sc[1][i], c2 = m.sc[2][i], c3 = m.sc[3][i];
+        if (lane == 0) { sm.knots[i] = k; sm.sc[0][i] = c0; sm.sc[1][i] = c1; sm.sc[2][i] = c2; sm.sc[3][i] = c3; }
+    }
+}
+
+__device__ __forceinline__ void load_spline_coef_smem(SplineCoefSmem& sm, const DevModel& m)
+{
+    copy_coef_rows(sm, m);
+    __syncthreads();
+}
+
 __device__ __forceinline__ void load_spline_smem(SplineSmem& sm, const DevModel& m)
 {
-    for (int i = threadIdx.x; i < m.N; i += blockDim.x) {
-        sm.knots[i] = m.knots[i];
-        sm.sc[0][i] = m.sc[0][i]; sm.sc[1][i] = m.sc[1][i]; sm.sc[2][i] = m.sc[2][i]; sm.sc[3][i] = m.sc[3][i];
+    copy_coef_rows(sm, m);
+    const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5, lane = threadIdx.x & 31;
+    for (int i = warp; i < m.nlut; i += nwarp) {
+        const uint8_t l = m.lut[i];
+        const double x = m.xk[i];
+        if (lane == 0) { sm.lut[i] = l; sm.xk[i] = x; }
     }
-    for (int i = threadIdx.x; i < m.nlut; i += blockDim.x) { sm.lut[i] = m.lut[i]; sm.xk[i] = m.xk[i]; }
     __syncthreads();
 }
 
@@ -127,7 +155,8 @@ __device__ __forceinline__ void spline_eval(const SplineSmem& sm, const DevModel
 
 // spline value on a known segment j (the segment pair of every point is computed once per point set, by the
 // boundary-check kernel of mipwa_set_*, and stored as one uint16 per point: j12 | j13 << 8)
-__device__ __forceinline__ void spline_eval_at(const SplineSmem& sm, double s, int j, double& re, double& im)
+template <class Tables>
+__device__ __forceinline__ void spline_eval_at(const Tables& sm, double s, int j, double& re, double& im)
 {
     const double t = s - sm.knots[j];
     const double2 c0 = sm.sc[0][j], c1 = sm.sc[1][j], c2 = sm.sc[2][j], c3 = sm.sc[3][j];
@@ -159,9 +188,10 @@ __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, dou
     c.lam2 = (m.s_hi - x) * (m.s_top - x);
     c.Z[0] = 1.0;
     if (FL & MIPWA_FL_EQM) {
-        // ql clamped at 0 and lam1 + 1e-300: a point within rounding below threshold gives width 0, not NaN
-        c.ql = fmax(x - m.t_lo, 0.0);
-        const double lc = fma(c.ql, x, 1e-300);
+        // |ql| x + 1e-300 under the root: a point within rounding of the threshold (the boundary check admits a
+        // relative 1e-12) gives a width of rounding size, not NaN or infinity
+        c.ql = x - m.t_lo;
+        const double lc = fma(fabs(c.ql), x, 1e-300);
         double y0;
         asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(lc));
         const double u = c.ql * y0, e = fma(-(lc * y0), y0, 1.0);      // ql rsqrt(lc), refinement merged in
@@ -329,8 +359,8 @@ __device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& 
 }
 
 // the same with the segment pair of the point known (seg = j12 | j13 << 8)
-template <int R1, int R2, int FL = 0>
-__device__ __forceinline__ void amplitude_seg(const SplineSmem& sm, const DevModel& m, double s12, double s13,
+template <int R1, int R2, int FL = 0, class Tables = SplineSmem>
+__device__ __forceinline__ void amplitude_seg(const Tables& sm, const DevModel& m, double s12, double s13,
                                               unsigned int seg, double& are, double& aim)
 {
     double r1, i1, r2, i2;

@@ -6,11 +6,19 @@
 #ifndef MIPWA_BLOCK
 #define MIPWA_BLOCK 256
 #endif
-#ifndef MIPWA_MINBLOCKS
-#define MIPWA_MINBLOCKS 3
+// launch shape of k_nll_recompute (measured, profiles/r1_recompute_shape.md): ONE block of 512 threads per SM with up
+// to 128 registers per thread, one point per thread and iteration.  With 128 registers the model constants stay in
+// registers instead of being re-read from the constant bank every point, and one big block per SM beat two or three
+// smaller ones at the same warp count (0.265 ms against 0.298 ms for 2 x 256 threads, 0.299 ms for 3 x 256 threads
+// at 80 registers, config 3).
+#ifndef MIPWA_REC_BLOCK
+#define MIPWA_REC_BLOCK 512
 #endif
-#ifndef MIPWA_PTS
-#define MIPWA_PTS 1
+#ifndef MIPWA_REC_MINBLOCKS
+#define MIPWA_REC_MINBLOCKS 1
+#endif
+#ifndef MIPWA_REC_PTS
+#define MIPWA_REC_PTS 1
 #endif
 
 // ---- deterministic block reduction of NV doubles per thread: warp shuffles, then shared memory -------------------
@@ -73,7 +81,7 @@ struct LogProd {
 // last block to finish adds them in block order (fixed order: bit-reproducible for a given grid) and writes the
 // two totals to `result` (mapped pinned host memory).
 template <int R1, int R2, int FL>
-__global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_MINBLOCKS)
+__global__ void __launch_bounds__(MIPWA_REC_BLOCK, MIPWA_REC_MINBLOCKS)
 k_nll_recompute(const __grid_constant__ DevModel m,
                 const double* __restrict__ e12, const double* __restrict__ e13, const unsigned short* __restrict__ eseg,
                 long long n_ev,
@@ -81,17 +89,17 @@ k_nll_recompute(const __grid_constant__ DevModel m,
                 const unsigned short* __restrict__ gseg, long long n_norm, double2* __restrict__ partials, unsigned int* __restrict__ ticket,
                 double* __restrict__ result)
 {
-    __shared__ SplineSmem sm;
+    __shared__ SplineCoefSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
-    load_spline_smem(sm, m);
+    load_spline_coef_smem(sm, m);
 
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
 
     // PTS points per thread and iteration: independent dependency chains for the FP64 pipe.  Out-of-range slots
     // evaluate a harmless in-range point and contribute ln 1 = 0 (events) or weight 0 (normalisation).
-    constexpr int PTS = MIPWA_PTS;
+    constexpr int PTS = MIPWA_REC_PTS;
     LogProd lp;
     {
         double a[PTS], b[PTS];
@@ -186,8 +194,8 @@ __global__ void __launch_bounds__(MIPWA_BLOCK)
 k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const double* __restrict__ s13,
        const unsigned short* __restrict__ seg, long long n, double* __restrict__ out)
 {
-    __shared__ SplineSmem sm;
-    load_spline_smem(sm, m);
+    __shared__ SplineCoefSmem sm;
+    load_spline_coef_smem(sm, m);
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         double re, im;

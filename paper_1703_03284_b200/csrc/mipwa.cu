@@ -379,7 +379,7 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     bool ok = true;
     MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
                        ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute<R1, R2, FL>,
-                                                                          MIPWA_BLOCK, 0) == cudaSuccess);
+                                                                          MIPWA_REC_BLOCK, 0) == cudaSuccess);
     if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
 #ifdef MIPWA_FORCE_BPS
     c->blocks_per_sm = MIPWA_FORCE_BPS;                    // experiments only
@@ -532,9 +532,10 @@ int mipwa_set_path(mipwa_ctx* c, int32_t path)
 
 static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
 {
-    const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->blocks_per_sm);
+    const int64_t need = (std::max(c->ev.n, c->nm.n) + MIPWA_REC_BLOCK - 1) / MIPWA_REC_BLOCK;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags, (k_nll_recompute<R1, R2, FL><<<grid, MIPWA_BLOCK, 0, c->stream>>>(
+    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags, (k_nll_recompute<R1, R2, FL><<<grid, MIPWA_REC_BLOCK, 0, c->stream>>>(
                                c->model, evs(c).s12, evs(c).s13, evs(c).seg, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w,
                                nms(c).seg, nms(c).n, c->d_partials, c->d_ticket, c->d_result)));
     ++c->launches;
