@@ -301,9 +301,10 @@ __device__ __forceinline__ void group_barrier(const ResDev& r, const Channel& c,
     FZ = (c.Z[LT] * DR) * fast_rsqrt(DR * DD);
 }
 
+// symmetrised terms T_r(s12,s13) + T_r(s13,s12) (without coefficient and sqrt(n_R n_D)) of the NR group members
 template <int LT, int NR>
-__device__ __forceinline__ void add_group_shared(const ResDev* rd, const Channel& ca, const Channel& cb, double& are,
-                                                 double& aim)
+__device__ __forceinline__ void group_shared_terms(const ResDev* rd, const Channel& ca, const Channel& cb,
+                                                   double* tr, double* ti)
 {
     double DRa, FZa, DRb, FZb;
     group_barrier<LT>(rd[0], ca, DRa, FZa);
@@ -313,9 +314,21 @@ __device__ __forceinline__ void add_group_shared(const ResDev* rd, const Channel
         const double Wa = rd[r].Kw * ca.w[LT], Wb = rd[r].Kw * cb.w[LT];
         const double da = (rd[r].m0sq - ca.x) * DRa, db = (rd[r].m0sq - cb.x) * DRb;
         const double ta = FZa * fast_rcp(fma(da, da, Wa * Wa)), tb = FZb * fast_rcp(fma(db, db, Wb * Wb));
-        const double tr = fma(ta, da, tb * db), ti = fma(ta, Wa, tb * Wb);
-        are = fma(rd[r].cre, tr, fma(-rd[r].cim, ti, are));
-        aim = fma(rd[r].cre, ti, fma(rd[r].cim, tr, aim));
+        tr[r] = fma(ta, da, tb * db);
+        ti[r] = fma(ta, Wa, tb * Wb);
+    }
+}
+
+template <int LT, int NR>
+__device__ __forceinline__ void add_group_shared(const ResDev* rd, const Channel& ca, const Channel& cb, double& are,
+                                                 double& aim)
+{
+    double tr[NR], ti[NR];
+    group_shared_terms<LT, NR>(rd, ca, cb, tr, ti);
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+        are = fma(rd[r].cre, tr[r], fma(-rd[r].cim, ti[r], are));
+        aim = fma(rd[r].cre, ti[r], fma(rd[r].cim, tr[r], aim));
     }
 }
 

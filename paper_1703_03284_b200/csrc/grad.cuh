@@ -35,24 +35,36 @@ __device__ __forceinline__ void spline_eval_jt(const SplineSmem& sm, const DevMo
 
 // amplitude with the pieces the gradient needs: segment/offset of both channels and every symmetrised resonance
 // term WITHOUT its coefficient (device slot order; the host multiplies by sqrt(n_R n_D))
-template <int R1, int R2>
-__device__ __forceinline__ void amplitude_parts(const SplineSmem& sm, const DevModel& m, double s12, double s13,
-                                                double& are, double& aim, int& j1, double& t1, int& j2, double& t2,
+template <int R1, int R2, int FL>
+__device__ __forceinline__ void amplitude_parts(const SplineCoefSmem& sm, const DevModel& m, double s12, double s13,
+                                                unsigned int seg, double& are, double& aim, int& j1, double& t1,
+                                                int& j2, double& t2,
                                                 double (&tr)[R1 >= 0 ? (R1 + R2 > 0 ? R1 + R2 : 1) : MIPWA_GRAD_MAXR],
                                                 double (&ti)[R1 >= 0 ? (R1 + R2 > 0 ? R1 + R2 : 1) : MIPWA_GRAD_MAXR])
 {
     double r1, i1, r2, i2;
-    spline_eval_jt(sm, m, s12, j1, t1, r1, i1);
-    spline_eval_jt(sm, m, s13, j2, t2, r2, i2);
+    j1 = (int)(seg & 0xffu); j2 = (int)(seg >> 8);         // segment pair stored by k_validate
+    t1 = s12 - sm.knots[j1]; t2 = s13 - sm.knots[j2];
+    spline_eval_at(sm, s12, j1, r1, i1);
+    spline_eval_at(sm, s13, j2, r2, i2);
     are = r1 + r2;
     aim = i1 + i2;
     if (R1 == 0 && R2 == 0) return;
-    const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
+    const Channel ca = make_channel<FL>(m, s12, s13), cb = make_channel<FL>(m, s13, s12);
     if (R1 >= 0) {
+        if ((FL & MIPWA_FL_SHR) && R1 >= 2) {
+            group_shared_terms<1, (R1 >= 2 ? R1 : 2)>(&m.res[0], ca, cb, &tr[0], &ti[0]);
+        } else {
 #pragma unroll
-        for (int r = 0; r < R1; ++r) resonance_sym<1>(m.res[r], ca, cb, tr[r], ti[r]);
+            for (int r = 0; r < R1; ++r) resonance_sym<1>(m.res[r], ca, cb, tr[r], ti[r]);
+        }
+        if ((FL & MIPWA_FL_SHR) && R2 >= 2) {
+            group_shared_terms<2, (R2 >= 2 ? R2 : 2)>(&m.res[R1 > 0 ? R1 : 0], ca, cb, &tr[R1 > 0 ? R1 : 0],
+                                                      &ti[R1 > 0 ? R1 : 0]);
+        } else {
 #pragma unroll
-        for (int r = 0; r < R2; ++r) resonance_sym<2>(m.res[R1 + r], ca, cb, tr[R1 + r], ti[R1 + r]);
+            for (int r = 0; r < R2; ++r) resonance_sym<2>(m.res[R1 + r], ca, cb, tr[R1 + r], ti[R1 + r]);
+        }
 #pragma unroll
         for (int r = 0; r < R1 + R2; ++r) {
             are = fma(m.res[r].cre, tr[r], fma(-m.res[r].cim, ti[r], are));
@@ -152,9 +164,10 @@ template <int R1, int R2> struct GradDims {
 
 // one pass over a cell-sorted point set.  EV: events (f = -2/conj(A), scalar = sum ln|A|^2);
 // otherwise normalisation points (f = w A, scalar = sum w |A|^2).
-template <int R1, int R2, bool EV>
-__device__ __forceinline__ void grad_pass(const SplineSmem& sm, const DevModel& m, const double* __restrict__ s12,
-                                          const double* __restrict__ s13, const double* __restrict__ w, long long n,
+template <int R1, int R2, int FL, bool EV>
+__device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevModel& m, const double* __restrict__ s12,
+                                          const double* __restrict__ s13, const double* __restrict__ w,
+                                          const unsigned short* __restrict__ sgp, long long n,
                                           double* bins, double& scalar, double (&Fr)[GradDims<R1, R2>::RR],
                                           double (&Fi)[GradDims<R1, R2>::RR])
 {
@@ -170,23 +183,25 @@ __device__ __forceinline__ void grad_pass(const SplineSmem& sm, const DevModel& 
     double integ = 0.0;
     const int nres = R1 >= 0 ? R1 + R2 : m.R;
     double nx = 1.0, ny = 1.0, nw = 0.0;                                   // next iteration's point, loaded one ahead
+    unsigned int nsg = 0u;
     if (lo < hi) {
         const long long ii = lo + lane < hi ? lo + lane : lo;
-        nx = s12[ii]; ny = s13[ii];
+        nx = s12[ii]; ny = s13[ii]; nsg = sgp[ii];
         if (!EV) nw = lo + lane < hi ? (w ? w[ii] : 1.0) : 0.0;
     }
     for (long long base = lo; base < hi; base += 32) {                     // warp-uniform trip count
         const long long i = base + lane;
         const bool valid = i < hi;
         const double x = nx, y = ny, wv = nw;
+        const unsigned int sg = nsg;
         if (base + 32 < hi) {
             const long long ii = i + 32 < hi ? i + 32 : lo;
-            nx = s12[ii]; ny = s13[ii];
+            nx = s12[ii]; ny = s13[ii]; nsg = sgp[ii];
             if (!EV) nw = i + 32 < hi ? (w ? w[ii] : 1.0) : 0.0;
         }
         double are, aim, t1, t2, tr[RR], ti[RR];
         int j1, j2;
-        amplitude_parts<R1, R2>(sm, m, x, y, are, aim, j1, t1, j2, t2, tr, ti);
+        amplitude_parts<R1, R2, FL>(sm, m, x, y, sg, are, aim, j1, t1, j2, t2, tr, ti);
         const double a2 = fma(are, are, aim * aim);
         double fr, fi;
         if (EV) {
@@ -230,23 +245,27 @@ __device__ __forceinline__ void grad_pass(const SplineSmem& sm, const DevModel& 
 
 // result / partial layout (doubles): [0] sum ln|A|^2, [1] sum w|A|^2, [2 + 2d + {0,1}] F_ev of device slot d,
 // [2 + 2R + 2d + {0,1}] F_nm, then bins_ev[4][N-1][2], bins_nm[4][N-1][2];  NV = 2 + 4R + 16 (N-1).
-#ifndef MIPWA_GRAD_MINBLOCKS
-#define MIPWA_GRAD_MINBLOCKS 2
+#ifndef MIPWA_GRAD_BLOCK
+#define MIPWA_GRAD_BLOCK 512
 #endif
-template <int R1, int R2>
-__global__ void __launch_bounds__(MIPWA_BLOCK, MIPWA_GRAD_MINBLOCKS)
+#ifndef MIPWA_GRAD_MINBLOCKS
+#define MIPWA_GRAD_MINBLOCKS 1
+#endif
+template <int R1, int R2, int FL>
+__global__ void __launch_bounds__(MIPWA_GRAD_BLOCK, MIPWA_GRAD_MINBLOCKS)
 k_grad_recompute(const __grid_constant__ DevModel m,
-                 const double* __restrict__ e12, const double* __restrict__ e13, long long n_ev,
+                 const double* __restrict__ e12, const double* __restrict__ e13,
+                 const unsigned short* __restrict__ eseg, long long n_ev,
                  const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
-                 long long n_norm, double* __restrict__ partials)
+                 const unsigned short* __restrict__ gseg, long long n_norm, double* __restrict__ partials)
 {
     constexpr int RR = GradDims<R1, R2>::RR;
     extern __shared__ double grad_bins[];                  // [2][4][N-1][2]
-    __shared__ SplineSmem sm;
+    __shared__ SplineCoefSmem sm;
     __shared__ double red32[32];
     const int NS = m.N - 1, R = m.R, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) grad_bins[k] = 0.0;
-    load_spline_smem(sm, m);                               // ends with __syncthreads()
+    load_spline_coef_smem(sm, m);                          // ends with __syncthreads()
 
     double* mine = partials + (size_t)blockIdx.x * NV;
     // events pass, then its scalars are reduced and stored before the second pass so that only one set of resonance
@@ -256,8 +275,8 @@ k_grad_recompute(const __grid_constant__ DevModel m,
         double Sc = 0.0, Fr[RR], Fi[RR];
 #pragma unroll
         for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
-        if (pass == 0) grad_pass<R1, R2, true>(sm, m, e12, e13, nullptr, n_ev, grad_bins, Sc, Fr, Fi);
-        else grad_pass<R1, R2, false>(sm, m, g12, g13, gw, n_norm, grad_bins + nb, Sc, Fr, Fi);
+        if (pass == 0) grad_pass<R1, R2, FL, true>(sm, m, e12, e13, nullptr, eseg, n_ev, grad_bins, Sc, Fr, Fi);
+        else grad_pass<R1, R2, FL, false>(sm, m, g12, g13, gw, gseg, n_norm, grad_bins + nb, Sc, Fr, Fi);
         double v = block_sum(Sc, red32);
         if (threadIdx.x == 0) mine[pass] = v;
         for (int r = 0; r < R; ++r) {

@@ -1148,13 +1148,14 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     const size_t smem = (size_t)2 * nb * sizeof(double);
     if (!c->grad_blocks_per_sm) {
         bool ok = true;
-        MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
-                           ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->grad_blocks_per_sm, k_grad_recompute<R1, R2>,
-                                                                              MIPWA_BLOCK, smem) == cudaSuccess);
+        MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
+                           ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->grad_blocks_per_sm, k_grad_recompute<R1, R2, FL>,
+                                                                              MIPWA_GRAD_BLOCK, smem) == cudaSuccess);
         if (!ok) return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
         if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
     }
-    const int grid = grid_for(c, std::max(c->ev.n, c->nm.n), c->grad_blocks_per_sm);   // small samples: fewer partial vectors
+    const int64_t gneed = (std::max(c->ev.n, c->nm.n) + MIPWA_GRAD_BLOCK - 1) / MIPWA_GRAD_BLOCK;   // small samples: fewer partial vectors
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->grad_blocks_per_sm, gneed));
     if (c->gpartials_len < (size_t)grid * NV) {
         if (c->d_gpartials) cudaFree(c->d_gpartials);
         c->d_gpartials = nullptr; c->gpartials_len = 0;
@@ -1162,10 +1163,11 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
         c->gpartials_len = (size_t)grid * NV;
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_SIG(c->n_spin[0], c->n_spin[1], c->n_spin[2],
-                       (k_grad_recompute<R1, R2><<<grid, MIPWA_BLOCK, smem, c->stream>>>(
-                           c->model, c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.n, c->nm_sorted.s12, c->nm_sorted.s13,
-                           c->nm_sorted.w, c->nm_sorted.n, c->d_gpartials)));
+    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
+                       (k_grad_recompute<R1, R2, FL><<<grid, MIPWA_GRAD_BLOCK, smem, c->stream>>>(
+                           c->model, c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, c->ev_sorted.n,
+                           c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w, c->nm_sorted.seg, c->nm_sorted.n,
+                           c->d_gpartials)));
     ++c->launches;
     CU(c, cudaGetLastError());
     k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
