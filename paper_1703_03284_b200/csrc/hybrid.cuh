@@ -15,12 +15,12 @@ struct HybCoef {
     double2 c[MIPWA_DEV_MAX_RES];
 };
 
-template <int R1, int R2, int RCT>
-__device__ __forceinline__ double hybrid_abs2(const SplineSmem& sm, const DevModel& m, const HybCoef& cc, double2 s,
-                                              const double2 (&b)[RCT])
+template <int R1, int R2, int RCT, int FL>
+__device__ __forceinline__ double hybrid_abs2(const SplineCoefSmem& sm, const DevModel& m, const HybCoef& cc, double2 s,
+                                              unsigned int sg, const double2 (&b)[RCT])
 {
     double re, im;
-    amplitude<R1, R2>(sm, m, s.x, s.y, re, im);            // spline + floating resonances
+    amplitude_seg<R1, R2, FL>(sm, m, s.x, s.y, sg, re, im);   // spline + floating resonances
 #pragma unroll
     for (int k = 0; k < RCT; ++k) {
         const double2 c = cc.c[k];
@@ -32,27 +32,31 @@ __device__ __forceinline__ double hybrid_abs2(const SplineSmem& sm, const DevMod
 
 // One launch over [events | normalisation points]; one point per thread and tile, the next tile's columns are
 // loaded before the current tile is evaluated.  result[0] = sum ln|A|^2, result[1] = sum w |A|^2 (w == NULL: weight 1).
-template <int R1, int R2, int RCT>
-__global__ void __launch_bounds__(MIPWA_TILE, 3)
+// eseg / gseg: the stored segment pairs of the same (cell-sorted or caller's) point order the caches were built in.
+template <int R1, int R2, int RCT, int FL>
+__global__ void __launch_bounds__(MIPWA_TILE, 2)
 k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef cc,
-             const double2* __restrict__ ev_cache, long long n_ev,
-             const double2* __restrict__ nm_cache, const double* __restrict__ gw, long long n_norm,
+             const double2* __restrict__ ev_cache, const unsigned short* __restrict__ eseg, long long n_ev,
+             const double2* __restrict__ nm_cache, const double* __restrict__ gw,
+             const unsigned short* __restrict__ gseg, long long n_norm,
              double2* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result)
 {
-    __shared__ SplineSmem sm;
+    __shared__ SplineCoefSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
-    load_spline_smem(sm, m);
+    load_spline_coef_smem(sm, m);
     constexpr int C = 1 + RCT;
     LogProd lp;
     double integ = 0.0;
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
         const double2* cache = pass == 0 ? ev_cache : nm_cache;
+        const unsigned short* segs = pass == 0 ? eseg : gseg;
         const long long n = pass == 0 ? n_ev : n_norm;
         const long long n_tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
         double2 s = make_double2(1.0, 1.0), b[RCT];
         double w = 0.0;
+        unsigned int sg = 0u;
 #pragma unroll
         for (int k = 0; k < RCT; ++k) b[k] = make_double2(0.0, 0.0);
         long long tile = blockIdx.x;
@@ -63,10 +67,12 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
             for (int k = 0; k < RCT; ++k) b[k] = ld_stream(p + (size_t)(1 + k) * MIPWA_TILE);
             const long long i = tile * MIPWA_TILE + threadIdx.x;
             if (pass == 1) w = i < n ? (gw ? gw[i] : 1.0) : 0.0;
+            if (i < n) sg = segs[i];
         }
         for (; tile < n_tiles; tile += gridDim.x) {
             double2 ns = make_double2(1.0, 1.0), nb[RCT];
             double nw = 0.0;
+            unsigned int nsg = 0u;
 #pragma unroll
             for (int k = 0; k < RCT; ++k) nb[k] = make_double2(0.0, 0.0);
             const long long nt = tile + gridDim.x;
@@ -77,13 +83,14 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
                 for (int k = 0; k < RCT; ++k) nb[k] = ld_stream(p + (size_t)(1 + k) * MIPWA_TILE);
                 const long long i = nt * MIPWA_TILE + threadIdx.x;
                 if (pass == 1) nw = i < n ? (gw ? gw[i] : 1.0) : 0.0;
+                if (i < n) nsg = segs[i];
             }
             const bool live = tile * MIPWA_TILE + threadIdx.x < n;
             // padding slots of the last tile hold (0, 0): evaluate a harmless point instead
-            const double v = hybrid_abs2<R1, R2, RCT>(sm, m, cc, live ? s : make_double2(1.0, 1.0), b);
+            const double v = hybrid_abs2<R1, R2, RCT, FL>(sm, m, cc, live ? s : make_double2(1.0, 1.0), live ? sg : 0u, b);
             if (pass == 0) lp.add(live ? v : 1.0);
             else integ = fma(w, v, integ);
-            s = ns; w = nw;
+            s = ns; w = nw; sg = nsg;
 #pragma unroll
             for (int k = 0; k < RCT; ++k) b[k] = nb[k];
         }
@@ -136,3 +143,11 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
         case MIPWA_HYB_CASE(1, 1, 4): { constexpr int R1 = 1, R2 = 1, RCT = 4; CALL; } break;                  \
         default: supported = false; break;                                                                      \
     }
+
+// the same with constexpr FL = the MIPWA_FL_EQM bit of the model flags (radii sharing needs two floating resonances
+// of one spin: only the <2, 0, *> signatures)
+#define MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl, CALL)                                                              \
+    if ((fl) & MIPWA_FL_EQM) {                                                                                  \
+        if (((fl) & MIPWA_FL_SHR) && (f1) == 2) { constexpr int FL = MIPWA_FL_EQM | MIPWA_FL_SHR; MIPWA_DISPATCH_HYB(f1, f2, rc, CALL) } \
+        else { constexpr int FL = MIPWA_FL_EQM; MIPWA_DISPATCH_HYB(f1, f2, rc, CALL) }                         \
+    } else { constexpr int FL = 0; MIPWA_DISPATCH_HYB(f1, f2, rc, CALL) }

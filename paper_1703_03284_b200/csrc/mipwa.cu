@@ -780,8 +780,8 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     }
     bool supported = true;
     if (!c->hyb_blocks_per_sm) {
-        MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, RC,
-                           supported = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->hyb_blocks_per_sm, k_nll_hybrid<R1, R2, RCT>,
+        MIPWA_DISPATCH_HYBFL(c->hyb_f1, c->hyb_f2, RC, c->model_flags,
+                           supported = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->hyb_blocks_per_sm, k_nll_hybrid<R1, R2, RCT, FL>,
                                                                                      MIPWA_TILE, 0) == cudaSuccess);
         if (!supported) return fail(c, MIPWA_ERR_CUDA, "hybrid: occupancy query failed");
         if (c->hyb_blocks_per_sm < 1) c->hyb_blocks_per_sm = 1;
@@ -789,9 +789,10 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     const int64_t tiles = (std::max(c->ev.n, c->nm.n) + MIPWA_TILE - 1) / MIPWA_TILE;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->hyb_blocks_per_sm));
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, RC,
-                       (k_nll_hybrid<R1, R2, RCT><<<grid, MIPWA_TILE, 0, c->stream>>>(
-                           c->model, cc, (const double2*)c->d_hyb_ev, c->ev.n, (const double2*)c->d_hyb_nm, nms(c).w, c->nm.n,
+    MIPWA_DISPATCH_HYBFL(c->hyb_f1, c->hyb_f2, RC, c->model_flags,
+                       (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_TILE, 0, c->stream>>>(
+                           c->model, cc, (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n, (const double2*)c->d_hyb_nm,
+                           nms(c).w, nms(c).seg, c->nm.n,
                            c->d_partials, c->d_ticket, c->d_result)));
     ++c->launches;
     CU(c, cudaGetLastError());
