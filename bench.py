@@ -34,15 +34,19 @@ UNIT = "events/s"
 
 # ---- algorithmic work per point: flops of the plain formulas, one per add / mul /
 # div / sqrt / log, fma = 2: two channels x [10 shared kinematics + 14 spline + 37 R] + 4, plus 2 (1 + 3R) divisions,
-# 2 (2 + R) square roots and one log = 59 + 82 R (305 at R = 3).  The kernel as built executes 297 (ncu-counted
-# dadd + dmul + 2 dfma per point, profiles/r1_k_nll_recompute_ncu.md), so nothing is padded. -------------------------------
+# 2 (2 + R) square roots and one log = 59 + 82 R (305 at R = 3).  The kernel as built executes 261 at config 3
+# (ncu-counted dadd + dmul + 2 dfma per point, profiles/r1_k_nll_recompute_ncu.md: the equal-mass and shared-radii
+# specialisations and one reciprocal (square root) per resonance and channel do the same arithmetic in fewer
+# operations), so nothing is padded; "executed_flops_per_point" in the roofline object gives the executed rate. ------
 def flops_per_point(resonances):
     return 59 + 82 * len(resonances)
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_nll_recompute launch at the bench size (10M events + 10M weighted
 # normalisation points), from the one `ncu --set full` capture summarised in profiles/r1_k_nll_recompute_ncu.md
-NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 404.4e6}
+NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 443.9e6}
+# executed FP64 flops per point in that capture (config 3's model): (dadd + dmul + 2 dfma) / points
+NCU_EXECUTED_FLOPS_PER_POINT = {(10_000_000, 10_000_000): 260.7}
 
 
 class ClockSampler:
@@ -347,13 +351,14 @@ def run_ours(args, cfg, workload):
     roofline = {"bound": "alu", "kernel": "k_nll_recompute", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((n_ev, n_norm)),
                 "traffic_source": "profiles/r1_k_nll_recompute_ncu.md (ncu --set full, bytes per launch); algorithmic bytes "
-                                  "per launch = 16 B x events + 24 B x weighted normalisation points",
+                                  "per launch = 18 B x events + 26 B x weighted normalisation points (s12, s13, (w), 2-byte segment pair)",
                 "peak_source": "measured on this GPU by mipwa_measure_fp64_peak (register-resident DFMA, 2 s sustained); "
                                "MEASURED_PEAKS.json has no FP64 entry; DESIGN.md section 6 derives the nominal peak",
                 "nominal_peak": nominal, "flops_per_point": flops_per_point(cfg.resonances),
                 "points_per_launch": n_ev + n_norm, "kernel_ms": k_ms,
-                "algorithmic_bytes": 16.0 * n_ev + 24.0 * n_norm,
-                "hbm_gbs": (16.0 * n_ev + 24.0 * n_norm) / (k_ms * 1e-3) * 1e-9}
+                "executed_flops_per_point": NCU_EXECUTED_FLOPS_PER_POINT.get((n_ev, n_norm)),
+                "algorithmic_bytes": 18.0 * n_ev + 26.0 * n_norm,
+                "hbm_gbs": (18.0 * n_ev + 26.0 * n_norm) / (k_ms * 1e-3) * 1e-9}
     hbm_peak, hbm_src = 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -390,7 +395,7 @@ def run_ours(args, cfg, workload):
 
 # ---- secondary measurements behind the numbers in BASELINE.md / profiles (not the driver's bench line) --------------
 def run_probe(args):
-    """--probe resonances | sweep4 | latency : prints one JSON line per row (kernel times: CUDA events in the library,
+    """--probe resonances | recompute-shape | sweep4 | latency : prints one JSON line per row (kernel times: CUDA events in the library,
     median over the calls after warm-up).  Phase-space points stand in for events where only the work per point
     matters; every mode cross-checks its NLL against another path."""
     import torch
@@ -424,6 +429,23 @@ def run_probe(args):
             print(json.dumps({"probe": "resonances", "model": name, "points": 2 * n, "kernel_ms": k, "nll": v,
                               "clk_per_warp_point_per_smsp_at_1965MHz": k * 1e-3 * 1.965e9 * 592 / (2 * n / 32)}), flush=True)
             m.close()
+    elif args.probe == "recompute-shape":
+        # kernel time of k_nll_recompute (value) and k_grad_recompute at configs[3]'s model on 10 M + 10 M weighted,
+        # cell-sorted phase-space points; MIPWA_LIB_PATH selects a library rebuilt with other -DMIPWA_REC_* switches
+        # (profiles/r1_recompute_shape.md)
+        c = I.Config(3)
+        n = args.events or 10_000_000
+        e12, e13 = I.phase_space_points(n, c.key(7)); g12, g13 = I.phase_space_points(n, c.key(8))
+        w = np.full(n, 5.06 / n)
+        d = [torch.from_numpy(a).cuda() for a in (e12, e13, g12, g13, w)]
+        m = B.Mipwa(c.kin, c.knots, c.resonances)
+        m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4]); m.set_path(B.PATH_RECOMPUTE)
+        m.prepare(); m.enable_timing(True)
+        k, v = timed(m, c.perturbed(0), calls=60, skip=10)
+        kg, vg = timed(m, c.perturbed(0), calls=30, skip=10, grad=True)
+        print(json.dumps({"probe": "recompute-shape", "library": os.environ.get("MIPWA_LIB_PATH", "default"),
+                          "points": 2 * n, "kernel_ms": k, "grad_kernel_ms": kg, "nll": v, "nll_grad_path": vg}), flush=True)
+        m.close()
     elif args.probe == "sweep4":
         # BASELINE.json configs[4]: K = 56 cached paths against the event count (default 1 M .. 100 M), 10 M-point Gram
         c = I.Config(4)
@@ -491,7 +513,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--events", type=int, default=None)
     ap.add_argument("--norm-points", type=int, default=None)
-    ap.add_argument("--probe", default=None, choices=["resonances", "sweep4", "latency"])
+    ap.add_argument("--probe", default=None, choices=["resonances", "recompute-shape", "sweep4", "latency"])
     args = ap.parse_args()
     if args.probe:
         return run_probe(args)
