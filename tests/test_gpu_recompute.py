@@ -281,3 +281,41 @@ def test_hybrid_path_matches_oracle():
     with pytest.raises(B.MipwaError):
         m.set_path(B.PATH_HYBRID)
     m.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("equal_masses", [True, False])
+@pytest.mark.parametrize("shared_radii", [True, False])
+def test_model_flag_variants(equal_masses, shared_radii):
+    """The recompute, |A|^2 and gradient kernels are specialised on two model flags (equal daughter masses m1 == m2;
+    radii shared by all resonances of one spin).  Two spin-1 and two spin-2 resonances make both flags matter; every
+    one of the four kernel variants must match the oracle, which knows nothing of the flags."""
+    B = _lib()
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    kin = {"M": 1.86966, "m1": 0.13957 if equal_masses else 0.493677, "m2": 0.13957, "m3": 0.13957}
+    rr = (1.5, 1.5, 1.5, 1.5) if shared_radii else (1.5, 2.5, 1.5, 3.0)
+    rp = (5.0, 5.0, 5.0, 5.0) if shared_radii else (5.0, 4.0, 5.0, 5.0)
+    res = [dict(mass=0.8955, width=0.047, spin=1, r_res=rr[0], r_parent=rp[0]),
+           dict(mass=1.2755, width=0.1867, spin=2, r_res=rr[2], r_parent=rp[2]),
+           dict(mass=1.414, width=0.232, spin=1, r_res=rr[1], r_parent=rp[1]),
+           dict(mass=1.5174, width=0.086, spin=2, r_res=rr[3], r_parent=rp[3])]
+    lo, hi = I.s_limits(kin)
+    knots = np.linspace(lo - 1e-3, hi + 1e-3, 23)
+    s12, s13 = I.phase_space_points(9000, I.stream_key(3, 11, 1), kin)
+    e12, e13, g12, g13 = s12[:4001], s13[:4001], s12[4001:], s13[4001:]
+    w = np.full(g12.size, 0.37 / g12.size)
+    o = orc.Oracle(kin, knots, res)
+    rng = np.random.default_rng(5)
+    p = np.concatenate([rng.uniform(0.5, 2, 23), rng.uniform(0, 3, 23), rng.uniform(0.3, 1.5, 8)])
+    m = B.Mipwa(kin, knots, res)
+    m.set_events(e12, e13); m.set_norm_points(g12, g13, w); m.set_path(B.PATH_RECOMPUTE)
+    got, ref = m.eval_abs2(p, 0), o.abs2(p, e12, e13)
+    assert np.max(np.abs(got - ref) / ref) < 1e-11
+    ref_n, sl, integ = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    assert abs(m.nll(p) - ref_n) <= nll_tol(ref_n, sl, integ, e12.size)
+    v, g = m.nll_grad(p)
+    _, gref = o.nll_grad(p, e12, e13, g12, g13, w)
+    assert abs(v - ref_n) <= nll_tol(ref_n, sl, integ, e12.size)
+    assert np.max(np.abs(g - gref)) <= 1e-9 * np.max(np.abs(gref))
+    m.close()
