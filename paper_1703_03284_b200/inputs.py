@@ -284,6 +284,9 @@ class Config:
                 cm = 0.1 + 1.9 * u[2 * r]
                 if self.idx == 4 and r == 5:
                     cm *= 0.01                                                         # reading P19 (narrow peak)
+                if self.idx == 5:
+                    cm *= 0.1          # |T| = 1/(m0 Gamma0) = 231 at the phi(1020) pole: this scale gives the phi a
+                                       # fit fraction of 29 % beside the S-wave instead of > 99 %
                 coef += [cm, 2.0 * math.pi * u[2 * r + 1]]
         shapes = []
         for r in self.resonances:
