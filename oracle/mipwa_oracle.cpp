@@ -17,7 +17,8 @@
 // PARITY UNPINNED at paper level: the paper prints no amplitude, NLL, parameter or input value.  Every function
 // below is instead pinned in tests/test_oracle_*.py by closed forms, invariants, library special cases
 // (scipy natural CubicSpline, spherical Hankel functions), independent four-vector kinematics and finite
-// differences; see DESIGN.md "Oracle pins".
+// differences; see DESIGN.md "Oracle pins".  The shape derivatives (O10) are pinned by Richardson-extrapolated central
+// differences of the separately pinned resonance term and NLL.
 //
 // Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (no fast-math).  Arithmetic is IEEE double, evaluated
 // formula by formula in the order written; sums over events use long double Neumaier-compensated accumulators.
@@ -180,6 +181,41 @@ cplx resonance_term(const orc_kin& k, const orc_res& r, double x, double y)
     const double FD = barrier(r.spin, r.r_parent * r.r_parent * pstar2_of(k, x),
                               r.r_parent * r.r_parent * pstar2_of(k, m0s));
     return FD * FR * zemach(k, r.spin, x, y) * breit_wigner(k, r, x);
+}
+
+// O10 (not in the paper)  Derivatives of T_r(x, y) with respect to the pole mass m0 and the pole width
+//     Gamma0, from the definitions above written out.  With D = m0^2 - x - i W, W = m0 Gamma(x), T = F_D F_R Z / D:
+//       dT/dGamma0 = T (i W / Gamma0) / D                                   (W is proportional to Gamma0)
+//       dT/dm0     = T [ dlnF_R/dm0 + dlnF_D/dm0 ] - T (2 m0 - i W dlnW/dm0) / D
+//     where only the pole quantities q0^2 = q^2(m0^2), p0*^2 = p*^2(m0^2) depend on m0:
+//       ln F = (1/2) [ln n_L(z0) - ln n_L(z)], n_1(z) = 1 + z, n_2(z) = 9 + 3z + z^2, z0 = r^2 k0^2
+//       dlnF_R/dm0 = (1/2) n_L'(z0R)/n_L(z0R) r_R^2 dq0^2/dm0,   dlnF_D/dm0 likewise with r_D, p0*^2
+//       ln W = 2 ln m0 + ln Gamma0 + (L + 1/2) (ln q^2 - ln q0^2) - (1/2) ln x + 2 ln F_R
+//       dlnW/dm0 = 2/m0 - (L + 1/2) (dq0^2/dm0)/q0^2 + 2 dlnF_R/dm0
+//       q0^2 = [s0 - 2(m1^2 + m2^2) + (m1^2 - m2^2)^2 / s0] / 4  (s0 = m0^2):  dq0^2/dm0 = 2 m0 [1 - (m1^2-m2^2)^2/s0^2]/4
+//       p0*^2 = lambda(M^2, s0, m3^2)/(4 M^2):                                 dp0*^2/dm0 = 2 m0 (2 s0 - 2 M^2 - 2 m3^2)/(4 M^2)
+double barrier_num_dlog(int L, double z0)   // n_L'(z0) / n_L(z0)
+{
+    if (L == 0) return 0.0;
+    if (L == 1) return 1.0 / (1.0 + z0);
+    return (3.0 + 2.0 * z0) / (9.0 + 3.0 * z0 + z0 * z0);
+}
+
+void resonance_term_dshape(const orc_kin& k, const orc_res& r, double x, double y, cplx* dT_dm0, cplx* dT_dG0)
+{
+    const double m0 = r.mass, s0 = m0 * m0, L = (double)r.spin;
+    const double m1s = k.m1 * k.m1, m2s = k.m2 * k.m2, m3s = k.m3 * k.m3, Ms = k.M * k.M;
+    const cplx T = resonance_term(k, r, x, y);
+    const double W = m0 * running_width(k, r, x);
+    const cplx D(s0 - x, -W);
+    const double q02 = q2_of(k, s0), p02 = pstar2_of(k, s0);
+    const double dq02 = 2.0 * m0 * (1.0 - (m1s - m2s) * (m1s - m2s) / (s0 * s0)) / 4.0;
+    const double dp02 = 2.0 * m0 * (2.0 * s0 - 2.0 * Ms - 2.0 * m3s) / (4.0 * Ms);
+    const double dlnFR = 0.5 * barrier_num_dlog(r.spin, r.r_res * r.r_res * q02) * r.r_res * r.r_res * dq02;
+    const double dlnFD = 0.5 * barrier_num_dlog(r.spin, r.r_parent * r.r_parent * p02) * r.r_parent * r.r_parent * dp02;
+    const double dlnW = 2.0 / m0 - (L + 0.5) * dq02 / q02 + 2.0 * dlnFR;
+    *dT_dG0 = T * cplx(0.0, W / r.width) / D;
+    *dT_dm0 = T * (dlnFR + dlnFD) - T * cplx(2.0 * m0, -W * dlnW) / D;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -526,6 +562,59 @@ void orc_nll_grad(const orc_kin* kin, int n, const double* knots, int R, const o
             grad[2 * n + 2 * r + 1] = (G * std::conj(cplx(0.0, 1.0) * u.c[r])).real();
         }
     }
+}
+
+// ---- O10: test access to the shape derivatives of one resonance term: out = (Re, Im dT/dm0, Re, Im dT/dGamma0) ----
+void orc_resonance_term_dshape(const orc_kin* k, const orc_res* r, double x, double y, double* out)
+{
+    cplx dm, dg;
+    resonance_term_dshape(*k, *r, x, y, &dm, &dg);
+    out[0] = dm.real(); out[1] = dm.imag(); out[2] = dg.real(); out[3] = dg.imag();
+}
+
+// ---- O10: derivatives of the NLL w.r.t. (mass, width) of every shape_floats resonance, in list order ---------------
+//   dA/dtheta = c_r [dT_r(s12,s13)/dtheta + dT_r(s13,s12)/dtheta]
+//   dNLL/dtheta = -2 sum_i Re(conj(A_i) dA_i) / |A_i|^2 + (2 n_ev / I) sum_j w_j Re(conj(A_j) dA_j)
+// grad_shape has 2F entries: (d/dmass, d/dwidth) per floating resonance.
+void orc_nll_grad_shape(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res,
+                        const double* params, int64_t n_ev, const double* e12, const double* e13,
+                        int64_t n_norm, const double* g12, const double* g13, const double* w,
+                        double* nll, double* grad_shape)
+{
+    const Model m = make_model(kin, n, knots, R, res);
+    const Unpacked u = unpack(m, params);
+    std::vector<int> fl;
+    for (int r = 0; r < R; ++r) if (m.res[r].shape_floats) fl.push_back(r);
+    const int F = (int)fl.size();
+    std::vector<Acc> ev(2 * F), nm(2 * F);
+    Acc S, I;
+    for (int64_t i = 0; i < n_ev; ++i) {
+        const cplx A = amplitude(m, u, e12[i], e13[i]);
+        S.add(std::log(std::norm(A)));
+        for (int f = 0; f < F; ++f) {
+            cplx am, ag, bm, bg;
+            resonance_term_dshape(m.kin, u.res[fl[f]], e12[i], e13[i], &am, &ag);
+            resonance_term_dshape(m.kin, u.res[fl[f]], e13[i], e12[i], &bm, &bg);
+            ev[2 * f].add((std::conj(A) * (u.c[fl[f]] * (am + bm))).real() / std::norm(A));
+            ev[2 * f + 1].add((std::conj(A) * (u.c[fl[f]] * (ag + bg))).real() / std::norm(A));
+        }
+    }
+    for (int64_t j = 0; j < n_norm; ++j) {
+        const cplx A = amplitude(m, u, g12[j], g13[j]);
+        const double wj = w ? w[j] : 1.0 / (double)n_norm;
+        I.add((long double)wj * std::norm(A));
+        for (int f = 0; f < F; ++f) {
+            cplx am, ag, bm, bg;
+            resonance_term_dshape(m.kin, u.res[fl[f]], g12[j], g13[j], &am, &ag);
+            resonance_term_dshape(m.kin, u.res[fl[f]], g13[j], g12[j], &bm, &bg);
+            nm[2 * f].add(wj * (std::conj(A) * (u.c[fl[f]] * (am + bm))).real());
+            nm[2 * f + 1].add(wj * (std::conj(A) * (u.c[fl[f]] * (ag + bg))).real());
+        }
+    }
+    const long double Iv = I.value();
+    *nll = (double)(-S.value() + (long double)n_ev * logl(Iv));
+    for (int t = 0; t < 2 * F; ++t)
+        grad_shape[t] = (double)(-2.0L * ev[t].value() + 2.0L * (long double)n_ev / Iv * nm[t].value());
 }
 
 }  // extern "C"

@@ -68,6 +68,9 @@ def lib():
         L.orc_gram.restype = None; L.orc_gram.argtypes = model + [_dp, i64, _dp, _dp, _dp, _dp]
         L.orc_nll_grad.restype = None
         L.orc_nll_grad.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp]
+        L.orc_nll_grad_shape.restype = None
+        L.orc_nll_grad_shape.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp]
+        L.orc_resonance_term_dshape.restype = None; L.orc_resonance_term_dshape.argtypes = [kp, rp, d, d, _dp]
         _lib = L
     return _lib
 
@@ -145,6 +148,24 @@ class Oracle:
         self.L.orc_nll_grad(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w),
                             C.byref(nll), _p(grad))
         return nll.value, grad
+
+    def nll_grad_shape(self, params, e12, e13, g12, g13, w=None):
+        """(NLL, [d/dmass, d/dwidth of every shape_floats resonance in list order])  -- O10"""
+        p, e12, e13, g12, g13 = self._params(params), _a(e12), _a(e13), _a(g12), _a(g13)
+        w = None if w is None else _a(w)
+        nll = C.c_double()
+        F = sum(1 for r in self.resonances if r.get("shape_floats"))
+        grad = np.zeros(max(2 * F, 1))
+        self.L.orc_nll_grad_shape(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w),
+                                  C.byref(nll), _p(grad))
+        return nll.value, grad[:2 * F]
+
+    def resonance_term_dshape(self, r, x, y):
+        """(dT/dm0, dT/dGamma0) of one resonance dict r at (x, y)  -- O10"""
+        out = np.zeros(4)
+        ra = res_array([r])
+        self.L.orc_resonance_term_dshape(C.byref(self.kin), ra, float(x), float(y), _p(out))
+        return complex(out[0], out[1]), complex(out[2], out[3])
 
     def basis(self, params, s12, s13):
         p, a, b = self._params(params), _a(s12), _a(s13)
