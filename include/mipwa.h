@@ -124,11 +124,23 @@ int mipwa_nll_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, doub
                     double* integral);
 
 /* NLL and its analytic gradient with respect to the first 2N + 2R parameters (the linear coefficients in polar
- * form; derivatives with respect to floating masses/widths are not provided, reading P16).
+ * form; reading P16; mipwa_nll_grad_full adds the derivatives with respect to floating masses/widths).
  * grad: HOST, 2N + 2R doubles, laid out like params.  Works on cell-sorted copies of the points (implies
  * mipwa_prepare).  With fixed shapes and the path MIPWA_PATH_CACHED_COMPACT (or AUTO) the events are streamed from
  * the compact cache and the normalisation part comes from the Gram matrix; otherwise every term is recomputed. */
 int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
+
+/* NLL and its gradient with respect to ALL n_params parameters: the 2N + 2R entries of mipwa_nll_grad followed by
+ * (d/dmass, d/dwidth) of every shape_floats resonance in list order (not in the paper).  With
+ * T = F_D F_R Z / D, D = m0^2 - x - i m0 Gamma(x) (readings P9/P10), only the pole quantities q0^2 = q^2(m0^2) and
+ * p0*^2 = p*^2(m0^2) depend on m0:
+ *     dT/dGamma0 = T (i m0 Gamma(x) / Gamma0) / D
+ *     dT/dm0     = T d ln(F_R F_D)/dm0 - T (2 m0 - i m0 Gamma(x) d ln(m0 Gamma(x))/dm0) / D
+ *     dNLL/dtheta = -2 sum_i Re(conj(A_i) dA_i)/|A_i|^2 + (2 n_ev / I) sum_j w_j Re(conj(A_j) dA_j),
+ *     dA = c_r [dT_r(s12,s13) + dT_r(s13,s12)].
+ * grad: HOST, n_params doubles.  One extra pass over both point sets (k_grad_shape) per call when a shape floats;
+ * identical to mipwa_nll_grad when none does.  Errors as mipwa_nll_grad. */
+int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
 /* TEST HOOK: per-point |A|^2 from the same device function the NLL kernels use.
  *   which = 0: the events slot, 1: the normalisation slot; out: HOST, n doubles, n = that slot's size. */

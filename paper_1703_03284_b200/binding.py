@@ -23,7 +23,7 @@ _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STAT
 # every symbol include/mipwa.h declares
 SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
            "mipwa_prepare", "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
-           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
+           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version"]
 
@@ -71,6 +71,7 @@ def load_library():
     L.mipwa_nll.restype = i32; L.mipwa_nll.argtypes = [vp, _dp, i64, _dp]
     L.mipwa_nll_parts.restype = i32; L.mipwa_nll_parts.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_nll_grad.restype = i32; L.mipwa_nll_grad.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_nll_grad_full.restype = i32; L.mipwa_nll_grad_full.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_eval_abs2.restype = i32; L.mipwa_eval_abs2.argtypes = [vp, _dp, i64, i32, _dp, i64]
     L.mipwa_eval_basis.restype = i32; L.mipwa_eval_basis.argtypes = [vp, _dp, i64, i32, i64, i64, _dp]
     L.mipwa_enable_timing.restype = i32; L.mipwa_enable_timing.argtypes = [vp, i32]
@@ -218,6 +219,14 @@ class Mipwa:
         out = C.c_double()
         grad = np.empty(2 * self.N + 2 * self.R)
         self._check(self.L.mipwa_nll_grad(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
+        return out.value, grad
+
+    def nll_grad_full(self, params):
+        """(NLL, gradient over all n_params parameters incl. floating masses and widths)"""
+        p, pp, n = self._params(params)
+        out = C.c_double()
+        grad = np.empty(p.size)
+        self._check(self.L.mipwa_nll_grad_full(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
         return out.value, grad
 
     def eval_abs2(self, params, which=0):

@@ -30,8 +30,13 @@ struct ResDev {
     double Kw;        // m0^2 Gamma0 n_R / (2 (4 q0^2)^L sqrt(q0^2))   (the 1/2 of g = sqrt(lam1)/(2x) lives here)
     double cre, cim;  // c_r * sqrt(n_R n_D)
     double pa, pb, pc;// barrier denominator den_L(z) = pc + z (pb + pa z)
+    // shape derivatives (mipwa_nll_grad_full; only the pole quantities depend on m0, so these are per-call constants):
+    double sh_a1;     // d ln sqrt(n_R n_D) / d m0
+    double sh_a2;     // d ln(m0 Gamma(x)) / d m0 = 2/m0 - (L + 1/2) (dq0^2/dm0)/q0^2 + n_R'/n_R r^2 dq0^2/dm0
+    double sh_2m0;    // 2 m0
+    double sh_ig0;    // 1 / Gamma0
     int32_t L;
-    int32_t pad;
+    int32_t fl;       // index among the floating resonances (caller's list order), -1: shape fixed
 };
 
 // Everything a kernel needs for one likelihood call; passed by value as a __grid_constant__ kernel parameter.

@@ -443,3 +443,93 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
     __syncthreads();
     for (int k2 = threadIdx.x; k2 < nb; k2 += blockDim.x) mine[1 + 2 * R + k2] = grad_bins[k2];
 }
+
+
+// ---- derivatives with respect to floating masses and widths (mipwa_nll_grad_full) ---------------------
+// For a floating resonance in one channel, with D_R, D_D, W' = m0 Gamma(x) D_R, dD = (m0^2 - x) D_R, E = dD^2 + W'^2
+// (dev_model.cuh) and u = (dD + i W') / E  (so BW = D_R u and BW m0 Gamma = W' u):
+//   T'        = Z D_R rsqrt(D_R D_D) u                          (T without sqrt(n_R n_D), as everywhere in the kernels)
+//   dT'/dG0   = T' (i W' / Gamma0) u
+//   dT'/dm0   = T' [ a1 + u (-2 m0 D_R + i a2 W') ]             (a1, a2: ResDev::sh_a1, sh_a2)
+// Per point the kernel forms A (generic run-time amplitude), f = -2/conj(A) (events) or w A (normalisation points) and
+// adds f conj(dT'_sym) into 4 doubles per floating resonance and pass.  The host multiplies by conj(c_r sqrt(n_R n_D))
+// and takes the real part.  One instantiation per number of floating resonances handled per launch (1..4).
+#define MIPWA_SHAPE_MAXF 4
+struct ShapeSel { int32_t slot[MIPWA_SHAPE_MAXF]; };       // device slots of the floating resonances of this launch
+
+__device__ __forceinline__ void shape_channel(const ResDev& r, const Channel& c, double& mr, double& mi, double& gr,
+                                              double& gi)
+{
+    const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
+    const double DR = fma(zR, fma(zR, r.pa, r.pb), r.pc), DD = fma(zD, fma(zD, r.pa, r.pb), r.pc);
+    const double W = r.Kw * pick(r.L, c.w), Z = pick(r.L, c.Z);
+    const double dD = (r.m0sq - c.x) * DR;
+    const double rE = fast_rcp(fma(dD, dD, W * W));
+    const double ur = dD * rE, ui = W * rE;
+    const double t = Z * DR * fast_rsqrt(DR * DD);
+    const double tr = t * ur, ti = t * ui;                 // T'
+    const double k = r.sh_ig0 * W;                         // dT'/dG0 = T' (i k u)
+    const double xr = -k * ui, xi = k * ur;
+    gr = fma(tr, xr, -ti * xi); gi = fma(tr, xi, ti * xr);
+    const double p = -r.sh_2m0 * DR, q = r.sh_a2 * W;      // dT'/dm0 = T' [a1 + u (p + i q)]
+    const double br = r.sh_a1 + fma(ur, p, -ui * q), bi = fma(ur, q, ui * p);
+    mr = fma(tr, br, -ti * bi); mi = fma(tr, bi, ti * br);
+}
+
+template <int NF>
+__global__ void __launch_bounds__(256, 2)
+k_grad_shape(const __grid_constant__ DevModel m, const ShapeSel sel,
+             const double* __restrict__ e12, const double* __restrict__ e13, const unsigned short* __restrict__ eseg,
+             long long n_ev,
+             const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
+             const unsigned short* __restrict__ gseg, long long n_norm, double* __restrict__ partials)
+{
+    __shared__ SplineCoefSmem sm;
+    __shared__ double red32[32];
+    load_spline_coef_smem(sm, m);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double* mine = partials + (size_t)blockIdx.x * (8 * NF);
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        const double* s12 = pass == 0 ? e12 : g12;
+        const double* s13 = pass == 0 ? e13 : g13;
+        const unsigned short* sg = pass == 0 ? eseg : gseg;
+        const long long n = pass == 0 ? n_ev : n_norm;
+        double acc[NF][4];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) acc[f][0] = acc[f][1] = acc[f][2] = acc[f][3] = 0.0;
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+            const double x = s12[i], y = s13[i];
+            double are, aim;
+            amplitude_seg<-1, -1, 0>(sm, m, x, y, sg[i], are, aim);
+            double fr, fi;
+            if (pass == 0) {
+                const double k = -2.0 * fast_rcp(fma(are, are, aim * aim));
+                fr = k * are; fi = k * aim;                // -2 / conj(A)
+            } else {
+                const double w = gw ? gw[i] : 1.0;
+                fr = w * are; fi = w * aim;
+            }
+            const Channel ca = make_channel<0>(m, x, y), cb = make_channel<0>(m, y, x);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                const ResDev& r = m.res[sel.slot[f]];
+                double amr, ami, agr, agi, bmr, bmi, bgr, bgi;
+                shape_channel(r, ca, amr, ami, agr, agi);
+                shape_channel(r, cb, bmr, bmi, bgr, bgi);
+                const double dmr = amr + bmr, dmi = ami + bmi, dgr = agr + bgr, dgi = agi + bgi;
+                acc[f][0] = fma(fr, dmr, fma(fi, dmi, acc[f][0]));      // f conj(dT'/dm0)
+                acc[f][1] = fma(fi, dmr, fma(-fr, dmi, acc[f][1]));
+                acc[f][2] = fma(fr, dgr, fma(fi, dgi, acc[f][2]));      // f conj(dT'/dG0)
+                acc[f][3] = fma(fi, dgr, fma(-fr, dgi, acc[f][3]));
+            }
+        }
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const double v = block_sum(acc[f][q], red32);
+                if (threadIdx.x == 0) mine[(pass * NF + f) * 4 + q] = v;
+            }
+    }
+}

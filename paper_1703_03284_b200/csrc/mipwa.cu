@@ -152,7 +152,20 @@ int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, 
     out->pb = L == 2 ? 3.0 : (L == 1 ? 1.0 : 0.0);
     out->pc = L == 2 ? 9.0 : 1.0;
     out->L = L;
-    out->pad = 0;
+    out->fl = -1;
+    // shape derivatives: only q0^2 and p0*^2 depend on m0 (include/mipwa.h, mipwa_nll_grad_full)
+    {
+        const double m1s = k.m1 * k.m1, m2s = k.m2 * k.m2, m3s = k.m3 * k.m3;
+        const double dq0 = 0.5 * m0 * (1.0 - (m1s - m2s) * (m1s - m2s) / (m0sq * m0sq));
+        const double dp0 = m0 * (m0sq - M2 - m3s) / M2;
+        auto dlog_num = [L](double z0) { return L == 0 ? 0.0 : (L == 1 ? 1.0 / (1.0 + z0) : (3.0 + 2.0 * z0) / (9.0 + 3.0 * z0 + z0 * z0)); };
+        const double rr = d.r_res * d.r_res, rp = d.r_parent * d.r_parent;
+        const double dlnFR = 0.5 * dlog_num(rr * q0sq) * rr * dq0, dlnFD = 0.5 * dlog_num(rp * p0sq) * rp * dp0;
+        out->sh_a1 = dlnFR + dlnFD;
+        out->sh_a2 = 2.0 / m0 - (L + 0.5) * dq0 / q0sq + 2.0 * dlnFR;
+        out->sh_2m0 = 2.0 * m0;
+        out->sh_ig0 = 1.0 / g0;
+    }
     return MIPWA_OK;
 }
 
@@ -265,6 +278,7 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
         if (fidx[r] >= 0) { m0 = p[2 * N + 2 * R + 2 * fidx[r]]; g0 = p[2 * N + 2 * R + 2 * fidx[r] + 1]; }
         const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[d], &c->res_fold[d]);
         if (rc) return rc;
+        m.res[d].fl = fidx[r];
     }
     return MIPWA_OK;
 }
@@ -1198,6 +1212,73 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
         Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
     }
     polar_chain(c, params, Gy.data(), Gr.data(), grad);
+    return MIPWA_OK;
+}
+
+// value + gradient over ALL n_params parameters: mipwa_nll_grad for the 2N + 2R linear-coefficient parameters, then
+// k_grad_shape for (mass, width) of every floating resonance (layout of grad = layout of params)
+int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+{
+    int rc = mipwa_nll_grad(c, params, n_params, nll, grad);
+    if (rc || c->F == 0) return rc;
+    const int N = c->N, R = c->R, F = c->F;
+    constexpr int SHAPE_OFF = 3900;                        // in h_result, clear of the main gradient's NV <= 2098 values
+    const double* h = c->h_result;
+    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
+    const double I = h[1] * wn, n_ev = (double)c->ev.n;
+    const double scale = c->ev.n > 0 ? 2.0 * n_ev / I * wn : 0.0;
+    std::vector<int> slots;                                // device slot of each floating resonance, list order
+    for (int f = 0; f < F; ++f)
+        for (int d = 0; d < R; ++d)
+            if (c->model.res[d].fl == f) slots.push_back(d);
+    if ((int)slots.size() != F) return fail(c, MIPWA_ERR_STATE, "floating resonance not found in the device model");
+    const int64_t need = (std::max(c->ev.n, c->nm.n) + 255) / 256;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * 2, need));
+    const size_t want = (size_t)grid * 8 * MIPWA_SHAPE_MAXF;
+    if (c->gpartials_len < want) {
+        if (c->d_gpartials) cudaFree(c->d_gpartials);
+        c->d_gpartials = nullptr; c->gpartials_len = 0;
+        CU(c, cudaMalloc(&c->d_gpartials, want * sizeof(double)));
+        c->gpartials_len = want;
+    }
+    const Slot& E = evs(c);
+    const Slot& G = nms(c);
+    float ms_total = c->last_ms;
+    for (int f0 = 0; f0 < F; f0 += MIPWA_SHAPE_MAXF) {
+        const int nf = std::min(MIPWA_SHAPE_MAXF, F - f0);
+        ShapeSel sel;
+        for (int q = 0; q < MIPWA_SHAPE_MAXF; ++q) sel.slot[q] = slots[f0 + std::min(q, nf - 1)];
+        if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+#define MIPWA_SHAPE_LAUNCH(NF)                                                                                     \
+    k_grad_shape<NF><<<grid, 256, 0, c->stream>>>(c->model, sel, E.s12, E.s13, E.seg, E.n, G.s12, G.s13, G.w, G.seg, \
+                                                  G.n, c->d_gpartials)
+        switch (nf) {
+            case 1: MIPWA_SHAPE_LAUNCH(1); break;
+            case 2: MIPWA_SHAPE_LAUNCH(2); break;
+            case 3: MIPWA_SHAPE_LAUNCH(3); break;
+            default: MIPWA_SHAPE_LAUNCH(4); break;
+        }
+#undef MIPWA_SHAPE_LAUNCH
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        k_grad_finalize<<<(8 * nf + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, 8 * nf, c->d_result + SHAPE_OFF);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        if (c->timing) { float ms = 0.f; CU(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1)); ms_total += ms; }
+        const double* D = c->h_result + SHAPE_OFF;         // [pass][f][dm_re, dm_im, dG_re, dG_im]
+        for (int q = 0; q < nf; ++q) {
+            const ResDev& rd = c->model.res[slots[f0 + q]];
+            const double* e = D + (0 * nf + q) * 4;
+            const double* g = D + (1 * nf + q) * 4;
+            for (int t = 0; t < 2; ++t) {                  // t = 0: mass, 1: width
+                const double dr = e[2 * t] + scale * g[2 * t], di = e[2 * t + 1] + scale * g[2 * t + 1];
+                grad[2 * N + 2 * R + 2 * (f0 + q) + t] = rd.cre * dr + rd.cim * di;   // Re(conj(c sqrt(n_R n_D)) D)
+            }
+        }
+    }
+    c->last_ms = ms_total;
     return MIPWA_OK;
 }
 

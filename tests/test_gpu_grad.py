@@ -143,3 +143,58 @@ def test_gradient_on_the_compact_cached_path(case):
         _, ref_g = o.nll_grad(p, data[0][:n], data[1][:n], data[2], data[3], data[4])
         _check(m.nll_grad(p)[1], ref_g)
     m.close()
+
+
+def test_full_gradient_with_floating_shapes_matches_oracle():
+    """mipwa_nll_grad_full: the 2N + 2R coefficient derivatives plus d/d(mass, width) of every floating resonance
+    (k_grad_shape) against the oracle's O10, which tests/test_oracle_shape.py pins to finite differences.
+    Config 3 (rho(770) floats; ragged sizes) and a K- pi+ pi+ like model with two floating resonances of spin 1
+    and 2 next to a fixed scalar, unweighted normalisation points."""
+    B = _lib()
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    c, o, (e12, e13, g12, g13, w) = make_case(3, n_ev=25_003, n_norm=31_001)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(e12, e13); m.set_norm_points(g12, g13, w); m.set_path(B.PATH_RECOMPUTE)
+    p = c.perturbed(1)
+    v, g = m.nll_grad_full(p)
+    ref_n, gref = o.nll_grad(p, e12, e13, g12, g13, w)
+    _, gs = o.nll_grad_shape(p, e12, e13, g12, g13, w)
+    full = np.concatenate([gref, gs])
+    assert g.size == c.n_params == full.size
+    _, sl, integ = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    assert abs(v - ref_n) <= nll_tol(ref_n, sl, integ, e12.size)
+    assert np.max(np.abs(g - full)) <= 1e-9 * np.max(np.abs(full))
+    assert np.max(np.abs(g[-2:] - gs)) <= 1e-9 * np.max(np.abs(gs))       # the shape entries on their own scale
+    m.close()
+
+    kin = {"M": 1.86966, "m1": 0.493677, "m2": 0.13957, "m3": 0.13957}
+    lo, hi = I.s_limits(kin)
+    res = [dict(mass=0.8955, width=0.047, spin=1, r_res=1.5, r_parent=5.0, shape_floats=1),
+           dict(mass=1.2, width=0.2, spin=0, r_res=1.5, r_parent=5.0, shape_floats=0),
+           dict(mass=1.4324, width=0.109, spin=2, r_res=2.0, r_parent=4.0, shape_floats=1)]
+    knots = np.linspace(lo - 1e-3, hi + 1e-3, 9)
+    o2 = orc.Oracle(kin, knots, res)
+    s12, s13 = I.phase_space_points(9000, I.stream_key(3, 12, 1), kin)
+    e12, e13, g12, g13 = s12[:4001], s13[:4001], s12[4001:], s13[4001:]
+    rng = np.random.default_rng(3)
+    p = np.concatenate([rng.uniform(0.5, 2, 9), rng.uniform(0, 3, 9), rng.uniform(0.3, 1.5, 6),
+                        [0.8955, 0.047, 1.4324, 0.109]])
+    m2 = B.Mipwa(kin, knots, res)
+    m2.set_events(e12, e13); m2.set_norm_points(g12, g13, None); m2.set_path(B.PATH_RECOMPUTE)
+    v, g = m2.nll_grad_full(p)
+    ref_n, gref = o2.nll_grad(p, e12, e13, g12, g13, None)
+    _, gs = o2.nll_grad_shape(p, e12, e13, g12, g13, None)
+    full = np.concatenate([gref, gs])
+    assert np.max(np.abs(g - full)) <= 1e-9 * np.max(np.abs(full))
+    assert np.max(np.abs(g[-4:] - gs)) <= 1e-9 * np.max(np.abs(gs))
+    m2.close()
+
+    # no floating shape: the same call as mipwa_nll_grad (shared-memory flush order may differ in the last bits)
+    c0, o0, (e12, e13, g12, g13, w) = make_case(0)
+    m0 = B.Mipwa(c0.kin, c0.knots, c0.resonances)
+    m0.set_events(e12, e13); m0.set_norm_points(g12, g13, w)
+    va, ga = m0.nll_grad(c0.truth)
+    vb, gb = m0.nll_grad_full(c0.truth)
+    assert va == vb and np.max(np.abs(ga - gb)) <= 1e-12 * np.max(np.abs(ga))
+    m0.close()
