@@ -260,6 +260,20 @@ def run_ours(args, cfg, workload):
     grad_info = {"ms_per_call": 1e3 * grad_wall, "kernel_ms": float(np.mean(grad_ms)),
                  "events_per_s": n_ev * world / grad_wall, "n_grad": int(grad.size), "nll": nll_g,
                  "what": "mipwa_nll_grad: NLL + d/d(a_k, phi_k, |c_r|, arg c_r), same sample, k_grad_recompute"}
+    # all n_params derivatives, incl. d/d(mass, width) of the floating rho(770) (k_grad_shape, one extra pass)
+    for t in range(2):
+        m.nll_grad_full(params[t])
+    full_ms = []
+    barrier()
+    t0 = time.perf_counter()
+    for t in range(sub_steps):
+        nll_f, grad_f = m.nll_grad_full(params[args.warmup + t % args.steps])
+        full_ms.append(m.last_kernel_ms())
+    barrier()
+    full_wall = (time.perf_counter() - t0) / sub_steps
+    grad_info["full"] = {"ms_per_call": 1e3 * full_wall, "kernel_ms": float(np.mean(full_ms)), "n_grad": int(grad_f.size),
+                         "d_mass_d_width": [float(x) for x in grad_f[grad.size:]],
+                         "what": "mipwa_nll_grad_full: the above + d/d(mass, width) of every floating resonance"}
 
     # ---- hybrid path (AUTO's choice for this model): rho(770) recomputed, rho(1450) and f2(1270) cached per point -------
     hybrid_info = None

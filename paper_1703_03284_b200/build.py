@@ -1,27 +1,40 @@
-"""Build libmipwa.so (CUDA, sm_100a only) in-tree with nvcc.  `python -m paper_1703_03284_b200.build [--force]`."""
+"""Build libmipwa.so (CUDA, sm_100a only) in-tree with nvcc.  `python -m paper_1703_03284_b200.build [--force]`.
+
+The heavily specialised kernel families live in their own translation units (csrc/tu_*.cu, csrc/launch.h); the
+objects are compiled in parallel and linked into one shared library."""
 import glob
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "csrc", "mipwa.cu")
+CSRC = os.path.join(HERE, "csrc")
+UNITS = ["mipwa.cu", "tu_recompute.cu", "tu_abs2.cu", "tu_grad.cu", "tu_hybrid.cu"]
 LIB = os.path.join(HERE, "libmipwa.so")
-NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-shared",
-              "-Xcompiler", "-fPIC"]
+OBJ_DIR = os.path.join(HERE, "_obj")
+NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
 def sources():
-    return sorted(f for f in glob.glob(os.path.join(HERE, "csrc", "*.cu*")) if not f.endswith("fp64_microbench.cu")) \
-        + [os.path.join(HERE, "..", "include", "mipwa.h")]
+    return sorted(f for f in glob.glob(os.path.join(CSRC, "*.cu*")) + glob.glob(os.path.join(CSRC, "*.h"))
+                  if not f.endswith("fp64_microbench.cu")) + [os.path.join(HERE, "..", "include", "mipwa.h")]
 
 
-def build(force=False, verbose=False):
+def build(force=False, verbose=False, extra=()):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in sources()):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB, SRC]
-    subprocess.run(cmd, check=True)
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    flags = NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + list(extra)
+
+    def compile_unit(u):
+        obj = os.path.join(OBJ_DIR, u.replace(".cu", ".o"))
+        subprocess.run([nvcc] + flags + ["-c", "-o", obj, os.path.join(CSRC, u)], check=True)
+        return obj
+    with ThreadPoolExecutor(max_workers=len(UNITS)) as pool:
+        objs = list(pool.map(compile_unit, UNITS))
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs, check=True)
     return LIB
 
 
@@ -30,7 +43,7 @@ def build_microbench():
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     out = os.path.join(HERE, "fp64_microbench")
     subprocess.run([nvcc, "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-o", out,
-                    os.path.join(HERE, "csrc", "fp64_microbench.cu")], check=True)
+                    os.path.join(CSRC, "fp64_microbench.cu")], check=True)
     return out
 
 
@@ -38,4 +51,5 @@ if __name__ == "__main__":
     if "--microbench" in sys.argv:
         print(build_microbench())
     else:
-        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                    extra=[a for a in sys.argv[1:] if a.startswith("-D")]))

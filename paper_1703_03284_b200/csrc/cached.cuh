@@ -99,7 +99,7 @@ k_basis_build(const __grid_constant__ DevModel m, const BasisAux aux, const doub
 }
 
 // ---- test hook: basis rows, row-major out[i*K + k] ----------------------------------------------------------------
-__global__ void __launch_bounds__(MIPWA_TILE)
+static __global__ void __launch_bounds__(MIPWA_TILE)
 k_basis_rows(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ s12,
              const double* __restrict__ s13, long long first, long long n, double2* __restrict__ out)
 {
@@ -172,7 +172,7 @@ __device__ __forceinline__ double2 ld_stream(const double2* p)
 #ifndef MIPWA_DENSE_MINBLOCKS
 #define MIPWA_DENSE_MINBLOCKS 4
 #endif
-__global__ void __launch_bounds__(MIPWA_TILE, MIPWA_DENSE_MINBLOCKS)
+static __global__ void __launch_bounds__(MIPWA_TILE, MIPWA_DENSE_MINBLOCKS)
 k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cache, long long n_ev,
             const double2* __restrict__ G, double* __restrict__ partials, unsigned int* __restrict__ ticket,
             double* __restrict__ result)
@@ -385,7 +385,7 @@ k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __r
     }
 }
 
-__global__ void k_gram_reduce(const double2* __restrict__ partial, int nblocks, int K, double2* __restrict__ G)
+static __global__ void k_gram_reduce(const double2* __restrict__ partial, int nblocks, int K, double2* __restrict__ G)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= K * K) return;

@@ -296,7 +296,7 @@ k_grad_recompute(const __grid_constant__ DevModel m,
 // fixed-order sum of the per-block partial vectors: one warp per value, lane l adds blocks l, l+32, .. then a shuffle
 // tree.  A separate tiny launch: done inside the last block of k_grad_recompute it would serialise ~NV x grid L2 reads
 // on one SM while the rest of the GPU idles.
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 k_grad_finalize(const double* __restrict__ partials, int nblocks, int NV, double* __restrict__ result)
 {
     const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
@@ -309,7 +309,7 @@ k_grad_finalize(const double* __restrict__ partials, int nblocks, int NV, double
 }
 
 // ---- cell sort (once per point set): key = seg(s12) * (N-1) + seg(s13) ---------------------------------------------
-__global__ void __launch_bounds__(MIPWA_TILE)
+static __global__ void __launch_bounds__(MIPWA_TILE)
 k_cell_keys(const unsigned short* __restrict__ seg, long long n, int NS, unsigned int* __restrict__ keys,
             unsigned int* __restrict__ idx)
 {
@@ -321,7 +321,7 @@ k_cell_keys(const unsigned short* __restrict__ seg, long long n, int NS, unsigne
     }
 }
 
-__global__ void __launch_bounds__(MIPWA_TILE)
+static __global__ void __launch_bounds__(MIPWA_TILE)
 k_gather(const unsigned int* __restrict__ idx, long long n, const double* __restrict__ a, const double* __restrict__ b,
          const double* __restrict__ c, const unsigned short* __restrict__ sg, double* __restrict__ oa,
          double* __restrict__ ob, double* __restrict__ oc, unsigned short* __restrict__ osg)

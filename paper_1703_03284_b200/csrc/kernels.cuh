@@ -211,7 +211,7 @@ struct DevKin { double M2, m1s, m2s, m3s, t_lo, t_d, s_hi, s_top; };
 
 // Also stores the spline segment pair of every point, seg[i] = j12 | j13 << 8 (knots are fixed at mipwa_create, so
 // the pair is a property of the point set): the per-call kernels then index the coefficient tables directly.
-__global__ void __launch_bounds__(MIPWA_BLOCK)
+static __global__ void __launch_bounds__(MIPWA_BLOCK)
 k_validate(const DevKin k, const __grid_constant__ DevModel m, const double* __restrict__ s12,
            const double* __restrict__ s13, long long n, unsigned short* __restrict__ seg,
            unsigned long long* __restrict__ bad)
@@ -240,7 +240,7 @@ k_validate(const DevKin k, const __grid_constant__ DevModel m, const double* __r
 }
 
 // ---- FP64 peak: register-resident dependent-chain DFMA loop, 8 independent chains per thread --------------------
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 k_dfma_peak(double* __restrict__ out, long long iters, double a, double b)
 {
     double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;

@@ -1,0 +1,37 @@
+// launch.h -- host launchers of the heavily specialised kernels (model signature x model flags), one translation unit
+// per kernel family so that the library builds in parallel (build.py).  Internal to libmipwa.so; plain pointers only.
+#pragma once
+#include <cuda_runtime.h>
+#include "dev_model.cuh"
+
+struct HybCoef;
+
+// n_spin = resonances of spin 0, 1, 2 (the kernel signature), fl = MIPWA_FL_* of the model.  Every launcher returns
+// cudaGetLastError() of its launch; the occupancy functions return the resident blocks per SM of the matching kernel.
+
+// tu_recompute.cu: k_nll_recompute; tu_abs2.cu: k_abs2 (kernels.cuh)
+cudaError_t mipwa_occupancy_nll_recompute(const int* n_spin, int fl, int* blocks_per_sm);
+cudaError_t mipwa_launch_nll_recompute(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
+                                       const double* e12, const double* e13, const unsigned short* eseg, long long n_ev,
+                                       const double* g12, const double* g13, const double* gw,
+                                       const unsigned short* gseg, long long n_norm, double2* partials,
+                                       unsigned int* ticket, double* result);
+cudaError_t mipwa_launch_abs2(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
+                              const double* s12, const double* s13, const unsigned short* seg, long long n, double* out);
+
+// tu_grad.cu: k_grad_recompute (grad.cuh)
+cudaError_t mipwa_occupancy_grad_recompute(const int* n_spin, int fl, size_t smem, int* blocks_per_sm);
+cudaError_t mipwa_launch_grad_recompute(const int* n_spin, int fl, int grid, size_t smem, cudaStream_t st,
+                                        const DevModel& m, const double* e12, const double* e13,
+                                        const unsigned short* eseg, long long n_ev, const double* g12,
+                                        const double* g13, const double* gw, const unsigned short* gseg,
+                                        long long n_norm, double* partials);
+
+// tu_hybrid.cu: k_nll_hybrid (hybrid.cuh); f1, f2 = floating resonances of spin 1, 2, rc = cached (fixed) resonances
+bool mipwa_hybrid_supported(int f1, int f2, int rc);
+cudaError_t mipwa_occupancy_nll_hybrid(int f1, int f2, int rc, int fl, int* blocks_per_sm);
+cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cudaStream_t st, const DevModel& m,
+                                    const HybCoef& cc, const double2* ev_cache, const unsigned short* eseg,
+                                    long long n_ev, const double2* nm_cache, const double* gw,
+                                    const unsigned short* gseg, long long n_norm, double2* partials,
+                                    unsigned int* ticket, double* result);

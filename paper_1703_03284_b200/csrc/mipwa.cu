@@ -9,6 +9,7 @@
 #include <string>
 #include <vector>
 
+#include "launch.h"
 #include "kernels.cuh"
 #include "cached.cuh"
 #include "grad.cuh"
@@ -359,7 +360,7 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     for (int r = 0; r < n_res; ++r) if (!res[r].shape_floats) c->hyb_fixed.push_back(r);
     {
         bool supported = (int)c->hyb_float.size() == c->F && c->F > 0 && !c->hyb_fixed.empty();   // no floating spin 0
-        if (supported) { MIPWA_DISPATCH_HYB(c->hyb_f1, c->hyb_f2, (int)c->hyb_fixed.size(), (void)0); }
+        if (supported) supported = mipwa_hybrid_supported(c->hyb_f1, c->hyb_f2, (int)c->hyb_fixed.size());
         c->hyb_ok = supported;
     }
     if (kin->m1 == kin->m2) c->model_flags |= MIPWA_FL_EQM;
@@ -391,9 +392,7 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     }
 
     bool ok = true;
-    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
-                       ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->blocks_per_sm, k_nll_recompute<R1, R2, FL>,
-                                                                          MIPWA_REC_BLOCK, 0) == cudaSuccess);
+    ok = mipwa_occupancy_nll_recompute(c->n_spin, c->model_flags, &c->blocks_per_sm) == cudaSuccess;
     if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
 #ifdef MIPWA_FORCE_BPS
     c->blocks_per_sm = MIPWA_FORCE_BPS;                    // experiments only
@@ -549,11 +548,11 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     const int64_t need = (std::max(c->ev.n, c->nm.n) + MIPWA_REC_BLOCK - 1) / MIPWA_REC_BLOCK;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags, (k_nll_recompute<R1, R2, FL><<<grid, MIPWA_REC_BLOCK, 0, c->stream>>>(
-                               c->model, evs(c).s12, evs(c).s13, evs(c).seg, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w,
-                               nms(c).seg, nms(c).n, c->d_partials, c->d_ticket, c->d_result)));
+    const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, evs(c).s12,
+                                                      evs(c).s13, evs(c).seg, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w,
+                                                      nms(c).seg, nms(c).n, c->d_partials, c->d_ticket, c->d_result);
     ++c->launches;
-    CU(c, cudaGetLastError());
+    CU(c, le);
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
@@ -794,22 +793,19 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     }
     bool supported = true;
     if (!c->hyb_blocks_per_sm) {
-        MIPWA_DISPATCH_HYBFL(c->hyb_f1, c->hyb_f2, RC, c->model_flags,
-                           supported = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->hyb_blocks_per_sm, k_nll_hybrid<R1, R2, RCT, FL>,
-                                                                                     MIPWA_TILE, 0) == cudaSuccess);
+        supported = mipwa_occupancy_nll_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, &c->hyb_blocks_per_sm) == cudaSuccess;
         if (!supported) return fail(c, MIPWA_ERR_CUDA, "hybrid: occupancy query failed");
         if (c->hyb_blocks_per_sm < 1) c->hyb_blocks_per_sm = 1;
     }
     const int64_t tiles = (std::max(c->ev.n, c->nm.n) + MIPWA_TILE - 1) / MIPWA_TILE;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->hyb_blocks_per_sm));
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_HYBFL(c->hyb_f1, c->hyb_f2, RC, c->model_flags,
-                       (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_TILE, 0, c->stream>>>(
-                           c->model, cc, (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n, (const double2*)c->d_hyb_nm,
-                           nms(c).w, nms(c).seg, c->nm.n,
-                           c->d_partials, c->d_ticket, c->d_result)));
+    const cudaError_t le = mipwa_launch_nll_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, grid, c->stream, c->model, cc,
+                                                   (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n,
+                                                   (const double2*)c->d_hyb_nm, nms(c).w, nms(c).seg, c->nm.n,
+                                                   c->d_partials, c->d_ticket, c->d_result);
     ++c->launches;
-    CU(c, cudaGetLastError());
+    CU(c, le);
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
@@ -856,10 +852,9 @@ int mipwa_eval_abs2(mipwa_ctx* c, const double* params, int64_t n_params, int32_
     if (n == 0) return MIPWA_OK;
     double* d_out = nullptr;
     CU(c, cudaMalloc(&d_out, (size_t)n * sizeof(double)));
-    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
-                       (k_abs2<R1, R2, FL><<<grid_for(c, n, 4), MIPWA_BLOCK, 0, c->stream>>>(c->model, s.s12, s.s13, s.seg, n, d_out)));
+    cudaError_t e = mipwa_launch_abs2(c->n_spin, c->model_flags, grid_for(c, n, 4), c->stream, c->model, s.s12, s.s13,
+                                      s.seg, n, d_out);
     ++c->launches;
-    cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     cudaFree(d_out);
@@ -1163,9 +1158,7 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     const size_t smem = (size_t)2 * nb * sizeof(double);
     if (!c->grad_blocks_per_sm) {
         bool ok = true;
-        MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
-                           ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->grad_blocks_per_sm, k_grad_recompute<R1, R2, FL>,
-                                                                              MIPWA_GRAD_BLOCK, smem) == cudaSuccess);
+        ok = mipwa_occupancy_grad_recompute(c->n_spin, c->model_flags, smem, &c->grad_blocks_per_sm) == cudaSuccess;
         if (!ok) return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
         if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
     }
@@ -1178,13 +1171,12 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
         c->gpartials_len = (size_t)grid * NV;
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    MIPWA_DISPATCH_SIGFL(c->n_spin[0], c->n_spin[1], c->n_spin[2], c->model_flags,
-                       (k_grad_recompute<R1, R2, FL><<<grid, MIPWA_GRAD_BLOCK, smem, c->stream>>>(
-                           c->model, c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, c->ev_sorted.n,
-                           c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w, c->nm_sorted.seg, c->nm_sorted.n,
-                           c->d_gpartials)));
+    const cudaError_t le = mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model,
+                                                       c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, c->ev_sorted.n,
+                                                       c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w, c->nm_sorted.seg,
+                                                       c->nm_sorted.n, c->d_gpartials);
     ++c->launches;
-    CU(c, cudaGetLastError());
+    CU(c, le);
     k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());

@@ -1,0 +1,34 @@
+// tu_hybrid.cu -- instantiations and launchers of k_nll_hybrid (hybrid.cuh); see launch.h
+#include "launch.h"
+#include "kernels.cuh"
+#include "hybrid.cuh"
+
+bool mipwa_hybrid_supported(int f1, int f2, int rc)
+{
+    bool supported = true;
+    MIPWA_DISPATCH_HYB(f1, f2, rc, (void)0);
+    return supported;
+}
+
+cudaError_t mipwa_occupancy_nll_hybrid(int f1, int f2, int rc, int fl, int* blocks_per_sm)
+{
+    bool supported = true;
+    cudaError_t e = cudaSuccess;
+    MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl,
+                         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_nll_hybrid<R1, R2, RCT, FL>,
+                                                                           MIPWA_TILE, 0));
+    return supported ? e : cudaErrorInvalidValue;
+}
+
+cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cudaStream_t st, const DevModel& m,
+                                    const HybCoef& cc, const double2* ev_cache, const unsigned short* eseg,
+                                    long long n_ev, const double2* nm_cache, const double* gw,
+                                    const unsigned short* gseg, long long n_norm, double2* partials,
+                                    unsigned int* ticket, double* result)
+{
+    bool supported = true;
+    MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl,
+                         (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_TILE, 0, st>>>(
+                             m, cc, ev_cache, eseg, n_ev, nm_cache, gw, gseg, n_norm, partials, ticket, result)));
+    return supported ? cudaGetLastError() : cudaErrorInvalidValue;
+}
