@@ -168,6 +168,7 @@ template <int R1, int R2, int FL, bool EV>
 __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevModel& m, const double* __restrict__ s12,
                                           const double* __restrict__ s13, const double* __restrict__ w,
                                           const unsigned short* __restrict__ sgp, long long n,
+                                          double2* __restrict__ fout,
                                           double* bins, double& scalar, double (&Fr)[GradDims<R1, R2>::RR],
                                           double (&Fi)[GradDims<R1, R2>::RR])
 {
@@ -212,6 +213,7 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
             fr = wv * are; fi = wv * aim;
             integ = fma(wv, a2, integ);
         }
+        if (fout && valid) fout[i] = make_double2(fr, fi);                // for k_grad_shape (mipwa_nll_grad_full)
         if (R1 >= 0) {
 #pragma unroll
             for (int r = 0; r < (R1 >= 0 ? R1 + R2 : 0); ++r) {
@@ -257,7 +259,8 @@ k_grad_recompute(const __grid_constant__ DevModel m,
                  const double* __restrict__ e12, const double* __restrict__ e13,
                  const unsigned short* __restrict__ eseg, long long n_ev,
                  const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
-                 const unsigned short* __restrict__ gseg, long long n_norm, double* __restrict__ partials)
+                 const unsigned short* __restrict__ gseg, long long n_norm, double* __restrict__ partials,
+                 double2* __restrict__ f_ev, double2* __restrict__ f_nm)
 {
     constexpr int RR = GradDims<R1, R2>::RR;
     extern __shared__ double grad_bins[];                  // [2][4][N-1][2]
@@ -275,8 +278,8 @@ k_grad_recompute(const __grid_constant__ DevModel m,
         double Sc = 0.0, Fr[RR], Fi[RR];
 #pragma unroll
         for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
-        if (pass == 0) grad_pass<R1, R2, FL, true>(sm, m, e12, e13, nullptr, eseg, n_ev, grad_bins, Sc, Fr, Fi);
-        else grad_pass<R1, R2, FL, false>(sm, m, g12, g13, gw, gseg, n_norm, grad_bins + nb, Sc, Fr, Fi);
+        if (pass == 0) grad_pass<R1, R2, FL, true>(sm, m, e12, e13, nullptr, eseg, n_ev, f_ev, grad_bins, Sc, Fr, Fi);
+        else grad_pass<R1, R2, FL, false>(sm, m, g12, g13, gw, gseg, n_norm, f_nm, grad_bins + nb, Sc, Fr, Fi);
         double v = block_sum(Sc, red32);
         if (threadIdx.x == 0) mine[pass] = v;
         for (int r = 0; r < R; ++r) {
@@ -451,9 +454,10 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
 //   T'        = Z D_R rsqrt(D_R D_D) u                          (T without sqrt(n_R n_D), as everywhere in the kernels)
 //   dT'/dG0   = T' (i W' / Gamma0) u
 //   dT'/dm0   = T' [ a1 + u (-2 m0 D_R + i a2 W') ]             (a1, a2: ResDev::sh_a1, sh_a2)
-// Per point the kernel forms A (generic run-time amplitude), f = -2/conj(A) (events) or w A (normalisation points) and
-// adds f conj(dT'_sym) into 4 doubles per floating resonance and pass.  The host multiplies by conj(c_r sqrt(n_R n_D))
-// and takes the real part.  One instantiation per number of floating resonances handled per launch (1..4).
+// k_grad_recompute stores its per-point factor f (-2/conj(A) for events, w A for normalisation points) when asked to;
+// this kernel streams (s12, s13, f), evaluates the two channels of every floating resonance and adds f conj(dT'_sym)
+// into 4 doubles per floating resonance and pass.  The host multiplies by conj(c_r sqrt(n_R n_D)) and takes the real
+// part.  One instantiation per number of floating resonances handled per launch (1..4).
 #define MIPWA_SHAPE_MAXF 4
 struct ShapeSel { int32_t slot[MIPWA_SHAPE_MAXF]; };       // device slots of the floating resonances of this launch
 
@@ -479,37 +483,27 @@ __device__ __forceinline__ void shape_channel(const ResDev& r, const Channel& c,
 template <int NF>
 __global__ void __launch_bounds__(256, 2)
 k_grad_shape(const __grid_constant__ DevModel m, const ShapeSel sel,
-             const double* __restrict__ e12, const double* __restrict__ e13, const unsigned short* __restrict__ eseg,
+             const double* __restrict__ e12, const double* __restrict__ e13, const double2* __restrict__ f_ev,
              long long n_ev,
-             const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
-             const unsigned short* __restrict__ gseg, long long n_norm, double* __restrict__ partials)
+             const double* __restrict__ g12, const double* __restrict__ g13, const double2* __restrict__ f_nm,
+             long long n_norm, double* __restrict__ partials)
 {
-    __shared__ SplineCoefSmem sm;
     __shared__ double red32[32];
-    load_spline_coef_smem(sm, m);
     const long long stride = (long long)gridDim.x * blockDim.x;
     double* mine = partials + (size_t)blockIdx.x * (8 * NF);
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
         const double* s12 = pass == 0 ? e12 : g12;
         const double* s13 = pass == 0 ? e13 : g13;
-        const unsigned short* sg = pass == 0 ? eseg : gseg;
+        const double2* fp = pass == 0 ? f_ev : f_nm;
         const long long n = pass == 0 ? n_ev : n_norm;
         double acc[NF][4];
 #pragma unroll
         for (int f = 0; f < NF; ++f) acc[f][0] = acc[f][1] = acc[f][2] = acc[f][3] = 0.0;
         for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
             const double x = s12[i], y = s13[i];
-            double are, aim;
-            amplitude_seg<-1, -1, 0>(sm, m, x, y, sg[i], are, aim);
-            double fr, fi;
-            if (pass == 0) {
-                const double k = -2.0 * fast_rcp(fma(are, are, aim * aim));
-                fr = k * are; fi = k * aim;                // -2 / conj(A)
-            } else {
-                const double w = gw ? gw[i] : 1.0;
-                fr = w * are; fi = w * aim;
-            }
+            const double2 fv = fp[i];
+            const double fr = fv.x, fi = fv.y;
             const Channel ca = make_channel<0>(m, x, y), cb = make_channel<0>(m, y, x);
 #pragma unroll
             for (int f = 0; f < NF; ++f) {

@@ -25,7 +25,7 @@ cudaError_t mipwa_launch_grad_recompute(const int* n_spin, int fl, int grid, siz
                                         const DevModel& m, const double* e12, const double* e13,
                                         const unsigned short* eseg, long long n_ev, const double* g12,
                                         const double* g13, const double* gw, const unsigned short* gseg,
-                                        long long n_norm, double* partials);
+                                        long long n_norm, double* partials, double2* f_ev, double2* f_nm);
 
 // tu_hybrid.cu: k_nll_hybrid (hybrid.cuh); f1, f2 = floating resonances of spin 1, 2, rc = cached (fixed) resonances
 bool mipwa_hybrid_supported(int f1, int f2, int rc);

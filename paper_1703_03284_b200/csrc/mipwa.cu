@@ -100,6 +100,9 @@ struct mipwa_ctx {
     int grad_blocks_per_sm = 0;
     double* d_gpartials = nullptr;
     size_t gpartials_len = 0;
+    double2* d_f_ev = nullptr; double2* d_f_nm = nullptr;   // per-point gradient factors for k_grad_shape
+    int64_t f_ev_len = 0, f_nm_len = 0;
+    bool want_f = false;
     double res_fold[MIPWA_MAX_RESONANCES];   // sqrt(n_R n_D) of device slot d for the current call
 
     bool timing = false;
@@ -425,6 +428,8 @@ void mipwa_destroy(mipwa_ctx* c)
     if (c->owned_cache) cudaFree(c->owned_cache);
     if (c->d_gram) cudaFree(c->d_gram);
     if (c->d_gpartials) cudaFree(c->d_gpartials);
+    if (c->d_f_ev) cudaFree(c->d_f_ev);
+    if (c->d_f_nm) cudaFree(c->d_f_nm);
     if (c->d_hyb_ev) cudaFree(c->d_hyb_ev);
     if (c->d_hyb_nm) cudaFree(c->d_hyb_nm);
     free_slot(c->ev_sorted); free_slot(c->nm_sorted);
@@ -1174,7 +1179,8 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     const cudaError_t le = mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model,
                                                        c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, c->ev_sorted.n,
                                                        c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w, c->nm_sorted.seg,
-                                                       c->nm_sorted.n, c->d_gpartials);
+                                                       c->nm_sorted.n, c->d_gpartials, c->want_f ? c->d_f_ev : nullptr,
+                                                       c->want_f ? c->d_f_nm : nullptr);
     ++c->launches;
     CU(c, le);
     k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
@@ -1211,7 +1217,26 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
 // k_grad_shape for (mass, width) of every floating resonance (layout of grad = layout of params)
 int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
 {
+    if (!c) return MIPWA_ERR_ARG;
+    if (c->F > 0 && c->ev.n >= 0 && c->nm.n >= 1) {        // room for the per-point factors k_grad_recompute leaves
+        int rc0 = use_device(c);
+        if (rc0) return rc0;
+        if (c->f_ev_len < c->ev.n) {
+            if (c->d_f_ev) cudaFree(c->d_f_ev);
+            c->d_f_ev = nullptr; c->f_ev_len = 0;
+            CU(c, cudaMalloc(&c->d_f_ev, (size_t)std::max<int64_t>(c->ev.n, 1) * sizeof(double2)));
+            c->f_ev_len = c->ev.n;
+        }
+        if (c->f_nm_len < c->nm.n) {
+            if (c->d_f_nm) cudaFree(c->d_f_nm);
+            c->d_f_nm = nullptr; c->f_nm_len = 0;
+            CU(c, cudaMalloc(&c->d_f_nm, (size_t)c->nm.n * sizeof(double2)));
+            c->f_nm_len = c->nm.n;
+        }
+        c->want_f = true;
+    }
     int rc = mipwa_nll_grad(c, params, n_params, nll, grad);
+    c->want_f = false;
     if (rc || c->F == 0) return rc;
     const int N = c->N, R = c->R, F = c->F;
     constexpr int SHAPE_OFF = 3900;                        // in h_result, clear of the main gradient's NV <= 2098 values
@@ -1242,7 +1267,7 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         for (int q = 0; q < MIPWA_SHAPE_MAXF; ++q) sel.slot[q] = slots[f0 + std::min(q, nf - 1)];
         if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
 #define MIPWA_SHAPE_LAUNCH(NF)                                                                                     \
-    k_grad_shape<NF><<<grid, 256, 0, c->stream>>>(c->model, sel, E.s12, E.s13, E.seg, E.n, G.s12, G.s13, G.w, G.seg, \
+    k_grad_shape<NF><<<grid, 256, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, G.s12, G.s13, c->d_f_nm, \
                                                   G.n, c->d_gpartials)
         switch (nf) {
             case 1: MIPWA_SHAPE_LAUNCH(1); break;

@@ -16,10 +16,10 @@ cudaError_t mipwa_launch_grad_recompute(const int* n_spin, int fl, int grid, siz
                                         const DevModel& m, const double* e12, const double* e13,
                                         const unsigned short* eseg, long long n_ev, const double* g12,
                                         const double* g13, const double* gw, const unsigned short* gseg,
-                                        long long n_norm, double* partials)
+                                        long long n_norm, double* partials, double2* f_ev, double2* f_nm)
 {
     MIPWA_DISPATCH_SIGFL(n_spin[0], n_spin[1], n_spin[2], fl,
                          (k_grad_recompute<R1, R2, FL><<<grid, MIPWA_GRAD_BLOCK, smem, st>>>(
-                             m, e12, e13, eseg, n_ev, g12, g13, gw, gseg, n_norm, partials)));
+                             m, e12, e13, eseg, n_ev, g12, g13, gw, gseg, n_norm, partials, f_ev, f_nm)));
     return cudaGetLastError();
 }
