@@ -225,13 +225,14 @@ k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cach
 template <int RT>      // RT >= 0: number of resonances known at compile time; -1: run-time
 __global__ void __launch_bounds__(MIPWA_TILE, 4)
 k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDev cc,
-              const double2* __restrict__ cache, long long n_ev, const double2* __restrict__ G,
+              const double2* __restrict__ cache, const unsigned short* __restrict__ seg, long long n_ev,
+              const double2* __restrict__ G,
               double* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result)
 {
-    __shared__ SplineSmem sm;
+    __shared__ SplineCoefSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
-    load_spline_smem(sm, m);
+    load_spline_coef_smem(sm, m);
     const int R = RT >= 0 ? RT : m.R, C = 1 + R, N = cc.N;
     const long long n_tiles = (n_ev + MIPWA_TILE - 1) / MIPWA_TILE;
     LogProd lp;
@@ -241,19 +242,22 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
         for (long long tile = blockIdx.x; tile < n_tiles; tile += 2LL * gridDim.x) {
             const long long tiles[2] = { tile, tile + gridDim.x };
             double2 s[2], b[2][RC];
+            unsigned int sg[2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const long long tt = tiles[u] < n_tiles ? tiles[u] : tile;
                 const double2* p = cache + (size_t)tt * C * MIPWA_TILE + threadIdx.x;
                 s[u] = ld_stream(p);
+                const long long ii = tt * MIPWA_TILE + threadIdx.x;
+                sg[u] = ii < n_ev ? seg[ii] : 0u;          // padding slots hold (0, 0): any segment will do
 #pragma unroll
                 for (int r = 0; r < RT; ++r) b[u][r] = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE);
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 double r1, i1, r2, i2;
-                spline_eval(sm, m, s[u].x, r1, i1);
-                spline_eval(sm, m, s[u].y, r2, i2);
+                spline_eval_at(sm, s[u].x, (int)(sg[u] & 0xffu), r1, i1);
+                spline_eval_at(sm, s[u].y, (int)(sg[u] >> 8), r2, i2);
                 double re = r1 + r2, im = i1 + i2;
 #pragma unroll
                 for (int r = 0; r < RT; ++r) {
@@ -269,9 +273,11 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
         for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             const double2* p = cache + (size_t)tile * C * MIPWA_TILE + threadIdx.x;
             const double2 s = ld_stream(p);
+            const long long ii = tile * MIPWA_TILE + threadIdx.x;
+            const unsigned int sg = ii < n_ev ? seg[ii] : 0u;
             double r1, i1, r2, i2;
-            spline_eval(sm, m, s.x, r1, i1);
-            spline_eval(sm, m, s.y, r2, i2);
+            spline_eval_at(sm, s.x, (int)(sg & 0xffu), r1, i1);
+            spline_eval_at(sm, s.y, (int)(sg >> 8), r2, i2);
             double re = r1 + r2, im = i1 + i2;
             for (int r = 0; r < R; ++r) {
                 const double2 b = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE), c = cc.c[N + r];

@@ -99,7 +99,8 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 
     // PTS points per thread and iteration: independent dependency chains for the FP64 pipe.  Out-of-range slots
     // evaluate a harmless in-range point and contribute ln 1 = 0 (events) or weight 0 (normalisation).
-    constexpr int PTS = MIPWA_REC_PTS;
+    // a pure S-wave model (R = 0) is bound by memory latency, not arithmetic: four points in flight per thread
+    constexpr int PTS = (R1 == 0 && R2 == 0) ? 4 : MIPWA_REC_PTS;
     LogProd lp;
     {
         double a[PTS], b[PTS];

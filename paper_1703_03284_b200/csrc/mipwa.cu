@@ -721,7 +721,7 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
         }
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->compact_blocks_per_sm));
 #define MIPWA_COMPACT_LAUNCH(T)                                                                                   \
-    k_nll_compact<T><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, cc, cache, c->ev.n, c->d_gram,                \
+    k_nll_compact<T><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, cc, cache, evs(c).seg, c->ev.n, c->d_gram,    \
                                                           (double*)c->d_partials, c->d_ticket, c->d_result)
         switch (c->R) {
             case 0: MIPWA_COMPACT_LAUNCH(0); break;
