@@ -142,6 +142,20 @@ int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, doubl
  * identical to mipwa_nll_grad when none does.  Errors as mipwa_nll_grad. */
 int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
+/* Toy Monte-Carlo generation on the device ("samples of 100K signal events are generated from a Dalitz
+ * plot PDF"): n events with density |A(params)|^2 / integral inside the Dalitz boundary, by
+ * accept-reject against a piecewise-constant envelope (reading P22): n_coarse x n_coarse cells over the
+ * bounding square [(m1+m2)^2, (M-m3)^2]^2, each 1.2 x the maximum of |A|^2 over the centres of an n_side x n_side
+ * fine grid that fall into it.  Candidate i uses uniforms 4i .. 4i+3 of the counter-based splitmix64 stream `key`
+ * (the scheme of paper_1703_03284_b200/inputs.py); the events are the first n accepted candidates in counter order,
+ * so the sample is a function of (model, params, key, n, n_side, n_coarse) only.
+ *   s12, s13: n doubles each, HOST or DEVICE according to mem (caller-allocated).
+ *   n_candidates (may be NULL): candidates drawn.  Independent of the event / normalisation slots.
+ * Errors: MIPWA_ERR_ARG (sizes, pointers), MIPWA_ERR_DOMAIN (|A|^2 zero or non-finite on the whole envelope grid,
+ * or acceptance below 1e-6), MIPWA_ERR_CUDA / MIPWA_ERR_NOMEM. */
+int mipwa_generate(mipwa_ctx* ctx, const double* params, int64_t n_params, uint64_t key, int64_t n, int32_t n_side,
+                   int32_t n_coarse, double* s12, double* s13, int32_t mem, int64_t* n_candidates);
+
 /* TEST HOOK: per-point |A|^2 from the same device function the NLL kernels use.
  *   which = 0: the events slot, 1: the normalisation slot; out: HOST, n doubles, n = that slot's size. */
 int mipwa_eval_abs2(mipwa_ctx* ctx, const double* params, int64_t n_params, int32_t which, double* out, int64_t n);

@@ -23,7 +23,7 @@ _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STAT
 # every symbol include/mipwa.h declares
 SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
            "mipwa_prepare", "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
-           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
+           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version"]
 
@@ -72,6 +72,8 @@ def load_library():
     L.mipwa_nll_parts.restype = i32; L.mipwa_nll_parts.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_nll_grad.restype = i32; L.mipwa_nll_grad.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_nll_grad_full.restype = i32; L.mipwa_nll_grad_full.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_generate.restype = i32
+    L.mipwa_generate.argtypes = [vp, _dp, i64, C.c_uint64, i64, i32, i32, vp, vp, i32, C.POINTER(i64)]
     L.mipwa_eval_abs2.restype = i32; L.mipwa_eval_abs2.argtypes = [vp, _dp, i64, i32, _dp, i64]
     L.mipwa_eval_basis.restype = i32; L.mipwa_eval_basis.argtypes = [vp, _dp, i64, i32, i64, i64, _dp]
     L.mipwa_enable_timing.restype = i32; L.mipwa_enable_timing.argtypes = [vp, i32]
@@ -228,6 +230,23 @@ class Mipwa:
         grad = np.empty(p.size)
         self._check(self.L.mipwa_nll_grad_full(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
         return out.value, grad
+
+    def generate(self, params, key, n, n_side=1024, n_coarse=64, device=False):
+        """n toy events with density |A(params)|^2 (accept-reject on the GPU, counter-based stream `key`).
+        Returns (s12, s13, candidates drawn); numpy arrays, or CUDA torch tensors if device=True."""
+        p, pp, npar = self._params(params)
+        tried = C.c_int64(0)
+        if device:
+            import torch
+            a = torch.empty(int(n), dtype=torch.float64, device=f"cuda:{self.device}")
+            b = torch.empty_like(a)
+            pa, pb, mem = C.c_void_p(a.data_ptr()), C.c_void_p(b.data_ptr()), MEM_DEVICE
+        else:
+            a, b = np.empty(int(n)), np.empty(int(n))
+            pa, pb, mem = C.c_void_p(a.ctypes.data), C.c_void_p(b.ctypes.data), MEM_HOST
+        self._check(self.L.mipwa_generate(self._h, pp, npar, C.c_uint64(int(key)), int(n), int(n_side), int(n_coarse),
+                                          pa, pb, mem, C.byref(tried)))
+        return a, b, tried.value
 
     def eval_abs2(self, params, which=0):
         p, pp, n = self._params(params)

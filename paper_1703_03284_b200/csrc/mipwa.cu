@@ -14,8 +14,10 @@
 #include "cached.cuh"
 #include "grad.cuh"
 #include "hybrid.cuh"
+#include "gen.cuh"
 
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_select.cuh>
 
 static_assert(MIPWA_DEV_MAX_KNOTS == MIPWA_MAX_KNOTS, "capacity mismatch");
 static_assert(MIPWA_DEV_MAX_RES == MIPWA_MAX_RESONANCES, "capacity mismatch");
@@ -1296,6 +1298,109 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         }
     }
     c->last_ms = ms_total;
+    return MIPWA_OK;
+}
+
+// ---- toy generation on the device (gen.cuh) -------------------------------------------------------------------------
+namespace {
+struct GenScratch {                 // device scratch of one mipwa_generate call; freed on every exit path
+    unsigned long long* own = nullptr;
+    double *cum = nullptr, *env = nullptr, *c12 = nullptr, *c13 = nullptr, *o12 = nullptr, *o13 = nullptr;
+    unsigned char* flag = nullptr;
+    int* nsel = nullptr;
+    void* tmp = nullptr;
+    ~GenScratch()
+    {
+        for (void* p : { (void*)own, (void*)cum, (void*)env, (void*)c12, (void*)c13, (void*)o12, (void*)o13,
+                         (void*)flag, (void*)nsel, tmp })
+            if (p) cudaFree(p);
+    }
+};
+}  // namespace
+
+int mipwa_generate(mipwa_ctx* c, const double* params, int64_t n_params, uint64_t key, int64_t n, int32_t n_side,
+                   int32_t n_coarse, double* s12, double* s13, int32_t mem, int64_t* n_candidates)
+{
+    if (!c || !params) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (n < 0 || (n > 0 && (!s12 || !s13)) || n_side < 1 || n_side > 16384 || n_coarse < 1 || n_coarse > 1024 ||
+        (mem != MIPWA_MEM_HOST && mem != MIPWA_MEM_DEVICE))
+        return fail(c, MIPWA_ERR_ARG, "mipwa_generate: bad count, grid size, pointer or mem flag");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    if (n_candidates) *n_candidates = 0;
+    if (n == 0) return MIPWA_OK;
+    const mipwa_kinematics& kk = c->kin;
+    const GenKin gk = { kk.m_parent * kk.m_parent, kk.m1 * kk.m1, kk.m2 * kk.m2, kk.m3 * kk.m3,
+                        (kk.m1 + kk.m2) * (kk.m1 + kk.m2), (kk.m_parent - kk.m3) * (kk.m_parent - kk.m3) };
+    const int nc = n_coarse, ncell = nc * nc;
+    const double h = (gk.hi - gk.lo) / n_side, H = (gk.hi - gk.lo) / nc;
+    const int64_t batch = 1 << 21;
+    GenScratch g;
+    size_t tmp_bytes = 0;
+    CU(c, cudaMalloc(&g.own, ncell * sizeof(unsigned long long)));
+    CU(c, cudaMemsetAsync(g.own, 0, ncell * sizeof(unsigned long long), c->stream));
+    CU(c, cudaMalloc(&g.cum, ncell * sizeof(double)));
+    CU(c, cudaMalloc(&g.env, ncell * sizeof(double)));
+    CU(c, cudaMalloc(&g.c12, batch * sizeof(double)));
+    CU(c, cudaMalloc(&g.c13, batch * sizeof(double)));
+    CU(c, cudaMalloc(&g.flag, batch));
+    CU(c, cudaMalloc(&g.nsel, sizeof(int)));
+    CU(c, cudaMalloc(&g.o12, (size_t)(n + batch) * sizeof(double)));
+    CU(c, cudaMalloc(&g.o13, (size_t)(n + batch) * sizeof(double)));
+    CU(c, cub::DeviceSelect::Flagged(nullptr, tmp_bytes, g.c12, g.flag, g.o12, g.nsel, (int)batch, c->stream));
+    CU(c, cudaMalloc(&g.tmp, tmp_bytes ? tmp_bytes : 16));
+
+    // envelope: fine-grid maxima per coarse cell on the device, neighbour fill and CDF on the host (O(n_coarse^2))
+    const int64_t fine = (int64_t)n_side * n_side;
+    k_gen_envelope<<<grid_for(c, fine, 8), 256, 0, c->stream>>>(c->model, gk, n_side, h, H, nc, g.own);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    std::vector<unsigned long long> own_bits(ncell);
+    CU(c, cudaMemcpyAsync(own_bits.data(), g.own, ncell * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    std::vector<double> own(ncell), env(ncell), cum(ncell);
+    for (int t = 0; t < ncell; ++t) std::memcpy(&own[t], &own_bits[t], sizeof(double));
+    for (int cx = 0; cx < nc; ++cx)
+        for (int cy = 0; cy < nc; ++cy) {
+            double v = own[cx * nc + cy];
+            if (!(v > 0.0))
+                for (int dx = -1; dx <= 1; ++dx)
+                    for (int dy = -1; dy <= 1; ++dy) {
+                        const int x = cx + dx, y = cy + dy;
+                        if (x >= 0 && x < nc && y >= 0 && y < nc) v = std::max(v, own[x * nc + y]);
+                    }
+            env[cx * nc + cy] = 1.2 * v;
+        }
+    double run = 0.0;
+    for (int t = 0; t < ncell; ++t) { run += env[t]; cum[t] = run; }
+    if (!(run > 0.0) || !std::isfinite(run))
+        return fail(c, MIPWA_ERR_DOMAIN, "mipwa_generate: |A|^2 vanishes or is not finite on the envelope grid");
+    for (int t = 0; t < ncell; ++t) cum[t] /= run;
+    CU(c, cudaMemcpyAsync(g.cum, cum.data(), ncell * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(g.env, env.data(), ncell * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+
+    int64_t have = 0, ctr = 0;
+    while (have < n) {
+        k_gen_candidates<<<grid_for(c, batch, 8), 256, 0, c->stream>>>(c->model, gk, (unsigned long long)key, ctr, batch,
+                                                                     nc, H, g.cum, g.env, g.c12, g.c13, g.flag);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        CU(c, cub::DeviceSelect::Flagged(g.tmp, tmp_bytes, g.c12, g.flag, g.o12 + have, g.nsel, (int)batch, c->stream));
+        CU(c, cub::DeviceSelect::Flagged(g.tmp, tmp_bytes, g.c13, g.flag, g.o13 + have, g.nsel, (int)batch, c->stream));
+        int nsel = 0;
+        CU(c, cudaMemcpyAsync(&nsel, g.nsel, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        have += nsel; ctr += batch;
+        if (ctr > ((int64_t)1 << 40))
+            return fail(c, MIPWA_ERR_DOMAIN, "mipwa_generate: acceptance below 1e-6, giving up");
+    }
+    const cudaMemcpyKind kind = mem == MIPWA_MEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    CU(c, cudaMemcpyAsync(s12, g.o12, (size_t)n * sizeof(double), kind, c->stream));
+    CU(c, cudaMemcpyAsync(s13, g.o13, (size_t)n * sizeof(double), kind, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (n_candidates) *n_candidates = ctr;
     return MIPWA_OK;
 }
 
