@@ -129,13 +129,10 @@ def run_reference(args, cfg, workload):
 
 
 def gpu_inputs(cfg, m, B, torch, rank):
-    """Events by accept-reject with the CUDA library's own per-point hook as the density,
-    normalisation points uniform in phase space; both end up resident in HBM as torch tensors."""
-    def abs2_fn(a, b):
-        m.set_events(np.ascontiguousarray(a), np.ascontiguousarray(b))
-        return m.eval_abs2(cfg.truth, 0)
-    env = I.envelope_of(abs2_fn, cfg.kin)
-    e12, e13 = cfg.events(abs2_fn, env, stream=rank, chunk=1 << 22)
+    """Events by accept-reject on the device (mipwa_generate: the recipe of DESIGN.md section 4 / reading P22, the
+    same stream key inputs.Config.events uses), normalisation points uniform in phase space; both end up resident
+    in HBM as torch tensors."""
+    e12, e13, _ = m.generate(cfg.truth, cfg.key(I.S_EVENTS + 16 * rank), cfg.n_ev, n_side=1024, n_coarse=64)
     g12, g13, w = cfg.norm_points(stream=rank)
     host = [np.ascontiguousarray(a) for a in (e12, e13, g12, g13, w)]
     dev = [torch.from_numpy(a).cuda() for a in host]
@@ -472,13 +469,11 @@ def run_probe(args):
         c = I.Config(5)
         m = B.Mipwa(c.kin, c.knots, c.resonances)
 
-        def abs2_fn(a, b):
-            m.set_events(np.ascontiguousarray(a), np.ascontiguousarray(b))
-            return m.eval_abs2(c.truth, 0)
         t0 = time.perf_counter()
-        e12, e13 = c.events(abs2_fn, I.envelope_of(abs2_fn, c.kin, n_side=2048, n_coarse=128))
+        e12, e13, _ = m.generate(c.truth, c.key(I.S_EVENTS), c.n_ev, n_side=2048, n_coarse=128, device=True)
+        torch.cuda.synchronize()
         gen_s = time.perf_counter() - t0
-        d_ev = [torch.from_numpy(a).cuda() for a in (e12, e13)]
+        d_ev = [e12, e13]
         lo, hi = I.s_limits(c.kin)
         N = c.N
         free = np.ones(c.n_params, dtype=bool)
@@ -509,7 +504,7 @@ def run_probe(args):
             dphi = fit[N:2 * N] - c.truth[N:2 * N]
             fits[spacing] = fit
             print(json.dumps({"probe": "grid-bias", "spacing_gev2": spacing, "grid_cells_inside": int(g12.size),
-                              "n_ev": int(e12.size), "n_free": int(free.sum()), "fit_wall_s": fit_s,
+                              "n_ev": int(e12.numel()), "n_free": int(free.sum()), "fit_wall_s": fit_s,
                               "nll_grad_calls": calls[0], "ms_per_call_incl_minimiser": fit_s / max(calls[0], 1) * 1e3,
                               "converged": bool(res.success), "nll_fit_minus_truth": float(res.fun - nll_truth),
                               "median_abs_da": float(np.median(np.abs(da))), "rms_da": float(np.sqrt(np.mean(da ** 2))),
