@@ -64,3 +64,30 @@ def test_generated_sample_follows_the_density():
     ndf = int(sel.sum()) - 1
     assert chi2 < ndf + 6 * np.sqrt(2 * ndf), (chi2, ndf)
     assert 0.02 < n / tried < 1.0                          # acceptance of the stratified envelope
+
+
+def test_generate_edge_cases_and_errors():
+    from paper_1703_03284_b200 import binding as B
+    c = I.Config(0)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    a, b, tried = m.generate(c.truth, 1, 0)                           # n = 0: nothing drawn
+    assert a.size == 0 and b.size == 0 and tried == 0
+    a1, b1, _ = m.generate(c.truth, 1, 1)                             # n = 1, and the stream is reproducible
+    a2, b2, _ = m.generate(c.truth, 1, 3)
+    assert a1[0] == a2[0] and b1[0] == b2[0]
+    x, y, _ = m.generate(c.truth, 2, 3)
+    assert not np.array_equal(x, a2)                                   # another key, another sample
+    with pytest.raises(B.MipwaError) as e:
+        m.generate(c.truth, 1, 10, n_side=0)
+    assert e.value.code == B.ERR_ARG
+    with pytest.raises(B.MipwaError) as e:
+        m.generate(c.truth[:-1], 1, 10)
+    assert e.value.code == B.ERR_ARG
+    zero = c.truth.copy(); zero[:c.N] = 0.0; zero[2 * c.N] = 0.0      # |A|^2 = 0 everywhere: nothing to sample from
+    with pytest.raises(B.MipwaError) as e:
+        m.generate(zero, 1, 10)
+    assert e.value.code == B.ERR_DOMAIN
+    with pytest.raises(B.MipwaError) as e:                            # gradient before any point set
+        m.nll_grad_full(c.truth)
+    assert e.value.code == B.ERR_STATE
+    m.close()
