@@ -617,4 +617,96 @@ void orc_nll_grad_shape(const orc_kin* kin, int n, const double* knots, int R, c
         grad_shape[t] = (double)(-2.0L * ev[t].value() + 2.0L * (long double)n_ev / Iv * nm[t].value());
 }
 
+// ---- O11 (not in the paper): Hessian of the NLL in the 2N + 2R linear-coefficient parameters, for
+// fixed resonance shapes.  With c = [y_0..y_{N-1}, c_0..c_{R-1}], A_i = sum_k c_k B_ik, I = c^H G c,
+// G_kl = sum_j w_j conj(B_jk) B_jl, and Wirtinger derivatives d/dc_k = (d/dRe c_k - i d/dIm c_k)/2:
+//     g_k       = dNLL/dc_k          = -sum_i B_ik/A_i + n_ev (c^H G)_k / I
+//     Hcc_kl    = d2NLL/dc_k dc_l    =  sum_i B_ik B_il / A_i^2 - n_ev (c^H G)_k (c^H G)_l / I^2
+//     Hcb_kl    = d2NLL/dc_k dconj(c_l) = n_ev G_lk / I - n_ev (c^H G)_k (G c)_l / I^2      (ln|A|^2 has no mixed part)
+// and for real parameters t_a, t_b with c = c(t):
+//     d2NLL/dt_a dt_b = 2 Re sum_kl [ Hcc_kl dc_k/dt_a dc_l/dt_b + Hcb_kl dc_k/dt_a conj(dc_l/dt_b) ]
+//                     + 2 Re sum_k g_k d2c_k/dt_a dt_b.
+// Polar form c = rho e^{i phi}: dc/drho = e^{i phi}, dc/dphi = i c, d2c/drho dphi = i e^{i phi}, d2c/dphi2 = -c.
+// hess: P x P row-major, P = 2N + 2R, same order as params / grad.  shape_floats entries of params are ignored.
+void orc_nll_hessian(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res, const double* params,
+                     int64_t n_ev, const double* e12, const double* e13,
+                     int64_t n_norm, const double* g12, const double* g13, const double* w, double* hess)
+{
+    const Model m = make_model(kin, n, knots, R, res);
+    const Unpacked u = unpack(m, params);
+    const std::vector<double> Mx = cardinal_second_derivs(m);
+    const int K = n + R, P = 2 * n + 2 * R;
+    std::vector<cplx> c(K), B(K);
+    for (int k = 0; k < n; ++k) c[k] = u.y[k];
+    for (int r = 0; r < R; ++r) c[n + r] = u.c[r];
+    std::vector<Acc> Mr((size_t)K * K), Mi((size_t)K * K), Gr((size_t)K * K), Gi((size_t)K * K), vr(K), vi(K);
+    for (int64_t i = 0; i < n_ev; ++i) {
+        basis_row(m, u.res, Mx, e12[i], e13[i], B.data());
+        cplx A = 0.0;
+        for (int k = 0; k < K; ++k) A += c[k] * B[k];
+        for (int k = 0; k < K; ++k) {
+            const cplx bk = B[k] / A;
+            vr[k].add(bk.real()); vi[k].add(bk.imag());
+            for (int l = 0; l < K; ++l) {
+                const cplx t = bk * (B[l] / A);
+                Mr[(size_t)k * K + l].add(t.real()); Mi[(size_t)k * K + l].add(t.imag());
+            }
+        }
+    }
+    for (int64_t j = 0; j < n_norm; ++j) {
+        basis_row(m, u.res, Mx, g12[j], g13[j], B.data());
+        const double wj = w ? w[j] : 1.0 / (double)n_norm;
+        for (int k = 0; k < K; ++k)
+            for (int l = 0; l < K; ++l) {
+                const cplx t = wj * std::conj(B[k]) * B[l];
+                Gr[(size_t)k * K + l].add(t.real()); Gi[(size_t)k * K + l].add(t.imag());
+            }
+    }
+    auto G = [&](int k, int l) { return cplx((double)Gr[(size_t)k * K + l].value(), (double)Gi[(size_t)k * K + l].value()); };
+    std::vector<cplx> cG(K), Gc(K);                       // (c^H G)_k and (G c)_k
+    cplx I = 0.0;
+    for (int k = 0; k < K; ++k) {
+        cplx a = 0.0, b = 0.0;
+        for (int l = 0; l < K; ++l) { a += std::conj(c[l]) * G(l, k); b += G(k, l) * c[l]; }
+        cG[k] = a; Gc[k] = b;
+    }
+    for (int k = 0; k < K; ++k) I += std::conj(c[k]) * Gc[k];
+    const double Iv = I.real(), nev = (double)n_ev;
+    std::vector<cplx> g(K), Hcc((size_t)K * K), Hcb((size_t)K * K);
+    for (int k = 0; k < K; ++k) {
+        g[k] = -cplx((double)vr[k].value(), (double)vi[k].value()) + nev * cG[k] / Iv;
+        for (int l = 0; l < K; ++l) {
+            Hcc[(size_t)k * K + l] = cplx((double)Mr[(size_t)k * K + l].value(), (double)Mi[(size_t)k * K + l].value())
+                                     - nev * cG[k] * cG[l] / (Iv * Iv);
+            Hcb[(size_t)k * K + l] = nev * G(l, k) / Iv - nev * cG[k] * Gc[l] / (Iv * Iv);
+        }
+    }
+    // polar Jacobians: column index of (rho_k, phi_k) in the parameter vector
+    std::vector<int> ir(K), ip(K);
+    std::vector<cplx> dr(K), dp(K);
+    for (int k = 0; k < K; ++k) {
+        ir[k] = k < n ? k : 2 * n + 2 * (k - n);
+        ip[k] = k < n ? n + k : 2 * n + 2 * (k - n) + 1;
+        const double phi = params[ip[k]];
+        dr[k] = cplx(std::cos(phi), std::sin(phi));
+        dp[k] = cplx(0.0, 1.0) * c[k];
+    }
+    for (int t = 0; t < P * P; ++t) hess[t] = 0.0;
+    for (int k = 0; k < K; ++k)
+        for (int l = 0; l < K; ++l) {
+            const cplx hcc = Hcc[(size_t)k * K + l], hcb = Hcb[(size_t)k * K + l];
+            const cplx dk[2] = { dr[k], dp[k] }, dl[2] = { dr[l], dp[l] };
+            const int ik[2] = { ir[k], ip[k] }, il[2] = { ir[l], ip[l] };
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < 2; ++b)
+                    hess[(size_t)ik[a] * P + il[b]] += 2.0 * (hcc * dk[a] * dl[b] + hcb * dk[a] * std::conj(dl[b])).real();
+        }
+    for (int k = 0; k < K; ++k) {
+        const cplx d2rp = cplx(0.0, 1.0) * dr[k], d2pp = -c[k];
+        hess[(size_t)ir[k] * P + ip[k]] += 2.0 * (g[k] * d2rp).real();
+        hess[(size_t)ip[k] * P + ir[k]] += 2.0 * (g[k] * d2rp).real();
+        hess[(size_t)ip[k] * P + ip[k]] += 2.0 * (g[k] * d2pp).real();
+    }
+}
+
 }  // extern "C"

@@ -68,6 +68,8 @@ def lib():
         L.orc_gram.restype = None; L.orc_gram.argtypes = model + [_dp, i64, _dp, _dp, _dp, _dp]
         L.orc_nll_grad.restype = None
         L.orc_nll_grad.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp]
+        L.orc_nll_hessian.restype = None
+        L.orc_nll_hessian.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp]
         L.orc_nll_grad_shape.restype = None
         L.orc_nll_grad_shape.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp]
         L.orc_resonance_term_dshape.restype = None; L.orc_resonance_term_dshape.argtypes = [kp, rp, d, d, _dp]
@@ -148,6 +150,15 @@ class Oracle:
         self.L.orc_nll_grad(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w),
                             C.byref(nll), _p(grad))
         return nll.value, grad
+
+    def nll_hessian(self, params, e12, e13, g12, g13, w=None):
+        """P x P Hessian of the NLL in the 2N + 2R linear-coefficient parameters (fixed shapes)  -- O11"""
+        p, e12, e13, g12, g13 = self._params(params), _a(e12), _a(e13), _a(g12), _a(g13)
+        w = None if w is None else _a(w)
+        P = 2 * self.n + 2 * self.R
+        H = np.zeros((P, P))
+        self.L.orc_nll_hessian(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w), _p(H))
+        return H
 
     def nll_grad_shape(self, params, e12, e13, g12, g13, w=None):
         """(NLL, [d/dmass, d/dwidth of every shape_floats resonance in list order])  -- O10"""

@@ -89,3 +89,31 @@ def test_nll_shape_gradient_two_floating_resonances_and_unweighted_norm():
             return o.nll(q, s12[:1000], s13[:1000], s12[1000:], s13[1000:], None)
         fd = _richardson(f, p[idx], 1e-4)
         assert gs[t] == pytest.approx(fd, rel=5e-6, abs=1e-6 * abs(nll))
+
+
+def test_hessian_matches_differences_of_the_pinned_gradient_and_the_invariance_identities():
+    """O11: the oracle's analytic Hessian against Richardson central differences of its (separately pinned) analytic
+    gradient, its symmetry, and the two exact identities that follow from differentiating the Euler relations
+    sum_b dNLL/dphi_b = 0 (global phase) and sum_b rho_b dNLL/drho_b = 0 (global scale):
+        sum_b H[a, phi_b] = 0    and    sum_b rho_b H[a, rho_b] + [a is a magnitude] g_a = 0   for every a."""
+    c = I.Config(1, n_ev=1500, n_norm=3000)
+    o = orc.Oracle(c.kin, c.knots, c.resonances)
+    e12, e13 = I.phase_space_points(1500, c.key(7), c.kin)
+    g12, g13, w = c.norm_points()
+    p = c.perturbed(3)
+    H = o.nll_hessian(p, e12, e13, g12, g13, w)
+    P, N, R = p.size, c.N, c.R
+    assert H.shape == (P, P)
+    scale = np.max(np.abs(H))
+    assert np.max(np.abs(H - H.T)) <= 1e-12 * scale
+    _, g = o.nll_grad(p, e12, e13, g12, g13, w)
+    is_phi = np.zeros(P, dtype=bool); is_phi[N:2 * N] = True; is_phi[2 * N + 1::2] = True
+    rho = np.where(is_phi, 0.0, p)
+    assert np.max(np.abs(H[:, is_phi].sum(axis=1))) <= 1e-10 * scale
+    assert np.max(np.abs(H @ rho + np.where(is_phi, 0.0, g))) <= 1e-10 * scale * np.max(np.abs(p))
+    for a in (0, 3, N - 1, N + 2, 2 * N - 1, 2 * N, 2 * N + 1, 2 * N + 3):
+        def grad_at(v):
+            q = p.copy(); q[a] = v
+            return o.nll_grad(q, e12, e13, g12, g13, w)[1]
+        col = _richardson(grad_at, p[a], 1e-5)             # 1e-4 still leaves 5e-7 of truncation error (narrow rho)
+        assert np.max(np.abs(col - H[a])) <= 1e-9 * scale
