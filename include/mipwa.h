@@ -142,6 +142,18 @@ int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, doubl
  * identical to mipwa_nll_grad when none does.  Errors as mipwa_nll_grad. */
 int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
+/* NLL, gradient and HESSIAN with respect to the 2N + 2R linear-coefficient parameters, for fixed resonance shapes
+ * (the parameter errors and correlations PAPER.md:29 alludes to are the inverse of this matrix at the
+ * minimum).  With c = [y_k, c_r], A_i = sum_k c_k B_ik, I = c^H G c and Wirtinger derivatives:
+ *     d2NLL/dc_k dc_l       = sum_i B_ik B_il / A_i^2 - n_ev (c^H G)_k (c^H G)_l / I^2
+ *     d2NLL/dc_k dconj(c_l) = n_ev G_lk / I - n_ev (c^H G)_k (G c)_l / I^2
+ * followed by the polar chain rule.  The K x K event sum is one more sweep of the Gram kernel over the events (complex
+ * weights 1/A_i^2, no conjugate: 4 K^2 flops per event); G comes from the Gram matrix of the cached paths.
+ *   grad: HOST, 2N + 2R doubles, may be NULL;  hess: HOST, (2N + 2R)^2 doubles, row-major, symmetric.
+ * Errors: MIPWA_ERR_STATE if a shape floats or before both mipwa_set_*; MIPWA_ERR_ARG if a magnitude is zero (the
+ * polar parametrisation is singular there). */
+int mipwa_nll_hessian(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad, double* hess);
+
 /* Toy Monte-Carlo generation on the device ("samples of 100K signal events are generated from a Dalitz
  * plot PDF"): n events with density |A(params)|^2 / integral inside the Dalitz boundary, by
  * accept-reject against a piecewise-constant envelope (reading P22): n_coarse x n_coarse cells over the

@@ -23,7 +23,7 @@ _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STAT
 # every symbol include/mipwa.h declares
 SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
            "mipwa_prepare", "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
-           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
+           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_nll_hessian", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version"]
 
@@ -72,6 +72,7 @@ def load_library():
     L.mipwa_nll_parts.restype = i32; L.mipwa_nll_parts.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_nll_grad.restype = i32; L.mipwa_nll_grad.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_nll_grad_full.restype = i32; L.mipwa_nll_grad_full.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_nll_hessian.restype = i32; L.mipwa_nll_hessian.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_generate.restype = i32
     L.mipwa_generate.argtypes = [vp, _dp, i64, C.c_uint64, i64, i32, i32, vp, vp, i32, C.POINTER(i64)]
     L.mipwa_eval_abs2.restype = i32; L.mipwa_eval_abs2.argtypes = [vp, _dp, i64, i32, _dp, i64]
@@ -230,6 +231,14 @@ class Mipwa:
         grad = np.empty(p.size)
         self._check(self.L.mipwa_nll_grad_full(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
         return out.value, grad
+
+    def nll_hessian(self, params):
+        """(NLL, gradient, Hessian) in the 2N + 2R linear-coefficient parameters; fixed shapes only."""
+        p, pp, n = self._params(params)
+        P = 2 * self.N + 2 * self.R
+        out, grad, H = C.c_double(), np.empty(P), np.empty((P, P))
+        self._check(self.L.mipwa_nll_hessian(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp), H.ctypes.data_as(_dp)))
+        return out.value, grad, H
 
     def generate(self, params, key, n, n_side=1024, n_coarse=64, device=False):
         """n toy events with density |A(params)|^2 (accept-reject on the GPU, counter-based stream `key`).

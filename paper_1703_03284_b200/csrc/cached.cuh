@@ -310,15 +310,17 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
 #define GRAM_P 32
 #define GRAM_LD (GRAM_P + 1)
 
-template <int TPT>
+// HESS = true (mipwa_nll_hessian): the same sweep over the EVENTS with the complex weight 1 / A_i^2, A_i = sum_k c_k B_ik,
+// and WITHOUT the conjugate: M_kl = sum_i B_ik B_il / A_i^2, the event part of d2NLL / dc_k dc_l (complex symmetric).
+template <int TPT, bool HESS>
 __global__ void __launch_bounds__(MIPWA_TILE, 1)
-k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ g12,
-       const double* __restrict__ g13, const double* __restrict__ gw, long long n, double w_default,
-       double2* __restrict__ partial)
+k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const __grid_constant__ CoefDev cc,
+       const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw, long long n,
+       double w_default, double2* __restrict__ partial)
 {
     extern __shared__ double2 gram_smem[];
     __shared__ SplineSmem sm;
-    __shared__ double ws[GRAM_P];
+    __shared__ double ws[GRAM_P], wsi[GRAM_P];
     load_spline_smem(sm, m);
     const int K = m.N + m.R, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, rows = 4 * nt;
     double2* Bs = gram_smem;                                       // [rows][GRAM_LD]
@@ -347,31 +349,46 @@ k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __r
         if (j < n) {
             basis_point(sm, m, aux, g12[j], g13[j], slice, MIPWA_TILE / 32, true,
                         [&](int k, double2 v) { Bs[k * GRAM_LD + p] = v; });
-            if (slice == 0) ws[p] = gw ? gw[j] : w_default;
+            if (slice == 0 && !HESS) ws[p] = gw ? gw[j] : w_default;
         } else if (slice == 0) {
-            ws[p] = 0.0;                                           // stale columns of an absent point get weight 0
+            ws[p] = 0.0; wsi[p] = 0.0;                             // stale columns of an absent point get weight 0
         }
         __syncthreads();
+        if (HESS) {
+            if (slice == 0 && j < n) {                             // A = sum_k c_k B_k of point p, weight 1 / A^2
+                double ar = 0.0, ai = 0.0;
+                for (int k = 0; k < K; ++k) {
+                    const double2 b = Bs[k * GRAM_LD + p], c = cc.c[k];
+                    ar = fma(c.x, b.x, fma(-c.y, b.y, ar));
+                    ai = fma(c.x, b.y, fma(c.y, b.x, ai));
+                }
+                const double qr = ar * ar - ai * ai, qi = 2.0 * ar * ai, d = 1.0 / (qr * qr + qi * qi);
+                ws[p] = qr * d; wsi[p] = -qi * d;
+            }
+            __syncthreads();
+        }
 #pragma unroll
         for (int u = 0; u < TPT; ++u) {
             if (ta[u] < 0) continue;
             const double2* ra = Bs + (4 * ta[u]) * GRAM_LD;
             const double2* rb = Bs + (4 * tb[u]) * GRAM_LD;
             for (int q = 0; q < GRAM_P; ++q) {
-                const double w = ws[q];
+                const double w = ws[q], wi = HESS ? wsi[q] : 0.0;
                 double2 x[4], y[4];
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                     x[i] = ra[i * GRAM_LD + q];
-                    y[i] = rb[i * GRAM_LD + q];
-                    y[i].x *= w; y[i].y *= w;
+                    const double2 t = rb[i * GRAM_LD + q];
+                    if (HESS) y[i] = make_double2(fma(w, t.x, -wi * t.y), fma(w, t.y, wi * t.x));
+                    else y[i] = make_double2(t.x * w, t.y * w);
                 }
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
 #pragma unroll
-                    for (int l = 0; l < 4; ++l) {                  // conj(x_i) * y_l
-                        acc[u][i][l].x = fma(x[i].x, y[l].x, fma(x[i].y, y[l].y, acc[u][i][l].x));
-                        acc[u][i][l].y = fma(x[i].x, y[l].y, fma(-x[i].y, y[l].x, acc[u][i][l].y));
+                    for (int l = 0; l < 4; ++l) {                  // conj(x_i) * y_l   (HESS: x_i * y_l)
+                        const double xi = HESS ? -x[i].y : x[i].y;
+                        acc[u][i][l].x = fma(x[i].x, y[l].x, fma(xi, y[l].y, acc[u][i][l].x));
+                        acc[u][i][l].y = fma(x[i].x, y[l].y, fma(-xi, y[l].x, acc[u][i][l].y));
                     }
             }
         }
@@ -391,7 +408,9 @@ k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const double* __r
     }
 }
 
-static __global__ void k_gram_reduce(const double2* __restrict__ partial, int nblocks, int K, double2* __restrict__ G)
+// hermitian = 1: G (lower triangle = conjugate, real diagonal); 0: the complex symmetric M of mipwa_nll_hessian
+static __global__ void k_gram_reduce(const double2* __restrict__ partial, int nblocks, int K, double2* __restrict__ G,
+                                     int hermitian)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= K * K) return;
@@ -402,7 +421,7 @@ static __global__ void k_gram_reduce(const double2* __restrict__ partial, int nb
         const double2 v = partial[(size_t)b * K * K + idx];
         s.x += v.x; s.y += v.y;
     }
-    if (k == l) s.y = 0.0;
+    if (k == l && hermitian) s.y = 0.0;
     G[k * K + l] = s;
-    G[l * K + k] = make_double2(s.x, -s.y);
+    G[l * K + k] = make_double2(s.x, hermitian ? -s.y : s.y);
 }

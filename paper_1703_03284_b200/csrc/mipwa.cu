@@ -3,6 +3,7 @@
 #include "../../include/mipwa.h"
 
 #include <cmath>
+#include <complex>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -657,20 +658,22 @@ static int ensure_gram(mipwa_ctx* c)
     double2* partial = nullptr;
     CU(c, cudaMalloc(&partial, (size_t)grid * K * K * sizeof(double2)));
     const double wd = 1.0 / (double)c->nm.n;
+    CoefDev cdummy{};                                      // unused by the Gram instantiation
+    cdummy.K = K; cdummy.N = c->N;
     cudaError_t e = cudaSuccess;
 #define MIPWA_GRAM_LAUNCH(T)                                                                                         \
     do {                                                                                                             \
-        e = cudaFuncSetAttribute(k_gram<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                 \
+        e = cudaFuncSetAttribute(k_gram<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
         if (e == cudaSuccess)                                                                                        \
-            k_gram<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), nms(c).s12, nms(c).s13, nms(c).w, \
-                                                              c->nm.n, wd, partial);                                 \
+            k_gram<T, false><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), cdummy, nms(c).s12,      \
+                                                                     nms(c).s13, nms(c).w, c->nm.n, wd, partial);    \
     } while (0)
     if (tpt <= 1) MIPWA_GRAM_LAUNCH(1); else if (tpt == 2) MIPWA_GRAM_LAUNCH(2); else MIPWA_GRAM_LAUNCH(3);
 #undef MIPWA_GRAM_LAUNCH
     ++c->launches;
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e == cudaSuccess) {
-        k_gram_reduce<<<(K * K + 255) / 256, 256, 0, c->stream>>>(partial, grid, K, c->d_gram);
+        k_gram_reduce<<<(K * K + 255) / 256, 256, 0, c->stream>>>(partial, grid, K, c->d_gram, 1);
         ++c->launches;
         e = cudaGetLastError();
     }
@@ -1298,6 +1301,106 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         }
     }
     c->last_ms = ms_total;
+    return MIPWA_OK;
+}
+
+// ---- Hessian in the linear-coefficient parameters, fixed shapes (include/mipwa.h) ---------------------------------------
+int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad, double* hess)
+{
+    if (!c || !params || !nll || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "mipwa_nll_hessian needs fixed resonance shapes");
+    const int N = c->N, R = c->R, K = N + R, P = 2 * N + 2 * R;
+    std::vector<double> gpol(P);
+    int rc = mipwa_nll_grad(c, params, n_params, nll, gpol.data());
+    if (rc) return rc;
+    if (grad) std::memcpy(grad, gpol.data(), P * sizeof(double));
+    rc = ensure_gram(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);                 // y_k of this call for fill_coef
+    if (rc) return rc;
+    CoefDev cc;
+    fill_coef(c, params, &cc);
+    rc = build_unit_model(c, nullptr);                     // the basis kernels evaluate the unit-coefficient model
+    if (rc) return rc;
+
+    // M_kl = sum_i B_ik B_il / A_i^2 over the events (k_gram in HESS mode), reduced in block order
+    const Slot& E = evs(c);
+    const int nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, tpt = (ntile + MIPWA_TILE - 1) / MIPWA_TILE;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((E.n + GRAM_P - 1) / GRAM_P, c->sm_count));
+    const size_t smem = (size_t)4 * nt * GRAM_LD * sizeof(double2);
+    double2 *partial = nullptr, *d_M = nullptr;
+    std::vector<double> hM((size_t)2 * K * K, 0.0);
+    cudaError_t e = cudaMalloc(&partial, (size_t)grid * K * K * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMalloc(&d_M, (size_t)K * K * sizeof(double2));
+    if (e == cudaSuccess && E.n > 0) {
+#define MIPWA_HESS_LAUNCH(T)                                                                                         \
+    do {                                                                                                             \
+        e = cudaFuncSetAttribute(k_gram<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
+        if (e == cudaSuccess)                                                                                        \
+            k_gram<T, true><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), cc, E.s12, E.s13, nullptr, \
+                                                                    E.n, 0.0, partial);                              \
+    } while (0)
+        if (tpt <= 1) MIPWA_HESS_LAUNCH(1); else if (tpt == 2) MIPWA_HESS_LAUNCH(2); else MIPWA_HESS_LAUNCH(3);
+#undef MIPWA_HESS_LAUNCH
+        ++c->launches;
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) {
+            k_gram_reduce<<<(K * K + 255) / 256, 256, 0, c->stream>>>(partial, grid, K, d_M, 0);
+            ++c->launches;
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(hM.data(), d_M, (size_t)K * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    }
+    if (partial) cudaFree(partial);
+    if (d_M) cudaFree(d_M);
+    if (e != cudaSuccess)
+        return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, std::string("hessian: ") + cudaGetErrorString(e));
+
+    // ---- host: O(K^2) assembly.  Wirtinger blocks from M, G, c, then the polar chain rule -------------------------------
+    typedef std::complex<double> cx;
+    auto Gm = [&](int k, int l) { return cx(c->h_gram[2 * ((size_t)k * K + l)], c->h_gram[2 * ((size_t)k * K + l) + 1]); };
+    auto Mm = [&](int k, int l) { return cx(hM[2 * ((size_t)k * K + l)], hM[2 * ((size_t)k * K + l) + 1]); };
+    std::vector<cx> cv(K), cG(K), Gc(K), e1(K), g(K);
+    std::vector<int> ir(K), ip(K);
+    for (int k = 0; k < K; ++k) {
+        cv[k] = cx(cc.c[k].x, cc.c[k].y);
+        ir[k] = k < N ? k : 2 * N + 2 * (k - N);
+        ip[k] = k < N ? N + k : 2 * N + 2 * (k - N) + 1;
+        e1[k] = cx(std::cos(params[ip[k]]), std::sin(params[ip[k]]));
+        if (!(std::fabs(params[ir[k]]) > 0.0))
+            return fail(c, MIPWA_ERR_ARG, "mipwa_nll_hessian: a zero magnitude makes the polar Hessian singular");
+    }
+    cx Iq = 0.0;
+    for (int k = 0; k < K; ++k) {
+        cx a = 0.0, b = 0.0;
+        for (int l = 0; l < K; ++l) { a += std::conj(cv[l]) * Gm(l, k); b += Gm(k, l) * cv[l]; }
+        cG[k] = a; Gc[k] = b;
+    }
+    for (int k = 0; k < K; ++k) Iq += std::conj(cv[k]) * Gc[k];
+    const double I = Iq.real(), nev = (double)c->ev.n;
+    // dNLL/dc_k from the polar gradient: dNLL/drho = 2 Re(g e^{i phi}), dNLL/dphi = 2 Re(g i c) = -2 rho Im(g e^{i phi})
+    for (int k = 0; k < K; ++k) {
+        const double rho = params[ir[k]];
+        g[k] = 0.5 * cx(gpol[ir[k]], -gpol[ip[k]] / rho) * std::conj(e1[k]);
+    }
+    for (int t = 0; t < P * P; ++t) hess[t] = 0.0;
+    for (int k = 0; k < K; ++k)
+        for (int l = 0; l < K; ++l) {
+            const cx hcc = Mm(k, l) - nev * cG[k] * cG[l] / (I * I);
+            const cx hcb = nev * Gm(l, k) / I - nev * cG[k] * Gc[l] / (I * I);
+            const cx dk[2] = { e1[k], cx(0.0, 1.0) * cv[k] }, dl[2] = { e1[l], cx(0.0, 1.0) * cv[l] };
+            const int ik[2] = { ir[k], ip[k] }, il[2] = { ir[l], ip[l] };
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < 2; ++b)
+                    hess[(size_t)ik[a] * P + il[b]] += 2.0 * (hcc * dk[a] * dl[b] + hcb * dk[a] * std::conj(dl[b])).real();
+        }
+    for (int k = 0; k < K; ++k) {
+        const double rp = 2.0 * (g[k] * cx(0.0, 1.0) * e1[k]).real(), pp = 2.0 * (g[k] * (-cv[k])).real();
+        hess[(size_t)ir[k] * P + ip[k]] += rp;
+        hess[(size_t)ip[k] * P + ir[k]] += rp;
+        hess[(size_t)ip[k] * P + ip[k]] += pp;
+    }
     return MIPWA_OK;
 }
 

@@ -198,3 +198,37 @@ def test_full_gradient_with_floating_shapes_matches_oracle():
     vb, gb = m0.nll_grad_full(c0.truth)
     assert va == vb and np.max(np.abs(ga - gb)) <= 1e-12 * np.max(np.abs(ga))
     m0.close()
+
+
+@pytest.mark.parametrize("idx,kw", [(0, dict()), (1, dict(n_ev=20_011, n_norm=30_000)), (4, dict(n_ev=4_000, n_norm=6_000))])
+def test_hessian_matches_oracle(idx, kw):
+    """mipwa_nll_hessian (k_gram in HESS mode over the events + Gram matrix + host assembly) against the oracle's O11
+    Hessian, which tests/test_oracle_shape.py pins to differences of the gradient and to the invariance identities.
+    Every entry within 1e-9 of the largest entry (same reasoning as the gradient tolerance, reading P26)."""
+    B = _lib()
+    c, o, (e12, e13, g12, g13, w) = make_case(idx, **kw)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(e12, e13); m.set_norm_points(g12, g13, w)
+    p = c.perturbed(1)
+    v, g, H = m.nll_hessian(p)
+    Href = o.nll_hessian(p, e12, e13, g12, g13, w)
+    ref_n, gref = o.nll_grad(p, e12, e13, g12, g13, w)
+    _, sl, integ = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    assert abs(v - ref_n) <= nll_tol(ref_n, sl, integ, e12.size)
+    _check(g, gref)
+    scale = np.max(np.abs(Href))
+    assert H.shape == Href.shape
+    assert np.max(np.abs(H - Href)) <= 1e-9 * scale, np.max(np.abs(H - Href)) / scale
+    assert np.max(np.abs(H - H.T)) <= 1e-11 * scale
+    m.close()
+
+
+def test_hessian_needs_fixed_shapes():
+    B = _lib()
+    c, o, (e12, e13, g12, g13, w) = make_case(3, n_ev=2_000, n_norm=2_000)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(e12, e13); m.set_norm_points(g12, g13, w)
+    with pytest.raises(B.MipwaError) as e:
+        m.nll_hessian(c.truth)
+    assert e.value.code == B.ERR_STATE
+    m.close()
