@@ -503,6 +503,13 @@ def run_probe(args):
             da = fit[:N] - c.truth[:N]
             dphi = fit[N:2 * N] - c.truth[N:2 * N]
             fits[spacing] = fit
+            # analytic Hessian at the minimum (mipwa_nll_hessian).  The knot errors are strongly correlated (a_0 at the
+            # threshold anchors the common scale weakly), so the closure check is the quadratic form
+            # d^T H d of d = fit - truth, which should equal 2 (NLL(truth) - NLL(fit)) and follow chi^2(n_free).
+            _, _, H = m.nll_hessian(fit)
+            Hf = H[np.ix_(free, free)]
+            dfree = (fit - c.truth)[free]
+            sig = np.sqrt(np.diag(np.linalg.inv(Hf)))
             print(json.dumps({"probe": "grid-bias", "spacing_gev2": spacing, "grid_cells_inside": int(g12.size),
                               "n_ev": int(e12.numel()), "n_free": int(free.sum()), "fit_wall_s": fit_s,
                               "nll_grad_calls": calls[0], "ms_per_call_incl_minimiser": fit_s / max(calls[0], 1) * 1e3,
@@ -510,6 +517,9 @@ def run_probe(args):
                               "median_abs_da": float(np.median(np.abs(da))), "rms_da": float(np.sqrt(np.mean(da ** 2))),
                               "median_abs_dphi": float(np.median(np.abs(dphi))), "rms_dphi": float(np.sqrt(np.mean(dphi ** 2))),
                               "d_phi1020_mag": float(fit[2 * N] - c.truth[2 * N]),
+                              "chi2_quadratic_form": float(dfree @ Hf @ dfree), "two_delta_nll": float(2 * (nll_truth - res.fun)),
+                              "median_sigma_a": float(np.median(sig[:N - 1])),
+                              "hessian_positive_definite": bool(np.all(np.linalg.eigvalsh(Hf) > 0)),
                               "event_generation_s": gen_s}), flush=True)
         # the same sample in every fit, so the statistical scatter is common: the shift against the finest grid is
         # the bias the coarser normalisation grid causes (the paper's Fig. 2 observation)
