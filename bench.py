@@ -389,7 +389,8 @@ def run_ours(args, cfg, workload):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": dict(workload, events_per_gpu=n_ev, norm_points_per_gpu=n_norm,
-                           l2="inputs (16 B x 2 x 10M = 320 MB per step) exceed the 126 MB L2; no flush needed",
+                           l2="inputs read per step (18 B x 10M events + 26 B x 10M weighted normalisation points = 440 MB) exceed the "
+                              "126 MB L2; no flush needed",
                            parallelism=f"dp{world} (events and normalisation points sharded; 3 doubles all-gathered per call)"),
             "nll_evals_per_s": 1e3 / ms_step, "points_per_s": (n_ev + n_norm) * world / (ms_step * 1e-3),
             "nll": nll, "clocks": clocks, "gpu_launches": int(launches) * world,
