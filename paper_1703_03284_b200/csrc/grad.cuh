@@ -265,14 +265,16 @@ k_grad_recompute(const __grid_constant__ DevModel m,
     constexpr int RR = GradDims<R1, R2>::RR;
     extern __shared__ double grad_bins[];                  // [2][4][N-1][2]
     __shared__ SplineCoefSmem sm;
-    __shared__ double red32[32];
     const int NS = m.N - 1, R = m.R, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) grad_bins[k] = 0.0;
     load_spline_coef_smem(sm, m);                          // ends with __syncthreads()
 
     double* mine = partials + (size_t)blockIdx.x * NV;
-    // events pass, then its scalars are reduced and stored before the second pass so that only one set of resonance
-    // accumulators is live at a time (register pressure)
+    // events pass, then normalisation pass; only one set of resonance accumulators is live at a time (register
+    // pressure).  After a pass every warp leaves its sums in shared memory and moves on: no block barrier between the
+    // passes, so a warp that finishes its chunk early starts the next pass at once.
+    __shared__ double wpart[2][MIPWA_GRAD_BLOCK / 32][1 + 2 * RR];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
         double Sc = 0.0, Fr[RR], Fi[RR];
@@ -280,17 +282,26 @@ k_grad_recompute(const __grid_constant__ DevModel m,
         for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
         if (pass == 0) grad_pass<R1, R2, FL, true>(sm, m, e12, e13, nullptr, eseg, n_ev, f_ev, grad_bins, Sc, Fr, Fi);
         else grad_pass<R1, R2, FL, false>(sm, m, g12, g13, gw, gseg, n_norm, f_nm, grad_bins + nb, Sc, Fr, Fi);
-        double v = block_sum(Sc, red32);
-        if (threadIdx.x == 0) mine[pass] = v;
-        for (int r = 0; r < R; ++r) {
-            double a = 0, b = 0;
-            if (R1 >= 0) {
 #pragma unroll
-                for (int q = 0; q < RR; ++q) if (q == r) { a = Fr[q]; b = Fi[q]; }
-            } else { a = Fr[r]; b = Fi[r]; }
-            a = block_sum(a, red32); if (threadIdx.x == 0) mine[2 + 2 * R * pass + 2 * r] = a;
-            b = block_sum(b, red32); if (threadIdx.x == 0) mine[2 + 2 * R * pass + 2 * r + 1] = b;
+        for (int off = 16; off > 0; off >>= 1) Sc += __shfl_down_sync(0xffffffffu, Sc, off);
+        if (lane == 0) wpart[pass][warp][0] = Sc;
+#pragma unroll
+        for (int r = 0; r < RR; ++r) {
+            double a = Fr[r], bq = Fi[r];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                a += __shfl_down_sync(0xffffffffu, a, off);
+                bq += __shfl_down_sync(0xffffffffu, bq, off);
+            }
+            if (lane == 0) { wpart[pass][warp][1 + 2 * r] = a; wpart[pass][warp][2 + 2 * r] = bq; }
         }
+    }
+    __syncthreads();                                       // every warp has left both sets of sums
+    for (int t = threadIdx.x; t < 2 * (1 + 2 * R); t += blockDim.x) {
+        const int pass = t / (1 + 2 * R), k = t - pass * (1 + 2 * R);
+        double v = 0.0;
+        for (int w = 0; w < nwarp; ++w) v += wpart[pass][w][k];            // fixed order
+        mine[k == 0 ? pass : 2 + 2 * R * pass + (k - 1)] = v;
     }
     __syncthreads();                                       // all flushes into grad_bins are done
     for (int k = threadIdx.x; k < 2 * nb; k += blockDim.x) mine[2 + 4 * R + k] = grad_bins[k];
