@@ -491,8 +491,8 @@ __device__ __forceinline__ void shape_channel(const ResDev& r, const Channel& c,
     mr = fma(tr, br, -ti * bi); mi = fma(tr, bi, ti * br);
 }
 
-template <int NF>
-__global__ void __launch_bounds__(256, 2)
+template <int NF, int FL>
+__global__ void __launch_bounds__(512, 1)
 k_grad_shape(const __grid_constant__ DevModel m, const ShapeSel sel,
              const double* __restrict__ e12, const double* __restrict__ e13, const double2* __restrict__ f_ev,
              long long n_ev,
@@ -511,11 +511,14 @@ k_grad_shape(const __grid_constant__ DevModel m, const ShapeSel sel,
         double acc[NF][4];
 #pragma unroll
         for (int f = 0; f < NF; ++f) acc[f][0] = acc[f][1] = acc[f][2] = acc[f][3] = 0.0;
-        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-            const double x = s12[i], y = s13[i];
-            const double2 fv = fp[i];
-            const double fr = fv.x, fi = fv.y;
-            const Channel ca = make_channel<0>(m, x, y), cb = make_channel<0>(m, y, x);
+        long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        double nx = 1.0, ny = 1.0;                         // the next point, loaded one iteration ahead
+        double2 nf = make_double2(0.0, 0.0);
+        if (i < n) { nx = s12[i]; ny = s13[i]; nf = fp[i]; }
+        for (; i < n; i += stride) {
+            const double x = nx, y = ny, fr = nf.x, fi = nf.y;
+            if (i + stride < n) { nx = s12[i + stride]; ny = s13[i + stride]; nf = fp[i + stride]; }
+            const Channel ca = make_channel<FL & MIPWA_FL_EQM>(m, x, y), cb = make_channel<FL & MIPWA_FL_EQM>(m, y, x);
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const ResDev& r = m.res[sel.slot[f]];

@@ -1254,8 +1254,8 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         for (int d = 0; d < R; ++d)
             if (c->model.res[d].fl == f) slots.push_back(d);
     if ((int)slots.size() != F) return fail(c, MIPWA_ERR_STATE, "floating resonance not found in the device model");
-    const int64_t need = (std::max(c->ev.n, c->nm.n) + 255) / 256;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * 2, need));
+    const int64_t need = (std::max(c->ev.n, c->nm.n) + 511) / 512;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count, need));
     const size_t want = (size_t)grid * 8 * MIPWA_SHAPE_MAXF;
     if (c->gpartials_len < want) {
         if (c->d_gpartials) cudaFree(c->d_gpartials);
@@ -1272,8 +1272,14 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         for (int q = 0; q < MIPWA_SHAPE_MAXF; ++q) sel.slot[q] = slots[f0 + std::min(q, nf - 1)];
         if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
 #define MIPWA_SHAPE_LAUNCH(NF)                                                                                     \
-    k_grad_shape<NF><<<grid, 256, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, G.s12, G.s13, c->d_f_nm, \
-                                                  G.n, c->d_gpartials)
+    do {                                                                                                           \
+        if (c->model_flags & MIPWA_FL_EQM)                                                                         \
+            k_grad_shape<NF, MIPWA_FL_EQM><<<grid, 512, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, \
+                                                                        G.s12, G.s13, c->d_f_nm, G.n, c->d_gpartials); \
+        else                                                                                                       \
+            k_grad_shape<NF, 0><<<grid, 512, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, G.s12,    \
+                                                             G.s13, c->d_f_nm, G.n, c->d_gpartials);               \
+    } while (0)
         switch (nf) {
             case 1: MIPWA_SHAPE_LAUNCH(1); break;
             case 2: MIPWA_SHAPE_LAUNCH(2); break;
