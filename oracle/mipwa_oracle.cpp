@@ -709,4 +709,74 @@ void orc_nll_hessian(const orc_kin* kin, int n, const double* knots, int R, cons
     }
 }
 
+// ---- O12 ("signal purity 90 %"): likelihood of a signal + background mixture.  Per event
+// the PDF is f_s |A_i|^2 / I + (1 - f_s) b_i with b_i the (normalised) background density at the event, supplied by
+// the caller, and f_s the signal fraction:
+//     NLL = - sum_i ln( f_s |A_i|^2 / I + (1 - f_s) b_i ),      I = sum_j w_j |A_j|^2.
+// Gradient with respect to the 2N + 2R linear-coefficient parameters through calG_k = dNLL/dRe c_k + i dNLL/dIm c_k:
+//     p_i = f_s |A_i|^2 / I + (1 - f_s) b_i
+//     calG_k = -(2 f_s / I) sum_i A_i conj(B_ik) / p_i + (2 f_s / I^2) [sum_i |A_i|^2 / p_i] sum_j w_j A_j conj(B_jk)
+// and dNLL/df_s = - sum_i ( |A_i|^2 / I - b_i ) / p_i.      grad: 2N + 2R entries (polar chain rule as O9).
+void orc_nll_mix(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res, const double* params,
+                 int64_t n_ev, const double* e12, const double* e13, const double* bkg, double f_sig,
+                 int64_t n_norm, const double* g12, const double* g13, const double* w,
+                 double* nll, double* grad, double* dnll_dfsig)
+{
+    const Model m = make_model(kin, n, knots, R, res);
+    const Unpacked u = unpack(m, params);
+    const std::vector<double> Mx = cardinal_second_derivs(m);
+    const int K = n + R;
+    std::vector<cplx> B(K);
+    Acc I;
+    std::vector<Acc> nr(K), ni(K);
+    for (int64_t j = 0; j < n_norm; ++j) {
+        const cplx A = amplitude(m, u, g12[j], g13[j]);
+        const double wj = w ? w[j] : 1.0 / (double)n_norm;
+        I.add((long double)wj * std::norm(A));
+        if (grad) {
+            basis_row(m, u.res, Mx, g12[j], g13[j], B.data());
+            for (int k = 0; k < K; ++k) {
+                const cplx v = wj * A * std::conj(B[k]);
+                nr[k].add(v.real()); ni[k].add(v.imag());
+            }
+        }
+    }
+    const double Iv = (double)I.value();
+    Acc S, Q, Fs;
+    std::vector<Acc> er(K), ei(K);
+    for (int64_t i = 0; i < n_ev; ++i) {
+        const cplx A = amplitude(m, u, e12[i], e13[i]);
+        const double a2 = std::norm(A);
+        const double p = f_sig * a2 / Iv + (1.0 - f_sig) * bkg[i];
+        S.add(std::log(p));
+        Q.add(a2 / p);
+        Fs.add((a2 / Iv - bkg[i]) / p);
+        if (grad) {
+            basis_row(m, u.res, Mx, e12[i], e13[i], B.data());
+            for (int k = 0; k < K; ++k) {
+                const cplx v = A * std::conj(B[k]) / p;
+                er[k].add(v.real()); ei[k].add(v.imag());
+            }
+        }
+    }
+    *nll = (double)(-S.value());
+    if (dnll_dfsig) *dnll_dfsig = (double)(-Fs.value());
+    if (!grad) return;
+    const double c1 = -2.0 * f_sig / Iv, c2 = 2.0 * f_sig / (Iv * Iv) * (double)Q.value();
+    for (int k = 0; k < K; ++k) {
+        const cplx G(c1 * (double)er[k].value() + c2 * (double)nr[k].value(),
+                     c1 * (double)ei[k].value() + c2 * (double)ni[k].value());
+        if (k < n) {
+            const double phi = params[n + k];
+            grad[k] = (G * cplx(std::cos(phi), -std::sin(phi))).real();
+            grad[n + k] = (G * std::conj(cplx(0.0, 1.0) * u.y[k])).real();
+        } else {
+            const int r = k - n;
+            const double th = params[2 * n + 2 * r + 1];
+            grad[2 * n + 2 * r] = (G * cplx(std::cos(th), -std::sin(th))).real();
+            grad[2 * n + 2 * r + 1] = (G * std::conj(cplx(0.0, 1.0) * u.c[r])).real();
+        }
+    }
+}
+
 }  // extern "C"

@@ -68,6 +68,8 @@ def lib():
         L.orc_gram.restype = None; L.orc_gram.argtypes = model + [_dp, i64, _dp, _dp, _dp, _dp]
         L.orc_nll_grad.restype = None
         L.orc_nll_grad.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp]
+        L.orc_nll_mix.restype = None
+        L.orc_nll_mix.argtypes = model + [_dp, i64, _dp, _dp, _dp, d, i64, _dp, _dp, _dp, _dp, _dp, _dp]
         L.orc_nll_hessian.restype = None
         L.orc_nll_hessian.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp]
         L.orc_nll_grad_shape.restype = None
@@ -150,6 +152,16 @@ class Oracle:
         self.L.orc_nll_grad(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w),
                             C.byref(nll), _p(grad))
         return nll.value, grad
+
+    def nll_mix(self, params, e12, e13, bkg, f_sig, g12, g13, w=None, grad=False):
+        """signal + background mixture (O12): NLL, or (NLL, gradient over 2N + 2R, dNLL/df_sig) if grad"""
+        p, e12, e13, bkg, g12, g13 = self._params(params), _a(e12), _a(e13), _a(bkg), _a(g12), _a(g13)
+        w = None if w is None else _a(w)
+        nll, dfs = C.c_double(), C.c_double()
+        g = np.zeros(2 * self.n + 2 * self.R) if grad else None
+        self.L.orc_nll_mix(*self._model, _p(p), e12.size, _p(e12), _p(e13), _p(bkg), float(f_sig), g12.size, _p(g12),
+                           _p(g13), _p(w), C.byref(nll), _p(g), C.byref(dfs))
+        return (nll.value, g, dfs.value) if grad else nll.value
 
     def nll_hessian(self, params, e12, e13, g12, g13, w=None):
         """P x P Hessian of the NLL in the 2N + 2R linear-coefficient parameters (fixed shapes)  -- O11"""
