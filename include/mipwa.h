@@ -142,6 +142,21 @@ int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, doubl
  * identical to mipwa_nll_grad when none does.  Errors as mipwa_nll_grad. */
 int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
+/* Signal + background mixture ("signal purity 90 %"): per event the PDF is
+ *     f_s |A_i|^2 / I + (1 - f_s) b_i ,      NLL = - sum_i ln( f_s |A_i|^2 / I + (1 - f_s) b_i ),
+ * with b_i the background density at event i (normalised over the Dalitz plot, supplied by the caller) and f_s the
+ * signal fraction.  Detector efficiency enters through the weights of the normalisation points, as for mipwa_nll.
+ *   mipwa_set_event_background: b = n_ev doubles (HOST: copied; DEVICE: borrowed), in the order of the arrays given
+ *     to the last mipwa_set_events, which it must follow (a new mipwa_set_events drops the densities); NULL clears.
+ *   mipwa_nll_mix: recompute path, two launches (normalisation integral first: the event sum needs I).
+ *   mipwa_nll_mix_grad: also the gradient over the 2N + 2R linear-coefficient parameters (layout of mipwa_nll_grad)
+ *     and dNLL/df_s (dnll_dfsig may be NULL).  Implies mipwa_prepare.
+ * Errors: MIPWA_ERR_STATE before the point sets or the densities are set, MIPWA_ERR_ARG unless 0 < f_sig <= 1. */
+int mipwa_set_event_background(mipwa_ctx* ctx, const double* b, int32_t mem);
+int mipwa_nll_mix(mipwa_ctx* ctx, const double* params, int64_t n_params, double f_sig, double* nll);
+int mipwa_nll_mix_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double f_sig, double* nll, double* grad,
+                       double* dnll_dfsig);
+
 /* NLL, gradient and HESSIAN with respect to the 2N + 2R linear-coefficient parameters, for fixed resonance shapes
  * (the parameter errors and correlations PAPER.md:29 alludes to are the inverse of this matrix at the
  * minimum).  With c = [y_k, c_r], A_i = sum_k c_k B_ik, I = c^H G c and Wirtinger derivatives:

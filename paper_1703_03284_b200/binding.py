@@ -23,7 +23,8 @@ _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STAT
 # every symbol include/mipwa.h declares
 SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
            "mipwa_prepare", "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
-           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_nll_hessian", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
+           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_nll_hessian", "mipwa_set_event_background", "mipwa_nll_mix",
+           "mipwa_nll_mix_grad", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version"]
 
@@ -73,6 +74,9 @@ def load_library():
     L.mipwa_nll_grad.restype = i32; L.mipwa_nll_grad.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_nll_grad_full.restype = i32; L.mipwa_nll_grad_full.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_nll_hessian.restype = i32; L.mipwa_nll_hessian.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
+    L.mipwa_set_event_background.restype = i32; L.mipwa_set_event_background.argtypes = [vp, vp, i32]
+    L.mipwa_nll_mix.restype = i32; L.mipwa_nll_mix.argtypes = [vp, _dp, i64, C.c_double, _dp]
+    L.mipwa_nll_mix_grad.restype = i32; L.mipwa_nll_mix_grad.argtypes = [vp, _dp, i64, C.c_double, _dp, _dp, _dp]
     L.mipwa_generate.restype = i32
     L.mipwa_generate.argtypes = [vp, _dp, i64, C.c_uint64, i64, i32, i32, vp, vp, i32, C.POINTER(i64)]
     L.mipwa_eval_abs2.restype = i32; L.mipwa_eval_abs2.argtypes = [vp, _dp, i64, i32, _dp, i64]
@@ -231,6 +235,34 @@ class Mipwa:
         grad = np.empty(p.size)
         self._check(self.L.mipwa_nll_grad_full(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
         return out.value, grad
+
+    def set_event_background(self, b):
+        """background density per event (numpy: copied; CUDA torch tensor: borrowed), in the order of set_events"""
+        if b is None:
+            self._check(self.L.mipwa_set_event_background(self._h, None, MEM_HOST))
+            self._bkg = None
+            return
+        if hasattr(b, "data_ptr"):
+            self._bkg = b                                  # keep the borrowed tensor alive
+            self._check(self.L.mipwa_set_event_background(self._h, C.c_void_p(b.data_ptr()), MEM_DEVICE))
+        else:
+            a = np.ascontiguousarray(b, dtype=np.float64)
+            self._check(self.L.mipwa_set_event_background(self._h, C.c_void_p(a.ctypes.data), MEM_HOST))
+
+    def nll_mix(self, params, f_sig):
+        p, pp, n = self._params(params)
+        out = C.c_double()
+        self._check(self.L.mipwa_nll_mix(self._h, pp, n, float(f_sig), C.byref(out)))
+        return out.value
+
+    def nll_mix_grad(self, params, f_sig):
+        """(NLL, gradient over 2N + 2R, dNLL/df_sig) of the signal + background mixture"""
+        p, pp, n = self._params(params)
+        out, dfs = C.c_double(), C.c_double()
+        grad = np.empty(2 * self.N + 2 * self.R)
+        self._check(self.L.mipwa_nll_mix_grad(self._h, pp, n, float(f_sig), C.byref(out), grad.ctypes.data_as(_dp),
+                                              C.byref(dfs)))
+        return out.value, grad, dfs.value
 
     def nll_hessian(self, params):
         """(NLL, gradient, Hessian) in the 2N + 2R linear-coefficient parameters; fixed shapes only."""

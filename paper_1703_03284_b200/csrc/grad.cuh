@@ -164,11 +164,13 @@ template <int R1, int R2> struct GradDims {
 
 // one pass over a cell-sorted point set.  EV: events (f = -2/conj(A), scalar = sum ln|A|^2);
 // otherwise normalisation points (f = w A, scalar = sum w |A|^2).
-template <int R1, int R2, int FL, bool EV>
+// MIX (EV only): background density w[i] per event and D = |A|^2 + kappa w: f = -2 A / D, scalar = sum ln D,
+// qsum = sum w / D (mipwa_nll_mix_grad).
+template <int R1, int R2, int FL, bool EV, bool MIX = false>
 __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevModel& m, const double* __restrict__ s12,
                                           const double* __restrict__ s13, const double* __restrict__ w,
                                           const unsigned short* __restrict__ sgp, long long n,
-                                          double2* __restrict__ fout,
+                                          double2* __restrict__ fout, double kappa, double& qsum,
                                           double* bins, double& scalar, double (&Fr)[GradDims<R1, R2>::RR],
                                           double (&Fi)[GradDims<R1, R2>::RR])
 {
@@ -189,6 +191,7 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
         const long long ii = lo + lane < hi ? lo + lane : lo;
         nx = s12[ii]; ny = s13[ii]; nsg = sgp[ii];
         if (!EV) nw = lo + lane < hi ? (w ? w[ii] : 1.0) : 0.0;
+        if (EV && MIX) nw = w[ii];
     }
     for (long long base = lo; base < hi; base += 32) {                     // warp-uniform trip count
         const long long i = base + lane;
@@ -199,6 +202,7 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
             const long long ii = i + 32 < hi ? i + 32 : lo;
             nx = s12[ii]; ny = s13[ii]; nsg = sgp[ii];
             if (!EV) nw = i + 32 < hi ? (w ? w[ii] : 1.0) : 0.0;
+            if (EV && MIX) nw = w[ii];
         }
         double are, aim, t1, t2, tr[RR], ti[RR];
         int j1, j2;
@@ -206,9 +210,12 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
         const double a2 = fma(are, are, aim * aim);
         double fr, fi;
         if (EV) {
-            const double k = valid ? -2.0 * fast_rcp(a2) : 0.0;
+            const double D = MIX ? fma(kappa, wv, a2) : a2;
+            const double rD = fast_rcp(D);
+            const double k = valid ? -2.0 * rD : 0.0;
             fr = k * are; fi = k * aim;
-            lp.add(valid ? a2 : 1.0);
+            lp.add(valid ? D : 1.0);
+            if (MIX) qsum += valid ? wv * rD : 0.0;
         } else {
             fr = wv * are; fi = wv * aim;
             integ = fma(wv, a2, integ);
@@ -253,11 +260,11 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
 #ifndef MIPWA_GRAD_MINBLOCKS
 #define MIPWA_GRAD_MINBLOCKS 1
 #endif
-template <int R1, int R2, int FL>
+template <int R1, int R2, int FL, bool MIX>
 __global__ void __launch_bounds__(MIPWA_GRAD_BLOCK, MIPWA_GRAD_MINBLOCKS)
 k_grad_recompute(const __grid_constant__ DevModel m,
                  const double* __restrict__ e12, const double* __restrict__ e13,
-                 const unsigned short* __restrict__ eseg, long long n_ev,
+                 const unsigned short* __restrict__ eseg, const double* __restrict__ eb, double kappa, long long n_ev,
                  const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
                  const unsigned short* __restrict__ gseg, long long n_norm, double* __restrict__ partials,
                  double2* __restrict__ f_ev, double2* __restrict__ f_nm)
@@ -280,11 +287,20 @@ k_grad_recompute(const __grid_constant__ DevModel m,
         double Sc = 0.0, Fr[RR], Fi[RR];
 #pragma unroll
         for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
-        if (pass == 0) grad_pass<R1, R2, FL, true>(sm, m, e12, e13, nullptr, eseg, n_ev, f_ev, grad_bins, Sc, Fr, Fi);
-        else grad_pass<R1, R2, FL, false>(sm, m, g12, g13, gw, gseg, n_norm, f_nm, grad_bins + nb, Sc, Fr, Fi);
+        double qsum = 0.0;
+        if (pass == 0) grad_pass<R1, R2, FL, true, MIX>(sm, m, e12, e13, eb, eseg, n_ev, f_ev, kappa, qsum, grad_bins, Sc, Fr, Fi);
+        else grad_pass<R1, R2, FL, false>(sm, m, g12, g13, gw, gseg, n_norm, f_nm, 0.0, qsum, grad_bins + nb, Sc, Fr, Fi);
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) Sc += __shfl_down_sync(0xffffffffu, Sc, off);
-        if (lane == 0) wpart[pass][warp][0] = Sc;
+        if (MIX) {
+            // the events-only launch of the mixture has no normalisation points: slot [1] carries sum b / D instead
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) qsum += __shfl_down_sync(0xffffffffu, qsum, off);
+            if (lane == 0) {
+                if (pass == 0) { wpart[0][warp][0] = Sc; wpart[1][warp][0] = qsum; }
+                else wpart[1][warp][0] += Sc;
+            }
+        } else if (lane == 0) wpart[pass][warp][0] = Sc;
 #pragma unroll
         for (int r = 0; r < RR; ++r) {
             double a = Fr[r], bq = Fi[r];

@@ -80,11 +80,13 @@ struct LogProd {
 // event), then over normalisation points.  Block partials go to partials[block] = (sum ln|A|^2, sum w|A|^2); the
 // last block to finish adds them in block order (fixed order: bit-reproducible for a given grid) and writes the
 // two totals to `result` (mapped pinned host memory).
-template <int R1, int R2, int FL>
+// MIX = true (mipwa_nll_mix, signal + background mixture): the events carry a background density eb[i] and the sum is
+// over ln(|A_i|^2 + kappa eb[i]) with kappa = I (1 - f_s) / f_s from a first, normalisation-only launch.
+template <int R1, int R2, int FL, bool MIX>
 __global__ void __launch_bounds__(MIPWA_REC_BLOCK, MIPWA_REC_MINBLOCKS)
 k_nll_recompute(const __grid_constant__ DevModel m,
                 const double* __restrict__ e12, const double* __restrict__ e13, const unsigned short* __restrict__ eseg,
-                long long n_ev,
+                const double* __restrict__ eb, double kappa, long long n_ev,
                 const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw,
                 const unsigned short* __restrict__ gseg, long long n_norm, double2* __restrict__ partials, unsigned int* __restrict__ ticket,
                 double* __restrict__ result)
@@ -103,22 +105,22 @@ k_nll_recompute(const __grid_constant__ DevModel m,
     constexpr int PTS = (R1 == 0 && R2 == 0) ? 4 : MIPWA_REC_PTS;
     LogProd lp;
     {
-        double a[PTS], b[PTS];
+        double a[PTS], b[PTS], bk[PTS];
         unsigned int sg[PTS];
 #pragma unroll
         for (int q = 0; q < PTS; ++q) {
             const long long i = t0 + q * stride;
-            a[q] = 1.0; b[q] = 1.0; sg[q] = 0u;
-            if (i < n_ev) { a[q] = e12[i]; b[q] = e13[i]; sg[q] = eseg[i]; }
+            a[q] = 1.0; b[q] = 1.0; sg[q] = 0u; bk[q] = 0.0;
+            if (i < n_ev) { a[q] = e12[i]; b[q] = e13[i]; sg[q] = eseg[i]; if (MIX) bk[q] = eb[i]; }
         }
         for (long long i = t0; i < n_ev; i += PTS * stride) {
-            double na[PTS], nb[PTS];
+            double na[PTS], nb[PTS], nbk[PTS];
             unsigned int ns[PTS];
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 const long long nx = i + (PTS + q) * stride;
-                na[q] = 1.0; nb[q] = 1.0; ns[q] = 0u;
-                if (nx < n_ev) { na[q] = e12[nx]; nb[q] = e13[nx]; ns[q] = eseg[nx]; }
+                na[q] = 1.0; nb[q] = 1.0; ns[q] = 0u; nbk[q] = 0.0;
+                if (nx < n_ev) { na[q] = e12[nx]; nb[q] = e13[nx]; ns[q] = eseg[nx]; if (MIX) nbk[q] = eb[nx]; }
             }
             double v[PTS];
 #pragma unroll
@@ -126,11 +128,13 @@ k_nll_recompute(const __grid_constant__ DevModel m,
                 double re, im;
                 amplitude_seg<R1, R2, FL>(sm, m, a[q], b[q], sg[q], re, im);
                 v[q] = fma(re, re, im * im);
+                if (MIX) v[q] = fma(kappa, bk[q], v[q]);
             }
 #pragma unroll
             for (int q = 0; q < PTS; ++q) {
                 lp.add(i + q * stride < n_ev ? v[q] : 1.0);
                 a[q] = na[q]; b[q] = nb[q]; sg[q] = ns[q];
+                if (MIX) bk[q] = nbk[q];
             }
         }
     }

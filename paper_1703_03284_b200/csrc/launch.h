@@ -11,21 +11,36 @@ struct HybCoef;
 
 // tu_recompute.cu: k_nll_recompute; tu_abs2.cu: k_abs2 (kernels.cuh)
 cudaError_t mipwa_occupancy_nll_recompute(const int* n_spin, int fl, int* blocks_per_sm);
+// eb != nullptr selects the mixture kernels (tu_recompute_mix.cu): sum of ln(|A|^2 + kappa eb[i]) over the events
 cudaError_t mipwa_launch_nll_recompute(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
-                                       const double* e12, const double* e13, const unsigned short* eseg, long long n_ev,
+                                       const double* e12, const double* e13, const unsigned short* eseg,
+                                       const double* eb, double kappa, long long n_ev,
                                        const double* g12, const double* g13, const double* gw,
                                        const unsigned short* gseg, long long n_norm, double2* partials,
                                        unsigned int* ticket, double* result);
+cudaError_t mipwa_launch_nll_recompute_mix(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
+                                           const double* e12, const double* e13, const unsigned short* eseg,
+                                           const double* eb, double kappa, long long n_ev, const double* g12,
+                                           const double* g13, const double* gw, const unsigned short* gseg,
+                                           long long n_norm, double2* partials, unsigned int* ticket, double* result);
 cudaError_t mipwa_launch_abs2(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
                               const double* s12, const double* s13, const unsigned short* seg, long long n, double* out);
 
 // tu_grad.cu: k_grad_recompute (grad.cuh)
 cudaError_t mipwa_occupancy_grad_recompute(const int* n_spin, int fl, size_t smem, int* blocks_per_sm);
+// eb != nullptr selects the mixture kernels (tu_grad_mix.cu): f = -2 A / (|A|^2 + kappa eb[i]), result[1] = sum eb / D
 cudaError_t mipwa_launch_grad_recompute(const int* n_spin, int fl, int grid, size_t smem, cudaStream_t st,
                                         const DevModel& m, const double* e12, const double* e13,
-                                        const unsigned short* eseg, long long n_ev, const double* g12,
+                                        const unsigned short* eseg, const double* eb, double kappa, long long n_ev,
+                                        const double* g12,
                                         const double* g13, const double* gw, const unsigned short* gseg,
                                         long long n_norm, double* partials, double2* f_ev, double2* f_nm);
+
+cudaError_t mipwa_launch_grad_recompute_mix(const int* n_spin, int fl, int grid, size_t smem, cudaStream_t st,
+                                            const DevModel& m, const double* e12, const double* e13,
+                                            const unsigned short* eseg, const double* eb, double kappa, long long n_ev,
+                                            const double* g12, const double* g13, const double* gw,
+                                            const unsigned short* gseg, long long n_norm, double* partials);
 
 // tu_hybrid.cu: k_nll_hybrid (hybrid.cuh); f1, f2 = floating resonances of spin 1, 2, rc = cached (fixed) resonances
 bool mipwa_hybrid_supported(int f1, int f2, int rc);

@@ -557,8 +557,9 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
     const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, evs(c).s12,
-                                                      evs(c).s13, evs(c).seg, evs(c).n, nms(c).s12, nms(c).s13, nms(c).w,
-                                                      nms(c).seg, nms(c).n, c->d_partials, c->d_ticket, c->d_result);
+                                                      evs(c).s13, evs(c).seg, nullptr, 0.0, evs(c).n, nms(c).s12,
+                                                      nms(c).s13, nms(c).w, nms(c).seg, nms(c).n, c->d_partials,
+                                                      c->d_ticket, c->d_result);
     ++c->launches;
     CU(c, le);
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
@@ -1182,9 +1183,10 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
     const cudaError_t le = mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model,
-                                                       c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, c->ev_sorted.n,
-                                                       c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w, c->nm_sorted.seg,
-                                                       c->nm_sorted.n, c->d_gpartials, c->want_f ? c->d_f_ev : nullptr,
+                                                       c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, nullptr, 0.0,
+                                                       c->ev_sorted.n, c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w,
+                                                       c->nm_sorted.seg, c->nm_sorted.n, c->d_gpartials,
+                                                       c->want_f ? c->d_f_ev : nullptr,
                                                        c->want_f ? c->d_f_nm : nullptr);
     ++c->launches;
     CU(c, le);
@@ -1307,6 +1309,150 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         }
     }
     c->last_ms = ms_total;
+    return MIPWA_OK;
+}
+
+// ---- signal + background mixture (include/mipwa.h): recompute path, two launches -----------------------------------
+int mipwa_set_event_background(mipwa_ctx* c, const double* b, int32_t mem)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    if (c->ev.n < 0) return fail(c, MIPWA_ERR_STATE, "set the events first");
+    if (mem != MIPWA_MEM_HOST && mem != MIPWA_MEM_DEVICE) return fail(c, MIPWA_ERR_ARG, "bad mem flag");
+    int rc = use_device(c);
+    if (rc) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    Slot& s = c->ev;
+    if (s.owned[2]) { cudaFree(s.owned[2]); s.owned[2] = nullptr; }
+    s.w = nullptr;
+    c->ev_sorted_valid = false;                            // the cell-sorted copy carries the densities along
+    c->cache_valid = false; c->hyb_ev_valid = false;       // the caches follow the event order of the sorted copy
+    if (!b || s.n == 0) return MIPWA_OK;                   // NULL clears
+    if (mem == MIPWA_MEM_HOST || ((uintptr_t)b & 7u)) {
+        CU(c, cudaMalloc(&s.owned[2], (size_t)s.n * sizeof(double)));
+        CU(c, cudaMemcpyAsync(s.owned[2], b, (size_t)s.n * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        s.w = (const double*)s.owned[2];
+    } else {
+        s.w = b;
+    }
+    return MIPWA_OK;
+}
+
+// I from a normalisation-only launch, then the event sum of ln(|A|^2 + kappa b), kappa = I (1 - f_s) / f_s:
+// NLL = -sum_i ln(f_s |A_i|^2 / I + (1 - f_s) b_i) = -sum_i ln(|A_i|^2 + kappa b_i) - n_ev ln(f_s / I)
+int mipwa_nll_mix(mipwa_ctx* c, const double* params, int64_t n_params, double f_sig, double* nll)
+{
+    if (!c || !params || !nll) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    if (c->ev.n > 0 && !c->ev.w) return fail(c, MIPWA_ERR_STATE, "set the background densities (mipwa_set_event_background)");
+    if (!(f_sig > 0.0 && f_sig <= 1.0)) return fail(c, MIPWA_ERR_ARG, "signal fraction must be in (0, 1]");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    const Slot& E = evs(c);
+    const Slot& G = nms(c);
+    const int64_t need = (std::max(E.n, G.n) + MIPWA_REC_BLOCK - 1) / MIPWA_REC_BLOCK;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, E.s12, E.s13, E.seg,
+                                                nullptr, 0.0, 0, G.s12, G.s13, G.w, G.seg, G.n, c->d_partials,
+                                                c->d_ticket, c->d_result);
+    ++c->launches;
+    CU(c, le);
+    CU(c, cudaStreamSynchronize(c->stream));
+    const double I = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
+    const double kappa = I * (1.0 - f_sig) / f_sig;
+    double S = 0.0;
+    if (E.n > 0) {
+        le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, E.s12, E.s13, E.seg, E.w, kappa,
+                                        E.n, G.s12, G.s13, G.w, G.seg, 0, c->d_partials, c->d_ticket, c->d_result);
+        ++c->launches;
+        CU(c, le);
+        if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        S = c->h_result[0];
+    } else {
+        if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+    }
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    *nll = -S - (double)c->ev.n * std::log(f_sig / I);
+    return MIPWA_OK;
+}
+
+// value + gradient of the mixture: k_grad_recompute twice.  Launch 1 over the normalisation points alone gives I, F_nm
+// and the normalisation moments; launch 2 over the events alone with kappa = I (1 - f_s) / f_s gives sum ln D_i,
+// Q = sum b_i / D_i (D_i = |A_i|^2 + kappa b_i), F_ev and the event moments, f_i = -2 A_i / D_i.  Then
+//   NLL = -sum ln D_i - n ln(f_s / I),  calG = G_ev + (2 / I) (n - kappa Q) G_nm,  dNLL/df_s = -(n - I Q / f_s) / f_s.
+int mipwa_nll_mix_grad(mipwa_ctx* c, const double* params, int64_t n_params, double f_sig, double* nll, double* grad,
+                       double* dnll_dfsig)
+{
+    if (!c || !params || !nll || !grad) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    if (c->ev.n > 0 && !c->ev.w) return fail(c, MIPWA_ERR_STATE, "set the background densities (mipwa_set_event_background)");
+    if (!(f_sig > 0.0 && f_sig <= 1.0)) return fail(c, MIPWA_ERR_ARG, "signal fraction must be in (0, 1]");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = prepare_sorted(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
+    const size_t smem = (size_t)2 * nb * sizeof(double);
+    if (!c->grad_blocks_per_sm) {
+        if (mipwa_occupancy_grad_recompute(c->n_spin, c->model_flags, smem, &c->grad_blocks_per_sm) != cudaSuccess)
+            return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
+        if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
+    }
+    const int64_t gneed = (std::max(c->ev.n, c->nm.n) + MIPWA_GRAD_BLOCK - 1) / MIPWA_GRAD_BLOCK;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->grad_blocks_per_sm, gneed));
+    if (c->gpartials_len < (size_t)grid * NV) {
+        if (c->d_gpartials) cudaFree(c->d_gpartials);
+        c->d_gpartials = nullptr; c->gpartials_len = 0;
+        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NV * sizeof(double)));
+        c->gpartials_len = (size_t)grid * NV;
+    }
+    const Slot& E = c->ev_sorted;
+    const Slot& G = c->nm_sorted;
+    std::vector<double> h1(NV), h2(NV, 0.0);
+    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    for (int launch = 0; launch < 2; ++launch) {
+        if (launch == 1 && E.n == 0) break;
+        const double I1 = launch == 1 ? h1[1] * (c->nm.w ? 1.0 : 1.0 / (double)c->nm.n) : 0.0;
+        const double kappa = launch == 1 ? I1 * (1.0 - f_sig) / f_sig : 0.0;
+        const cudaError_t le = launch == 0
+            ? mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model, E.s12, E.s13, E.seg,
+                                          nullptr, 0.0, 0, G.s12, G.s13, G.w, G.seg, G.n, c->d_gpartials, nullptr, nullptr)
+            : mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model, E.s12, E.s13, E.seg,
+                                          E.w, kappa, E.n, G.s12, G.s13, G.w, G.seg, 0, c->d_gpartials, nullptr, nullptr);
+        ++c->launches;
+        CU(c, le);
+        k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        if (launch == 1 || E.n == 0) { if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream)); }
+        CU(c, cudaStreamSynchronize(c->stream));
+        std::memcpy(launch == 0 ? h1.data() : h2.data(), c->h_result, NV * sizeof(double));
+    }
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+
+    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
+    const double I = h1[1] * wn, n_ev = (double)c->ev.n, kappa = I * (1.0 - f_sig) / f_sig;
+    const double S = h2[0], Q = h2[1];
+    *nll = -S - n_ev * std::log(f_sig / I);
+    if (dnll_dfsig) *dnll_dfsig = -(n_ev - I * Q / f_sig) / f_sig;
+    const double scale = 2.0 * (n_ev - kappa * Q) / I * wn;
+    const double *Fe = h2.data() + 2, *Fn = h1.data() + 2 + 2 * R, *Be = h2.data() + 2 + 4 * R, *Bn = h1.data() + 2 + 4 * R + nb;
+    std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * R);
+    for (int k = 0; k < nb; ++k) Gsc[k] = Be[k] + scale * Bn[k];
+    spline_adjoint(c, Gsc.data(), Gy.data());
+    for (int d = 0; d < R; ++d) {
+        const int r = c->perm[d];
+        Gr[2 * r] = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
+        Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
+    }
+    polar_chain(c, params, Gy.data(), Gr.data(), grad);
     return MIPWA_OK;
 }
 
