@@ -272,6 +272,26 @@ def run_ours(args, cfg, workload):
                          "d_mass_d_width": [float(x) for x in grad_f[grad.size:]],
                          "what": "mipwa_nll_grad_full: the above + d/d(mass, width) of every floating resonance"}
 
+    # ---- signal + background mixture (purity 90 %): flat background density, two launches per call ----------
+    m.set_event_background(torch.full((n_ev,), 1.0 / I.dalitz_area(cfg.kin), dtype=torch.float64, device=dev))
+    for t in range(3):
+        m.nll_mix(params[t], 0.9)
+    mix_ms = []
+    for t in range(sub_steps):
+        nll_mix = m.nll_mix(params[args.warmup + t % args.steps], 0.9)
+        mix_ms.append(m.last_kernel_ms())
+    for t in range(2):
+        m.nll_mix_grad(params[t], 0.9)
+    mixg_ms = []
+    for t in range(sub_steps):
+        nll_mixg, g_mix, dfs_mix = m.nll_mix_grad(params[args.warmup + t % args.steps], 0.9)
+        mixg_ms.append(m.last_kernel_ms())
+    mix_info = {"f_sig": 0.9, "value_kernel_ms": float(np.mean(mix_ms)), "grad_kernel_ms": float(np.mean(mixg_ms)),
+                "nll": nll_mix, "nll_grad_path": nll_mixg, "dnll_dfsig": dfs_mix,
+                "what": "mipwa_nll_mix / mipwa_nll_mix_grad: -sum ln(f_s |A|^2 / I + (1 - f_s) b), normalisation launch then "
+                        "event launch (kernel_ms spans both and the host read of I between them)"}
+    m.set_event_background(None)
+
     # ---- hybrid path (AUTO's choice for this model): rho(770) recomputed, rho(1450) and f2(1270) cached per point -------
     hybrid_info = None
     try:
@@ -399,7 +419,7 @@ def run_ours(args, cfg, workload):
                     "what": "mipwa_set_events + mipwa_set_norm_points from pinned HOST arrays + mipwa_nll, every step"},
             "fit_step": {"ms_per_call": 1e3 * fit_step_s, "nll_evals_per_s": 1.0 / fit_step_s,
                          "what": "wall clock of mipwa_nll(host params) -> host fp64 with events resident (what a minimiser sees)"},
-            "prepare_s": t_prep, "roofline": roofline, "grad": grad_info, "hybrid": hybrid_info, "cached": cached_info, "cpu_baseline": cpu, "input_generation_s": t_gen, "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
+            "prepare_s": t_prep, "roofline": roofline, "grad": grad_info, "mixture": mix_info, "hybrid": hybrid_info, "cached": cached_info, "cpu_baseline": cpu, "input_generation_s": t_gen, "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
