@@ -80,7 +80,11 @@ int mipwa_set_stream(mipwa_ctx* ctx, void* cuda_stream);
 
 /* Data events: n pairs (s12[i], s13[i]).  Every point is checked ON THE DEVICE against the Dalitz boundary
  * ((m1+m2)^2 <= s12 <= (M-m3)^2 and s13 inside its band); a point outside -> MIPWA_ERR_DOMAIN and the slot is
- * left empty.  n = 0 is allowed (the NLL is then 0).  Invalidates the cached basis. */
+ * left empty.  n = 0 is allowed (the NLL is then 0).  Invalidates the cached basis.
+ * The same pass stores, in library-owned memory, the spline segment of s12[i] and of s13[i] as one uint16 per point
+ * (knots are fixed at mipwa_create, so the pair is a property of the point set; +2 B per point): the per-call kernels
+ * index the spline tables with it.  Borrowed (MIPWA_MEM_DEVICE) arrays must therefore not change while they are set;
+ * a device array that is not 16-byte aligned is copied instead of borrowed. */
 int mipwa_set_events(mipwa_ctx* ctx, const double* s12, const double* s13, int64_t n, int32_t mem);
 
 /* Normalisation points with weights w (NULL: w_j = 1/n).  I = sum_j w_j |A_j|^2 stands for the integral of
