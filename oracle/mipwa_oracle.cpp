@@ -497,10 +497,13 @@ void orc_gram(const orc_kin* kin, int n, const double* knots, int R, const orc_r
 //   calG_k = dNLL/dRe c_k + i dNLL/dIm c_k = -2 sum_i conj(B_ik)/conj(A_i) + (2 n_ev/I) sum_j w_j A_j conj(B_jk)
 //   c = rho e^{i theta}:  dNLL/drho = Re(calG e^{-i theta}),  dNLL/dtheta = Re(calG conj(i c)).
 // grad layout = params layout: [d/da_k | d/dphi_k | (d/d|c_r|, d/d arg c_r)].
-void orc_nll_grad(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res, const double* params,
-                  int64_t n_ev, const double* e12, const double* e13,
-                  int64_t n_norm, const double* g12, const double* g13, const double* w,
-                  double* nll, double* grad)
+// The same sums also give the two pieces a sharded likelihood exchanges: with S = sum_i ln|A_i|^2,
+//   grad_ev = d(-S)/dtheta  (calG_k = -2 sum_i conj(B_ik)/conj(A_i)),   grad_nm = dI/dtheta  (calG_k = 2 sum_j w_j A_j conj(B_jk)),
+// so that grad = grad_ev + (n_ev / I) grad_nm.  Optional outputs; the arithmetic of nll and grad does not depend on them.
+static void nll_grad_linear(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res, const double* params,
+                            int64_t n_ev, const double* e12, const double* e13,
+                            int64_t n_norm, const double* g12, const double* g13, const double* w,
+                            double* nll, double* grad, double* sum_log, double* integral, double* grad_ev, double* grad_nm)
 {
     const Model m = make_model(kin, n, knots, R, res);
     const Unpacked u = unpack(m, params);
@@ -551,17 +554,35 @@ void orc_nll_grad(const orc_kin* kin, int n, const double* knots, int R, const o
         }
         const long double f = 2.0L * (long double)n_ev / Iv;
         const cplx G((double)(-2.0L * er.value() + f * nr.value()), (double)(-2.0L * ei.value() + f * ni.value()));
-        if (k < n) {
-            const double phi = params[n + k];
-            grad[k] = (G * cplx(std::cos(phi), -std::sin(phi))).real();
-            grad[n + k] = (G * std::conj(cplx(0.0, 1.0) * u.y[k])).real();
-        } else {
-            const int r = k - n;
-            const double th = params[2 * n + 2 * r + 1];
-            grad[2 * n + 2 * r] = (G * cplx(std::cos(th), -std::sin(th))).real();
-            grad[2 * n + 2 * r + 1] = (G * std::conj(cplx(0.0, 1.0) * u.c[r])).real();
+        const cplx Ge((double)(-2.0L * er.value()), (double)(-2.0L * ei.value()));
+        const cplx Gn((double)(2.0L * nr.value()), (double)(2.0L * ni.value()));
+        const cplx calG[3] = { G, Ge, Gn };
+        double* out[3] = { grad, grad_ev, grad_nm };
+        for (int q = 0; q < 3; ++q) {
+            if (!out[q]) continue;
+            if (k < n) {
+                const double phi = params[n + k];
+                out[q][k] = (calG[q] * cplx(std::cos(phi), -std::sin(phi))).real();
+                out[q][n + k] = (calG[q] * std::conj(cplx(0.0, 1.0) * u.y[k])).real();
+            } else {
+                const int r = k - n;
+                const double th = params[2 * n + 2 * r + 1];
+                out[q][2 * n + 2 * r] = (calG[q] * cplx(std::cos(th), -std::sin(th))).real();
+                out[q][2 * n + 2 * r + 1] = (calG[q] * std::conj(cplx(0.0, 1.0) * u.c[r])).real();
+            }
         }
     }
+    if (sum_log) *sum_log = (double)Sv;
+    if (integral) *integral = (double)Iv;
+}
+
+void orc_nll_grad(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res, const double* params,
+                  int64_t n_ev, const double* e12, const double* e13,
+                  int64_t n_norm, const double* g12, const double* g13, const double* w,
+                  double* nll, double* grad)
+{
+    nll_grad_linear(kin, n, knots, R, res, params, n_ev, e12, e13, n_norm, g12, g13, w, nll, grad, nullptr, nullptr,
+                    nullptr, nullptr);
 }
 
 // ---- O10: test access to the shape derivatives of one resonance term: out = (Re, Im dT/dm0, Re, Im dT/dGamma0) ----
@@ -576,10 +597,11 @@ void orc_resonance_term_dshape(const orc_kin* k, const orc_res* r, double x, dou
 //   dA/dtheta = c_r [dT_r(s12,s13)/dtheta + dT_r(s13,s12)/dtheta]
 //   dNLL/dtheta = -2 sum_i Re(conj(A_i) dA_i) / |A_i|^2 + (2 n_ev / I) sum_j w_j Re(conj(A_j) dA_j)
 // grad_shape has 2F entries: (d/dmass, d/dwidth) per floating resonance.
-void orc_nll_grad_shape(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res,
-                        const double* params, int64_t n_ev, const double* e12, const double* e13,
-                        int64_t n_norm, const double* g12, const double* g13, const double* w,
-                        double* nll, double* grad_shape)
+// Optional pieces as in O9b: shape_ev = d(-S)/dtheta, shape_nm = dI/dtheta (2F entries each).
+static void nll_grad_shape_impl(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res,
+                                const double* params, int64_t n_ev, const double* e12, const double* e13,
+                                int64_t n_norm, const double* g12, const double* g13, const double* w,
+                                double* nll, double* grad_shape, double* shape_ev, double* shape_nm)
 {
     const Model m = make_model(kin, n, knots, R, res);
     const Unpacked u = unpack(m, params);
@@ -613,8 +635,35 @@ void orc_nll_grad_shape(const orc_kin* kin, int n, const double* knots, int R, c
     }
     const long double Iv = I.value();
     *nll = (double)(-S.value() + (long double)n_ev * logl(Iv));
-    for (int t = 0; t < 2 * F; ++t)
-        grad_shape[t] = (double)(-2.0L * ev[t].value() + 2.0L * (long double)n_ev / Iv * nm[t].value());
+    for (int t = 0; t < 2 * F; ++t) {
+        if (grad_shape) grad_shape[t] = (double)(-2.0L * ev[t].value() + 2.0L * (long double)n_ev / Iv * nm[t].value());
+        if (shape_ev) shape_ev[t] = (double)(-2.0L * ev[t].value());
+        if (shape_nm) shape_nm[t] = (double)(2.0L * nm[t].value());
+    }
+}
+
+void orc_nll_grad_shape(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res,
+                        const double* params, int64_t n_ev, const double* e12, const double* e13,
+                        int64_t n_norm, const double* g12, const double* g13, const double* w,
+                        double* nll, double* grad_shape)
+{
+    nll_grad_shape_impl(kin, n, knots, R, res, params, n_ev, e12, e13, n_norm, g12, g13, w, nll, grad_shape, nullptr,
+                        nullptr);
+}
+
+// ---- O9b: the pieces one rank of a sharded likelihood contributes: S = sum_i ln|A_i|^2, I, and
+// grad_ev = d(-S)/dtheta, grad_nm = dI/dtheta over ALL parameters (2N + 2R linear ones, then (mass, width) of every
+// floating resonance), so that NLL = -sum_r S_r + n ln(sum_r I_r) and grad = sum_r grad_ev_r + (n / I) sum_r grad_nm_r.
+void orc_nll_grad_parts(const orc_kin* kin, int n, const double* knots, int R, const orc_res* res, const double* params,
+                        int64_t n_ev, const double* e12, const double* e13,
+                        int64_t n_norm, const double* g12, const double* g13, const double* w,
+                        double* sum_log, double* integral, double* grad_ev, double* grad_nm)
+{
+    double nll;
+    nll_grad_linear(kin, n, knots, R, res, params, n_ev, e12, e13, n_norm, g12, g13, w, &nll, nullptr, sum_log, integral,
+                    grad_ev, grad_nm);
+    nll_grad_shape_impl(kin, n, knots, R, res, params, n_ev, e12, e13, n_norm, g12, g13, w, &nll, nullptr,
+                        grad_ev + 2 * n + 2 * R, grad_nm + 2 * n + 2 * R);
 }
 
 // ---- O11 (not in the paper): Hessian of the NLL in the 2N + 2R linear-coefficient parameters, for

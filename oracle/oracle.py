@@ -75,6 +75,8 @@ def lib():
         L.orc_nll_grad_shape.restype = None
         L.orc_nll_grad_shape.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp]
         L.orc_resonance_term_dshape.restype = None; L.orc_resonance_term_dshape.argtypes = [kp, rp, d, d, _dp]
+        L.orc_nll_grad_parts.restype = None
+        L.orc_nll_grad_parts.argtypes = model + [_dp, i64, _dp, _dp, i64, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -182,6 +184,18 @@ class Oracle:
         self.L.orc_nll_grad_shape(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w),
                                   C.byref(nll), _p(grad))
         return nll.value, grad[:2 * F]
+
+    def nll_grad_parts(self, params, e12, e13, g12, g13, w=None):
+        """(S = sum ln|A|^2, I, d(-S)/dtheta, dI/dtheta) over all parameters, floating shapes last  -- O9b"""
+        p, e12, e13, g12, g13 = self._params(params), _a(e12), _a(e13), _a(g12), _a(g13)
+        w = None if w is None else _a(w)
+        S, Iv = C.c_double(), C.c_double()
+        F = sum(1 for r in self.resonances if r.get("shape_floats"))
+        P = 2 * self.n + 2 * self.R + 2 * F
+        gev, gnm = np.zeros(P + 1), np.zeros(P + 1)
+        self.L.orc_nll_grad_parts(*self._model, _p(p), e12.size, _p(e12), _p(e13), g12.size, _p(g12), _p(g13), _p(w),
+                                  C.byref(S), C.byref(Iv), _p(gev), _p(gnm))
+        return S.value, Iv.value, gev[:P], gnm[:P]
 
     def resonance_term_dshape(self, r, x, y):
         """(dT/dm0, dT/dGamma0) of one resonance dict r at (x, y)  -- O10"""

@@ -117,3 +117,42 @@ def test_hessian_matches_differences_of_the_pinned_gradient_and_the_invariance_i
             return o.nll_grad(q, e12, e13, g12, g13, w)[1]
         col = _richardson(grad_at, p[a], 1e-5)             # 1e-4 still leaves 5e-7 of truncation error (narrow rho)
         assert np.max(np.abs(col - H[a])) <= 1e-9 * scale
+
+
+def test_gradient_parts_match_differences_of_the_two_sums_and_recombine():
+    """O9b: the per-rank pieces grad_ev = d(-S)/dtheta and grad_nm = dI/dtheta against Richardson
+    differences of S = sum ln|A|^2 and I as orc_nll returns them (pinned on their own), over every kind of parameter
+    (knot magnitude and phase, resonance magnitude and phase, floating mass and width); grad_ev + (n/I) grad_nm must
+    be the pinned gradients of O9 and O10; an empty event set leaves grad_ev = 0."""
+    kin = KIN_KPIPI
+    lo, hi = I.s_limits(kin)
+    res = [dict(mass=0.8955, width=0.047, spin=1, r_res=1.5, r_parent=5.0, shape_floats=1),
+           dict(mass=1.2, width=0.2, spin=0, r_res=1.5, r_parent=5.0, shape_floats=0),
+           dict(mass=1.4324, width=0.109, spin=2, r_res=2.0, r_parent=4.0, shape_floats=1)]
+    knots = np.linspace(lo - 1e-3, hi + 1e-3, 9)
+    o = orc.Oracle(kin, knots, res)
+    s12, s13 = I.phase_space_points(2500, I.stream_key(3, 13, 1), kin)
+    rng = np.random.default_rng(5)
+    e12, e13, g12, g13 = s12[:900], s13[:900], s12[900:], s13[900:]
+    w = rng.uniform(0.5, 1.5, g12.size) / g12.size
+    p = np.concatenate([rng.uniform(0.5, 2, 9), rng.uniform(0, 3, 9), rng.uniform(0.3, 1.5, 6),
+                        [0.8955, 0.047, 1.4324, 0.109]])
+    S, Iv, gev, gnm = o.nll_grad_parts(p, e12, e13, g12, g13, w)
+    nll, S0, I0 = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    assert S == pytest.approx(S0, rel=1e-14) and Iv == pytest.approx(I0, rel=1e-14)
+    assert gev.size == gnm.size == p.size == 28
+    _, g_lin = o.nll_grad(p, e12, e13, g12, g13, w)
+    _, g_shape = o.nll_grad_shape(p, e12, e13, g12, g13, w)
+    total = gev + (e12.size / Iv) * gnm
+    ref = np.concatenate([g_lin, g_shape])
+    assert np.max(np.abs(total - ref)) <= 1e-13 * np.max(np.abs(ref))
+    for idx in (0, 4, 8, 9, 13, 17, 18, 19, 22, 23, 24, 25, 26, 27):
+        def parts_at(v):
+            q = p.copy(); q[idx] = v
+            _, s_, i_ = o.nll(q, e12, e13, g12, g13, w, parts=True)
+            return np.array([-s_, i_])
+        fd = _richardson(parts_at, p[idx], 1e-4)
+        assert gev[idx] == pytest.approx(fd[0], rel=5e-6, abs=1e-7 * np.max(np.abs(gev)))
+        assert gnm[idx] == pytest.approx(fd[1], rel=5e-6, abs=1e-7 * np.max(np.abs(gnm)))
+    _, _, gev0, gnm0 = o.nll_grad_parts(p, e12[:0], e13[:0], g12, g13, w)
+    assert not gev0.any() and np.array_equal(gnm0, gnm)
