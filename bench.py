@@ -272,6 +272,21 @@ def run_ours(args, cfg, workload):
                          "d_mass_d_width": [float(x) for x in grad_f[grad.size:]],
                          "what": "mipwa_nll_grad_full: the above + d/d(mass, width) of every floating resonance"}
 
+    # the sharded form of the same call: per-rank pieces, one all_gather of 3 + 2 n_params doubles, combine
+    for t in range(2):
+        m.nll_grad_parts(params[t])
+    barrier()
+    t0 = time.perf_counter()
+    for t in range(sub_steps):
+        S_p, I_p, g_ev, g_nm = m.nll_grad_parts(params[args.warmup + t % args.steps])
+        nll_s, grad_s = sharding.combine_grad_parts(S_p, I_p, n_ev, g_ev, g_nm, device=dev)[:2]
+    barrier()
+    sh_wall = (time.perf_counter() - t0) / sub_steps
+    grad_info["sharded"] = {"ms_per_call": 1e3 * sh_wall, "events_per_s": n_ev * world / sh_wall, "n_grad": int(grad_s.size),
+                            "nll": nll_s, "max_abs_diff_vs_full_at_1gpu": (float(np.max(np.abs(grad_s - grad_f))) if world == 1 else None),
+                            "what": "mipwa_nll_grad_parts + sharding.combine_grad_parts: whole-job NLL and all n_params "
+                                    "derivatives from per-rank (S, I, d(-S), dI); 3 + 2 n_params doubles all-gathered per call"}
+
     # ---- signal + background mixture (purity 90 %): flat background density, two launches per call ----------
     m.set_event_background(torch.full((n_ev,), 1.0 / I.dalitz_area(cfg.kin), dtype=torch.float64, device=dev))
     for t in range(3):

@@ -146,6 +146,18 @@ int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, doubl
  * identical to mipwa_nll_grad when none does.  Errors as mipwa_nll_grad. */
 int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
+/* The pieces ONE RANK of a sharded likelihood contributes (events and normalisation points are
+ * independent units, so rank g holds a slice of each, with normalisation weights of the WHOLE sample):
+ *     *sum_log = S = sum_i ln|A_i|^2,   *integral = I = sum_j w_j |A_j|^2,
+ *     grad_ev = d(-S)/dtheta,           grad_nm = dI/dtheta,
+ * over all n_params parameters in the layout of mipwa_nll_grad_full.  Summed over the ranks (S, I, n_ev and both
+ * vectors: 3 + 2 n_params doubles per rank and call),
+ *     NLL = -S + n_ev ln I,             dNLL/dtheta = grad_ev + (n_ev / I) grad_nm.
+ * A per-rank mipwa_nll_grad cannot be combined that way: it already holds its own rank's n_ev / I.
+ * grad_ev, grad_nm: HOST, n_params doubles each.  Same launches, paths and errors as mipwa_nll_grad_full. */
+int mipwa_nll_grad_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, double* sum_log, double* integral,
+                         double* grad_ev, double* grad_nm);
+
 /* Signal + background mixture ("signal purity 90 %"): per event the PDF is
  *     f_s |A_i|^2 / I + (1 - f_s) b_i ,      NLL = - sum_i ln( f_s |A_i|^2 / I + (1 - f_s) b_i ),
  * with b_i the background density at event i (normalised over the Dalitz plot, supplied by the caller) and f_s the

@@ -23,7 +23,7 @@ _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STAT
 # every symbol include/mipwa.h declares
 SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_events", "mipwa_set_norm_points",
            "mipwa_prepare", "mipwa_n_params", "mipwa_set_path", "mipwa_basis_bytes", "mipwa_set_basis_buffer", "mipwa_nll",
-           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_nll_hessian", "mipwa_set_event_background", "mipwa_nll_mix",
+           "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_nll_grad_parts", "mipwa_nll_hessian", "mipwa_set_event_background", "mipwa_nll_mix",
            "mipwa_nll_mix_grad", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version"]
@@ -73,6 +73,7 @@ def load_library():
     L.mipwa_nll_parts.restype = i32; L.mipwa_nll_parts.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_nll_grad.restype = i32; L.mipwa_nll_grad.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_nll_grad_full.restype = i32; L.mipwa_nll_grad_full.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_nll_grad_parts.restype = i32; L.mipwa_nll_grad_parts.argtypes = [vp, _dp, i64, _dp, _dp, _dp, _dp]
     L.mipwa_nll_hessian.restype = i32; L.mipwa_nll_hessian.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_set_event_background.restype = i32; L.mipwa_set_event_background.argtypes = [vp, vp, i32]
     L.mipwa_nll_mix.restype = i32; L.mipwa_nll_mix.argtypes = [vp, _dp, i64, C.c_double, _dp]
@@ -235,6 +236,15 @@ class Mipwa:
         grad = np.empty(p.size)
         self._check(self.L.mipwa_nll_grad_full(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp)))
         return out.value, grad
+
+    def nll_grad_parts(self, params):
+        """one rank's pieces of a sharded likelihood: (sum ln|A|^2, I, d(-sum ln|A|^2)/dtheta, dI/dtheta)"""
+        p, pp, n = self._params(params)
+        S, Iv = C.c_double(), C.c_double()
+        gev, gnm = np.empty(p.size), np.empty(p.size)
+        self._check(self.L.mipwa_nll_grad_parts(self._h, pp, n, C.byref(S), C.byref(Iv), gev.ctypes.data_as(_dp),
+                                                gnm.ctypes.data_as(_dp)))
+        return S.value, Iv.value, gev, gnm
 
     def set_event_background(self, b):
         """background density per event (numpy: copied; CUDA torch tensor: borrowed), in the order of set_events"""

@@ -45,6 +45,8 @@ struct mipwa_ctx {
     int n_spin[3] = { 0, 0, 0 };   // resonances of spin 0, 1, 2 (the kernel signature)
     int model_flags = 0;           // MIPWA_FL_*: equal daughter masses m1 == m2; radii shared within each spin
     std::vector<int> perm;          // device slot d holds resonance perm[d]: spin 1 first, then spin 2, then spin 0
+    double *parts_ev = nullptr, *parts_nm = nullptr;   // mipwa_nll_grad_parts: host outputs of the running call
+    double parts_S = 0.0, parts_I = 0.0;
     int device = 0;
     int sm_count = 0;
     cudaStream_t stream = nullptr;
@@ -1150,6 +1152,15 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
         Gr[2 * r + 1] = h[1 + 2 * r + 1] + scale * gc[2 * (N + r) + 1];
     }
     polar_chain(c, params, Gy.data(), Gr.data(), grad);
+    if (c->parts_ev) {                                     // mipwa_nll_grad_parts: d(-S)/dtheta and dI/dtheta = 2 G c apart
+        spline_adjoint(c, h + 1 + 2 * R, Gy.data());
+        for (int r = 0; r < R; ++r) { Gr[2 * r] = h[1 + 2 * r]; Gr[2 * r + 1] = h[1 + 2 * r + 1]; }
+        polar_chain(c, params, Gy.data(), Gr.data(), c->parts_ev);
+        for (int k = 0; k < 2 * N; ++k) Gy[k] = 2.0 * gc[k];
+        for (int r = 0; r < 2 * R; ++r) Gr[r] = 2.0 * gc[2 * N + r];
+        polar_chain(c, params, Gy.data(), Gr.data(), c->parts_nm);
+        c->parts_S = S; c->parts_I = I;
+    }
     return MIPWA_OK;
 }
 
@@ -1209,14 +1220,22 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
     const double* Be = h + 2 + 4 * R;
     const double* Bn = Be + nb;
     std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * R);
-    for (int k = 0; k < nb; ++k) Gsc[k] = Be[k] + scale * Bn[k];
-    spline_adjoint(c, Gsc.data(), Gy.data());
-    for (int d = 0; d < R; ++d) {
-        const int r = c->perm[d];
-        Gr[2 * r] = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
-        Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
+    auto emit = [&](double se, double sn, double* out) {   // out = se * (event part) + sn * (normalisation part)
+        for (int k = 0; k < nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
+        spline_adjoint(c, Gsc.data(), Gy.data());
+        for (int d = 0; d < R; ++d) {
+            const int r = c->perm[d];
+            Gr[2 * r] = c->res_fold[d] * (se * Fe[2 * d] + sn * Fn[2 * d]);
+            Gr[2 * r + 1] = c->res_fold[d] * (se * Fe[2 * d + 1] + sn * Fn[2 * d + 1]);
+        }
+        polar_chain(c, params, Gy.data(), Gr.data(), out);
+    };
+    emit(1.0, scale, grad);
+    if (c->parts_ev) {                                     // mipwa_nll_grad_parts: d(-S)/dtheta and dI/dtheta apart
+        emit(1.0, 0.0, c->parts_ev);
+        emit(0.0, 2.0 * wn, c->parts_nm);
+        c->parts_S = S; c->parts_I = I;
     }
-    polar_chain(c, params, Gy.data(), Gr.data(), grad);
     return MIPWA_OK;
 }
 
@@ -1305,10 +1324,32 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
             for (int t = 0; t < 2; ++t) {                  // t = 0: mass, 1: width
                 const double dr = e[2 * t] + scale * g[2 * t], di = e[2 * t + 1] + scale * g[2 * t + 1];
                 grad[2 * N + 2 * R + 2 * (f0 + q) + t] = rd.cre * dr + rd.cim * di;   // Re(conj(c sqrt(n_R n_D)) D)
+                if (c->parts_ev) {
+                    c->parts_ev[2 * N + 2 * R + 2 * (f0 + q) + t] = rd.cre * e[2 * t] + rd.cim * e[2 * t + 1];
+                    c->parts_nm[2 * N + 2 * R + 2 * (f0 + q) + t] = 2.0 * wn * (rd.cre * g[2 * t] + rd.cim * g[2 * t + 1]);
+                }
             }
         }
     }
     c->last_ms = ms_total;
+    return MIPWA_OK;
+}
+
+// the pieces one rank of a sharded likelihood contributes (include/mipwa.h): same launches as
+// mipwa_nll_grad_full, the host combine run once more per piece
+int mipwa_nll_grad_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* sum_log, double* integral,
+                         double* grad_ev, double* grad_nm)
+{
+    if (!c) return MIPWA_ERR_ARG;
+    if (!params || !sum_log || !integral || !grad_ev || !grad_nm) return fail(c, MIPWA_ERR_ARG, "null argument");
+    if (n_params != 2 * c->N + 2 * c->R + 2 * c->F) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
+    std::vector<double> total((size_t)std::max<int64_t>(n_params, 1));
+    double nll = 0.0;
+    c->parts_ev = grad_ev; c->parts_nm = grad_nm;
+    const int rc = mipwa_nll_grad_full(c, params, n_params, &nll, total.data());
+    c->parts_ev = c->parts_nm = nullptr;
+    if (rc) return rc;
+    *sum_log = c->parts_S; *integral = c->parts_I;
     return MIPWA_OK;
 }
 
@@ -1445,14 +1486,22 @@ int mipwa_nll_mix_grad(mipwa_ctx* c, const double* params, int64_t n_params, dou
     const double scale = 2.0 * (n_ev - kappa * Q) / I * wn;
     const double *Fe = h2.data() + 2, *Fn = h1.data() + 2 + 2 * R, *Be = h2.data() + 2 + 4 * R, *Bn = h1.data() + 2 + 4 * R + nb;
     std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * R);
-    for (int k = 0; k < nb; ++k) Gsc[k] = Be[k] + scale * Bn[k];
-    spline_adjoint(c, Gsc.data(), Gy.data());
-    for (int d = 0; d < R; ++d) {
-        const int r = c->perm[d];
-        Gr[2 * r] = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
-        Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
+    auto emit = [&](double se, double sn, double* out) {   // out = se * (event part) + sn * (normalisation part)
+        for (int k = 0; k < nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
+        spline_adjoint(c, Gsc.data(), Gy.data());
+        for (int d = 0; d < R; ++d) {
+            const int r = c->perm[d];
+            Gr[2 * r] = c->res_fold[d] * (se * Fe[2 * d] + sn * Fn[2 * d]);
+            Gr[2 * r + 1] = c->res_fold[d] * (se * Fe[2 * d + 1] + sn * Fn[2 * d + 1]);
+        }
+        polar_chain(c, params, Gy.data(), Gr.data(), out);
+    };
+    emit(1.0, scale, grad);
+    if (c->parts_ev) {                                     // mipwa_nll_grad_parts: d(-S)/dtheta and dI/dtheta apart
+        emit(1.0, 0.0, c->parts_ev);
+        emit(0.0, 2.0 * wn, c->parts_nm);
+        c->parts_S = S; c->parts_I = I;
     }
-    polar_chain(c, params, Gy.data(), Gr.data(), grad);
     return MIPWA_OK;
 }
 

@@ -67,3 +67,56 @@ def test_two_rank_combine_matches_single_process():
 def test_combine_without_process_group_is_step_a7():
     nll, S, Iv, n = sharding.combine_parts(12.5, 3.0, 7)
     assert (S, Iv, n) == (12.5, 3.0, 7) and nll == -12.5 + 7 * np.log(3.0)
+
+
+def _grad_worker(rank, world, port, q):
+    import torch.distributed as dist
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    c = I.Config(3, n_ev=1501, n_norm=2001)            # rho(770) floats: 108 parameters, shape derivatives included
+    o = orc.Oracle(c.kin, c.knots, c.resonances)
+    g12, g13, w = c.norm_points()
+    e12, e13 = I.phase_space_points(c.n_ev, c.key(I.S_EVENTS))
+    p = c.perturbed(2)
+    lo, hi = sharding.shard_range(c.n_ev, rank, world)
+    glo, ghi = sharding.shard_range(g12.size, rank, world)
+    S, Iv, gev, gnm = o.nll_grad_parts(p, e12[lo:hi], e13[lo:hi], g12[glo:ghi], g13[glo:ghi], w[glo:ghi])
+    nll, grad, St, It, nt = sharding.combine_grad_parts(S, Iv, hi - lo, gev, gnm)
+    ref_nll, g_lin = o.nll_grad(p, e12, e13, g12, g13, w)
+    _, g_shape = o.nll_grad_shape(p, e12, e13, g12, g13, w)
+    q.put((rank, nll, grad, nt, ref_nll, np.concatenate([g_lin, g_shape])))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_gradient_combine_matches_single_process():
+    """grad = sum_r grad_ev_r + (n / I) sum_r grad_nm_r against the oracle's whole-sample gradient (O9 + O10)."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_grad_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = [q.get(timeout=240) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    grads = []
+    for rank, nll, grad, nt, ref_nll, ref_grad in out:
+        assert nt == 1501 and grad.size == 108
+        assert abs(nll - ref_nll) <= 1e-10 * max(abs(ref_nll), 1.0) * 50
+        assert np.max(np.abs(grad - ref_grad)) <= 1e-11 * np.max(np.abs(ref_grad))
+        grads.append(grad)
+    assert np.array_equal(grads[0], grads[1])          # every rank forms the same bits
+
+
+def test_gradient_combine_without_process_group():
+    ge, gn = np.array([1.0, -2.0]), np.array([0.5, 4.0])
+    nll, g, S, Iv, n = sharding.combine_grad_parts(12.5, 3.0, 7, ge, gn)
+    assert nll == -12.5 + 7 * np.log(3.0) and np.array_equal(g, ge + (7 / 3.0) * gn) and n == 7
+    assert sharding.combine_grad_parts(0.0, 3.0, 0, ge, gn)[0] == 0.0
