@@ -6,7 +6,7 @@
 bool mipwa_hybrid_supported(int f1, int f2, int rc)
 {
     bool supported = true;
-    MIPWA_DISPATCH_HYB(f1, f2, rc, (void)0);
+    MIPWA_DISPATCH_HYB(f1, f2, rc, ((void)R1, (void)R2, (void)RCT));
     return supported;
 }
 
