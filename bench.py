@@ -442,7 +442,7 @@ def run_ours(args, cfg, workload):
 
 # ---- secondary measurements behind the numbers in BASELINE.md / profiles (not the driver's bench line) --------------
 def run_probe(args):
-    """--probe resonances | recompute-shape | grid-bias | sweep4 | latency : prints one JSON line per row (kernel times: CUDA events in the library,
+    """--probe resonances | hybrid | recompute-shape | grid-bias | sweep4 | latency : prints one JSON line per row (kernel times: CUDA events in the library,
     median over the calls after warm-up).  Phase-space points stand in for events where only the work per point
     matters; every mode cross-checks its NLL against another path."""
     import torch
@@ -475,6 +475,29 @@ def run_probe(args):
             k, v = timed(m, p)
             print(json.dumps({"probe": "resonances", "model": name, "points": 2 * n, "kernel_ms": k, "nll": v,
                               "clk_per_warp_point_per_smsp_at_1965MHz": k * 1e-3 * 1.965e9 * 592 / (2 * n / 32)}), flush=True)
+            m.close()
+    elif args.probe == "hybrid":
+        # the rule behind MIPWA_PATH_AUTO when some shapes float: rho(770) floating + k fixed-shape resonances,
+        # full recompute against the hybrid path (fixed terms streamed from the per-point cache), 10 M + 10 M points
+        c = I.Config(3)
+        n = args.events or 10_000_000
+        e12, e13 = I.phase_space_points(n, c.key(7)); g12, g13 = I.phase_space_points(n, c.key(8))
+        d = [torch.from_numpy(a).cuda() for a in (e12, e13, g12, g13)]
+        fixed = [I._res(*I.RHO1450), I._res(*I.F2_1270), I._res(*I.SYN_A), I._res(*I.SYN_B), I._res(*I.SYN_C)]
+        for k in range(1, 6):
+            res = [I._res(*I.RHO770, shape_floats=1)] + fixed[:k]
+            m = B.Mipwa(c.kin, c.knots, res)
+            m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], None)
+            m.prepare(); m.enable_timing(True)
+            p = np.concatenate([c.truth[:100], np.tile([1.0, 0.3], len(res)), [0.775, 0.149]])
+            row = {"probe": "hybrid", "fixed": k, "spins": [r["spin"] for r in res], "points": 2 * n}
+            for name, path in (("recompute", B.PATH_RECOMPUTE), ("hybrid", B.PATH_HYBRID), ("auto", B.PATH_AUTO)):
+                try:
+                    m.set_path(path)
+                    row[name + "_ms"], row[name + "_nll"] = timed(m, p)
+                except B.MipwaError as e:
+                    row[name + "_ms"] = None
+            print(json.dumps(row), flush=True)
             m.close()
     elif args.probe == "recompute-shape":
         # kernel time of k_nll_recompute (value) and k_grad_recompute at configs[3]'s model on 10 M + 10 M weighted,
@@ -633,7 +656,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--events", type=int, default=None)
     ap.add_argument("--norm-points", type=int, default=None)
-    ap.add_argument("--probe", default=None, choices=["resonances", "recompute-shape", "grid-bias", "sweep4", "latency"])
+    ap.add_argument("--probe", default=None, choices=["resonances", "hybrid", "recompute-shape", "grid-bias", "sweep4", "latency"])
     args = ap.parse_args()
     if args.probe:
         return run_probe(args)

@@ -30,70 +30,151 @@ __device__ __forceinline__ double hybrid_abs2(const SplineCoefSmem& sm, const De
     return fma(re, re, im * im);
 }
 
-// One launch over [events | normalisation points]; one point per thread and tile, the next tile's columns are
-// loaded before the current tile is evaluated.  result[0] = sum ln|A|^2, result[1] = sum w |A|^2 (w == NULL: weight 1).
-// eseg / gseg: the stored segment pairs of the same (cell-sorted or caller's) point order the caches were built in.
+// ---- staging ring ------------------------------------------------------------------------------------------------------
+// At 16 + 16 RC bytes per point this kernel needs 3-6 TB/s while the FP64 pipe is busy with the floating terms, and a
+// register prefetch one tile ahead keeps only ~17 KB per SM in flight (measured: 2.8 TB/s, latency bound, slower than
+// the full recompute at RC = 1).  The cache columns therefore go through a shared-memory ring filled by per-thread
+// 16-byte cp.async copies MIPWA_HYB_STAGES - 1 tiles ahead: every thread copies exactly the slots it later reads, so
+// cp.async.wait_group is the only synchronisation (no barrier, no mbarrier), the data in flight cost no registers,
+// and (STAGES - 1) x 512 threads x 16 (1 + RC) B = 50-110 KB per SM are on their way at any time.
+// threads per block (a multiple of the 256-point cache tile), resident blocks per SM, and points per thread and
+// iteration: a block takes MIPWA_HYB_PTS * MIPWA_HYB_BLOCK / MIPWA_TILE tiles per iteration.  One floating resonance is
+// a single dependent chain of ~100 FP64 instructions per point; with four warps per scheduler that does not fill the
+// pipe (k_nll_recompute with one resonance: 0.19 ms where the instruction count says 0.14), so two independent points
+// are evaluated side by side.
+#ifndef MIPWA_HYB_BLOCK
+#define MIPWA_HYB_BLOCK 512
+#endif
+#ifndef MIPWA_HYB_MINBLOCKS
+#define MIPWA_HYB_MINBLOCKS 1
+#endif
+// points per thread and iteration: two while the ring still gets >= 3 stages (RC <= 3), else one
+#ifndef MIPWA_HYB_PTS
+#define MIPWA_HYB_PTS(rct) ((rct) <= 3 ? 2 : 1)
+#endif
+// ring stages: as many as fit 200 KB of shared memory, at most 4, at least 2
+__host__ __device__ constexpr int mipwa_hyb_stages(int rct)
+{
+    const size_t per_stage = (size_t)MIPWA_HYB_PTS(rct) * (1 + rct) * MIPWA_HYB_BLOCK * sizeof(double2);
+    const size_t fit = (size_t)200 * 1024 / per_stage;
+    return fit >= 4 ? 4 : (fit >= 2 ? (int)fit : 2);
+}
+#define MIPWA_HYB_STAGES(rct) mipwa_hyb_stages(rct)
+__host__ __device__ constexpr size_t mipwa_hyb_ring_bytes(int rct)
+{
+    return (size_t)mipwa_hyb_stages(rct) * MIPWA_HYB_PTS(rct) * (1 + rct) * MIPWA_HYB_BLOCK * sizeof(double2);
+}
+
+__device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsrc)
+{
+    const unsigned int sa = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
+
+// One launch over [events | normalisation points]; one point per thread and tile.  result[0] = sum ln|A|^2,
+// result[1] = sum w |A|^2 (w == NULL: weight 1).
+// eseg / gseg: the stored segment pairs of the same (cell-sorted or caller's) point order the caches were built in;
+// they and the weights (2 + 8 B per point) are prefetched through registers, as far ahead as the ring.
+// Dynamic shared memory: mipwa_hyb_ring_bytes(RCT).
 template <int R1, int R2, int RCT, int FL>
-__global__ void __launch_bounds__(MIPWA_TILE, 2)
+__global__ void __launch_bounds__(MIPWA_HYB_BLOCK, MIPWA_HYB_MINBLOCKS)
 k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef cc,
              const double2* __restrict__ ev_cache, const unsigned short* __restrict__ eseg, long long n_ev,
              const double2* __restrict__ nm_cache, const double* __restrict__ gw,
              const unsigned short* __restrict__ gseg, long long n_norm,
              double2* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result)
 {
+    extern __shared__ __align__(16) unsigned char hyb_ring_raw[];
     __shared__ SplineCoefSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
     load_spline_coef_smem(sm, m);
-    constexpr int C = 1 + RCT;
+    constexpr int C = 1 + RCT, ST = MIPWA_HYB_STAGES(RCT), AHEAD = ST - 1, PTS = MIPWA_HYB_PTS(RCT);
+    constexpr int TPB = MIPWA_HYB_BLOCK / MIPWA_TILE;                                  // tiles per block and point slot
+    constexpr int STAGE = PTS * C * MIPWA_HYB_BLOCK;                                   // double2 per ring stage
+    // slot (stage, point u, column k) of this thread: ring[stage * STAGE + (u * C + k) * BLOCK]
+    double2* const ring = reinterpret_cast<double2*>(hyb_ring_raw) + threadIdx.x;
+    const int sub = threadIdx.x / MIPWA_TILE, lane_t = threadIdx.x % MIPWA_TILE;       // this thread's tile of the TPB, slot in it
+    const int G = (int)gridDim.x * TPB * PTS;                                          // tiles per grid iteration
     LogProd lp;
     double integ = 0.0;
+    // The FP64 pipe and the other instructions share the scheduler's issue slots (profiles/r1_k_nll_hybrid_ncu.md), so the
+    // bookkeeping is kept to 32-bit tile counters, one compare per point and pointers advanced by a constant.
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
         const double2* cache = pass == 0 ? ev_cache : nm_cache;
         const unsigned short* segs = pass == 0 ? eseg : gseg;
         const long long n = pass == 0 ? n_ev : n_norm;
-        const long long n_tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
-        double2 s = make_double2(1.0, 1.0), b[RCT];
-        double w = 0.0;
-        unsigned int sg = 0u;
+        const bool has_w = pass == 1 && gw != nullptr;
+        const int n_tiles = (int)((n + MIPWA_TILE - 1) / MIPWA_TILE);
+        // this thread's slot of tile t holds a point iff t < lim (the last tile may be partly filled)
+        const int lim = (int)(n / MIPWA_TILE) + (lane_t < (int)(n % MIPWA_TILE) ? 1 : 0);
+        int tile = (int)blockIdx.x * TPB * PTS + sub;       // point u of this thread: tile + u * TPB
+        // cursors of the next tile to fetch (AHEAD iterations ahead of `tile`)
+        int ft = tile;
+        const double2* fc = cache + (size_t)tile * C * MIPWA_TILE + lane_t;
+        const unsigned short* fs = segs + (size_t)tile * MIPWA_TILE + lane_t;
+        const double* fw = gw + (size_t)tile * MIPWA_TILE + lane_t;
+        const size_t dcache = (size_t)G * C * MIPWA_TILE, dpts = (size_t)G * MIPWA_TILE;
+        int wr = 0, rd = 0;                                   // ring offsets (double2) of the stage to fill / to read
+        // one commit group per iteration (empty past the end, so that the group count stays uniform)
+        auto fetch = [&](unsigned int (&sg)[PTS], double (&w)[PTS]) {
 #pragma unroll
-        for (int k = 0; k < RCT; ++k) b[k] = make_double2(0.0, 0.0);
-        long long tile = blockIdx.x;
-        if (tile < n_tiles) {
-            const double2* p = cache + (size_t)tile * C * MIPWA_TILE + threadIdx.x;
-            s = ld_stream(p);
+            for (int u = 0; u < PTS; ++u) {
+                if (ft + u * TPB < n_tiles) {
 #pragma unroll
-            for (int k = 0; k < RCT; ++k) b[k] = ld_stream(p + (size_t)(1 + k) * MIPWA_TILE);
-            const long long i = tile * MIPWA_TILE + threadIdx.x;
-            if (pass == 1) w = i < n ? (gw ? gw[i] : 1.0) : 0.0;
-            if (i < n) sg = segs[i];
-        }
-        for (; tile < n_tiles; tile += gridDim.x) {
-            double2 ns = make_double2(1.0, 1.0), nb[RCT];
-            double nw = 0.0;
-            unsigned int nsg = 0u;
-#pragma unroll
-            for (int k = 0; k < RCT; ++k) nb[k] = make_double2(0.0, 0.0);
-            const long long nt = tile + gridDim.x;
-            if (nt < n_tiles) {
-                const double2* p = cache + (size_t)nt * C * MIPWA_TILE + threadIdx.x;
-                ns = ld_stream(p);
-#pragma unroll
-                for (int k = 0; k < RCT; ++k) nb[k] = ld_stream(p + (size_t)(1 + k) * MIPWA_TILE);
-                const long long i = nt * MIPWA_TILE + threadIdx.x;
-                if (pass == 1) nw = i < n ? (gw ? gw[i] : 1.0) : 0.0;
-                if (i < n) nsg = segs[i];
+                    for (int k = 0; k < C; ++k)
+                        cp_async16(ring + wr + (u * C + k) * MIPWA_HYB_BLOCK, fc + (size_t)(u * TPB * C + k) * MIPWA_TILE);
+                }
+                const bool in = ft + u * TPB < lim;
+                sg[u] = in ? fs[(size_t)u * TPB * MIPWA_TILE] : 0u;
+                w[u] = pass == 1 && in ? (has_w ? fw[(size_t)u * TPB * MIPWA_TILE] : 1.0) : 0.0;
             }
-            const bool live = tile * MIPWA_TILE + threadIdx.x < n;
-            // padding slots of the last tile hold (0, 0): evaluate a harmless point instead
-            const double v = hybrid_abs2<R1, R2, RCT, FL>(sm, m, cc, live ? s : make_double2(1.0, 1.0), live ? sg : 0u, b);
-            if (pass == 0) lp.add(live ? v : 1.0);
-            else integ = fma(w, v, integ);
-            s = ns; w = nw; sg = nsg;
+            cp_async_commit();
+            ft += G; fc += dcache; fs += dpts; fw += dpts;
+            wr = wr + STAGE == ST * STAGE ? 0 : wr + STAGE;
+        };
+        unsigned int sgq[AHEAD][PTS];
+        double wq[AHEAD][PTS];
 #pragma unroll
-            for (int k = 0; k < RCT; ++k) b[k] = nb[k];
+        for (int q = 0; q < AHEAD; ++q) fetch(sgq[q], wq[q]);
+        for (; tile - sub < n_tiles; tile += G) {          // block-uniform trip count
+            unsigned int nsg[PTS];
+            double nw[PTS];
+            fetch(nsg, nw);
+            cp_async_wait<AHEAD>();                                        // this iteration's group has landed
+            double vv[PTS];
+            bool live[PTS];
+#pragma unroll
+            for (int u = 0; u < PTS; ++u) {
+                const double2* slot = ring + rd + u * C * MIPWA_HYB_BLOCK;
+                double2 b[RCT];
+                const double2 s = slot[0];
+#pragma unroll
+                for (int k = 0; k < RCT; ++k) b[k] = slot[(1 + k) * MIPWA_HYB_BLOCK];
+                live[u] = tile + u * TPB < lim;
+                // padding slots of the last tile hold (0, 0), slots of tiles past the end are stale: evaluate a
+                // harmless point instead and drop its value below
+                vv[u] = hybrid_abs2<R1, R2, RCT, FL>(sm, m, cc, live[u] ? s : make_double2(1.0, 1.0), sgq[0][u], b);
+            }
+#pragma unroll
+            for (int u = 0; u < PTS; ++u) {
+                if (pass == 0) lp.add(live[u] ? vv[u] : 1.0);
+                else integ = fma(wq[0][u], live[u] ? vv[u] : 0.0, integ);
+            }
+#pragma unroll
+            for (int q = 0; q + 1 < AHEAD; ++q) {
+#pragma unroll
+                for (int u = 0; u < PTS; ++u) { sgq[q][u] = sgq[q + 1][u]; wq[q][u] = wq[q + 1][u]; }
+            }
+#pragma unroll
+            for (int u = 0; u < PTS; ++u) { sgq[AHEAD - 1][u] = nsg[u]; wq[AHEAD - 1][u] = nw[u]; }
+            rd = rd + STAGE == ST * STAGE ? 0 : rd + STAGE;
         }
+        cp_async_wait<0>();                                                // nothing of this pass lands in the next pass's stages
     }
     double v[2] = { lp.value(), integ };
     block_reduce<2>(v, red);

@@ -44,6 +44,7 @@ cudaError_t mipwa_launch_grad_recompute_mix(const int* n_spin, int fl, int grid,
 
 // tu_hybrid.cu: k_nll_hybrid (hybrid.cuh); f1, f2 = floating resonances of spin 1, 2, rc = cached (fixed) resonances
 bool mipwa_hybrid_supported(int f1, int f2, int rc);
+int mipwa_hybrid_tiles_per_block(int rc);                  // 256-point cache tiles one block takes per iteration
 cudaError_t mipwa_occupancy_nll_hybrid(int f1, int f2, int rc, int fl, int* blocks_per_sm);
 cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cudaStream_t st, const DevModel& m,
                                     const HybCoef& cc, const double2* ev_cache, const unsigned short* eseg,

@@ -810,8 +810,9 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
         if (!supported) return fail(c, MIPWA_ERR_CUDA, "hybrid: occupancy query failed");
         if (c->hyb_blocks_per_sm < 1) c->hyb_blocks_per_sm = 1;
     }
+    const int64_t tpb = mipwa_hybrid_tiles_per_block(RC);
     const int64_t tiles = (std::max(c->ev.n, c->nm.n) + MIPWA_TILE - 1) / MIPWA_TILE;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->hyb_blocks_per_sm));
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((tiles + tpb - 1) / tpb, (int64_t)c->sm_count * c->hyb_blocks_per_sm));
     if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
     const cudaError_t le = mipwa_launch_nll_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, grid, c->stream, c->model, cc,
                                                    (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n,

@@ -3,6 +3,8 @@
 #include "kernels.cuh"
 #include "hybrid.cuh"
 
+int mipwa_hybrid_tiles_per_block(int rc) { return MIPWA_HYB_PTS(rc) * MIPWA_HYB_BLOCK / MIPWA_TILE; }
+
 bool mipwa_hybrid_supported(int f1, int f2, int rc)
 {
     bool supported = true;
@@ -15,8 +17,11 @@ cudaError_t mipwa_occupancy_nll_hybrid(int f1, int f2, int rc, int fl, int* bloc
     bool supported = true;
     cudaError_t e = cudaSuccess;
     MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl,
-                         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_nll_hybrid<R1, R2, RCT, FL>,
-                                                                           MIPWA_TILE, 0));
+                         e = cudaFuncSetAttribute(k_nll_hybrid<R1, R2, RCT, FL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                  (int)mipwa_hyb_ring_bytes(RCT));
+                         if (e == cudaSuccess)
+                             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_nll_hybrid<R1, R2, RCT, FL>,
+                                                                               MIPWA_HYB_BLOCK, mipwa_hyb_ring_bytes(RCT)));
     return supported ? e : cudaErrorInvalidValue;
 }
 
@@ -28,7 +33,7 @@ cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cu
 {
     bool supported = true;
     MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl,
-                         (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_TILE, 0, st>>>(
+                         (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_HYB_BLOCK, mipwa_hyb_ring_bytes(RCT), st>>>(
                              m, cc, ev_cache, eseg, n_ev, nm_cache, gw, gseg, n_norm, partials, ticket, result)));
     return supported ? cudaGetLastError() : cudaErrorInvalidValue;
 }

@@ -283,6 +283,41 @@ def test_hybrid_path_matches_oracle():
     m.close()
 
 
+@pytest.mark.parametrize("n_fixed", [1, 2, 3, 4, 5])
+def test_hybrid_ring_ragged_sizes(n_fixed):
+    """k_nll_hybrid stages its cache columns through a cp.async ring, 1024 (RC <= 3: two points per thread) or 512
+    points per block and iteration, two to four stages deep.  Sizes around the 256-point tile and the block iteration,
+    fewer points than one block, more iterations than stages, an empty event set, both kinematics (equal and unequal
+    daughter masses): NLL pieces against the oracle, and against the recompute kernel on the same context."""
+    B = _lib()
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import inputs as I
+    fixed = [I._res(*I.RHO1450), I._res(*I.F2_1270), I._res(*I.SYN_A), I._res(*I.SYN_B), I._res(*I.SYN_C)][:n_fixed]
+    for kin in (I.KIN, {"M": 1.86966, "m1": 0.493677, "m2": 0.13957, "m3": 0.13957}):
+        lo, hi = I.s_limits(kin)
+        knots = np.linspace(lo - 1e-3, hi + 1e-3, 12)
+        res = [I._res(*I.RHO770, shape_floats=1)] + fixed
+        o = orc.Oracle(kin, knots, res)
+        rng = np.random.default_rng(10 + n_fixed)
+        p = np.concatenate([rng.uniform(0.5, 2, 12), rng.uniform(0, 3, 12), rng.uniform(0.3, 1.5, 2 * len(res)),
+                            [0.78, 0.15]])
+        s12, s13 = I.phase_space_points(400_000, I.stream_key(5, 20 + n_fixed, 1), kin)
+        m = B.Mipwa(kin, knots, res)
+        for n_ev, n_norm in ((0, 1), (1, 255), (257, 256), (1023, 1025), (513, 2049), (3, 5000), (160_001, 239_999)):
+            e12, e13, g12, g13 = s12[:n_ev], s13[:n_ev], s12[n_ev:n_ev + n_norm], s13[n_ev:n_ev + n_norm]
+            w = rng.uniform(0.5, 1.5, n_norm) / n_norm
+            m.set_events(e12, e13); m.set_norm_points(g12, g13, w)
+            ref, sl, integ = o.nll(p, e12, e13, g12, g13, w, parts=True)
+            m.set_path(B.PATH_HYBRID)
+            got, gsl, ginteg = m.nll_parts(p)
+            assert abs(got - ref) <= nll_tol(ref, sl, integ, n_ev), (n_ev, n_norm, got, ref)
+            assert gsl == pytest.approx(sl, rel=1e-12, abs=1e-12) and ginteg == pytest.approx(integ, rel=1e-12)
+            m.set_path(B.PATH_RECOMPUTE)
+            rec, rsl, rinteg = m.nll_parts(p)
+            assert gsl == pytest.approx(rsl, rel=1e-13, abs=1e-12) and ginteg == pytest.approx(rinteg, rel=1e-13)
+        m.close()
+
+
 @pytest.mark.gpu
 @pytest.mark.parametrize("equal_masses", [True, False])
 @pytest.mark.parametrize("shared_radii", [True, False])
