@@ -104,6 +104,56 @@ k_nll_recompute(const __grid_constant__ DevModel m,
     // a pure S-wave model (R = 0) is bound by memory latency, not arithmetic: four points in flight per thread
     constexpr int PTS = (R1 == 0 && R2 == 0) ? 4 : MIPWA_REC_PTS;
     LogProd lp;
+    double integ = 0.0;
+    if constexpr (PTS == 1) {
+        // One point per thread and iteration.  Every non-FP64 instruction costs the issue slot an FP64 instruction
+        // could have used (cycles per warp-point ~ 2 x FP64 + others, profiles/r1_k_nll_recompute_ncu.md), so the loop
+        // bookkeeping is a 32-bit trip count, cursors advanced by a constant and no tail predicates: all `iters` points
+        // of a thread exist, and the prefetch of the last iteration is skipped, its registers never read.
+        {
+            const long long rem = n_ev - t0;
+            const int iters = rem > 0 ? (int)((rem + stride - 1) / stride) : 0;
+            const double *pa = e12 + t0, *pb = e13 + t0, *pk = eb + t0;
+            const unsigned short* ps = eseg + t0;
+            double a = 1.0, b = 1.0, bk = 0.0;
+            unsigned int sg = 0u;
+            if (iters > 0) { a = *pa; b = *pb; sg = *ps; if (MIX) bk = *pk; }
+            double na = a, nb = b, nbk = bk;
+            unsigned int ns = sg;
+            for (int it = 0; it < iters; ++it) {
+                pa += stride; pb += stride; ps += stride;
+                if (MIX) pk += stride;
+                if (it + 1 < iters) { na = *pa; nb = *pb; ns = *ps; if (MIX) nbk = *pk; }
+                double re, im;
+                amplitude_seg<R1, R2, FL>(sm, m, a, b, sg, re, im);
+                double v = fma(re, re, im * im);
+                if (MIX) v = fma(kappa, bk, v);
+                lp.add(v);
+                a = na; b = nb; sg = ns;
+                if (MIX) bk = nbk;
+            }
+        }
+        {
+            const long long rem = n_norm - t0;
+            const int iters = rem > 0 ? (int)((rem + stride - 1) / stride) : 0;
+            const bool has_w = gw != nullptr;
+            const double *pa = g12 + t0, *pb = g13 + t0, *pw = gw + t0;
+            const unsigned short* ps = gseg + t0;
+            double a = 1.0, b = 1.0, w = 1.0;
+            unsigned int sg = 0u;
+            if (iters > 0) { a = *pa; b = *pb; sg = *ps; if (has_w) w = *pw; }
+            double na = a, nb = b, nw = w;
+            unsigned int ns = sg;
+            for (int it = 0; it < iters; ++it) {
+                pa += stride; pb += stride; ps += stride; pw += stride;
+                if (it + 1 < iters) { na = *pa; nb = *pb; ns = *ps; if (has_w) nw = *pw; }
+                double re, im;
+                amplitude_seg<R1, R2, FL>(sm, m, a, b, sg, re, im);
+                integ = fma(w, fma(re, re, im * im), integ);
+                a = na; b = nb; w = nw; sg = ns;
+            }
+        }
+    } else {
     {
         double a[PTS], b[PTS], bk[PTS];
         unsigned int sg[PTS];
@@ -138,7 +188,6 @@ k_nll_recompute(const __grid_constant__ DevModel m,
             }
         }
     }
-    double integ = 0.0;
     {
         double a[PTS], b[PTS], w[PTS];
         unsigned int sg[PTS];
@@ -166,6 +215,7 @@ k_nll_recompute(const __grid_constant__ DevModel m,
 #pragma unroll
             for (int q = 0; q < PTS; ++q) { a[q] = na[q]; b[q] = nb[q]; w[q] = nw[q]; sg[q] = ns[q]; }
         }
+    }
     }
 
     double v[2] = { lp.value(), integ };
