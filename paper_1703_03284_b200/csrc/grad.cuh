@@ -185,24 +185,34 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
     LogProd lp;
     double integ = 0.0;
     const int nres = R1 >= 0 ? R1 + R2 : m.R;
+    // Non-FP64 instructions cost the issue slots the FP64 pipe needs (profiles/r1_k_grad_recompute_ncu.md): the loop runs
+    // on 32-bit offsets into this warp's chunk (CH <= 2^31 - 32: mipwa_nll_grad admits at most 2^31 - 1 points per set).
+    const int cnt = lo < hi ? (int)(hi - lo) : 0;
+    const double* const p12 = s12 + lo;
+    const double* const p13 = s13 + lo;
+    const double* const pw = w + lo;
+    const unsigned short* const psg = sgp + lo;
+    double2* const pf = fout + lo;
+    const bool has_w = w != nullptr;
     double nx = 1.0, ny = 1.0, nw = 0.0;                                   // next iteration's point, loaded one ahead
     unsigned int nsg = 0u;
-    if (lo < hi) {
-        const long long ii = lo + lane < hi ? lo + lane : lo;
-        nx = s12[ii]; ny = s13[ii]; nsg = sgp[ii];
-        if (!EV) nw = lo + lane < hi ? (w ? w[ii] : 1.0) : 0.0;
-        if (EV && MIX) nw = w[ii];
+    if (cnt > 0) {
+        const int ii = lane < cnt ? lane : 0;
+        nx = p12[ii]; ny = p13[ii]; nsg = psg[ii];
+        if (!EV) nw = lane < cnt ? (has_w ? pw[ii] : 1.0) : 0.0;
+        if (EV && MIX) nw = pw[ii];
     }
-    for (long long base = lo; base < hi; base += 32) {                     // warp-uniform trip count
-        const long long i = base + lane;
-        const bool valid = i < hi;
+    for (int base = 0; base < cnt; base += 32) {                           // warp-uniform trip count
+        const int i = base + lane;
+        const bool valid = i < cnt;
         const double x = nx, y = ny, wv = nw;
         const unsigned int sg = nsg;
-        if (base + 32 < hi) {
-            const long long ii = i + 32 < hi ? i + 32 : lo;
-            nx = s12[ii]; ny = s13[ii]; nsg = sgp[ii];
-            if (!EV) nw = i + 32 < hi ? (w ? w[ii] : 1.0) : 0.0;
-            if (EV && MIX) nw = w[ii];
+        if (base + 32 < cnt) {
+            const bool more = i + 32 < cnt;
+            const int ii = more ? i + 32 : 0;
+            nx = p12[ii]; ny = p13[ii]; nsg = psg[ii];
+            if (!EV) nw = more ? (has_w ? pw[ii] : 1.0) : 0.0;
+            if (EV && MIX) nw = pw[ii];
         }
         double are, aim, t1, t2, tr[RR], ti[RR];
         int j1, j2;
@@ -220,7 +230,7 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
             fr = wv * are; fi = wv * aim;
             integ = fma(wv, a2, integ);
         }
-        if (fout && valid) fout[i] = make_double2(fr, fi);                // for k_grad_shape (mipwa_nll_grad_full)
+        if (fout && valid) pf[i] = make_double2(fr, fi);                  // for k_grad_shape (mipwa_nll_grad_full)
         if (R1 >= 0) {
 #pragma unroll
             for (int r = 0; r < (R1 >= 0 ? R1 + R2 : 0); ++r) {
