@@ -44,7 +44,7 @@ def flops_per_point(resonances):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_nll_recompute launch at the bench size (10M events + 10M weighted
 # normalisation points), from the one `ncu --set full` capture summarised in profiles/r1_k_nll_recompute_ncu.md
-NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 443.9e6}
+NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 445.3e6}
 # executed FP64 flops per point in that capture (config 3's model): (dadd + dmul + 2 dfma) / points
 NCU_EXECUTED_FLOPS_PER_POINT = {(10_000_000, 10_000_000): 260.7}
 
