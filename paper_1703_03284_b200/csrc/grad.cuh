@@ -498,12 +498,24 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
 #define MIPWA_SHAPE_MAXF 4
 struct ShapeSel { int32_t slot[MIPWA_SHAPE_MAXF]; };       // device slots of the floating resonances of this launch
 
+// LT = 0, 1, 2: spin known at compile time (one floating resonance per launch: the usual case); LT < 0: read from r.
+template <int LT>
 __device__ __forceinline__ void shape_channel(const ResDev& r, const Channel& c, double& mr, double& mi, double& gr,
                                               double& gi)
 {
-    const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
-    const double DR = fma(zR, fma(zR, r.pa, r.pb), r.pc), DD = fma(zD, fma(zD, r.pa, r.pb), r.pc);
-    const double W = r.Kw * pick(r.L, c.w), Z = pick(r.L, c.Z);
+    double DR, DD, W, Z;
+    if (LT == 0) {
+        DR = 1.0; DD = 1.0; W = r.Kw * c.w[0]; Z = 1.0;
+    } else if (LT == 1) {
+        DR = fma(r.cR, c.ql, 1.0); DD = fma(r.cD, c.lam2, 1.0); W = r.Kw * c.w[1]; Z = c.Z[1];
+    } else if (LT == 2) {
+        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
+        DR = fma(zR, zR + 3.0, 9.0); DD = fma(zD, zD + 3.0, 9.0); W = r.Kw * c.w[2]; Z = c.Z[2];
+    } else {
+        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
+        DR = fma(zR, fma(zR, r.pa, r.pb), r.pc); DD = fma(zD, fma(zD, r.pa, r.pb), r.pc);
+        W = r.Kw * pick(r.L, c.w); Z = pick(r.L, c.Z);
+    }
     const double dD = (r.m0sq - c.x) * DR;
     const double rE = fast_rcp(fma(dD, dD, W * W));
     const double ur = dD * rE, ui = W * rE;
@@ -517,7 +529,7 @@ __device__ __forceinline__ void shape_channel(const ResDev& r, const Channel& c,
     mr = fma(tr, br, -ti * bi); mi = fma(tr, bi, ti * br);
 }
 
-template <int NF, int FL>
+template <int NF, int FL, int LT = -1>
 __global__ void __launch_bounds__(512, 1)
 k_grad_shape(const __grid_constant__ DevModel m, const ShapeSel sel,
              const double* __restrict__ e12, const double* __restrict__ e13, const double2* __restrict__ f_ev,
@@ -537,20 +549,25 @@ k_grad_shape(const __grid_constant__ DevModel m, const ShapeSel sel,
         double acc[NF][4];
 #pragma unroll
         for (int f = 0; f < NF; ++f) acc[f][0] = acc[f][1] = acc[f][2] = acc[f][3] = 0.0;
-        long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        // 32-bit trip count and cursor pointers, as in k_nll_recompute (issue slots: DESIGN.md section 6)
+        const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        const int iters = n > t0 ? (int)((n - t0 + stride - 1) / stride) : 0;
+        const double *pa = s12 + t0, *pb = s13 + t0;
+        const double2* pf = fp + t0;
         double nx = 1.0, ny = 1.0;                         // the next point, loaded one iteration ahead
         double2 nf = make_double2(0.0, 0.0);
-        if (i < n) { nx = s12[i]; ny = s13[i]; nf = fp[i]; }
-        for (; i < n; i += stride) {
+        if (iters > 0) { nx = *pa; ny = *pb; nf = *pf; }
+        for (int it = 0; it < iters; ++it) {
             const double x = nx, y = ny, fr = nf.x, fi = nf.y;
-            if (i + stride < n) { nx = s12[i + stride]; ny = s13[i + stride]; nf = fp[i + stride]; }
+            pa += stride; pb += stride; pf += stride;
+            if (it + 1 < iters) { nx = *pa; ny = *pb; nf = *pf; }
             const Channel ca = make_channel<FL & MIPWA_FL_EQM>(m, x, y), cb = make_channel<FL & MIPWA_FL_EQM>(m, y, x);
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const ResDev& r = m.res[sel.slot[f]];
                 double amr, ami, agr, agi, bmr, bmi, bgr, bgi;
-                shape_channel(r, ca, amr, ami, agr, agi);
-                shape_channel(r, cb, bmr, bmi, bgr, bgi);
+                shape_channel<LT>(r, ca, amr, ami, agr, agi);
+                shape_channel<LT>(r, cb, bmr, bmi, bgr, bgi);
                 const double dmr = amr + bmr, dmi = ami + bmi, dgr = agr + bgr, dgi = agi + bgi;
                 acc[f][0] = fma(fr, dmr, fma(fi, dmi, acc[f][0]));      // f conj(dT'/dm0)
                 acc[f][1] = fma(fi, dmr, fma(-fr, dmi, acc[f][1]));

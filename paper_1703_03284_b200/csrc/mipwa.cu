@@ -1293,20 +1293,26 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         ShapeSel sel;
         for (int q = 0; q < MIPWA_SHAPE_MAXF; ++q) sel.slot[q] = slots[f0 + std::min(q, nf - 1)];
         if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-#define MIPWA_SHAPE_LAUNCH(NF)                                                                                     \
+#define MIPWA_SHAPE_LAUNCH(NF, LT)                                                                                 \
     do {                                                                                                           \
         if (c->model_flags & MIPWA_FL_EQM)                                                                         \
-            k_grad_shape<NF, MIPWA_FL_EQM><<<grid, 512, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, \
-                                                                        G.s12, G.s13, c->d_f_nm, G.n, c->d_gpartials); \
+            k_grad_shape<NF, MIPWA_FL_EQM, LT><<<grid, 512, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, \
+                                                                            G.s12, G.s13, c->d_f_nm, G.n, c->d_gpartials); \
         else                                                                                                       \
-            k_grad_shape<NF, 0><<<grid, 512, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, G.s12,    \
-                                                             G.s13, c->d_f_nm, G.n, c->d_gpartials);               \
+            k_grad_shape<NF, 0, LT><<<grid, 512, 0, c->stream>>>(c->model, sel, E.s12, E.s13, c->d_f_ev, E.n, G.s12, \
+                                                                 G.s13, c->d_f_nm, G.n, c->d_gpartials);           \
     } while (0)
         switch (nf) {
-            case 1: MIPWA_SHAPE_LAUNCH(1); break;
-            case 2: MIPWA_SHAPE_LAUNCH(2); break;
-            case 3: MIPWA_SHAPE_LAUNCH(3); break;
-            default: MIPWA_SHAPE_LAUNCH(4); break;
+            case 1:                                        // one floating resonance: its spin is a template argument
+                switch (c->model.res[sel.slot[0]].L) {
+                    case 0: MIPWA_SHAPE_LAUNCH(1, 0); break;
+                    case 1: MIPWA_SHAPE_LAUNCH(1, 1); break;
+                    default: MIPWA_SHAPE_LAUNCH(1, 2); break;
+                }
+                break;
+            case 2: MIPWA_SHAPE_LAUNCH(2, -1); break;
+            case 3: MIPWA_SHAPE_LAUNCH(3, -1); break;
+            default: MIPWA_SHAPE_LAUNCH(4, -1); break;
         }
 #undef MIPWA_SHAPE_LAUNCH
         ++c->launches;
