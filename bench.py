@@ -139,6 +139,14 @@ def gpu_inputs(cfg, m, B, torch, rank):
     return host, dev
 
 
+def m_grad_full_ref(m, B, p):
+    """the same gradient through the full-recompute kernels (cross-check of the hybrid gradient leg)"""
+    m.set_path(B.PATH_RECOMPUTE)
+    g = m.nll_grad_full(p)[1]
+    m.set_path(B.PATH_HYBRID)
+    return g
+
+
 def run_ours(args, cfg, workload):
     import torch
     import torch.distributed as dist
@@ -322,10 +330,21 @@ def run_ours(args, cfg, workload):
             kms.append(m.last_kernel_ms())
         barrier()
         wall = (time.perf_counter() - t0) / sub_steps
+        for t in range(3):
+            m.nll_grad_full(params[t])
+        gms = []
+        for t in range(sub_steps):
+            nll_hg, grad_hg = m.nll_grad_full(params[args.warmup + t % args.steps])
+            gms.append(m.last_kernel_ms())
         hybrid_info = {"ms_per_call": 1e3 * wall, "kernel_ms": float(np.mean(kms)), "events_per_s": n_ev * world / wall,
+                       "grad_full_kernel_ms": float(np.mean(gms)), "grad_full_nll": nll_hg,
+                       "grad_full_max_abs_diff_vs_recompute": float(np.max(np.abs(
+                           grad_hg - m_grad_full_ref(m, B, params[args.warmup + (sub_steps - 1) % args.steps])))),
                        "cache_bytes": m.basis_bytes(), "first_call_s": setup_s, "nll": nll_h,
                        "what": "MIPWA_PATH_HYBRID: floating resonances and spline recomputed, fixed-shape resonance terms "
-                               "streamed from a per-point cache (not the headline: part of the work is cached)"}
+                               "streamed from a per-point cache (not the headline: part of the work is cached); grad_full_*: "
+                               "mipwa_nll_grad_full under an explicit MIPWA_PATH_HYBRID (k_grad_hybrid + k_grad_shape), "
+                               "cross-checked against the full-recompute gradient"}
     except B.MipwaError:
         pass
     m.set_path(B.PATH_RECOMPUTE)

@@ -131,7 +131,9 @@ int mipwa_nll_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, doub
  * form; reading P16; mipwa_nll_grad_full adds the derivatives with respect to floating masses/widths).
  * grad: HOST, 2N + 2R doubles, laid out like params.  Works on cell-sorted copies of the points (implies
  * mipwa_prepare).  With fixed shapes and the path MIPWA_PATH_CACHED_COMPACT (or AUTO) the events are streamed from
- * the compact cache and the normalisation part comes from the Gram matrix; otherwise every term is recomputed. */
+ * the compact cache and the normalisation part comes from the Gram matrix; otherwise every term is recomputed, except
+ * under an explicit MIPWA_PATH_HYBRID, where the fixed-shape resonance terms are read from the hybrid path's per-point
+ * caches (k_grad_hybrid; AUTO does not choose it for gradients: not yet faster than the full recompute). */
 int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
 /* NLL and its gradient with respect to ALL n_params parameters: the 2N + 2R entries of mipwa_nll_grad followed by

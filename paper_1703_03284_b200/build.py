@@ -10,7 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-UNITS = ["mipwa.cu", "tu_recompute.cu", "tu_recompute_mix.cu", "tu_abs2.cu", "tu_grad.cu", "tu_grad_mix.cu", "tu_hybrid.cu"]
+UNITS = ["mipwa.cu", "tu_recompute.cu", "tu_recompute_mix.cu", "tu_abs2.cu", "tu_grad.cu", "tu_grad_mix.cu", "tu_hybrid.cu", "tu_grad_hybrid.cu"]
 LIB = os.path.join(HERE, "libmipwa.so")
 OBJ_DIR = os.path.join(HERE, "_obj")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]

@@ -158,6 +158,21 @@ __device__ __forceinline__ double block_sum(double x, double* red32)
     return x;
 }
 
+#ifndef MIPWA_GRAD_RING_STAGES
+#define MIPWA_GRAD_RING_STAGES 4
+#endif
+#ifndef MIPWA_CP_ASYNC_DEFINED
+#define MIPWA_CP_ASYNC_DEFINED
+__device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsrc)
+{
+    const unsigned int sa = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
+#endif
+
 template <int R1, int R2> struct GradDims {
     static constexpr int RR = R1 >= 0 ? (R1 + R2 > 0 ? R1 + R2 : 1) : MIPWA_GRAD_MAXR;
 };
@@ -166,13 +181,19 @@ template <int R1, int R2> struct GradDims {
 // otherwise normalisation points (f = w A, scalar = sum w |A|^2).
 // MIX (EV only): background density w[i] per event and D = |A|^2 + kappa w: f = -2 A / D, scalar = sum ln D,
 // qsum = sum w / D (mipwa_nll_mix_grad).
-template <int R1, int R2, int FL, bool EV, bool MIX = false>
+// RCT > 0 (k_grad_hybrid, grad_hybrid.cuh): `m` holds only the floating resonances; the symmetrised values of RCT
+// fixed-shape resonances are read from the per-point cache of MIPWA_PATH_HYBRID (tile layout of cached.cuh, column 1 + k,
+// same point order as s12/s13), enter the amplitude with the coefficients coef[k] and get their own accumulators
+// Cr/Ci = sum f conj(b_k): for a cached term the basis function IS the cache column.
+template <int R1, int R2, int FL, bool EV, bool MIX = false, int RCT = 0>
 __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevModel& m, const double* __restrict__ s12,
                                           const double* __restrict__ s13, const double* __restrict__ w,
                                           const unsigned short* __restrict__ sgp, long long n,
                                           double2* __restrict__ fout, double kappa, double& qsum,
                                           double* bins, double& scalar, double (&Fr)[GradDims<R1, R2>::RR],
-                                          double (&Fi)[GradDims<R1, R2>::RR])
+                                          double (&Fi)[GradDims<R1, R2>::RR],
+                                          const double2* __restrict__ cache = nullptr, const double2* coef = nullptr,
+                                          double* Cr = nullptr, double* Ci = nullptr, double2* ring = nullptr)
 {
     constexpr int RR = GradDims<R1, R2>::RR;
     const int NS = m.N - 1, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
@@ -196,18 +217,73 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
     const bool has_w = w != nullptr;
     double nx = 1.0, ny = 1.0, nw = 0.0;                                   // next iteration's point, loaded one ahead
     unsigned int nsg = 0u;
+    // cache columns of the warp's 32 points: lo is a multiple of 32, so they share one 256-point tile
+    constexpr int RCN = RCT > 0 ? RCT : 1, CC = 1 + RCT;
+    const double2* const cbase = RCT > 0 ? cache + (size_t)(lo / MIPWA_TILE) * CC * MIPWA_TILE : nullptr;
+    const int coff = (int)(lo % MIPWA_TILE);
+    auto cidx = [&](int ii) { const int g = coff + ii; return (g / MIPWA_TILE) * (CC * MIPWA_TILE) + (g % MIPWA_TILE); };
+    // The cache columns go through a per-thread cp.async ring (as in k_nll_hybrid: every lane copies the slots it later
+    // reads, cp.async.wait_group is the only synchronisation), GRAD_RING_AHEAD warp-iterations ahead; slot (stage, k) of
+    // this thread: ring[(stage * (1 + RCT) + k) * blockDim.x], `ring` already offset by threadIdx.x.  Column 0 is the
+    // point (s12, s13) itself, so only the segment pair and the weight (2 + 8 B) still come through registers - two
+    // iterations ahead: with the resonance arithmetic gone an iteration is too short to cover a DRAM round trip.
+    constexpr int AHEAD = MIPWA_GRAD_RING_STAGES - 1;
+    const int rstage = (RCT > 0 ? CC : 1) * (int)blockDim.x;
+    int wr = 0, rd = 0;
+    auto fetch = [&](int i_next) {                        // i_next: this lane's offset AHEAD iterations on (or past the end)
+        if (RCT > 0) {
+            if (i_next - lane < cnt) {                     // warp-uniform: the iteration exists
+                const double2* q = cbase + cidx(i_next < cnt ? i_next : 0);
+#pragma unroll
+                for (int k = 0; k < CC; ++k) cp_async16(ring + wr + k * (int)blockDim.x, q + k * MIPWA_TILE);
+            }
+            cp_async_commit();
+            wr = wr + rstage == MIPWA_GRAD_RING_STAGES * rstage ? 0 : wr + rstage;
+        }
+    };
+    if (RCT > 0) {
+#pragma unroll
+        for (int q = 0; q < AHEAD; ++q) fetch(lane + 32 * q);
+    }
+    double n2w = 0.0;                                                      // RCT > 0: the point after the next
+    unsigned int n2sg = 0u;
+    auto side = [&](int i_at, unsigned int& sgo, double& wo) {            // segment pair and weight at offset i_at
+        const bool in = i_at < cnt;
+        const int ii = in ? i_at : 0;
+        sgo = psg[ii];
+        wo = 0.0;
+        if (!EV) wo = in ? (has_w ? pw[ii] : 1.0) : 0.0;
+        if (EV && MIX) wo = pw[ii];
+    };
     if (cnt > 0) {
-        const int ii = lane < cnt ? lane : 0;
-        nx = p12[ii]; ny = p13[ii]; nsg = psg[ii];
-        if (!EV) nw = lane < cnt ? (has_w ? pw[ii] : 1.0) : 0.0;
-        if (EV && MIX) nw = pw[ii];
+        if (RCT > 0) {
+            side(lane, nsg, nw);
+            if (32 < cnt) side(lane + 32, n2sg, n2w);
+        } else {
+            const int ii = lane < cnt ? lane : 0;
+            nx = p12[ii]; ny = p13[ii]; nsg = psg[ii];
+            if (!EV) nw = lane < cnt ? (has_w ? pw[ii] : 1.0) : 0.0;
+            if (EV && MIX) nw = pw[ii];
+        }
     }
     for (int base = 0; base < cnt; base += 32) {                           // warp-uniform trip count
         const int i = base + lane;
         const bool valid = i < cnt;
-        const double x = nx, y = ny, wv = nw;
+        double x = nx, y = ny;
+        const double wv = nw;
         const unsigned int sg = nsg;
-        if (base + 32 < cnt) {
+        double2 bk[RCN];
+        if (RCT > 0) {
+            nsg = n2sg; nw = n2w;
+            if (base + 64 < cnt) side(i + 64, n2sg, n2w);
+            fetch(i + 32 * AHEAD);
+            cp_async_wait<AHEAD>();                        // this iteration's columns have landed
+            const double2 pt = ring[rd];
+            x = pt.x; y = pt.y;
+#pragma unroll
+            for (int k = 0; k < RCT; ++k) bk[k] = ring[rd + (1 + k) * (int)blockDim.x];
+            rd = rd + rstage == MIPWA_GRAD_RING_STAGES * rstage ? 0 : rd + rstage;
+        } else if (base + 32 < cnt) {
             const bool more = i + 32 < cnt;
             const int ii = more ? i + 32 : 0;
             nx = p12[ii]; ny = p13[ii]; nsg = psg[ii];
@@ -217,6 +293,14 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
         double are, aim, t1, t2, tr[RR], ti[RR];
         int j1, j2;
         amplitude_parts<R1, R2, FL>(sm, m, x, y, sg, are, aim, j1, t1, j2, t2, tr, ti);
+        if (RCT > 0) {
+#pragma unroll
+            for (int k = 0; k < RCT; ++k) {
+                const double2 ck = coef[k];
+                are = fma(ck.x, bk[k].x, fma(-ck.y, bk[k].y, are));
+                aim = fma(ck.x, bk[k].y, fma(ck.y, bk[k].x, aim));
+            }
+        }
         const double a2 = fma(are, are, aim * aim);
         double fr, fi;
         if (EV) {
@@ -231,6 +315,13 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
             integ = fma(wv, a2, integ);
         }
         if (fout && valid) pf[i] = make_double2(fr, fi);                  // for k_grad_shape (mipwa_nll_grad_full)
+        if (RCT > 0) {
+#pragma unroll
+            for (int k = 0; k < RCT; ++k) {
+                Cr[k] = fma(fr, bk[k].x, fma(fi, bk[k].y, Cr[k]));         // f conj(b_k)
+                Ci[k] = fma(fi, bk[k].x, fma(-fr, bk[k].y, Ci[k]));
+            }
+        }
         if (R1 >= 0) {
 #pragma unroll
             for (int r = 0; r < (R1 >= 0 ? R1 + R2 : 0); ++r) {
@@ -259,6 +350,7 @@ __device__ __forceinline__ void grad_pass(const SplineCoefSmem& sm, const DevMod
         }
     }
     flush_warp(acc, bins, NS);
+    if (RCT > 0) cp_async_wait<0>();                       // nothing of this pass lands in the next pass's stages
     scalar = EV ? lp.value() : integ;
 }
 

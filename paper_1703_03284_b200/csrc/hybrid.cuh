@@ -65,6 +65,8 @@ __host__ __device__ constexpr size_t mipwa_hyb_ring_bytes(int rct)
     return (size_t)mipwa_hyb_stages(rct) * MIPWA_HYB_PTS(rct) * (1 + rct) * MIPWA_HYB_BLOCK * sizeof(double2);
 }
 
+#ifndef MIPWA_CP_ASYNC_DEFINED
+#define MIPWA_CP_ASYNC_DEFINED
 __device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsrc)
 {
     const unsigned int sa = (unsigned int)__cvta_generic_to_shared(smem_dst);
@@ -73,6 +75,7 @@ __device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsr
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NPENDING>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
+#endif
 
 // One launch over [events | normalisation points]; one point per thread and tile.  result[0] = sum ln|A|^2,
 // result[1] = sum w |A|^2 (w == NULL: weight 1).

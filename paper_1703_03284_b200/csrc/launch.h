@@ -51,3 +51,14 @@ cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cu
                                     long long n_ev, const double2* nm_cache, const double* gw,
                                     const unsigned short* gseg, long long n_norm, double2* partials,
                                     unsigned int* ticket, double* result);
+
+// tu_grad_hybrid.cu: k_grad_hybrid (grad_hybrid.cuh): the gradient passes with the fixed-shape terms read from the
+// hybrid path's per-point caches; smem = 16 (N - 1) doubles x 2 passes of segment moments
+cudaError_t mipwa_occupancy_grad_hybrid(int f1, int f2, int rc, int fl, size_t smem, int* blocks_per_sm);
+cudaError_t mipwa_launch_grad_hybrid(int f1, int f2, int rc, int fl, int grid, size_t smem, cudaStream_t st,
+                                     const DevModel& m, const HybCoef& cc, const double* e12, const double* e13,
+                                     const unsigned short* eseg, const double2* ev_cache, long long n_ev, const double* g12,
+                                     const double* g13, const double* gw, const unsigned short* gseg,
+                                     const double2* nm_cache, long long n_norm, double* partials, double2* f_ev,
+                                     double2* f_nm);
+

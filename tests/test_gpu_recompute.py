@@ -263,9 +263,13 @@ def test_hybrid_path_matches_oracle():
             assert abs(m.nll(p2) - ref2) <= nll_tol(ref2, sl2, integ2, data[0].size)
             m.set_path(B.PATH_AUTO)                          # AUTO picks the hybrid path here
             assert m.basis_bytes() > 0 and abs(m.nll(p) - ref) <= tol
-            _, g = m.nll_grad(p)                             # gradient falls back to the recompute kernel
+            _, g = m.nll_grad(p)                             # AUTO: gradients stay on k_grad_recompute
+            m.set_path(B.PATH_HYBRID)
+            _, gh = m.nll_grad(p)                            # explicit hybrid path: k_grad_hybrid
+            m.set_path(B.PATH_AUTO)
             _, ref_g = oo.nll_grad(p, *data)
             assert np.max(np.abs(g - ref_g)) <= 1e-9 * np.max(np.abs(ref_g))
+            assert np.max(np.abs(gh - ref_g)) <= 1e-9 * np.max(np.abs(ref_g))
             m.set_norm_points(data[2][:5000], data[3][:5000], None)     # uniform weights, new normalisation cache
             ref3, sl3, integ3 = oo.nll(p, data[0], data[1], data[2][:5000], data[3][:5000], None, parts=True)
             assert abs(m.nll(p) - ref3) <= nll_tol(ref3, sl3, integ3, data[0].size)
@@ -315,6 +319,14 @@ def test_hybrid_ring_ragged_sizes(n_fixed):
             m.set_path(B.PATH_RECOMPUTE)
             rec, rsl, rinteg = m.nll_parts(p)
             assert gsl == pytest.approx(rsl, rel=1e-13, abs=1e-12) and ginteg == pytest.approx(rinteg, rel=1e-13)
+            if n_ev in (257, 513, 160_001):                  # k_grad_hybrid + k_grad_shape: all 2N + 2R + 2 derivatives
+                m.set_path(B.PATH_HYBRID)
+                hn, hg = m.nll_grad_full(p)
+                _, g_lin = o.nll_grad(p, e12, e13, g12, g13, w)
+                _, g_shape = o.nll_grad_shape(p, e12, e13, g12, g13, w)
+                ref_g = np.concatenate([g_lin, g_shape])
+                assert abs(hn - ref) <= nll_tol(ref, sl, integ, n_ev)
+                assert np.max(np.abs(hg - ref_g)) <= 1e-9 * np.max(np.abs(ref_g)), (n_ev, n_fixed)
         m.close()
 
 

@@ -35,7 +35,9 @@ def case(request):
 
 
 def _paths(B, c):
-    return [B.PATH_RECOMPUTE] if any(r.get("shape_floats") for r in c.resonances) else [B.PATH_RECOMPUTE, B.PATH_AUTO]
+    if any(r.get("shape_floats") for r in c.resonances):
+        return [B.PATH_RECOMPUTE, B.PATH_HYBRID]           # k_grad_recompute / k_grad_hybrid, both followed by k_grad_shape
+    return [B.PATH_RECOMPUTE, B.PATH_AUTO]                 # AUTO: compact cache + Gram matrix
 
 
 def test_parts_match_oracle(case):
