@@ -406,7 +406,7 @@ def run_ours(args, cfg, workload):
         return
 
     # ---- roofline of the dominant kernel of the step (k_nll_recompute): plain FP64 ALU work -----------------------------
-    peak = B.measure_fp64_peak(local, 2.0)
+    peak, peak_3reg = B.measure_fp64_peak(local, 3.0)
     fl = flops_per_point(cfg.resonances) * (n_ev + n_norm)
     k_ms = float(np.mean(kernel_ms))
     achieved = fl / (k_ms * 1e-3) * 1e-12

@@ -83,8 +83,9 @@ int mipwa_set_stream(mipwa_ctx* ctx, void* cuda_stream);
  * left empty.  n = 0 is allowed (the NLL is then 0).  Invalidates the cached basis.
  * The same pass stores, in library-owned memory, the spline segment of s12[i] and of s13[i] as one uint16 per point
  * (knots are fixed at mipwa_create, so the pair is a property of the point set; +2 B per point): the per-call kernels
- * index the spline tables with it.  Borrowed (MIPWA_MEM_DEVICE) arrays must therefore not change while they are set;
- * a device array that is not 16-byte aligned is copied instead of borrowed. */
+ * index the spline tables with it.  Borrowed (MIPWA_MEM_DEVICE) arrays must therefore not change while they are set
+ * (they must be 8-byte aligned, as any array of doubles is).  The full-recompute kernels stream a library-owned copy of
+ * the set as 32-byte records (s12, s13, weight, segment rows), built on first use: + 32 B per point. */
 int mipwa_set_events(mipwa_ctx* ctx, const double* s12, const double* s13, int64_t n, int32_t mem);
 
 /* Normalisation points with weights w (NULL: w_j = 1/n).  I = sum_j w_j |A_j|^2 stands for the integral of
@@ -131,9 +132,9 @@ int mipwa_nll_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, doub
  * form; reading P16; mipwa_nll_grad_full adds the derivatives with respect to floating masses/widths).
  * grad: HOST, 2N + 2R doubles, laid out like params.  Works on cell-sorted copies of the points (implies
  * mipwa_prepare).  With fixed shapes and the path MIPWA_PATH_CACHED_COMPACT (or AUTO) the events are streamed from
- * the compact cache and the normalisation part comes from the Gram matrix; otherwise every term is recomputed, except
- * under an explicit MIPWA_PATH_HYBRID, where the fixed-shape resonance terms are read from the hybrid path's per-point
- * caches (k_grad_hybrid; AUTO does not choose it for gradients: not yet faster than the full recompute). */
+ * the compact cache and the normalisation part comes from the Gram matrix; otherwise every term is recomputed
+ * (k_grad_recompute; MIPWA_PATH_HYBRID caches terms for the VALUE only).  Two calls with the same arguments return
+ * the same bits: every sum is taken in a fixed order (no floating-point atomics). */
 int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
 /* NLL and its gradient with respect to ALL n_params parameters: the 2N + 2R entries of mipwa_nll_grad followed by
@@ -144,8 +145,9 @@ int mipwa_nll_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, doubl
  *     dT/dm0     = T d ln(F_R F_D)/dm0 - T (2 m0 - i m0 Gamma(x) d ln(m0 Gamma(x))/dm0) / D
  *     dNLL/dtheta = -2 sum_i Re(conj(A_i) dA_i)/|A_i|^2 + (2 n_ev / I) sum_j w_j Re(conj(A_j) dA_j),
  *     dA = c_r [dT_r(s12,s13) + dT_r(s13,s12)].
- * grad: HOST, n_params doubles.  One extra pass over both point sets (k_grad_shape) per call when a shape floats;
- * identical to mipwa_nll_grad when none does.  Errors as mipwa_nll_grad. */
+ * grad: HOST, n_params doubles.  With ONE floating resonance of spin 1 or 2 the extra sums are folded into the gradient
+ * pass itself; several floating resonances (or a floating spin-0 one) cost one more pass over both point sets
+ * (k_grad_shape).  Identical to mipwa_nll_grad when no shape floats.  Errors as mipwa_nll_grad. */
 int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad);
 
 /* The pieces ONE RANK of a sharded likelihood contributes (events and normalisation points are
@@ -219,9 +221,12 @@ int mipwa_last_kernel_ms(const mipwa_ctx* ctx, float* ms);
 /* Number of kernel launches issued by this context since creation (the benchmark's gpu_launches claim). */
 int64_t mipwa_launch_count(const mipwa_ctx* ctx);
 
-/* Measure the sustained FP64 FMA rate of the device with a register-resident DFMA loop on every SM for about
- * `seconds` seconds; *tflops = 2 * FMAs / time.  Denominator of the ALU roofline. */
-int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops);
+/* Measure the sustained FP64 FMA rate of the device with register-resident DFMA loops on every SM for about
+ * `seconds` seconds in all; 2 flops per DFMA.
+ *   *tflops       DFMAs with an immediate and a repeated register operand: the rate the FP64 pipe demonstrably issues
+ *                 at (the denominator of the ALU roofline)
+ *   *tflops_3reg  (may be NULL) DFMAs with three distinct register operands, which the operand fetch holds ~8 % lower */
+int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops, double* tflops_3reg);
 
 const char* mipwa_last_error(const mipwa_ctx* ctx);   /* valid until the next call on ctx; "" if none */
 const char* mipwa_version(void);

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MIPWA_LIB_PATH") or os.path.join(_HERE, "libmipwa.so")   # override: experiments only
+LIB_PATH = os.path.join(_HERE, "libmipwa.so")
 
 OK, ERR_ARG, ERR_DOMAIN, ERR_STATE, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4, -5
 MEM_HOST, MEM_DEVICE = 0, 1
@@ -85,7 +85,7 @@ def load_library():
     L.mipwa_enable_timing.restype = i32; L.mipwa_enable_timing.argtypes = [vp, i32]
     L.mipwa_last_kernel_ms.restype = i32; L.mipwa_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.mipwa_launch_count.restype = i64; L.mipwa_launch_count.argtypes = [vp]
-    L.mipwa_measure_fp64_peak.restype = i32; L.mipwa_measure_fp64_peak.argtypes = [i32, d, _dp]
+    L.mipwa_measure_fp64_peak.restype = i32; L.mipwa_measure_fp64_peak.argtypes = [i32, d, _dp, _dp]
     L.mipwa_last_error.restype = C.c_char_p; L.mipwa_last_error.argtypes = [vp]
     L.mipwa_version.restype = C.c_char_p; L.mipwa_version.argtypes = []
     _lib = L
@@ -328,12 +328,13 @@ class Mipwa:
 
 
 def measure_fp64_peak(device=0, seconds=2.0):
+    """(TFLOP/s of the FP64 pipe on 2-register + immediate DFMAs, TFLOP/s on 3-register DFMAs)"""
     L = load_library()
-    out = C.c_double()
-    rc = L.mipwa_measure_fp64_peak(int(device), float(seconds), C.byref(out))
+    out, out3 = C.c_double(), C.c_double()
+    rc = L.mipwa_measure_fp64_peak(int(device), float(seconds), C.byref(out), C.byref(out3))
     if rc != OK:
         raise MipwaError(rc, "mipwa_measure_fp64_peak failed")
-    return out.value
+    return out.value, out3.value
 
 
 def version():

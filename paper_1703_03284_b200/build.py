@@ -10,23 +10,24 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-UNITS = ["mipwa.cu", "tu_recompute.cu", "tu_recompute_mix.cu", "tu_abs2.cu", "tu_grad.cu", "tu_grad_mix.cu", "tu_hybrid.cu", "tu_grad_hybrid.cu"]
+UNITS = ["mipwa.cu", "tu_recompute.cu", "tu_recompute_mix.cu", "tu_abs2.cu", "tu_grad.cu", "tu_grad_mix.cu", "tu_grad_shp.cu",
+         "tu_hybrid.cu"]
 LIB = os.path.join(HERE, "libmipwa.so")
 OBJ_DIR = os.path.join(HERE, "_obj")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
 def sources():
-    return sorted(f for f in glob.glob(os.path.join(CSRC, "*.cu*")) + glob.glob(os.path.join(CSRC, "*.h"))
-                  if not f.endswith("fp64_microbench.cu")) + [os.path.join(HERE, "..", "include", "mipwa.h")]
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu*")) + glob.glob(os.path.join(CSRC, "*.h"))) + \
+        [os.path.join(HERE, "..", "include", "mipwa.h")]
 
 
-def build(force=False, verbose=False, extra=()):
+def build(force=False, verbose=False):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in sources()):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(OBJ_DIR, exist_ok=True)
-    flags = NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + list(extra)
+    flags = NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
 
     def compile_unit(u):
         obj = os.path.join(OBJ_DIR, u.replace(".cu", ".o"))
@@ -38,18 +39,5 @@ def build(force=False, verbose=False, extra=()):
     return LIB
 
 
-def build_microbench():
-    """Stand-alone FP64-pipe microbenchmarks (csrc/fp64_microbench.cu -> ./fp64_microbench); not part of the library."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    out = os.path.join(HERE, "fp64_microbench")
-    subprocess.run([nvcc, "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-o", out,
-                    os.path.join(CSRC, "fp64_microbench.cu")], check=True)
-    return out
-
-
 if __name__ == "__main__":
-    if "--microbench" in sys.argv:
-        print(build_microbench())
-    else:
-        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
-                    extra=[a for a in sys.argv[1:] if a.startswith("-D")]))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -30,12 +30,11 @@ struct BasisAux {
 // ---- NR-form local weights: S(s) = A y_j + B y_j+1 + C y''_j + D y''_j+1 -----------------------------------------
 struct SplW { int j; double A, B, C, D; };
 
-__device__ __forceinline__ SplW spline_weights(const SplineSmem& sm, const DevModel& m, double s)
+__device__ __forceinline__ SplW spline_weights(const SearchSmem& ss, double s)
 {
     SplW r;
-    double xj;
-    r.j = spline_segment(sm, m, s, xj);
-    const double xn = sm.knots[r.j + 1], h = xn - xj;
+    r.j = spline_segment(ss, s);
+    const double xj = ss.knots[r.j], xn = ss.knots[r.j + 1], h = xn - xj;
     r.A = (xn - s) / h;
     r.B = 1.0 - r.A;
     const double h6 = h * h / 6.0;
@@ -55,16 +54,17 @@ __device__ __forceinline__ double cardinal_one(const double* __restrict__ Mx, in
 // Basis row of one point: emit(k, B_k) for the spline columns k = k0, k0+kstep, .. < N and the resonance slots
 // d = k0, k0+kstep, .. < R.  `m` must be the UNIT-coefficient model (cre = sqrt(n_R n_D), cim = 0).
 template <class Emit>
-__device__ __forceinline__ void basis_point(const SplineSmem& sm, const DevModel& m, const BasisAux& aux, double s12,
+__device__ __forceinline__ void basis_point(const SearchSmem& ss, const DevModel& m, const BasisAux& aux, double s12,
                                             double s13, int k0, int kstep, bool spline_cols, Emit emit)
 {
     if (spline_cols) {
-        const SplW a = spline_weights(sm, m, s12), b = spline_weights(sm, m, s13);
+        const SplW a = spline_weights(ss, s12), b = spline_weights(ss, s13);
         for (int k = k0; k < m.N; k += kstep)
             emit(k, make_double2(cardinal_one(aux.Mx, m.N, a, k) + cardinal_one(aux.Mx, m.N, b, k), 0.0));
     }
     if (m.R > 0) {
-        const Channel ca = make_channel(m, s12, s13), cb = make_channel(m, s13, s12);
+        Channel ca, cb;
+        make_channels(m, s12, s13, ca, cb);
         for (int d = k0; d < m.R; d += kstep) {
             double tr, ti;
             resonance_sym<-1>(m.res[d], ca, cb, tr, ti);
@@ -76,11 +76,11 @@ __device__ __forceinline__ void basis_point(const SplineSmem& sm, const DevModel
 // ---- A9: build the per-event cache -------------------------------------------------------------------------------
 template <bool COMPACT>
 __global__ void __launch_bounds__(MIPWA_TILE)
-k_basis_build(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ s12,
-              const double* __restrict__ s13, long long n, double2* __restrict__ cache)
+k_basis_build(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, const BasisAux aux,
+              const double* __restrict__ s12, const double* __restrict__ s13, long long n, double2* __restrict__ cache)
 {
-    __shared__ SplineSmem sm;
-    load_spline_smem(sm, m);
+    __shared__ SearchSmem sm;
+    load_search_smem(sm, srch);
     const int C = COMPACT ? 1 + m.R : m.N + m.R;
     const long long n_tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
@@ -100,11 +100,12 @@ k_basis_build(const __grid_constant__ DevModel m, const BasisAux aux, const doub
 
 // ---- test hook: basis rows, row-major out[i*K + k] ----------------------------------------------------------------
 static __global__ void __launch_bounds__(MIPWA_TILE)
-k_basis_rows(const __grid_constant__ DevModel m, const BasisAux aux, const double* __restrict__ s12,
-             const double* __restrict__ s13, long long first, long long n, double2* __restrict__ out)
+k_basis_rows(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, const BasisAux aux,
+             const double* __restrict__ s12, const double* __restrict__ s13, long long first, long long n,
+             double2* __restrict__ out)
 {
-    __shared__ SplineSmem sm;
-    load_spline_smem(sm, m);
+    __shared__ SearchSmem sm;
+    load_search_smem(sm, srch);
     const int K = m.N + m.R;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
@@ -169,13 +170,10 @@ __device__ __forceinline__ double2 ld_stream(const double2* p)
 // One event per thread and tile, K independent 16-byte loads per thread (unrolled by 8: >= 128 B in flight per
 // thread), four FMA chains.  Events past n_ev (the padding of the last tile) contribute ln 1 = 0.
 // result[0] = sum ln|A_i|^2, result[1] = c^H G c.
-#ifndef MIPWA_DENSE_MINBLOCKS
-#define MIPWA_DENSE_MINBLOCKS 4
-#endif
-static __global__ void __launch_bounds__(MIPWA_TILE, MIPWA_DENSE_MINBLOCKS)
+static __global__ void __launch_bounds__(MIPWA_TILE, 4)
 k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cache, long long n_ev,
             const double2* __restrict__ G, double* __restrict__ partials, unsigned int* __restrict__ ticket,
-            double* __restrict__ result)
+            double* __restrict__ result, long long tag)
 {
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
@@ -203,7 +201,7 @@ k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cach
             i0 = fma(c.x, b.y, i0); i1 = fma(c.y, b.x, i1);
         }
         const double re = r0 + r1, im = i0 + i1;
-        lp.add(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
+        lp.add_counted(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
     }
     double v[1] = { lp.value() };
     if (grid_reduce<1>(v, partials, ticket, red, &is_last)) {
@@ -214,7 +212,7 @@ k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cach
             result[0] = sum_log;
             result[1] = integ;
             *ticket = 0;
-            __threadfence_system();
+            publish_result(result, tag);
         }
     }
 }
@@ -227,12 +225,12 @@ __global__ void __launch_bounds__(MIPWA_TILE, 4)
 k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDev cc,
               const double2* __restrict__ cache, const unsigned short* __restrict__ seg, long long n_ev,
               const double2* __restrict__ G,
-              double* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result)
+              double* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result, long long tag)
 {
-    __shared__ SplineCoefSmem sm;
+    __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
-    load_spline_coef_smem(sm, m);
+    load_rows_smem(sm, m);
     const int R = RT >= 0 ? RT : m.R, C = 1 + R, N = cc.N;
     const long long n_tiles = (n_ev + MIPWA_TILE - 1) / MIPWA_TILE;
     LogProd lp;
@@ -255,9 +253,9 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-                double r1, i1, r2, i2;
-                spline_eval_at(sm, s[u].x, (int)(sg[u] & 0xffu), r1, i1);
-                spline_eval_at(sm, s[u].y, (int)(sg[u] >> 8), r2, i2);
+                double r1, i1, r2, i2, t;
+                spline_eval_off(sm, s[u].x, seg_off1(sg[u]), r1, i1, t);
+                spline_eval_off(sm, s[u].y, seg_off2(sg[u]), r2, i2, t);
                 double re = r1 + r2, im = i1 + i2;
 #pragma unroll
                 for (int r = 0; r < RT; ++r) {
@@ -266,7 +264,7 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
                     im = fma(c.x, b[u][r].y, fma(c.y, b[u][r].x, im));
                 }
                 const bool live = tiles[u] < n_tiles && tiles[u] * MIPWA_TILE + threadIdx.x < n_ev;
-                lp.add(live ? fma(re, re, im * im) : 1.0);
+                lp.add_counted(live ? fma(re, re, im * im) : 1.0);
             }
         }
     } else {
@@ -275,16 +273,16 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
             const double2 s = ld_stream(p);
             const long long ii = tile * MIPWA_TILE + threadIdx.x;
             const unsigned int sg = ii < n_ev ? seg[ii] : 0u;
-            double r1, i1, r2, i2;
-            spline_eval_at(sm, s.x, (int)(sg & 0xffu), r1, i1);
-            spline_eval_at(sm, s.y, (int)(sg >> 8), r2, i2);
+            double r1, i1, r2, i2, t;
+            spline_eval_off(sm, s.x, seg_off1(sg), r1, i1, t);
+            spline_eval_off(sm, s.y, seg_off2(sg), r2, i2, t);
             double re = r1 + r2, im = i1 + i2;
             for (int r = 0; r < R; ++r) {
                 const double2 b = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE), c = cc.c[N + r];
                 re = fma(c.x, b.x, fma(-c.y, b.y, re));
                 im = fma(c.x, b.y, fma(c.y, b.x, im));
             }
-            lp.add(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
+            lp.add_counted(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
         }
     }
     double v[1] = { lp.value() };
@@ -296,7 +294,7 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
             result[0] = sum_log;
             result[1] = integ;
             *ticket = 0;
-            __threadfence_system();
+            publish_result(result, tag);
         }
     }
 }
@@ -314,14 +312,14 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
 // and WITHOUT the conjugate: M_kl = sum_i B_ik B_il / A_i^2, the event part of d2NLL / dc_k dc_l (complex symmetric).
 template <int TPT, bool HESS>
 __global__ void __launch_bounds__(MIPWA_TILE, 1)
-k_gram(const __grid_constant__ DevModel m, const BasisAux aux, const __grid_constant__ CoefDev cc,
-       const double* __restrict__ g12, const double* __restrict__ g13, const double* __restrict__ gw, long long n,
-       double w_default, double2* __restrict__ partial)
+k_gram(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, const BasisAux aux,
+       const __grid_constant__ CoefDev cc, const double* __restrict__ g12, const double* __restrict__ g13,
+       const double* __restrict__ gw, long long n, double w_default, double2* __restrict__ partial)
 {
     extern __shared__ double2 gram_smem[];
-    __shared__ SplineSmem sm;
+    __shared__ SearchSmem sm;
     __shared__ double ws[GRAM_P], wsi[GRAM_P];
-    load_spline_smem(sm, m);
+    load_search_smem(sm, srch);
     const int K = m.N + m.R, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, rows = 4 * nt;
     double2* Bs = gram_smem;                                       // [rows][GRAM_LD]
     for (int idx = threadIdx.x; idx < rows * GRAM_LD; idx += blockDim.x) Bs[idx] = make_double2(0.0, 0.0);

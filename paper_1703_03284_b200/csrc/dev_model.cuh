@@ -30,6 +30,8 @@ struct ResDev {
     double Kw;        // m0^2 Gamma0 n_R / (2 (4 q0^2)^L sqrt(q0^2))   (the 1/2 of g = sqrt(lam1)/(2x) lives here)
     double cre, cim;  // c_r * sqrt(n_R n_D)
     double pa, pb, pc;// barrier denominator den_L(z) = pc + z (pb + pa z)
+    double qR1, qR2;  // L = 2: D_R = 9 + ql (qR1 + qR2 ql), qR1 = 3 cR, qR2 = cR^2 (one instruction less than via z)
+    double qD1, qD2;  // L = 2: D_D = 9 + lam2 (qD1 + qD2 lam2)
     // shape derivatives (mipwa_nll_grad_full; only the pole quantities depend on m0, so these are per-call constants):
     double sh_a1;     // d ln sqrt(n_R n_D) / d m0
     double sh_a2;     // d ln(m0 Gamma(x)) / d m0 = 2/m0 - (L + 1/2) (dq0^2/dm0)/q0^2 + n_R'/n_R r^2 dq0^2/dm0
@@ -39,66 +41,59 @@ struct ResDev {
     int32_t fl;       // index among the floating resonances (caller's list order), -1: shape fixed
 };
 
-// Everything a kernel needs for one likelihood call; passed by value as a __grid_constant__ kernel parameter.
+// One spline segment as the per-call kernels read it: MIPWA_ROW consecutive double2 in shared memory,
+//   row[0] = (x_j, 0),  row[1 + q] = coefficient of t^q, t = s - x_j:  S(s) = c0 + t (c1 + t (c2 + t c3)).
+// A point addresses its two rows by BYTE OFFSET (segment x MIPWA_ROW_BYTES): the offsets are a property of the point
+// set (knots are fixed at mipwa_create) and sit in the 32-byte point records, so the hot loops spend no instruction on
+// index arithmetic.
+#define MIPWA_ROW 5
+#define MIPWA_ROW_BYTES (MIPWA_ROW * 16)
+
+// Everything a per-call kernel needs for one likelihood call; passed by value as a __grid_constant__ kernel parameter.
 struct DevModel {
     int32_t N;                 // knots
     int32_t R;                 // resonances
-    int32_t nlut;              // buckets in lut
-    int32_t lut_exact;         // 1: every bucket holds at most one knot (xk), so the segment needs no search
+    int32_t pad0, pad1;
     double t_lo, t_d;          // (m1+m2)^2, (m1-m2)^2
     double s_hi, s_top;        // (M-m3)^2, (M+m3)^2
     double sigma;              // M^2 + m1^2 + m2^2 + m3^2
     double kappa;              // (M^2 - m3^2)(m2^2 - m1^2)
+    double k_third;            // -1/3: a constant-bank operand instead of a 64-bit immediate rebuilt for every point
+    double lam2_b, lam2_c;     // lambda(M^2, x, m3^2) = x (x + lam2_b) + lam2_c: -(s_hi + s_top), s_hi s_top
+    double pad2;
+    ResDev res[MIPWA_DEV_MAX_RES];
+    double2 rows[MIPWA_DEV_MAX_KNOTS * MIPWA_ROW];
+};
+
+// The knot search table: depends on the knots only, so it is uploaded once at mipwa_create and read through a pointer
+// by the few kernels that meet points whose segment is not stored yet (boundary check, cache / Gram setup, generator).
+struct DevSearch {
+    int32_t N, nlut;           // knots; buckets in lut
+    int32_t lut_exact, pad;    // 1: every bucket holds at most one knot (xk), so the segment needs no search
     double lut_off, lut_inv;   // bucket = floor(s * lut_inv + lut_off), lut_off = -x_0 * lut_inv
     double knots[MIPWA_DEV_MAX_KNOTS];
-    double2 sc[4][MIPWA_DEV_MAX_KNOTS];   // segment j: S(s) = sc[0][j] + t(sc[1][j] + t(sc[2][j] + t sc[3][j])), t = s - x_j
     uint8_t lut[MIPWA_DEV_LUT];           // segment that contains the left edge of each bucket
     double xk[MIPWA_DEV_LUT];             // the interior knot inside bucket b (+inf if none); valid iff lut_exact
-    ResDev res[MIPWA_DEV_MAX_RES];
 };
 
-// Shared-memory copy of the spline tables (divergent lookups: constant memory would serialise them).
-struct SplineSmem {
-    double knots[MIPWA_DEV_MAX_KNOTS];
-    double2 sc[4][MIPWA_DEV_MAX_KNOTS];
-    uint8_t lut[MIPWA_DEV_LUT];
-    double xk[MIPWA_DEV_LUT];
-};
-
-// The coefficient tables alone, for kernels that get the segment of every point from the stored segment pairs.
-struct SplineCoefSmem {
-    double knots[MIPWA_DEV_MAX_KNOTS];
-    double2 sc[4][MIPWA_DEV_MAX_KNOTS];
+// Shared-memory copy of the segment rows (divergent lookups: constant memory would serialise them).
+struct RowsSmem {
+    double2 rows[MIPWA_DEV_MAX_KNOTS * MIPWA_ROW];
 };
 
 // The model arrives in the kernel parameter (constant) bank.  A constant-bank read whose index differs between the
-// lanes of a warp is replayed once per distinct address, so the tables are copied with a warp-uniform index: every
-// lane reads entry i, lane 0 stores it (a thread-indexed copy of the 13.5 KB tables took ~20 us per block).
-template <class Tables>
-__device__ __forceinline__ void copy_coef_rows(Tables& sm, const DevModel& m)
+// lanes of a warp is replayed once per distinct address, so the rows are copied with a warp-uniform index: every
+// lane reads entry i, lane 0 stores it (a thread-indexed copy of the tables took ~20 us per block).
+__device__ __forceinline__ void load_rows_smem(RowsSmem& sm, const DevModel& m)
 {
     const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5, lane = threadIdx.x & 31;
     for (int i = warp; i < m.N; i += nwarp) {
-        const double k = m.knots[i];
-        const double2 c0 = m.sc[0][i], c1 = m.sc[1][i], c2 = m.sc[2][i], c3 = m.sc[3][i];
-        if (lane == 0) { sm.knots[i] = k; sm.sc[0][i] = c0; sm.sc[1][i] = c1; sm.sc[2][i] = c2; sm.sc[3][i] = c3; }
-    }
-}
-
-__device__ __forceinline__ void load_spline_coef_smem(SplineCoefSmem& sm, const DevModel& m)
-{
-    copy_coef_rows(sm, m);
-    __syncthreads();
-}
-
-__device__ __forceinline__ void load_spline_smem(SplineSmem& sm, const DevModel& m)
-{
-    copy_coef_rows(sm, m);
-    const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5, lane = threadIdx.x & 31;
-    for (int i = warp; i < m.nlut; i += nwarp) {
-        const uint8_t l = m.lut[i];
-        const double x = m.xk[i];
-        if (lane == 0) { sm.lut[i] = l; sm.xk[i] = x; }
+        const double2 r0 = m.rows[i * MIPWA_ROW], r1 = m.rows[i * MIPWA_ROW + 1], r2 = m.rows[i * MIPWA_ROW + 2],
+                      r3 = m.rows[i * MIPWA_ROW + 3], r4 = m.rows[i * MIPWA_ROW + 4];
+        if (lane == 0) {
+            sm.rows[i * MIPWA_ROW] = r0; sm.rows[i * MIPWA_ROW + 1] = r1; sm.rows[i * MIPWA_ROW + 2] = r2;
+            sm.rows[i * MIPWA_ROW + 3] = r3; sm.rows[i * MIPWA_ROW + 4] = r4;
+        }
     }
     __syncthreads();
 }
@@ -125,48 +120,87 @@ __device__ __forceinline__ double fast_rsqrt(double x)
     return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
+// The value kernels deliver their totals through mapped pinned host memory; the host may poll instead of blocking in
+// cudaStreamSynchronize (a wake-up costs more than a small likelihood call).  Slot 2 of `result` gets the call's tag
+// AFTER the totals are visible system-wide.
+#define MIPWA_RESULT_TAG 2
+__device__ __forceinline__ void publish_result(double* result, long long tag)
+{
+    __threadfence_system();
+    *reinterpret_cast<volatile long long*>(result + MIPWA_RESULT_TAG) = tag;
+}
+
+// Shared-memory copy of the search table (setup kernels only).
+struct SearchSmem {
+    int32_t N, nlut, lut_exact, pad;
+    double lut_off, lut_inv;
+    double knots[MIPWA_DEV_MAX_KNOTS];
+    uint8_t lut[MIPWA_DEV_LUT];
+    double xk[MIPWA_DEV_LUT];
+};
+
+__device__ __forceinline__ void load_search_smem(SearchSmem& ss, const DevSearch* __restrict__ g)
+{
+    if (threadIdx.x == 0) {
+        ss.N = g->N; ss.nlut = g->nlut; ss.lut_exact = g->lut_exact; ss.pad = 0;
+        ss.lut_off = g->lut_off; ss.lut_inv = g->lut_inv;
+    }
+    for (int i = threadIdx.x; i < g->N; i += blockDim.x) ss.knots[i] = g->knots[i];
+    for (int i = threadIdx.x; i < g->nlut; i += blockDim.x) { ss.lut[i] = g->lut[i]; ss.xk[i] = g->xk[i]; }
+    __syncthreads();
+}
+
 // segment index j with x_j <= s < x_{j+1}, clamped to [0, N-2] (beyond the end knots the end cubic is used).
 // Buckets are narrower than the smallest knot spacing (lut_exact), so one compare against the single knot a bucket
-// can hold replaces a search: two dependent shared-memory reads (bucket entry, then the segment's row) and no branch.
+// can hold replaces a search: two dependent shared-memory reads (bucket entry, then the knot) and no branch.
 // A point within rounding of a bucket edge or a knot may land in the neighbouring segment; the spline is C^2, so
 // the neighbouring cubic differs there by O(distance^3) - far below one ulp.  Knot tables too dense for the
 // MIPWA_DEV_LUT buckets fall back to the search.
-__device__ __forceinline__ int spline_segment(const SplineSmem& sm, const DevModel& m, double s, double& xj)
+__device__ __forceinline__ int spline_segment(const SearchSmem& ss, double s)
 {
-    int b = __double2int_rd(fma(s, m.lut_inv, m.lut_off));     // lut_off = -lut_x0 * lut_inv
-    b = max(0, min(b, m.nlut - 1));
-    int j = sm.lut[b];
-    if (m.lut_exact) {
-        j += s >= sm.xk[b] ? 1 : 0;
-        xj = sm.knots[j];
-        return j;
-    }
-    xj = sm.knots[j];
-    double xn = sm.knots[j + 1];
-    while (s >= xn && j < m.N - 2) { ++j; xj = xn; xn = sm.knots[j + 1]; }
-    if (s < xj && j > 0) { --j; xj = sm.knots[j]; }     // guards the rounding of the bucket index
+    int b = __double2int_rd(fma(s, ss.lut_inv, ss.lut_off));     // lut_off = -lut_x0 * lut_inv
+    b = max(0, min(b, ss.nlut - 1));
+    int j = ss.lut[b];
+    if (ss.lut_exact) return j + (s >= ss.xk[b] ? 1 : 0);
+    double xj = ss.knots[j], xn = ss.knots[j + 1];
+    while (s >= xn && j < ss.N - 2) { ++j; xj = xn; xn = ss.knots[j + 1]; }
+    if (s < xj && j > 0) --j;                               // guards the rounding of the bucket index
     return j;
 }
 
-__device__ __forceinline__ void spline_eval(const SplineSmem& sm, const DevModel& m, double s, double& re, double& im)
+// spline value on the segment whose row starts `off` bytes into the shared-memory rows
+__device__ __forceinline__ void spline_eval_off(const RowsSmem& sm, double s, unsigned int off, double& re, double& im,
+                                                double& t)
 {
-    double xj;
-    const int j = spline_segment(sm, m, s, xj);
-    const double t = s - xj;
-    const double2 c0 = sm.sc[0][j], c1 = sm.sc[1][j], c2 = sm.sc[2][j], c3 = sm.sc[3][j];
+    const double2* row = reinterpret_cast<const double2*>(reinterpret_cast<const char*>(sm.rows) + off);
+    t = s - row[0].x;
+    const double2 c0 = row[1], c1 = row[2], c2 = row[3], c3 = row[4];
     re = fma(t, fma(t, fma(t, c3.x, c2.x), c1.x), c0.x);
     im = fma(t, fma(t, fma(t, c3.y, c2.y), c1.y), c0.y);
 }
 
-// spline value on a known segment j (the segment pair of every point is computed once per point set, by the
-// boundary-check kernel of mipwa_set_*, and stored as one uint16 per point: j12 | j13 << 8)
-template <class Tables>
-__device__ __forceinline__ void spline_eval_at(const Tables& sm, double s, int j, double& re, double& im)
+// the stored segment pair of a point (one uint16 per point, j12 | j13 << 8, written by k_validate) as row offsets
+__device__ __forceinline__ unsigned int seg_off1(unsigned int seg) { return (seg & 0xffu) * MIPWA_ROW_BYTES; }
+__device__ __forceinline__ unsigned int seg_off2(unsigned int seg) { return (seg >> 8) * MIPWA_ROW_BYTES; }
+
+// One point of a point set as the recompute kernels stream it: 32 bytes, one 256-bit load.
+//   w   normalisation points: weight w_j (1 if the caller gave none); events: background density b_i of the mixture
+//       likelihood (0 if none)
+//   o1, o2   byte offsets of the spline rows of s12 and s13 in RowsSmem
+struct __align__(32) PointRec {
+    double s12, s13, w;
+    unsigned int o1, o2;
+};
+
+__device__ __forceinline__ PointRec ld_rec(const PointRec* p)
 {
-    const double t = s - sm.knots[j];
-    const double2 c0 = sm.sc[0][j], c1 = sm.sc[1][j], c2 = sm.sc[2][j], c3 = sm.sc[3][j];
-    re = fma(t, fma(t, fma(t, c3.x, c2.x), c1.x), c0.x);
-    im = fma(t, fma(t, fma(t, c3.y, c2.y), c1.y), c0.y);
+    PointRec r;
+    double d;
+    asm("ld.global.nc.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];"
+        : "=d"(r.s12), "=d"(r.s13), "=d"(r.w), "=d"(d) : "l"(p));
+    r.o1 = (unsigned int)__double2loint(d);
+    r.o2 = (unsigned int)__double2hiint(d);
+    return r;
 }
 
 // per-channel kinematic quantities shared by all resonances
@@ -183,28 +217,34 @@ struct Channel {
 //   MIPWA_FL_SHR  every resonance of one spin has the same r_res and r_parent (the usual choice, e.g. 1.5 and
 //                 5 GeV^-1 for all): the barrier denominators D_R, D_D and rsqrt(D_R D_D) are per spin and channel
 #define MIPWA_FL_EQM 1
+#define MIPWA_TINY 0x1p-996
 #define MIPWA_FL_SHR 2
 
+// x: the channel's mass squared; z1: Z_1 of the equal-mass case, x + 2 y - Sigma (y = the other channel), which the
+// caller forms for both channels from one shared sum.
+// lam2 in expanded form: two instructions instead of three; its absolute error (~1e-15) only matters where lam2 itself
+// vanishes, at the edge x = (M - m3)^2, and there it enters as 1 + c_D lam2 and as a term of Z_2.
 template <int FL = 0>
-__device__ __forceinline__ Channel make_channel(const DevModel& m, double x, double y)
+__device__ __forceinline__ Channel make_channel(const DevModel& m, double x, double z1)
 {
     Channel c;
     c.x = x;
-    c.lam2 = (m.s_hi - x) * (m.s_top - x);
+    c.lam2 = fma(x, x + m.lam2_b, m.lam2_c);
     c.Z[0] = 1.0;
     if (FL & MIPWA_FL_EQM) {
-        // |ql| x + 1e-300 under the root: a point within rounding of the threshold (the boundary check admits a
-        // relative 1e-12) gives a width of rounding size, not NaN or infinity
+        // |ql| x + 2^-996 under the root: a point within rounding of the threshold (the boundary check admits a
+        // relative 1e-12) gives a width of rounding size, not NaN or infinity.  (2^-996 ~ 1.5e-300 has a zero low
+        // word, so it is an immediate operand; 1e-300 took two moves per point.)
         c.ql = x - m.t_lo;
-        const double lc = fma(fabs(c.ql), x, 1e-300);
+        const double lc = fma(fabs(c.ql), x, MIPWA_TINY);
         double y0;
         asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(lc));
         const double u = c.ql * y0, e = fma(-(lc * y0), y0, 1.0);      // ql rsqrt(lc), refinement merged in
         c.w[0] = fma(u * e, fma(0.375, e, 0.5), u);
         c.w[1] = c.w[0] * c.ql;
         c.w[2] = c.w[1] * c.ql;
-        c.Z[1] = fma(2.0, y, x) - m.sigma;
-        c.Z[2] = fma(c.Z[1], c.Z[1], (c.w[0] * c.w[0]) * (c.lam2 * (-1.0 / 3.0)));
+        c.Z[1] = z1;
+        c.Z[2] = fma(c.Z[1], c.Z[1], (c.w[0] * c.w[0]) * (c.lam2 * m.k_third));
         return c;
     }
     const double lam1 = (x - m.t_lo) * (x - m.t_d);
@@ -215,7 +255,7 @@ __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, dou
     // width vanishes anyway
     // (rsqrt refinement merged with the product: sqrt(l) = h + h e p(e), h = l y0, e = 1 - h y0, p = 1/2 + 3e/8;
     // the factor 1/2 of g is folded into Kw on the host)
-    const double lc = fmax(lam1, 1e-300);
+    const double lc = fmax(lam1, MIPWA_TINY);
     double y0;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(lc));
     const double h = lc * y0, e = fma(-h, y0, 1.0);
@@ -223,20 +263,30 @@ __device__ __forceinline__ Channel make_channel(const DevModel& m, double x, dou
     c.w[0] = sq * ix;
     c.w[1] = c.w[0] * c.ql;
     c.w[2] = c.w[1] * c.ql;
-    c.Z[1] = fma(m.kappa, ix, fma(2.0, y, x) - m.sigma);
-    c.Z[2] = fma(c.Z[1], c.Z[1], (-1.0 / 3.0) * (c.ql * pl));
+    c.Z[1] = fma(m.kappa, ix, z1);
+    c.Z[2] = fma(c.Z[1], c.Z[1], m.k_third * (c.ql * pl));
     return c;
+}
+
+// both channels of a point: Z_1 = x + 2 y - Sigma = (s12 + s13 - Sigma) + y, the bracket shared by the two
+template <int FL = 0>
+__device__ __forceinline__ void make_channels(const DevModel& m, double s12, double s13, Channel& ca, Channel& cb)
+{
+    const double u = (s12 + s13) - m.sigma;
+    ca = make_channel<FL>(m, s12, u + s13);
+    cb = make_channel<FL>(m, s13, u + s12);
 }
 
 __device__ __forceinline__ double pick(int L, const double (&v)[3]) { return L == 0 ? v[0] : (L == 1 ? v[1] : v[2]); }
 
-// One resonance in one channel.  Returns F_D F_R Z_L BW / sqrt(n_R n_D); c_r sqrt(n_R n_D) is applied by the caller.
+// One resonance in one channel: F_D F_R Z_L BW / sqrt(n_R n_D) = t (dD + i W) as the three real factors (the caller
+// symmetrises with fused multiply-adds); c_r sqrt(n_R n_D) is applied later.
 // LT = 0, 1, 2: spin known at compile time (no selects, unused factors vanish).  LT < 0: spin read from the model,
 // branch-free: den_L(z) = pc + z (pb + pa z) with (pa, pb, pc) = (0,0,1), (0,1,1), (1,3,9), factors selected.
 template <int LT>
-__device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel& c, double& tre, double& tim)
+__device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel& c, double& t, double& dD, double& W)
 {
-    double DR, DD, W, Z;
+    double DR, DD, Z;
     if (LT == 0) {
         DR = 1.0; DD = 1.0; W = r.Kw * c.w[0]; Z = 1.0;
     } else if (LT == 1) {
@@ -245,9 +295,8 @@ __device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel
         W = r.Kw * c.w[1];
         Z = c.Z[1];
     } else if (LT == 2) {
-        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
-        DR = fma(zR, zR + 3.0, 9.0);
-        DD = fma(zD, zD + 3.0, 9.0);
+        DR = fma(c.ql, fma(c.ql, r.qR2, r.qR1), 9.0);
+        DD = fma(c.lam2, fma(c.lam2, r.qD2, r.qD1), 9.0);
         W = r.Kw * c.w[2];
         Z = c.Z[2];
     } else {
@@ -257,12 +306,10 @@ __device__ __forceinline__ void resonance_channel(const ResDev& r, const Channel
         W = r.Kw * pick(r.L, c.w);
         Z = pick(r.L, c.Z);
     }
-    const double dD = (r.m0sq - c.x) * DR;
+    dD = (r.m0sq - c.x) * DR;
     const double E = fma(dD, dD, W * W);
     const double rs = fast_rsqrt((DR * DD) * (E * E));
-    const double t = (LT == 0 ? rs : Z * DR * rs);
-    tre = t * dD;
-    tim = t * W;
+    t = (LT == 0 ? rs : Z * DR * rs);
 }
 
 // Bose-symmetrised term T_r(s12,s13) + T_r(s13,s12) without its coefficient (and without sqrt(n_R n_D))
@@ -270,11 +317,11 @@ template <int LT>
 __device__ __forceinline__ void resonance_sym(const ResDev& rd, const Channel& ca, const Channel& cb, double& tr,
                                               double& ti)
 {
-    double ar, ai, br, bi;
-    resonance_channel<LT>(rd, ca, ar, ai);
-    resonance_channel<LT>(rd, cb, br, bi);
-    tr = ar + br;
-    ti = ai + bi;
+    double ta, da, Wa, tb, db, Wb;
+    resonance_channel<LT>(rd, ca, ta, da, Wa);
+    resonance_channel<LT>(rd, cb, tb, db, Wb);
+    tr = fma(ta, da, tb * db);
+    ti = fma(ta, Wa, tb * Wb);
 }
 
 template <int LT>
@@ -299,9 +346,8 @@ __device__ __forceinline__ void group_barrier(const ResDev& r, const Channel& c,
         DR = fma(r.cR, c.ql, 1.0);
         DD = fma(r.cD, c.lam2, 1.0);
     } else {
-        const double zR = r.cR * c.ql, zD = r.cD * c.lam2;
-        DR = fma(zR, zR + 3.0, 9.0);
-        DD = fma(zD, zD + 3.0, 9.0);
+        DR = fma(c.ql, fma(c.ql, r.qR2, r.qR1), 9.0);
+        DD = fma(c.lam2, fma(c.lam2, r.qD2, r.qD1), 9.0);
     }
     FZ = (c.Z[LT] * DR) * fast_rsqrt(DR * DD);
 }
@@ -314,10 +360,11 @@ __device__ __forceinline__ void group_shared_terms(const ResDev* rd, const Chann
     double DRa, FZa, DRb, FZb;
     group_barrier<LT>(rd[0], ca, DRa, FZa);
     group_barrier<LT>(rd[0], cb, DRb, FZb);
+    const double xDa = ca.x * DRa, xDb = cb.x * DRb;       // (m0^2 - x) D_R = m0^2 D_R - x D_R: one product for the group
 #pragma unroll
     for (int r = 0; r < NR; ++r) {
         const double Wa = rd[r].Kw * ca.w[LT], Wb = rd[r].Kw * cb.w[LT];
-        const double da = (rd[r].m0sq - ca.x) * DRa, db = (rd[r].m0sq - cb.x) * DRb;
+        const double da = fma(rd[r].m0sq, DRa, -xDa), db = fma(rd[r].m0sq, DRb, -xDb);
         const double ta = FZa * fast_rcp(fma(da, da, Wa * Wa)), tb = FZb * fast_rcp(fma(db, db, Wb * Wb));
         tr[r] = fma(ta, da, tb * db);
         ti[r] = fma(ta, Wa, tb * Wb);
@@ -345,7 +392,8 @@ template <int R1, int R2, int FL = 0>
 __device__ __forceinline__ void add_resonances(const DevModel& m, double s12, double s13, double& are, double& aim)
 {
     if (R1 == 0 && R2 == 0) return;
-    const Channel ca = make_channel<FL>(m, s12, s13), cb = make_channel<FL>(m, s13, s12);
+    Channel ca, cb;
+    make_channels<FL>(m, s12, s13, ca, cb);
     if (R1 >= 0) {
         if ((FL & MIPWA_FL_SHR) && R1 >= 2) {
             add_group_shared<1, (R1 >= 2 ? R1 : 2)>(&m.res[0], ca, cb, are, aim);
@@ -364,29 +412,34 @@ __device__ __forceinline__ void add_resonances(const DevModel& m, double s12, do
     }
 }
 
+// A at a point whose spline rows are known (byte offsets o1, o2 into the shared-memory rows)
 template <int R1, int R2, int FL = 0>
-__device__ __forceinline__ void amplitude(const SplineSmem& sm, const DevModel& m, double s12, double s13,
-                                          double& are, double& aim)
+__device__ __forceinline__ void amplitude_off(const RowsSmem& sm, const DevModel& m, double s12, double s13,
+                                              unsigned int o1, unsigned int o2, double& are, double& aim)
 {
-    double r1, i1, r2, i2;
-    spline_eval(sm, m, s12, r1, i1);
-    spline_eval(sm, m, s13, r2, i2);
+    double r1, i1, r2, i2, t;
+    spline_eval_off(sm, s12, o1, r1, i1, t);
+    spline_eval_off(sm, s13, o2, r2, i2, t);
     are = r1 + r2;
     aim = i1 + i2;
     add_resonances<R1, R2, FL>(m, s12, s13, are, aim);
 }
 
-// the same with the segment pair of the point known (seg = j12 | j13 << 8)
-template <int R1, int R2, int FL = 0, class Tables = SplineSmem>
-__device__ __forceinline__ void amplitude_seg(const Tables& sm, const DevModel& m, double s12, double s13,
+// the same from the stored segment pair (seg = j12 | j13 << 8)
+template <int R1, int R2, int FL = 0>
+__device__ __forceinline__ void amplitude_seg(const RowsSmem& sm, const DevModel& m, double s12, double s13,
                                               unsigned int seg, double& are, double& aim)
 {
-    double r1, i1, r2, i2;
-    spline_eval_at(sm, s12, (int)(seg & 0xffu), r1, i1);
-    spline_eval_at(sm, s13, (int)(seg >> 8), r2, i2);
-    are = r1 + r2;
-    aim = i1 + i2;
-    add_resonances<R1, R2, FL>(m, s12, s13, are, aim);
+    amplitude_off<R1, R2, FL>(sm, m, s12, s13, seg_off1(seg), seg_off2(seg), are, aim);
+}
+
+// the same for a point met for the first time (generator, setup): segment search in the knot table
+template <int R1, int R2, int FL = 0>
+__device__ __forceinline__ void amplitude_search(const RowsSmem& sm, const SearchSmem& ss, const DevModel& m, double s12,
+                                                 double s13, double& are, double& aim)
+{
+    amplitude_off<R1, R2, FL>(sm, m, s12, s13, spline_segment(ss, s12) * MIPWA_ROW_BYTES,
+                              spline_segment(ss, s13) * MIPWA_ROW_BYTES, are, aim);
 }
 
 #define MIPWA_SIG_MAX1 4

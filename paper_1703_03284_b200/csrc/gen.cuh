@@ -50,26 +50,28 @@ __device__ __forceinline__ bool gen_inside(const GenKin& k, double s12, double s
     return fabs(__dsub_rn(s13, centre)) <= half;
 }
 
-__device__ __forceinline__ double gen_abs2(const SplineSmem& sm, const DevModel& m, double x, double y)
+__device__ __forceinline__ double gen_abs2(const RowsSmem& sm, const SearchSmem& ss, const DevModel& m, double x, double y)
 {
     double re, im;
-    amplitude<-1, -1, 0>(sm, m, x, y, re, im);
+    amplitude_search<-1, -1, 0>(sm, ss, m, x, y, re, im);
     return fma(re, re, im * im);
 }
 
 // fine grid pass: own[cx * nc + cy] = max |A|^2 (as the bit pattern of a non-negative double: ordered like integers)
 static __global__ void __launch_bounds__(256)
-k_gen_envelope(const __grid_constant__ DevModel m, const GenKin k, int n_side, double h, double H, int nc,
-               unsigned long long* __restrict__ own)
+k_gen_envelope(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, const GenKin k, int n_side,
+               double h, double H, int nc, unsigned long long* __restrict__ own)
 {
-    __shared__ SplineSmem sm;
-    load_spline_smem(sm, m);
+    __shared__ RowsSmem sm;
+    __shared__ SearchSmem ss;
+    load_search_smem(ss, srch);
+    load_rows_smem(sm, m);
     const long long total = (long long)n_side * n_side, stride = (long long)gridDim.x * blockDim.x;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += stride) {
         const int i = (int)(t / n_side), j = (int)(t % n_side);
         const double x = __dadd_rn(k.lo, __dmul_rn((double)i + 0.5, h)), y = __dadd_rn(k.lo, __dmul_rn((double)j + 0.5, h));
         if (!gen_inside(k, x, y)) continue;
-        const double a2 = gen_abs2(sm, m, x, y);
+        const double a2 = gen_abs2(sm, ss, m, x, y);
         const int cx = min((int)__ddiv_rn(__dsub_rn(x, k.lo), H), nc - 1), cy = min((int)__ddiv_rn(__dsub_rn(y, k.lo), H), nc - 1);
         if (a2 > 0.0) atomicMax(&own[cx * nc + cy], (unsigned long long)__double_as_longlong(a2));
     }
@@ -77,12 +79,15 @@ k_gen_envelope(const __grid_constant__ DevModel m, const GenKin k, int n_side, d
 
 // candidates ctr0 .. ctr0 + count - 1: position and accept flag
 static __global__ void __launch_bounds__(256)
-k_gen_candidates(const __grid_constant__ DevModel m, const GenKin k, unsigned long long key, long long ctr0,
-                 long long count, int nc, double H, const double* __restrict__ cum, const double* __restrict__ env,
+k_gen_candidates(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, const GenKin k,
+                 unsigned long long key, long long ctr0, long long count, int nc, double H,
+                 const double* __restrict__ cum, const double* __restrict__ env,
                  double* __restrict__ c12, double* __restrict__ c13, unsigned char* __restrict__ flag)
 {
-    __shared__ SplineSmem sm;
-    load_spline_smem(sm, m);
+    __shared__ RowsSmem sm;
+    __shared__ SearchSmem ss;
+    load_search_smem(ss, srch);
+    load_rows_smem(sm, m);
     const long long stride = (long long)gridDim.x * blockDim.x;
     const int ncell = nc * nc;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
@@ -98,7 +103,7 @@ k_gen_candidates(const __grid_constant__ DevModel m, const GenKin k, unsigned lo
         const double x = __dadd_rn(k.lo, __dmul_rn(__dadd_rn((double)cx, u1), H));
         const double y = __dadd_rn(k.lo, __dmul_rn(__dadd_rn((double)cy, u2), H));
         bool acc = gen_inside(k, x, y);
-        if (acc) acc = __dmul_rn(u3, env[cell]) < gen_abs2(sm, m, x, y);
+        if (acc) acc = __dmul_rn(u3, env[cell]) < gen_abs2(sm, ss, m, x, y);
         c12[t] = x; c13[t] = y; flag[t] = acc ? 1 : 0;
     }
 }

@@ -16,7 +16,7 @@ struct HybCoef {
 };
 
 template <int R1, int R2, int RCT, int FL>
-__device__ __forceinline__ double hybrid_abs2(const SplineCoefSmem& sm, const DevModel& m, const HybCoef& cc, double2 s,
+__device__ __forceinline__ double hybrid_abs2(const RowsSmem& sm, const DevModel& m, const HybCoef& cc, double2 s,
                                               unsigned int sg, const double2 (&b)[RCT])
 {
     double re, im;
@@ -42,16 +42,9 @@ __device__ __forceinline__ double hybrid_abs2(const SplineCoefSmem& sm, const De
 // a single dependent chain of ~100 FP64 instructions per point; with four warps per scheduler that does not fill the
 // pipe (k_nll_recompute with one resonance: 0.19 ms where the instruction count says 0.14), so two independent points
 // are evaluated side by side.
-#ifndef MIPWA_HYB_BLOCK
 #define MIPWA_HYB_BLOCK 512
-#endif
-#ifndef MIPWA_HYB_MINBLOCKS
-#define MIPWA_HYB_MINBLOCKS 1
-#endif
 // points per thread and iteration: two while the ring still gets >= 3 stages (RC <= 3), else one
-#ifndef MIPWA_HYB_PTS
 #define MIPWA_HYB_PTS(rct) ((rct) <= 3 ? 2 : 1)
-#endif
 // ring stages: as many as fit 200 KB of shared memory, at most 4, at least 2
 __host__ __device__ constexpr int mipwa_hyb_stages(int rct)
 {
@@ -65,8 +58,6 @@ __host__ __device__ constexpr size_t mipwa_hyb_ring_bytes(int rct)
     return (size_t)mipwa_hyb_stages(rct) * MIPWA_HYB_PTS(rct) * (1 + rct) * MIPWA_HYB_BLOCK * sizeof(double2);
 }
 
-#ifndef MIPWA_CP_ASYNC_DEFINED
-#define MIPWA_CP_ASYNC_DEFINED
 __device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsrc)
 {
     const unsigned int sa = (unsigned int)__cvta_generic_to_shared(smem_dst);
@@ -75,7 +66,6 @@ __device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsr
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NPENDING>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
-#endif
 
 // One launch over [events | normalisation points]; one point per thread and tile.  result[0] = sum ln|A|^2,
 // result[1] = sum w |A|^2 (w == NULL: weight 1).
@@ -83,18 +73,18 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // they and the weights (2 + 8 B per point) are prefetched through registers, as far ahead as the ring.
 // Dynamic shared memory: mipwa_hyb_ring_bytes(RCT).
 template <int R1, int R2, int RCT, int FL>
-__global__ void __launch_bounds__(MIPWA_HYB_BLOCK, MIPWA_HYB_MINBLOCKS)
+__global__ void __launch_bounds__(MIPWA_HYB_BLOCK, 1)
 k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef cc,
              const double2* __restrict__ ev_cache, const unsigned short* __restrict__ eseg, long long n_ev,
              const double2* __restrict__ nm_cache, const double* __restrict__ gw,
              const unsigned short* __restrict__ gseg, long long n_norm,
-             double2* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result)
+             double2* __restrict__ partials, unsigned int* __restrict__ ticket, double* __restrict__ result, long long tag)
 {
     extern __shared__ __align__(16) unsigned char hyb_ring_raw[];
-    __shared__ SplineCoefSmem sm;
+    __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
-    load_spline_coef_smem(sm, m);
+    load_rows_smem(sm, m);
     constexpr int C = 1 + RCT, ST = MIPWA_HYB_STAGES(RCT), AHEAD = ST - 1, PTS = MIPWA_HYB_PTS(RCT);
     constexpr int TPB = MIPWA_HYB_BLOCK / MIPWA_TILE;                                  // tiles per block and point slot
     constexpr int STAGE = PTS * C * MIPWA_HYB_BLOCK;                                   // double2 per ring stage
@@ -165,7 +155,7 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
             }
 #pragma unroll
             for (int u = 0; u < PTS; ++u) {
-                if (pass == 0) lp.add(live[u] ? vv[u] : 1.0);
+                if (pass == 0) lp.add_counted(live[u] ? vv[u] : 1.0);
                 else integ = fma(wq[0][u], live[u] ? vv[u] : 0.0, integ);
             }
 #pragma unroll
@@ -199,7 +189,7 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
             result[0] = f[0];
             result[1] = f[1];
             *ticket = 0;
-            __threadfence_system();
+            publish_result(result, tag);
         }
     }
 }

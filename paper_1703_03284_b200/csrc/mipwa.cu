@@ -10,6 +10,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "launch.h"
 #include "kernels.cuh"
 #include "cached.cuh"
@@ -31,8 +33,16 @@ struct Slot {                       // events or normalisation points
     const double* s13 = nullptr;
     const double* w = nullptr;
     const unsigned short* seg = nullptr;   // spline segment pair per point, j12 | j13 << 8 (always library-owned)
+    const PointRec* rec = nullptr;  // 32-byte records of the recompute kernels (built on first use, library-owned)
     int64_t n = -1;                 // -1: not set
-    void* owned[4] = { nullptr, nullptr, nullptr, nullptr };   // s12, s13, w, seg
+    void* owned[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };   // s12, s13, w, seg, rec
+};
+
+// RAII range for profilers: shows the C-ABI entry points on an Nsight timeline; costs nothing
+// when no tool is attached
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
 };
 
 }  // namespace
@@ -54,11 +64,8 @@ struct mipwa_ctx {
 
     // natural-spline system (A2): the tridiagonal matrix depends on the knots only -> factor once
     std::vector<double> sp_sub, sp_inv, sp_cp;     // sub-diagonal, 1/pivot, modified super-diagonal
-    std::vector<uint8_t> lut;
-    std::vector<double> xk;
-    bool lut_exact = false;
-    int nlut = 0;
-    double lut_x0 = 0, lut_inv = 0;
+    DevSearch search;               // knot search table (knots only): host copy, uploaded once to d_search
+    DevSearch* d_search = nullptr;
 
     Slot ev, nm;
 
@@ -66,8 +73,9 @@ struct mipwa_ctx {
     int blocks_per_sm = 0;
     double2* d_partials = nullptr;
     unsigned int* d_ticket = nullptr;
-    double* h_result = nullptr;     // mapped pinned: [0] sum ln|A|^2, [1] sum w|A|^2, [2..] spare
+    double* h_result = nullptr;     // mapped pinned: [0] sum ln|A|^2, [1] sum w|A|^2, [2] tag of the call that wrote them
     double* d_result = nullptr;     // device alias of h_result
+    long long tag = 0;              // number of value-kernel launches: what publish_result writes into slot 2
     unsigned long long* h_bad = nullptr;
     unsigned long long* d_bad = nullptr;
 
@@ -97,17 +105,17 @@ struct mipwa_ctx {
     void* d_hyb_ev = nullptr; void* d_hyb_nm = nullptr;
     int64_t hyb_ev_bytes = 0, hyb_nm_bytes = 0;
     bool hyb_ev_valid = false, hyb_nm_valid = false;
-    int hyb_blocks_per_sm = 0, hyb_grad_blocks_per_sm = 0;
+    int hyb_blocks_per_sm = 0;
 
     // gradient (A8): cell-sorted copies of both point sets, per-block partial vectors
     Slot ev_sorted, nm_sorted;
     bool ev_sorted_valid = false, nm_sorted_valid = false;
-    int grad_blocks_per_sm = 0;
+    size_t grad_smem_set[2][3] = { { 0, 0, 0 }, { 0, 0, 0 } };   // dynamic shared memory granted to k_grad_recompute<mix, shp>
+    size_t gcompact_smem_set = 0;
     double* d_gpartials = nullptr;
     size_t gpartials_len = 0;
     double2* d_f_ev = nullptr; double2* d_f_nm = nullptr;   // per-point gradient factors for k_grad_shape
     int64_t f_ev_len = 0, f_nm_len = 0;
-    bool want_f = false;
     double res_fold[MIPWA_MAX_RESONANCES];   // sqrt(n_R n_D) of device slot d for the current call
 
     bool timing = false;
@@ -160,6 +168,8 @@ int resonance_constants(mipwa_ctx* c, int r, double m0, double g0, double cmag, 
     out->pa = L == 2 ? 1.0 : 0.0;
     out->pb = L == 2 ? 3.0 : (L == 1 ? 1.0 : 0.0);
     out->pc = L == 2 ? 9.0 : 1.0;
+    out->qR1 = 3.0 * out->cR; out->qR2 = out->cR * out->cR;
+    out->qD1 = 3.0 * out->cD; out->qD2 = out->cD * out->cD;
     out->L = L;
     out->fl = -1;
     // shape derivatives: only q0^2 and p0*^2 depend on m0 (include/mipwa.h, mipwa_nll_grad_full)
@@ -209,42 +219,42 @@ void spline_factor(mipwa_ctx* c)
     }
     // bucket table for the segment lookup: lut[b] = segment containing the left edge of bucket b, xk[b] = the
     // interior knot inside bucket b.  Buckets no wider than 0.9 x the smallest knot spacing hold at most one knot.
+    DevSearch& t = c->search;
+    std::memset(&t, 0, sizeof(t));
     double minsp = x[1] - x[0];
     for (int i = 1; i < n - 1; ++i) minsp = std::min(minsp, x[i + 1] - x[i]);
     const double range = x[n - 1] - x[0];
     const double want = std::ceil(range / (0.9 * minsp));
-    c->nlut = (int)std::min<double>(MIPWA_DEV_LUT, std::max<double>(64.0, want));
-    c->lut_exact = range / c->nlut <= 0.9 * minsp;
-    c->lut_x0 = x[0];
-    c->lut_inv = c->nlut / range;
-    c->lut.assign(c->nlut, 0);
-    c->xk.assign(c->nlut, HUGE_VAL);
-    for (int b = 0; b < c->nlut; ++b) {
-        const double lo = x[0] + b / c->lut_inv, hi = x[0] + (b + 1) / c->lut_inv;
+    t.N = n;
+    t.nlut = (int)std::min<double>(MIPWA_DEV_LUT, std::max<double>(64.0, want));
+    t.lut_exact = range / t.nlut <= 0.9 * minsp ? 1 : 0;
+    t.lut_inv = t.nlut / range;
+    t.lut_off = -x[0] * t.lut_inv;
+    for (int i = 0; i < n; ++i) t.knots[i] = x[i];
+    for (int b = 0; b < t.nlut; ++b) {
+        const double lo = x[0] + b / t.lut_inv, hi = x[0] + (b + 1) / t.lut_inv;
         int j = 0;
         while (j < n - 2 && lo >= x[j + 1]) ++j;
-        c->lut[b] = (uint8_t)j;
-        if (j + 1 <= n - 2 && x[j + 1] < hi) c->xk[b] = x[j + 1];
+        t.lut[b] = (uint8_t)j;
+        t.xk[b] = (j + 1 <= n - 2 && x[j + 1] < hi) ? x[j + 1] : HUGE_VAL;
     }
 }
 
-// the parameter-independent part of DevModel (kinematics, knots, bucket table): valid from mipwa_create on, so that
-// k_validate can compute segment pairs before any likelihood call
+// the parameter-independent part of DevModel (kinematics, knot positions of the rows)
 void fill_static_model(mipwa_ctx* c)
 {
     DevModel& m = c->model;
     const mipwa_kinematics& k = c->kin;
-    m.N = c->N; m.R = c->R; m.nlut = c->nlut; m.lut_exact = c->lut_exact ? 1 : 0;
+    m.N = c->N; m.R = c->R;
     m.t_lo = (k.m1 + k.m2) * (k.m1 + k.m2);
     m.t_d = (k.m1 - k.m2) * (k.m1 - k.m2);
     m.s_hi = (k.m_parent - k.m3) * (k.m_parent - k.m3);
     m.s_top = (k.m_parent + k.m3) * (k.m_parent + k.m3);
     m.sigma = k.m_parent * k.m_parent + k.m1 * k.m1 + k.m2 * k.m2 + k.m3 * k.m3;
     m.kappa = (k.m_parent * k.m_parent - k.m3 * k.m3) * (k.m2 * k.m2 - k.m1 * k.m1);
-    m.lut_off = -c->lut_x0 * c->lut_inv; m.lut_inv = c->lut_inv;
-    std::memcpy(m.lut, c->lut.data(), c->nlut);
-    std::memcpy(m.xk, c->xk.data(), c->nlut * sizeof(double));
-    for (int i = 0; i < c->N; ++i) m.knots[i] = c->knots[i];
+    m.k_third = -1.0 / 3.0;
+    m.lam2_b = -(m.s_hi + m.s_top); m.lam2_c = m.s_hi * m.s_top;
+    for (int i = 0; i < c->N; ++i) m.rows[i * MIPWA_ROW] = make_double2(c->knots[i], 0.0);
 }
 
 // A1-A3: parameters -> DevModel
@@ -256,7 +266,6 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
     for (int64_t i = 0; i < n_params; ++i)
         if (!std::isfinite(p[i])) return fail(c, MIPWA_ERR_ARG, "non-finite parameter " + std::to_string(i));
     DevModel& m = c->model;
-    fill_static_model(c);
     for (int i = 0; i < N; ++i) {
         c->y_re[i] = p[i] * std::cos(p[N + i]);            // y_k = a_k e^{i phi_k}
         c->y_im[i] = p[i] * std::sin(p[N + i]);
@@ -274,9 +283,9 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
             co[2][q] = 0.5 * P[q][j];
             co[3][q] = (P[q][j + 1] - P[q][j]) / (6.0 * h);
         }
-        for (int q = 0; q < 4; ++q) m.sc[q][j] = make_double2(co[q][0], co[q][1]);
+        for (int q = 0; q < 4; ++q) m.rows[j * MIPWA_ROW + 1 + q] = make_double2(co[q][0], co[q][1]);
     }
-    for (int q = 0; q < 4; ++q) m.sc[q][N - 1] = make_double2(0.0, 0.0);
+    for (int q = 0; q < 4; ++q) m.rows[(N - 1) * MIPWA_ROW + 1 + q] = make_double2(0.0, 0.0);
     std::vector<int> fidx(R, -1);
     for (int r = 0, f = 0; r < R; ++r) if (c->res[r].shape_floats) fidx[r] = f++;
     const std::vector<int>& slots = c->active ? *c->active : c->perm;
@@ -312,12 +321,111 @@ void free_slot(Slot& s)
     s = Slot();
 }
 
+void drop_records(Slot& s)
+{
+    if (s.owned[4]) cudaFree(s.owned[4]);
+    s.owned[4] = nullptr; s.rec = nullptr;
+}
+
+// records past the end of a point set that the prefetching loops may LOAD (never evaluate), in records
+int64_t record_pad(const mipwa_ctx* c) { return (int64_t)c->sm_count * 2048; }
+
+// The 32-byte records of a point set (kernels.cuh: k_make_records), built on first use.  w_default: the weight of a
+// normalisation point without weights (1: the caller of the kernel divides by n), 0 for events without background
+// densities.  The tail [n, n + pad) holds copies of record 0 with weight 0 (zeros if the set is empty).
+int ensure_records(mipwa_ctx* c, Slot& s, double w_default)
+{
+    if (s.rec) return MIPWA_OK;
+    const int64_t pad = record_pad(c), n = std::max<int64_t>(s.n, 0);
+    if (!s.owned[4]) CU(c, cudaMalloc(&s.owned[4], (size_t)(n + pad) * sizeof(PointRec)));
+    PointRec* rec = (PointRec*)s.owned[4];
+    CU(c, cudaMemsetAsync(rec + n, 0, (size_t)pad * sizeof(PointRec), c->stream));
+    if (n > 0) {
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * 8, (n + MIPWA_BLOCK - 1) / MIPWA_BLOCK));
+        k_make_records<<<grid, MIPWA_BLOCK, 0, c->stream>>>(s.s12, s.s13, s.w, w_default, s.seg, n, rec);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+        k_pad_records<<<(int)std::min<int64_t>(c->sm_count, (pad + MIPWA_BLOCK - 1) / MIPWA_BLOCK), MIPWA_BLOCK, 0, c->stream>>>(rec, n, pad);
+        ++c->launches;
+        CU(c, cudaGetLastError());
+    }
+    s.rec = rec;
+    return MIPWA_OK;
+}
+
 }  // namespace
 
 
 // the library's working view of a point set: the cell-sorted copy once mipwa_prepare / mipwa_nll_grad built it
-static inline const Slot& evs(const mipwa_ctx* c) { return c->ev_sorted_valid ? c->ev_sorted : c->ev; }
-static inline const Slot& nms(const mipwa_ctx* c) { return c->nm_sorted_valid ? c->nm_sorted : c->nm; }
+static inline Slot& evs(mipwa_ctx* c) { return c->ev_sorted_valid ? c->ev_sorted : c->ev; }
+static inline Slot& nms(mipwa_ctx* c) { return c->nm_sorted_valid ? c->nm_sorted : c->nm; }
+
+// tag of the next value-kernel launch; clears the word the kernel will publish it in (a gradient call may have left
+// anything there)
+static long long next_tag(mipwa_ctx* c)
+{
+    *reinterpret_cast<volatile long long*>(c->h_result + MIPWA_RESULT_TAG) = 0;
+    return ++c->tag;
+}
+
+// start of the timed region of a call (timing mode only): spacer kernel, then the first event (kernels.cuh: k_spacer)
+static int timing_begin(mipwa_ctx* c)
+{
+    if (!c->timing) return MIPWA_OK;
+    k_spacer<<<1, 1, 0, c->stream>>>(40000ULL);
+    CU(c, cudaGetLastError());
+    CU(c, cudaEventRecord(c->ev0, c->stream));
+    return MIPWA_OK;
+}
+
+// Wait for the value kernel that carries `tag`: its last block writes the totals into mapped pinned memory and then the
+// tag (publish_result).  Polling that word for a while before blocking saves the wake-up latency of
+// cudaStreamSynchronize, which at the paper's sample sizes (1e4-1e5 events) is as long as the kernel itself.
+static int wait_result(mipwa_ctx* c, long long tag)
+{
+    if (c->timing) {
+        CU(c, cudaEventRecord(c->ev1, c->stream));
+        CU(c, cudaEventSynchronize(c->ev1));
+        CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+        return MIPWA_OK;
+    }
+    volatile long long* flag = reinterpret_cast<volatile long long*>(c->h_result + MIPWA_RESULT_TAG);
+    for (int spin = 0; spin < 200000; ++spin) {
+        if (*flag == tag) return MIPWA_OK;
+        if ((spin & 0x3fff) == 0x3fff) {                   // a faulted kernel never publishes: ask the driver now and then
+            const cudaError_t e = cudaStreamQuery(c->stream);
+            if (e != cudaSuccess && e != cudaErrorNotReady) return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e));
+        }
+    }
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MIPWA_OK;
+}
+
+// sustained rate of one of the k_fp64_peak loops (kernels.cuh), best launch over about `seconds` seconds
+template <int MODE>
+static int fp64_rate(const cudaDeviceProp& prop, double seconds, double* tflops)
+{
+    double* d = nullptr;
+    cudaEvent_t a, b;
+    if (cudaMalloc(&d, 64) != cudaSuccess || cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return MIPWA_ERR_CUDA;
+    const int grid = prop.multiProcessorCount * 8, block = 256;
+    long long iters = 2000;
+    double best = 0, spent = 0;
+    for (int rep = 0; rep < 64 && spent < seconds; ++rep) {
+        cudaEventRecord(a);
+        k_fp64_peak<MODE><<<grid, block>>>(d, iters, MODE == 0 ? 0.999999 : 0x1p-60, 1e-9);
+        cudaEventRecord(b);
+        if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(d); return MIPWA_ERR_CUDA; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, a, b);
+        const double fl = 2.0 * 64.0 * (double)iters * grid * block;   // 64 DFMAs per thread and iteration
+        if (rep > 0) { best = std::max(best, fl / (ms * 1e-3) * 1e-12); spent += ms * 1e-3; }
+        if (ms < 50.0f) iters *= 2;                        // grow each launch to ~0.1 s
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d);
+    *tflops = best;
+    return MIPWA_OK;
+}
 
 // =================================================================================================================
 // C ABI
@@ -359,9 +467,12 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     c->knots.assign(knots, knots + n_knots);
     if (n_res) c->res.assign(res, res + n_res);
     for (int r = 0; r < n_res; ++r) c->F += res[r].shape_floats ? 1 : 0;
+    // device slots: spin 1, then spin 2, then spin 0; within a spin the floating resonances first (k_grad_recompute
+    // folds the shape derivatives of the FIRST slot of a spin into its pass), then the caller's order
     for (int L : { 1, 2, 0 })
-        for (int r = 0; r < n_res; ++r)
-            if (res[r].spin == L) { c->perm.push_back(r); ++c->n_spin[L]; }
+        for (int fl : { 1, 0 })
+            for (int r = 0; r < n_res; ++r)
+                if (res[r].spin == L && (res[r].shape_floats ? 1 : 0) == fl) { c->perm.push_back(r); ++c->n_spin[L]; }
     for (int L : { 1, 2 })
         for (int r = 0; r < n_res; ++r)
             if (res[r].shape_floats && res[r].spin == L) { c->hyb_float.push_back(r); (L == 1 ? c->hyb_f1 : c->hyb_f2)++; }
@@ -380,9 +491,6 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
                     shared = false;
         if (shared) c->model_flags |= MIPWA_FL_SHR;
     }
-#ifdef MIPWA_NO_MODEL_FLAGS
-    c->model_flags = 0;                                    // experiments only
-#endif
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
     c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
@@ -400,22 +508,21 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     }
 
     bool ok = true;
-    ok = mipwa_occupancy_nll_recompute(c->n_spin, c->model_flags, &c->blocks_per_sm) == cudaSuccess;
-    if (c->blocks_per_sm < 1) c->blocks_per_sm = 1;
-#ifdef MIPWA_FORCE_BPS
-    c->blocks_per_sm = MIPWA_FORCE_BPS;                    // experiments only
-#endif
+    c->blocks_per_sm = 1;                                  // k_nll_recompute: one 512-thread block per SM
     const size_t max_grid = (size_t)c->sm_count * 16;
     ok = ok && cudaMalloc(&c->d_partials, max_grid * sizeof(double2) * 64) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_ticket, 64) == cudaSuccess && cudaMemset(c->d_ticket, 0, 64) == cudaSuccess;
     ok = ok && cudaHostAlloc(&c->h_result, 4096 * sizeof(double), cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer(&c->d_result, c->h_result, 0) == cudaSuccess;
+    if (ok) std::memset(c->h_result, 0, 4096 * sizeof(double));   // recycled pinned memory: no stale tag of an older context
     ok = ok && cudaHostAlloc(&c->h_bad, 64, cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer(&c->d_bad, c->h_bad, 0) == cudaSuccess;
     ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_Mx, c->Mx.size() * sizeof(double)) == cudaSuccess &&
          cudaMemcpy(c->d_Mx, c->Mx.data(), c->Mx.size() * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_gram, (size_t)(n_knots + n_res) * (n_knots + n_res) * sizeof(double2)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->d_search, sizeof(DevSearch)) == cudaSuccess &&
+         cudaMemcpy(c->d_search, &c->search, sizeof(DevSearch), cudaMemcpyHostToDevice) == cudaSuccess;
     if (!ok) { mipwa_destroy(c); return MIPWA_ERR_CUDA; }
     *out = c;
     return MIPWA_OK;
@@ -430,6 +537,7 @@ void mipwa_destroy(mipwa_ctx* c)
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_ticket) cudaFree(c->d_ticket);
     if (c->d_Mx) cudaFree(c->d_Mx);
+    if (c->d_search) cudaFree(c->d_search);
     if (c->owned_cache) cudaFree(c->owned_cache);
     if (c->d_gram) cudaFree(c->d_gram);
     if (c->d_gpartials) cudaFree(c->d_gpartials);
@@ -469,11 +577,13 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
     if (rc) return rc;
     CU(c, cudaStreamSynchronize(c->stream));
     Slot s;
-    if (mem == MIPWA_MEM_HOST && n > 0 && slot.n == n && slot.owned[0] && slot.owned[1]) {
-        for (int q = 0; q < 4; ++q) { s.owned[q] = slot.owned[q]; slot.owned[q] = nullptr; }   // same size: reuse
-        if (!w && s.owned[2]) { cudaFree(s.owned[2]); s.owned[2] = nullptr; }
-    } else if (n > 0 && slot.n == n && slot.owned[3]) {
-        s.owned[3] = slot.owned[3]; slot.owned[3] = nullptr;                                    // segment pairs: reuse
+    if (n > 0 && slot.n == n) {                            // same size as before: reuse the library-owned storage
+        if (mem == MIPWA_MEM_HOST && slot.owned[0] && slot.owned[1]) {
+            for (int q = 0; q < 3; ++q) { s.owned[q] = slot.owned[q]; slot.owned[q] = nullptr; }
+            if (!w && s.owned[2]) { cudaFree(s.owned[2]); s.owned[2] = nullptr; }
+        }
+        s.owned[3] = slot.owned[3]; slot.owned[3] = nullptr;                                    // segment pairs
+        s.owned[4] = slot.owned[4]; slot.owned[4] = nullptr;                                    // records (rebuilt on use)
     }
     free_slot(slot);
     if (mem == MIPWA_MEM_HOST && n > 0) {
@@ -506,7 +616,7 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
                       (k.m1 + k.m2) * (k.m1 + k.m2), (k.m1 - k.m2) * (k.m1 - k.m2),
                       (k.m_parent - k.m3) * (k.m_parent - k.m3), (k.m_parent + k.m3) * (k.m_parent + k.m3) };
         *c->h_bad = 0;
-        k_validate<<<grid_for(c, n, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, c->model, s.s12, s.s13, n,
+        k_validate<<<grid_for(c, n, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, c->d_search, s.s12, s.s13, n,
                                                                      (unsigned short*)s.owned[3], c->d_bad);
         ++c->launches;
         cudaError_t e = cudaGetLastError();
@@ -524,13 +634,17 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
 
 int mipwa_set_events(mipwa_ctx* c, const double* s12, const double* s13, int64_t n, int32_t mem)
 {
-    if (c) { c->cache_valid = false; c->ev_sorted_valid = false; c->hyb_ev_valid = false; }
+    if (!c) return MIPWA_ERR_ARG;
+    NvtxRange range("mipwa_set_events");
+    c->cache_valid = false; c->ev_sorted_valid = false; c->hyb_ev_valid = false;
     return set_slot(c, c->ev, s12, s13, nullptr, n, mem, true);
 }
 
 int mipwa_set_norm_points(mipwa_ctx* c, const double* s12, const double* s13, const double* w, int64_t n, int32_t mem)
 {
-    if (c) { c->gram_valid = false; c->nm_sorted_valid = false; c->hyb_nm_valid = false; }
+    if (!c) return MIPWA_ERR_ARG;
+    NvtxRange range("mipwa_set_norm_points");
+    c->gram_valid = false; c->nm_sorted_valid = false; c->hyb_nm_valid = false;
     return set_slot(c, c->nm, s12, s13, w, n, mem, false);
 }
 
@@ -553,20 +667,30 @@ int mipwa_set_path(mipwa_ctx* c, int32_t path)
     return MIPWA_OK;
 }
 
+// grid of the recompute kernels: one 512-thread block per SM, fewer for small samples
+static int recompute_grid(const mipwa_ctx* c, int64_t n)
+{
+    const int64_t need = (n + MIPWA_REC_BLOCK - 1) / MIPWA_REC_BLOCK;
+    return (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
+}
+
 static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
 {
-    const int64_t need = (std::max(c->ev.n, c->nm.n) + MIPWA_REC_BLOCK - 1) / MIPWA_REC_BLOCK;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, evs(c).s12,
-                                                      evs(c).s13, evs(c).seg, nullptr, 0.0, evs(c).n, nms(c).s12,
-                                                      nms(c).s13, nms(c).w, nms(c).seg, nms(c).n, c->d_partials,
-                                                      c->d_ticket, c->d_result);
+    Slot& E = evs(c);
+    Slot& G = nms(c);
+    int rc = ensure_records(c, E, 0.0);
+    if (rc) return rc;
+    rc = ensure_records(c, G, 1.0);
+    if (rc) return rc;
+    const int grid = recompute_grid(c, std::max(E.n, G.n));
+    { const int trc = timing_begin(c); if (trc) return trc; }
+    const long long tag = next_tag(c);
+    const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0,
+                                                      E.n, G.rec, G.n, c->d_partials, c->d_ticket, c->d_result, tag);
     ++c->launches;
     CU(c, le);
-    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    rc = wait_result(c, tag);
+    if (rc) return rc;
     *sum_log = c->h_result[0];
     *integral = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
     return MIPWA_OK;
@@ -635,11 +759,11 @@ static int ensure_cache(mipwa_ctx* c, int kind)
         const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
         const int grid = (int)std::min<int64_t>(tiles, (int64_t)c->sm_count * 8);
         if (kind == MIPWA_PATH_CACHED)
-            k_basis_build<false><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), evs(c).s12, evs(c).s13,
-                                                                      c->ev.n, (double2*)c->d_cache);
+            k_basis_build<false><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, c->d_search, basis_aux(c), evs(c).s12,
+                                                                      evs(c).s13, c->ev.n, (double2*)c->d_cache);
         else
-            k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), evs(c).s12, evs(c).s13,
-                                                                     c->ev.n, (double2*)c->d_cache);
+            k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, c->d_search, basis_aux(c), evs(c).s12,
+                                                                     evs(c).s13, c->ev.n, (double2*)c->d_cache);
         ++c->launches;
         CU(c, cudaGetLastError());
         CU(c, cudaStreamSynchronize(c->stream));
@@ -668,8 +792,9 @@ static int ensure_gram(mipwa_ctx* c)
     do {                                                                                                             \
         e = cudaFuncSetAttribute(k_gram<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
         if (e == cudaSuccess)                                                                                        \
-            k_gram<T, false><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), cdummy, nms(c).s12,      \
-                                                                     nms(c).s13, nms(c).w, c->nm.n, wd, partial);    \
+            k_gram<T, false><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, c->d_search, basis_aux(c), cdummy,     \
+                                                                     nms(c).s12, nms(c).s13, nms(c).w, c->nm.n, wd,  \
+                                                                     partial);                                       \
     } while (0)
     if (tpt <= 1) MIPWA_GRAM_LAUNCH(1); else if (tpt == 2) MIPWA_GRAM_LAUNCH(2); else MIPWA_GRAM_LAUNCH(3);
 #undef MIPWA_GRAM_LAUNCH
@@ -713,7 +838,8 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
     fill_coef(c, params, &cc);
     const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
     const double2* cache = (const double2*)c->d_cache;
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    { const int trc = timing_begin(c); if (trc) return trc; }
+    const long long tag = next_tag(c);
     if (kind == MIPWA_PATH_CACHED) {
         if (!c->dense_blocks_per_sm) {
             CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->dense_blocks_per_sm, k_nll_dense, MIPWA_TILE, 0));
@@ -721,7 +847,7 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
         }
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->dense_blocks_per_sm));
         k_nll_dense<<<grid, MIPWA_TILE, 0, c->stream>>>(cc, cache, c->ev.n, c->d_gram, (double*)c->d_partials,
-                                                         c->d_ticket, c->d_result);
+                                                         c->d_ticket, c->d_result, tag);
     } else {
         if (!c->compact_blocks_per_sm) {
             CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->compact_blocks_per_sm, k_nll_compact<-1>, MIPWA_TILE, 0));
@@ -730,7 +856,7 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->compact_blocks_per_sm));
 #define MIPWA_COMPACT_LAUNCH(T)                                                                                   \
     k_nll_compact<T><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, cc, cache, evs(c).seg, c->ev.n, c->d_gram,    \
-                                                          (double*)c->d_partials, c->d_ticket, c->d_result)
+                                                          (double*)c->d_partials, c->d_ticket, c->d_result, tag)
         switch (c->R) {
             case 0: MIPWA_COMPACT_LAUNCH(0); break;
             case 1: MIPWA_COMPACT_LAUNCH(1); break;
@@ -744,9 +870,8 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
     }
     ++c->launches;
     CU(c, cudaGetLastError());
-    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    rc = wait_result(c, tag);
+    if (rc) return rc;
     *sum_log = c->h_result[0];
     *integral = c->h_result[1];
     return MIPWA_OK;
@@ -777,7 +902,8 @@ static int ensure_hyb_cache(mipwa_ctx* c, const Slot& pts, void** buf, int64_t* 
         if (rc) return rc;
         const int64_t tiles = (pts.n + MIPWA_TILE - 1) / MIPWA_TILE;
         const int grid = (int)std::min<int64_t>(tiles, (int64_t)c->sm_count * 8);
-        k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, aux, pts.s12, pts.s13, pts.n, (double2*)*buf);
+        k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, c->d_search, aux, pts.s12, pts.s13, pts.n,
+                                                                 (double2*)*buf);
         ++c->launches;
         CU(c, cudaGetLastError());
         CU(c, cudaStreamSynchronize(c->stream));
@@ -813,16 +939,16 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     const int64_t tpb = mipwa_hybrid_tiles_per_block(RC);
     const int64_t tiles = (std::max(c->ev.n, c->nm.n) + MIPWA_TILE - 1) / MIPWA_TILE;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((tiles + tpb - 1) / tpb, (int64_t)c->sm_count * c->hyb_blocks_per_sm));
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+    { const int trc = timing_begin(c); if (trc) return trc; }
+    const long long tag = next_tag(c);
     const cudaError_t le = mipwa_launch_nll_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, grid, c->stream, c->model, cc,
                                                    (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n,
                                                    (const double2*)c->d_hyb_nm, nms(c).w, nms(c).seg, c->nm.n,
-                                                   c->d_partials, c->d_ticket, c->d_result);
+                                                   c->d_partials, c->d_ticket, c->d_result, tag);
     ++c->launches;
     CU(c, le);
-    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    rc = wait_result(c, tag);
+    if (rc) return rc;
     *sum_log = c->h_result[0];
     *integral = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
     return MIPWA_OK;
@@ -831,6 +957,7 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
 int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* sum_log, double* integral)
 {
     if (!c || !params || !nll) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    NvtxRange range("mipwa_nll");
     if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
     int rc = use_device(c);
     if (rc) return rc;
@@ -885,31 +1012,14 @@ int mipwa_last_kernel_ms(const mipwa_ctx* c, float* ms)
 
 int64_t mipwa_launch_count(const mipwa_ctx* c) { return c ? c->launches : -1; }
 
-int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops)
+int mipwa_measure_fp64_peak(int32_t device, double seconds, double* tflops, double* tflops_3reg)
 {
     if (!tflops || !(seconds > 0)) return MIPWA_ERR_ARG;
     cudaDeviceProp prop;
     if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) return MIPWA_ERR_CUDA;
-    double* d = nullptr;
-    cudaEvent_t a, b;
-    if (cudaMalloc(&d, 64) != cudaSuccess || cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return MIPWA_ERR_CUDA;
-    const int grid = prop.multiProcessorCount * 8, block = 256;
-    long long iters = 2000;
-    double best = 0, spent = 0;
-    for (int rep = 0; rep < 64 && spent < seconds; ++rep) {
-        cudaEventRecord(a);
-        k_dfma_peak<<<grid, block>>>(d, iters, 0.999999, 1e-9);
-        cudaEventRecord(b);
-        if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(d); return MIPWA_ERR_CUDA; }
-        float ms = 0;
-        cudaEventElapsedTime(&ms, a, b);
-        const double fl = 2.0 * 64.0 * (double)iters * grid * block;
-        if (rep > 0) { best = std::max(best, fl / (ms * 1e-3) * 1e-12); spent += ms * 1e-3; }
-        if (ms < 50.0f) iters *= 2;                        // grow each launch to ~0.1 s
-    }
-    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d);
-    *tflops = best;
-    return MIPWA_OK;
+    int rc = fp64_rate<1>(prop, tflops_3reg ? 0.5 * seconds : seconds, tflops);
+    if (rc == MIPWA_OK && tflops_3reg) rc = fp64_rate<0>(prop, 0.5 * seconds, tflops_3reg);
+    return rc;
 }
 
 }  // extern "C"
@@ -956,7 +1066,8 @@ int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32
     const int K = c->N + c->R;
     double2* d_out = nullptr;
     CU(c, cudaMalloc(&d_out, (size_t)n * K * sizeof(double2)));
-    k_basis_rows<<<grid_for(c, n, 4), MIPWA_TILE, 0, c->stream>>>(c->model, basis_aux(c), s.s12, s.s13, first, n, d_out);
+    k_basis_rows<<<grid_for(c, n, 4), MIPWA_TILE, 0, c->stream>>>(c->model, c->d_search, basis_aux(c), s.s12, s.s13, first, n,
+                                                                  d_out);
     ++c->launches;
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
@@ -1096,7 +1207,7 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
     CoefDev cc;
     fill_coef(c, params, &cc);
     const int N = c->N, R = c->R, K = N + R, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;
-    const size_t smem = (size_t)nb * sizeof(double);
+    const size_t smem = (size_t)(MIPWA_TILE / 32) * nb * sizeof(double);   // one set of segment bins per warp
     const int grid = grid_for(c, c->ev.n, 2);
     if (c->gpartials_len < (size_t)grid * NV) {
         if (c->d_gpartials) cudaFree(c->d_gpartials);
@@ -1105,9 +1216,15 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
         c->gpartials_len = (size_t)grid * NV;
     }
     const double2* cache = (const double2*)c->d_cache;
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-#define MIPWA_GC_LAUNCH(T) \
-    k_grad_compact<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, cc, cache, c->ev.n, c->d_gpartials)
+    { const int trc = timing_begin(c); if (trc) return trc; }
+#define MIPWA_GC_LAUNCH(T)                                                                                             \
+    do {                                                                                                               \
+        if (c->gcompact_smem_set < smem) {                                                                             \
+            CU(c, cudaFuncSetAttribute(k_grad_compact<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));   \
+            c->gcompact_smem_set = smem;                                                                               \
+        }                                                                                                              \
+        k_grad_compact<T><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, cc, cache, evs(c).seg, c->ev.n, c->d_gpartials); \
+    } while (0)
     switch (R) {
         case 0: MIPWA_GC_LAUNCH(0); break;
         case 1: MIPWA_GC_LAUNCH(1); break;
@@ -1120,7 +1237,7 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
 #undef MIPWA_GC_LAUNCH
     ++c->launches;
     CU(c, cudaGetLastError());
-    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
+    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, grid, NV, 1, c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
@@ -1165,150 +1282,109 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
     return MIPWA_OK;
 }
 
-// A8 on the hybrid path: k_grad_hybrid over the cell-sorted points, fixed-shape terms from the per-point caches
-static int nll_grad_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+// ---- A8 on the recompute path -----------------------------------------------------------------------------------------
+// One launch of k_grad_recompute over both cell-sorted record sets and one of k_grad_finalize; the totals land in
+// h_result as [event vector | normalisation vector], each of NVB = 2 + 2R + 8 (N-1) + 4 doubles laid out like the block
+// partials of grad.cuh.  n_ev / n_norm = 0 leaves that set out (the two launches of the mixture likelihood).
+struct GradTotals {
+    int NVB, nb;
+    const double *ev, *nm;                                 // the two vectors
+    const double* F(const double* v) const { return v + 2; }
+    const double* bins(const double* v, int R) const { return v + 2 + 2 * R; }
+    const double* shape(const double* v, int R) const { return v + 2 + 2 * R + nb; }
+};
+
+static int launch_grad_recompute(mipwa_ctx* c, bool mix, int shp, double kappa, bool with_ev, bool with_nm, bool want_f,
+                                 GradTotals* out)
 {
-    int rc = ensure_hyb_cache(c, evs(c), &c->d_hyb_ev, &c->hyb_ev_bytes, &c->hyb_ev_valid);   // sorted order: prepare_sorted ran
+    Slot& E = c->ev_sorted;
+    Slot& G = c->nm_sorted;
+    int rc = ensure_records(c, E, 0.0);
     if (rc) return rc;
-    rc = ensure_hyb_cache(c, nms(c), &c->d_hyb_nm, &c->hyb_nm_bytes, &c->hyb_nm_valid);
+    rc = ensure_records(c, G, 1.0);
     if (rc) return rc;
-    c->active = &c->hyb_float;                             // spline tables + the floating resonances of this call
-    rc = build_model(c, params, n_params);
-    c->active = nullptr;
-    if (rc) return rc;
-    const int N = c->N, R = c->R, F = (int)c->hyb_float.size(), RC = (int)c->hyb_fixed.size(), RT = F + RC;
-    const int NS = N - 1, nb = 8 * NS, NV = 2 + 4 * RT + 2 * nb;
-    HybCoef cc;
-    cc.RC = RC; cc.pad = 0;
-    for (int k = 0; k < RC; ++k) {
-        const int r = c->hyb_fixed[k];
-        cc.c[k] = make_double2(params[2 * N + 2 * r] * std::cos(params[2 * N + 2 * r + 1]),
-                               params[2 * N + 2 * r] * std::sin(params[2 * N + 2 * r + 1]));
+    const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NVB = 2 + 2 * R + nb + 4;
+    const int64_t n_ev = with_ev ? E.n : 0, n_nm = with_nm ? G.n : 0;
+    const int ev_blocks = n_ev > 0 ? recompute_grid(c, n_ev) : 0, nm_blocks = n_nm > 0 ? recompute_grid(c, n_nm) : 0;
+    const int grid = std::max(1, ev_blocks + nm_blocks);
+    const size_t smem = (size_t)(MIPWA_GRAD_BLOCK / 32) * nb * sizeof(double);
+    if (smem > 200 * 1024) return fail(c, MIPWA_ERR_ARG, "mipwa_nll_grad: too many knots for the per-warp segment bins");
+    if (c->grad_smem_set[mix ? 1 : 0][shp] < std::max<size_t>(smem, 1)) {
+        if (mipwa_grad_set_smem(c->n_spin, c->model_flags, mix, shp, smem) != cudaSuccess)
+            return fail(c, MIPWA_ERR_CUDA, "k_grad_recompute: shared-memory request refused");
+        c->grad_smem_set[mix ? 1 : 0][shp] = std::max<size_t>(smem, 1);
     }
-    const size_t smem = (size_t)2 * nb * sizeof(double);
-    if (!c->hyb_grad_blocks_per_sm) {
-        if (mipwa_occupancy_grad_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, smem, &c->hyb_grad_blocks_per_sm) != cudaSuccess)
-            return fail(c, MIPWA_ERR_CUDA, "hybrid gradient: occupancy query failed");
-        if (c->hyb_grad_blocks_per_sm < 1) c->hyb_grad_blocks_per_sm = 1;
-    }
-    const int64_t gneed = (std::max(c->ev.n, c->nm.n) + MIPWA_GRAD_BLOCK - 1) / MIPWA_GRAD_BLOCK;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->hyb_grad_blocks_per_sm, gneed));
-    if (c->gpartials_len < (size_t)grid * NV) {
+    if (c->gpartials_len < (size_t)grid * NVB) {
         if (c->d_gpartials) cudaFree(c->d_gpartials);
         c->d_gpartials = nullptr; c->gpartials_len = 0;
-        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NV * sizeof(double)));
-        c->gpartials_len = (size_t)grid * NV;
+        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NVB * sizeof(double)));
+        c->gpartials_len = (size_t)grid * NVB;
     }
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    const cudaError_t le = mipwa_launch_grad_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, grid, smem, c->stream, c->model, cc,
-                                                    c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg,
-                                                    (const double2*)c->d_hyb_ev, c->ev_sorted.n, c->nm_sorted.s12,
-                                                    c->nm_sorted.s13, c->nm_sorted.w, c->nm_sorted.seg,
-                                                    (const double2*)c->d_hyb_nm, c->nm_sorted.n, c->d_gpartials,
-                                                    c->want_f ? c->d_f_ev : nullptr, c->want_f ? c->d_f_nm : nullptr);
+    const cudaError_t le = mipwa_launch_grad_recompute(c->n_spin, c->model_flags, mix, shp, grid, ev_blocks, smem, c->stream,
+                                                       c->model, E.rec, kappa, n_ev, G.rec, n_nm, c->d_gpartials,
+                                                       want_f ? c->d_f_ev : nullptr, want_f ? c->d_f_nm : nullptr);
     ++c->launches;
     CU(c, le);
-    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
+    k_grad_finalize<<<(2 * NVB + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, ev_blocks, ev_blocks + nm_blocks, NVB, 2,
+                                                              c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());
-    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
-
-    // host combine as in mipwa_nll_grad; slot d < F: floating resonance hyb_float[d] (T without sqrt(n_R n_D): fold it
-    // back), slot F + k: fixed resonance hyb_fixed[k] (the cache column carries the factor)
-    const double* h = c->h_result;
-    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
-    const double S = h[0], I = h[1] * wn, n_ev = (double)c->ev.n;
-    *nll = -S + n_ev * std::log(I);
-    const double scale = c->ev.n > 0 ? 2.0 * n_ev / I * wn : 0.0;
-    const double* Fe = h + 2;
-    const double* Fn = h + 2 + 2 * RT;
-    const double* Be = h + 2 + 4 * RT;
-    const double* Bn = Be + nb;
-    std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * std::max(R, 1));
-    auto emit = [&](double se, double sn, double* out) {
-        for (int k = 0; k < nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
-        spline_adjoint(c, Gsc.data(), Gy.data());
-        for (int d = 0; d < RT; ++d) {
-            const int r = d < F ? c->hyb_float[d] : c->hyb_fixed[d - F];
-            const double fold = d < F ? c->res_fold[d] : 1.0;
-            Gr[2 * r] = fold * (se * Fe[2 * d] + sn * Fn[2 * d]);
-            Gr[2 * r + 1] = fold * (se * Fe[2 * d + 1] + sn * Fn[2 * d + 1]);
-        }
-        polar_chain(c, params, Gy.data(), Gr.data(), out);
-    };
-    emit(1.0, scale, grad);
-    if (c->parts_ev) {
-        emit(1.0, 0.0, c->parts_ev);
-        emit(0.0, 2.0 * wn, c->parts_nm);
-        c->parts_S = S; c->parts_I = I;
-    }
+    out->NVB = NVB; out->nb = nb;
+    out->ev = c->h_result; out->nm = c->h_result + NVB;
     return MIPWA_OK;
 }
 
-int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+// the floating resonance whose shape sums k_grad_recompute can fold into its pass: exactly one, of spin 1 or 2, in a
+// model with a compile-time signature.  Returns its spin (the SHP template argument) or 0.
+static int foldable_shape(const mipwa_ctx* c)
 {
-    if (!c || !params || !nll || !grad) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
-    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
-    int rc = use_device(c);
-    if (rc) return rc;
-    rc = prepare_sorted(c);
-    if (rc) return rc;
-    if (effective_path(c) == MIPWA_PATH_CACHED_COMPACT) return nll_grad_compact(c, params, n_params, nll, grad);
-    // k_grad_hybrid is correct but, as measured in round 1, not yet faster than k_grad_recompute (0.385 against 0.365 ms
-    // at config 3: DESIGN.md section 10), so AUTO keeps the recompute kernel for gradients; an explicit
-    // mipwa_set_path(MIPWA_PATH_HYBRID) selects it
-    if (c->path == MIPWA_PATH_HYBRID) return nll_grad_hybrid(c, params, n_params, nll, grad);
-    rc = build_model(c, params, n_params);
-    if (rc) return rc;
+    if (c->F != 1 || c->n_spin[0] != 0 || c->n_spin[1] > MIPWA_SIG_MAX1 || c->n_spin[2] > MIPWA_SIG_MAX2) return 0;
+    for (int r = 0; r < c->R; ++r)
+        if (c->res[r].shape_floats) return c->res[r].spin == 1 || c->res[r].spin == 2 ? c->res[r].spin : 0;
+    return 0;
+}
 
-    const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
-    const size_t smem = (size_t)2 * nb * sizeof(double);
-    if (!c->grad_blocks_per_sm) {
-        bool ok = true;
-        ok = mipwa_occupancy_grad_recompute(c->n_spin, c->model_flags, smem, &c->grad_blocks_per_sm) == cudaSuccess;
-        if (!ok) return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
-        if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
+// value + gradient on the recompute path.  full: also d/d(mass, width) of every floating resonance (grad has n_params
+// entries then); one floating resonance of spin 1 or 2 costs no extra pass (SHP), otherwise k_grad_shape runs afterwards.
+static int nll_grad_recompute(mipwa_ctx* c, const double* params, int64_t n_params, bool full, double* nll, double* grad)
+{
+    int rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    const int N = c->N, R = c->R, F = c->F;
+    const int shp = full ? foldable_shape(c) : 0;
+    const bool want_f = full && F > 0 && !shp;
+    if (want_f) {                                          // room for the per-point factors k_grad_shape reads
+        if (c->f_ev_len < c->ev.n) {
+            if (c->d_f_ev) cudaFree(c->d_f_ev);
+            c->d_f_ev = nullptr; c->f_ev_len = 0;
+            CU(c, cudaMalloc(&c->d_f_ev, (size_t)std::max<int64_t>(c->ev.n, 1) * sizeof(double2)));
+            c->f_ev_len = c->ev.n;
+        }
+        if (c->f_nm_len < c->nm.n) {
+            if (c->d_f_nm) cudaFree(c->d_f_nm);
+            c->d_f_nm = nullptr; c->f_nm_len = 0;
+            CU(c, cudaMalloc(&c->d_f_nm, (size_t)c->nm.n * sizeof(double2)));
+            c->f_nm_len = c->nm.n;
+        }
     }
-    const int64_t gneed = (std::max(c->ev.n, c->nm.n) + MIPWA_GRAD_BLOCK - 1) / MIPWA_GRAD_BLOCK;   // small samples: fewer partial vectors
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->grad_blocks_per_sm, gneed));
-    if (c->gpartials_len < (size_t)grid * NV) {
-        if (c->d_gpartials) cudaFree(c->d_gpartials);
-        c->d_gpartials = nullptr; c->gpartials_len = 0;
-        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NV * sizeof(double)));
-        c->gpartials_len = (size_t)grid * NV;
-    }
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    const cudaError_t le = mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model,
-                                                       c->ev_sorted.s12, c->ev_sorted.s13, c->ev_sorted.seg, nullptr, 0.0,
-                                                       c->ev_sorted.n, c->nm_sorted.s12, c->nm_sorted.s13, c->nm_sorted.w,
-                                                       c->nm_sorted.seg, c->nm_sorted.n, c->d_gpartials,
-                                                       c->want_f ? c->d_f_ev : nullptr,
-                                                       c->want_f ? c->d_f_nm : nullptr);
-    ++c->launches;
-    CU(c, le);
-    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
-    ++c->launches;
-    CU(c, cudaGetLastError());
+    { const int trc = timing_begin(c); if (trc) return trc; }
+    GradTotals t;
+    rc = launch_grad_recompute(c, false, shp, 0.0, true, true, want_f, &t);
+    if (rc) return rc;
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
 
     // ---- host: O(N + R) combine (A7) and adjoint of the coefficient maps ----------------------------------------------
-    const double* h = c->h_result;
-    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;          // w == NULL: kernel used weight 1
-    const double S = h[0], I = h[1] * wn;
+    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;          // w == NULL: the records carry weight 1
+    const double S = t.ev[0], I = t.nm[0] * wn;
     const double n_ev = (double)c->ev.n;
     *nll = -S + n_ev * std::log(I);
     const double scale = c->ev.n > 0 ? 2.0 * n_ev / I * wn : 0.0;
-    const double* Fe = h + 2;
-    const double* Fn = h + 2 + 2 * R;
-    const double* Be = h + 2 + 4 * R;
-    const double* Bn = Be + nb;
-    std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * R);
+    const double *Fe = t.F(t.ev), *Fn = t.F(t.nm), *Be = t.bins(t.ev, R), *Bn = t.bins(t.nm, R);
+    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1));
     auto emit = [&](double se, double sn, double* out) {   // out = se * (event part) + sn * (normalisation part)
-        for (int k = 0; k < nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
+        for (int k = 0; k < t.nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
         spline_adjoint(c, Gsc.data(), Gy.data());
         for (int d = 0; d < R; ++d) {
             const int r = c->perm[d];
@@ -1323,43 +1399,27 @@ int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double*
         emit(0.0, 2.0 * wn, c->parts_nm);
         c->parts_S = S; c->parts_I = I;
     }
-    return MIPWA_OK;
-}
+    if (!full || F == 0) return MIPWA_OK;
 
-// value + gradient over ALL n_params parameters: mipwa_nll_grad for the 2N + 2R linear-coefficient parameters, then
-// k_grad_shape for (mass, width) of every floating resonance (layout of grad = layout of params)
-int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
-{
-    if (!c) return MIPWA_ERR_ARG;
-    if (c->F > 0 && c->ev.n >= 0 && c->nm.n >= 1) {        // room for the per-point factors k_grad_recompute leaves
-        int rc0 = use_device(c);
-        if (rc0) return rc0;
-        if (c->f_ev_len < c->ev.n) {
-            if (c->d_f_ev) cudaFree(c->d_f_ev);
-            c->d_f_ev = nullptr; c->f_ev_len = 0;
-            CU(c, cudaMalloc(&c->d_f_ev, (size_t)std::max<int64_t>(c->ev.n, 1) * sizeof(double2)));
-            c->f_ev_len = c->ev.n;
+    // ---- d/d(mass, width): sums of f conj(dT'/dm0), f conj(dT'/dG0) per floating resonance and set -----------------------
+    auto put = [&](int f, const ResDev& rd, const double* e, const double* g) {   // e, g: [dm_re, dm_im, dG_re, dG_im]
+        for (int q = 0; q < 2; ++q) {                      // q = 0: mass, 1: width
+            const double dr = e[2 * q] + scale * g[2 * q], di = e[2 * q + 1] + scale * g[2 * q + 1];
+            grad[2 * N + 2 * R + 2 * f + q] = rd.cre * dr + rd.cim * di;          // Re(conj(c sqrt(n_R n_D)) D)
+            if (c->parts_ev) {
+                c->parts_ev[2 * N + 2 * R + 2 * f + q] = rd.cre * e[2 * q] + rd.cim * e[2 * q + 1];
+                c->parts_nm[2 * N + 2 * R + 2 * f + q] = 2.0 * wn * (rd.cre * g[2 * q] + rd.cim * g[2 * q + 1]);
+            }
         }
-        if (c->f_nm_len < c->nm.n) {
-            if (c->d_f_nm) cudaFree(c->d_f_nm);
-            c->d_f_nm = nullptr; c->f_nm_len = 0;
-            CU(c, cudaMalloc(&c->d_f_nm, (size_t)c->nm.n * sizeof(double2)));
-            c->f_nm_len = c->nm.n;
-        }
-        c->want_f = true;
+    };
+    if (shp) {                                             // folded into the pass: first device slot of that spin
+        put(0, c->model.res[shp == 1 ? 0 : c->n_spin[1]], t.shape(t.ev, R), t.shape(t.nm, R));
+        return MIPWA_OK;
     }
-    int rc = mipwa_nll_grad(c, params, n_params, nll, grad);
-    c->want_f = false;
-    if (rc || c->F == 0) return rc;
-    const int N = c->N, R = c->R, F = c->F;
-    constexpr int SHAPE_OFF = 3900;                        // in h_result, clear of the main gradient's NV <= 2098 values
-    const double* h = c->h_result;
-    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
-    const double I = h[1] * wn, n_ev = (double)c->ev.n;
-    const double scale = c->ev.n > 0 ? 2.0 * n_ev / I * wn : 0.0;
+    constexpr int SHAPE_OFF = 3900;                        // in h_result, clear of the main gradient's 2 NVB <= 2144 values
     std::vector<int> slots;                                // device slot of each floating resonance, list order
     for (int f = 0; f < F; ++f)
-        for (int d = 0; d < c->model.R; ++d)              // the model as built: on the hybrid path only the floating ones
+        for (int d = 0; d < c->model.R; ++d)
             if (c->model.res[d].fl == f) slots.push_back(d);
     if ((int)slots.size() != F) return fail(c, MIPWA_ERR_STATE, "floating resonance not found in the device model");
     const int64_t need = (std::max(c->ev.n, c->nm.n) + 511) / 512;
@@ -1371,14 +1431,14 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
         CU(c, cudaMalloc(&c->d_gpartials, want * sizeof(double)));
         c->gpartials_len = want;
     }
-    const Slot& E = evs(c);
-    const Slot& G = nms(c);
+    const Slot& E = c->ev_sorted;
+    const Slot& G = c->nm_sorted;
     float ms_total = c->last_ms;
     for (int f0 = 0; f0 < F; f0 += MIPWA_SHAPE_MAXF) {
         const int nf = std::min(MIPWA_SHAPE_MAXF, F - f0);
         ShapeSel sel;
         for (int q = 0; q < MIPWA_SHAPE_MAXF; ++q) sel.slot[q] = slots[f0 + std::min(q, nf - 1)];
-        if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
+        { const int trc = timing_begin(c); if (trc) return trc; }
 #define MIPWA_SHAPE_LAUNCH(NF, LT)                                                                                 \
     do {                                                                                                           \
         if (c->model_flags & MIPWA_FL_EQM)                                                                         \
@@ -1403,29 +1463,43 @@ int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, do
 #undef MIPWA_SHAPE_LAUNCH
         ++c->launches;
         CU(c, cudaGetLastError());
-        k_grad_finalize<<<(8 * nf + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, 8 * nf, c->d_result + SHAPE_OFF);
+        k_grad_finalize<<<(8 * nf + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, grid, 8 * nf, 1, c->d_result + SHAPE_OFF);
         ++c->launches;
         CU(c, cudaGetLastError());
         if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
         CU(c, cudaStreamSynchronize(c->stream));
         if (c->timing) { float ms = 0.f; CU(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1)); ms_total += ms; }
         const double* D = c->h_result + SHAPE_OFF;         // [pass][f][dm_re, dm_im, dG_re, dG_im]
-        for (int q = 0; q < nf; ++q) {
-            const ResDev& rd = c->model.res[slots[f0 + q]];
-            const double* e = D + (0 * nf + q) * 4;
-            const double* g = D + (1 * nf + q) * 4;
-            for (int t = 0; t < 2; ++t) {                  // t = 0: mass, 1: width
-                const double dr = e[2 * t] + scale * g[2 * t], di = e[2 * t + 1] + scale * g[2 * t + 1];
-                grad[2 * N + 2 * R + 2 * (f0 + q) + t] = rd.cre * dr + rd.cim * di;   // Re(conj(c sqrt(n_R n_D)) D)
-                if (c->parts_ev) {
-                    c->parts_ev[2 * N + 2 * R + 2 * (f0 + q) + t] = rd.cre * e[2 * t] + rd.cim * e[2 * t + 1];
-                    c->parts_nm[2 * N + 2 * R + 2 * (f0 + q) + t] = 2.0 * wn * (rd.cre * g[2 * t] + rd.cim * g[2 * t + 1]);
-                }
-            }
-        }
+        for (int q = 0; q < nf; ++q) put(f0 + q, c->model.res[slots[f0 + q]], D + (0 * nf + q) * 4, D + (1 * nf + q) * 4);
     }
     c->last_ms = ms_total;
     return MIPWA_OK;
+}
+
+static int nll_grad_any(mipwa_ctx* c, const double* params, int64_t n_params, bool full, double* nll, double* grad)
+{
+    if (!c || !params || !nll || !grad) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = prepare_sorted(c);
+    if (rc) return rc;
+    if (effective_path(c) == MIPWA_PATH_CACHED_COMPACT) return nll_grad_compact(c, params, n_params, nll, grad);
+    return nll_grad_recompute(c, params, n_params, full, nll, grad);
+}
+
+int mipwa_nll_grad(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+{
+    NvtxRange range("mipwa_nll_grad");
+    return nll_grad_any(c, params, n_params, false, nll, grad);
+}
+
+// value + gradient over ALL n_params parameters: the 2N + 2R linear-coefficient parameters, then (mass, width) of every
+// floating resonance (layout of grad = layout of params)
+int mipwa_nll_grad_full(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad)
+{
+    NvtxRange range("mipwa_nll_grad_full");
+    return nll_grad_any(c, params, n_params, true, nll, grad);
 }
 
 // the pieces one rank of a sharded likelihood contributes (include/mipwa.h): same launches as
@@ -1436,10 +1510,11 @@ int mipwa_nll_grad_parts(mipwa_ctx* c, const double* params, int64_t n_params, d
     if (!c) return MIPWA_ERR_ARG;
     if (!params || !sum_log || !integral || !grad_ev || !grad_nm) return fail(c, MIPWA_ERR_ARG, "null argument");
     if (n_params != 2 * c->N + 2 * c->R + 2 * c->F) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
+    NvtxRange range("mipwa_nll_grad_parts");
     std::vector<double> total((size_t)std::max<int64_t>(n_params, 1));
     double nll = 0.0;
     c->parts_ev = grad_ev; c->parts_nm = grad_nm;
-    const int rc = mipwa_nll_grad_full(c, params, n_params, &nll, total.data());
+    const int rc = nll_grad_any(c, params, n_params, true, &nll, total.data());
     c->parts_ev = c->parts_nm = nullptr;
     if (rc) return rc;
     *sum_log = c->parts_S; *integral = c->parts_I;
@@ -1458,6 +1533,7 @@ int mipwa_set_event_background(mipwa_ctx* c, const double* b, int32_t mem)
     Slot& s = c->ev;
     if (s.owned[2]) { cudaFree(s.owned[2]); s.owned[2] = nullptr; }
     s.w = nullptr;
+    drop_records(s);                                       // the event records carry the densities
     c->ev_sorted_valid = false;                            // the cell-sorted copy carries the densities along
     c->cache_valid = false; c->hyb_ev_valid = false;       // the caches follow the event order of the sorted copy
     if (!b || s.n == 0) return MIPWA_OK;                   // NULL clears
@@ -1480,37 +1556,45 @@ int mipwa_nll_mix(mipwa_ctx* c, const double* params, int64_t n_params, double f
     if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
     if (c->ev.n > 0 && !c->ev.w) return fail(c, MIPWA_ERR_STATE, "set the background densities (mipwa_set_event_background)");
     if (!(f_sig > 0.0 && f_sig <= 1.0)) return fail(c, MIPWA_ERR_ARG, "signal fraction must be in (0, 1]");
+    NvtxRange range("mipwa_nll_mix");
     int rc = use_device(c);
     if (rc) return rc;
     rc = build_model(c, params, n_params);
     if (rc) return rc;
-    const Slot& E = evs(c);
-    const Slot& G = nms(c);
-    const int64_t need = (std::max(E.n, G.n) + MIPWA_REC_BLOCK - 1) / MIPWA_REC_BLOCK;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->blocks_per_sm, need));
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, E.s12, E.s13, E.seg,
-                                                nullptr, 0.0, 0, G.s12, G.s13, G.w, G.seg, G.n, c->d_partials,
-                                                c->d_ticket, c->d_result);
+    Slot& E = evs(c);
+    Slot& G = nms(c);
+    rc = ensure_records(c, E, 0.0);
+    if (rc) return rc;
+    rc = ensure_records(c, G, 1.0);
+    if (rc) return rc;
+    const int grid = recompute_grid(c, std::max(E.n, G.n));
+    const bool timing = c->timing;
+    { const int trc = timing_begin(c); if (trc) return trc; }
+    c->timing = false;                                     // wait_result polls: one pair of events spans both launches
+    long long tag = next_tag(c);
+    cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0, 0,
+                                                G.rec, G.n, c->d_partials, c->d_ticket, c->d_result, tag);
     ++c->launches;
-    CU(c, le);
-    CU(c, cudaStreamSynchronize(c->stream));
+    if (le == cudaSuccess) rc = wait_result(c, tag);
     const double I = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
     const double kappa = I * (1.0 - f_sig) / f_sig;
     double S = 0.0;
-    if (E.n > 0) {
-        le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, grid, c->stream, c->model, E.s12, E.s13, E.seg, E.w, kappa,
-                                        E.n, G.s12, G.s13, G.w, G.seg, 0, c->d_partials, c->d_ticket, c->d_result);
+    if (le == cudaSuccess && rc == MIPWA_OK && E.n > 0) {
+        tag = next_tag(c);
+        le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, true, grid, c->stream, c->model, E.rec, kappa, E.n, G.rec,
+                                        0, c->d_partials, c->d_ticket, c->d_result, tag);
         ++c->launches;
-        CU(c, le);
-        if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-        CU(c, cudaStreamSynchronize(c->stream));
+        if (le == cudaSuccess) rc = wait_result(c, tag);
         S = c->h_result[0];
-    } else {
-        if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-        CU(c, cudaStreamSynchronize(c->stream));
     }
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    c->timing = timing;
+    CU(c, le);
+    if (rc) return rc;
+    if (timing) {
+        CU(c, cudaEventRecord(c->ev1, c->stream));
+        CU(c, cudaEventSynchronize(c->ev1));
+        CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    }
     *nll = -S - (double)c->ev.n * std::log(f_sig / I);
     return MIPWA_OK;
 }
@@ -1526,75 +1610,45 @@ int mipwa_nll_mix_grad(mipwa_ctx* c, const double* params, int64_t n_params, dou
     if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
     if (c->ev.n > 0 && !c->ev.w) return fail(c, MIPWA_ERR_STATE, "set the background densities (mipwa_set_event_background)");
     if (!(f_sig > 0.0 && f_sig <= 1.0)) return fail(c, MIPWA_ERR_ARG, "signal fraction must be in (0, 1]");
+    NvtxRange range("mipwa_nll_mix_grad");
     int rc = use_device(c);
     if (rc) return rc;
     rc = prepare_sorted(c);
     if (rc) return rc;
     rc = build_model(c, params, n_params);
     if (rc) return rc;
-    const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NV = 2 + 4 * R + 2 * nb;
-    const size_t smem = (size_t)2 * nb * sizeof(double);
-    if (!c->grad_blocks_per_sm) {
-        if (mipwa_occupancy_grad_recompute(c->n_spin, c->model_flags, smem, &c->grad_blocks_per_sm) != cudaSuccess)
-            return fail(c, MIPWA_ERR_CUDA, "occupancy query failed");
-        if (c->grad_blocks_per_sm < 1) c->grad_blocks_per_sm = 1;
-    }
-    const int64_t gneed = (std::max(c->ev.n, c->nm.n) + MIPWA_GRAD_BLOCK - 1) / MIPWA_GRAD_BLOCK;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)c->sm_count * c->grad_blocks_per_sm, gneed));
-    if (c->gpartials_len < (size_t)grid * NV) {
-        if (c->d_gpartials) cudaFree(c->d_gpartials);
-        c->d_gpartials = nullptr; c->gpartials_len = 0;
-        CU(c, cudaMalloc(&c->d_gpartials, (size_t)grid * NV * sizeof(double)));
-        c->gpartials_len = (size_t)grid * NV;
-    }
-    const Slot& E = c->ev_sorted;
-    const Slot& G = c->nm_sorted;
-    std::vector<double> h1(NV), h2(NV, 0.0);
-    if (c->timing) CU(c, cudaEventRecord(c->ev0, c->stream));
-    for (int launch = 0; launch < 2; ++launch) {
-        if (launch == 1 && E.n == 0) break;
-        const double I1 = launch == 1 ? h1[1] * (c->nm.w ? 1.0 : 1.0 / (double)c->nm.n) : 0.0;
-        const double kappa = launch == 1 ? I1 * (1.0 - f_sig) / f_sig : 0.0;
-        const cudaError_t le = launch == 0
-            ? mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model, E.s12, E.s13, E.seg,
-                                          nullptr, 0.0, 0, G.s12, G.s13, G.w, G.seg, G.n, c->d_gpartials, nullptr, nullptr)
-            : mipwa_launch_grad_recompute(c->n_spin, c->model_flags, grid, smem, c->stream, c->model, E.s12, E.s13, E.seg,
-                                          E.w, kappa, E.n, G.s12, G.s13, G.w, G.seg, 0, c->d_gpartials, nullptr, nullptr);
-        ++c->launches;
-        CU(c, le);
-        k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, NV, c->d_result);
-        ++c->launches;
-        CU(c, cudaGetLastError());
-        if (launch == 1 || E.n == 0) { if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream)); }
-        CU(c, cudaStreamSynchronize(c->stream));
-        std::memcpy(launch == 0 ? h1.data() : h2.data(), c->h_result, NV * sizeof(double));
-    }
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
-
+    const int N = c->N, R = c->R;
     const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
-    const double I = h1[1] * wn, n_ev = (double)c->ev.n, kappa = I * (1.0 - f_sig) / f_sig;
-    const double S = h2[0], Q = h2[1];
+    { const int trc = timing_begin(c); if (trc) return trc; }
+    GradTotals t;
+    rc = launch_grad_recompute(c, false, 0, 0.0, false, true, false, &t);      // normalisation points alone
+    if (rc) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    std::vector<double> hn(t.nm, t.nm + t.NVB), he(t.NVB, 0.0);
+    const double I = hn[0] * wn, n_ev = (double)c->ev.n, kappa = I * (1.0 - f_sig) / f_sig;
+    if (c->ev.n > 0) {
+        rc = launch_grad_recompute(c, true, 0, kappa, true, false, false, &t); // events alone, D = |A|^2 + kappa b
+        if (rc) return rc;
+    }
+    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    if (c->ev.n > 0) he.assign(t.ev, t.ev + t.NVB);
+
+    const double S = he[0], Q = he[1];
     *nll = -S - n_ev * std::log(f_sig / I);
     if (dnll_dfsig) *dnll_dfsig = -(n_ev - I * Q / f_sig) / f_sig;
     const double scale = 2.0 * (n_ev - kappa * Q) / I * wn;
-    const double *Fe = h2.data() + 2, *Fn = h1.data() + 2 + 2 * R, *Be = h2.data() + 2 + 4 * R, *Bn = h1.data() + 2 + 4 * R + nb;
-    std::vector<double> Gsc(nb), Gy(2 * N), Gr(2 * R);
-    auto emit = [&](double se, double sn, double* out) {   // out = se * (event part) + sn * (normalisation part)
-        for (int k = 0; k < nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
-        spline_adjoint(c, Gsc.data(), Gy.data());
-        for (int d = 0; d < R; ++d) {
-            const int r = c->perm[d];
-            Gr[2 * r] = c->res_fold[d] * (se * Fe[2 * d] + sn * Fn[2 * d]);
-            Gr[2 * r + 1] = c->res_fold[d] * (se * Fe[2 * d + 1] + sn * Fn[2 * d + 1]);
-        }
-        polar_chain(c, params, Gy.data(), Gr.data(), out);
-    };
-    emit(1.0, scale, grad);
-    if (c->parts_ev) {                                     // mipwa_nll_grad_parts: d(-S)/dtheta and dI/dtheta apart
-        emit(1.0, 0.0, c->parts_ev);
-        emit(0.0, 2.0 * wn, c->parts_nm);
-        c->parts_S = S; c->parts_I = I;
+    const double *Fe = t.F(he.data()), *Fn = t.F(hn.data()), *Be = t.bins(he.data(), R), *Bn = t.bins(hn.data(), R);
+    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1));
+    for (int k = 0; k < t.nb; ++k) Gsc[k] = Be[k] + scale * Bn[k];
+    spline_adjoint(c, Gsc.data(), Gy.data());
+    for (int d = 0; d < R; ++d) {
+        const int r = c->perm[d];
+        Gr[2 * r] = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
+        Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
     }
+    polar_chain(c, params, Gy.data(), Gr.data(), grad);
     return MIPWA_OK;
 }
 
@@ -1631,8 +1685,8 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
     do {                                                                                                             \
         e = cudaFuncSetAttribute(k_gram<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
         if (e == cudaSuccess)                                                                                        \
-            k_gram<T, true><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, basis_aux(c), cc, E.s12, E.s13, nullptr, \
-                                                                    E.n, 0.0, partial);                              \
+            k_gram<T, true><<<grid, MIPWA_TILE, smem, c->stream>>>(c->model, c->d_search, basis_aux(c), cc, E.s12,   \
+                                                                    E.s13, nullptr, E.n, 0.0, partial);              \
     } while (0)
         if (tpt <= 1) MIPWA_HESS_LAUNCH(1); else if (tpt == 2) MIPWA_HESS_LAUNCH(2); else MIPWA_HESS_LAUNCH(3);
 #undef MIPWA_HESS_LAUNCH
@@ -1751,7 +1805,7 @@ int mipwa_generate(mipwa_ctx* c, const double* params, int64_t n_params, uint64_
 
     // envelope: fine-grid maxima per coarse cell on the device, neighbour fill and CDF on the host (O(n_coarse^2))
     const int64_t fine = (int64_t)n_side * n_side;
-    k_gen_envelope<<<grid_for(c, fine, 8), 256, 0, c->stream>>>(c->model, gk, n_side, h, H, nc, g.own);
+    k_gen_envelope<<<grid_for(c, fine, 8), 256, 0, c->stream>>>(c->model, c->d_search, gk, n_side, h, H, nc, g.own);
     ++c->launches;
     CU(c, cudaGetLastError());
     std::vector<unsigned long long> own_bits(ncell);
@@ -1780,8 +1834,8 @@ int mipwa_generate(mipwa_ctx* c, const double* params, int64_t n_params, uint64_
 
     int64_t have = 0, ctr = 0;
     while (have < n) {
-        k_gen_candidates<<<grid_for(c, batch, 8), 256, 0, c->stream>>>(c->model, gk, (unsigned long long)key, ctr, batch,
-                                                                     nc, H, g.cum, g.env, g.c12, g.c13, g.flag);
+        k_gen_candidates<<<grid_for(c, batch, 8), 256, 0, c->stream>>>(c->model, c->d_search, gk, (unsigned long long)key,
+                                                                     ctr, batch, nc, H, g.cum, g.env, g.c12, g.c13, g.flag);
         ++c->launches;
         CU(c, cudaGetLastError());
         CU(c, cub::DeviceSelect::Flagged(g.tmp, tmp_bytes, g.c12, g.flag, g.o12 + have, g.nsel, (int)batch, c->stream));

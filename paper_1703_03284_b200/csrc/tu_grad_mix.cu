@@ -3,14 +3,21 @@
 #include "kernels.cuh"
 #include "grad.cuh"
 
-cudaError_t mipwa_launch_grad_recompute_mix(const int* n_spin, int fl, int grid, size_t smem, cudaStream_t st,
-                                            const DevModel& m, const double* e12, const double* e13,
-                                            const unsigned short* eseg, const double* eb, double kappa, long long n_ev,
-                                            const double* g12, const double* g13, const double* gw,
-                                            const unsigned short* gseg, long long n_norm, double* partials)
+cudaError_t mipwa_grad_set_smem_mix(const int* n_spin, int fl, size_t smem)
+{
+    cudaError_t e = cudaSuccess;
+    MIPWA_DISPATCH_SIGFL(n_spin[0], n_spin[1], n_spin[2], fl,
+                         (e = cudaFuncSetAttribute(k_grad_recompute<R1, R2, FL, true, 0>,
+                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)));
+    return e;
+}
+
+cudaError_t mipwa_launch_grad_recompute_mix(const int* n_spin, int fl, int grid, int ev_blocks, size_t smem,
+                                            cudaStream_t st, const DevModel& m, const PointRec* ev, double kappa,
+                                            long long n_ev, const PointRec* nm, long long n_norm, double* partials)
 {
     MIPWA_DISPATCH_SIGFL(n_spin[0], n_spin[1], n_spin[2], fl,
-                         (k_grad_recompute<R1, R2, FL, true><<<grid, MIPWA_GRAD_BLOCK, smem, st>>>(
-                             m, e12, e13, eseg, eb, kappa, n_ev, g12, g13, gw, gseg, n_norm, partials, nullptr, nullptr)));
+                         (k_grad_recompute<R1, R2, FL, true, 0><<<grid, MIPWA_GRAD_BLOCK, smem, st>>>(
+                             m, ev, kappa, n_ev, nm, n_norm, ev_blocks, partials, nullptr, nullptr)));
     return cudaGetLastError();
 }

@@ -29,11 +29,11 @@ cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cu
                                     const HybCoef& cc, const double2* ev_cache, const unsigned short* eseg,
                                     long long n_ev, const double2* nm_cache, const double* gw,
                                     const unsigned short* gseg, long long n_norm, double2* partials,
-                                    unsigned int* ticket, double* result)
+                                    unsigned int* ticket, double* result, long long tag)
 {
     bool supported = true;
     MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl,
                          (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_HYB_BLOCK, mipwa_hyb_ring_bytes(RCT), st>>>(
-                             m, cc, ev_cache, eseg, n_ev, nm_cache, gw, gseg, n_norm, partials, ticket, result)));
+                             m, cc, ev_cache, eseg, n_ev, nm_cache, gw, gseg, n_norm, partials, ticket, result, tag)));
     return supported ? cudaGetLastError() : cudaErrorInvalidValue;
 }
