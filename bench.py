@@ -11,6 +11,9 @@ is three doubles per rank per call (paper_1703_03284_b200/sharding.py).
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--events E] [--norm-points G]
 
 --impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+Besides the contract's keys the line carries: grad (value + analytic gradient), mixture, hybrid, cached (the fixed-shape
+paths on config 3's sample and `sweep4`: BASELINE.json configs[4] at 10 M and 100 M events, K = 56), latency (wall clock
+per call at configs 0, 1, 5).  --probe grid-bias | sweep4 | latency print the longer tables behind BASELINE.md.
 """
 import argparse
 import json
@@ -34,19 +37,13 @@ UNIT = "events/s"
 
 # ---- algorithmic work per point: flops of the plain formulas, one per add / mul /
 # div / sqrt / log, fma = 2: two channels x [10 shared kinematics + 14 spline + 37 R] + 4, plus 2 (1 + 3R) divisions,
-# 2 (2 + R) square roots and one log = 59 + 82 R (305 at R = 3).  The kernel as built executes 261 at config 3
-# (ncu-counted dadd + dmul + 2 dfma per point, profiles/r1_k_nll_recompute_ncu.md: the equal-mass and shared-radii
+# 2 (2 + R) square roots and one log = 59 + 82 R (305 at R = 3).  The kernel as built executes
+# fewer (ncu-counted dadd + dmul + 2 dfma per point, profiles/r2_k_nll_recompute_ncu.md: the equal-mass and shared-radii
 # specialisations and one reciprocal (square root) per resonance and channel do the same arithmetic in fewer
-# operations), so nothing is padded; "executed_flops_per_point" in the roofline object gives the executed rate. ------
+# operations), so nothing is padded; the roofline object reports the fraction on the executed count beside it. --------
 def flops_per_point(resonances):
     return 59 + 82 * len(resonances)
 
-
-# dram__bytes_read.sum + dram__bytes_write.sum per k_nll_recompute launch at the bench size (10M events + 10M weighted
-# normalisation points), from the one `ncu --set full` capture summarised in profiles/r1_k_nll_recompute_ncu.md
-NCU_TRAFFIC_BYTES = {(10_000_000, 10_000_000): 445.3e6}
-# executed FP64 flops per point in that capture (config 3's model): (dadd + dmul + 2 dfma) / points
-NCU_EXECUTED_FLOPS_PER_POINT = {(10_000_000, 10_000_000): 260.7}
 
 
 class ClockSampler:
@@ -128,23 +125,140 @@ def run_reference(args, cfg, workload):
     print(json.dumps(line), flush=True)
 
 
-def gpu_inputs(cfg, m, B, torch, rank):
+def gpu_inputs(cfg, m, torch, rank, n_ev):
     """Events by accept-reject on the device (mipwa_generate: the recipe of DESIGN.md section 4 / reading P22, the
     same stream key inputs.Config.events uses), normalisation points uniform in phase space; both end up resident
     in HBM as torch tensors."""
-    e12, e13, _ = m.generate(cfg.truth, cfg.key(I.S_EVENTS + 16 * rank), cfg.n_ev, n_side=1024, n_coarse=64)
+    e12, e13, _ = m.generate(cfg.truth, cfg.key(I.S_EVENTS + 16 * rank), n_ev, n_side=1024, n_coarse=64)
     g12, g13, w = cfg.norm_points(stream=rank)
     host = [np.ascontiguousarray(a) for a in (e12, e13, g12, g13, w)]
     dev = [torch.from_numpy(a).cuda() for a in host]
     return host, dev
 
 
-def m_grad_full_ref(m, B, p):
-    """the same gradient through the full-recompute kernels (cross-check of the hybrid gradient leg)"""
-    m.set_path(B.PATH_RECOMPUTE)
-    g = m.nll_grad_full(p)[1]
-    m.set_path(B.PATH_HYBRID)
-    return g
+def source_sha():
+    """fingerprint of the kernel sources a profile belongs to (profiles/*.md carry it in their `bench:` line)"""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("dev_model.cuh", "kernels.cuh"):
+        with open(os.path.join(ROOT, "paper_1703_03284_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def profile_numbers(name):
+    """The `bench: {...}` line of profiles/<name>: numbers read off one `ncu --set full` capture (executed flops per
+    point, DRAM bytes per launch, FP64-pipe activity).  Returned only while the kernel sources still hash to the value
+    recorded with them; otherwise None: a stale capture must not decorate a fresh timing."""
+    try:
+        with open(os.path.join(ROOT, "profiles", name)) as f:
+            for line in f:
+                if line.startswith("bench:"):
+                    d = json.loads(line[len("bench:"):])
+                    return d if d.get("source_sha") == source_sha() else None
+    except (OSError, ValueError):
+        pass
+    return None
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (copy, read+write)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+def kernel_ms_of(m, call, params, n):
+    """mean device duration of the kernels of `call` over n calls (library timing mode: a spacer kernel in front of
+    the first event keeps the host's launch latency out of the bracket, see csrc/kernels.cuh k_spacer)"""
+    m.enable_timing(True)
+    for t in range(3):
+        call(params[t % len(params)])
+    ms = []
+    for t in range(n):
+        call(params[t % len(params)])
+        ms.append(m.last_kernel_ms())
+    m.enable_timing(False)
+    return float(np.mean(ms)), float(np.min(ms))
+
+
+def wall_of(call, params, n):
+    t0 = time.perf_counter()
+    for t in range(n):
+        out = call(params[t % len(params)])
+    return (time.perf_counter() - t0) / n, out
+
+
+def sweep4_leg(B, torch, stream, local, sizes, hbm, hbm_src):
+    """BASELINE.json configs[4]: the cached-basis paths at K = 56 (50 knots + 6 fixed-shape resonances) against the
+    event count, 10 M-point Gram matrix; events drawn ON THE DEVICE from the PDF (mipwa_generate)."""
+    c = I.Config(4)
+    m = B.Mipwa(c.kin, c.knots, c.resonances, device=local)
+    m.set_stream(stream)
+    g12, g13 = I.phase_space_points(10_000_000, c.key(I.S_NORM))
+    dg = [torch.from_numpy(a).cuda() for a in (g12, g13)]
+    m.set_norm_points(dg[0], dg[1], None)
+    ps = [c.perturbed(t)[:c.n_params] for t in range(8)]
+    rows, first = [], None
+    t0 = time.perf_counter()
+    E12, E13, tried = m.generate(c.truth, c.key(I.S_EVENTS), max(sizes), n_side=1024, n_coarse=64, device=True)
+    torch.cuda.synchronize()
+    gen_s = time.perf_counter() - t0
+    for n in sizes:
+        e12, e13 = E12[:n], E13[:n]
+        m.set_events(e12, e13); m.prepare()
+        row = {"n_ev": n, "K": c.N + c.R}
+        for name, path, kernel in (("dense", B.PATH_CACHED, "k_nll_dense"), ("compact", B.PATH_CACHED_COMPACT, "k_nll_compact")):
+            m.set_path(path)
+            t0 = time.perf_counter(); v0 = m.nll(ps[0]); setup = time.perf_counter() - t0
+            k, kmin = kernel_ms_of(m, m.nll, ps, 12)
+            byt = m.basis_bytes() + (2 * n if name == "compact" else 0)      # + the 2-byte segment pairs
+            row[name] = {"kernel_ms": k, "cache_bytes": m.basis_bytes(), "events_per_s": n / (k * 1e-3),
+                         "nll_evals_per_s": 1e3 / k, "first_call_s": setup, "nll": v0,
+                         "roofline": {"bound": "hbm", "kernel": kernel, "achieved": byt / (k * 1e-3) * 1e-9, "peak": hbm,
+                                      "unit": "GB/s", "frac": byt / (k * 1e-3) * 1e-9 / hbm, "traffic": None,
+                                      "algorithmic_bytes": byt, "peak_source": hbm_src}}
+        row["dense_minus_compact_nll"] = row["dense"]["nll"] - row["compact"]["nll"]
+        if n <= 10_000_000:
+            m.set_path(B.PATH_RECOMPUTE)
+            row["recompute_minus_compact_nll"] = m.nll(ps[0]) - row["compact"]["nll"]
+        rows.append(row)
+        if first is None:                                  # kept for the oracle spot check of the cpu_baseline leg
+            first = (e12[:200_000].cpu().numpy(), e13[:200_000].cpu().numpy(), g12[:1_000_000], g13[:1_000_000], ps[0])
+    m.close()
+    del E12, E13, dg
+    torch.cuda.empty_cache()
+    return {"what": "BASELINE.json configs[4]: K = 56 complex basis functions; dense cache 896 B/event (k_nll_dense) and compact "
+                    "cache 112 B/event + 2 B segment pair (k_nll_compact); I = c^H G c from a 10 M-point Gram matrix; events "
+                    "generated on the device from |A|^2 (mipwa_generate); kernel_ms = mean of 12 perturbed calls",
+            "event_generation_s": gen_s, "candidates_drawn": int(tried), "rows": rows}, first
+
+
+def latency_leg(B, torch, stream, local):
+    """wall clock per blocking call at the paper's scale (100 K-event fits): configs 0, 1 and 5"""
+    out = []
+    for idx in (0, 1, 5):
+        c = I.Config(idx)
+        m = B.Mipwa(c.kin, c.knots, c.resonances, device=local)
+        m.set_stream(stream)
+        e12, e13, _ = m.generate(c.truth, c.key(I.S_EVENTS), c.n_ev, n_side=512, n_coarse=32, device=True)
+        g12, g13, w = c.norm_points()
+        d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (g12, g13, w)]
+        m.set_events(e12, e13); m.set_norm_points(d[0], d[1], d[2]); m.prepare()
+        ps = [c.perturbed(t) for t in range(64)]
+        row = {"config": idx, "n_ev": c.n_ev, "n_norm": int(g12.size), "n_params": int(c.n_params)}
+        for name, path, call in (("nll_recompute", B.PATH_RECOMPUTE, m.nll), ("nll_auto", B.PATH_AUTO, m.nll),
+                                 ("nll_grad_recompute", B.PATH_RECOMPUTE, m.nll_grad), ("nll_grad_auto", B.PATH_AUTO, m.nll_grad)):
+            m.set_path(path)
+            for t in range(10):
+                call(ps[t])
+            wall, _ = wall_of(call, ps, 300)
+            k, _ = kernel_ms_of(m, call, ps, 20)
+            row[name] = {"wall_us": wall * 1e6, "kernel_us": k * 1e3}
+        out.append(row)
+        m.close()
+    return out
 
 
 def run_ours(args, cfg, workload):
@@ -162,14 +276,20 @@ def run_ours(args, cfg, workload):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
+    strong = args.scaling == "strong"
 
     m = B.Mipwa(cfg.kin, cfg.knots, cfg.resonances, device=local)
     stream = torch.cuda.Stream(device=dev)
     m.set_stream(stream)
     t_gen = time.perf_counter()
-    host, d = gpu_inputs(cfg, m, B, torch, rank)
+    host, d = gpu_inputs(cfg, m, torch, rank, cfg.n_ev)
     t_gen = time.perf_counter() - t_gen
-    if world > 1:                                    # whole-sample weights so that per-rank integrals add
+    if strong and world > 1:                         # one sample for the whole job, sliced
+        lo, hi = sharding.shard_range(cfg.n_ev, rank, world)
+        glo, ghi = sharding.shard_range(host[2].size, rank, world)
+        host = [host[0][lo:hi], host[1][lo:hi], host[2][glo:ghi], host[3][glo:ghi], host[4][glo:ghi]]
+        d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in host]
+    elif world > 1:                                  # whole-sample weights so that per-rank integrals add
         d[4] = d[4] / world
         host[4] = host[4] / world
     m.set_events(d[0], d[1])
@@ -179,7 +299,6 @@ def run_ours(args, cfg, workload):
     m.prepare()                                      # once per sample: cell-sorted copies (a fit reuses them every call)
     torch.cuda.synchronize(dev)
     t_prep = time.perf_counter() - t_prep
-    m.enable_timing(True)
     n_ev, n_norm = d[0].numel(), d[2].numel()
 
     params = [cfg.perturbed(t) for t in range(args.warmup + args.steps)]
@@ -203,12 +322,10 @@ def run_ours(args, cfg, workload):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     launches0 = m.launch_count()
-    kernel_ms = []
     w0 = time.perf_counter()
     ev0.record(stream)
     for t in range(args.steps):
         nll = step(params[args.warmup + t])
-        kernel_ms.append(m.last_kernel_ms())
     ev1.record(stream)
     barrier()
     w1 = time.perf_counter()
@@ -219,6 +336,8 @@ def run_ours(args, cfg, workload):
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         ms_total = float(tt.item())
     ms_step = ms_total / args.steps
+    # device duration of the kernel alone, same calls (separate loop: timing mode adds a spacer kernel per call)
+    k_ms, k_ms_min = kernel_ms_of(m, m.nll, params[args.warmup:], min(args.steps, 200))
 
     # ---- e2e: the same evaluation through the C ABI from HOST buffers: H2D of the step's inputs (pinned), the
     # boundary check, the NLL kernel and the D2H of the result are all inside the timed region -----------------------
@@ -242,54 +361,45 @@ def run_ours(args, cfg, workload):
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         e2e_s = float(tt.item())
     h2d = sum(a.nbytes for a in ph) + params[0].nbytes
-    d2h = 16 + 16                                     # two boundary-check counters + (sum ln|A|^2, I)
+    d2h = 16 + 24                                     # two boundary-check counters + (sum ln|A|^2, I, tag)
     # back to resident device arrays for the fit-step latency number
     m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4]); m.prepare()
-    t0 = time.perf_counter()
-    for t in range(args.steps):
-        step(params[args.warmup + t])
-    fit_step_s = (time.perf_counter() - t0) / args.steps
+    fit_step_s, _ = wall_of(step, params[args.warmup:], args.steps)
 
     # ---- A8: value + analytic gradient (BASELINE configs[3]: "plus analytic gradient w.r.t. all 2N+2*3 parameters") ----
     sub_steps = max(3, min(args.steps, 30))
+    sub = params[args.warmup:args.warmup + sub_steps]
     for t in range(3):
         m.nll_grad(params[t])
-    grad_ms = []
     barrier()
-    t0 = time.perf_counter()
-    for t in range(sub_steps):
-        nll_g, grad = m.nll_grad(params[args.warmup + t % args.steps])
-        grad_ms.append(m.last_kernel_ms())
+    grad_wall, (nll_g, grad) = wall_of(m.nll_grad, sub, sub_steps)
     barrier()
-    grad_wall = (time.perf_counter() - t0) / sub_steps
-    grad_info = {"ms_per_call": 1e3 * grad_wall, "kernel_ms": float(np.mean(grad_ms)),
+    gk, _ = kernel_ms_of(m, m.nll_grad, sub, sub_steps)
+    grad_info = {"ms_per_call": 1e3 * grad_wall, "kernel_ms": gk, "kernel_ms_over_value_kernel_ms": gk / k_ms,
                  "events_per_s": n_ev * world / grad_wall, "n_grad": int(grad.size), "nll": nll_g,
-                 "what": "mipwa_nll_grad: NLL + d/d(a_k, phi_k, |c_r|, arg c_r), same sample, k_grad_recompute"}
-    # all n_params derivatives, incl. d/d(mass, width) of the floating rho(770) (k_grad_shape, one extra pass)
+                 "bitwise_reproducible": bool(np.array_equal(m.nll_grad(sub[0])[1], m.nll_grad(sub[0])[1])),
+                 "what": "mipwa_nll_grad: NLL + d/d(a_k, phi_k, |c_r|, arg c_r), same sample; k_grad_recompute (one launch over "
+                         "both cell-sorted record sets, per-warp segment bins, no atomics) + k_grad_finalize"}
+    # all n_params derivatives, incl. d/d(mass, width) of the floating rho(770), folded into the same pass
     for t in range(2):
         m.nll_grad_full(params[t])
-    full_ms = []
     barrier()
-    t0 = time.perf_counter()
-    for t in range(sub_steps):
-        nll_f, grad_f = m.nll_grad_full(params[args.warmup + t % args.steps])
-        full_ms.append(m.last_kernel_ms())
+    full_wall, (nll_f, grad_f) = wall_of(m.nll_grad_full, sub, sub_steps)
     barrier()
-    full_wall = (time.perf_counter() - t0) / sub_steps
-    grad_info["full"] = {"ms_per_call": 1e3 * full_wall, "kernel_ms": float(np.mean(full_ms)), "n_grad": int(grad_f.size),
-                         "d_mass_d_width": [float(x) for x in grad_f[grad.size:]],
-                         "what": "mipwa_nll_grad_full: the above + d/d(mass, width) of every floating resonance"}
+    fk, _ = kernel_ms_of(m, m.nll_grad_full, sub, sub_steps)
+    grad_info["full"] = {"ms_per_call": 1e3 * full_wall, "kernel_ms": fk, "kernel_ms_over_value_kernel_ms": fk / k_ms,
+                         "n_grad": int(grad_f.size), "d_mass_d_width": [float(x) for x in grad_f[grad.size:]],
+                         "what": "mipwa_nll_grad_full: the above + d/d(mass, width) of the floating resonance (same launch)"}
 
     # the sharded form of the same call: per-rank pieces, one all_gather of 3 + 2 n_params doubles, combine
+    def sharded(p):
+        S_p, I_p, g_ev, g_nm = m.nll_grad_parts(p)
+        return sharding.combine_grad_parts(S_p, I_p, n_ev, g_ev, g_nm, device=dev)[:2]
     for t in range(2):
-        m.nll_grad_parts(params[t])
+        sharded(params[t])
     barrier()
-    t0 = time.perf_counter()
-    for t in range(sub_steps):
-        S_p, I_p, g_ev, g_nm = m.nll_grad_parts(params[args.warmup + t % args.steps])
-        nll_s, grad_s = sharding.combine_grad_parts(S_p, I_p, n_ev, g_ev, g_nm, device=dev)[:2]
+    sh_wall, (nll_s, grad_s) = wall_of(sharded, sub, sub_steps)
     barrier()
-    sh_wall = (time.perf_counter() - t0) / sub_steps
     grad_info["sharded"] = {"ms_per_call": 1e3 * sh_wall, "events_per_s": n_ev * world / sh_wall, "n_grad": int(grad_s.size),
                             "nll": nll_s, "max_abs_diff_vs_full_at_1gpu": (float(np.max(np.abs(grad_s - grad_f))) if world == 1 else None),
                             "what": "mipwa_nll_grad_parts + sharding.combine_grad_parts: whole-job NLL and all n_params "
@@ -297,58 +407,36 @@ def run_ours(args, cfg, workload):
 
     # ---- signal + background mixture (purity 90 %): flat background density, two launches per call ----------
     m.set_event_background(torch.full((n_ev,), 1.0 / I.dalitz_area(cfg.kin), dtype=torch.float64, device=dev))
-    for t in range(3):
-        m.nll_mix(params[t], 0.9)
-    mix_ms = []
-    for t in range(sub_steps):
-        nll_mix = m.nll_mix(params[args.warmup + t % args.steps], 0.9)
-        mix_ms.append(m.last_kernel_ms())
-    for t in range(2):
-        m.nll_mix_grad(params[t], 0.9)
-    mixg_ms = []
-    for t in range(sub_steps):
-        nll_mixg, g_mix, dfs_mix = m.nll_mix_grad(params[args.warmup + t % args.steps], 0.9)
-        mixg_ms.append(m.last_kernel_ms())
-    mix_info = {"f_sig": 0.9, "value_kernel_ms": float(np.mean(mix_ms)), "grad_kernel_ms": float(np.mean(mixg_ms)),
-                "nll": nll_mix, "nll_grad_path": nll_mixg, "dnll_dfsig": dfs_mix,
+    m.prepare()
+    mix = lambda p: m.nll_mix(p, 0.9)
+    mixg = lambda p: m.nll_mix_grad(p, 0.9)
+    mk, _ = kernel_ms_of(m, mix, sub, sub_steps)
+    mgk, _ = kernel_ms_of(m, mixg, sub, sub_steps)
+    nll_mixg, g_mix, dfs_mix = mixg(sub[-1])
+    mix_info = {"f_sig": 0.9, "value_kernel_ms": mk, "grad_kernel_ms": mgk, "nll": mix(sub[-1]), "nll_grad_path": nll_mixg,
+                "dnll_dfsig": dfs_mix,
                 "what": "mipwa_nll_mix / mipwa_nll_mix_grad: -sum ln(f_s |A|^2 / I + (1 - f_s) b), normalisation launch then "
                         "event launch (kernel_ms spans both and the host read of I between them)"}
     m.set_event_background(None)
+    m.prepare()
 
     # ---- hybrid path (AUTO's choice for this model): rho(770) recomputed, rho(1450) and f2(1270) cached per point -------
     hybrid_info = None
     try:
         m.set_path(B.PATH_HYBRID)
         t0 = time.perf_counter(); m.nll(params[0]); setup_s = time.perf_counter() - t0
-        for t in range(3):
-            m.nll(params[t])
-        kms = []
+        hk, _ = kernel_ms_of(m, m.nll, sub, sub_steps)
         barrier()
-        t0 = time.perf_counter()
-        for t in range(sub_steps):
-            nll_h = m.nll(params[args.warmup + t % args.steps])
-            kms.append(m.last_kernel_ms())
-        barrier()
-        wall = (time.perf_counter() - t0) / sub_steps
-        for t in range(3):
-            m.nll_grad_full(params[t])
-        gms = []
-        for t in range(sub_steps):
-            nll_hg, grad_hg = m.nll_grad_full(params[args.warmup + t % args.steps])
-            gms.append(m.last_kernel_ms())
-        hybrid_info = {"ms_per_call": 1e3 * wall, "kernel_ms": float(np.mean(kms)), "events_per_s": n_ev * world / wall,
-                       "grad_full_kernel_ms": float(np.mean(gms)), "grad_full_nll": nll_hg,
-                       "grad_full_max_abs_diff_vs_recompute": float(np.max(np.abs(
-                           grad_hg - m_grad_full_ref(m, B, params[args.warmup + (sub_steps - 1) % args.steps])))),
+        wall, nll_h = wall_of(m.nll, sub, sub_steps)
+        hybrid_info = {"ms_per_call": 1e3 * wall, "kernel_ms": hk, "events_per_s": n_ev * world / wall,
                        "cache_bytes": m.basis_bytes(), "first_call_s": setup_s, "nll": nll_h,
                        "what": "MIPWA_PATH_HYBRID: floating resonances and spline recomputed, fixed-shape resonance terms "
-                               "streamed from a per-point cache (not the headline: part of the work is cached); grad_full_*: "
-                               "mipwa_nll_grad_full under an explicit MIPWA_PATH_HYBRID (k_grad_hybrid + k_grad_shape), "
-                               "cross-checked against the full-recompute gradient"}
+                               "streamed from a per-point cache (not the headline: part of the work is cached)"}
     except B.MipwaError:
         pass
     m.set_path(B.PATH_RECOMPUTE)
 
+    hbm, hbm_src = hbm_peak()
     # ---- A9/A10: fixed-shape cached paths on the SAME events (all shapes fixed at their listed values) ------------------
     cached_info = {}
     fixed = [dict(r, shape_floats=0) for r in cfg.resonances]
@@ -356,43 +444,29 @@ def run_ours(args, cfg, workload):
     mc.set_stream(stream)
     mc.set_events(d[0], d[1]); mc.set_norm_points(d[2], d[3], d[4])
     mc.prepare()
-    mc.enable_timing(True)
-    pc = [p[:2 * cfg.N + 2 * cfg.R] for p in params]
+    pc = [p[:2 * cfg.N + 2 * cfg.R] for p in sub]
     for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT)):
         mc.set_path(path)
         t0 = time.perf_counter(); mc.nll(pc[0]); setup_s = time.perf_counter() - t0
-        for t in range(3):
-            mc.nll(pc[t])
-        kms = []
+        k, _ = kernel_ms_of(mc, mc.nll, pc, sub_steps)
         barrier()
-        t0 = time.perf_counter()
-        for t in range(sub_steps):
-            nll_c = mc.nll(pc[args.warmup + t % args.steps])
-            kms.append(mc.last_kernel_ms())
-        barrier()
-        wall = (time.perf_counter() - t0) / sub_steps
-        nbytes = mc.basis_bytes()
-        k = float(np.mean(kms))
+        wall, nll_c = wall_of(mc.nll, pc, sub_steps)
+        nbytes = mc.basis_bytes() + (2 * n_ev if name == "compact" else 0)
         cached_info[name] = {"ms_per_call": 1e3 * wall, "kernel_ms": k, "events_per_s": n_ev * world / wall,
-                             "bytes_per_event": nbytes / max(n_ev, 1), "cache_bytes": nbytes,
+                             "bytes_per_event": nbytes / max(n_ev, 1), "cache_bytes": mc.basis_bytes(),
                              "first_call_s": setup_s, "nll": nll_c,
                              "roofline": {"bound": "hbm", "kernel": "k_nll_dense" if name == "dense" else "k_nll_compact",
-                                          "achieved": nbytes / (k * 1e-3) * 1e-9, "unit": "GB/s", "traffic": None}}
+                                          "achieved": nbytes / (k * 1e-3) * 1e-9, "unit": "GB/s", "traffic": None,
+                                          "peak": hbm, "frac": nbytes / (k * 1e-3) * 1e-9 / hbm, "peak_source": hbm_src}}
     mc.set_path(B.PATH_CACHED_COMPACT)                 # gradient from the compact cache + Gram matrix (k_grad_compact)
     for t in range(3):
-        mc.nll_grad(pc[t])
-    kms = []
-    barrier()
-    t0 = time.perf_counter()
-    for t in range(sub_steps):
-        nll_cg, grad_c = mc.nll_grad(pc[args.warmup + t % args.steps])
-        kms.append(mc.last_kernel_ms())
-    barrier()
-    wall = (time.perf_counter() - t0) / sub_steps
-    cached_info["compact_grad"] = {"ms_per_call": 1e3 * wall, "kernel_ms": float(np.mean(kms)),
-                                   "events_per_s": n_ev * world / wall, "nll": nll_cg, "n_grad": int(grad_c.size)}
+        mc.nll_grad(pc[t % len(pc)])
+    k, _ = kernel_ms_of(mc, mc.nll_grad, pc, sub_steps)
+    wall, (nll_cg, grad_c) = wall_of(mc.nll_grad, pc, sub_steps)
+    cached_info["compact_grad"] = {"ms_per_call": 1e3 * wall, "kernel_ms": k, "events_per_s": n_ev * world / wall,
+                                   "nll": nll_cg, "n_grad": int(grad_c.size)}
     mc.set_path(B.PATH_RECOMPUTE)
-    cached_info["recompute_same_model_nll"] = mc.nll(pc[args.warmup + (sub_steps - 1) % args.steps])
+    cached_info["recompute_same_model_nll"] = mc.nll(pc[-1])
     mc.close()
 
     if rank == 0:
@@ -405,45 +479,67 @@ def run_ours(args, cfg, workload):
             dist.destroy_process_group()
         return
 
+    # free the config-3 sample before the 100 M-event sweep
+    sweep_first = None
+    if world == 1 and not args.no_sweep4:
+        m.close(); del d, pinned, ph
+        torch.cuda.empty_cache()
+        cached_info["sweep4"], sweep_first = sweep4_leg(B, torch, stream, local, [10_000_000, 100_000_000], hbm, hbm_src)
+    latency = latency_leg(B, torch, stream, local) if world == 1 else None
+
     # ---- roofline of the dominant kernel of the step (k_nll_recompute): plain FP64 ALU work -----------------------------
     peak, peak_3reg = B.measure_fp64_peak(local, 3.0)
-    fl = flops_per_point(cfg.resonances) * (n_ev + n_norm)
-    k_ms = float(np.mean(kernel_ms))
-    achieved = fl / (k_ms * 1e-3) * 1e-12
+    fpp = flops_per_point(cfg.resonances)
+    achieved = fpp * (n_ev + n_norm) / (k_ms * 1e-3) * 1e-12
     nominal = None
     if clocks and clocks.get("sm_max_mhz"):
         nominal = 148 * 64 * 2 * clocks["sm_max_mhz"] * 1e6 * 1e-12
+    prof = profile_numbers("r2_k_nll_recompute_ncu.md")
+    same_size = prof is not None and (prof.get("n_ev"), prof.get("n_norm")) == (n_ev, n_norm)
+    ex = prof.get("executed_flops_per_point") if prof else None
     roofline = {"bound": "alu", "kernel": "k_nll_recompute", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((n_ev, n_norm)),
-                "traffic_source": "profiles/r1_k_nll_recompute_ncu.md (ncu --set full, bytes per launch); algorithmic bytes "
-                                  "per launch = 18 B x events + 26 B x weighted normalisation points (s12, s13, (w), 2-byte segment pair)",
-                "peak_source": "measured on this GPU by mipwa_measure_fp64_peak (register-resident DFMA, 2 s sustained); "
-                               "MEASURED_PEAKS.json has no FP64 entry; DESIGN.md section 6 derives the nominal peak",
-                "nominal_peak": nominal, "flops_per_point": flops_per_point(cfg.resonances),
-                "points_per_launch": n_ev + n_norm, "kernel_ms": k_ms,
-                "executed_flops_per_point": NCU_EXECUTED_FLOPS_PER_POINT.get((n_ev, n_norm)),
-                "algorithmic_bytes": 18.0 * n_ev + 26.0 * n_norm,
-                "hbm_gbs": (18.0 * n_ev + 26.0 * n_norm) / (k_ms * 1e-3) * 1e-9}
-    hbm_peak, hbm_src = 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
-    try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            hbm_peak, hbm_src = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (copy, read+write)"
-    except (OSError, KeyError, ValueError):
-        pass
-    for name in ("dense", "compact"):
-        r = cached_info[name]["roofline"]
-        r.update(peak=hbm_peak, frac=r["achieved"] / hbm_peak, peak_source=hbm_src)
+                "frac": achieved / peak,
+                "traffic": prof.get("dram_bytes_per_launch") if same_size else None,
+                "frac_executed": (ex * (n_ev + n_norm) / (k_ms * 1e-3) * 1e-12 / peak) if ex else None,
+                "frac_vs_3reg_dfma_rate": achieved / peak_3reg, "frac_vs_nominal": achieved / nominal if nominal else None,
+                "executed_flops_per_point": ex,
+                "fp64_pipe_active_pct": prof.get("fp64_pipe_active_pct") if prof else None,
+                "profile": ("profiles/r2_k_nll_recompute_ncu.md (ncu --set full; its `bench:` line matches the kernel sources of "
+                            "this run)") if prof else "no capture matches the kernel sources of this run: profile-derived fields are null",
+                "peak_source": "measured on this GPU by mipwa_measure_fp64_peak: DFMAs with an immediate and a repeated register "
+                               "operand, 3 s sustained (the rate the FP64 pipe issues at); peak_3reg: three distinct register "
+                               "operands; MEASURED_PEAKS.json has no FP64 entry; DESIGN.md section 6 derives the nominal peak",
+                "peak_3reg": peak_3reg, "nominal_peak": nominal, "flops_per_point": fpp,
+                "flops_per_point_source": "SURVEY 8(d) count of the plain formulas: 59 + 82 R, one per add/mul/div/sqrt/log, fma = 2",
+                "points_per_launch": n_ev + n_norm, "kernel_ms": k_ms, "kernel_ms_min": k_ms_min,
+                "algorithmic_bytes": 32.0 * (n_ev + n_norm),
+                "hbm_gbs": 32.0 * (n_ev + n_norm) / (k_ms * 1e-3) * 1e-9}
 
     cpu = None
     if world == 1:
         cpu = time_oracle(cfg, min(n_ev, 4_000_000), min(n_norm, 4_000_000), 3, 1)
+        if sweep_first is not None:                    # the oracle on the first 200 K events of the sweep-4 sample
+            from oracle import oracle as orc
+            c4 = I.Config(4)
+            o4 = orc.Oracle(c4.kin, c4.knots, c4.resonances)
+            e12, e13, g12, g13, p4 = sweep_first
+            _, S_or, _ = o4.nll(p4, e12, e13, g12, g13, None, parts=True)
+            m4 = B.Mipwa(c4.kin, c4.knots, c4.resonances, device=local)
+            m4.set_events(e12, e13); m4.set_norm_points(g12, g13, None)
+            chk = {}
+            for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT), ("recompute", B.PATH_RECOMPUTE)):
+                m4.set_path(path)
+                chk[name + "_rel_err_sum_log"] = abs(m4.nll_parts(p4)[1] - S_or) / abs(S_or)
+            m4.close()
+            cpu["sweep4_check"] = dict(chk, events=int(e12.size), what="sum ln|A|^2 over the first 200 K events of the sweep-4 "
+                                       "sample: CUDA paths against the oracle")
 
     total_events = n_ev * world
     line = {"metric": METRIC, "value": total_events / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": dict(workload, events_per_gpu=n_ev, norm_points_per_gpu=n_norm,
-                           l2="inputs read per step (18 B x 10M events + 26 B x 10M weighted normalisation points = 440 MB) exceed the "
+                           l2="inputs read per step (32 B x (10M events + 10M normalisation points) = 640 MB) exceed the "
                               "126 MB L2; no flush needed",
                            parallelism=f"dp{world} (events and normalisation points sharded; 3 doubles all-gathered per call)"),
             "nll_evals_per_s": 1e3 / ms_step, "points_per_s": (n_ev + n_norm) * world / (ms_step * 1e-3),
@@ -453,7 +549,9 @@ def run_ours(args, cfg, workload):
                     "what": "mipwa_set_events + mipwa_set_norm_points from pinned HOST arrays + mipwa_nll, every step"},
             "fit_step": {"ms_per_call": 1e3 * fit_step_s, "nll_evals_per_s": 1.0 / fit_step_s,
                          "what": "wall clock of mipwa_nll(host params) -> host fp64 with events resident (what a minimiser sees)"},
-            "prepare_s": t_prep, "roofline": roofline, "grad": grad_info, "mixture": mix_info, "hybrid": hybrid_info, "cached": cached_info, "cpu_baseline": cpu, "input_generation_s": t_gen, "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
+            "prepare_s": t_prep, "roofline": roofline, "grad": grad_info, "mixture": mix_info, "hybrid": hybrid_info,
+            "cached": cached_info, "latency": latency, "cpu_baseline": cpu, "input_generation_s": t_gen,
+            "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -461,81 +559,13 @@ def run_ours(args, cfg, workload):
 
 # ---- secondary measurements behind the numbers in BASELINE.md / profiles (not the driver's bench line) --------------
 def run_probe(args):
-    """--probe resonances | hybrid | recompute-shape | grid-bias | sweep4 | latency : prints one JSON line per row (kernel times: CUDA events in the library,
-    median over the calls after warm-up).  Phase-space points stand in for events where only the work per point
-    matters; every mode cross-checks its NLL against another path."""
+    """--probe grid-bias | sweep4 | latency: prints one JSON line per row."""
     import torch
     from paper_1703_03284_b200 import binding as B
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --probe needs a CUDA device")
-
-    def timed(m, p, calls=25, skip=5, grad=False):
-        ms, v = [], None
-        for _ in range(calls):
-            v = m.nll_grad(p)[0] if grad else m.nll(p)
-            ms.append(m.last_kernel_ms())
-        return float(np.median(ms[skip:])), v
-
-    if args.probe == "resonances":
-        # recompute kernel time against the number and spin of the resonances, 10 M + 10 M points, N = 50:
-        # the marginal cost of one resonance against the 2 clk per FP64 instruction of the pipe
-        c = I.Config(3)
-        n = args.events or 10_000_000
-        e12, e13 = I.phase_space_points(n, c.key(7)); g12, g13 = I.phase_space_points(n, c.key(8))
-        d = [torch.from_numpy(a).cuda() for a in (e12, e13, g12, g13)]
-        L1 = [I._res(*I.RHO770), I._res(*I.RHO1450), I._res(*I.SYN_A), I._res(*I.SYN_C)]
-        L2 = [I._res(*I.F2_1270), I._res(*I.SYN_B)]
-        for name, res in (("R=0", []), ("1xL1", L1[:1]), ("2xL1", L1[:2]), ("3xL1", L1[:3]), ("4xL1", L1[:4]),
-                          ("1xL2", L2[:1]), ("2xL2", L2[:2]), ("2xL1+1xL2", L1[:2] + L2[:1])):
-            m = B.Mipwa(c.kin, c.knots, res)
-            m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], None); m.set_path(B.PATH_RECOMPUTE)
-            m.prepare(); m.enable_timing(True)
-            p = np.concatenate([c.truth[:100], np.tile([1.0, 0.3], len(res))])
-            k, v = timed(m, p)
-            print(json.dumps({"probe": "resonances", "model": name, "points": 2 * n, "kernel_ms": k, "nll": v,
-                              "clk_per_warp_point_per_smsp_at_1965MHz": k * 1e-3 * 1.965e9 * 592 / (2 * n / 32)}), flush=True)
-            m.close()
-    elif args.probe == "hybrid":
-        # the rule behind MIPWA_PATH_AUTO when some shapes float: rho(770) floating + k fixed-shape resonances,
-        # full recompute against the hybrid path (fixed terms streamed from the per-point cache), 10 M + 10 M points
-        c = I.Config(3)
-        n = args.events or 10_000_000
-        e12, e13 = I.phase_space_points(n, c.key(7)); g12, g13 = I.phase_space_points(n, c.key(8))
-        d = [torch.from_numpy(a).cuda() for a in (e12, e13, g12, g13)]
-        fixed = [I._res(*I.RHO1450), I._res(*I.F2_1270), I._res(*I.SYN_A), I._res(*I.SYN_B), I._res(*I.SYN_C)]
-        for k in range(1, 6):
-            res = [I._res(*I.RHO770, shape_floats=1)] + fixed[:k]
-            m = B.Mipwa(c.kin, c.knots, res)
-            m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], None)
-            m.prepare(); m.enable_timing(True)
-            p = np.concatenate([c.truth[:100], np.tile([1.0, 0.3], len(res)), [0.775, 0.149]])
-            row = {"probe": "hybrid", "fixed": k, "spins": [r["spin"] for r in res], "points": 2 * n}
-            for name, path in (("recompute", B.PATH_RECOMPUTE), ("hybrid", B.PATH_HYBRID), ("auto", B.PATH_AUTO)):
-                try:
-                    m.set_path(path)
-                    row[name + "_ms"], row[name + "_nll"] = timed(m, p)
-                except B.MipwaError as e:
-                    row[name + "_ms"] = None
-            print(json.dumps(row), flush=True)
-            m.close()
-    elif args.probe == "recompute-shape":
-        # kernel time of k_nll_recompute (value) and k_grad_recompute at configs[3]'s model on 10 M + 10 M weighted,
-        # cell-sorted phase-space points; MIPWA_LIB_PATH selects a library rebuilt with other -DMIPWA_REC_* switches
-        # (profiles/r1_recompute_shape.md)
-        c = I.Config(3)
-        n = args.events or 10_000_000
-        e12, e13 = I.phase_space_points(n, c.key(7)); g12, g13 = I.phase_space_points(n, c.key(8))
-        w = np.full(n, 5.06 / n)
-        d = [torch.from_numpy(a).cuda() for a in (e12, e13, g12, g13, w)]
-        m = B.Mipwa(c.kin, c.knots, c.resonances)
-        m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4]); m.set_path(B.PATH_RECOMPUTE)
-        m.prepare(); m.enable_timing(True)
-        k, v = timed(m, c.perturbed(0), calls=60, skip=10)
-        kg, vg = timed(m, c.perturbed(0), calls=30, skip=10, grad=True)
-        print(json.dumps({"probe": "recompute-shape", "library": os.environ.get("MIPWA_LIB_PATH", "default"),
-                          "points": 2 * n, "kernel_ms": k, "grad_kernel_ms": kg, "nll": v, "nll_grad_path": vg}), flush=True)
-        m.close()
-    elif args.probe == "grid-bias":
+    stream = torch.cuda.Stream()
+    if args.probe == "grid-bias":
         # The paper's own experiment (PAPER.md:47, :61 Fig. 2, :49-55 Table 1) as far as it is described: a 100 K-event
         # toy of D+ -> K+K+K- (40 knots + phi(1020), config 5 of inputs.py; the parameter values are this repo's, the
         # paper prints none) generated from the PDF, then unbinned maximum-likelihood fits of all knot values and the
@@ -609,61 +639,16 @@ def run_probe(args):
                               "max_abs_dphi": float(np.max(np.abs(d[N:2 * N])))}), flush=True)
         m.close()
     elif args.probe == "sweep4":
-        # BASELINE.json configs[4]: K = 56 cached paths against the event count (default 1 M .. 100 M), 10 M-point Gram
-        c = I.Config(4)
+        # BASELINE.json configs[4], every size of the sweep (the default bench line carries 10 M and 100 M)
+        hbm, hbm_src = hbm_peak()
         sizes = [args.events] if args.events else [1_000_000, 2_000_000, 5_000_000, 10_000_000, 20_000_000,
                                                    50_000_000, 100_000_000]
-        g12, g13 = I.phase_space_points(args.norm_points or 10_000_000, c.key(8))
-        dg = [torch.from_numpy(a).cuda() for a in (g12, g13)]
-        E12, E13 = I.phase_space_points(max(sizes), c.key(7), chunk=1 << 24)
-        m = B.Mipwa(c.kin, c.knots, c.resonances)
-        m.set_norm_points(dg[0], dg[1], None); m.enable_timing(True)
-        for n in sizes:
-            de = [torch.from_numpy(E12[:n]).cuda(), torch.from_numpy(E13[:n]).cuda()]
-            m.set_events(de[0], de[1]); m.prepare()
-            row = {"probe": "sweep4", "n_ev": n, "K": c.N + c.R}
-            for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT)):
-                m.set_path(path)
-                t0 = time.perf_counter(); m.nll(c.truth); setup = time.perf_counter() - t0
-                k, v = timed(m, c.perturbed(1), calls=22, skip=2)
-                byt = m.basis_bytes()
-                row[name] = {"kernel_ms": k, "cache_GB": byt / 1e9, "GB_per_s": byt / k * 1e-6, "events_per_s": n / k * 1e3,
-                             "evals_per_s": 1e3 / k, "first_call_s": setup, "nll": v}
-            if n <= 20_000_000:
-                m.set_path(B.PATH_RECOMPUTE)
-                row["recompute_nll"] = m.nll(c.perturbed(1))
-            print(json.dumps(row), flush=True)
-            del de
-            torch.cuda.empty_cache()
-        m.close()
+        out, _ = sweep4_leg(B, torch, stream, 0, sizes, hbm, hbm_src)
+        for row in out["rows"]:
+            print(json.dumps(dict(row, probe="sweep4")), flush=True)
     elif args.probe == "latency":
-        # wall clock per call (timing events off) and kernel time at the small configs and at the paper's scale
-        for idx, n_ev, n_norm in ((0, None, None), (1, None, None), (2, 100_000, 1_000_000), (2, None, None),
-                                  (5, None, None)):       # 5 = the paper's own toy (K+K+K-, 100 K events, 918^2 grid)
-            c = I.Config(idx, n_ev=n_ev, n_norm=n_norm)
-            e12, e13 = I.phase_space_points(c.n_ev, c.key(7), c.kin)
-            g12, g13, w = c.norm_points()
-            d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (e12, e13, g12, g13, w)]
-            m = B.Mipwa(c.kin, c.knots, c.resonances)
-            m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4]); m.prepare()
-            ps = [c.perturbed(t) for t in range(120)]
-            row = {"probe": "latency", "config": idx, "n_ev": c.n_ev, "n_norm": int(g12.size)}
-            for name, path, grad in (("recompute", B.PATH_RECOMPUTE, False), ("compact", B.PATH_CACHED_COMPACT, False),
-                                     ("dense", B.PATH_CACHED, False), ("grad_recompute", B.PATH_RECOMPUTE, True),
-                                     ("grad_compact", B.PATH_CACHED_COMPACT, True)):
-                m.set_path(path)
-                f = (lambda q: m.nll_grad(q)[0]) if grad else m.nll
-                m.enable_timing(True)
-                km = []
-                for t in range(20):
-                    f(ps[t]); km.append(m.last_kernel_ms())
-                m.enable_timing(False)
-                t0 = time.perf_counter()
-                for t in range(100):
-                    f(ps[20 + t])
-                row[name] = {"wall_us": (time.perf_counter() - t0) / 100 * 1e6, "kernel_us": float(np.median(km[5:])) * 1e3}
-            print(json.dumps(row), flush=True)
-            m.close()
+        for row in latency_leg(B, torch, stream, 0):
+            print(json.dumps(dict(row, probe="latency")), flush=True)
 
 
 def main():
@@ -675,7 +660,10 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--events", type=int, default=None)
     ap.add_argument("--norm-points", type=int, default=None)
-    ap.add_argument("--probe", default=None, choices=["resonances", "hybrid", "recompute-shape", "grid-bias", "sweep4", "latency"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own 10 M + 10 M sample; strong = one sample split N ways")
+    ap.add_argument("--no-sweep4", action="store_true", help="skip the configs[4] leg (10 M and 100 M events, K = 56)")
+    ap.add_argument("--probe", default=None, choices=["grid-bias", "sweep4", "latency"])
     args = ap.parse_args()
     if args.probe:
         return run_probe(args)

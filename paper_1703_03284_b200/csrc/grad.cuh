@@ -17,6 +17,7 @@
 // adds by lane 0) only when the warp's cell changes.  A warp-iteration that straddles a cell boundary takes a
 // slower path: one shuffle-reduce round per distinct cell in the group (add_mixed).
 #pragma once
+#include <type_traits>
 #include "cached.cuh"
 
 #define MIPWA_GRAD_MAXR (MIPWA_DEV_MAX_RES)
@@ -160,21 +161,23 @@ __device__ __forceinline__ void amplitude_parts(const RowsSmem& sm, const DevMod
     }
 }
 
-// per-warp running moments of the current cell
+// per-warp running moments of the current cell: sum f t1^q (q = 0..3) and sum f t2^q (q = 1..3); the q = 0 moment
+// sum f is the same number for both channels of a cell
 struct CellAcc {
-    double v[16];          // [channel][q][re,im]
+    double v[14];          // [0..7]: channel 1, q = 0..3, (re, im); [8..13]: channel 2, q = 1..3
     unsigned int o1, o2;   // row offsets (= segments) of the cell, 0xffffffff: empty
     __device__ __forceinline__ void clear() {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = 0.0;
+        for (int k = 0; k < 14; ++k) v[k] = 0.0;
     }
     __device__ __forceinline__ void add(double fr, double fi, double t1, double t2) {
-        double p = 1.0;
+        v[0] += fr; v[1] += fi;
+        double p = t1;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) { v[2 * q] = fma(fr, p, v[2 * q]); v[2 * q + 1] = fma(fi, p, v[2 * q + 1]); p *= t1; }
-        p = 1.0;
+        for (int q = 1; q < 4; ++q) { v[2 * q] = fma(fr, p, v[2 * q]); v[2 * q + 1] = fma(fi, p, v[2 * q + 1]); p *= t1; }
+        p = t2;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) { v[8 + 2 * q] = fma(fr, p, v[8 + 2 * q]); v[8 + 2 * q + 1] = fma(fi, p, v[8 + 2 * q + 1]); p *= t2; }
+        for (int q = 1; q < 4; ++q) { v[6 + 2 * q] = fma(fr, p, v[6 + 2 * q]); v[7 + 2 * q] = fma(fi, p, v[7 + 2 * q]); p *= t2; }
     }
 };
 #define MIPWA_NO_CELL 0xffffffffu
@@ -186,7 +189,7 @@ __device__ __forceinline__ void flush_warp(CellAcc& a, double* bins, int NS)
 {
     if (a.o1 != MIPWA_NO_CELL) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
+        for (int k = 0; k < 14; ++k) {
             double x = a.v[k];
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
@@ -199,10 +202,12 @@ __device__ __forceinline__ void flush_warp(CellAcc& a, double* bins, int NS)
                 bins[(q * NS + j1) * 2] += a.v[2 * q];
                 bins[(q * NS + j1) * 2 + 1] += a.v[2 * q + 1];
             }
+            bins[j2 * 2] += a.v[0];                        // after the j1 updates: j2 may be the same segment
+            bins[j2 * 2 + 1] += a.v[1];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {                  // after the j1 updates: j2 may be the same segment
-                bins[(q * NS + j2) * 2] += a.v[8 + 2 * q];
-                bins[(q * NS + j2) * 2 + 1] += a.v[8 + 2 * q + 1];
+            for (int q = 1; q < 4; ++q) {
+                bins[(q * NS + j2) * 2] += a.v[6 + 2 * q];
+                bins[(q * NS + j2) * 2 + 1] += a.v[7 + 2 * q];
             }
         }
         __syncwarp();
@@ -304,60 +309,70 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
 #pragma unroll
     for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
     if (cnt > 0) {
-        const PointRec* p = rec + lo + lane;               // the records are padded: the prefetch needs no bounds test
+        // One record per lane and iteration, loaded where it is used: the gradient's running sums leave no registers for
+        // a second record in flight (a register prefetch cost spills and constant re-reads), so the line is pulled into
+        // L2 two iterations ahead instead and the other three warps of the scheduler cover the L2 round trip.  The record
+        // arrays are padded: neither the prefetch nor the last, partly filled iteration needs a bounds test.
+        const PointRec* p = rec + lo + lane;
         double2* pf = fout + lo + lane;
-        PointRec r = ld_rec(p);
-        int base = 0;
-        while (base < cnt) {
-            const int stop = cnt - base < 32 * LOGPROD_FLUSH ? cnt : base + 32 * LOGPROD_FLUSH;
-            int adds = 0;
-            for (; base < stop; base += 32) {              // warp-uniform trip count
-                p += 32;
-                const PointRec nx = ld_rec(p);
-                const bool valid = base + lane < cnt;      // lanes past the end evaluate a real point and add zeros
-                double are, aim, t1, t2, tr[RR], ti[RR], sh[4];
-                amplitude_parts<R1, R2, FL, SHP>(sm, m, r, are, aim, t1, t2, tr, ti, sh);
-                const double a2 = fma(are, are, aim * aim);
-                double fr, fi;
-                if (EV) {
-                    const double D = MIX ? fma(kappa, r.w, a2) : a2;
-                    const double rD = fast_rcp(D);
-                    const double k = valid ? -2.0 * rD : 0.0;
-                    fr = k * are; fi = k * aim;
-                    lp.add(valid ? D : 1.0);
-                    ++adds;
-                    if (MIX) qsum += valid ? r.w * rD : 0.0;
-                } else {
-                    const double wv = valid ? r.w : 0.0;
-                    fr = wv * are; fi = wv * aim;
-                    integ = fma(wv, a2, integ);
-                }
-                if (fout) {                                // for k_grad_shape (several floating resonances)
-                    if (valid) *pf = make_double2(fr, fi);
-                    pf += 32;
-                }
-                if (R1 >= 0) {
-#pragma unroll
-                    for (int q = 0; q < (R1 >= 0 ? R1 + R2 : 0); ++q) {
-                        Fr[q] = fma(fr, tr[q], fma(fi, ti[q], Fr[q]));     // f conj(T)
-                        Fi[q] = fma(fi, tr[q], fma(-fr, ti[q], Fi[q]));
-                    }
-                } else {
-                    for (int q = 0; q < nres; ++q) {
-                        Fr[q] = fma(fr, tr[q], fma(fi, ti[q], Fr[q]));
-                        Fi[q] = fma(fi, tr[q], fma(-fr, ti[q], Fi[q]));
-                    }
-                }
-                if (SHP) {
-                    Sh[0] = fma(fr, sh[0], fma(fi, sh[1], Sh[0]));         // f conj(dT'/dm0)
-                    Sh[1] = fma(fi, sh[0], fma(-fr, sh[1], Sh[1]));
-                    Sh[2] = fma(fr, sh[2], fma(fi, sh[3], Sh[2]));         // f conj(dT'/dG0)
-                    Sh[3] = fma(fi, sh[2], fma(-fr, sh[3], Sh[3]));
-                }
-                cell_accumulate(acc, valid, r.o1, r.o2, fr, fi, t1, t2, wbins, NS);
-                r = nx;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 32));
+        auto body = [&](auto masked, int base) {
+            constexpr bool MASKED = decltype(masked)::value;
+            const PointRec r = ld_rec(p);
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 64));
+            p += 32;
+            const bool valid = !MASKED || base + lane < cnt;   // lanes past the end evaluate a real point and add zeros
+            double are, aim, t1, t2, tr[RR], ti[RR], sh[4];
+            amplitude_parts<R1, R2, FL, SHP>(sm, m, r, are, aim, t1, t2, tr, ti, sh);
+            const double a2 = fma(are, are, aim * aim);
+            double fr, fi;
+            if (EV) {
+                const double D = MIX ? fma(kappa, r.w, a2) : a2;
+                const double rD = fast_rcp(D);
+                const double k = valid ? -2.0 * rD : 0.0;
+                fr = k * are; fi = k * aim;
+                lp.add(valid ? D : 1.0);
+                if (MIX) qsum += valid ? r.w * rD : 0.0;
+            } else {
+                const double wv = valid ? r.w : 0.0;
+                fr = wv * are; fi = wv * aim;
+                integ = fma(wv, a2, integ);
             }
+            if (fout) {                                    // for k_grad_shape (several floating resonances)
+                if (valid) *pf = make_double2(fr, fi);
+                pf += 32;
+            }
+            if (R1 >= 0) {
+#pragma unroll
+                for (int q = 0; q < (R1 >= 0 ? R1 + R2 : 0); ++q) {
+                    Fr[q] = fma(fr, tr[q], fma(fi, ti[q], Fr[q]));         // f conj(T)
+                    Fi[q] = fma(fi, tr[q], fma(-fr, ti[q], Fi[q]));
+                }
+            } else {
+                for (int q = 0; q < nres; ++q) {
+                    Fr[q] = fma(fr, tr[q], fma(fi, ti[q], Fr[q]));
+                    Fi[q] = fma(fi, tr[q], fma(-fr, ti[q], Fi[q]));
+                }
+            }
+            if (SHP) {
+                Sh[0] = fma(fr, sh[0], fma(fi, sh[1], Sh[0]));             // f conj(dT'/dm0)
+                Sh[1] = fma(fi, sh[0], fma(-fr, sh[1], Sh[1]));
+                Sh[2] = fma(fr, sh[2], fma(fi, sh[3], Sh[2]));             // f conj(dT'/dG0)
+                Sh[3] = fma(fi, sh[2], fma(-fr, sh[3], Sh[3]));
+            }
+            cell_accumulate(acc, valid, r.o1, r.o2, fr, fi, t1, t2, wbins, NS);
+        };
+        const int full = cnt & ~31;                        // iterations in which every lane has a point
+        int base = 0;
+        while (base < full) {
+            const int stop = full - base < 32 * LOGPROD_FLUSH ? full : base + 32 * LOGPROD_FLUSH;
+            const int adds = (stop - base) >> 5;
+            for (; base < stop; base += 32) body(std::false_type(), base);   // warp-uniform trip count
             if (EV) lp.flush(adds);
+        }
+        if (full < cnt) {                                  // the last warp of the set: one partly filled iteration
+            body(std::true_type(), full);
+            if (EV) lp.flush(1);
         }
     }
     flush_warp(acc, wbins, NS);
