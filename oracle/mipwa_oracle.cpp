@@ -120,6 +120,7 @@ void spline_weights(int n, const double* x, double s, int* j_out, double w[4])
 
 cplx spline_eval(int n, const double* x, const cplx* y, const cplx* ypp, double s)
 {
+    if (n == 0) return cplx(0.0, 0.0);                                    // no MIPWA S-wave (Isobar model, O6b)
     int j;
     double w[4];
     spline_weights(n, x, s, &j, w);
@@ -268,14 +269,27 @@ Unpacked unpack(const Model& m, const double* p)
     return u;
 }
 
+// O6b Isobar-model pieces ("the S-wave is represented by a sum of a constant non-resonant term and
+//     Breit-Wigner functions"; "a constant nonresonant amplitude"; reading P27):
+//     a list entry with spin = ORC_SPIN_NONRES is the constant term: its basis function is 1 over the whole Dalitz
+//     plot (one term, not doubled by the symmetrisation: a constant is its own mirror image and any factor is
+//     absorbed by its coefficient); mass, width and radii of that entry are not used.  Scalar Breit-Wigners are the
+//     spin-0 case of O5 (F_R = F_D = Z_0 = 1).  n = 0 knots switches the spline S-wave off.
+const int ORC_SPIN_NONRES = -1;
+
+cplx symmetrised_term(const orc_kin& k, const orc_res& r, double s12, double s13)
+{
+    if (r.spin == ORC_SPIN_NONRES) return cplx(1.0, 0.0);
+    return resonance_term(k, r, s12, s13) + resonance_term(k, r, s13, s12);
+}
+
 // O6  A(s12,s13) = S(s12) + S(s13) + sum_r c_r [T_r(s12,s13) + T_r(s13,s12)]
 //     (Eq. 1; symmetrisation PAPER.md:47, reading P8 plain sum; S-wave has no coefficient PAPER.md:37)
 cplx amplitude(const Model& m, const Unpacked& u, double s12, double s13)
 {
     cplx A = spline_eval(m.n, m.x.data(), u.y.data(), u.ypp.data(), s12)
            + spline_eval(m.n, m.x.data(), u.y.data(), u.ypp.data(), s13);
-    for (int r = 0; r < m.R; ++r)
-        A += u.c[r] * (resonance_term(m.kin, u.res[r], s12, s13) + resonance_term(m.kin, u.res[r], s13, s12));
+    for (int r = 0; r < m.R; ++r) A += u.c[r] * symmetrised_term(m.kin, u.res[r], s12, s13);
     return A;
 }
 
@@ -439,7 +453,7 @@ static void basis_row(const Model& m, const std::vector<orc_res>& res, const std
 {
     for (int k = 0; k < m.n; ++k) B[k] = 0.0;
     const double ss[2] = { s12, s13 };
-    for (int ch = 0; ch < 2; ++ch) {
+    for (int ch = 0; ch < 2 && m.n > 0; ++ch) {
         int j;
         double w[4];
         spline_weights(m.n, m.x.data(), ss[ch], &j, w);
@@ -450,8 +464,7 @@ static void basis_row(const Model& m, const std::vector<orc_res>& res, const std
             B[k] += b;
         }
     }
-    for (int r = 0; r < m.R; ++r)
-        B[m.n + r] = resonance_term(m.kin, res[r], s12, s13) + resonance_term(m.kin, res[r], s13, s12);
+    for (int r = 0; r < m.R; ++r) B[m.n + r] = symmetrised_term(m.kin, res[r], s12, s13);
 }
 
 // basis rows for npts points, row-major out[(i*K + k)*2 + {0,1}] = Re, Im.  params only supplies floating shapes.
