@@ -47,9 +47,15 @@ typedef struct {
     double m_parent, m1, m2, m3;                    /* GeV; m2 == m3 */
 } mipwa_kinematics;
 
+/* spin of the list entry that stands for the CONSTANT NON-RESONANT amplitude of the Isobar model ("a sum of
+ * a constant non-resonant term and Breit-Wigner functions"): it contributes c_r x 1 over the whole Dalitz
+ * plot (not doubled by the symmetrisation: DESIGN.md reading P27); its mass, width and radii are ignored, its
+ * (|c_r|, arg c_r) sit in the parameter vector like those of a resonance.  At most one per model, never floating. */
+#define MIPWA_SPIN_NONRES (-1)
+
 typedef struct {
     double  mass, width;                            /* m0, Gamma0 in GeV (initial values when shape_floats = 1) */
-    int32_t spin;                                   /* L = 0, 1, 2; larger -> MIPWA_ERR_ARG */
+    int32_t spin;                                   /* L = 0, 1, 2 or MIPWA_SPIN_NONRES; else MIPWA_ERR_ARG */
     int32_t shape_floats;                           /* 1: (mass, width) are read from the parameter vector */
     double  r_res, r_parent;                        /* Blatt-Weisskopf radii, GeV^-1 */
 } mipwa_resonance;
@@ -68,8 +74,11 @@ enum { MIPWA_PATH_AUTO = 0,            /* no shape floats: cached-compact; some 
 #define MIPWA_MAX_RESONANCES 16
 
 /* Create a context for one model on CUDA device `device`.
- *   knots: n_knots strictly increasing positions in m^2 (HOST), 2 <= n_knots <= MIPWA_MAX_KNOTS
- *   res:   n_res resonance descriptions (HOST), 0 <= n_res <= MIPWA_MAX_RESONANCES
+ *   knots: n_knots strictly increasing positions in m^2 (HOST), 2 <= n_knots <= MIPWA_MAX_KNOTS;
+ *          n_knots = 0 (knots may be NULL): no spline S-wave - the Isobar comparison model of PAPER.md:27, whose
+ *          S-wave is scalar (spin 0) Breit-Wigners plus the MIPWA_SPIN_NONRES term
+ *   res:   n_res resonance descriptions (HOST), 0 <= n_res <= MIPWA_MAX_RESONANCES;
+ *          n_knots + n_res >= 1
  * Errors: MIPWA_ERR_ARG (bad masses / knots / spin / radii / counts), MIPWA_ERR_CUDA (no device, not sm_100). */
 int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_knots,
                  const mipwa_resonance* res, int32_t n_res, int32_t device, mipwa_ctx** out);

@@ -25,6 +25,8 @@ struct CoefDev {                    // the linear coefficients of one call, a __
 struct BasisAux {
     const double* Mx;               // N x N row-major: y''_j = sum_k Mx[j*N + k] y_k (natural spline, knots only)
     uint8_t col_of_slot[MIPWA_DEV_MAX_RES];   // device slot d holds the caller's resonance col_of_slot[d]
+    int32_t nonres_col;             // caller's index of the constant non-resonant term (its basis function is 1), -1: none
+    int32_t n_res_cols;             // resonance columns of the basis (the caller's list length: m.R + the constant term)
 };
 
 // ---- NR-form local weights: S(s) = A y_j + B y_j+1 + C y''_j + D y''_j+1 -----------------------------------------
@@ -71,6 +73,9 @@ __device__ __forceinline__ void basis_point(const SearchSmem& ss, const DevModel
             emit(m.N + aux.col_of_slot[d], make_double2(m.res[d].cre * tr, m.res[d].cre * ti));
         }
     }
+    // the constant term: a column of ones in the dense basis; the compact layouts carry it in the spline tables
+    // (mipwa.cu: build_model) and keep a column of zeros in its place
+    if (aux.nonres_col >= 0 && k0 == 0) emit(m.N + aux.nonres_col, make_double2(spline_cols ? 1.0 : 0.0, 0.0));
 }
 
 // ---- A9: build the per-event cache -------------------------------------------------------------------------------
@@ -81,7 +86,7 @@ k_basis_build(const __grid_constant__ DevModel m, const DevSearch* __restrict__ 
 {
     __shared__ SearchSmem sm;
     load_search_smem(sm, srch);
-    const int C = COMPACT ? 1 + m.R : m.N + m.R;
+    const int C = COMPACT ? 1 + aux.n_res_cols : m.N + aux.n_res_cols;
     const long long n_tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const long long i = tile * MIPWA_TILE + threadIdx.x;
@@ -106,7 +111,7 @@ k_basis_rows(const __grid_constant__ DevModel m, const DevSearch* __restrict__ s
 {
     __shared__ SearchSmem sm;
     load_search_smem(sm, srch);
-    const int K = m.N + m.R;
+    const int K = m.N + aux.n_res_cols;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
         basis_point(sm, m, aux, s12[first + i], s13[first + i], 0, 1, true,
@@ -231,7 +236,7 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
     load_rows_smem(sm, m);
-    const int R = RT >= 0 ? RT : m.R, C = 1 + R, N = cc.N;
+    const int R = RT >= 0 ? RT : cc.K - cc.N, C = 1 + R, N = cc.N;
     const long long n_tiles = (n_ev + MIPWA_TILE - 1) / MIPWA_TILE;
     LogProd lp;
     if (RT >= 0) {
@@ -320,7 +325,7 @@ k_gram(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, c
     __shared__ SearchSmem sm;
     __shared__ double ws[GRAM_P], wsi[GRAM_P];
     load_search_smem(sm, srch);
-    const int K = m.N + m.R, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, rows = 4 * nt;
+    const int K = m.N + aux.n_res_cols, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, rows = 4 * nt;
     double2* Bs = gram_smem;                                       // [rows][GRAM_LD]
     for (int idx = threadIdx.x; idx < rows * GRAM_LD; idx += blockDim.x) Bs[idx] = make_double2(0.0, 0.0);
 

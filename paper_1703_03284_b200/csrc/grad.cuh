@@ -488,7 +488,7 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
     extern __shared__ double grad_bins[];                  // [warp][4][N-1][2]
     __shared__ RowsSmem sm;
     __shared__ double red32[32];
-    const int R = RT >= 0 ? RT : m.R, C = 1 + R, N = cc.N, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;
+    const int R = RT >= 0 ? RT : cc.K - cc.N, C = 1 + R, N = cc.N, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
     for (int k = threadIdx.x; k < wpb * nb; k += blockDim.x) grad_bins[k] = 0.0;
     load_rows_smem(sm, m);

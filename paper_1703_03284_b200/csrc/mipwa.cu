@@ -49,7 +49,12 @@ struct NvtxRange {
 
 struct mipwa_ctx {
     mipwa_kinematics kin;
-    int N = 0, R = 0, F = 0;
+    // N: knots of the spline tables the kernels use (>= 2); Np: knots in the parameter vector (the caller's n_knots: 0
+    // for an Isobar model, whose constant term rides on a two-knot table); R: resonance-list entries, the constant
+    // non-resonant one (index nr_idx, -1: none) included; F: floating shapes
+    int N = 0, Np = 0, R = 0, F = 0, nr_idx = -1;
+    int n_par() const { return 2 * Np + 2 * R + 2 * F; }   // length of the parameter vector
+    int pb() const { return 2 * Np; }                      // first entry of the resonance block
     std::vector<double> knots;
     std::vector<mipwa_resonance> res;
     int n_spin[3] = { 0, 0, 0 };   // resonances of spin 0, 1, 2 (the kernel signature)
@@ -80,7 +85,9 @@ struct mipwa_ctx {
     unsigned long long* d_bad = nullptr;
 
     DevModel model;                 // staging for the current call
-    std::vector<double> y_re, y_im, ypp_re, ypp_im;
+    std::vector<double> y_re, y_im;          // knot values a_k e^{i phi_k} of the call (zero for the two stand-in knots)
+    std::vector<double> ys_re, ys_im;        // the values the tables are built from: y_k + c_nr / 2
+    std::vector<double> ypp_re, ypp_im;
 
     // fixed-shape path (A9, A10)
     std::vector<double> Mx;         // N x N: y'' = Mx y (knots only)
@@ -260,21 +267,29 @@ void fill_static_model(mipwa_ctx* c)
 // A1-A3: parameters -> DevModel
 int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
 {
-    const int N = c->N, R = c->R;
-    if (n_params != 2 * N + 2 * R + 2 * c->F)
-        return fail(c, MIPWA_ERR_ARG, "n_params must be " + std::to_string(2 * N + 2 * R + 2 * c->F));
+    const int N = c->N, Np = c->Np, R = c->R, pb = c->pb();
+    if (n_params != c->n_par()) return fail(c, MIPWA_ERR_ARG, "n_params must be " + std::to_string(c->n_par()));
     for (int64_t i = 0; i < n_params; ++i)
         if (!std::isfinite(p[i])) return fail(c, MIPWA_ERR_ARG, "non-finite parameter " + std::to_string(i));
     DevModel& m = c->model;
-    for (int i = 0; i < N; ++i) {
-        c->y_re[i] = p[i] * std::cos(p[N + i]);            // y_k = a_k e^{i phi_k}
-        c->y_im[i] = p[i] * std::sin(p[N + i]);
+    for (int i = 0; i < Np; ++i) {
+        c->y_re[i] = p[i] * std::cos(p[Np + i]);           // y_k = a_k e^{i phi_k}
+        c->y_im[i] = p[i] * std::sin(p[Np + i]);
     }
-    spline_solve(c, c->y_re.data(), c->ypp_re.data());
-    spline_solve(c, c->y_im.data(), c->ypp_im.data());
+    // The constant non-resonant term c_nr rides on the spline tables: the natural spline through
+    // y_k + c_nr / 2 is S + c_nr / 2 (constant data have no curvature), and the two channels add up to S(s12) + S(s13)
+    // + c_nr.  No kernel knows about it; the gradient of c_nr is half the sum of the knot gradients (polar_chain).
+    double off_re = 0.0, off_im = 0.0;
+    if (c->nr_idx >= 0) {
+        off_re = 0.5 * p[pb + 2 * c->nr_idx] * std::cos(p[pb + 2 * c->nr_idx + 1]);
+        off_im = 0.5 * p[pb + 2 * c->nr_idx] * std::sin(p[pb + 2 * c->nr_idx + 1]);
+    }
+    for (int i = 0; i < N; ++i) { c->ys_re[i] = c->y_re[i] + off_re; c->ys_im[i] = c->y_im[i] + off_im; }
+    spline_solve(c, c->ys_re.data(), c->ypp_re.data());
+    spline_solve(c, c->ys_im.data(), c->ypp_im.data());
     for (int j = 0; j < N - 1; ++j) {                       // cubic in t = s - x_j on segment j
         const double h = c->knots[j + 1] - c->knots[j];
-        const double* Y[2] = { c->y_re.data(), c->y_im.data() };
+        const double* Y[2] = { c->ys_re.data(), c->ys_im.data() };
         const double* P[2] = { c->ypp_re.data(), c->ypp_im.data() };
         double co[4][2];
         for (int q = 0; q < 2; ++q) {
@@ -293,8 +308,8 @@ int build_model(mipwa_ctx* c, const double* p, int64_t n_params)
     for (int d = 0; d < (int)slots.size(); ++d) {
         const int r = slots[d];
         double m0 = c->res[r].mass, g0 = c->res[r].width;
-        if (fidx[r] >= 0) { m0 = p[2 * N + 2 * R + 2 * fidx[r]]; g0 = p[2 * N + 2 * R + 2 * fidx[r] + 1]; }
-        const int rc = resonance_constants(c, r, m0, g0, p[2 * N + 2 * r], p[2 * N + 2 * r + 1], &m.res[d], &c->res_fold[d]);
+        if (fidx[r] >= 0) { m0 = p[pb + 2 * R + 2 * fidx[r]]; g0 = p[pb + 2 * R + 2 * fidx[r] + 1]; }
+        const int rc = resonance_constants(c, r, m0, g0, p[pb + 2 * r], p[pb + 2 * r + 1], &m.res[d], &c->res_fold[d]);
         if (rc) return rc;
         m.res[d].fl = fidx[r];
     }
@@ -441,17 +456,24 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
 {
     if (!out) return MIPWA_ERR_ARG;
     *out = nullptr;
-    if (!kin || !knots || n_knots < 2 || n_knots > MIPWA_MAX_KNOTS || n_res < 0 || n_res > MIPWA_MAX_RESONANCES ||
-        (n_res > 0 && !res))
+    if (!kin || (n_knots > 0 && !knots) || n_knots < 0 || n_knots == 1 || n_knots > MIPWA_MAX_KNOTS || n_res < 0 ||
+        n_res > MIPWA_MAX_RESONANCES || (n_res > 0 && !res) || n_knots + n_res == 0)
         return MIPWA_ERR_ARG;
     if (!(kin->m1 > 0 && kin->m2 > 0 && kin->m3 > 0) || kin->m2 != kin->m3 || !(kin->m_parent > kin->m1 + kin->m2 + kin->m3))
         return MIPWA_ERR_ARG;
     for (int i = 0; i < n_knots; ++i)
         if (!std::isfinite(knots[i]) || (i > 0 && !(knots[i] > knots[i - 1]))) return MIPWA_ERR_ARG;
-    for (int r = 0; r < n_res; ++r)
+    int nr_idx = -1;
+    for (int r = 0; r < n_res; ++r) {
+        if (res[r].spin == MIPWA_SPIN_NONRES) {            // the constant term: one at most, nothing to float
+            if (nr_idx >= 0 || res[r].shape_floats) return MIPWA_ERR_ARG;
+            nr_idx = r;
+            continue;
+        }
         if (res[r].spin < 0 || res[r].spin > 2 || !(res[r].r_res >= 0) || !(res[r].r_parent >= 0) ||
             !(res[r].mass > kin->m1 + kin->m2) || !(res[r].mass < kin->m_parent - kin->m3) || !(res[r].width > 0))
             return MIPWA_ERR_ARG;
+    }
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return MIPWA_ERR_CUDA;
@@ -463,8 +485,15 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     mipwa_ctx* c = new (std::nothrow) mipwa_ctx();
     if (!c) return MIPWA_ERR_NOMEM;
     c->kin = *kin;
-    c->N = n_knots; c->R = n_res;
-    c->knots.assign(knots, knots + n_knots);
+    c->Np = n_knots; c->R = n_res; c->nr_idx = nr_idx;
+    if (n_knots >= 2) {
+        c->N = n_knots;
+        c->knots.assign(knots, knots + n_knots);
+    } else {                                               // no spline S-wave: a two-knot table carries the constant term
+        c->N = 2;
+        c->knots = { (kin->m1 + kin->m2) * (kin->m1 + kin->m2), (kin->m_parent - kin->m3) * (kin->m_parent - kin->m3) };
+    }
+    n_knots = c->N;
     if (n_res) c->res.assign(res, res + n_res);
     for (int r = 0; r < n_res; ++r) c->F += res[r].shape_floats ? 1 : 0;
     // device slots: spin 1, then spin 2, then spin 0; within a spin the floating resonances first (k_grad_recompute
@@ -476,7 +505,7 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     for (int L : { 1, 2 })
         for (int r = 0; r < n_res; ++r)
             if (res[r].shape_floats && res[r].spin == L) { c->hyb_float.push_back(r); (L == 1 ? c->hyb_f1 : c->hyb_f2)++; }
-    for (int r = 0; r < n_res; ++r) if (!res[r].shape_floats) c->hyb_fixed.push_back(r);
+    for (int r = 0; r < n_res; ++r) if (!res[r].shape_floats && res[r].spin >= 0) c->hyb_fixed.push_back(r);
     {
         bool supported = (int)c->hyb_float.size() == c->F && c->F > 0 && !c->hyb_fixed.empty();   // no floating spin 0
         if (supported) supported = mipwa_hybrid_supported(c->hyb_f1, c->hyb_f2, (int)c->hyb_fixed.size());
@@ -487,13 +516,15 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
         bool shared = true;
         for (int a = 0; a < n_res; ++a)
             for (int b = a + 1; b < n_res; ++b)
-                if (res[a].spin == res[b].spin && (res[a].r_res != res[b].r_res || res[a].r_parent != res[b].r_parent))
+                if (res[a].spin >= 0 && res[a].spin == res[b].spin &&
+                    (res[a].r_res != res[b].r_res || res[a].r_parent != res[b].r_parent))
                     shared = false;
         if (shared) c->model_flags |= MIPWA_FL_SHR;
     }
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
-    c->y_re.resize(n_knots); c->y_im.resize(n_knots); c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
+    c->y_re.assign(n_knots, 0.0); c->y_im.assign(n_knots, 0.0); c->ys_re.resize(n_knots); c->ys_im.resize(n_knots);
+    c->ypp_re.resize(n_knots); c->ypp_im.resize(n_knots);
     spline_factor(c);
     std::memset(&c->model, 0, sizeof(DevModel));
     fill_static_model(c);
@@ -651,7 +682,7 @@ int mipwa_set_norm_points(mipwa_ctx* c, const double* s12, const double* s13, co
 int mipwa_n_params(const mipwa_ctx* c, int64_t* n)
 {
     if (!c || !n) return MIPWA_ERR_ARG;
-    *n = 2 * c->N + 2 * c->R + 2 * c->F;
+    *n = c->n_par();
     return MIPWA_OK;
 }
 
@@ -714,14 +745,14 @@ static int64_t cache_bytes_for(const mipwa_ctx* c, int kind, int64_t n)
 // unit-coefficient model (a_k = 1, phi_k = 0, c_r = 1) with the shapes of `params` (or the listed ones) -> c->model
 static int build_unit_model(mipwa_ctx* c, const double* params)
 {
-    const int N = c->N, R = c->R;
-    std::vector<double> p(2 * N + 2 * R + 2 * c->F, 0.0);
-    for (int i = 0; i < N; ++i) p[i] = 1.0;
-    for (int r = 0; r < R; ++r) p[2 * N + 2 * r] = 1.0;
+    const int Np = c->Np, R = c->R, pb = c->pb();
+    std::vector<double> p(c->n_par(), 0.0);
+    for (int i = 0; i < Np; ++i) p[i] = 1.0;
+    for (int r = 0; r < R; ++r) p[pb + 2 * r] = r == c->nr_idx ? 0.0 : 1.0;   // the basis kernels emit the constant column themselves
     for (int r = 0, f = 0; r < R; ++r)
         if (c->res[r].shape_floats) {
-            p[2 * N + 2 * R + 2 * f] = params ? params[2 * N + 2 * R + 2 * f] : c->res[r].mass;
-            p[2 * N + 2 * R + 2 * f + 1] = params ? params[2 * N + 2 * R + 2 * f + 1] : c->res[r].width;
+            p[pb + 2 * R + 2 * f] = params ? params[pb + 2 * R + 2 * f] : c->res[r].mass;
+            p[pb + 2 * R + 2 * f + 1] = params ? params[pb + 2 * R + 2 * f + 1] : c->res[r].width;
             ++f;
         }
     return build_model(c, p.data(), (int64_t)p.size());
@@ -733,7 +764,9 @@ static BasisAux basis_aux(const mipwa_ctx* c)
     a.Mx = c->d_Mx;
     std::memset(a.col_of_slot, 0, sizeof(a.col_of_slot));
     if (c->active) for (int d = 0; d < (int)c->active->size(); ++d) a.col_of_slot[d] = (uint8_t)d;   // subset: own order
-    else for (int d = 0; d < c->R; ++d) a.col_of_slot[d] = (uint8_t)c->perm[d];
+    else for (int d = 0; d < (int)c->perm.size(); ++d) a.col_of_slot[d] = (uint8_t)c->perm[d];
+    a.nonres_col = c->active ? -1 : c->nr_idx;             // the hybrid caches hold fixed-shape resonances only
+    a.n_res_cols = c->active ? (int)c->active->size() : c->R;
     return a;
 }
 
@@ -818,12 +851,11 @@ static int ensure_gram(mipwa_ctx* c)
 // A1 for the cached kernels: c = [y_0 .. y_{N-1}, c_0 .. c_{R-1}] (caller's resonance order); needs build_model first
 static void fill_coef(const mipwa_ctx* c, const double* p, CoefDev* cc)
 {
-    const int N = c->N, R = c->R;
+    const int N = c->N, R = c->R, pb = c->pb();
     cc->K = N + R; cc->N = N;
     for (int k = 0; k < N; ++k) cc->c[k] = make_double2(c->y_re[k], c->y_im[k]);
-    for (int r = 0; r < R; ++r)
-        cc->c[N + r] = make_double2(p[2 * N + 2 * r] * std::cos(p[2 * N + 2 * r + 1]),
-                                    p[2 * N + 2 * r] * std::sin(p[2 * N + 2 * r + 1]));
+    for (int r = 0; r < R; ++r)                             // the constant term included: its dense column is 1
+        cc->c[N + r] = make_double2(p[pb + 2 * r] * std::cos(p[pb + 2 * r + 1]), p[pb + 2 * r] * std::sin(p[pb + 2 * r + 1]));
 }
 
 static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_log, double* integral)
@@ -832,7 +864,7 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
     if (rc) return rc;
     rc = ensure_gram(c);
     if (rc) return rc;
-    rc = build_model(c, params, 2 * c->N + 2 * c->R);      // after the ensure_* calls: they overwrite c->model
+    rc = build_model(c, params, c->n_par());               // after the ensure_* calls: they overwrite c->model
     if (rc) return rc;
     CoefDev cc;
     fill_coef(c, params, &cc);
@@ -922,13 +954,13 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     rc = build_model(c, params, n_params);
     c->active = nullptr;
     if (rc) return rc;
-    const int N = c->N, RC = (int)c->hyb_fixed.size();
+    const int pb = c->pb(), RC = (int)c->hyb_fixed.size();
     HybCoef cc;
     cc.RC = RC; cc.pad = 0;
     for (int k = 0; k < RC; ++k) {
         const int r = c->hyb_fixed[k];
-        cc.c[k] = make_double2(params[2 * N + 2 * r] * std::cos(params[2 * N + 2 * r + 1]),
-                               params[2 * N + 2 * r] * std::sin(params[2 * N + 2 * r + 1]));
+        cc.c[k] = make_double2(params[pb + 2 * r] * std::cos(params[pb + 2 * r + 1]),
+                               params[pb + 2 * r] * std::sin(params[pb + 2 * r + 1]));
     }
     bool supported = true;
     if (!c->hyb_blocks_per_sm) {
@@ -1057,7 +1089,7 @@ int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32
     const Slot& s = which == 0 ? c->ev : c->nm;
     if (s.n < 0) return fail(c, MIPWA_ERR_STATE, "slot not set");
     if (first < 0 || n < 0 || first + n > s.n || (n > 0 && !out)) return fail(c, MIPWA_ERR_ARG, "bad range");
-    if (n_params != 2 * c->N + 2 * c->R + 2 * c->F) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
+    if (n_params != c->n_par()) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
     int rc = use_device(c);
     if (rc) return rc;
     rc = build_unit_model(c, params);
@@ -1070,10 +1102,17 @@ int mipwa_eval_basis(mipwa_ctx* c, const double* params, int64_t n_params, int32
                                                                   d_out);
     ++c->launches;
     cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
+    const int skip = c->N - c->Np;                         // stand-in knots of a model without spline: not the caller's columns
+    std::vector<double> tmp;
+    double* dst = out;
+    if (skip) { tmp.resize((size_t)n * K * 2); dst = tmp.data(); }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dst, d_out, (size_t)n * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     cudaFree(d_out);
     if (e != cudaSuccess) return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e));
+    if (skip)
+        for (int64_t i = 0; i < n; ++i)
+            std::memcpy(out + (size_t)i * (K - skip) * 2, tmp.data() + ((size_t)i * K + skip) * 2, (size_t)(K - skip) * 2 * sizeof(double));
     return MIPWA_OK;
 }
 
@@ -1109,17 +1148,29 @@ static void spline_adjoint(const mipwa_ctx* c, const double* Gsc, double* Gy)
 // Gy: calG of the knot values (2N), Gr: calG of the resonance coefficients in the caller's order (2R).
 static void polar_chain(const mipwa_ctx* c, const double* params, const double* Gy, const double* Gr, double* grad)
 {
-    const int N = c->N, R = c->R;
-    for (int k = 0; k < N; ++k) {
-        const double ph = params[N + k];
+    const int Np = c->Np, R = c->R, pb = c->pb();
+    for (int k = 0; k < Np; ++k) {
+        const double ph = params[Np + k];
         grad[k] = Gy[2 * k] * std::cos(ph) + Gy[2 * k + 1] * std::sin(ph);
-        grad[N + k] = -Gy[2 * k] * c->y_im[k] + Gy[2 * k + 1] * c->y_re[k];
+        grad[Np + k] = -Gy[2 * k] * c->y_im[k] + Gy[2 * k + 1] * c->y_re[k];
     }
     for (int r = 0; r < R; ++r) {
-        const double mag = params[2 * N + 2 * r], th = params[2 * N + 2 * r + 1];
-        grad[2 * N + 2 * r] = Gr[2 * r] * std::cos(th) + Gr[2 * r + 1] * std::sin(th);
-        grad[2 * N + 2 * r + 1] = mag * (-Gr[2 * r] * std::sin(th) + Gr[2 * r + 1] * std::cos(th));
+        const double mag = params[pb + 2 * r], th = params[pb + 2 * r + 1];
+        grad[pb + 2 * r] = Gr[2 * r] * std::cos(th) + Gr[2 * r + 1] * std::sin(th);
+        grad[pb + 2 * r + 1] = mag * (-Gr[2 * r] * std::sin(th) + Gr[2 * r + 1] * std::cos(th));
     }
+}
+
+// The constant non-resonant term enters the kernels as an offset c_nr / 2 of every knot value (build_model), so its calG
+// is half the sum of the knot calGs of the SPLINE-TABLE parametrisation (Gy: what spline_adjoint returns).  Sets Gr of
+// the constant's slot; nothing to do for a model without one.
+static void offset_rule(const mipwa_ctx* c, const double* Gy, double* Gr)
+{
+    if (c->nr_idx < 0) return;
+    double sr = 0.0, si = 0.0;
+    for (int k = 0; k < c->N; ++k) { sr += Gy[2 * k]; si += Gy[2 * k + 1]; }
+    Gr[2 * c->nr_idx] = 0.5 * sr;
+    Gr[2 * c->nr_idx + 1] = 0.5 * si;
 }
 
 // ---- A8: gradient on the recompute path ---------------------------------------------------------------------------
@@ -1263,16 +1314,18 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
     *nll = -S + n_ev * std::log(I);
     const double scale = c->ev.n > 0 ? 2.0 * n_ev / I : 0.0;
     std::vector<double> Gy(2 * N), Gr(2 * std::max(R, 1));
+    // event part: the spline tables carry the constant term (offset rule); normalisation part: I = c^H G c in the dense
+    // parametrisation, where the constant has a column (and a coefficient) of its own
     spline_adjoint(c, h + 1 + 2 * R, Gy.data());
+    for (int r = 0; r < R; ++r) { Gr[2 * r] = h[1 + 2 * r]; Gr[2 * r + 1] = h[1 + 2 * r + 1]; }   // caller's order, fold included
+    offset_rule(c, Gy.data(), Gr.data());
     for (int k = 0; k < 2 * N; ++k) Gy[k] += scale * gc[k];
-    for (int r = 0; r < R; ++r) {                           // cache columns are in the caller's order, fold included
-        Gr[2 * r] = h[1 + 2 * r] + scale * gc[2 * (N + r)];
-        Gr[2 * r + 1] = h[1 + 2 * r + 1] + scale * gc[2 * (N + r) + 1];
-    }
+    for (int r = 0; r < 2 * R; ++r) Gr[r] += scale * gc[2 * N + r];
     polar_chain(c, params, Gy.data(), Gr.data(), grad);
     if (c->parts_ev) {                                     // mipwa_nll_grad_parts: d(-S)/dtheta and dI/dtheta = 2 G c apart
         spline_adjoint(c, h + 1 + 2 * R, Gy.data());
         for (int r = 0; r < R; ++r) { Gr[2 * r] = h[1 + 2 * r]; Gr[2 * r + 1] = h[1 + 2 * r + 1]; }
+        offset_rule(c, Gy.data(), Gr.data());
         polar_chain(c, params, Gy.data(), Gr.data(), c->parts_ev);
         for (int k = 0; k < 2 * N; ++k) Gy[k] = 2.0 * gc[k];
         for (int r = 0; r < 2 * R; ++r) Gr[r] = 2.0 * gc[2 * N + r];
@@ -1303,7 +1356,7 @@ static int launch_grad_recompute(mipwa_ctx* c, bool mix, int shp, double kappa, 
     if (rc) return rc;
     rc = ensure_records(c, G, 1.0);
     if (rc) return rc;
-    const int N = c->N, R = c->R, NS = N - 1, nb = 8 * NS, NVB = 2 + 2 * R + nb + 4;
+    const int N = c->N, R = (int)c->perm.size(), NS = N - 1, nb = 8 * NS, NVB = 2 + 2 * R + nb + 4;   // R: device slots
     const int64_t n_ev = with_ev ? E.n : 0, n_nm = with_nm ? G.n : 0;
     const int ev_blocks = n_ev > 0 ? recompute_grid(c, n_ev) : 0, nm_blocks = n_nm > 0 ? recompute_grid(c, n_nm) : 0;
     const int grid = std::max(1, ev_blocks + nm_blocks);
@@ -1350,7 +1403,7 @@ static int nll_grad_recompute(mipwa_ctx* c, const double* params, int64_t n_para
 {
     int rc = build_model(c, params, n_params);
     if (rc) return rc;
-    const int N = c->N, R = c->R, F = c->F;
+    const int N = c->N, R = c->R, Rd = (int)c->perm.size(), F = c->F, pb = c->pb();
     const int shp = full ? foldable_shape(c) : 0;
     const bool want_f = full && F > 0 && !shp;
     if (want_f) {                                          // room for the per-point factors k_grad_shape reads
@@ -1381,16 +1434,17 @@ static int nll_grad_recompute(mipwa_ctx* c, const double* params, int64_t n_para
     const double n_ev = (double)c->ev.n;
     *nll = -S + n_ev * std::log(I);
     const double scale = c->ev.n > 0 ? 2.0 * n_ev / I * wn : 0.0;
-    const double *Fe = t.F(t.ev), *Fn = t.F(t.nm), *Be = t.bins(t.ev, R), *Bn = t.bins(t.nm, R);
-    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1));
+    const double *Fe = t.F(t.ev), *Fn = t.F(t.nm), *Be = t.bins(t.ev, Rd), *Bn = t.bins(t.nm, Rd);
+    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1), 0.0);
     auto emit = [&](double se, double sn, double* out) {   // out = se * (event part) + sn * (normalisation part)
         for (int k = 0; k < t.nb; ++k) Gsc[k] = se * Be[k] + sn * Bn[k];
         spline_adjoint(c, Gsc.data(), Gy.data());
-        for (int d = 0; d < R; ++d) {
+        for (int d = 0; d < Rd; ++d) {
             const int r = c->perm[d];
             Gr[2 * r] = c->res_fold[d] * (se * Fe[2 * d] + sn * Fn[2 * d]);
             Gr[2 * r + 1] = c->res_fold[d] * (se * Fe[2 * d + 1] + sn * Fn[2 * d + 1]);
         }
+        offset_rule(c, Gy.data(), Gr.data());
         polar_chain(c, params, Gy.data(), Gr.data(), out);
     };
     emit(1.0, scale, grad);
@@ -1405,15 +1459,15 @@ static int nll_grad_recompute(mipwa_ctx* c, const double* params, int64_t n_para
     auto put = [&](int f, const ResDev& rd, const double* e, const double* g) {   // e, g: [dm_re, dm_im, dG_re, dG_im]
         for (int q = 0; q < 2; ++q) {                      // q = 0: mass, 1: width
             const double dr = e[2 * q] + scale * g[2 * q], di = e[2 * q + 1] + scale * g[2 * q + 1];
-            grad[2 * N + 2 * R + 2 * f + q] = rd.cre * dr + rd.cim * di;          // Re(conj(c sqrt(n_R n_D)) D)
+            grad[pb + 2 * R + 2 * f + q] = rd.cre * dr + rd.cim * di;             // Re(conj(c sqrt(n_R n_D)) D)
             if (c->parts_ev) {
-                c->parts_ev[2 * N + 2 * R + 2 * f + q] = rd.cre * e[2 * q] + rd.cim * e[2 * q + 1];
-                c->parts_nm[2 * N + 2 * R + 2 * f + q] = 2.0 * wn * (rd.cre * g[2 * q] + rd.cim * g[2 * q + 1]);
+                c->parts_ev[pb + 2 * R + 2 * f + q] = rd.cre * e[2 * q] + rd.cim * e[2 * q + 1];
+                c->parts_nm[pb + 2 * R + 2 * f + q] = 2.0 * wn * (rd.cre * g[2 * q] + rd.cim * g[2 * q + 1]);
             }
         }
     };
     if (shp) {                                             // folded into the pass: first device slot of that spin
-        put(0, c->model.res[shp == 1 ? 0 : c->n_spin[1]], t.shape(t.ev, R), t.shape(t.nm, R));
+        put(0, c->model.res[shp == 1 ? 0 : c->n_spin[1]], t.shape(t.ev, Rd), t.shape(t.nm, Rd));
         return MIPWA_OK;
     }
     constexpr int SHAPE_OFF = 3900;                        // in h_result, clear of the main gradient's 2 NVB <= 2144 values
@@ -1509,7 +1563,7 @@ int mipwa_nll_grad_parts(mipwa_ctx* c, const double* params, int64_t n_params, d
 {
     if (!c) return MIPWA_ERR_ARG;
     if (!params || !sum_log || !integral || !grad_ev || !grad_nm) return fail(c, MIPWA_ERR_ARG, "null argument");
-    if (n_params != 2 * c->N + 2 * c->R + 2 * c->F) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
+    if (n_params != c->n_par()) return fail(c, MIPWA_ERR_ARG, "wrong n_params");
     NvtxRange range("mipwa_nll_grad_parts");
     std::vector<double> total((size_t)std::max<int64_t>(n_params, 1));
     double nll = 0.0;
@@ -1617,7 +1671,7 @@ int mipwa_nll_mix_grad(mipwa_ctx* c, const double* params, int64_t n_params, dou
     if (rc) return rc;
     rc = build_model(c, params, n_params);
     if (rc) return rc;
-    const int N = c->N, R = c->R;
+    const int N = c->N, R = c->R, Rd = (int)c->perm.size();
     const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
     { const int trc = timing_begin(c); if (trc) return trc; }
     GradTotals t;
@@ -1639,15 +1693,16 @@ int mipwa_nll_mix_grad(mipwa_ctx* c, const double* params, int64_t n_params, dou
     *nll = -S - n_ev * std::log(f_sig / I);
     if (dnll_dfsig) *dnll_dfsig = -(n_ev - I * Q / f_sig) / f_sig;
     const double scale = 2.0 * (n_ev - kappa * Q) / I * wn;
-    const double *Fe = t.F(he.data()), *Fn = t.F(hn.data()), *Be = t.bins(he.data(), R), *Bn = t.bins(hn.data(), R);
-    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1));
+    const double *Fe = t.F(he.data()), *Fn = t.F(hn.data()), *Be = t.bins(he.data(), Rd), *Bn = t.bins(hn.data(), Rd);
+    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1), 0.0);
     for (int k = 0; k < t.nb; ++k) Gsc[k] = Be[k] + scale * Bn[k];
     spline_adjoint(c, Gsc.data(), Gy.data());
-    for (int d = 0; d < R; ++d) {
+    for (int d = 0; d < Rd; ++d) {
         const int r = c->perm[d];
         Gr[2 * r] = c->res_fold[d] * (Fe[2 * d] + scale * Fn[2 * d]);
         Gr[2 * r + 1] = c->res_fold[d] * (Fe[2 * d + 1] + scale * Fn[2 * d + 1]);
     }
+    offset_rule(c, Gy.data(), Gr.data());
     polar_chain(c, params, Gy.data(), Gr.data(), grad);
     return MIPWA_OK;
 }
@@ -1657,7 +1712,9 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
 {
     if (!c || !params || !nll || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
     if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "mipwa_nll_hessian needs fixed resonance shapes");
-    const int N = c->N, R = c->R, K = N + R, P = 2 * N + 2 * R;
+    // dense parametrisation: c = [y_k (knot values), c_r (list order, the constant term with its column of ones)];
+    // a model without spline has two stand-in knots in its tables (k < k0) that are no parameters
+    const int N = c->N, Np = c->Np, R = c->R, K = N + R, P = c->n_par(), pb = c->pb(), k0 = N - Np;
     std::vector<double> gpol(P);
     int rc = mipwa_nll_grad(c, params, n_params, nll, gpol.data());
     if (rc) return rc;
@@ -1710,11 +1767,11 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
     auto Gm = [&](int k, int l) { return cx(c->h_gram[2 * ((size_t)k * K + l)], c->h_gram[2 * ((size_t)k * K + l) + 1]); };
     auto Mm = [&](int k, int l) { return cx(hM[2 * ((size_t)k * K + l)], hM[2 * ((size_t)k * K + l) + 1]); };
     std::vector<cx> cv(K), cG(K), Gc(K), e1(K), g(K);
-    std::vector<int> ir(K), ip(K);
-    for (int k = 0; k < K; ++k) {
-        cv[k] = cx(cc.c[k].x, cc.c[k].y);
-        ir[k] = k < N ? k : 2 * N + 2 * (k - N);
-        ip[k] = k < N ? N + k : 2 * N + 2 * (k - N) + 1;
+    std::vector<int> ir(K, 0), ip(K, 0);
+    for (int k = 0; k < K; ++k) cv[k] = cx(cc.c[k].x, cc.c[k].y);
+    for (int k = k0; k < K; ++k) {
+        ir[k] = k < N ? k : pb + 2 * (k - N);
+        ip[k] = k < N ? Np + k : pb + 2 * (k - N) + 1;
         e1[k] = cx(std::cos(params[ip[k]]), std::sin(params[ip[k]]));
         if (!(std::fabs(params[ir[k]]) > 0.0))
             return fail(c, MIPWA_ERR_ARG, "mipwa_nll_hessian: a zero magnitude makes the polar Hessian singular");
@@ -1728,13 +1785,13 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
     for (int k = 0; k < K; ++k) Iq += std::conj(cv[k]) * Gc[k];
     const double I = Iq.real(), nev = (double)c->ev.n;
     // dNLL/dc_k from the polar gradient: dNLL/drho = 2 Re(g e^{i phi}), dNLL/dphi = 2 Re(g i c) = -2 rho Im(g e^{i phi})
-    for (int k = 0; k < K; ++k) {
+    for (int k = k0; k < K; ++k) {
         const double rho = params[ir[k]];
         g[k] = 0.5 * cx(gpol[ir[k]], -gpol[ip[k]] / rho) * std::conj(e1[k]);
     }
     for (int t = 0; t < P * P; ++t) hess[t] = 0.0;
-    for (int k = 0; k < K; ++k)
-        for (int l = 0; l < K; ++l) {
+    for (int k = k0; k < K; ++k)
+        for (int l = k0; l < K; ++l) {
             const cx hcc = Mm(k, l) - nev * cG[k] * cG[l] / (I * I);
             const cx hcb = nev * Gm(l, k) / I - nev * cG[k] * Gc[l] / (I * I);
             const cx dk[2] = { e1[k], cx(0.0, 1.0) * cv[k] }, dl[2] = { e1[l], cx(0.0, 1.0) * cv[l] };
@@ -1743,7 +1800,7 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
                 for (int b = 0; b < 2; ++b)
                     hess[(size_t)ik[a] * P + il[b]] += 2.0 * (hcc * dk[a] * dl[b] + hcb * dk[a] * std::conj(dl[b])).real();
         }
-    for (int k = 0; k < K; ++k) {
+    for (int k = k0; k < K; ++k) {
         const double rp = 2.0 * (g[k] * cx(0.0, 1.0) * e1[k]).real(), pp = 2.0 * (g[k] * (-cv[k])).real();
         hess[(size_t)ir[k] * P + ip[k]] += rp;
         hess[(size_t)ip[k] * P + ir[k]] += rp;
