@@ -67,8 +67,12 @@ enum { MIPWA_PATH_AUTO = 0,            /* no shape floats: cached-compact; some 
        MIPWA_PATH_RECOMPUTE = 1,       /* every call re-evaluates every amplitude term (FP64-ALU bound) */
        MIPWA_PATH_CACHED = 2,          /* fixed shapes: dense n_ev x K complex basis + K x K Gram (HBM bound) */
        MIPWA_PATH_CACHED_COMPACT = 3,  /* fixed shapes: R complex resonance values per event; spline re-evaluated */
-       MIPWA_PATH_HYBRID = 4 };        /* some shapes float: their terms and the spline are recomputed, the fixed-shape
+       MIPWA_PATH_HYBRID = 4,          /* some shapes float: their terms and the spline are recomputed, the fixed-shape
                                           resonance terms are cached per event AND per normalisation point */
+       MIPWA_PATH_CACHED_REAL = 5,     /* fixed shapes: dense basis with the N spline columns stored as REAL numbers (they
+                                          are): 8 N + 16 R bytes per event instead of 16 (N + R); exact like CACHED */
+       MIPWA_PATH_CACHED_F32 = 6 };    /* OPT-IN, outside the 1e-12 contract: the columns of CACHED_REAL stored as fp32
+                                          (4 N + 8 R bytes per event), every sum still in fp64; |A|^2 good to ~1e-7 */
 
 #define MIPWA_MAX_KNOTS      128
 #define MIPWA_MAX_RESONANCES 16
@@ -114,13 +118,13 @@ int mipwa_prepare(mipwa_ctx* ctx);
 /* Length of the parameter vector: 2N + 2R + 2F (F = resonances with shape_floats). */
 int mipwa_n_params(const mipwa_ctx* ctx, int64_t* n);
 
-/* Select the evaluation path.  CACHED / CACHED_COMPACT with F > 0 -> MIPWA_ERR_STATE; HYBRID needs 1-2 floating
+/* Select the evaluation path.  CACHED* with F > 0 -> MIPWA_ERR_STATE; HYBRID needs 1-2 floating
  * resonances of spin 1 or 2 and 1-5 fixed-shape ones (else MIPWA_ERR_STATE; AUTO then recomputes). */
 int mipwa_set_path(mipwa_ctx* ctx, int32_t path);
 
 /* Bytes of device memory the current path needs for its per-event cache with the current events, n_ev rounded up
- * to a multiple of 256 (dense: n_ev * K * 16; compact: n_ev * (R * 16 + 16); hybrid: (n_ev + n_norm) * (16 +
- * 16 x fixed resonances), library-owned; recompute: 0), or a negative error
+ * to a multiple of 256 (dense: n_ev * K * 16; real: n_ev * (8 N + 16 R); f32: n_ev * (4 N + 8 R); compact:
+ * n_ev * (R * 16 + 16); hybrid: (n_ev + n_norm) * (16 + 16 x fixed resonances), library-owned; recompute: 0), or a negative error
  * code (MIPWA_ERR_STATE before mipwa_set_events). */
 int64_t mipwa_basis_bytes(const mipwa_ctx* ctx);
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmipwa.so")
 
 OK, ERR_ARG, ERR_DOMAIN, ERR_STATE, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4, -5
 MEM_HOST, MEM_DEVICE = 0, 1
-PATH_AUTO, PATH_RECOMPUTE, PATH_CACHED, PATH_CACHED_COMPACT, PATH_HYBRID = 0, 1, 2, 3, 4
+PATH_AUTO, PATH_RECOMPUTE, PATH_CACHED, PATH_CACHED_COMPACT, PATH_HYBRID, PATH_CACHED_REAL, PATH_CACHED_F32 = 0, 1, 2, 3, 4, 5, 6
 _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STATE: "MIPWA_ERR_STATE",
               ERR_CUDA: "MIPWA_ERR_CUDA", ERR_NOMEM: "MIPWA_ERR_NOMEM"}
 

@@ -222,6 +222,118 @@ k_nll_dense(const __grid_constant__ CoefDev cc, const double2* __restrict__ cach
     }
 }
 
+// ---- A10 dense with REAL spline columns (SURVEY 8(d) bytes table, row "cached, real spline columns") ------------------
+// The spline columns B_k = beta_k(s12) + beta_k(s13), k < N, are real: storing them as complex (BASELINE.json's layout,
+// k_nll_dense) spends 8 of every 16 bytes on zeros.  Here a tile of 256 events holds N real columns followed by R complex
+// ones:   MIPWA_PATH_CACHED_REAL  fp64 columns, 8 N + 16 R bytes per event, exact;
+//         MIPWA_PATH_CACHED_F32   the same columns stored as fp32 (4 N + 8 R bytes per event), accumulated in fp64:
+//                                 OPT-IN, outside the 1e-12 contract (each column carries a relative 6e-8 rounding).
+// TS / TR: storage types of a spline / resonance column element (double, double2 or float, float2).
+template <class TS, class TR> struct RealTile {
+    static __host__ __device__ constexpr size_t bytes(int N, int R) { return (size_t)MIPWA_TILE * (N * sizeof(TS) + R * sizeof(TR)); }
+};
+
+template <class T> __device__ __forceinline__ T ld_stream_t(const T* p);
+template <> __device__ __forceinline__ double ld_stream_t<double>(const double* p)
+{
+    double v; asm volatile("ld.global.cs.f64 %0, [%1];" : "=d"(v) : "l"(p)); return v;
+}
+template <> __device__ __forceinline__ float ld_stream_t<float>(const float* p)
+{
+    float v; asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v;
+}
+template <> __device__ __forceinline__ double2 ld_stream_t<double2>(const double2* p)
+{
+    double2 v; asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p)); return v;
+}
+template <> __device__ __forceinline__ float2 ld_stream_t<float2>(const float2* p)
+{
+    float2 v; asm volatile("ld.global.cs.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p)); return v;
+}
+
+template <class TS, class TR>
+__global__ void __launch_bounds__(MIPWA_TILE)
+k_basis_build_real(const __grid_constant__ DevModel m, const DevSearch* __restrict__ srch, const BasisAux aux,
+                   const double* __restrict__ s12, const double* __restrict__ s13, long long n,
+                   unsigned char* __restrict__ cache)
+{
+    __shared__ SearchSmem sm;
+    load_search_smem(sm, srch);
+    const int N = m.N, R = aux.n_res_cols;
+    const size_t tile_bytes = RealTile<TS, TR>::bytes(N, R);
+    const long long n_tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const long long i = tile * MIPWA_TILE + threadIdx.x;
+        TS* sp = reinterpret_cast<TS*>(cache + (size_t)tile * tile_bytes) + threadIdx.x;
+        TR* rs = reinterpret_cast<TR*>(cache + (size_t)tile * tile_bytes + (size_t)MIPWA_TILE * N * sizeof(TS)) + threadIdx.x;
+        if (i < n) {
+            basis_point(sm, m, aux, s12[i], s13[i], 0, 1, true, [&](int k, double2 v) {
+                if (k < N) sp[(size_t)k * MIPWA_TILE] = (TS)v.x;
+                else { TR t; t.x = v.x; t.y = v.y; rs[(size_t)(k - N) * MIPWA_TILE] = t; }
+            });
+        } else {
+            for (int k = 0; k < N; ++k) sp[(size_t)k * MIPWA_TILE] = (TS)0;
+            for (int r = 0; r < R; ++r) { TR t; t.x = 0; t.y = 0; rs[(size_t)r * MIPWA_TILE] = t; }
+        }
+    }
+}
+
+// One event per thread and tile; the N spline loads are unrolled by 8 (8 independent loads in flight per thread).
+template <class TS, class TR>
+__global__ void __launch_bounds__(MIPWA_TILE, 4)
+k_nll_dense_real(const __grid_constant__ CoefDev cc, const unsigned char* __restrict__ cache, long long n_ev,
+                 const double2* __restrict__ G, double* __restrict__ partials, unsigned int* __restrict__ ticket,
+                 double* __restrict__ result, long long tag)
+{
+    __shared__ double red[2 * 32];
+    __shared__ bool is_last;
+    const int N = cc.N, R = cc.K - cc.N;
+    const size_t tile_bytes = RealTile<TS, TR>::bytes(N, R);
+    const long long n_tiles = (n_ev + MIPWA_TILE - 1) / MIPWA_TILE;
+    LogProd lp;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const TS* sp = reinterpret_cast<const TS*>(cache + (size_t)tile * tile_bytes) + threadIdx.x;
+        const TR* rs = reinterpret_cast<const TR*>(cache + (size_t)tile * tile_bytes + (size_t)MIPWA_TILE * N * sizeof(TS)) + threadIdx.x;
+        double r0 = 0.0, r1 = 0.0, i0 = 0.0, i1 = 0.0;
+        int k = 0;
+        for (; k + 8 <= N; k += 8) {
+            TS b[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) b[u] = ld_stream_t<TS>(sp + (size_t)(k + u) * MIPWA_TILE);
+#pragma unroll
+            for (int u = 0; u < 8; u += 2) {
+                const double2 c0 = cc.c[k + u], c1 = cc.c[k + u + 1];
+                r0 = fma(c0.x, (double)b[u], r0); i0 = fma(c0.y, (double)b[u], i0);
+                r1 = fma(c1.x, (double)b[u + 1], r1); i1 = fma(c1.y, (double)b[u + 1], i1);
+            }
+        }
+        for (; k < N; ++k) {
+            const double b = (double)ld_stream_t<TS>(sp + (size_t)k * MIPWA_TILE);
+            r0 = fma(cc.c[k].x, b, r0); i0 = fma(cc.c[k].y, b, i0);
+        }
+        for (int r = 0; r < R; ++r) {
+            const TR t = ld_stream_t<TR>(rs + (size_t)r * MIPWA_TILE);
+            const double2 c = cc.c[N + r];
+            r1 = fma(c.x, (double)t.x, fma(-c.y, (double)t.y, r1));
+            i1 = fma(c.x, (double)t.y, fma(c.y, (double)t.x, i1));
+        }
+        const double re = r0 + r1, im = i0 + i1;
+        lp.add_counted(tile * MIPWA_TILE + threadIdx.x < n_ev ? fma(re, re, im * im) : 1.0);
+    }
+    double v[1] = { lp.value() };
+    if (grid_reduce<1>(v, partials, ticket, red, &is_last)) {
+        const double sum_log = v[0];
+        __syncthreads();
+        const double integ = quadratic_form(cc, G, red);
+        if (threadIdx.x == 0) {
+            result[0] = sum_log;
+            result[1] = integ;
+            *ticket = 0;
+            publish_result(result, tag);
+        }
+    }
+}
+
 // ---- A10 compact: A_i = S(s12_i) + S(s13_i) + sum_r c_r B_{i,N+r} ----------------------------------------------------
 // Streams 16 + 16 R bytes per event; the spline part comes from the per-call segment coefficients in shared memory
 // (same Horner evaluation as the recompute path).  cc.c[N + r] = c_r in the caller's resonance order.

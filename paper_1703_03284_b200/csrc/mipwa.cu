@@ -97,7 +97,7 @@ struct mipwa_ctx {
     int64_t owned_cache_bytes = 0;
     void* user_cache = nullptr;
     int64_t user_cache_bytes = 0;
-    int cache_kind = 0;             // MIPWA_PATH_CACHED / MIPWA_PATH_CACHED_COMPACT, valid iff cache_valid
+    int cache_kind = 0;             // MIPWA_PATH_CACHED / _COMPACT / _REAL / _F32, valid iff cache_valid
     bool cache_valid = false;
     double2* d_gram = nullptr;
     std::vector<double> h_gram;     // host copy (K x K complex, row-major) for the cached-path gradient
@@ -689,10 +689,11 @@ int mipwa_n_params(const mipwa_ctx* c, int64_t* n)
 int mipwa_set_path(mipwa_ctx* c, int32_t path)
 {
     if (!c) return MIPWA_ERR_ARG;
-    if (path < MIPWA_PATH_AUTO || path > MIPWA_PATH_HYBRID) return fail(c, MIPWA_ERR_ARG, "unknown path");
+    if (path < MIPWA_PATH_AUTO || path > MIPWA_PATH_CACHED_F32) return fail(c, MIPWA_ERR_ARG, "unknown path");
     if (path == MIPWA_PATH_HYBRID && !c->hyb_ok)
         return fail(c, MIPWA_ERR_STATE, "the hybrid path needs 1-2 floating spin-1/2 resonances and 1-5 fixed ones");
-    if ((path == MIPWA_PATH_CACHED || path == MIPWA_PATH_CACHED_COMPACT) && c->F > 0)
+    if ((path == MIPWA_PATH_CACHED || path == MIPWA_PATH_CACHED_COMPACT || path == MIPWA_PATH_CACHED_REAL ||
+         path == MIPWA_PATH_CACHED_F32) && c->F > 0)
         return fail(c, MIPWA_ERR_STATE, "cached paths need fixed resonance shapes");
     c->path = path;
     return MIPWA_OK;
@@ -737,8 +738,10 @@ static int effective_path(const mipwa_ctx* c)
 
 static int64_t cache_bytes_for(const mipwa_ctx* c, int kind, int64_t n)
 {
-    const int64_t cols = kind == MIPWA_PATH_CACHED ? c->N + c->R : 1 + c->R;
     const int64_t tiles = (n + MIPWA_TILE - 1) / MIPWA_TILE;
+    if (kind == MIPWA_PATH_CACHED_REAL) return tiles * (int64_t)RealTile<double, double2>::bytes(c->N, c->R);
+    if (kind == MIPWA_PATH_CACHED_F32) return tiles * (int64_t)RealTile<float, float2>::bytes(c->N, c->R);
+    const int64_t cols = kind == MIPWA_PATH_CACHED ? c->N + c->R : 1 + c->R;
     return tiles * MIPWA_TILE * cols * (int64_t)sizeof(double2);
 }
 
@@ -794,6 +797,12 @@ static int ensure_cache(mipwa_ctx* c, int kind)
         if (kind == MIPWA_PATH_CACHED)
             k_basis_build<false><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, c->d_search, basis_aux(c), evs(c).s12,
                                                                       evs(c).s13, c->ev.n, (double2*)c->d_cache);
+        else if (kind == MIPWA_PATH_CACHED_REAL)
+            k_basis_build_real<double, double2><<<grid, MIPWA_TILE, 0, c->stream>>>(
+                c->model, c->d_search, basis_aux(c), evs(c).s12, evs(c).s13, c->ev.n, (unsigned char*)c->d_cache);
+        else if (kind == MIPWA_PATH_CACHED_F32)
+            k_basis_build_real<float, float2><<<grid, MIPWA_TILE, 0, c->stream>>>(
+                c->model, c->d_search, basis_aux(c), evs(c).s12, evs(c).s13, c->ev.n, (unsigned char*)c->d_cache);
         else
             k_basis_build<true><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, c->d_search, basis_aux(c), evs(c).s12,
                                                                      evs(c).s13, c->ev.n, (double2*)c->d_cache);
@@ -880,6 +889,14 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->dense_blocks_per_sm));
         k_nll_dense<<<grid, MIPWA_TILE, 0, c->stream>>>(cc, cache, c->ev.n, c->d_gram, (double*)c->d_partials,
                                                          c->d_ticket, c->d_result, tag);
+    } else if (kind == MIPWA_PATH_CACHED_REAL || kind == MIPWA_PATH_CACHED_F32) {
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * 8));
+        if (kind == MIPWA_PATH_CACHED_REAL)
+            k_nll_dense_real<double, double2><<<grid, MIPWA_TILE, 0, c->stream>>>(
+                cc, (const unsigned char*)c->d_cache, c->ev.n, c->d_gram, (double*)c->d_partials, c->d_ticket, c->d_result, tag);
+        else
+            k_nll_dense_real<float, float2><<<grid, MIPWA_TILE, 0, c->stream>>>(
+                cc, (const unsigned char*)c->d_cache, c->ev.n, c->d_gram, (double*)c->d_partials, c->d_ticket, c->d_result, tag);
     } else {
         if (!c->compact_blocks_per_sm) {
             CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->compact_blocks_per_sm, k_nll_compact<-1>, MIPWA_TILE, 0));

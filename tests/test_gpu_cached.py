@@ -215,3 +215,42 @@ def test_maximum_model_size():
         B.Mipwa(c.kin, I.knots_uniform(129), res)
     with pytest.raises(B.MipwaError):
         B.Mipwa(c.kin, knots, res + [res[0]])
+
+
+def test_real_column_and_fp32_dense_layouts():
+    """MIPWA_PATH_CACHED_REAL (real spline columns, 8 N + 16 R bytes per event) is exact like the dense path;
+    MIPWA_PATH_CACHED_F32 (the same columns stored as fp32: opt-in) is outside the 1e-12 contract: every
+    column carries a relative 6e-8 rounding, so sum ln|A|^2 is held to a relative 1e-6 of n_ev here and the Gram integral,
+    which does not touch the cache, stays exact."""
+    B = _lib()
+    c, o, data = make_case(2, n_ev=30_011, n_norm=20_003)       # ragged last tile, non-uniform knots
+    n, N, R = data[0].size, c.N, c.R
+    tiles = -(-n // 256)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], data[4])
+    for t in range(2):
+        p = c.perturbed(t)
+        ref, sl, integ = o.nll(p, *data, parts=True)
+        m.set_path(B.PATH_CACHED_REAL)
+        assert m.basis_bytes() == tiles * 256 * (8 * N + 16 * R)
+        got, gsl, ginteg = m.nll_parts(p)
+        assert abs(got - ref) <= nll_tol(ref, sl, integ, n)
+        assert gsl == pytest.approx(sl, rel=1e-12) and ginteg == pytest.approx(integ, rel=1e-12)
+        assert m.nll(p) == got
+        m.set_path(B.PATH_CACHED_F32)
+        assert m.basis_bytes() == tiles * 256 * (4 * N + 8 * R)
+        got32, gsl32, ginteg32 = m.nll_parts(p)
+        assert abs(gsl32 - sl) <= 1e-6 * n
+        assert abs(gsl32 - sl) > 0.0                             # it IS a different precision: not silently the fp64 cache
+        assert ginteg32 == pytest.approx(integ, rel=1e-12)
+    m.prepare()                                                  # cell-sorted order: the caches are rebuilt
+    m.set_path(B.PATH_CACHED_REAL)
+    p = c.perturbed(0)
+    ref, sl, integ = o.nll(p, *data, parts=True)
+    assert abs(m.nll(p) - ref) <= nll_tol(ref, sl, integ, n)
+    m.close()
+    mf = B.Mipwa(c.kin, c.knots, [dict(r, shape_floats=1) if i == 0 else r for i, r in enumerate(c.resonances)])
+    for path in (B.PATH_CACHED_REAL, B.PATH_CACHED_F32):
+        with pytest.raises(B.MipwaError):
+            mf.set_path(path)                                    # a floating shape cannot be cached
+    mf.close()
