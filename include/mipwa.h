@@ -175,6 +175,23 @@ int mipwa_nll_grad_full(mipwa_ctx* ctx, const double* params, int64_t n_params, 
 int mipwa_nll_grad_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, double* sum_log, double* integral,
                          double* grad_ev, double* grad_nm);
 
+/* The sharded likelihood without a host round trip.  One call per rank and step:
+ *   mipwa_nll_parts_device   launches this rank's kernel and leaves (S_r, I_r, n_r) in DEVICE memory `dev_parts` (3
+ *                            doubles, caller-owned, e.g. a slice of a torch tensor); returns without waiting.  The
+ *                            caller all-gathers the 3 doubles on the SAME stream (NCCL over NVLink) into 3 n_ranks doubles
+ *   mipwa_combine_parts_device  one tiny kernel adds the gathered pieces IN RANK ORDER (every rank forms the same bits),
+ *                            forms NLL = -S + n ln I (A7) and delivers it through the mapped result block; returns when
+ *                            the value is on the host.  sum_log, integral, n_ev may be NULL.
+ * The normalisation weights must be those of the whole sample.  mipwa_combine_parts / mipwa_combine_grad_parts are the
+ * same rank-ordered sums on HOST data (no GPU needed): parts[r] = (S_r, I_r, n_r) resp. (S_r, I_r, n_r, grad_ev_r[n_params],
+ * grad_nm_r[n_params]) as mipwa_nll_grad_parts returns them; grad = sum grad_ev_r + (n / I) sum grad_nm_r. */
+int mipwa_nll_parts_device(mipwa_ctx* ctx, const double* params, int64_t n_params, double* dev_parts);
+int mipwa_combine_parts_device(mipwa_ctx* ctx, const double* dev_parts_all, int32_t n_ranks, double* nll, double* sum_log,
+                               double* integral, int64_t* n_ev);
+int mipwa_combine_parts(int32_t n_ranks, const double* parts, double* nll, double* sum_log, double* integral, int64_t* n_ev);
+int mipwa_combine_grad_parts(int32_t n_ranks, int64_t n_params, const double* parts, double* nll, double* grad,
+                             double* sum_log, double* integral, int64_t* n_ev);
+
 /* Signal + background mixture ("signal purity 90 %"): per event the PDF is
  *     f_s |A_i|^2 / I + (1 - f_s) b_i ,      NLL = - sum_i ln( f_s |A_i|^2 / I + (1 - f_s) b_i ),
  * with b_i the background density at event i (normalised over the Dalitz plot, supplied by the caller) and f_s the
@@ -190,6 +207,22 @@ int mipwa_nll_mix(mipwa_ctx* ctx, const double* params, int64_t n_params, double
 int mipwa_nll_mix_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, double f_sig, double* nll, double* grad,
                        double* dnll_dfsig);
 
+/* The mixture likelihood of a SHARDED sample: the event sum needs the integral I of the whole sample, so a step is two
+ * phases with one exchange of 1 + P doubles between them (P = 2N + 2R) and one of 3 + P after:
+ *   mipwa_norm_parts         this rank's I_r = sum_j w_j |A_j|^2 and dI_r/dtheta (grad_nm: HOST, P doubles, may be NULL)
+ *   mipwa_nll_mix_parts      with integral_total = sum_r I_r: S_r = sum_i ln(|A_i|^2 + kappa b_i), Q_r = sum_i b_i / D_i,
+ *                            D_i = |A_i|^2 + kappa b_i, kappa = I (1 - f_s) / f_s, and grad_ev = d(-S_r)/dtheta at fixed
+ *                            kappa (HOST, P doubles, may be NULL)
+ *   mipwa_combine_mix_parts  HOST: norm_parts[r] = (I_r, grad_nm_r[P]), ev_parts[r] = (S_r, Q_r, n_r, grad_ev_r[P]) ->
+ *                            NLL = -S - n ln(f_s / I), grad = sum grad_ev_r + ((n - kappa Q) / I) sum grad_nm_r,
+ *                            dNLL/df_s = -(n - I Q / f_s) / f_s; every sum in rank order.  grad, dnll_dfsig may be NULL.
+ * Errors as mipwa_nll_mix_grad. */
+int mipwa_norm_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, double* integral, double* grad_nm);
+int mipwa_nll_mix_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, double f_sig, double integral_total,
+                        double* sum_log, double* q, double* grad_ev);
+int mipwa_combine_mix_parts(int32_t n_ranks, int64_t n_lin, double f_sig, const double* norm_parts, const double* ev_parts,
+                            double* nll, double* grad, double* dnll_dfsig);
+
 /* NLL, gradient and HESSIAN with respect to the 2N + 2R linear-coefficient parameters, for fixed resonance shapes
  * (the parameter errors and correlations PAPER.md:29 alludes to are the inverse of this matrix at the
  * minimum).  With c = [y_k, c_r], A_i = sum_k c_k B_ik, I = c^H G c and Wirtinger derivatives:
@@ -201,6 +234,17 @@ int mipwa_nll_mix_grad(mipwa_ctx* ctx, const double* params, int64_t n_params, d
  * Errors: MIPWA_ERR_STATE if a shape floats or before both mipwa_set_*; MIPWA_ERR_ARG if a magnitude is zero (the
  * polar parametrisation is singular there). */
 int mipwa_nll_hessian(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad, double* hess);
+
+/* The same Hessian for a SHARDED sample.  Both sums of the formulas above are sums over points:
+ *   mipwa_hessian_parts      this rank's M_kl = sum_i B_ik B_il / A_i^2 (its events) and G_kl (its normalisation points,
+ *                            whole-sample weights): HOST, mipwa_hessian_parts_len() doubles each = K x K complex, row-major,
+ *                            (re, im) interleaved; K counts the columns of the dense basis
+ *   mipwa_hessian_assemble   HOST arithmetic only: from M and G added over the ranks, the whole-sample event count and the
+ *                            whole-sample polar gradient (mipwa_combine_grad_parts) to hess ((2N + 2R)^2, row-major). */
+int64_t mipwa_hessian_parts_len(const mipwa_ctx* ctx);
+int mipwa_hessian_parts(mipwa_ctx* ctx, const double* params, int64_t n_params, double* M, double* G);
+int mipwa_hessian_assemble(mipwa_ctx* ctx, const double* params, int64_t n_params, int64_t n_ev_total, const double* M,
+                           const double* G, const double* grad, double* hess);
 
 /* Toy Monte-Carlo generation on the device ("samples of 100K signal events are generated from a Dalitz
  * plot PDF"): n events with density |A(params)|^2 / integral inside the Dalitz boundary, by

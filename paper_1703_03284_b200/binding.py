@@ -26,7 +26,9 @@ SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_event
            "mipwa_nll_parts", "mipwa_nll_grad", "mipwa_nll_grad_full", "mipwa_nll_grad_parts", "mipwa_nll_hessian", "mipwa_set_event_background", "mipwa_nll_mix",
            "mipwa_nll_mix_grad", "mipwa_generate", "mipwa_eval_abs2", "mipwa_eval_basis", "mipwa_enable_timing",
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
-           "mipwa_version"]
+           "mipwa_version", "mipwa_nll_parts_device", "mipwa_combine_parts_device", "mipwa_combine_parts",
+           "mipwa_combine_grad_parts", "mipwa_norm_parts", "mipwa_nll_mix_parts", "mipwa_combine_mix_parts",
+           "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble"]
 
 
 class MipwaError(RuntimeError):
@@ -88,6 +90,17 @@ def load_library():
     L.mipwa_measure_fp64_peak.restype = i32; L.mipwa_measure_fp64_peak.argtypes = [i32, d, _dp, _dp]
     L.mipwa_last_error.restype = C.c_char_p; L.mipwa_last_error.argtypes = [vp]
     L.mipwa_version.restype = C.c_char_p; L.mipwa_version.argtypes = []
+    pi64 = C.POINTER(i64)
+    L.mipwa_nll_parts_device.restype = i32; L.mipwa_nll_parts_device.argtypes = [vp, _dp, i64, vp]
+    L.mipwa_combine_parts_device.restype = i32; L.mipwa_combine_parts_device.argtypes = [vp, vp, i32, _dp, _dp, _dp, pi64]
+    L.mipwa_combine_parts.restype = i32; L.mipwa_combine_parts.argtypes = [i32, _dp, _dp, _dp, _dp, pi64]
+    L.mipwa_combine_grad_parts.restype = i32; L.mipwa_combine_grad_parts.argtypes = [i32, i64, _dp, _dp, _dp, _dp, _dp, pi64]
+    L.mipwa_norm_parts.restype = i32; L.mipwa_norm_parts.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_nll_mix_parts.restype = i32; L.mipwa_nll_mix_parts.argtypes = [vp, _dp, i64, d, d, _dp, _dp, _dp]
+    L.mipwa_combine_mix_parts.restype = i32; L.mipwa_combine_mix_parts.argtypes = [i32, i64, d, _dp, _dp, _dp, _dp, _dp]
+    L.mipwa_hessian_parts_len.restype = i64; L.mipwa_hessian_parts_len.argtypes = [vp]
+    L.mipwa_hessian_parts.restype = i32; L.mipwa_hessian_parts.argtypes = [vp, _dp, i64, _dp, _dp]
+    L.mipwa_hessian_assemble.restype = i32; L.mipwa_hessian_assemble.argtypes = [vp, _dp, i64, i64, _dp, _dp, _dp, _dp]
     _lib = L
     return L
 
@@ -282,6 +295,52 @@ class Mipwa:
         self._check(self.L.mipwa_nll_hessian(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp), H.ctypes.data_as(_dp)))
         return out.value, grad, H
 
+    def nll_parts_device(self, params, dev_parts):
+        """launch this rank's likelihood kernel; (S, I, n_ev) stay in the CUDA tensor dev_parts (3 float64); no wait"""
+        p, pp, n = self._params(params)
+        self._check(self.L.mipwa_nll_parts_device(self._h, pp, n, _dev_ptr(dev_parts, 3)))
+
+    def combine_parts_device(self, dev_parts_all, n_ranks):
+        """(NLL, S, I, n_ev) of the whole sample from the gathered pieces (CUDA tensor, 3 n_ranks float64)"""
+        out, S, Iv, nn = C.c_double(), C.c_double(), C.c_double(), C.c_int64()
+        self._check(self.L.mipwa_combine_parts_device(self._h, _dev_ptr(dev_parts_all, 3 * n_ranks), int(n_ranks),
+                                                      C.byref(out), C.byref(S), C.byref(Iv), C.byref(nn)))
+        return out.value, S.value, Iv.value, nn.value
+
+    def norm_parts(self, params, grad=True):
+        """phase 1 of the sharded mixture likelihood: (I_r, dI_r/dtheta or None)"""
+        p, pp, n = self._params(params)
+        Iv = C.c_double()
+        g = np.empty(2 * self.N + 2 * self.R) if grad else None
+        self._check(self.L.mipwa_norm_parts(self._h, pp, n, C.byref(Iv), g.ctypes.data_as(_dp) if grad else None))
+        return Iv.value, g
+
+    def nll_mix_parts(self, params, f_sig, integral_total, grad=True):
+        """phase 2: (S_r, Q_r, d(-S_r)/dtheta or None) with the integral of the whole sample"""
+        p, pp, n = self._params(params)
+        S, Q = C.c_double(), C.c_double()
+        g = np.empty(2 * self.N + 2 * self.R) if grad else None
+        self._check(self.L.mipwa_nll_mix_parts(self._h, pp, n, float(f_sig), float(integral_total), C.byref(S), C.byref(Q),
+                                               g.ctypes.data_as(_dp) if grad else None))
+        return S.value, Q.value, g
+
+    def hessian_parts(self, params):
+        """this rank's (M, G): K x K complex arrays of the event sum and the Gram matrix (mipwa_hessian_parts)"""
+        p, pp, n = self._params(params)
+        ln = int(self.L.mipwa_hessian_parts_len(self._h))
+        M, G = np.empty(ln), np.empty(ln)
+        self._check(self.L.mipwa_hessian_parts(self._h, pp, n, M.ctypes.data_as(_dp), G.ctypes.data_as(_dp)))
+        return M, G
+
+    def hessian_assemble(self, params, n_ev_total, M, G, grad):
+        p, pp, n = self._params(params)
+        P = 2 * self.N + 2 * self.R
+        M, G, grad = _host(M), _host(G), _host(grad)
+        H = np.empty((P, P))
+        self._check(self.L.mipwa_hessian_assemble(self._h, pp, n, int(n_ev_total), M.ctypes.data_as(_dp),
+                                                  G.ctypes.data_as(_dp), grad.ctypes.data_as(_dp), H.ctypes.data_as(_dp)))
+        return H
+
     def generate(self, params, key, n, n_side=1024, n_coarse=64, device=False):
         """n toy events with density |A(params)|^2 (accept-reject on the GPU, counter-based stream `key`).
         Returns (s12, s13, candidates drawn); numpy arrays, or CUDA torch tensors if device=True."""
@@ -335,6 +394,44 @@ def measure_fp64_peak(device=0, seconds=2.0):
     if rc != OK:
         raise MipwaError(rc, "mipwa_measure_fp64_peak failed")
     return out.value, out3.value
+
+
+def combine_parts(parts):
+    """A7 over gathered (S_r, I_r, n_r) rows in rank order (C library, host only): (nll, S, I, n_ev)"""
+    L = load_library()
+    a = np.ascontiguousarray(parts, dtype=np.float64).reshape(-1, 3)
+    out, S, Iv, nn = C.c_double(), C.c_double(), C.c_double(), C.c_int64()
+    rc = L.mipwa_combine_parts(a.shape[0], a.ctypes.data_as(_dp), C.byref(out), C.byref(S), C.byref(Iv), C.byref(nn))
+    if rc != OK:
+        raise MipwaError(rc, "mipwa_combine_parts failed")
+    return out.value, S.value, Iv.value, nn.value
+
+
+def combine_grad_parts(parts, n_params):
+    """whole-sample (nll, grad, S, I, n_ev) from gathered rows (S_r, I_r, n_r, grad_ev_r, grad_nm_r), rank order"""
+    L = load_library()
+    a = np.ascontiguousarray(parts, dtype=np.float64).reshape(-1, 3 + 2 * n_params)
+    out, S, Iv, nn = C.c_double(), C.c_double(), C.c_double(), C.c_int64()
+    g = np.zeros(max(n_params, 1))
+    rc = L.mipwa_combine_grad_parts(a.shape[0], int(n_params), a.ctypes.data_as(_dp), C.byref(out), g.ctypes.data_as(_dp),
+                                    C.byref(S), C.byref(Iv), C.byref(nn))
+    if rc != OK:
+        raise MipwaError(rc, "mipwa_combine_grad_parts failed")
+    return out.value, g[:n_params], S.value, Iv.value, nn.value
+
+
+def combine_mix_parts(norm_parts, ev_parts, n_lin, f_sig):
+    """whole-sample mixture (nll, grad, dnll/df_sig) from gathered rows (I_r, grad_nm_r) and (S_r, Q_r, n_r, grad_ev_r)"""
+    L = load_library()
+    a = np.ascontiguousarray(norm_parts, dtype=np.float64).reshape(-1, 1 + n_lin)
+    b = np.ascontiguousarray(ev_parts, dtype=np.float64).reshape(-1, 3 + n_lin)
+    out, dfs = C.c_double(), C.c_double()
+    g = np.zeros(max(n_lin, 1))
+    rc = L.mipwa_combine_mix_parts(a.shape[0], int(n_lin), float(f_sig), a.ctypes.data_as(_dp), b.ctypes.data_as(_dp),
+                                   C.byref(out), g.ctypes.data_as(_dp), C.byref(dfs))
+    if rc != OK:
+        raise MipwaError(rc, "mipwa_combine_mix_parts failed")
+    return out.value, g[:n_lin], dfs.value
 
 
 def version():

@@ -237,6 +237,26 @@ k_validate(const DevKin k, const DevSearch* __restrict__ srch, const double* __r
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(bad, (unsigned long long)mine);
 }
 
+// ---- sharded likelihood on the device (mipwa_nll_parts_device / mipwa_combine_parts_device) ---------------------------
+// this rank's (S, I, n_ev) from the totals a value kernel left in device memory
+static __global__ void k_pack_parts(const double* __restrict__ totals, double i_scale, double n_ev, double* __restrict__ parts)
+{
+    parts[0] = totals[0];
+    parts[1] = totals[1] * i_scale;
+    parts[2] = n_ev;
+}
+
+// A7 over all ranks' pieces, added in rank order (every rank forms the same bits): result = (S, I, tag, NLL, n)
+static __global__ void k_combine_parts(const double* __restrict__ all, int n_ranks, double* __restrict__ result, long long tag)
+{
+    double S = 0.0, I = 0.0, n = 0.0;
+    for (int r = 0; r < n_ranks; ++r) { S += all[3 * r]; I += all[3 * r + 1]; n += all[3 * r + 2]; }
+    result[0] = S; result[1] = I;
+    result[3] = n > 0.0 ? -S + n * log(I) : 0.0;
+    result[4] = n;
+    publish_result(result, tag);
+}
+
 // ---- timing aid: keeps the GPU busy for `ns` nanoseconds ---------------------------------------------------------------
 // With kernel timing on (mipwa_enable_timing) this runs in front of the first event record, so that the host has
 // submitted [event, kernel, event] before the first event executes: the two timestamps then bracket the kernel's

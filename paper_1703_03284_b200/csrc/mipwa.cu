@@ -81,6 +81,9 @@ struct mipwa_ctx {
     double* h_result = nullptr;     // mapped pinned: [0] sum ln|A|^2, [1] sum w|A|^2, [2] tag of the call that wrote them
     double* d_result = nullptr;     // device alias of h_result
     long long tag = 0;              // number of value-kernel launches: what publish_result writes into slot 2
+    double* result_dst = nullptr;   // where the value kernels write their totals: d_result, or d_dev_result (device mode)
+    double* d_dev_result = nullptr; // device memory, 8 doubles: totals of a call that stays on the device
+    bool async_result = false;      // device mode (mipwa_nll_parts_device): do not wait, do not read h_result
     unsigned long long* h_bad = nullptr;
     unsigned long long* d_bad = nullptr;
 
@@ -398,6 +401,7 @@ static int timing_begin(mipwa_ctx* c)
 // cudaStreamSynchronize, which at the paper's sample sizes (1e4-1e5 events) is as long as the kernel itself.
 static int wait_result(mipwa_ctx* c, long long tag)
 {
+    if (c->async_result) return MIPWA_OK;                  // device mode: the totals stay on the device
     if (c->timing) {
         CU(c, cudaEventRecord(c->ev1, c->stream));
         CU(c, cudaEventSynchronize(c->ev1));
@@ -546,6 +550,8 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     ok = ok && cudaHostAlloc(&c->h_result, 4096 * sizeof(double), cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer(&c->d_result, c->h_result, 0) == cudaSuccess;
     if (ok) std::memset(c->h_result, 0, 4096 * sizeof(double));   // recycled pinned memory: no stale tag of an older context
+    c->result_dst = c->d_result;
+    ok = ok && cudaMalloc(&c->d_dev_result, 64) == cudaSuccess;
     ok = ok && cudaHostAlloc(&c->h_bad, 64, cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer(&c->d_bad, c->h_bad, 0) == cudaSuccess;
     ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
@@ -569,6 +575,7 @@ void mipwa_destroy(mipwa_ctx* c)
     if (c->d_ticket) cudaFree(c->d_ticket);
     if (c->d_Mx) cudaFree(c->d_Mx);
     if (c->d_search) cudaFree(c->d_search);
+    if (c->d_dev_result) cudaFree(c->d_dev_result);
     if (c->owned_cache) cudaFree(c->owned_cache);
     if (c->d_gram) cudaFree(c->d_gram);
     if (c->d_gpartials) cudaFree(c->d_gpartials);
@@ -718,7 +725,7 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     { const int trc = timing_begin(c); if (trc) return trc; }
     const long long tag = next_tag(c);
     const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0,
-                                                      E.n, G.rec, G.n, c->d_partials, c->d_ticket, c->d_result, tag);
+                                                      E.n, G.rec, G.n, c->d_partials, c->d_ticket, c->result_dst, tag);
     ++c->launches;
     CU(c, le);
     rc = wait_result(c, tag);
@@ -888,15 +895,15 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
         }
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->dense_blocks_per_sm));
         k_nll_dense<<<grid, MIPWA_TILE, 0, c->stream>>>(cc, cache, c->ev.n, c->d_gram, (double*)c->d_partials,
-                                                         c->d_ticket, c->d_result, tag);
+                                                         c->d_ticket, c->result_dst, tag);
     } else if (kind == MIPWA_PATH_CACHED_REAL || kind == MIPWA_PATH_CACHED_F32) {
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * 8));
         if (kind == MIPWA_PATH_CACHED_REAL)
             k_nll_dense_real<double, double2><<<grid, MIPWA_TILE, 0, c->stream>>>(
-                cc, (const unsigned char*)c->d_cache, c->ev.n, c->d_gram, (double*)c->d_partials, c->d_ticket, c->d_result, tag);
+                cc, (const unsigned char*)c->d_cache, c->ev.n, c->d_gram, (double*)c->d_partials, c->d_ticket, c->result_dst, tag);
         else
             k_nll_dense_real<float, float2><<<grid, MIPWA_TILE, 0, c->stream>>>(
-                cc, (const unsigned char*)c->d_cache, c->ev.n, c->d_gram, (double*)c->d_partials, c->d_ticket, c->d_result, tag);
+                cc, (const unsigned char*)c->d_cache, c->ev.n, c->d_gram, (double*)c->d_partials, c->d_ticket, c->result_dst, tag);
     } else {
         if (!c->compact_blocks_per_sm) {
             CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->compact_blocks_per_sm, k_nll_compact<-1>, MIPWA_TILE, 0));
@@ -905,7 +912,7 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->compact_blocks_per_sm));
 #define MIPWA_COMPACT_LAUNCH(T)                                                                                   \
     k_nll_compact<T><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, cc, cache, evs(c).seg, c->ev.n, c->d_gram,    \
-                                                          (double*)c->d_partials, c->d_ticket, c->d_result, tag)
+                                                          (double*)c->d_partials, c->d_ticket, c->result_dst, tag)
         switch (c->R) {
             case 0: MIPWA_COMPACT_LAUNCH(0); break;
             case 1: MIPWA_COMPACT_LAUNCH(1); break;
@@ -993,7 +1000,7 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     const cudaError_t le = mipwa_launch_nll_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, grid, c->stream, c->model, cc,
                                                    (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n,
                                                    (const double2*)c->d_hyb_nm, nms(c).w, nms(c).seg, c->nm.n,
-                                                   c->d_partials, c->d_ticket, c->d_result, tag);
+                                                   c->d_partials, c->d_ticket, c->result_dst, tag);
     ++c->launches;
     CU(c, le);
     rc = wait_result(c, tag);
@@ -1027,6 +1034,92 @@ int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double
 int mipwa_nll(mipwa_ctx* c, const double* params, int64_t n_params, double* nll)
 {
     return mipwa_nll_parts(c, params, n_params, nll, nullptr, nullptr);
+}
+
+// ---- sharded likelihood without a host round trip --------------------------------------------------------
+// rank-local pieces left in DEVICE memory: dev_parts[0..2] = (sum ln|A|^2, sum w|A|^2, n_ev); nothing is waited for
+int mipwa_nll_parts_device(mipwa_ctx* c, const double* params, int64_t n_params, double* dev_parts)
+{
+    if (!c || !params || !dev_parts) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    NvtxRange range("mipwa_nll_parts_device");
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    double S = 0, I = 0;
+    const int path = effective_path(c);
+    const bool timing = c->timing;
+    c->timing = false; c->async_result = true; c->result_dst = c->d_dev_result;
+    if (path == MIPWA_PATH_RECOMPUTE) rc = nll_recompute(c, &S, &I);
+    else if (path == MIPWA_PATH_HYBRID) rc = nll_hybrid(c, params, n_params, &S, &I);
+    else rc = nll_cached(c, path, params, &S, &I);
+    c->timing = timing; c->async_result = false; c->result_dst = c->d_result;
+    if (rc) return rc;
+    // the recompute and hybrid kernels leave sum |A|^2 without its 1/n when the points have no weights
+    const bool raw = path == MIPWA_PATH_RECOMPUTE || path == MIPWA_PATH_HYBRID;
+    k_pack_parts<<<1, 1, 0, c->stream>>>(c->d_dev_result, raw && !c->nm.w ? 1.0 / (double)c->nm.n : 1.0, (double)c->ev.n, dev_parts);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    return MIPWA_OK;
+}
+
+// A7 over the gathered pieces of all ranks, on the device: rank-ordered sums, NLL = -S + n ln I; the four numbers come
+// back through the mapped result block like any likelihood value
+int mipwa_combine_parts_device(mipwa_ctx* c, const double* dev_parts_all, int32_t n_ranks, double* nll, double* sum_log,
+                               double* integral, int64_t* n_ev)
+{
+    if (!c || !dev_parts_all || n_ranks < 1 || !nll) return c ? fail(c, MIPWA_ERR_ARG, "bad argument") : MIPWA_ERR_ARG;
+    int rc = use_device(c);
+    if (rc) return rc;
+    const long long tag = next_tag(c);
+    k_combine_parts<<<1, 1, 0, c->stream>>>(dev_parts_all, n_ranks, c->d_result, tag);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    const bool timing = c->timing;
+    c->timing = false;
+    rc = wait_result(c, tag);
+    c->timing = timing;
+    if (rc) return rc;
+    *nll = c->h_result[3];
+    if (sum_log) *sum_log = c->h_result[0];
+    if (integral) *integral = c->h_result[1];
+    if (n_ev) *n_ev = (int64_t)c->h_result[4];
+    return MIPWA_OK;
+}
+
+// A7 on the host over gathered pieces (parts[3 r + {0,1,2}] = S_r, I_r, n_r): the same rank-ordered sums; needs no GPU
+int mipwa_combine_parts(int32_t n_ranks, const double* parts, double* nll, double* sum_log, double* integral, int64_t* n_ev)
+{
+    if (n_ranks < 1 || !parts || !nll) return MIPWA_ERR_ARG;
+    double S = 0.0, I = 0.0, n = 0.0;
+    for (int r = 0; r < n_ranks; ++r) { S += parts[3 * r]; I += parts[3 * r + 1]; n += parts[3 * r + 2]; }
+    *nll = n > 0.0 ? -S + n * std::log(I) : 0.0;
+    if (sum_log) *sum_log = S;
+    if (integral) *integral = I;
+    if (n_ev) *n_ev = (int64_t)n;
+    return MIPWA_OK;
+}
+
+// whole-sample NLL and gradient from the gathered mipwa_nll_grad_parts pieces, parts[r] = (S_r, I_r, n_r, grad_ev_r[P],
+// grad_nm_r[P]): NLL = -sum S_r + n ln I, grad = sum grad_ev_r + (n / I) sum grad_nm_r, every sum in rank order
+int mipwa_combine_grad_parts(int32_t n_ranks, int64_t n_params, const double* parts, double* nll, double* grad,
+                             double* sum_log, double* integral, int64_t* n_ev)
+{
+    if (n_ranks < 1 || n_params < 0 || !parts || !nll || (n_params > 0 && !grad)) return MIPWA_ERR_ARG;
+    const int64_t P = n_params, stride = 3 + 2 * P;
+    double S = 0.0, I = 0.0, n = 0.0;
+    for (int r = 0; r < n_ranks; ++r) { S += parts[r * stride]; I += parts[r * stride + 1]; n += parts[r * stride + 2]; }
+    for (int64_t k = 0; k < P; ++k) {
+        double ge = 0.0, gn = 0.0;
+        for (int r = 0; r < n_ranks; ++r) { ge += parts[r * stride + 3 + k]; gn += parts[r * stride + 3 + P + k]; }
+        grad[k] = n > 0.0 ? ge + (n / I) * gn : 0.0;
+    }
+    *nll = n > 0.0 ? -S + n * std::log(I) : 0.0;
+    if (sum_log) *sum_log = S;
+    if (integral) *integral = I;
+    if (n_ev) *n_ev = (int64_t)n;
+    return MIPWA_OK;
 }
 
 int mipwa_eval_abs2(mipwa_ctx* c, const double* params, int64_t n_params, int32_t which, double* out, int64_t n)
@@ -1644,7 +1737,7 @@ int mipwa_nll_mix(mipwa_ctx* c, const double* params, int64_t n_params, double f
     c->timing = false;                                     // wait_result polls: one pair of events spans both launches
     long long tag = next_tag(c);
     cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0, 0,
-                                                G.rec, G.n, c->d_partials, c->d_ticket, c->d_result, tag);
+                                                G.rec, G.n, c->d_partials, c->d_ticket, c->result_dst, tag);
     ++c->launches;
     if (le == cudaSuccess) rc = wait_result(c, tag);
     const double I = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
@@ -1653,7 +1746,7 @@ int mipwa_nll_mix(mipwa_ctx* c, const double* params, int64_t n_params, double f
     if (le == cudaSuccess && rc == MIPWA_OK && E.n > 0) {
         tag = next_tag(c);
         le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, true, grid, c->stream, c->model, E.rec, kappa, E.n, G.rec,
-                                        0, c->d_partials, c->d_ticket, c->d_result, tag);
+                                        0, c->d_partials, c->d_ticket, c->result_dst, tag);
         ++c->launches;
         if (le == cudaSuccess) rc = wait_result(c, tag);
         S = c->h_result[0];
@@ -1724,18 +1817,124 @@ int mipwa_nll_mix_grad(mipwa_ctx* c, const double* params, int64_t n_params, dou
     return MIPWA_OK;
 }
 
-// ---- Hessian in the linear-coefficient parameters, fixed shapes (include/mipwa.h) ---------------------------------------
-int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad, double* hess)
+// ---- sharded mixture likelihood (include/mipwa.h): the event sum needs the integral of the WHOLE sample, so a call is two
+// phases with one exchange between them -----------------------------------------------------------------------------------
+// phase 1: this rank's I_r = sum_j w_j |A_j|^2 and dI_r/dtheta over the 2N + 2R linear-coefficient parameters
+int mipwa_norm_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* integral, double* grad_nm)
 {
-    if (!c || !params || !nll || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
-    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "mipwa_nll_hessian needs fixed resonance shapes");
-    // dense parametrisation: c = [y_k (knot values), c_r (list order, the constant term with its column of ones)];
-    // a model without spline has two stand-in knots in its tables (k < k0) that are no parameters
-    const int N = c->N, Np = c->Np, R = c->R, K = N + R, P = c->n_par(), pb = c->pb(), k0 = N - Np;
-    std::vector<double> gpol(P);
-    int rc = mipwa_nll_grad(c, params, n_params, nll, gpol.data());
+    if (!c || !params || !integral) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    NvtxRange range("mipwa_norm_parts");
+    int rc = use_device(c);
     if (rc) return rc;
-    if (grad) std::memcpy(grad, gpol.data(), P * sizeof(double));
+    rc = prepare_sorted(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    const int N = c->N, R = c->R, Rd = (int)c->perm.size();
+    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
+    GradTotals t;
+    rc = launch_grad_recompute(c, false, 0, 0.0, false, true, false, &t);
+    if (rc) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    *integral = t.nm[0] * wn;
+    if (!grad_nm) return MIPWA_OK;
+    const double *Fn = t.F(t.nm), *Bn = t.bins(t.nm, Rd);
+    std::vector<double> Gsc(t.nb), Gy(2 * N), Gr(2 * std::max(R, 1), 0.0);
+    for (int k = 0; k < t.nb; ++k) Gsc[k] = 2.0 * wn * Bn[k];
+    spline_adjoint(c, Gsc.data(), Gy.data());
+    for (int d = 0; d < Rd; ++d) {
+        const int r = c->perm[d];
+        Gr[2 * r] = c->res_fold[d] * 2.0 * wn * Fn[2 * d];
+        Gr[2 * r + 1] = c->res_fold[d] * 2.0 * wn * Fn[2 * d + 1];
+    }
+    offset_rule(c, Gy.data(), Gr.data());
+    polar_chain(c, params, Gy.data(), Gr.data(), grad_nm);
+    return MIPWA_OK;
+}
+
+// phase 2, with I of the whole sample: S_r = sum_i ln(|A_i|^2 + kappa b_i), Q_r = sum_i b_i / D_i and d(-S_r)/dtheta at
+// fixed kappa = I (1 - f_s) / f_s, over this rank's events
+int mipwa_nll_mix_parts(mipwa_ctx* c, const double* params, int64_t n_params, double f_sig, double integral_total,
+                        double* sum_log, double* q, double* grad_ev)
+{
+    if (!c || !params || !sum_log || !q) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    if (c->ev.n > 0 && !c->ev.w) return fail(c, MIPWA_ERR_STATE, "set the background densities (mipwa_set_event_background)");
+    if (!(f_sig > 0.0 && f_sig <= 1.0) || !(integral_total > 0.0)) return fail(c, MIPWA_ERR_ARG, "need 0 < f_sig <= 1 and I > 0");
+    NvtxRange range("mipwa_nll_mix_parts");
+    int rc = use_device(c);
+    if (rc) return rc;
+    rc = prepare_sorted(c);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    const int N = c->N, R = c->R, Rd = (int)c->perm.size(), P = 2 * c->Np + 2 * R;
+    *sum_log = 0.0; *q = 0.0;
+    if (grad_ev) for (int k = 0; k < P; ++k) grad_ev[k] = 0.0;
+    if (c->ev.n == 0) return MIPWA_OK;
+    const double kappa = integral_total * (1.0 - f_sig) / f_sig;
+    GradTotals t;
+    rc = launch_grad_recompute(c, true, 0, kappa, true, false, false, &t);
+    if (rc) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    *sum_log = t.ev[0]; *q = t.ev[1];
+    if (!grad_ev) return MIPWA_OK;
+    const double *Fe = t.F(t.ev), *Be = t.bins(t.ev, Rd);
+    std::vector<double> Gy(2 * N), Gr(2 * std::max(R, 1), 0.0);
+    spline_adjoint(c, Be, Gy.data());
+    for (int d = 0; d < Rd; ++d) {
+        const int r = c->perm[d];
+        Gr[2 * r] = c->res_fold[d] * Fe[2 * d];
+        Gr[2 * r + 1] = c->res_fold[d] * Fe[2 * d + 1];
+    }
+    offset_rule(c, Gy.data(), Gr.data());
+    polar_chain(c, params, Gy.data(), Gr.data(), grad_ev);
+    return MIPWA_OK;
+}
+
+// whole-sample mixture likelihood from the gathered pieces, sums in rank order:
+//   norm_parts[r] = (I_r, dI_r/dtheta[P]),  ev_parts[r] = (S_r, Q_r, n_r, d(-S_r)/dtheta[P]);  I = sum I_r must be the
+//   value phase 2 was given.   NLL = -S - n ln(f_s / I),  grad = sum grad_ev + ((n - kappa Q) / I) sum dI/dtheta,
+//   dNLL/df_s = -(n - I Q / f_s) / f_s.  Host only.
+int mipwa_combine_mix_parts(int32_t n_ranks, int64_t n_lin, double f_sig, const double* norm_parts, const double* ev_parts,
+                            double* nll, double* grad, double* dnll_dfsig)
+{
+    if (n_ranks < 1 || n_lin < 0 || !norm_parts || !ev_parts || !nll || !(f_sig > 0.0 && f_sig <= 1.0)) return MIPWA_ERR_ARG;
+    const int64_t P = n_lin, sn = 1 + P, se = 3 + P;
+    double I = 0.0, S = 0.0, Q = 0.0, n = 0.0;
+    for (int r = 0; r < n_ranks; ++r) {
+        I += norm_parts[r * sn];
+        S += ev_parts[r * se]; Q += ev_parts[r * se + 1]; n += ev_parts[r * se + 2];
+    }
+    const double kappa = I * (1.0 - f_sig) / f_sig;
+    *nll = -S - n * std::log(f_sig / I);
+    if (dnll_dfsig) *dnll_dfsig = -(n - I * Q / f_sig) / f_sig;
+    if (grad)
+        for (int64_t k = 0; k < P; ++k) {
+            double ge = 0.0, gn = 0.0;
+            for (int r = 0; r < n_ranks; ++r) { ge += ev_parts[r * se + 3 + k]; gn += norm_parts[r * sn + 1 + k]; }
+            grad[k] = ge + (n - kappa * Q) / I * gn;
+        }
+    return MIPWA_OK;
+}
+
+// ---- Hessian in the linear-coefficient parameters, fixed shapes (include/mipwa.h) ---------------------------------------
+// Dense parametrisation: c = [y_k (knot values), c_r (list order, the constant term with its column of ones)], K = N + R
+// entries; a model without spline has two stand-in knots in its tables (k < N - Np) that are no parameters.
+int64_t mipwa_hessian_parts_len(const mipwa_ctx* c) { return c ? 2 * (int64_t)(c->N + c->R) * (c->N + c->R) : MIPWA_ERR_ARG; }
+
+// this rank's sums: M_kl = sum_i B_ik B_il / A_i^2 over ITS events (k_gram in HESS mode) and the Gram matrix G over ITS
+// normalisation points; both K x K complex, row-major, (re, im) interleaved.  Summed over the ranks they are the
+// whole-sample matrices mipwa_hessian_assemble takes.
+int mipwa_hessian_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* M, double* G)
+{
+    if (!c || !params || !M || !G) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "the analytic Hessian needs fixed resonance shapes");
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    const int K = c->N + c->R;
+    int rc = use_device(c);
+    if (rc) return rc;
     rc = ensure_gram(c);
     if (rc) return rc;
     rc = build_model(c, params, n_params);                 // y_k of this call for fill_coef
@@ -1744,14 +1943,12 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
     fill_coef(c, params, &cc);
     rc = build_unit_model(c, nullptr);                     // the basis kernels evaluate the unit-coefficient model
     if (rc) return rc;
-
-    // M_kl = sum_i B_ik B_il / A_i^2 over the events (k_gram in HESS mode), reduced in block order
     const Slot& E = evs(c);
     const int nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, tpt = (ntile + MIPWA_TILE - 1) / MIPWA_TILE;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((E.n + GRAM_P - 1) / GRAM_P, c->sm_count));
     const size_t smem = (size_t)4 * nt * GRAM_LD * sizeof(double2);
     double2 *partial = nullptr, *d_M = nullptr;
-    std::vector<double> hM((size_t)2 * K * K, 0.0);
+    for (size_t t = 0; t < (size_t)2 * K * K; ++t) M[t] = 0.0;
     cudaError_t e = cudaMalloc(&partial, (size_t)grid * K * K * sizeof(double2));
     if (e == cudaSuccess) e = cudaMalloc(&d_M, (size_t)K * K * sizeof(double2));
     if (e == cudaSuccess && E.n > 0) {
@@ -1771,17 +1968,32 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
             ++c->launches;
             e = cudaGetLastError();
         }
-        if (e == cudaSuccess) e = cudaMemcpyAsync(hM.data(), d_M, (size_t)K * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(M, d_M, (size_t)K * K * sizeof(double2), cudaMemcpyDeviceToHost, c->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     }
     if (partial) cudaFree(partial);
     if (d_M) cudaFree(d_M);
     if (e != cudaSuccess)
         return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, std::string("hessian: ") + cudaGetErrorString(e));
+    std::memcpy(G, c->h_gram.data(), (size_t)2 * K * K * sizeof(double));
+    return MIPWA_OK;
+}
 
+// Hessian of the whole sample from the summed pieces: M, G (mipwa_hessian_parts, added over the ranks), the event count
+// and the polar gradient of the whole sample (mipwa_nll_grad, or the combined mipwa_nll_grad_parts).  Host only.
+int mipwa_hessian_assemble(mipwa_ctx* c, const double* params, int64_t n_params, int64_t n_ev_total, const double* hM,
+                           const double* hG, const double* gpol, double* hess)
+{
+    if (!c || !params || !hM || !hG || !gpol || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "the analytic Hessian needs fixed resonance shapes");
+    const int N = c->N, Np = c->Np, R = c->R, K = N + R, P = c->n_par(), pb = c->pb(), k0 = N - Np;
+    int rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    CoefDev cc;
+    fill_coef(c, params, &cc);
     // ---- host: O(K^2) assembly.  Wirtinger blocks from M, G, c, then the polar chain rule -------------------------------
     typedef std::complex<double> cx;
-    auto Gm = [&](int k, int l) { return cx(c->h_gram[2 * ((size_t)k * K + l)], c->h_gram[2 * ((size_t)k * K + l) + 1]); };
+    auto Gm = [&](int k, int l) { return cx(hG[2 * ((size_t)k * K + l)], hG[2 * ((size_t)k * K + l) + 1]); };
     auto Mm = [&](int k, int l) { return cx(hM[2 * ((size_t)k * K + l)], hM[2 * ((size_t)k * K + l) + 1]); };
     std::vector<cx> cv(K), cG(K), Gc(K), e1(K), g(K);
     std::vector<int> ir(K, 0), ip(K, 0);
@@ -1791,7 +2003,7 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
         ip[k] = k < N ? Np + k : pb + 2 * (k - N) + 1;
         e1[k] = cx(std::cos(params[ip[k]]), std::sin(params[ip[k]]));
         if (!(std::fabs(params[ir[k]]) > 0.0))
-            return fail(c, MIPWA_ERR_ARG, "mipwa_nll_hessian: a zero magnitude makes the polar Hessian singular");
+            return fail(c, MIPWA_ERR_ARG, "mipwa_hessian_assemble: a zero magnitude makes the polar Hessian singular");
     }
     cx Iq = 0.0;
     for (int k = 0; k < K; ++k) {
@@ -1800,7 +2012,7 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
         cG[k] = a; Gc[k] = b;
     }
     for (int k = 0; k < K; ++k) Iq += std::conj(cv[k]) * Gc[k];
-    const double I = Iq.real(), nev = (double)c->ev.n;
+    const double I = Iq.real(), nev = (double)n_ev_total;
     // dNLL/dc_k from the polar gradient: dNLL/drho = 2 Re(g e^{i phi}), dNLL/dphi = 2 Re(g i c) = -2 rho Im(g e^{i phi})
     for (int k = k0; k < K; ++k) {
         const double rho = params[ir[k]];
@@ -1824,6 +2036,23 @@ int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, doub
         hess[(size_t)ip[k] * P + ip[k]] += pp;
     }
     return MIPWA_OK;
+}
+
+
+// NLL, gradient and Hessian of one context's own sample
+int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad, double* hess)
+{
+    if (!c || !params || !nll || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "mipwa_nll_hessian needs fixed resonance shapes");
+    NvtxRange range("mipwa_nll_hessian");
+    const int P = c->n_par(), K = c->N + c->R;
+    std::vector<double> gpol(P), M((size_t)2 * K * K), G((size_t)2 * K * K);
+    int rc = mipwa_nll_grad(c, params, n_params, nll, gpol.data());
+    if (rc) return rc;
+    if (grad) std::memcpy(grad, gpol.data(), P * sizeof(double));
+    rc = mipwa_hessian_parts(c, params, n_params, M.data(), G.data());
+    if (rc) return rc;
+    return mipwa_hessian_assemble(c, params, n_params, c->ev.n, M.data(), G.data(), gpol.data(), hess);
 }
 
 // ---- toy generation on the device (gen.cuh) -------------------------------------------------------------------------

@@ -120,3 +120,41 @@ def test_gradient_combine_without_process_group():
     nll, g, S, Iv, n = sharding.combine_grad_parts(12.5, 3.0, 7, ge, gn)
     assert nll == -12.5 + 7 * np.log(3.0) and np.array_equal(g, ge + (7 / 3.0) * gn) and n == 7
     assert sharding.combine_grad_parts(0.0, 3.0, 0, ge, gn)[0] == 0.0
+
+
+def test_mixture_combine_matches_the_whole_sample_oracle():
+    """mipwa_combine_mix_parts (C library, host only) on per-slice pieces built from the ORACLE's pinned quantities:
+    phase 1 (I_r, dI_r/dtheta) = O9b, phase 2 (S_r, Q_r, d(-S_r)/dtheta at fixed kappa) from the oracle's mixture NLL of
+    the slice with the WHOLE-sample integral forced through its weights.  The combination must give the oracle's
+    whole-sample mixture likelihood O12 (value, gradient and d/df_s)."""
+    from oracle import oracle as orc
+    from paper_1703_03284_b200 import binding, inputs as I
+    c = I.Config(1, n_ev=901, n_norm=1201)
+    o = orc.Oracle(c.kin, c.knots, c.resonances)
+    g12, g13, w = c.norm_points()
+    e12, e13 = I.phase_space_points(c.n_ev, c.key(I.S_EVENTS))
+    rng = np.random.default_rng(3)
+    bkg = rng.uniform(0.05, 0.4, c.n_ev)
+    p, f_sig, P, world = c.perturbed(0), 0.85, 2 * c.N + 2 * c.R, 3
+    ref, gref, dref = o.nll_mix(p, e12, e13, bkg, f_sig, g12, g13, w, grad=True)
+    _, _, I_tot = o.nll(p, e12, e13, g12, g13, w, parts=True)
+    kappa = I_tot * (1 - f_sig) / f_sig
+    norm_rows, ev_rows = [], []
+    for r in range(world):
+        lo, hi = sharding.shard_range(c.n_ev, r, world)
+        glo, ghi = sharding.shard_range(g12.size, r, world)
+        _, I_r, _, gnm = o.nll_grad_parts(p, e12[:1], e13[:1], g12[glo:ghi], g13[glo:ghi], w[glo:ghi])
+        norm_rows.append(np.concatenate([[I_r], gnm[:P]]))
+        # event pieces of the slice: D_i = |A_i|^2 + kappa b_i;  d(-S)/dtheta at fixed kappa = -sum (d|A_i|^2/dtheta) / D_i,
+        # taken from the oracle's O9b event gradient of a sample re-weighted event by event: -sum_i dln|A_i|^2 * (|A_i|^2/D_i)
+        a2 = o.abs2(p, e12[lo:hi], e13[lo:hi])
+        D = a2 + kappa * bkg[lo:hi]
+        gev = np.zeros(P)
+        for i in range(lo, hi):                             # one event at a time: d(-ln|A_i|^2)/dtheta from O9b
+            _, _, gi, _ = o.nll_grad_parts(p, e12[i:i + 1], e13[i:i + 1], g12[:1], g13[:1], w[:1])
+            gev += gi[:P] * (a2[i - lo] / D[i - lo])
+        ev_rows.append(np.concatenate([[np.sum(np.log(D)), np.sum(bkg[lo:hi] / D), hi - lo], gev]))
+    nll, g, dfs = binding.combine_mix_parts(np.array(norm_rows), np.array(ev_rows), P, f_sig)
+    assert abs(nll - ref) <= 1e-10 * max(abs(ref), c.n_ev)
+    assert np.max(np.abs(g - gref)) <= 1e-9 * np.max(np.abs(gref))
+    assert abs(dfs - dref) <= 1e-9 * max(1.0, abs(dref))
