@@ -235,6 +235,14 @@ int mipwa_combine_mix_parts(int32_t n_ranks, int64_t n_lin, double f_sig, const 
  * polar parametrisation is singular there). */
 int mipwa_nll_hessian(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad, double* hess);
 
+/* The Hessian over ALL n_params parameters, floating masses and widths included (the full error matrix of a fit whose
+ * resonance shapes float).  Block of the linear coefficients: the formulas above with the basis at the current masses and
+ * widths.  Rows and columns of a floating mass or width: central differences of the analytic gradient
+ * (mipwa_nll_grad_full) in that parameter, Richardson-extrapolated from the steps h and h / 2 with h = 1e-3 x the width
+ * (four gradient calls per floating shape parameter; relative accuracy ~1e-8).  Identical to mipwa_nll_hessian when no
+ * shape floats.  grad: HOST, n_params doubles, may be NULL;  hess: HOST, n_params^2 doubles, row-major, symmetric. */
+int mipwa_nll_hessian_full(mipwa_ctx* ctx, const double* params, int64_t n_params, double* nll, double* grad, double* hess);
+
 /* The same Hessian for a SHARDED sample.  Both sums of the formulas above are sums over points:
  *   mipwa_hessian_parts      this rank's M_kl = sum_i B_ik B_il / A_i^2 (its events) and G_kl (its normalisation points,
  *                            whole-sample weights): HOST, mipwa_hessian_parts_len() doubles each = K x K complex, row-major,

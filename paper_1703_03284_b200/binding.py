@@ -28,7 +28,7 @@ SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_event
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version", "mipwa_nll_parts_device", "mipwa_combine_parts_device", "mipwa_combine_parts",
            "mipwa_combine_grad_parts", "mipwa_norm_parts", "mipwa_nll_mix_parts", "mipwa_combine_mix_parts",
-           "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble"]
+           "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble", "mipwa_nll_hessian_full"]
 
 
 class MipwaError(RuntimeError):
@@ -98,6 +98,7 @@ def load_library():
     L.mipwa_norm_parts.restype = i32; L.mipwa_norm_parts.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_nll_mix_parts.restype = i32; L.mipwa_nll_mix_parts.argtypes = [vp, _dp, i64, d, d, _dp, _dp, _dp]
     L.mipwa_combine_mix_parts.restype = i32; L.mipwa_combine_mix_parts.argtypes = [i32, i64, d, _dp, _dp, _dp, _dp, _dp]
+    L.mipwa_nll_hessian_full.restype = i32; L.mipwa_nll_hessian_full.argtypes = [vp, _dp, i64, _dp, _dp, _dp]
     L.mipwa_hessian_parts_len.restype = i64; L.mipwa_hessian_parts_len.argtypes = [vp]
     L.mipwa_hessian_parts.restype = i32; L.mipwa_hessian_parts.argtypes = [vp, _dp, i64, _dp, _dp]
     L.mipwa_hessian_assemble.restype = i32; L.mipwa_hessian_assemble.argtypes = [vp, _dp, i64, i64, _dp, _dp, _dp, _dp]
@@ -293,6 +294,13 @@ class Mipwa:
         P = 2 * self.N + 2 * self.R
         out, grad, H = C.c_double(), np.empty(P), np.empty((P, P))
         self._check(self.L.mipwa_nll_hessian(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp), H.ctypes.data_as(_dp)))
+        return out.value, grad, H
+
+    def nll_hessian_full(self, params):
+        """(NLL, gradient, Hessian) over all n_params parameters, floating masses and widths included"""
+        p, pp, n = self._params(params)
+        out, grad, H = C.c_double(), np.empty(p.size), np.empty((p.size, p.size))
+        self._check(self.L.mipwa_nll_hessian_full(self._h, pp, n, C.byref(out), grad.ctypes.data_as(_dp), H.ctypes.data_as(_dp)))
         return out.value, grad, H
 
     def nll_parts_device(self, params, dev_parts):

@@ -822,10 +822,13 @@ static int ensure_cache(mipwa_ctx* c, int kind)
     return MIPWA_OK;
 }
 
-static int ensure_gram(mipwa_ctx* c)
+// shapes: parameter vector whose floating masses and widths the basis is built with (mipwa_nll_hessian_full: the Gram
+// matrix is then rebuilt on every call); nullptr: the listed shapes, built once per set of normalisation points
+static int ensure_gram(mipwa_ctx* c, const double* shapes = nullptr)
 {
-    if (c->gram_valid) return MIPWA_OK;
-    int rc = build_unit_model(c, nullptr);
+    if (c->gram_valid && !(shapes && c->F > 0)) return MIPWA_OK;
+    c->gram_valid = false;
+    int rc = build_unit_model(c, shapes);
     if (rc) return rc;
     const int K = c->N + c->R, nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2;
     const int tpt = (ntile + MIPWA_TILE - 1) / MIPWA_TILE;
@@ -860,7 +863,7 @@ static int ensure_gram(mipwa_ctx* c)
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     cudaFree(partial);
     if (e != cudaSuccess) return fail(c, MIPWA_ERR_CUDA, std::string("gram: ") + cudaGetErrorString(e));
-    c->gram_valid = true;
+    c->gram_valid = !(shapes && c->F > 0);
     return MIPWA_OK;
 }
 
@@ -1927,21 +1930,19 @@ int64_t mipwa_hessian_parts_len(const mipwa_ctx* c) { return c ? 2 * (int64_t)(c
 // this rank's sums: M_kl = sum_i B_ik B_il / A_i^2 over ITS events (k_gram in HESS mode) and the Gram matrix G over ITS
 // normalisation points; both K x K complex, row-major, (re, im) interleaved.  Summed over the ranks they are the
 // whole-sample matrices mipwa_hessian_assemble takes.
-int mipwa_hessian_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* M, double* G)
+static int hessian_parts_at(mipwa_ctx* c, const double* params, int64_t n_params, double* M, double* G)
 {
-    if (!c || !params || !M || !G) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
-    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "the analytic Hessian needs fixed resonance shapes");
     if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
     const int K = c->N + c->R;
     int rc = use_device(c);
     if (rc) return rc;
-    rc = ensure_gram(c);
+    rc = ensure_gram(c, params);                           // floating shapes: the basis at the shapes of `params`
     if (rc) return rc;
     rc = build_model(c, params, n_params);                 // y_k of this call for fill_coef
     if (rc) return rc;
     CoefDev cc;
     fill_coef(c, params, &cc);
-    rc = build_unit_model(c, nullptr);                     // the basis kernels evaluate the unit-coefficient model
+    rc = build_unit_model(c, params);                      // the basis kernels evaluate the unit-coefficient model
     if (rc) return rc;
     const Slot& E = evs(c);
     const int nt = (K + 3) / 4, ntile = nt * (nt + 1) / 2, tpt = (ntile + MIPWA_TILE - 1) / MIPWA_TILE;
@@ -1979,13 +1980,20 @@ int mipwa_hessian_parts(mipwa_ctx* c, const double* params, int64_t n_params, do
     return MIPWA_OK;
 }
 
+int mipwa_hessian_parts(mipwa_ctx* c, const double* params, int64_t n_params, double* M, double* G)
+{
+    if (!c || !params || !M || !G) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "the analytic Hessian needs fixed resonance shapes");
+    return hessian_parts_at(c, params, n_params, M, G);
+}
+
 // Hessian of the whole sample from the summed pieces: M, G (mipwa_hessian_parts, added over the ranks), the event count
 // and the polar gradient of the whole sample (mipwa_nll_grad, or the combined mipwa_nll_grad_parts).  Host only.
-int mipwa_hessian_assemble(mipwa_ctx* c, const double* params, int64_t n_params, int64_t n_ev_total, const double* hM,
-                           const double* hG, const double* gpol, double* hess)
+// the block of the linear-coefficient parameters of a P x P matrix (P = n_params: the rows and columns of floating masses
+// and widths, if any, are left at zero)
+static int hessian_assemble_at(mipwa_ctx* c, const double* params, int64_t n_params, int64_t n_ev_total, const double* hM,
+                               const double* hG, const double* gpol, double* hess)
 {
-    if (!c || !params || !hM || !hG || !gpol || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
-    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "the analytic Hessian needs fixed resonance shapes");
     const int N = c->N, Np = c->Np, R = c->R, K = N + R, P = c->n_par(), pb = c->pb(), k0 = N - Np;
     int rc = build_model(c, params, n_params);
     if (rc) return rc;
@@ -2038,6 +2046,61 @@ int mipwa_hessian_assemble(mipwa_ctx* c, const double* params, int64_t n_params,
     return MIPWA_OK;
 }
 
+
+int mipwa_hessian_assemble(mipwa_ctx* c, const double* params, int64_t n_params, int64_t n_ev_total, const double* hM,
+                           const double* hG, const double* gpol, double* hess)
+{
+    if (!c || !params || !hM || !hG || !gpol || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F > 0) return fail(c, MIPWA_ERR_STATE, "the analytic Hessian needs fixed resonance shapes");
+    return hessian_assemble_at(c, params, n_params, n_ev_total, hM, hG, gpol, hess);
+}
+
+// Hessian over ALL n_params parameters ("correlations between the parameters").  The block of
+// the linear coefficients is the analytic one, evaluated with the basis at the CURRENT masses and widths; the rows and
+// columns of the floating masses and widths are central differences of the analytic gradient (mipwa_nll_grad_full) in
+// that one parameter, Richardson-extrapolated from the steps h and h / 2, h = 1e-3 x the resonance's width: four
+// gradient calls per floating shape parameter, relative accuracy ~1e-8.
+int mipwa_nll_hessian_full(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad, double* hess)
+{
+    if (!c || !params || !nll || !hess) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    if (c->F == 0) return mipwa_nll_hessian(c, params, n_params, nll, grad, hess);
+    NvtxRange range("mipwa_nll_hessian_full");
+    const int P = c->n_par(), K = c->N + c->R, Pl = c->pb() + 2 * c->R;
+    std::vector<double> g0(P), M((size_t)2 * K * K), G((size_t)2 * K * K);
+    int rc = mipwa_nll_grad_full(c, params, n_params, nll, g0.data());
+    if (rc) return rc;
+    if (grad) std::memcpy(grad, g0.data(), P * sizeof(double));
+    rc = hessian_parts_at(c, params, n_params, M.data(), G.data());
+    if (rc) return rc;
+    rc = hessian_assemble_at(c, params, n_params, c->ev.n, M.data(), G.data(), g0.data(), hess);
+    if (rc) return rc;
+    std::vector<double> p(params, params + P), gp(P), gm(P), row(P);
+    for (int s = 0; s < 2 * c->F; ++s) {
+        const int idx = Pl + s;
+        const double h = 1e-3 * params[Pl + (s | 1)];      // the width of that resonance sets the scale of both
+        for (int k = 0; k < P; ++k) row[k] = 0.0;
+        for (int level = 0; level < 2; ++level) {
+            const double hh = level == 0 ? h : 0.5 * h, wgt = level == 0 ? -1.0 / 3.0 : 4.0 / 3.0;
+            double dummy;
+            p[idx] = params[idx] + hh;
+            rc = mipwa_nll_grad_full(c, p.data(), n_params, &dummy, gp.data());
+            if (rc) return rc;
+            p[idx] = params[idx] - hh;
+            rc = mipwa_nll_grad_full(c, p.data(), n_params, &dummy, gm.data());
+            if (rc) return rc;
+            p[idx] = params[idx];
+            for (int k = 0; k < P; ++k) row[k] += wgt * (gp[k] - gm[k]) / (2.0 * hh);
+        }
+        for (int k = 0; k < P; ++k) {
+            if (k >= Pl && k < idx) {                      // shape-shape pair met from both sides: the mean of the two
+                hess[(size_t)idx * P + k] = hess[(size_t)k * P + idx] = 0.5 * (hess[(size_t)k * P + idx] + row[k]);
+            } else {
+                hess[(size_t)idx * P + k] = hess[(size_t)k * P + idx] = row[k];
+            }
+        }
+    }
+    return MIPWA_OK;
+}
 
 // NLL, gradient and Hessian of one context's own sample
 int mipwa_nll_hessian(mipwa_ctx* c, const double* params, int64_t n_params, double* nll, double* grad, double* hess)
