@@ -360,11 +360,32 @@ def run_ours(args, cfg, workload):
         tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         e2e_s = float(tt.item())
+    # what the bus alone does: the same pinned arrays copied to the device, nothing else
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        tmp = [t.to(dev, non_blocking=True) for t in pinned]
+        torch.cuda.synchronize(dev)
+    h2d_only_s = (time.perf_counter() - t0) / 3
+    del tmp
     h2d = sum(a.nbytes for a in ph) + params[0].nbytes
     d2h = 16 + 24                                     # two boundary-check counters + (sum ln|A|^2, I, tag)
     # back to resident device arrays for the fit-step latency number
     m.set_events(d[0], d[1]); m.set_norm_points(d[2], d[3], d[4]); m.prepare()
     fit_step_s, _ = wall_of(step, params[args.warmup:], args.steps)
+
+    # the sharded step that stays on the device (mipwa_nll_parts_device -> all_gather -> mipwa_combine_parts_device)
+    with torch.cuda.stream(stream):
+        bufs = (torch.empty(3, dtype=torch.float64, device=dev), torch.empty(3 * world, dtype=torch.float64, device=dev))
+        dev_step = lambda p: sharding.nll_sharded_device(m, p, bufs)[0]
+        for t in range(5):
+            dev_step(params[t])
+        barrier()
+        dev_step_s, nll_dev = wall_of(dev_step, params[args.warmup:], min(args.steps, 200))
+        barrier()
+    sharded_device = {"ms_per_call": 1e3 * dev_step_s, "nll": nll_dev, "extra_us_over_fit_step": 1e6 * (dev_step_s - fit_step_s),
+                      "what": "mipwa_nll_parts_device + all_gather_into_tensor (N > 1) + mipwa_combine_parts_device: no host "
+                              "round trip between the likelihood kernel and the combined value"}
 
     # ---- A8: value + analytic gradient (BASELINE configs[3]: "plus analytic gradient w.r.t. all 2N+2*3 parameters") ----
     sub_steps = max(3, min(args.steps, 30))
@@ -445,7 +466,10 @@ def run_ours(args, cfg, workload):
     mc.set_events(d[0], d[1]); mc.set_norm_points(d[2], d[3], d[4])
     mc.prepare()
     pc = [p[:2 * cfg.N + 2 * cfg.R] for p in sub]
-    for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT)):
+    kernels = {"dense": "k_nll_dense", "compact": "k_nll_compact", "dense_real": "k_nll_dense_real<double>",
+               "dense_f32": "k_nll_dense_real<float> (opt-in: fp32-stored columns, outside the 1e-12 contract)"}
+    for name, path in (("dense", B.PATH_CACHED), ("compact", B.PATH_CACHED_COMPACT), ("dense_real", B.PATH_CACHED_REAL),
+                       ("dense_f32", B.PATH_CACHED_F32)):
         mc.set_path(path)
         t0 = time.perf_counter(); mc.nll(pc[0]); setup_s = time.perf_counter() - t0
         k, _ = kernel_ms_of(mc, mc.nll, pc, sub_steps)
@@ -455,7 +479,7 @@ def run_ours(args, cfg, workload):
         cached_info[name] = {"ms_per_call": 1e3 * wall, "kernel_ms": k, "events_per_s": n_ev * world / wall,
                              "bytes_per_event": nbytes / max(n_ev, 1), "cache_bytes": mc.basis_bytes(),
                              "first_call_s": setup_s, "nll": nll_c,
-                             "roofline": {"bound": "hbm", "kernel": "k_nll_dense" if name == "dense" else "k_nll_compact",
+                             "roofline": {"bound": "hbm", "kernel": kernels[name],
                                           "achieved": nbytes / (k * 1e-3) * 1e-9, "unit": "GB/s", "traffic": None,
                                           "peak": hbm, "frac": nbytes / (k * 1e-3) * 1e-9 / hbm, "peak_source": hbm_src}}
     mc.set_path(B.PATH_CACHED_COMPACT)                 # gradient from the compact cache + Gram matrix (k_grad_compact)
@@ -546,10 +570,11 @@ def run_ours(args, cfg, workload):
             "nll": nll, "clocks": clocks, "gpu_launches": int(launches) * world,
             "e2e": {"value": total_events / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_s, "nll": nll_e2e,
+                    "h2d_copy_alone_ms": 1e3 * h2d_only_s, "h2d_copy_alone_gbs": (h2d - params[0].nbytes) / h2d_only_s * 1e-9,
                     "what": "mipwa_set_events + mipwa_set_norm_points from pinned HOST arrays + mipwa_nll, every step"},
             "fit_step": {"ms_per_call": 1e3 * fit_step_s, "nll_evals_per_s": 1.0 / fit_step_s,
                          "what": "wall clock of mipwa_nll(host params) -> host fp64 with events resident (what a minimiser sees)"},
-            "prepare_s": t_prep, "roofline": roofline, "grad": grad_info, "mixture": mix_info, "hybrid": hybrid_info,
+            "sharded_device_step": sharded_device, "prepare_s": t_prep, "roofline": roofline, "grad": grad_info, "mixture": mix_info, "hybrid": hybrid_info,
             "cached": cached_info, "latency": latency, "cpu_baseline": cpu, "input_generation_s": t_gen,
             "wall_ms_per_step": 1e3 * (w1 - w0) / args.steps}
     print(json.dumps(line), flush=True)

@@ -209,11 +209,12 @@ k_abs2(const __grid_constant__ DevModel m, const double* __restrict__ s12, const
 struct DevKin { double M2, m1s, m2s, m3s, t_lo, t_d, s_hi, s_top; };
 
 // Also stores the spline segment pair of every point, seg[i] = j12 | j13 << 8 (knots are fixed at mipwa_create, so
-// the pair is a property of the point set): the per-call kernels then index the coefficient rows directly.
+// the pair is a property of the point set): the per-call kernels then index the coefficient rows directly.  With `rec` it
+// also writes the 32-byte records the recompute kernels stream (what k_make_records does on first use otherwise).
 static __global__ void __launch_bounds__(MIPWA_BLOCK)
 k_validate(const DevKin k, const DevSearch* __restrict__ srch, const double* __restrict__ s12,
-           const double* __restrict__ s13, long long n, unsigned short* __restrict__ seg,
-           unsigned long long* __restrict__ bad)
+           const double* __restrict__ s13, const double* __restrict__ w, double w_default, long long n,
+           unsigned short* __restrict__ seg, PointRec* __restrict__ rec, unsigned long long* __restrict__ bad)
 {
     __shared__ SearchSmem ss;
     load_search_smem(ss, srch);
@@ -232,6 +233,12 @@ k_validate(const DevKin k, const DevSearch* __restrict__ srch, const double* __r
         mine += ok ? 0u : 1u;                             // NaN compares false above -> counted as bad
         const int j1 = spline_segment(ss, x), j2 = spline_segment(ss, y);
         seg[i] = (unsigned short)(j1 | (j2 << 8));
+        if (rec) {                                        // the record of the point, while it is in registers anyway
+            PointRec r;
+            r.s12 = x; r.s13 = y; r.w = w ? w[i] : w_default;
+            r.o1 = j1 * MIPWA_ROW_BYTES; r.o2 = j2 * MIPWA_ROW_BYTES;
+            rec[i] = r;
+        }
     }
     mine = __reduce_add_sync(0xffffffffu, mine);
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(bad, (unsigned long long)mine);

@@ -65,6 +65,8 @@ struct mipwa_ctx {
     int device = 0;
     int sm_count = 0;
     cudaStream_t stream = nullptr;
+    cudaStream_t copy_stream = nullptr;   // host -> device uploads of mipwa_set_*, overlapped with the boundary check
+    cudaEvent_t copy_done[2] = { nullptr, nullptr };
     int path = MIPWA_PATH_AUTO;
 
     // natural-spline system (A2): the tridiagonal matrix depends on the knots only -> factor once
@@ -555,6 +557,9 @@ int mipwa_create(const mipwa_kinematics* kin, const double* knots, int32_t n_kno
     ok = ok && cudaHostAlloc(&c->h_bad, 64, cudaHostAllocMapped) == cudaSuccess;
     ok = ok && cudaHostGetDevicePointer(&c->d_bad, c->h_bad, 0) == cudaSuccess;
     ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&c->copy_done[0], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->copy_done[1], cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_Mx, c->Mx.size() * sizeof(double)) == cudaSuccess &&
          cudaMemcpy(c->d_Mx, c->Mx.data(), c->Mx.size() * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_gram, (size_t)(n_knots + n_res) * (n_knots + n_res) * sizeof(double2)) == cudaSuccess;
@@ -586,6 +591,8 @@ void mipwa_destroy(mipwa_ctx* c)
     free_slot(c->ev_sorted); free_slot(c->nm_sorted);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_bad) cudaFreeHost(c->h_bad);
+    if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
+    for (cudaEvent_t e : c->copy_done) if (e) cudaEventDestroy(e);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     delete c;
@@ -627,9 +634,8 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
     if (mem == MIPWA_MEM_HOST && n > 0) {
         const double* src[3] = { s12, s13, w };
         for (int q = 0; q < 3; ++q) {
-            if (!src[q]) continue;
-            cudaError_t e = s.owned[q] ? cudaSuccess : cudaMalloc(&s.owned[q], (size_t)n * sizeof(double));
-            if (e == cudaSuccess) e = cudaMemcpyAsync(s.owned[q], src[q], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+            if (!src[q] || s.owned[q]) continue;
+            const cudaError_t e = cudaMalloc(&s.owned[q], (size_t)n * sizeof(double));
             if (e != cudaSuccess) {
                 free_slot(s);
                 return fail(c, e == cudaErrorMemoryAllocation ? MIPWA_ERR_NOMEM : MIPWA_ERR_CUDA, cudaGetErrorString(e));
@@ -648,23 +654,56 @@ static int set_slot(mipwa_ctx* c, Slot& slot, const double* s12, const double* s
         }
     }
     s.seg = (const unsigned short*)s.owned[3];
-    if (n > 0) {                                           // boundary check on the device (north_star invariant)
+    if (n > 0) {
+        // Boundary check on the device (north_star invariant), which also stores the segment pairs and - when the slot
+        // keeps record storage from an earlier set of the same size (a caller that re-sends its sample every step) -
+        // the 32-byte records, so that the likelihood call that follows finds everything in place.
+        // Host arrays go up in chunks on a second stream: chunk k + 1 is on the bus while chunk k is checked.
         const mipwa_kinematics& k = c->kin;
         DevKin dk = { k.m_parent * k.m_parent, k.m1 * k.m1, k.m2 * k.m2, k.m3 * k.m3,
                       (k.m1 + k.m2) * (k.m1 + k.m2), (k.m1 - k.m2) * (k.m1 - k.m2),
                       (k.m_parent - k.m3) * (k.m_parent - k.m3), (k.m_parent + k.m3) * (k.m_parent + k.m3) };
         *c->h_bad = 0;
-        k_validate<<<grid_for(c, n, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, c->d_search, s.s12, s.s13, n,
-                                                                     (unsigned short*)s.owned[3], c->d_bad);
-        ++c->launches;
-        cudaError_t e = cudaGetLastError();
+        PointRec* rec = (PointRec*)s.owned[4];             // may be null: records are then built on first use
+        const double w_default = allow_empty ? 0.0 : 1.0;  // events carry no weight, unweighted normalisation points 1
+        const bool host = mem == MIPWA_MEM_HOST;
+        const int64_t chunk = host ? (int64_t)1 << 21 : n; // 16 MB per array and chunk
+        cudaError_t e = cudaSuccess;
+        int slot_ev = 0;
+        for (int64_t lo = 0; lo < n && e == cudaSuccess; lo += chunk) {
+            const int64_t len = std::min(chunk, n - lo);
+            if (host) {
+                const double* src[3] = { s12, s13, w };
+                for (int q = 0; q < 3 && e == cudaSuccess; ++q)
+                    if (src[q])
+                        e = cudaMemcpyAsync((double*)s.owned[q] + lo, src[q] + lo, (size_t)len * sizeof(double),
+                                            cudaMemcpyHostToDevice, c->copy_stream);
+                if (e == cudaSuccess) e = cudaEventRecord(c->copy_done[slot_ev], c->copy_stream);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(c->stream, c->copy_done[slot_ev], 0);
+                slot_ev ^= 1;
+            }
+            if (e != cudaSuccess) break;
+            k_validate<<<grid_for(c, len, 8), MIPWA_BLOCK, 0, c->stream>>>(dk, c->d_search, s.s12 + lo, s.s13 + lo,
+                                                                       s.w ? s.w + lo : nullptr, w_default, len,
+                                                                       (unsigned short*)s.owned[3] + lo,
+                                                                       rec ? rec + lo : nullptr, c->d_bad);
+            ++c->launches;
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess && rec) {
+            const int64_t pad = record_pad(c);
+            k_pad_records<<<(int)std::min<int64_t>(c->sm_count, (pad + MIPWA_BLOCK - 1) / MIPWA_BLOCK), MIPWA_BLOCK, 0, c->stream>>>(rec, n, pad);
+            ++c->launches;
+            e = cudaGetLastError();
+        }
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-        if (e != cudaSuccess) { free_slot(s); return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e)); }
+        if (e != cudaSuccess) { cudaStreamSynchronize(c->copy_stream); free_slot(s); return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e)); }
         if (*c->h_bad) {
             const unsigned long long nb = *c->h_bad;
             free_slot(s);
             return fail(c, MIPWA_ERR_DOMAIN, std::to_string(nb) + " point(s) outside the Dalitz boundary");
         }
+        s.rec = rec;
     }
     slot = s;
     return MIPWA_OK;
