@@ -118,17 +118,17 @@ k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__
     __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
-    load_rows_smem(sm, m);
-
     const unsigned int stride = gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const PointRec* p = ev + t0;
+    PointRec r = ld_rec(p);                                // the first record is on its way while the rows are copied
+    load_rows_smem(sm, m);
+
     LogProd lp;
     double integ = 0.0;
     {
         const long long rem = n_ev - t0;
         int left = rem > 0 ? (int)((rem + stride - 1) / stride) : 0;
-        const PointRec* p = ev + t0;
-        PointRec r = ld_rec(p);
         while (left > 0) {
             const int chunk = left < LOGPROD_FLUSH ? left : LOGPROD_FLUSH;
 #pragma unroll 2
@@ -149,8 +149,8 @@ k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__
     {
         const long long rem = n_norm - t0;
         const int iters = rem > 0 ? (int)((rem + stride - 1) / stride) : 0;
-        const PointRec* p = nm + t0;
-        PointRec r = ld_rec(p);
+        p = nm + t0;
+        r = ld_rec(p);
 #pragma unroll 2
         for (int it = 0; it < iters; ++it) {
             p += stride;
