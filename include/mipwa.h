@@ -192,6 +192,27 @@ int mipwa_combine_parts(int32_t n_ranks, const double* parts, double* nll, doubl
 int mipwa_combine_grad_parts(int32_t n_ranks, int64_t n_params, const double* parts, double* nll, double* grad,
                              double* sum_log, double* integral, int64_t* n_ev);
 
+/* mipwa_nll_parts_device for callers that cannot allocate device memory (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same likelihood kernel (steps A4-A6 on the full-recompute path, whatever
+ * mipwa_set_path says), but its scratch memory - one partial pair per block, the ticket counter, the totals - is a
+ * file-scope device array of 512 + 16 * MIPWA_STATIC_MAX_BLOCKS bytes (8.5 KB) that every GPU holds from the moment it
+ * loads the library until the process exits.  The call makes NO cudaMalloc / cudaFree and calls no allocating library
+ * routine; it enqueues three launches on the context's stream and returns without waiting.
+ *   params     HOST, n_params doubles, as mipwa_nll
+ *   blocks     thread blocks (of 512 threads) to run on: 0 = one per SM as mipwa_nll does, otherwise the caller's number
+ *              (part of the GPU); more than MIPWA_STATIC_MAX_BLOCKS, either way, or more than 4 per SM (the padding
+ *              of the record arrays covers that many threads) -> MIPWA_ERR_ARG, nothing launched
+ *   dev_parts  DEVICE, 3 doubles, caller-owned: (S, I, n_ev) as mipwa_nll_parts_device leaves them; valid once the
+ *              context's stream has reached this point (mipwa_combine_parts_device on the same context waits for it)
+ * The 32-byte point records must exist already (building them allocates): one mipwa_nll / mipwa_nll_parts_device on
+ * the recompute path after the mipwa_set_* calls does that, else MIPWA_ERR_STATE.  The first call on each device asks
+ * the runtime for the array's address (no allocation): make it before a capture starts.
+ * ALL calls, of all contexts on a GPU, share the one array: calls that overlap on the GPU (two streams, two contexts,
+ * two threads) race on it and give garbage; calls on one stream are safe, each clears the ticket and totals first.
+ * Other errors as mipwa_nll. */
+#define MIPWA_STATIC_MAX_BLOCKS 512
+int mipwa_nll_parts_static(mipwa_ctx* ctx, const double* params, int64_t n_params, int32_t blocks, double* dev_parts);
+
 /* Signal + background mixture ("signal purity 90 %"): per event the PDF is
  *     f_s |A_i|^2 / I + (1 - f_s) b_i ,      NLL = - sum_i ln( f_s |A_i|^2 / I + (1 - f_s) b_i ),
  * with b_i the background density at event i (normalised over the Dalitz plot, supplied by the caller) and f_s the

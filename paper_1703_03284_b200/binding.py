@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmipwa.so")
 OK, ERR_ARG, ERR_DOMAIN, ERR_STATE, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4, -5
 MEM_HOST, MEM_DEVICE = 0, 1
 PATH_AUTO, PATH_RECOMPUTE, PATH_CACHED, PATH_CACHED_COMPACT, PATH_HYBRID, PATH_CACHED_REAL, PATH_CACHED_F32 = 0, 1, 2, 3, 4, 5, 6
+STATIC_MAX_BLOCKS = 512           # MIPWA_STATIC_MAX_BLOCKS of include/mipwa.h
 _ERR_NAMES = {ERR_ARG: "MIPWA_ERR_ARG", ERR_DOMAIN: "MIPWA_ERR_DOMAIN", ERR_STATE: "MIPWA_ERR_STATE",
               ERR_CUDA: "MIPWA_ERR_CUDA", ERR_NOMEM: "MIPWA_ERR_NOMEM"}
 
@@ -28,7 +29,8 @@ SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_event
            "mipwa_last_kernel_ms", "mipwa_launch_count", "mipwa_measure_fp64_peak", "mipwa_last_error",
            "mipwa_version", "mipwa_nll_parts_device", "mipwa_combine_parts_device", "mipwa_combine_parts",
            "mipwa_combine_grad_parts", "mipwa_norm_parts", "mipwa_nll_mix_parts", "mipwa_combine_mix_parts",
-           "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble", "mipwa_nll_hessian_full"]
+           "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble", "mipwa_nll_hessian_full",
+           "mipwa_nll_parts_static"]
 
 
 class MipwaError(RuntimeError):
@@ -92,6 +94,7 @@ def load_library():
     L.mipwa_version.restype = C.c_char_p; L.mipwa_version.argtypes = []
     pi64 = C.POINTER(i64)
     L.mipwa_nll_parts_device.restype = i32; L.mipwa_nll_parts_device.argtypes = [vp, _dp, i64, vp]
+    L.mipwa_nll_parts_static.restype = i32; L.mipwa_nll_parts_static.argtypes = [vp, _dp, i64, i32, vp]
     L.mipwa_combine_parts_device.restype = i32; L.mipwa_combine_parts_device.argtypes = [vp, vp, i32, _dp, _dp, _dp, pi64]
     L.mipwa_combine_parts.restype = i32; L.mipwa_combine_parts.argtypes = [i32, _dp, _dp, _dp, _dp, pi64]
     L.mipwa_combine_grad_parts.restype = i32; L.mipwa_combine_grad_parts.argtypes = [i32, i64, _dp, _dp, _dp, _dp, _dp, pi64]
@@ -307,6 +310,12 @@ class Mipwa:
         """launch this rank's likelihood kernel; (S, I, n_ev) stay in the CUDA tensor dev_parts (3 float64); no wait"""
         p, pp, n = self._params(params)
         self._check(self.L.mipwa_nll_parts_device(self._h, pp, n, _dev_ptr(dev_parts, 3)))
+
+    def nll_parts_static(self, params, dev_parts, blocks=0):
+        """nll_parts_device on the recompute path with the kernel's scratch in the library's static device array: no
+        device allocation in the call (include/mipwa.h); blocks > STATIC_MAX_BLOCKS is refused"""
+        p, pp, n = self._params(params)
+        self._check(self.L.mipwa_nll_parts_static(self._h, pp, n, int(blocks), _dev_ptr(dev_parts, 3)))
 
     def combine_parts_device(self, dev_parts_all, n_ranks):
         """(NLL, S, I, n_ev) of the whole sample from the gathered pieces (CUDA tensor, 3 n_ranks float64)"""

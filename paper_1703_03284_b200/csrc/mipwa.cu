@@ -2261,3 +2261,86 @@ int mipwa_generate(mipwa_ctx* c, const double* params, int64_t n_params, uint64_
 }
 
 }  // extern "C"
+
+// ---- allocation-free likelihood pieces (mipwa_nll_parts_static) --------------------------------------------------------
+// For callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses that forbid
+// cudaMalloc): k_nll_recompute needs one partial pair per block, a ticket counter and a block for its totals.  Here they
+// live in a file-scope device array instead of the context's cudaMalloc'ed buffers: MIPWA_STATIC_SCRATCH_BYTES on every
+// GPU that loads the library, until the process exits.  Layout: [0, 256) ticket, [256, 512) totals (S, I, tag),
+// [512, ..) double2 partials of up to MIPWA_STATIC_MAX_BLOCKS blocks.
+// In HOST code the array's name is a host-side stand-in, not a device address: the address is taken once per device,
+// with that device current, by cudaGetSymbolAddress, and only that pointer goes to the kernels.
+#define MIPWA_STATIC_SCRATCH_BYTES (512 + MIPWA_STATIC_MAX_BLOCKS * 16)
+#define MIPWA_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) unsigned char g_static_scratch[MIPWA_STATIC_SCRATCH_BYTES];
+
+// The array keeps what the last call (of any context) left: ticket and totals start every call at zero.  Device code names
+// the array directly.
+static __global__ void k_static_clear()
+{
+    reinterpret_cast<unsigned long long*>(g_static_scratch)[threadIdx.x] = 0ULL;   // 64 threads x 8 B = [0, 512)
+}
+
+namespace {
+unsigned char* g_static_scratch_ptr[MIPWA_STATIC_MAX_DEVICES];   // device address of g_static_scratch, per device ordinal
+
+int static_scratch(mipwa_ctx* c, unsigned char** out)           // the context's device must be current
+{
+    if (c->device < 0 || c->device >= MIPWA_STATIC_MAX_DEVICES)
+        return fail(c, MIPWA_ERR_ARG, "mipwa_nll_parts_static: device ordinal beyond " + std::to_string(MIPWA_STATIC_MAX_DEVICES - 1));
+    unsigned char* p = __atomic_load_n(&g_static_scratch_ptr[c->device], __ATOMIC_ACQUIRE);
+    if (!p) {                                              // two threads may both ask: they get the same answer
+        void* q = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&q, g_static_scratch);
+        if (e != cudaSuccess || !q)
+            return fail(c, MIPWA_ERR_CUDA, std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e));
+        p = (unsigned char*)q;
+        __atomic_store_n(&g_static_scratch_ptr[c->device], p, __ATOMIC_RELEASE);
+    }
+    *out = p;
+    return MIPWA_OK;
+}
+}  // namespace
+
+extern "C" int mipwa_nll_parts_static(mipwa_ctx* c, const double* params, int64_t n_params, int32_t blocks, double* dev_parts)
+{
+    if (!c || !params || !dev_parts) return c ? fail(c, MIPWA_ERR_ARG, "null argument") : MIPWA_ERR_ARG;
+    NvtxRange range("mipwa_nll_parts_static");
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    if (blocks < 0) return fail(c, MIPWA_ERR_ARG, "mipwa_nll_parts_static: blocks must be >= 0");
+    Slot& E = evs(c);
+    Slot& G = nms(c);
+    const int grid = blocks > 0 ? blocks : recompute_grid(c, std::max(E.n, G.n));
+    if (grid > MIPWA_STATIC_MAX_BLOCKS)
+        return fail(c, MIPWA_ERR_ARG, "mipwa_nll_parts_static: " + std::to_string(grid) + " blocks need more than the " +
+                    std::to_string(MIPWA_STATIC_SCRATCH_BYTES) + "-byte static scratch (at most " +
+                    std::to_string(MIPWA_STATIC_MAX_BLOCKS) + " blocks)");
+    // every thread loads the record at its own index before it looks at the counts: the grid must stay inside the padding
+    if ((int64_t)grid * MIPWA_REC_BLOCK > record_pad(c))
+        return fail(c, MIPWA_ERR_ARG, "mipwa_nll_parts_static: at most " + std::to_string(record_pad(c) / MIPWA_REC_BLOCK) +
+                    " blocks on this GPU (4 per SM: the padding of the record arrays)");
+    if (!E.rec || !G.rec)                                  // building them would allocate
+        return fail(c, MIPWA_ERR_STATE, "mipwa_nll_parts_static: point records not built yet; call mipwa_nll or "
+                                        "mipwa_nll_parts_device once on the recompute path after mipwa_set_* (they allocate)");
+    int rc = use_device(c);
+    if (rc) return rc;
+    unsigned char* scratch = nullptr;
+    rc = static_scratch(c, &scratch);
+    if (rc) return rc;
+    rc = build_model(c, params, n_params);
+    if (rc) return rc;
+    k_static_clear<<<1, 64, 0, c->stream>>>();
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    unsigned int* ticket = reinterpret_cast<unsigned int*>(scratch);
+    double* totals = reinterpret_cast<double*>(scratch + 256);
+    double2* partials = reinterpret_cast<double2*>(scratch + 512);
+    const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0,
+                                                      E.n, G.rec, G.n, partials, ticket, totals, ++c->tag);
+    ++c->launches;
+    CU(c, le);
+    k_pack_parts<<<1, 1, 0, c->stream>>>(totals, c->nm.w ? 1.0 : 1.0 / (double)c->nm.n, (double)c->ev.n, dev_parts);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    return MIPWA_OK;
+}
