@@ -153,9 +153,17 @@ __device__ __forceinline__ double quadratic_form(const CoefDev& cc, const double
 {
     const int K = cc.K;
     double acc[1] = { 0.0 };
+    // c_k, c_l through the generic address of the parameter block: indexed by thread, a constant-bank read would be
+    // replayed once per distinct address (dev_model.cuh: load_rows_smem)
+    const double2* cg = cc.c;
+    auto coef = [&](int k) {
+        double2 v;
+        asm volatile("ld.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(cg + k));
+        return v;
+    };
     for (int idx = threadIdx.x; idx < K * K; idx += blockDim.x) {
         const int k = idx / K, l = idx - k * K;
-        const double2 g = G[idx], a = cc.c[k], b = cc.c[l];
+        const double2 g = G[idx], a = coef(k), b = coef(l);
         const double gr = g.x * b.x - g.y * b.y, gi = g.x * b.y + g.y * b.x;     // G_kl c_l
         acc[0] += a.x * gr + a.y * gi;                                          // Re(conj(c_k) ...)
     }

@@ -81,19 +81,20 @@ struct RowsSmem {
     double2 rows[MIPWA_DEV_MAX_KNOTS * MIPWA_ROW];
 };
 
-// The model arrives in the kernel parameter (constant) bank.  A constant-bank read whose index differs between the
-// lanes of a warp is replayed once per distinct address, so the rows are copied with a warp-uniform index: every
-// lane reads entry i, lane 0 stores it (a thread-indexed copy of the tables took ~20 us per block).
+// The model arrives as a __grid_constant__ kernel parameter.  Read as a parameter (LDC from the constant bank) the copy is
+// slow either way: a thread-indexed LDC is replayed once per distinct address (~20 us per block), and a warp-uniform one
+// walks the table in dependent constant-cache misses (1.0 us at N = 40 in a 512-thread block, 3 us in a 256-thread block,
+// 10 us at N = 128: a quarter of a likelihood call at the paper's sample size).  So the table is read through the
+// GENERIC address of the parameter block with plain 16-byte loads, one entry per thread, all in flight together
+// (0.5 us whatever N is).  `m` must be the kernel's own __grid_constant__ parameter.
 __device__ __forceinline__ void load_rows_smem(RowsSmem& sm, const DevModel& m)
 {
-    const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5, lane = threadIdx.x & 31;
-    for (int i = warp; i < m.N; i += nwarp) {
-        const double2 r0 = m.rows[i * MIPWA_ROW], r1 = m.rows[i * MIPWA_ROW + 1], r2 = m.rows[i * MIPWA_ROW + 2],
-                      r3 = m.rows[i * MIPWA_ROW + 3], r4 = m.rows[i * MIPWA_ROW + 4];
-        if (lane == 0) {
-            sm.rows[i * MIPWA_ROW] = r0; sm.rows[i * MIPWA_ROW + 1] = r1; sm.rows[i * MIPWA_ROW + 2] = r2;
-            sm.rows[i * MIPWA_ROW + 3] = r3; sm.rows[i * MIPWA_ROW + 4] = r4;
-        }
+    const double2* g = m.rows;
+    const int n = m.N * MIPWA_ROW;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        double2 v;
+        asm volatile("ld.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(g + i));
+        sm.rows[i] = v;
     }
     __syncthreads();
 }

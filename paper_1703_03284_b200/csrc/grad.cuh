@@ -289,7 +289,8 @@ template <int R1, int R2> struct GradDims {
 template <int R1, int R2, int FL, bool EV, bool MIX, int SHP>
 __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m, const PointRec* __restrict__ rec,
                                           long long n, int set_block, int set_blocks, double kappa,
-                                          double2* __restrict__ fout, double* bins, double* __restrict__ mine,
+                                          double2* __restrict__ fout, double* bins, double2* stage,
+                                          double* __restrict__ mine,
                                           double (*wpart)[2 + 2 * GradDims<R1, R2>::RR + 4])
 {
     constexpr int RR = GradDims<R1, R2>::RR;
@@ -309,18 +310,34 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
 #pragma unroll
     for (int r = 0; r < RR; ++r) Fr[r] = Fi[r] = 0.0;
     if (cnt > 0) {
-        // One record per lane and iteration, loaded where it is used: the gradient's running sums leave no registers for
-        // a second record in flight (a register prefetch cost spills and constant re-reads), so the line is pulled into
-        // L2 two iterations ahead instead and the other three warps of the scheduler cover the L2 round trip.  The record
-        // arrays are padded: neither the prefetch nor the last, partly filled iteration needs a bounds test.
-        const PointRec* p = rec + lo + lane;
+        // The gradient's running sums leave no registers for a second record in flight, so the next iteration's 32 records
+        // (1 KB, contiguous) travel through shared memory: cp.async, two 16-byte units per lane, issued one iteration
+        // ahead (the scheduler's other warps run ~3 iterations meanwhile: DRAM latency is covered) and read back with two
+        // conflict-free LDS.128.  Unit u = 2 * record + half of the warp's 1 KB lands in slot half * 32 + record.  The
+        // record arrays are padded: the copy issued by the last iteration needs no bounds test.
+        double2* const st = stage + warp * 128;            // 2 stages x 64 units
+        const unsigned st0 = (unsigned)__cvta_generic_to_shared(st);
+        const unsigned dst = st0 + 16u * ((lane & 1) * 32 + (lane >> 1));
+        const char* g = reinterpret_cast<const char*>(rec + lo) + 16 * lane;
         double2* pf = fout + lo + lane;
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 32));
+        auto issue = [&](unsigned sbytes) {
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + sbytes), "l"(g) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + sbytes + 256u), "l"(g + 512) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            g += 1024;
+        };
+        issue(0u);
+        unsigned cur = 0u;                                 // stage being read, in 16-byte units (0 or 64)
         auto body = [&](auto masked, int base) {
             constexpr bool MASKED = decltype(masked)::value;
-            const PointRec r = ld_rec(p);
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 64));
-            p += 32;
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();
+            const double2 ra = st[cur + lane], rb = st[cur + 32 + lane];
+            cur ^= 64u;
+            issue(cur * 16u);
+            PointRec r;
+            r.s12 = ra.x; r.s13 = ra.y; r.w = rb.x;
+            { const unsigned long long ob = (unsigned long long)__double_as_longlong(rb.y); r.o1 = (unsigned)ob; r.o2 = (unsigned)(ob >> 32); }
             const bool valid = !MASKED || base + lane < cnt;   // lanes past the end evaluate a real point and add zeros
             double are, aim, t1, t2, tr[RR], ti[RR], sh[4];
             amplitude_parts<R1, R2, FL, SHP>(sm, m, r, are, aim, t1, t2, tr, ti, sh);
@@ -414,18 +431,19 @@ k_grad_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict_
                  double2* __restrict__ f_ev, double2* __restrict__ f_nm)
 {
     constexpr int RR = GradDims<R1, R2>::RR;
-    extern __shared__ double grad_bins[];                  // [warp][4][N-1][2]
+    extern __shared__ __align__(16) double grad_bins[];                  // [warp][4][N-1][2]
     __shared__ RowsSmem sm;
     __shared__ double wpart[MIPWA_GRAD_BLOCK / 32][2 + 2 * RR + 4];
     const int NS = m.N - 1, nb = 8 * NS, NVB = 2 + 2 * m.R + nb + 4;
     for (int k = threadIdx.x; k < (int)(blockDim.x >> 5) * nb; k += blockDim.x) grad_bins[k] = 0.0;
+    double2* const stage = reinterpret_cast<double2*>(grad_bins + (blockDim.x >> 5) * nb);   // [warp][2][64] record halves
     load_rows_smem(sm, m);                                 // ends with __syncthreads()
     double* mine = partials + (size_t)blockIdx.x * NVB;
     if ((int)blockIdx.x < ev_blocks)
-        grad_body<R1, R2, FL, true, MIX, SHP>(sm, m, ev, n_ev, (int)blockIdx.x, ev_blocks, kappa, f_ev, grad_bins, mine, wpart);
+        grad_body<R1, R2, FL, true, MIX, SHP>(sm, m, ev, n_ev, (int)blockIdx.x, ev_blocks, kappa, f_ev, grad_bins, stage, mine, wpart);
     else
         grad_body<R1, R2, FL, false, false, SHP>(sm, m, nm, n_norm, (int)blockIdx.x - ev_blocks,
-                                                 (int)gridDim.x - ev_blocks, 0.0, f_nm, grad_bins, mine, wpart);
+                                                 (int)gridDim.x - ev_blocks, 0.0, f_nm, grad_bins, stage, mine, wpart);
 }
 
 // Fixed-order sums of the per-block partial vectors, one warp per value: lane l adds blocks l, l+32, .. then a shuffle
@@ -485,7 +503,7 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
                double* __restrict__ partials)
 {
     constexpr int RC = RT > 0 ? RT : (RT == 0 ? 1 : MIPWA_GRAD_MAXR);
-    extern __shared__ double grad_bins[];                  // [warp][4][N-1][2]
+    extern __shared__ __align__(16) double grad_bins[];                  // [warp][4][N-1][2]
     __shared__ RowsSmem sm;
     __shared__ double red32[32];
     const int R = RT >= 0 ? RT : cc.K - cc.N, C = 1 + R, N = cc.N, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;

@@ -918,12 +918,16 @@ static void fill_coef(const mipwa_ctx* c, const double* p, CoefDev* cc)
 
 static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_log, double* integral)
 {
+    // both callers have built c->model from `params`; a cache or Gram (re)build overwrites it with the unit model
+    const bool rebuilt = !(c->cache_valid && c->cache_kind == kind && c->gram_valid);
     int rc = ensure_cache(c, kind);
     if (rc) return rc;
     rc = ensure_gram(c);
     if (rc) return rc;
-    rc = build_model(c, params, c->n_par());               // after the ensure_* calls: they overwrite c->model
-    if (rc) return rc;
+    if (rebuilt) {
+        rc = build_model(c, params, c->n_par());
+        if (rc) return rc;
+    }
     CoefDev cc;
     fill_coef(c, params, &cc);
     const int64_t tiles = (c->ev.n + MIPWA_TILE - 1) / MIPWA_TILE;
@@ -1512,7 +1516,8 @@ static int launch_grad_recompute(mipwa_ctx* c, bool mix, int shp, double kappa, 
     const int64_t n_ev = with_ev ? E.n : 0, n_nm = with_nm ? G.n : 0;
     const int ev_blocks = n_ev > 0 ? recompute_grid(c, n_ev) : 0, nm_blocks = n_nm > 0 ? recompute_grid(c, n_nm) : 0;
     const int grid = std::max(1, ev_blocks + nm_blocks);
-    const size_t smem = (size_t)(MIPWA_GRAD_BLOCK / 32) * nb * sizeof(double);
+    // per-warp segment bins + per-warp record staging (2 stages x 32 records x 32 B), grad.cuh: grad_body
+    const size_t smem = (size_t)(MIPWA_GRAD_BLOCK / 32) * (nb * sizeof(double) + 2 * 32 * sizeof(PointRec));
     if (smem > 200 * 1024) return fail(c, MIPWA_ERR_ARG, "mipwa_nll_grad: too many knots for the per-warp segment bins");
     if (c->grad_smem_set[mix ? 1 : 0][shp] < std::max<size_t>(smem, 1)) {
         if (mipwa_grad_set_smem(c->n_spin, c->model_flags, mix, shp, smem) != cudaSuccess)
