@@ -30,7 +30,7 @@ SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_event
            "mipwa_version", "mipwa_nll_parts_device", "mipwa_combine_parts_device", "mipwa_combine_parts",
            "mipwa_combine_grad_parts", "mipwa_norm_parts", "mipwa_nll_mix_parts", "mipwa_combine_mix_parts",
            "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble", "mipwa_nll_hessian_full",
-           "mipwa_nll_parts_static"]
+           "mipwa_nll_parts_static", "mipwa_nll_batch"]
 
 
 class MipwaError(RuntimeError):
@@ -95,6 +95,7 @@ def load_library():
     pi64 = C.POINTER(i64)
     L.mipwa_nll_parts_device.restype = i32; L.mipwa_nll_parts_device.argtypes = [vp, _dp, i64, vp]
     L.mipwa_nll_parts_static.restype = i32; L.mipwa_nll_parts_static.argtypes = [vp, _dp, i64, i32, vp]
+    L.mipwa_nll_batch.restype = i32; L.mipwa_nll_batch.argtypes = [vp, _dp, i64, i32, _dp, _dp, _dp]
     L.mipwa_combine_parts_device.restype = i32; L.mipwa_combine_parts_device.argtypes = [vp, vp, i32, _dp, _dp, _dp, pi64]
     L.mipwa_combine_parts.restype = i32; L.mipwa_combine_parts.argtypes = [i32, _dp, _dp, _dp, _dp, pi64]
     L.mipwa_combine_grad_parts.restype = i32; L.mipwa_combine_grad_parts.argtypes = [i32, i64, _dp, _dp, _dp, _dp, _dp, pi64]
@@ -232,6 +233,19 @@ class Mipwa:
         out = C.c_double()
         self._check(self.L.mipwa_nll(self._h, pp, n, C.byref(out)))
         return out.value
+
+    def nll_batch(self, params, parts=False):
+        """NLL at every row of params (n_batch x n_params), kernels pipelined, one wait; parts: also (S, I) per row"""
+        p = np.ascontiguousarray(params, dtype=np.float64)
+        if p.ndim != 2:
+            raise ValueError("params must be n_batch x n_params")
+        nb, n = p.shape
+        out = np.empty(nb)
+        sl, integ = (np.empty(nb), np.empty(nb)) if parts else (None, None)
+        self._check(self.L.mipwa_nll_batch(self._h, p.ctypes.data_as(_dp), n, nb, out.ctypes.data_as(_dp),
+                                           sl.ctypes.data_as(_dp) if parts else None,
+                                           integ.ctypes.data_as(_dp) if parts else None))
+        return (out, sl, integ) if parts else out
 
     def nll_parts(self, params):
         p, pp, n = self._params(params)

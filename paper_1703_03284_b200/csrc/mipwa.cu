@@ -86,6 +86,9 @@ struct mipwa_ctx {
     double* result_dst = nullptr;   // where the value kernels write their totals: d_result, or d_dev_result (device mode)
     double* d_dev_result = nullptr; // device memory, 8 doubles: totals of a call that stays on the device
     bool async_result = false;      // device mode (mipwa_nll_parts_device): do not wait, do not read h_result
+    double* h_batch = nullptr;      // mapped pinned, 4 doubles per slot (S, I, tag, -): totals of mipwa_nll_batch's calls
+    double* d_batch = nullptr;      // device alias of h_batch
+    int64_t batch_cap = 0;          // slots
     unsigned long long* h_bad = nullptr;
     unsigned long long* d_bad = nullptr;
 
@@ -590,6 +593,7 @@ void mipwa_destroy(mipwa_ctx* c)
     if (c->d_hyb_nm) cudaFree(c->d_hyb_nm);
     free_slot(c->ev_sorted); free_slot(c->nm_sorted);
     if (c->h_result) cudaFreeHost(c->h_result);
+    if (c->h_batch) cudaFreeHost(c->h_batch);
     if (c->h_bad) cudaFreeHost(c->h_bad);
     if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
     for (cudaEvent_t e : c->copy_done) if (e) cudaEventDestroy(e);
@@ -1080,6 +1084,70 @@ int mipwa_nll_parts(mipwa_ctx* c, const double* params, int64_t n_params, double
 int mipwa_nll(mipwa_ctx* c, const double* params, int64_t n_params, double* nll)
 {
     return mipwa_nll_parts(c, params, n_params, nll, nullptr, nullptr);
+}
+
+// n_batch likelihood values of the same sample, pipelined: every call's kernel is enqueued behind the previous one without
+// waiting, its last block writes (S, I, tag) into the call's own slot of a mapped host block, and the host waits once, for
+// the last slot (the stream runs the kernels in order).  Same kernels, same grid, same bits as n_batch mipwa_nll calls.
+int mipwa_nll_batch(mipwa_ctx* c, const double* params, int64_t n_params, int32_t n_batch, double* nll, double* sum_log,
+                    double* integral)
+{
+    if (!c || !params || !nll || n_batch < 0) return c ? fail(c, MIPWA_ERR_ARG, "bad argument") : MIPWA_ERR_ARG;
+    NvtxRange range("mipwa_nll_batch");
+    if (c->ev.n < 0 || c->nm.n < 1) return fail(c, MIPWA_ERR_STATE, "set events and normalisation points first");
+    if (n_params != c->n_par()) return fail(c, MIPWA_ERR_ARG, "n_params must be " + std::to_string(c->n_par()));
+    if (n_batch == 0) return MIPWA_OK;
+    int rc = use_device(c);
+    if (rc) return rc;
+    if (c->batch_cap < n_batch) {
+        if (c->h_batch) cudaFreeHost(c->h_batch);
+        c->h_batch = nullptr; c->d_batch = nullptr; c->batch_cap = 0;
+        const int64_t cap = std::max<int64_t>(256, n_batch);
+        CU(c, cudaHostAlloc(&c->h_batch, (size_t)cap * 4 * sizeof(double), cudaHostAllocMapped));
+        CU(c, cudaHostGetDevicePointer(&c->d_batch, c->h_batch, 0));
+        c->batch_cap = cap;
+    }
+    std::memset(c->h_batch, 0, (size_t)n_batch * 4 * sizeof(double));     // no stale tag in any slot
+    const int path = effective_path(c);
+    const bool timing = c->timing;
+    c->timing = false; c->async_result = true;
+    long long last_tag = 0;
+    int32_t launched = 0;
+    for (int32_t b = 0; b < n_batch && rc == MIPWA_OK; ++b) {
+        const double* p = params + (size_t)b * n_params;
+        rc = build_model(c, p, n_params);
+        if (rc) break;
+        double S = 0, I = 0;
+        c->result_dst = c->d_batch + 4 * (size_t)b;
+        if (path == MIPWA_PATH_RECOMPUTE) rc = nll_recompute(c, &S, &I);
+        else if (path == MIPWA_PATH_HYBRID) rc = nll_hybrid(c, p, n_params, &S, &I);
+        else rc = nll_cached(c, path, p, &S, &I);
+        if (rc == MIPWA_OK) { last_tag = c->tag; ++launched; }
+    }
+    c->timing = timing; c->async_result = false; c->result_dst = c->d_result;
+    if (launched > 0) {                                    // also after an error: nothing of this call stays in flight
+        volatile long long* flag = reinterpret_cast<volatile long long*>(c->h_batch + 4 * (size_t)(launched - 1) + MIPWA_RESULT_TAG);
+        bool seen = false;
+        for (long long spin = 0; spin < 4000000 && !seen; ++spin) {
+            seen = *flag == last_tag;
+            if (!seen && (spin & 0xffff) == 0xffff) {
+                const cudaError_t e = cudaStreamQuery(c->stream);
+                if (e == cudaSuccess) break;
+                if (e != cudaErrorNotReady) return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e));
+            }
+        }
+        if (!seen) CU(c, cudaStreamSynchronize(c->stream));
+    }
+    if (rc) return rc;
+    const bool raw = path == MIPWA_PATH_RECOMPUTE || path == MIPWA_PATH_HYBRID;   // sum |A|^2 without its 1/n when unweighted
+    for (int32_t b = 0; b < n_batch; ++b) {
+        const double S = c->h_batch[4 * (size_t)b];
+        const double I = raw && !c->nm.w ? c->h_batch[4 * (size_t)b + 1] / (double)c->nm.n : c->h_batch[4 * (size_t)b + 1];
+        nll[b] = -S + (double)c->ev.n * std::log(I);       // A7
+        if (sum_log) sum_log[b] = S;
+        if (integral) integral[b] = I;
+    }
+    return MIPWA_OK;
 }
 
 // ---- sharded likelihood without a host round trip --------------------------------------------------------

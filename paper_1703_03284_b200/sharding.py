@@ -6,8 +6,9 @@ the CPU tests).  This module only moves the pieces; the sums themselves (always 
 the same bits) and step A7 are done by the C library: mipwa_combine_parts / mipwa_combine_grad_parts /
 mipwa_combine_mix_parts on host data, mipwa_combine_parts_device on the GPU.
 
-Two routes for the value:
+Three routes for the value:
   combine_parts          the pieces come from the host (mipwa_nll_parts); gloo, or NCCL through a staging tensor
+  combine_parts_batch    B parameter vectors at once (mipwa_nll_batch): one all_gather for the whole batch
   nll_sharded_device     nothing touches the host between the likelihood kernel and the result: mipwa_nll_parts_device
                          leaves (S, I, n) in device memory, one all_gather on the same stream, mipwa_combine_parts_device
 """
@@ -51,6 +52,22 @@ def combine_parts(sum_log, integral, n_ev, group=None, device=None):
     """
     rows = _gather_rows([sum_log, integral, float(n_ev)], group, device)
     return binding.combine_parts(rows)
+
+
+def combine_parts_batch(sum_log, integral, n_ev, group=None, device=None):
+    """NLL of the whole sample at every one of B parameter vectors from one rank's pieces (mipwa_nll_batch with
+    parts: sum_log[b], integral[b]): ONE all_gather of 2 B + 1 doubles per rank, then step A7 per vector in the C library
+    (rank-ordered sums, the same bits on every rank).  Returns the B values."""
+    S = np.ascontiguousarray(sum_log, dtype=np.float64)
+    Iv = np.ascontiguousarray(integral, dtype=np.float64)
+    if S.shape != Iv.shape or S.ndim != 1:
+        raise ValueError("sum_log and integral must be vectors of the same length")
+    rows = _gather_rows(np.concatenate([S, Iv, [float(n_ev)]]), group, device)
+    B = S.size
+    out = np.empty(B)
+    for b in range(B):
+        out[b] = binding.combine_parts(np.stack([rows[:, b], rows[:, B + b], rows[:, 2 * B]], axis=1))[0]
+    return out
 
 
 def combine_grad_parts(sum_log, integral, n_ev, grad_ev, grad_nm, group=None, device=None):

@@ -37,7 +37,12 @@ def _worker(rank, world, port, q):
     glo, ghi = sharding.shard_range(g12.size, rank, world)
     _, S, Iv = o.nll(p, e12[lo:hi], e13[lo:hi], g12[glo:ghi], g13[glo:ghi], w[glo:ghi], parts=True)
     nll, St, It, nt = sharding.combine_parts(S, Iv, hi - lo)
-    q.put((rank, nll, St, It, nt, full))
+    # the batched form (mipwa_nll_batch pieces): three parameter vectors, ONE all_gather
+    ps = [p, c.perturbed(2), c.perturbed(3)]
+    pieces = [o.nll(v, e12[lo:hi], e13[lo:hi], g12[glo:ghi], g13[glo:ghi], w[glo:ghi], parts=True) for v in ps]
+    batch = sharding.combine_parts_batch([v[1] for v in pieces], [v[2] for v in pieces], hi - lo)
+    batch_ref = [o.nll(v, e12, e13, g12, g13, w) for v in ps]
+    q.put((rank, nll, St, It, nt, full, list(batch), batch_ref))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -56,17 +61,25 @@ def test_two_rank_combine_matches_single_process():
         p.join(timeout=60)
         assert p.exitcode == 0
     nlls = set()
-    for rank, nll, St, It, nt, (full, fS, fI) in out:
+    batches = set()
+    for rank, nll, St, It, nt, (full, fS, fI), batch, batch_ref in out:
         assert nt == 4001
         assert abs(St - fS) <= 1e-11 * abs(fS) and abs(It - fI) <= 1e-12 * abs(fI)
         assert abs(nll - full) <= 1e-10 * max(abs(full), abs(fS) + nt * abs(np.log(fI)))
         nlls.add(nll)
+        assert batch[0] == nll                         # vector 0 of the batch is the single call
+        for got, ref in zip(batch, batch_ref):
+            assert abs(got - ref) <= 1e-10 * max(abs(ref), abs(fS) + nt * abs(np.log(fI)))
+        batches.add(tuple(batch))
     assert len(nlls) == 1                              # every rank forms the same bits (rank-ordered sum)
+    assert len(batches) == 1
 
 
 def test_combine_without_process_group_is_step_a7():
     nll, S, Iv, n = sharding.combine_parts(12.5, 3.0, 7)
     assert (S, Iv, n) == (12.5, 3.0, 7) and nll == -12.5 + 7 * np.log(3.0)
+    batch = sharding.combine_parts_batch([12.5, -4.0], [3.0, 0.5], 7)
+    assert list(batch) == [-12.5 + 7 * np.log(3.0), 4.0 + 7 * np.log(0.5)]
 
 
 def _grad_worker(rank, world, port, q):
