@@ -256,6 +256,15 @@ def latency_leg(B, torch, stream, local):
             wall, _ = wall_of(call, ps, 300)
             k, _ = kernel_ms_of(m, call, ps, 20)
             row[name] = {"wall_us": wall * 1e6, "kernel_us": k * 1e3}
+        pm = np.array(ps)
+        for name, path in (("nll_batch_recompute", B.PATH_RECOMPUTE), ("nll_batch_auto", B.PATH_AUTO)):
+            m.set_path(path)
+            m.nll_batch(pm)
+            t0 = time.perf_counter()
+            for _ in range(20):
+                vals = m.nll_batch(pm)
+            row[name] = {"wall_us_per_evaluation": (time.perf_counter() - t0) / (20 * len(ps)) * 1e6, "batch": len(ps),
+                         "same_bits_as_blocking": bool(vals[3] == m.nll(ps[3]))}
         out.append(row)
         m.close()
     return out
