@@ -43,6 +43,11 @@ def test_full_size_nll_and_sampled_abs2(full):
     m.prepare()                                             # cell-sorted copies, as bench.py runs it
     got2 = m.nll(p)
     assert abs(got2 - ref) <= tol and m.nll(p) == got2
+    # the call bench.py times: the evaluations enqueued back to back (same launch shape, hence the same bits)
+    ps = np.array([p, c.perturbed(5), p])
+    b_nll, b_sl, b_integ = m.nll_batch(ps, parts=True)
+    assert b_nll[0] == got2 and b_nll[2] == got2 and b_nll[1] == m.nll(ps[1])
+    assert abs(b_sl[0] - sl) <= tol and b_integ[0] == pytest.approx(integ, rel=1e-12)
     a2 = m.eval_abs2(p, 0)
     idx = np.arange(0, a2.size, 997)
     refa = o.abs2(p, data[0][idx], data[1][idx])
