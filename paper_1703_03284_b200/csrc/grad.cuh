@@ -531,6 +531,14 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
         const double2 s = ld_stream(p);
         const unsigned int sg = seg[ii], o1 = seg_off1(sg), o2 = seg_off2(sg);
         double2 b[RC];
+        {   // the next iteration's lines on their way into L2 (the running sums leave no registers for a second set of
+            // columns in flight: with a register prefetch ptxas spilled and the kernel lost 9 %)
+            const long long nx = i + 32 < hi ? i + 32 : lo;
+            const double2* q = cache + (size_t)(nx / MIPWA_TILE) * C * MIPWA_TILE + (nx % MIPWA_TILE);
+#pragma unroll
+            for (int r = 0; r < (RT >= 0 ? 1 + RT : 1); ++r)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(q + (size_t)r * MIPWA_TILE));
+        }
         if (RT >= 0) {
 #pragma unroll
             for (int r = 0; r < RT; ++r) b[r] = ld_stream(p + (size_t)(1 + r) * MIPWA_TILE);
