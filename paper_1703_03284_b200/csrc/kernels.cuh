@@ -137,6 +137,11 @@ k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__
     __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
+    // Launched with programmatic stream serialisation (mipwa_nll_batch: the same kernel enqueued back to back) the next
+    // launch's blocks may be scheduled as this one's leave their SMs, before the last block's epilogue is over; they read
+    // only the point records and their own parameter block until griddepcontrol.wait below.  Both instructions do nothing
+    // in an ordinary launch.
+    asm volatile("griddepcontrol.launch_dependents;");
     const unsigned int stride = gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const PointRec* p = ev + t0;
@@ -197,6 +202,7 @@ k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__
     }
     double v[2] = { lp.sum, integ };
     block_reduce<2>(v, red);
+    asm volatile("griddepcontrol.wait;" ::: "memory");     // the previous launch has left the partials and the ticket
     if (threadIdx.x == 0) {
         partials[blockIdx.x] = make_double2(v[0], v[1]);
         __threadfence();

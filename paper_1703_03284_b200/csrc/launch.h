@@ -15,6 +15,10 @@ cudaError_t mipwa_launch_nll_recompute(const int* n_spin, int fl, bool mix, int 
                                        const PointRec* ev, double kappa, long long n_ev, const PointRec* nm,
                                        long long n_norm, double2* partials, unsigned int* ticket, double* result,
                                        long long tag);
+// the same (no mixture) as a launch that may overlap the end of the previous launch on the stream (tu_recompute.cu)
+cudaError_t mipwa_launch_nll_recompute_overlapped(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
+                                                  const PointRec* ev, long long n_ev, const PointRec* nm, long long n_norm,
+                                                  double2* partials, unsigned int* ticket, double* result, long long tag);
 cudaError_t mipwa_launch_nll_recompute_mix(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
                                            const PointRec* ev, double kappa, long long n_ev, const PointRec* nm,
                                            long long n_norm, double2* partials, unsigned int* ticket, double* result,

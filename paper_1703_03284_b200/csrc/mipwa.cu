@@ -89,6 +89,7 @@ struct mipwa_ctx {
     double* h_batch = nullptr;      // mapped pinned, 4 doubles per slot (S, I, tag, -): totals of mipwa_nll_batch's calls
     double* d_batch = nullptr;      // device alias of h_batch
     int64_t batch_cap = 0;          // slots
+    bool overlap_launch = false;    // mipwa_nll_batch, vectors 1..: the value kernel may start while its predecessor drains
     unsigned long long* h_bad = nullptr;
     unsigned long long* d_bad = nullptr;
 
@@ -767,8 +768,11 @@ static int nll_recompute(mipwa_ctx* c, double* sum_log, double* integral)
     const int grid = recompute_grid(c, std::max(E.n, G.n));
     { const int trc = timing_begin(c); if (trc) return trc; }
     const long long tag = next_tag(c);
-    const cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0,
-                                                      E.n, G.rec, G.n, c->d_partials, c->d_ticket, c->result_dst, tag);
+    const cudaError_t le = c->overlap_launch
+        ? mipwa_launch_nll_recompute_overlapped(c->n_spin, c->model_flags, grid, c->stream, c->model, E.rec, E.n, G.rec, G.n,
+                                                c->d_partials, c->d_ticket, c->result_dst, tag)
+        : mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0,
+                                     E.n, G.rec, G.n, c->d_partials, c->d_ticket, c->result_dst, tag);
     ++c->launches;
     CU(c, le);
     rc = wait_result(c, tag);
@@ -1119,12 +1123,13 @@ int mipwa_nll_batch(mipwa_ctx* c, const double* params, int64_t n_params, int32_
         if (rc) break;
         double S = 0, I = 0;
         c->result_dst = c->d_batch + 4 * (size_t)b;
+        c->overlap_launch = b > 0;                         // its predecessor on the stream is the same kernel on the same records
         if (path == MIPWA_PATH_RECOMPUTE) rc = nll_recompute(c, &S, &I);
         else if (path == MIPWA_PATH_HYBRID) rc = nll_hybrid(c, p, n_params, &S, &I);
         else rc = nll_cached(c, path, p, &S, &I);
         if (rc == MIPWA_OK) { last_tag = c->tag; ++launched; }
     }
-    c->timing = timing; c->async_result = false; c->result_dst = c->d_result;
+    c->timing = timing; c->async_result = false; c->result_dst = c->d_result; c->overlap_launch = false;
     if (launched > 0) {                                    // also after an error: nothing of this call stays in flight
         volatile long long* flag = reinterpret_cast<volatile long long*>(c->h_batch + 4 * (size_t)(launched - 1) + MIPWA_RESULT_TAG);
         bool seen = false;
