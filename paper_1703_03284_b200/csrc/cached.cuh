@@ -126,6 +126,7 @@ __device__ __forceinline__ bool grid_reduce(double (&v)[NV], double* __restrict_
                                             unsigned int* __restrict__ ticket, double* red, bool* flag)
 {
     block_reduce<NV>(v, red);
+    asm volatile("griddepcontrol.wait;" ::: "memory");     // an overlapped launch (k_nll_compact): the previous one is done with these
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int k = 0; k < NV; ++k) partials[(size_t)blockIdx.x * NV + k] = v[k];
@@ -355,6 +356,7 @@ k_nll_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefDe
     __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
+    asm volatile("griddepcontrol.launch_dependents;");     // mipwa_nll_batch: as k_nll_recompute (kernels.cuh); otherwise nothing
     load_rows_smem(sm, m);
     const int R = RT >= 0 ? RT : cc.K - cc.N, C = 1 + R, N = cc.N;
     const long long n_tiles = (n_ev + MIPWA_TILE - 1) / MIPWA_TILE;

@@ -964,9 +964,20 @@ static int nll_cached(mipwa_ctx* c, int kind, const double* params, double* sum_
             if (c->compact_blocks_per_sm < 1) c->compact_blocks_per_sm = 1;
         }
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)c->sm_count * c->compact_blocks_per_sm));
+        // overlap_launch (mipwa_nll_batch, vectors 1..): programmatic stream serialisation, as for k_nll_recompute
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(MIPWA_TILE); cfg.stream = c->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = c->overlap_launch ? 1 : 0;
+        const unsigned short* segp = evs(c).seg;
+        const long long n_ev_ll = c->ev.n;
+        const double2* gram = c->d_gram;
+        double* parts = (double*)c->d_partials;
 #define MIPWA_COMPACT_LAUNCH(T)                                                                                   \
-    k_nll_compact<T><<<grid, MIPWA_TILE, 0, c->stream>>>(c->model, cc, cache, evs(c).seg, c->ev.n, c->d_gram,    \
-                                                          (double*)c->d_partials, c->d_ticket, c->result_dst, tag)
+    (void)cudaLaunchKernelEx(&cfg, k_nll_compact<T>, c->model, cc, cache, segp, n_ev_ll, gram, parts, c->d_ticket, \
+                             c->result_dst, tag)
         switch (c->R) {
             case 0: MIPWA_COMPACT_LAUNCH(0); break;
             case 1: MIPWA_COMPACT_LAUNCH(1); break;
