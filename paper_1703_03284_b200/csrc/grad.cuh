@@ -435,6 +435,7 @@ k_grad_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict_
     __shared__ RowsSmem sm;
     __shared__ double wpart[MIPWA_GRAD_BLOCK / 32][2 + 2 * RR + 4];
     const int NS = m.N - 1, nb = 8 * NS, NVB = 2 + 2 * m.R + nb + 4;
+    asm volatile("griddepcontrol.launch_dependents;");     // k_grad_finalize may be scheduled behind this grid's blocks
     for (int k = threadIdx.x; k < (int)(blockDim.x >> 5) * nb; k += blockDim.x) grad_bins[k] = 0.0;
     double2* const stage = reinterpret_cast<double2*>(grad_bins + (blockDim.x >> 5) * nb);   // [warp][2][64] record halves
     load_rows_smem(sm, m);                                 // ends with __syncthreads()
@@ -453,6 +454,9 @@ static __global__ void __launch_bounds__(256)
 k_grad_finalize(const double* __restrict__ partials, int split, int nblocks, int NV, int sets,
                 double* __restrict__ result)
 {
+    // launched with programmatic stream serialisation right behind the kernel that writes `partials`: its blocks may be
+    // resident before that kernel has finished; nothing is read before this point
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int kk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (kk >= sets * NV) return;
     const int set = kk / NV, k = kk - set * NV;
@@ -508,6 +512,7 @@ k_grad_compact(const __grid_constant__ DevModel m, const __grid_constant__ CoefD
     __shared__ double red32[32];
     const int R = RT >= 0 ? RT : cc.K - cc.N, C = 1 + R, N = cc.N, NS = N - 1, nb = 8 * NS, NV = 1 + 2 * R + nb;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+    asm volatile("griddepcontrol.launch_dependents;");     // k_grad_finalize may be scheduled behind this grid's blocks
     for (int k = threadIdx.x; k < wpb * nb; k += blockDim.x) grad_bins[k] = 0.0;
     load_rows_smem(sm, m);
     double* const wbins = grad_bins + warp * nb;

@@ -392,6 +392,20 @@ static long long next_tag(mipwa_ctx* c)
     return ++c->tag;
 }
 
+// k_grad_finalize right behind the kernel that writes the block partials, launched with programmatic stream serialisation:
+// its launch latency runs under the producer's tail (the kernel itself waits in griddepcontrol.wait, grad.cuh)
+static cudaError_t launch_finalize(mipwa_ctx* c, int blocks, const double* partials, int split, int nblocks, int NV, int sets,
+                                   double* result)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3(256); cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_grad_finalize, partials, split, nblocks, NV, sets, result);
+}
+
 // start of the timed region of a call (timing mode only): spacer kernel, then the first event (kernels.cuh: k_spacer)
 static int timing_begin(mipwa_ctx* c)
 {
@@ -1528,7 +1542,7 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
 #undef MIPWA_GC_LAUNCH
     ++c->launches;
     CU(c, cudaGetLastError());
-    k_grad_finalize<<<(NV + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, grid, NV, 1, c->d_result);
+    (void)launch_finalize(c, (NV + 7) / 8, c->d_gpartials, grid, grid, NV, 1, c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());
     if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
@@ -1619,8 +1633,7 @@ static int launch_grad_recompute(mipwa_ctx* c, bool mix, int shp, double kappa, 
                                                        want_f ? c->d_f_ev : nullptr, want_f ? c->d_f_nm : nullptr);
     ++c->launches;
     CU(c, le);
-    k_grad_finalize<<<(2 * NVB + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, ev_blocks, ev_blocks + nm_blocks, NVB, 2,
-                                                              c->d_result);
+    (void)launch_finalize(c, (2 * NVB + 7) / 8, c->d_gpartials, ev_blocks, ev_blocks + nm_blocks, NVB, 2, c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());
     out->NVB = NVB; out->nb = nb;
