@@ -328,8 +328,8 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
         };
         issue(0u);
         unsigned cur = 0u;                                 // stage being read, in 16-byte units (0 or 64)
-        auto body = [&](auto masked, int base) {
-            constexpr bool MASKED = decltype(masked)::value;
+        // the record of the iteration after the one last returned (the copy of the one after that is issued behind it)
+        auto next_record = [&]() {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncwarp();
             const double2 ra = st[cur + lane], rb = st[cur + 32 + lane];
@@ -337,26 +337,30 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
             issue(cur * 16u);
             PointRec r;
             r.s12 = ra.x; r.s13 = ra.y; r.w = rb.x;
-            { const unsigned long long ob = (unsigned long long)__double_as_longlong(rb.y); r.o1 = (unsigned)ob; r.o2 = (unsigned)(ob >> 32); }
-            const bool valid = !MASKED || base + lane < cnt;   // lanes past the end evaluate a real point and add zeros
-            double are, aim, t1, t2, tr[RR], ti[RR], sh[4];
+            const unsigned long long ob = (unsigned long long)__double_as_longlong(rb.y);
+            r.o1 = (unsigned)ob; r.o2 = (unsigned)(ob >> 32);
+            return r;
+        };
+        // one point: amplitude, f, the scalar sums and the resonance sums - everything but the spline moments
+        auto point = [&](auto masked, const PointRec& r, bool valid, double& fr, double& fi, double& t1, double& t2) {
+            constexpr bool MASKED = decltype(masked)::value;   // lanes past the end evaluate a real point and add zeros
+            double are, aim, tr[RR], ti[RR], sh[4];
             amplitude_parts<R1, R2, FL, SHP>(sm, m, r, are, aim, t1, t2, tr, ti, sh);
             const double a2 = fma(are, are, aim * aim);
-            double fr, fi;
             if (EV) {
                 const double D = MIX ? fma(kappa, r.w, a2) : a2;
                 const double rD = fast_rcp(D);
-                const double k = valid ? -2.0 * rD : 0.0;
+                const double k = !MASKED || valid ? -2.0 * rD : 0.0;
                 fr = k * are; fi = k * aim;
-                lp.add(valid ? D : 1.0);
-                if (MIX) qsum += valid ? r.w * rD : 0.0;
+                lp.add(!MASKED || valid ? D : 1.0);
+                if (MIX) qsum += !MASKED || valid ? r.w * rD : 0.0;
             } else {
-                const double wv = valid ? r.w : 0.0;
+                const double wv = !MASKED || valid ? r.w : 0.0;
                 fr = wv * are; fi = wv * aim;
                 integ = fma(wv, a2, integ);
             }
             if (fout) {                                    // for k_grad_shape (several floating resonances)
-                if (valid) *pf = make_double2(fr, fi);
+                if (!MASKED || valid) *pf = make_double2(fr, fi);
                 pf += 32;
             }
             if (R1 >= 0) {
@@ -377,19 +381,34 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
                 Sh[2] = fma(fr, sh[2], fma(fi, sh[3], Sh[2]));             // f conj(dT'/dG0)
                 Sh[3] = fma(fi, sh[2], fma(-fr, sh[3], Sh[3]));
             }
-            cell_accumulate(acc, valid, r.o1, r.o2, fr, fi, t1, t2, wbins, NS);
         };
+        // Two loops.  The HOT one takes the iterations whose 32 points all lie in the warp's current cell (cell-sorted
+        // points: all but a few per warp): straight-line code, moments into the register accumulators.  Whatever else -
+        // the first iteration, a cell change, an iteration that straddles cells, the partly filled last one - leaves it
+        // and is handled once by the general code below (flush into the warp's bins, shuffles, masks), which then hands
+        // back.  With the flush inside the one loop ptxas re-read 19 model constants per point and spilled.
         const int full = cnt & ~31;                        // iterations in which every lane has a point
-        int base = 0;
-        while (base < full) {
-            const int stop = full - base < 32 * LOGPROD_FLUSH ? full : base + 32 * LOGPROD_FLUSH;
-            const int adds = (stop - base) >> 5;
-            for (; base < stop; base += 32) body(std::false_type(), base);   // warp-uniform trip count
-            if (EV) lp.flush(adds);
-        }
-        if (full < cnt) {                                  // the last warp of the set: one partly filled iteration
-            body(std::true_type(), full);
-            if (EV) lp.flush(1);
+        int base = 0, adds = 0;
+        PointRec r = next_record();
+        while (base < cnt) {
+            const int room = LOGPROD_FLUSH - adds;         // iterations until the log-product has to be flushed
+            const int stop = (full - base) >> 5 < room ? full : base + 32 * room;
+            while (base < stop && __all_sync(0xffffffffu, r.o1 == acc.o1 && r.o2 == acc.o2)) {
+                double fr, fi, t1, t2;
+                point(std::false_type(), r, true, fr, fi, t1, t2);
+                acc.add(fr, fi, t1, t2);
+                base += 32; ++adds;
+                r = next_record();
+            }
+            if (base < stop || (base == full && full < cnt)) {
+                const bool valid = base + lane < cnt;
+                double fr, fi, t1, t2;
+                point(std::true_type(), r, valid, fr, fi, t1, t2);
+                cell_accumulate(acc, valid, r.o1, r.o2, fr, fi, t1, t2, wbins, NS);
+                base += 32; ++adds;
+                r = next_record();
+            }
+            if (EV && (adds == LOGPROD_FLUSH || base >= cnt)) { lp.flush(adds); adds = 0; }
         }
     }
     flush_warp(acc, wbins, NS);
