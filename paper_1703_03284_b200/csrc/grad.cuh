@@ -319,7 +319,6 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
         const unsigned st0 = (unsigned)__cvta_generic_to_shared(st);
         const unsigned dst = st0 + 16u * ((lane & 1) * 32 + (lane >> 1));
         const char* g = reinterpret_cast<const char*>(rec + lo) + 16 * lane;
-        double2* pf = fout + lo + lane;
         auto issue = [&](unsigned sbytes) {
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + sbytes), "l"(g) : "memory");
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + sbytes + 256u), "l"(g + 512) : "memory");
@@ -328,6 +327,7 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
         };
         issue(0u);
         unsigned cur = 0u;                                 // stage being read, in 16-byte units (0 or 64)
+        int base = 0, adds = 0;                            // offset of the current iteration in the chunk; adds since the last flush
         // the record of the iteration after the one last returned (the copy of the one after that is issued behind it)
         auto next_record = [&]() {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -359,10 +359,8 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
                 fr = wv * are; fi = wv * aim;
                 integ = fma(wv, a2, integ);
             }
-            if (fout) {                                    // for k_grad_shape (several floating resonances)
-                if (!MASKED || valid) *pf = make_double2(fr, fi);
-                pf += 32;
-            }
+            if (fout && (!MASKED || valid))                // for k_grad_shape (several floating resonances)
+                fout[lo + base + lane] = make_double2(fr, fi);
             if (R1 >= 0) {
 #pragma unroll
                 for (int q = 0; q < (R1 >= 0 ? R1 + R2 : 0); ++q) {
@@ -388,7 +386,6 @@ __device__ __forceinline__ void grad_body(const RowsSmem& sm, const DevModel& m,
         // and is handled once by the general code below (flush into the warp's bins, shuffles, masks), which then hands
         // back.  With the flush inside the one loop ptxas re-read 19 model constants per point and spilled.
         const int full = cnt & ~31;                        // iterations in which every lane has a point
-        int base = 0, adds = 0;
         PointRec r = next_record();
         while (base < cnt) {
             const int room = LOGPROD_FLUSH - adds;         // iterations until the log-product has to be flushed
