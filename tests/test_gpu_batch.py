@@ -62,3 +62,34 @@ def test_batch_sizes_unweighted_points_and_errors():
         m.nll_batch(ps[:, :-1])
     assert m.nll(ps[0]) == got[0]                          # the context is usable after a failed batch
     m.close()
+
+
+@pytest.mark.parametrize("idx,n_ev,n_norm", [(1, 300, 500), (3, 700, 900), (2, 1, 40)])
+def test_overlapped_launches_of_tiny_kernels(idx, n_ev, n_norm):
+    """From the second vector on, the kernels of a batch are launched with programmatic stream serialisation: a kernel's
+    blocks may be resident while its predecessor is still in its epilogue and wait (griddepcontrol.wait) before they touch the
+    shared partials.  Samples of one or two blocks make every kernel catch up with its predecessor; random batch sizes,
+    gradient and blocking calls in between.  Every value must keep the bits of the blocking call."""
+    B = _lib()
+    c, _, data = make_case(idx, n_ev=n_ev, n_norm=n_norm)
+    m = B.Mipwa(c.kin, c.knots, c.resonances)
+    m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], data[4])
+    m.prepare()                                            # the order every later call uses (mipwa_nll_grad implies it)
+    fixed = not any(r.get("shape_floats") for r in c.resonances)
+    paths = [B.PATH_RECOMPUTE] + ([B.PATH_CACHED_COMPACT] if fixed else [])
+    ps = np.array([c.perturbed(t) for t in range(32)])
+    ref = {}
+    for path in paths:
+        m.set_path(path)
+        ref[path] = np.array([m.nll(p) for p in ps])
+    rng = np.random.default_rng(idx)
+    for it in range(60):
+        path = paths[rng.integers(len(paths))]
+        m.set_path(path)
+        sel = rng.integers(0, 32, size=int(rng.integers(1, 300)))
+        assert np.array_equal(m.nll_batch(ps[sel]), ref[path][sel]), (it, path, sel.size)
+        if it % 7 == 0:
+            m.nll_grad(ps[it % 32])
+        if it % 11 == 0:
+            assert m.nll(ps[3]) == ref[path][3]
+    m.close()
