@@ -84,6 +84,7 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
     __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
     __shared__ bool is_last;
+    asm volatile("griddepcontrol.launch_dependents;");     // mipwa_nll_batch: as k_nll_recompute (kernels.cuh); otherwise nothing
     load_rows_smem(sm, m);
     constexpr int C = 1 + RCT, ST = MIPWA_HYB_STAGES(RCT), AHEAD = ST - 1, PTS = MIPWA_HYB_PTS(RCT);
     constexpr int TPB = MIPWA_HYB_BLOCK / MIPWA_TILE;                                  // tiles per block and point slot
@@ -171,6 +172,7 @@ k_nll_hybrid(const __grid_constant__ DevModel m, const __grid_constant__ HybCoef
     }
     double v[2] = { lp.value(), integ };
     block_reduce<2>(v, red);
+    asm volatile("griddepcontrol.wait;" ::: "memory");     // the previous launch has left the partials and the ticket
     if (threadIdx.x == 0) {
         partials[blockIdx.x] = make_double2(v[0], v[1]);
         __threadfence();

@@ -51,4 +51,4 @@ cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cu
                                     const HybCoef& cc, const double2* ev_cache, const unsigned short* eseg,
                                     long long n_ev, const double2* nm_cache, const double* gw,
                                     const unsigned short* gseg, long long n_norm, double2* partials,
-                                    unsigned int* ticket, double* result, long long tag);
+                                    unsigned int* ticket, double* result, long long tag, bool overlapped = false);

@@ -1079,7 +1079,7 @@ static int nll_hybrid(mipwa_ctx* c, const double* params, int64_t n_params, doub
     const cudaError_t le = mipwa_launch_nll_hybrid(c->hyb_f1, c->hyb_f2, RC, c->model_flags, grid, c->stream, c->model, cc,
                                                    (const double2*)c->d_hyb_ev, evs(c).seg, c->ev.n,
                                                    (const double2*)c->d_hyb_nm, nms(c).w, nms(c).seg, c->nm.n,
-                                                   c->d_partials, c->d_ticket, c->result_dst, tag);
+                                                   c->d_partials, c->d_ticket, c->result_dst, tag, c->overlap_launch);
     ++c->launches;
     CU(c, le);
     rc = wait_result(c, tag);

@@ -29,11 +29,21 @@ cudaError_t mipwa_launch_nll_hybrid(int f1, int f2, int rc, int fl, int grid, cu
                                     const HybCoef& cc, const double2* ev_cache, const unsigned short* eseg,
                                     long long n_ev, const double2* nm_cache, const double* gw,
                                     const unsigned short* gseg, long long n_norm, double2* partials,
-                                    unsigned int* ticket, double* result, long long tag)
+                                    unsigned int* ticket, double* result, long long tag, bool overlapped)
 {
     bool supported = true;
+    // overlapped (mipwa_nll_batch, vectors 1..): programmatic stream serialisation, as for k_nll_recompute (kernels.cuh)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(MIPWA_HYB_BLOCK); cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = overlapped ? 1 : 0;
+    cudaError_t e = cudaSuccess;
     MIPWA_DISPATCH_HYBFL(f1, f2, rc, fl,
-                         (k_nll_hybrid<R1, R2, RCT, FL><<<grid, MIPWA_HYB_BLOCK, mipwa_hyb_ring_bytes(RCT), st>>>(
-                             m, cc, ev_cache, eseg, n_ev, nm_cache, gw, gseg, n_norm, partials, ticket, result, tag)));
-    return supported ? cudaGetLastError() : cudaErrorInvalidValue;
+                         (cfg.dynamicSmemBytes = mipwa_hyb_ring_bytes(RCT),
+                          e = cudaLaunchKernelEx(&cfg, k_nll_hybrid<R1, R2, RCT, FL>, m, cc, ev_cache, eseg, n_ev, nm_cache, gw,
+                                                 gseg, n_norm, partials, ticket, result, tag)));
+    if (!supported) return cudaErrorInvalidValue;
+    return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -76,7 +76,7 @@ def test_overlapped_launches_of_tiny_kernels(idx, n_ev, n_norm):
     m.set_events(data[0], data[1]); m.set_norm_points(data[2], data[3], data[4])
     m.prepare()                                            # the order every later call uses (mipwa_nll_grad implies it)
     fixed = not any(r.get("shape_floats") for r in c.resonances)
-    paths = [B.PATH_RECOMPUTE] + ([B.PATH_CACHED_COMPACT] if fixed else [])
+    paths = [B.PATH_RECOMPUTE] + ([B.PATH_CACHED_COMPACT] if fixed else [B.PATH_AUTO])      # AUTO: the hybrid kernel
     ps = np.array([c.perturbed(t) for t in range(32)])
     ref = {}
     for path in paths:
