@@ -572,6 +572,12 @@ def run_ours(args, cfg, workload):
                 "peak_3reg": peak_3reg, "nominal_peak": nominal, "flops_per_point": fpp,
                 "flops_per_point_source": "SURVEY 8(d) count of the plain formulas: 59 + 82 R, one per add/mul/div/sqrt/log, fma = 2",
                 "points_per_launch": n_ev + n_norm, "kernel_ms": k_ms, "kernel_ms_min": k_ms_min,
+                "kernel_ms_what": "one launch timed ALONE between two events behind a spacer kernel (prologue and epilogue "
+                                  "included): what achieved / frac use",
+                "timed_region": {"ms_per_launch": ms_step, "achieved": fpp * (n_ev + n_norm) / (ms_step * 1e-3) * 1e-12,
+                                 "frac": fpp * (n_ev + n_norm) / (ms_step * 1e-3) * 1e-12 / peak,
+                                 "what": "the same per launch of the timed region, where consecutive launches overlap "
+                                         "prologue and epilogue (programmatic stream serialisation)"},
                 "algorithmic_bytes": 32.0 * (n_ev + n_norm),
                 "hbm_gbs": 32.0 * (n_ev + n_norm) / (k_ms * 1e-3) * 1e-9}
 

@@ -202,6 +202,9 @@ int mipwa_nll_parts_device(mipwa_ctx* ctx, const double* params, int64_t n_param
 int mipwa_combine_parts_device(mipwa_ctx* ctx, const double* dev_parts_all, int32_t n_ranks, double* nll, double* sum_log,
                                double* integral, int64_t* n_ev);
 int mipwa_combine_parts(int32_t n_ranks, const double* parts, double* nll, double* sum_log, double* integral, int64_t* n_ev);
+/* the same for a batch (mipwa_nll_batch with its pieces): parts[r] = (S_r[0..n_batch), I_r[0..n_batch), n_r), 2 n_batch + 1
+ * doubles per rank; nll: n_batch doubles.  Same sums, same bits per vector as mipwa_combine_parts. */
+int mipwa_combine_parts_batch(int32_t n_ranks, int32_t n_batch, const double* parts, double* nll);
 int mipwa_combine_grad_parts(int32_t n_ranks, int64_t n_params, const double* parts, double* nll, double* grad,
                              double* sum_log, double* integral, int64_t* n_ev);
 

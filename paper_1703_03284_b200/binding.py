@@ -30,7 +30,7 @@ SYMBOLS = ["mipwa_create", "mipwa_destroy", "mipwa_set_stream", "mipwa_set_event
            "mipwa_version", "mipwa_nll_parts_device", "mipwa_combine_parts_device", "mipwa_combine_parts",
            "mipwa_combine_grad_parts", "mipwa_norm_parts", "mipwa_nll_mix_parts", "mipwa_combine_mix_parts",
            "mipwa_hessian_parts_len", "mipwa_hessian_parts", "mipwa_hessian_assemble", "mipwa_nll_hessian_full",
-           "mipwa_nll_parts_static", "mipwa_nll_batch"]
+           "mipwa_nll_parts_static", "mipwa_nll_batch", "mipwa_combine_parts_batch"]
 
 
 class MipwaError(RuntimeError):
@@ -95,6 +95,7 @@ def load_library():
     pi64 = C.POINTER(i64)
     L.mipwa_nll_parts_device.restype = i32; L.mipwa_nll_parts_device.argtypes = [vp, _dp, i64, vp]
     L.mipwa_nll_parts_static.restype = i32; L.mipwa_nll_parts_static.argtypes = [vp, _dp, i64, i32, vp]
+    L.mipwa_combine_parts_batch.restype = i32; L.mipwa_combine_parts_batch.argtypes = [i32, i32, _dp, _dp]
     L.mipwa_nll_batch.restype = i32; L.mipwa_nll_batch.argtypes = [vp, _dp, i64, i32, _dp, _dp, _dp]
     L.mipwa_combine_parts_device.restype = i32; L.mipwa_combine_parts_device.argtypes = [vp, vp, i32, _dp, _dp, _dp, pi64]
     L.mipwa_combine_parts.restype = i32; L.mipwa_combine_parts.argtypes = [i32, _dp, _dp, _dp, _dp, pi64]
@@ -436,6 +437,17 @@ def combine_parts(parts):
     if rc != OK:
         raise MipwaError(rc, "mipwa_combine_parts failed")
     return out.value, S.value, Iv.value, nn.value
+
+
+def combine_parts_batch(parts, n_batch):
+    """A7 at every vector of a batch over gathered rows (S_r[0..B), I_r[0..B), n_r), rank order (C library): B values"""
+    L = load_library()
+    a = np.ascontiguousarray(parts, dtype=np.float64).reshape(-1, 2 * n_batch + 1)
+    out = np.empty(n_batch)
+    rc = L.mipwa_combine_parts_batch(a.shape[0], int(n_batch), a.ctypes.data_as(_dp), out.ctypes.data_as(_dp))
+    if rc != OK:
+        raise MipwaError(rc, "mipwa_combine_parts_batch failed")
+    return out
 
 
 def combine_grad_parts(parts, n_params):

@@ -1245,6 +1245,20 @@ int mipwa_combine_parts(int32_t n_ranks, const double* parts, double* nll, doubl
     return MIPWA_OK;
 }
 
+// A7 at every vector of a batch from gathered rows parts[r] = (S_r[0..B), I_r[0..B), n_r): the same rank-ordered sums as
+// mipwa_combine_parts, hence the same bits per vector
+int mipwa_combine_parts_batch(int32_t n_ranks, int32_t n_batch, const double* parts, double* nll)
+{
+    if (n_ranks < 1 || n_batch < 0 || !parts || (!nll && n_batch > 0)) return MIPWA_ERR_ARG;
+    const size_t row = 2 * (size_t)n_batch + 1;
+    for (int32_t b = 0; b < n_batch; ++b) {
+        double S = 0.0, I = 0.0, n = 0.0;
+        for (int r = 0; r < n_ranks; ++r) { S += parts[r * row + b]; I += parts[r * row + n_batch + b]; n += parts[r * row + 2 * (size_t)n_batch]; }
+        nll[b] = n > 0.0 ? -S + n * std::log(I) : 0.0;
+    }
+    return MIPWA_OK;
+}
+
 // whole-sample NLL and gradient from the gathered mipwa_nll_grad_parts pieces, parts[r] = (S_r, I_r, n_r, grad_ev_r[P],
 // grad_nm_r[P]): NLL = -sum S_r + n ln I, grad = sum grad_ev_r + (n / I) sum grad_nm_r, every sum in rank order
 int mipwa_combine_grad_parts(int32_t n_ranks, int64_t n_params, const double* parts, double* nll, double* grad,

@@ -57,17 +57,13 @@ def combine_parts(sum_log, integral, n_ev, group=None, device=None):
 def combine_parts_batch(sum_log, integral, n_ev, group=None, device=None):
     """NLL of the whole sample at every one of B parameter vectors from one rank's pieces (mipwa_nll_batch with
     parts: sum_log[b], integral[b]): ONE all_gather of 2 B + 1 doubles per rank, then step A7 per vector in the C library
-    (rank-ordered sums, the same bits on every rank).  Returns the B values."""
+    (mipwa_combine_parts_batch: rank-ordered sums, the same bits on every rank).  Returns the B values."""
     S = np.ascontiguousarray(sum_log, dtype=np.float64)
     Iv = np.ascontiguousarray(integral, dtype=np.float64)
     if S.shape != Iv.shape or S.ndim != 1:
         raise ValueError("sum_log and integral must be vectors of the same length")
     rows = _gather_rows(np.concatenate([S, Iv, [float(n_ev)]]), group, device)
-    B = S.size
-    out = np.empty(B)
-    for b in range(B):
-        out[b] = binding.combine_parts(np.stack([rows[:, b], rows[:, B + b], rows[:, 2 * B]], axis=1))[0]
-    return out
+    return binding.combine_parts_batch(rows, S.size)
 
 
 def combine_grad_parts(sum_log, integral, n_ev, grad_ev, grad_nm, group=None, device=None):
