@@ -468,20 +468,31 @@ k_grad_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict_
 // reads on one SM while the rest of the GPU idles.
 static __global__ void __launch_bounds__(256)
 k_grad_finalize(const double* __restrict__ partials, int split, int nblocks, int NV, int sets,
-                double* __restrict__ result)
+                double* __restrict__ result, unsigned int* __restrict__ ticket, double* __restrict__ tag_word, long long tag)
 {
     // launched with programmatic stream serialisation right behind the kernel that writes `partials`: its blocks may be
     // resident before that kernel has finished; nothing is read before this point
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const int kk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (kk >= sets * NV) return;
-    const int set = kk / NV, k = kk - set * NV;
-    const int b0 = set == 0 ? 0 : split, b1 = set == 0 ? split : nblocks;
-    double s = 0.0;
-    for (int b = b0 + lane; b < b1; b += 32) s += partials[(size_t)b * NV + k];
+    if (kk < sets * NV) {
+        const int set = kk / NV, k = kk - set * NV;
+        const int b0 = set == 0 ? 0 : split, b1 = set == 0 ? split : nblocks;
+        double s = 0.0;
+        for (int b = b0 + lane; b < b1; b += 32) s += partials[(size_t)b * NV + k];
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
-    if (lane == 0) result[kk] = s;
+        for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+        if (lane == 0) { result[kk] = s; __threadfence_system(); }
+    }
+    if (ticket) {
+        // `result` is mapped host memory: the last block to finish writes the call's tag behind everybody's values, and the
+        // host polls that word instead of sleeping in cudaStreamSynchronize (as the value kernels do, dev_model.cuh)
+        __syncthreads();
+        if (threadIdx.x == 0 && atomicAdd(ticket, 1u) == gridDim.x - 1) {
+            *ticket = 0;
+            __threadfence_system();
+            *reinterpret_cast<volatile long long*>(tag_word) = tag;
+        }
+    }
 }
 
 // ---- cell sort (once per point set): key = seg(s12) * (N-1) + seg(s13) ---------------------------------------------

@@ -89,6 +89,7 @@ struct mipwa_ctx {
     double* h_batch = nullptr;      // mapped pinned, 4 doubles per slot (S, I, tag, -): totals of mipwa_nll_batch's calls
     double* d_batch = nullptr;      // device alias of h_batch
     int64_t batch_cap = 0;          // slots
+    long long grad_tag = 0;         // tag of the last k_grad_finalize launch (wait_grad)
     bool overlap_launch = false;    // mipwa_nll_batch, vectors 1..: the value kernel may start while its predecessor drains
     unsigned long long* h_bad = nullptr;
     unsigned long long* d_bad = nullptr;
@@ -394,6 +395,7 @@ static long long next_tag(mipwa_ctx* c)
 
 // k_grad_finalize right behind the kernel that writes the block partials, launched with programmatic stream serialisation:
 // its launch latency runs under the producer's tail (the kernel itself waits in griddepcontrol.wait, grad.cuh)
+#define MIPWA_GRAD_TAG_SLOT 4095                           // h_result word the gradient's tag goes to (the vectors end below 4030)
 static cudaError_t launch_finalize(mipwa_ctx* c, int blocks, const double* partials, int split, int nblocks, int NV, int sets,
                                    double* result)
 {
@@ -403,7 +405,32 @@ static cudaError_t launch_finalize(mipwa_ctx* c, int blocks, const double* parti
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k_grad_finalize, partials, split, nblocks, NV, sets, result);
+    // the tag of this call behind the values: d_ticket + 1 is the finalize kernel's own counter
+    *reinterpret_cast<volatile long long*>(c->h_result + MIPWA_GRAD_TAG_SLOT) = 0;
+    c->grad_tag = ++c->tag;
+    return cudaLaunchKernelEx(&cfg, k_grad_finalize, partials, split, nblocks, NV, sets, result, c->d_ticket + 1,
+                              c->d_result + MIPWA_GRAD_TAG_SLOT, c->grad_tag);
+}
+
+// wait for the gradient sums of the call launch_finalize just enqueued (polls the tag, then falls back to the stream)
+static int wait_grad(mipwa_ctx* c)
+{
+    if (c->timing) {
+        CU(c, cudaEventRecord(c->ev1, c->stream));
+        CU(c, cudaEventSynchronize(c->ev1));
+        CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+        return MIPWA_OK;
+    }
+    volatile long long* flag = reinterpret_cast<volatile long long*>(c->h_result + MIPWA_GRAD_TAG_SLOT);
+    for (int spin = 0; spin < 400000; ++spin) {
+        if (*flag == c->grad_tag) return MIPWA_OK;
+        if ((spin & 0x3fff) == 0x3fff) {
+            const cudaError_t e = cudaStreamQuery(c->stream);
+            if (e != cudaSuccess && e != cudaErrorNotReady) return fail(c, MIPWA_ERR_CUDA, cudaGetErrorString(e));
+        }
+    }
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MIPWA_OK;
 }
 
 // start of the timed region of a call (timing mode only): spacer kernel, then the first event (kernels.cuh: k_spacer)
@@ -1559,11 +1586,8 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
     (void)launch_finalize(c, (NV + 7) / 8, c->d_gpartials, grid, grid, NV, 1, c->d_result);
     ++c->launches;
     CU(c, cudaGetLastError());
-    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
 
-    // host: g = G c, I = Re(c^H g) (K^2 complex MACs), then the adjoint maps
+    // host, while the kernels run: g = G c, I = Re(c^H g) (K^2 complex MACs); after the wait the adjoint maps
     const double* h = c->h_result;
     const double* G = c->h_gram.data();
     std::vector<double> gc(2 * K, 0.0);
@@ -1578,6 +1602,7 @@ static int nll_grad_compact(mipwa_ctx* c, const double* params, int64_t n_params
         gc[2 * k] = gr; gc[2 * k + 1] = gi;
         I += cc.c[k].x * gr + cc.c[k].y * gi;
     }
+    { const int wrc = wait_grad(c); if (wrc) return wrc; }
     const double S = h[0], n_ev = (double)c->ev.n;
     *nll = -S + n_ev * std::log(I);
     const double scale = c->ev.n > 0 ? 2.0 * n_ev / I : 0.0;
@@ -1692,9 +1717,8 @@ static int nll_grad_recompute(mipwa_ctx* c, const double* params, int64_t n_para
     GradTotals t;
     rc = launch_grad_recompute(c, false, shp, 0.0, true, true, want_f, &t);
     if (rc) return rc;
-    if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if (c->timing) CU(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1));
+    rc = wait_grad(c);
+    if (rc) return rc;
 
     // ---- host: O(N + R) combine (A7) and adjoint of the coefficient maps ----------------------------------------------
     const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;          // w == NULL: the records carry weight 1
@@ -1785,7 +1809,8 @@ static int nll_grad_recompute(mipwa_ctx* c, const double* params, int64_t n_para
 #undef MIPWA_SHAPE_LAUNCH
         ++c->launches;
         CU(c, cudaGetLastError());
-        k_grad_finalize<<<(8 * nf + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, grid, 8 * nf, 1, c->d_result + SHAPE_OFF);
+        k_grad_finalize<<<(8 * nf + 7) / 8, 256, 0, c->stream>>>(c->d_gpartials, grid, grid, 8 * nf, 1, c->d_result + SHAPE_OFF,
+                                                                 nullptr, nullptr, 0);
         ++c->launches;
         CU(c, cudaGetLastError());
         if (c->timing) CU(c, cudaEventRecord(c->ev1, c->stream));
