@@ -132,7 +132,8 @@ template <int R1, int R2, int FL, bool MIX>
 __global__ void __launch_bounds__(MIPWA_REC_BLOCK, 1)
 k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__ ev, double kappa, long long n_ev,
                 const PointRec* __restrict__ nm, long long n_norm, double2* __restrict__ partials,
-                unsigned int* __restrict__ ticket, double* __restrict__ result, long long tag)
+                unsigned int* __restrict__ ticket, double* __restrict__ result, long long tag,
+                const double* __restrict__ integral_src)
 {
     __shared__ RowsSmem sm;
     __shared__ double red[2 * 32];
@@ -147,6 +148,9 @@ k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__
     const PointRec* p = ev + t0;
     PointRec r = ld_rec(p);                                // the first record is on its way while the rows are copied
     load_rows_smem(sm, m);
+    // MIX with integral_src: the integral of the normalisation launch that ran just before on this stream is read from device
+    // memory (no host round trip between the two launches of mipwa_nll_mix); `kappa` then carries (1 - f_s) / f_s x weight scale
+    if (MIX && integral_src) kappa *= __ldcg(integral_src);
 
     LogProd lp;
     double integ = 0.0;
@@ -219,7 +223,7 @@ k_nll_recompute(const __grid_constant__ DevModel m, const PointRec* __restrict__
         block_reduce<2>(f, red);
         if (threadIdx.x == 0) {
             result[0] = f[0];
-            result[1] = f[1];
+            result[1] = MIX && integral_src ? __ldcg(integral_src) : f[1];   // the mixture's event launch hands the integral on
             *ticket = 0;                                  // ready for the next call
             publish_result(result, tag);
         }

@@ -22,7 +22,8 @@ cudaError_t mipwa_launch_nll_recompute_overlapped(const int* n_spin, int fl, int
 cudaError_t mipwa_launch_nll_recompute_mix(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
                                            const PointRec* ev, double kappa, long long n_ev, const PointRec* nm,
                                            long long n_norm, double2* partials, unsigned int* ticket, double* result,
-                                           long long tag);
+                                           long long tag,
+                                           const double* integral_src);
 cudaError_t mipwa_launch_abs2(const int* n_spin, int fl, int grid, cudaStream_t st, const DevModel& m,
                               const double* s12, const double* s13, const unsigned short* seg, long long n, double* out);
 

@@ -1918,22 +1918,26 @@ int mipwa_nll_mix(mipwa_ctx* c, const double* params, int64_t n_params, double f
     const bool timing = c->timing;
     { const int trc = timing_begin(c); if (trc) return trc; }
     c->timing = false;                                     // wait_result polls: one pair of events spans both launches
+    // Launch 1: the normalisation points alone; with events to follow its totals stay in DEVICE memory and launch 2 (events,
+    // D_i = |A_i|^2 + kappa b_i) reads the integral from there: kappa = I (1 - f_s) / f_s is formed on the device, the host
+    // waits once, and launch 2 hands the integral on beside its own sum.
+    const double wn = c->nm.w ? 1.0 : 1.0 / (double)c->nm.n;
     long long tag = next_tag(c);
     cudaError_t le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, false, grid, c->stream, c->model, E.rec, 0.0, 0,
-                                                G.rec, G.n, c->d_partials, c->d_ticket, c->result_dst, tag);
+                                                G.rec, G.n, c->d_partials, c->d_ticket,
+                                                E.n > 0 ? c->d_dev_result : c->result_dst, tag);
     ++c->launches;
-    if (le == cudaSuccess) rc = wait_result(c, tag);
-    const double I = c->nm.w ? c->h_result[1] : c->h_result[1] / (double)c->nm.n;
-    const double kappa = I * (1.0 - f_sig) / f_sig;
     double S = 0.0;
-    if (le == cudaSuccess && rc == MIPWA_OK && E.n > 0) {
+    if (le == cudaSuccess && E.n > 0) {
         tag = next_tag(c);
-        le = mipwa_launch_nll_recompute(c->n_spin, c->model_flags, true, grid, c->stream, c->model, E.rec, kappa, E.n, G.rec,
-                                        0, c->d_partials, c->d_ticket, c->result_dst, tag);
+        le = mipwa_launch_nll_recompute_mix(c->n_spin, c->model_flags, grid, c->stream, c->model, E.rec,
+                                            wn * (1.0 - f_sig) / f_sig, E.n, G.rec, 0, c->d_partials, c->d_ticket,
+                                            c->result_dst, tag, c->d_dev_result + 1);
         ++c->launches;
-        if (le == cudaSuccess) rc = wait_result(c, tag);
-        S = c->h_result[0];
     }
+    if (le == cudaSuccess) rc = wait_result(c, tag);
+    if (E.n > 0) S = c->h_result[0];
+    const double I = c->h_result[1] * wn;
     c->timing = timing;
     CU(c, le);
     if (rc) return rc;

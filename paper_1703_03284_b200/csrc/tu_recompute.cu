@@ -9,10 +9,10 @@ cudaError_t mipwa_launch_nll_recompute(const int* n_spin, int fl, bool mix, int 
 {
     if (mix)
         return mipwa_launch_nll_recompute_mix(n_spin, fl, grid, st, m, ev, kappa, n_ev, nm, n_norm, partials, ticket,
-                                              result, tag);
+                                              result, tag, nullptr);
     MIPWA_DISPATCH_SIGFL(n_spin[0], n_spin[1], n_spin[2], fl,
                          (k_nll_recompute<R1, R2, FL, false><<<grid, MIPWA_REC_BLOCK, 0, st>>>(
-                             m, ev, 0.0, n_ev, nm, n_norm, partials, ticket, result, tag)));
+                             m, ev, 0.0, n_ev, nm, n_norm, partials, ticket, result, tag, nullptr)));
     return cudaGetLastError();
 }
 
@@ -38,6 +38,6 @@ cudaError_t mipwa_launch_nll_recompute_overlapped(const int* n_spin, int fl, int
     cudaError_t e = cudaSuccess;
     MIPWA_DISPATCH_SIGFL(n_spin[0], n_spin[1], n_spin[2], fl,
                          (e = launch_serialised(k_nll_recompute<R1, R2, FL, false>, grid, st, m, ev, 0.0, n_ev, nm, n_norm,
-                                                partials, ticket, result, tag)));
+                                                partials, ticket, result, tag, (const double*)nullptr)));
     return e != cudaSuccess ? e : cudaGetLastError();
 }
